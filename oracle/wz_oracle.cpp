@@ -1,0 +1,586 @@
+// oracle/wz_oracle.cpp -- CPU ORACLE.  TEST INFRASTRUCTURE, NOT THE PRODUCT.
+//
+// A plain, slow, fp64 CPU statement of what the hot path of arXiv 1005.3276
+// computes: the 4D DFT of a 4-spinor lattice field with antiperiodic time
+// boundary conditions, the fermion matrix M of Eq. (2.19) applied by the
+// "FFT trick" of Sec. VII.B, M^dag M, and textbook conjugate gradient on
+// M^dag M x = b (Eq. 7.8).  Only tests/, __graft_entry__.smoke() and bench.py's
+// cpu_baseline / --impl reference legs may load this library.  It shares no
+// code, header, table or constant with the CUDA path under
+// paper_1005_3276_b200/csrc/ and neither includes the other.
+//
+// Every function cites the passage of /root/reference/PAPER.md it follows
+// ("PAPER.md:<line>, Eq. ...").  Readings of garbled / silent passages are the
+// G-numbers of SURVEY.md 8(c), restated in DESIGN.md.
+//
+// Parity pins (tests/test_oracle_*.py, all "-m 'not gpu'"):
+//   dft4d_naive / fft4d_radix2 : numpy.fft.fftn, delta/plane-wave closed forms,
+//                                Parseval, round trip, each other.
+//   dslash_symbol              : overlap_D_symbol (Eq. 2.9 by 4x4 matrix algebra),
+//                                Eqs. 3.1/3.3/3.4/3.5/3.6/2.18/2.20/7.11, GW relation,
+//                                small-p limit, golden extremes of d^2(p).
+//   apply_M / apply_MdagM      : dense position-space route oracle/dense_route.py
+//                                (no Fourier transform anywhere) on 2^4 and 4^4,
+//                                stencil identities, constant-phi closed form,
+//                                adjoint / Hermiticity / positivity.
+//   cg / cg_c64ru              : dense Cholesky solve on 2^4, 4^4; constant-phi closed
+//                                form; true residual recomputed independently.
+//   The solve at 16^4 and above with non-constant phi has no printed value in the
+//   paper to compare with: there "parity unpinned by a printed value" -- it is
+//   covered by the same code path pinned at 2^4/4^4 plus the residual check.
+//
+// Layout everywhere: spinor = [spin 0..3][x0=t][x1][x2][x3], x3 fastest,
+// complex128 interleaved (re, im); phi = [x0][x1][x2][x3].
+// Spin basis: Eq. (2.2): gamma5 = diag(-1,-1,+1,+1).
+
+#include <cmath>
+#include <complex>
+#include <cstdint>
+#include <cstdlib>
+#include <cstring>
+#include <vector>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+typedef std::complex<double> cd;
+static const double PI = 3.14159265358979323846264338327950288;
+
+// ----------------------------------------------------------------------------
+// Gamma matrices, Eq. (2.2), written out entry by entry.
+//   gamma_0 = [[0, 1],[1, 0]],  gamma_i = [[0, i sigma_i],[-i sigma_i, 0]].
+// ----------------------------------------------------------------------------
+static void gamma_matrix(int mu, cd g[4][4]) {
+  const cd I(0.0, 1.0);
+  for (int a = 0; a < 4; ++a)
+    for (int b = 0; b < 4; ++b) g[a][b] = 0.0;
+  if (mu == 0) {
+    g[0][2] = 1.0; g[1][3] = 1.0; g[2][0] = 1.0; g[3][1] = 1.0;
+    return;
+  }
+  cd s[2][2];
+  if (mu == 1) { s[0][0] = 0; s[0][1] = 1; s[1][0] = 1; s[1][1] = 0; }
+  if (mu == 2) { s[0][0] = 0; s[0][1] = -I; s[1][0] = I; s[1][1] = 0; }
+  if (mu == 3) { s[0][0] = 1; s[0][1] = 0; s[1][0] = 0; s[1][1] = -1; }
+  for (int a = 0; a < 2; ++a)
+    for (int b = 0; b < 2; ++b) {
+      g[a][2 + b] = I * s[a][b];    // upper right block  +i sigma_i
+      g[2 + a][b] = -I * s[a][b];   // lower left block   -i sigma_i
+    }
+}
+
+// Lattice momentum of bin n on an axis of length L (fermion
+// antiperiodic in time => p0 = 2 pi (n0 + 1/2)/T; periodic in space).
+static double momentum(int n, int L, int half) {
+  return 2.0 * PI * (double(n) + (half ? 0.5 : 0.0)) / double(L);
+}
+
+extern "C" {
+
+int orc_set_threads(int n) {
+#ifdef _OPENMP
+  if (n > 0) omp_set_num_threads(n);
+  return omp_get_max_threads();
+#else
+  (void)n;
+  return 1;
+#endif
+}
+
+void orc_gamma(int mu, double* out /* 4x4 complex, row major; mu=5 gives gamma5 */) {
+  cd g[4][4];
+  if (mu == 5) {
+    for (int a = 0; a < 4; ++a)
+      for (int b = 0; b < 4; ++b) g[a][b] = 0.0;
+    g[0][0] = -1; g[1][1] = -1; g[2][2] = 1; g[3][3] = 1;   // Eq. (2.2)
+  } else {
+    gamma_matrix(mu, g);
+  }
+  for (int a = 0; a < 4; ++a)
+    for (int b = 0; b < 4; ++b) {
+      out[2 * (4 * a + b)] = g[a][b].real();
+      out[2 * (4 * a + b) + 1] = g[a][b].imag();
+    }
+}
+
+// ----------------------------------------------------------------------------
+// O1. Discrete Fourier transforms ("fast Fourier transform the
+// in vector to momentum space ... then fast Fourier transform back").
+// forward : F[n] = sum_x exp(-2 pi i n x / L) f[x]      (unnormalised)
+// inverse : f[x] = (1/L) sum_n exp(+2 pi i n x / L) F[n]
+// ----------------------------------------------------------------------------
+
+// One axis, naive O(L^2) sum.  Twiddle argument reduced mod L in integers.
+static void dft_axis_naive(cd* a, long outer, int L, long inner, int dir) {
+  std::vector<cd> w(L);
+  for (int k = 0; k < L; ++k) {
+    double ang = 2.0 * PI * double(k) / double(L);
+    w[k] = cd(std::cos(ang), dir > 0 ? -std::sin(ang) : std::sin(ang));
+  }
+  const double scale = dir > 0 ? 1.0 : 1.0 / double(L);
+#pragma omp parallel
+  {
+    std::vector<cd> line(L), res(L);
+#pragma omp for collapse(2) schedule(static)
+    for (long o = 0; o < outer; ++o)
+      for (long i = 0; i < inner; ++i) {
+        cd* base = a + o * L * inner + i;
+        for (int x = 0; x < L; ++x) line[x] = base[x * inner];
+        for (int n = 0; n < L; ++n) {
+          cd acc = 0.0;
+          for (int x = 0; x < L; ++x) acc += w[(int)(((long)n * x) % L)] * line[x];
+          res[n] = acc * scale;
+        }
+        for (int n = 0; n < L; ++n) base[n * inner] = res[n];
+      }
+  }
+}
+
+// One axis, iterative radix-2 Cooley-Tukey (bit reversal + log2 L stages).
+static int is_pow2(int L) { return L > 0 && (L & (L - 1)) == 0; }
+
+static void fft_axis_radix2(cd* a, long outer, int L, long inner, int dir) {
+  int logL = 0;
+  while ((1 << logL) < L) ++logL;
+  std::vector<int> rev(L);
+  for (int i = 0; i < L; ++i) {
+    int r = 0;
+    for (int b = 0; b < logL; ++b)
+      if (i & (1 << b)) r |= 1 << (logL - 1 - b);
+    rev[i] = r;
+  }
+  std::vector<cd> w(L / 2 > 0 ? L / 2 : 1);
+  for (int k = 0; k < L / 2; ++k) {
+    double ang = 2.0 * PI * double(k) / double(L);
+    w[k] = cd(std::cos(ang), dir > 0 ? -std::sin(ang) : std::sin(ang));
+  }
+  const double scale = dir > 0 ? 1.0 : 1.0 / double(L);
+#pragma omp parallel
+  {
+    std::vector<cd> line(L);
+#pragma omp for collapse(2) schedule(static)
+    for (long o = 0; o < outer; ++o)
+      for (long i = 0; i < inner; ++i) {
+        cd* base = a + o * L * inner + i;
+        for (int x = 0; x < L; ++x) line[rev[x]] = base[x * inner];
+        for (int len = 2; len <= L; len <<= 1) {
+          int half = len / 2, step = L / len;
+          for (int s = 0; s < L; s += len)
+            for (int k = 0; k < half; ++k) {
+              cd u = line[s + k];
+              cd v = line[s + k + half] * w[k * step];
+              line[s + k] = u + v;
+              line[s + k + half] = u - v;
+            }
+        }
+        for (int n = 0; n < L; ++n) base[n * inner] = line[n] * scale;
+      }
+  }
+}
+
+// Antiperiodic time boundary condition as a twist:
+// psi(x0 + T) = -psi(x0)  <=>  psi(x) = sum_p exp(i p x) with p0 = 2 pi (n0 + 1/2)/T
+// so forward = multiply by exp(-i pi x0 / T), then the periodic transform;
+// inverse = periodic inverse, then multiply by exp(+i pi x0 / T).
+static void time_twist(cd* a, const int L[4], int sign) {
+  long inner = (long)L[1] * L[2] * L[3];
+  for (int x0 = 0; x0 < L[0]; ++x0) {
+    double ang = PI * double(x0) / double(L[0]);
+    cd t(std::cos(ang), sign * std::sin(ang));
+    for (long i = 0; i < inner; ++i) a[x0 * inner + i] *= t;
+  }
+}
+
+// method: 0 = naive O(L^2) per axis (any L), 1 = radix-2 (power-of-two L only).
+// dir: +1 forward, -1 inverse.  apbc: 1 = half-integer time momenta.
+// `a` holds ncomp fields of L0*L1*L2*L3 complex128, transformed in place.
+int orc_dft4d(int method, int dir, int apbc, const int* L, double* a_, int ncomp) {
+  cd* a = reinterpret_cast<cd*>(a_);
+  long V = (long)L[0] * L[1] * L[2] * L[3];
+  if (method == 1)
+    for (int mu = 0; mu < 4; ++mu)
+      if (!is_pow2(L[mu])) return 1;
+  for (int c = 0; c < ncomp; ++c) {
+    cd* f = a + c * V;
+    if (apbc && dir > 0) time_twist(f, L, -1);
+    long outer = 1;
+    for (int mu = 0; mu < 4; ++mu) {
+      long inner = 1;
+      for (int nu = mu + 1; nu < 4; ++nu) inner *= L[nu];
+      if (method == 1) fft_axis_radix2(f, outer, L[mu], inner, dir);
+      else dft_axis_naive(f, outer, L[mu], inner, dir);
+      outer *= L[mu];
+    }
+    if (apbc && dir < 0) time_twist(f, L, +1);
+  }
+  return 0;
+}
+
+// ----------------------------------------------------------------------------
+// O2. Momentum-space symbols.
+// ----------------------------------------------------------------------------
+
+// The overlap operator D(p) of PAPER.md:89-98 Eq. (2.9) evaluated on a plane wave
+// exp(+i p x) by 4x4 matrix algebra, with no closed form used:
+//   forward/backward differences  d -> e^{ip}-1,  d* -> 1-e^{-ip}
+//   D_W = 1/2 gamma_mu (d*_mu + d_mu) - 1/2 d*_mu d_mu          (reading G1: Wilson sign)
+//   A   = rho - D_W                                               (reading G2: rho)
+//   D   = rho (1 - A (A^dag A)^{-1/2})
+// A^dag A must come out proportional to the unit matrix (checked; returns 1 if not).
+// Outputs D (4x4), and its split D = D1 + D2 with D2 = (tr D / 4) 1 (scalar part).
+int orc_overlap_D_symbol(const double* p, double rho, double* D_out, double* D1_out, double* D2_out) {
+  const cd I(0.0, 1.0);
+  cd A[4][4], g[4][4];
+  for (int a = 0; a < 4; ++a)
+    for (int b = 0; b < 4; ++b) A[a][b] = (a == b) ? rho : 0.0;
+  for (int mu = 0; mu < 4; ++mu) {
+    gamma_matrix(mu, g);
+    cd fwd = std::exp(I * p[mu]) - 1.0;     // forward difference on exp(ipx)
+    cd bwd = 1.0 - std::exp(-I * p[mu]);    // backward difference
+    cd sym = 0.5 * (bwd + fwd);
+    cd lap = bwd * fwd;                     // d* d  (= -4 sin^2(p/2))
+    for (int a = 0; a < 4; ++a)
+      for (int b = 0; b < 4; ++b) {
+        cd dw = g[a][b] * sym - ((a == b) ? 0.5 * lap : cd(0.0));
+        A[a][b] -= dw;
+      }
+  }
+  cd AA[4][4];
+  for (int a = 0; a < 4; ++a)
+    for (int b = 0; b < 4; ++b) {
+      cd acc = 0.0;
+      for (int c = 0; c < 4; ++c) acc += std::conj(A[c][a]) * A[c][b];
+      AA[a][b] = acc;
+    }
+  double s2 = AA[0][0].real();
+  for (int a = 0; a < 4; ++a)
+    for (int b = 0; b < 4; ++b) {
+      cd want = (a == b) ? cd(s2) : cd(0.0);
+      if (std::abs(AA[a][b] - want) > 1e-12 * (1.0 + s2)) return 1;
+    }
+  double inv_s = 1.0 / std::sqrt(s2);
+  cd D[4][4];
+  cd tr = 0.0;
+  for (int a = 0; a < 4; ++a)
+    for (int b = 0; b < 4; ++b) {
+      D[a][b] = rho * (((a == b) ? cd(1.0) : cd(0.0)) - A[a][b] * inv_s);
+      if (a == b) tr += D[a][b];
+    }
+  for (int a = 0; a < 4; ++a)
+    for (int b = 0; b < 4; ++b) {
+      cd d2 = (a == b) ? tr / 4.0 : cd(0.0);
+      cd d1 = D[a][b] - d2;
+      int k = 2 * (4 * a + b);
+      D_out[k] = D[a][b].real();  D_out[k + 1] = D[a][b].imag();
+      D1_out[k] = d1.real();      D1_out[k + 1] = d1.imag();
+      D2_out[k] = d2.real();      D2_out[k + 1] = d2.imag();
+    }
+  return 0;
+}
+
+// Scalar factor c(p) of  Dslash(p) = (1 - D2/2rho)^{-1} D1 = i c(p) sum_mu gamma_mu sin p_mu.
+// From PAPER.md:210-213 Eq. (3.1), 224-225 Eq. (3.3), 382-390 Eq. (4.1)-(4.2):
+//   S2 = sum sin^2 p_mu,  Mw = rho - 2 sum sin^2(p_mu/2),  s = sqrt(Mw^2 + S2),
+//   (1 - D2/2rho)(p) = 1/2 + Mw/(2 s),  D1(p) = i rho X / s   (sign: reading G3)
+//   => c = 2 rho / (s + Mw).
+// For Mw < 0 the sum s + Mw cancels; the algebraically identical
+// form c = 2 rho (s - Mw)/S2 is used there (since (s+Mw)(s-Mw) = S2).
+static double dslash_c(const double sn[4], const double sh2[4], double rho, double* d2_out) {
+  double S2 = 0.0, H = 0.0;
+  for (int mu = 0; mu < 4; ++mu) { S2 += sn[mu] * sn[mu]; H += sh2[mu]; }
+  double Mw = rho - 2.0 * H;
+  double s = std::sqrt(Mw * Mw + S2);
+  double c = (Mw >= 0.0) ? 2.0 * rho / (s + Mw) : 2.0 * rho * (s - Mw) / S2;
+  if (d2_out) *d2_out = c * c * S2;
+  return c;
+}
+
+// Dslash(p) as an explicit 4x4 complex matrix for the momentum vector p.
+void orc_dslash_symbol_p(const double* p, double rho, double* out) {
+  const cd I(0.0, 1.0);
+  double sn[4], sh2[4];
+  for (int mu = 0; mu < 4; ++mu) {
+    sn[mu] = std::sin(p[mu]);
+    double h = std::sin(0.5 * p[mu]);
+    sh2[mu] = h * h;
+  }
+  double c = dslash_c(sn, sh2, rho, nullptr);
+  cd M[4][4], g[4][4];
+  for (int a = 0; a < 4; ++a)
+    for (int b = 0; b < 4; ++b) M[a][b] = 0.0;
+  for (int mu = 0; mu < 4; ++mu) {
+    gamma_matrix(mu, g);
+    for (int a = 0; a < 4; ++a)
+      for (int b = 0; b < 4; ++b) M[a][b] += I * c * sn[mu] * g[a][b];
+  }
+  for (int a = 0; a < 4; ++a)
+    for (int b = 0; b < 4; ++b) {
+      out[2 * (4 * a + b)] = M[a][b].real();
+      out[2 * (4 * a + b) + 1] = M[a][b].imag();
+    }
+}
+
+// d^2(p) = Dslash(p)^dag Dslash(p) (a multiple of 1) over the whole momentum lattice;
+// returns min and max (the maximum grows without bound with T;
+// PAPER.md:916-919 Eq. 7.11: free M0^dag M0 = d^2(p) + |m|^2).
+void orc_dslash_d2_extremes(const int* L, double rho, int apbc, double* dmin, double* dmax) {
+  double lo = 1e300, hi = 0.0;
+  for (int n0 = 0; n0 < L[0]; ++n0)
+    for (int n1 = 0; n1 < L[1]; ++n1)
+      for (int n2 = 0; n2 < L[2]; ++n2)
+        for (int n3 = 0; n3 < L[3]; ++n3) {
+          int n[4] = {n0, n1, n2, n3};
+          double sn[4], sh2[4];
+          for (int mu = 0; mu < 4; ++mu) {
+            double p = momentum(n[mu], L[mu], mu == 0 && apbc);
+            sn[mu] = std::sin(p);
+            double h = std::sin(0.5 * p);
+            sh2[mu] = h * h;
+          }
+          double d2;
+          dslash_c(sn, sh2, rho, &d2);
+          if (d2 < lo) lo = d2;
+          if (d2 > hi) hi = d2;
+        }
+  *dmin = lo;
+  *dmax = hi;
+}
+
+// ----------------------------------------------------------------------------
+// O2. The fermion matrix, Eq. (2.19) (Yukawa factor 2g: reading G4):
+//   M = Dslash + m P+ + m* P- + 2 g phi P+ + 2 g* phi* P-,
+//   Dslash = (1 - a/2 D2)^{-1} D1, applied by FFT -> Dslash(p) -> inverse FFT
+//   (PAPER.md:896).  P+ = diag(0,0,1,1), P- = diag(1,1,0,0) from Eq. (2.2).
+//   M^dag = Dslash^dag + conj(m + 2 g phi) P+ + (m + 2 g phi) P-, and
+//   Dslash(p)^dag is taken as the explicit conjugate transpose of the 4x4 matrix.
+// method selects the DFT (0 naive, 1 radix-2).
+// ----------------------------------------------------------------------------
+int orc_apply_M(int method, const int* L, const double* phi_, const double* m_, const double* g_,
+                double rho, int dagger, const double* in_, double* out_) {
+  const cd* phi = reinterpret_cast<const cd*>(phi_);
+  const cd* in = reinterpret_cast<const cd*>(in_);
+  cd* out = reinterpret_cast<cd*>(out_);
+  const cd m(m_[0], m_[1]), g(g_[0], g_[1]);
+  const cd I(0.0, 1.0);
+  const long V = (long)L[0] * L[1] * L[2] * L[3];
+  std::vector<cd> f(in, in + 4 * V);
+  int rc = orc_dft4d(method, +1, 1, L, reinterpret_cast<double*>(f.data()), 4);
+  if (rc) return rc;
+  cd gam[4][4][4];
+  for (int mu = 0; mu < 4; ++mu) gamma_matrix(mu, gam[mu]);
+  std::vector<double> sn[4], sh2[4];
+  for (int mu = 0; mu < 4; ++mu) {
+    sn[mu].resize(L[mu]);
+    sh2[mu].resize(L[mu]);
+    for (int n = 0; n < L[mu]; ++n) {
+      double p = momentum(n, L[mu], mu == 0);
+      sn[mu][n] = std::sin(p);
+      double h = std::sin(0.5 * p);
+      sh2[mu][n] = h * h;
+    }
+  }
+#pragma omp parallel for collapse(2) schedule(static)
+  for (int n0 = 0; n0 < L[0]; ++n0)
+    for (int n1 = 0; n1 < L[1]; ++n1)
+      for (int n2 = 0; n2 < L[2]; ++n2)
+        for (int n3 = 0; n3 < L[3]; ++n3) {
+          long site = (((long)n0 * L[1] + n1) * L[2] + n2) * L[3] + n3;
+          double s4[4] = {sn[0][n0], sn[1][n1], sn[2][n2], sn[3][n3]};
+          double h4[4] = {sh2[0][n0], sh2[1][n1], sh2[2][n2], sh2[3][n3]};
+          double c = dslash_c(s4, h4, rho, nullptr);
+          cd D[4][4];
+          for (int a = 0; a < 4; ++a)
+            for (int b = 0; b < 4; ++b) {
+              cd acc = 0.0;
+              for (int mu = 0; mu < 4; ++mu) acc += I * c * s4[mu] * gam[mu][a][b];
+              D[a][b] = acc;
+            }
+          cd v[4], r[4];
+          for (int a = 0; a < 4; ++a) v[a] = f[a * V + site];
+          for (int a = 0; a < 4; ++a) {
+            cd acc = 0.0;
+            for (int b = 0; b < 4; ++b) acc += (dagger ? std::conj(D[b][a]) : D[a][b]) * v[b];
+            r[a] = acc;
+          }
+          for (int a = 0; a < 4; ++a) f[a * V + site] = r[a];
+        }
+  orc_dft4d(method, -1, 1, L, reinterpret_cast<double*>(f.data()), 4);
+#pragma omp parallel for schedule(static)
+  for (long x = 0; x < V; ++x) {
+    cd w = m + 2.0 * g * phi[x];                 // coefficient of P+ in M
+    cd wplus = dagger ? std::conj(w) : w;        // acts on spin 2,3 (P+)
+    cd wminus = dagger ? w : std::conj(w);       // acts on spin 0,1 (P-)
+    out[0 * V + x] = f[0 * V + x] + wminus * in[0 * V + x];
+    out[1 * V + x] = f[1 * V + x] + wminus * in[1 * V + x];
+    out[2 * V + x] = f[2 * V + x] + wplus * in[2 * V + x];
+    out[3 * V + x] = f[3 * V + x] + wplus * in[3 * V + x];
+  }
+  return 0;
+}
+
+// M^dag M ("In computing the M^dag M matrix multiplication, we
+// encounter M f_in = f_out and a similar expression involving M^dag").
+int orc_apply_MdagM(int method, const int* L, const double* phi, const double* m, const double* g,
+                    double rho, const double* in, double* out) {
+  const long V = (long)L[0] * L[1] * L[2] * L[3];
+  std::vector<double> tmp(8 * V);
+  int rc = orc_apply_M(method, L, phi, m, g, rho, 0, in, tmp.data());
+  if (rc) return rc;
+  return orc_apply_M(method, L, phi, m, g, rho, 1, tmp.data(), out);
+}
+
+// ----------------------------------------------------------------------------
+// O4. Conjugate gradient on A = M^dag M (Eq. 7.7, 904 Eq. 7.8;
+// stop rule PAPER.md:944: "relative residual less than ...").  Reading G8:
+// x0 = 0, 2-norm, relative to ||b||, test on the recursive residual each
+// iteration, true residual recomputed once at exit.  Textbook Hestenes-Stiefel:
+//   r = b, p = r, rho0 = <r,r>
+//   k = 1,2,..: q = A p; alpha = rho_{k-1}/Re<p,q>; x += alpha p; r -= alpha q;
+//               rho_k = <r,r>; stop if sqrt(rho_k) <= tol ||b||;
+//               beta = rho_k/rho_{k-1}; p = r + beta p.
+// ----------------------------------------------------------------------------
+struct orc_cg_info {
+  int iterations;
+  int reliable_updates;
+  int converged;
+  double rel_residual_recursive;
+  double rel_residual_true;
+};
+
+static double dot_re(const cd* a, const cd* b, long n) {
+  double acc = 0.0;
+#pragma omp parallel for reduction(+ : acc) schedule(static)
+  for (long i = 0; i < n; ++i) acc += a[i].real() * b[i].real() + a[i].imag() * b[i].imag();
+  return acc;
+}
+
+int orc_cg(int method, const int* L, const double* phi, const double* b_, double* x_,
+           const double* m, const double* g, double rho, double tol, int max_iter,
+           orc_cg_info* info, double* history /* may be null; max_iter+1 entries */) {
+  const long V = (long)L[0] * L[1] * L[2] * L[3];
+  const long n = 4 * V;
+  const cd* b = reinterpret_cast<const cd*>(b_);
+  cd* x = reinterpret_cast<cd*>(x_);
+  std::vector<cd> r(b, b + n), p(b, b + n), q(n);
+  for (long i = 0; i < n; ++i) x[i] = 0.0;
+  double bnorm = std::sqrt(dot_re(b, b, n));
+  double rr = bnorm * bnorm;
+  if (history) history[0] = 1.0;
+  int k = 0, converged = 0;
+  if (bnorm == 0.0) converged = 1;
+  while (!converged && k < max_iter) {
+    ++k;
+    int rc = orc_apply_MdagM(method, L, phi, m, g, rho, reinterpret_cast<double*>(p.data()),
+                             reinterpret_cast<double*>(q.data()));
+    if (rc) return rc;
+    double alpha = rr / dot_re(p.data(), q.data(), n);
+#pragma omp parallel for schedule(static)
+    for (long i = 0; i < n; ++i) {
+      x[i] += alpha * p[i];
+      r[i] -= alpha * q[i];
+    }
+    double rr_new = dot_re(r.data(), r.data(), n);
+    if (history) history[k] = std::sqrt(rr_new) / bnorm;
+    if (std::sqrt(rr_new) <= tol * bnorm) {
+      rr = rr_new;
+      converged = 1;
+      break;
+    }
+    double beta = rr_new / rr;
+    rr = rr_new;
+#pragma omp parallel for schedule(static)
+    for (long i = 0; i < n; ++i) p[i] = r[i] + beta * p[i];
+  }
+  // true residual b - A x
+  orc_apply_MdagM(method, L, phi, m, g, rho, x_, reinterpret_cast<double*>(q.data()));
+  double tr = 0.0;
+  for (long i = 0; i < n; ++i) tr += std::norm(b[i] - q[i]);
+  info->iterations = k;
+  info->reliable_updates = 0;
+  info->converged = converged;
+  info->rel_residual_recursive = bnorm > 0 ? std::sqrt(rr) / bnorm : 0.0;
+  info->rel_residual_true = bnorm > 0 ? std::sqrt(tr) / bnorm : 0.0;
+  return 0;
+}
+
+// O4'. The complex64 variant (the paper only suggests mixed
+// precision).  Same loop, but the iteration vectors x, r, p, q are
+// rounded to float after every update (reductions stay in double), and a
+// reliable update keeps the true residual honest:
+//   X (complex128) accumulates the solution; rmax = max ||r|| since the last update;
+//   after each iteration, if ||r|| < delta * rmax  or  ||r|| <= tol ||b||:
+//       X += x; x = 0; r = b - A X in double, rounded to float;
+//       rho_k = ||r||^2 of that residual; rmax = ||r||; p is kept;
+//   converged only when that recomputed (true) ||r|| <= tol ||b||.
+static inline cd round_c64(cd z) { return cd((double)(float)z.real(), (double)(float)z.imag()); }
+
+int orc_cg_c64ru(int method, const int* L, const double* phi, const double* b_, double* X_,
+                 const double* m, const double* g, double rho, double tol, int max_iter,
+                 double delta, orc_cg_info* info, double* history) {
+  const long V = (long)L[0] * L[1] * L[2] * L[3];
+  const long n = 4 * V;
+  const cd* b = reinterpret_cast<const cd*>(b_);
+  cd* X = reinterpret_cast<cd*>(X_);
+  std::vector<cd> x(n, 0.0), r(n), p(n), q(n);
+  for (long i = 0; i < n; ++i) { X[i] = 0.0; r[i] = round_c64(b[i]); p[i] = r[i]; }
+  double bnorm = std::sqrt(dot_re(b, b, n));
+  double rr = dot_re(r.data(), r.data(), n);
+  double rmax = std::sqrt(rr);
+  if (history) history[0] = 1.0;
+  int k = 0, converged = 0, nru = 0;
+  double true_rel = 1.0;
+  if (bnorm == 0.0) { converged = 1; true_rel = 0.0; }
+  while (!converged && k < max_iter) {
+    ++k;
+    int rc = orc_apply_MdagM(method, L, phi, m, g, rho, reinterpret_cast<double*>(p.data()),
+                             reinterpret_cast<double*>(q.data()));
+    if (rc) return rc;
+    for (long i = 0; i < n; ++i) q[i] = round_c64(q[i]);
+    double alpha = rr / dot_re(p.data(), q.data(), n);
+#pragma omp parallel for schedule(static)
+    for (long i = 0; i < n; ++i) {
+      x[i] = round_c64(x[i] + alpha * p[i]);
+      r[i] = round_c64(r[i] - alpha * q[i]);
+    }
+    double rr_new = dot_re(r.data(), r.data(), n);
+    double rn = std::sqrt(rr_new);
+    if (rn > rmax) rmax = rn;
+    if (rn < delta * rmax || rn <= tol * bnorm) {
+      ++nru;
+      for (long i = 0; i < n; ++i) { X[i] += x[i]; x[i] = 0.0; }
+      orc_apply_MdagM(method, L, phi, m, g, rho, X_, reinterpret_cast<double*>(q.data()));
+      double tr = 0.0;
+      for (long i = 0; i < n; ++i) {
+        cd d = b[i] - q[i];
+        tr += std::norm(d);
+        r[i] = round_c64(d);
+      }
+      rr_new = tr;
+      rn = std::sqrt(tr);
+      rmax = rn;
+      true_rel = rn / bnorm;
+      if (rn <= tol * bnorm) converged = 1;
+    }
+    if (history) history[k] = rn / bnorm;
+    double beta = rr_new / rr;
+    rr = rr_new;
+    if (converged) break;
+#pragma omp parallel for schedule(static)
+    for (long i = 0; i < n; ++i) p[i] = round_c64(r[i] + beta * p[i]);
+  }
+  if (!converged) {
+    for (long i = 0; i < n; ++i) X[i] += x[i];
+    orc_apply_MdagM(method, L, phi, m, g, rho, X_, reinterpret_cast<double*>(q.data()));
+    double tr = 0.0;
+    for (long i = 0; i < n; ++i) tr += std::norm(b[i] - q[i]);
+    true_rel = bnorm > 0 ? std::sqrt(tr) / bnorm : 0.0;
+  }
+  info->iterations = k;
+  info->reliable_updates = nru;
+  info->converged = converged;
+  info->rel_residual_recursive = bnorm > 0 ? std::sqrt(rr) / bnorm : 0.0;
+  info->rel_residual_true = true_rel;
+  return 0;
+}
+
+}  // extern "C"

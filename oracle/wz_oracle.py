@@ -1,0 +1,179 @@
+"""ctypes binding of oracle/wz_oracle.cpp (the CPU oracle; test infrastructure only).
+
+The arithmetic lives in wz_oracle.cpp, each function there cites the passage of
+PAPER.md it follows.  This file only builds the shared object with g++ and
+marshals numpy arrays.  All arrays are complex128 in the external layout
+spinor = [spin][x0][x1][x2][x3], phi = [x0][x1][x2][x3].
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+from dataclasses import dataclass
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "wz_oracle.cpp")
+_LIB = os.path.join(_HERE, "liboracle_wz.so")
+_lib = None
+
+
+def build(force: bool = False) -> str:
+    """Compile the oracle with g++ (OpenMP) if the .so is missing or stale."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        tmp = _LIB + ".tmp.%d" % os.getpid()
+        cmd = ["g++", "-O2", "-std=c++17", "-fopenmp", "-shared", "-fPIC", "-o", tmp, _SRC]
+        subprocess.check_call(cmd)
+        os.replace(tmp, _LIB)
+    return _LIB
+
+
+class _Info(ctypes.Structure):
+    _fields_ = [("iterations", ctypes.c_int), ("reliable_updates", ctypes.c_int),
+                ("converged", ctypes.c_int), ("rel_residual_recursive", ctypes.c_double),
+                ("rel_residual_true", ctypes.c_double)]
+
+
+@dataclass
+class CGInfo:
+    iterations: int
+    reliable_updates: int
+    converged: bool
+    rel_residual_recursive: float
+    rel_residual_true: float
+    history: np.ndarray
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = ctypes.CDLL(build())
+        _lib.orc_set_threads.restype = ctypes.c_int
+    return _lib
+
+
+def set_threads(n: int = 0) -> int:
+    """Set (n > 0) or query (n = 0) the OpenMP thread count the oracle uses."""
+    return int(lib().orc_set_threads(int(n)))
+
+
+def _dp(a):
+    return a.ctypes.data_as(ctypes.POINTER(ctypes.c_double))
+
+
+def _dims(dims):
+    return (ctypes.c_int * 4)(*[int(d) for d in dims])
+
+
+def _c2(z):
+    z = complex(z)
+    return (ctypes.c_double * 2)(z.real, z.imag)
+
+
+def _method(dims, method):
+    if method == "auto":
+        pow2 = all(d & (d - 1) == 0 for d in dims)
+        return 1 if (pow2 and max(dims) >= 16) else 0
+    return {"naive": 0, "radix2": 1}[method]
+
+
+def gamma(mu: int) -> np.ndarray:
+    out = np.zeros((4, 4), dtype=np.complex128)
+    lib().orc_gamma(int(mu), _dp(out))
+    return out
+
+
+def dft4d(a: np.ndarray, direction: int, apbc: bool, method: str = "auto") -> np.ndarray:
+    """4D DFT over the last four axes of `a` (any leading component axes)."""
+    a = np.array(a, dtype=np.complex128, order="C", copy=True)
+    dims = a.shape[-4:]
+    ncomp = int(np.prod(a.shape[:-4], dtype=np.int64)) if a.ndim > 4 else 1
+    rc = lib().orc_dft4d(_method(dims, method), int(direction), int(bool(apbc)), _dims(dims), _dp(a), ncomp)
+    if rc:
+        raise ValueError("radix-2 oracle FFT needs power-of-two extents")
+    return a
+
+
+def overlap_D_symbol(p, rho: float = 1.0):
+    """(D, D1, D2) of Eq. (2.9) on the plane wave exp(+ipx), by 4x4 matrix algebra."""
+    p = np.ascontiguousarray(p, dtype=np.float64)
+    D, D1, D2 = (np.zeros((4, 4), dtype=np.complex128) for _ in range(3))
+    rc = lib().orc_overlap_D_symbol(_dp(p), ctypes.c_double(rho), _dp(D), _dp(D1), _dp(D2))
+    if rc:
+        raise ArithmeticError("A^dag A is not proportional to the unit matrix")
+    return D, D1, D2
+
+
+def dslash_symbol(p, rho: float = 1.0) -> np.ndarray:
+    """Dslash(p) = (1 - D2/2rho)^-1 D1 as the 4x4 matrix the oracle operator applies."""
+    p = np.ascontiguousarray(p, dtype=np.float64)
+    out = np.zeros((4, 4), dtype=np.complex128)
+    lib().orc_dslash_symbol_p(_dp(p), ctypes.c_double(rho), _dp(out))
+    return out
+
+
+def d2_extremes(dims, rho: float = 1.0, apbc: bool = True):
+    lo, hi = ctypes.c_double(), ctypes.c_double()
+    lib().orc_dslash_d2_extremes(_dims(dims), ctypes.c_double(rho), int(apbc), ctypes.byref(lo), ctypes.byref(hi))
+    return lo.value, hi.value
+
+
+def apply_M(phi, psi, m, g, rho=1.0, dagger=False, method="auto") -> np.ndarray:
+    phi = np.ascontiguousarray(phi, dtype=np.complex128)
+    psi = np.ascontiguousarray(psi, dtype=np.complex128)
+    dims = phi.shape
+    assert psi.shape == (4,) + tuple(dims)
+    out = np.empty_like(psi)
+    rc = lib().orc_apply_M(_method(dims, method), _dims(dims), _dp(phi), _c2(m), _c2(g),
+                           ctypes.c_double(rho), int(bool(dagger)), _dp(psi), _dp(out))
+    if rc:
+        raise ValueError("oracle apply_M failed")
+    return out
+
+
+def apply_MdagM(phi, psi, m, g, rho=1.0, method="auto") -> np.ndarray:
+    phi = np.ascontiguousarray(phi, dtype=np.complex128)
+    psi = np.ascontiguousarray(psi, dtype=np.complex128)
+    dims = phi.shape
+    assert psi.shape == (4,) + tuple(dims)
+    out = np.empty_like(psi)
+    rc = lib().orc_apply_MdagM(_method(dims, method), _dims(dims), _dp(phi), _c2(m), _c2(g),
+                               ctypes.c_double(rho), _dp(psi), _dp(out))
+    if rc:
+        raise ValueError("oracle apply_MdagM failed")
+    return out
+
+
+def cg(phi, b, m, g, rho=1.0, tol=1e-10, max_iter=100000, method="auto"):
+    """Textbook CG on M^dag M x = b in complex128.  Returns (x, CGInfo)."""
+    phi = np.ascontiguousarray(phi, dtype=np.complex128)
+    b = np.ascontiguousarray(b, dtype=np.complex128)
+    dims = phi.shape
+    x = np.zeros_like(b)
+    hist = np.zeros(max_iter + 1, dtype=np.float64)
+    info = _Info()
+    rc = lib().orc_cg(_method(dims, method), _dims(dims), _dp(phi), _dp(b), _dp(x), _c2(m), _c2(g),
+                      ctypes.c_double(rho), ctypes.c_double(tol), int(max_iter), ctypes.byref(info), _dp(hist))
+    if rc:
+        raise ValueError("oracle cg failed")
+    return x, CGInfo(info.iterations, info.reliable_updates, bool(info.converged),
+                     info.rel_residual_recursive, info.rel_residual_true, hist[: info.iterations + 1].copy())
+
+
+def cg_c64ru(phi, b, m, g, rho=1.0, tol=1e-6, max_iter=100000, delta=0.1, method="auto"):
+    """complex64-vector CG with reliable updates (oracle variant O4').  Returns (X, CGInfo)."""
+    phi = np.ascontiguousarray(phi, dtype=np.complex128)
+    b = np.ascontiguousarray(b, dtype=np.complex128)
+    dims = phi.shape
+    X = np.zeros_like(b)
+    hist = np.zeros(max_iter + 1, dtype=np.float64)
+    info = _Info()
+    rc = lib().orc_cg_c64ru(_method(dims, method), _dims(dims), _dp(phi), _dp(b), _dp(X), _c2(m), _c2(g),
+                            ctypes.c_double(rho), ctypes.c_double(tol), int(max_iter), ctypes.c_double(delta),
+                            ctypes.byref(info), _dp(hist))
+    if rc:
+        raise ValueError("oracle cg_c64ru failed")
+    return X, CGInfo(info.iterations, info.reliable_updates, bool(info.converged),
+                     info.rel_residual_recursive, info.rel_residual_true, hist[: info.iterations + 1].copy())

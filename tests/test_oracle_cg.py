@@ -1,0 +1,63 @@
+"""Pins for the oracle's CG.  CPU only."""
+import numpy as np
+
+from oracle import dense_route
+from paper_1005_3276_b200 import inputs
+
+
+def test_cg_matches_dense_solve_2222(orc):
+    dims = (2, 2, 2, 2)
+    phi = inputs.make_phi(4, dims, 0.4)
+    b = inputs.make_source(4, 0, dims)
+    m, g = 0.3 - 0.1j, 0.4 + 0.2j
+    M = dense_route.fermion_matrix_dense(dims, phi, m, g, 1.0)
+    xd = dense_route.solve_normal_equations(M, b).reshape(b.shape)
+    x, info = orc.cg(phi, b, m, g, 1.0, 1e-13, 1000, "naive")
+    assert info.converged and info.iterations <= 64 + 5      # at most dim steps (+rounding)
+    assert np.linalg.norm(x - xd) <= 1e-9 * np.linalg.norm(xd)
+    assert info.rel_residual_true <= 1e-12
+
+
+def test_cg_residuals_and_energy_norm_config1(orc):
+    # P10: recursive and true residuals agree; the energy-norm error decreases monotonically.
+    cfg = inputs.CONFIGS[1]
+    dims = cfg["dims"]
+    phi = inputs.make_phi(cfg["seed"], dims, cfg["sigma"])
+    b = inputs.make_source(cfg["seed"], 0, dims)
+    M = dense_route.fermion_matrix_dense(dims, phi, cfg["m"], cfg["g"], 1.0)
+    A = M.conj().T @ M
+    xd = np.linalg.solve(A, b.reshape(-1))
+    x, info = orc.cg(phi, b, cfg["m"], cfg["g"], 1.0, cfg["tol"], 5000, "naive")
+    assert info.converged
+    assert info.rel_residual_recursive <= cfg["tol"]
+    assert abs(info.rel_residual_true - info.rel_residual_recursive) <= 1e-3 * info.rel_residual_recursive
+    res = np.linalg.norm(b.reshape(-1) - A @ x.reshape(-1)) / np.linalg.norm(b)
+    assert abs(res - info.rel_residual_true) <= 1e-3 * res
+    assert 100 <= info.iterations <= 300                     # survey estimate with numpy's RNG: 163
+    errs = []
+    for k in (10, 40, 80, 120):
+        xk, _ = orc.cg(phi, b, cfg["m"], cfg["g"], 1.0, 1e-30, k, "naive")
+        e = xk.reshape(-1) - xd
+        errs.append(np.vdot(e, A @ e).real)
+    assert all(errs[i + 1] < errs[i] for i in range(len(errs) - 1))
+    # history is the recursive relative residual per iteration
+    assert info.history[0] == 1.0 and info.history[-1] <= cfg["tol"]
+
+
+def test_cg_c64ru_reaches_true_tolerance(orc):
+    # G9: float-rounded vectors, reliable updates; converged means the TRUE residual <= tol.
+    dims = (8, 8, 8, 8)
+    phi = inputs.make_phi(3, dims, 0.5).astype(np.complex64).astype(np.complex128)
+    b = inputs.make_source(3, 0, dims).astype(np.complex64).astype(np.complex128)
+    m, g, tol = 0.02, 1.0, 1e-6
+    X, info = orc.cg_c64ru(phi, b, m, g, 1.0, tol, 20000, 0.1, "naive")
+    assert info.converged and info.reliable_updates >= 1
+    r = b - orc.apply_MdagM(phi, X, m, g, 1.0, "naive")
+    true_rel = np.linalg.norm(r) / np.linalg.norm(b)
+    assert true_rel <= tol
+    assert abs(true_rel - info.rel_residual_true) <= 1e-6 * tol + 1e-3 * true_rel
+    xd, infod = orc.cg(phi, b, m, g, 1.0, tol, 20000, "naive")
+    assert infod.converged
+    # the complex64 variant needs at least as many iterations as exact-arithmetic-like complex128
+    assert info.iterations >= infod.iterations - 2
+    assert info.iterations <= 1.3 * infod.iterations + 20
