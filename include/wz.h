@@ -1,0 +1,116 @@
+/* wz.h -- C-ABI of the B200 (sm_100a) hot path of arXiv:1005.3276:
+ * conjugate-gradient solve of  M^dag M x = b  for the lattice Wess-Zumino
+ * fermion matrix with the overlap (Neuberger) operator,
+ *
+ *   M = Dslash + m P+ + m* P- + 2g phi P+ + 2g* phi* P-,
+ *   Dslash = (1 - D2/2)^-1 D1                       (Eq. 2.19)
+ *
+ * applied as the paper does (Sec. 7): the phi-free part is
+ * diagonal in momentum space and is reached by a forward and an inverse 4D FFT
+ * with antiperiodic time boundary conditions; the Yukawa
+ * part is a site-local multiply in position space.
+ *
+ * Conventions:
+ *  - every data pointer is a DEVICE pointer owned by the caller; the library
+ *    allocates only the workspace and tables held by the plan;
+ *  - spinor field  = [batch][spin 0..3][x0 = t][x1][x2][x3], x3 fastest,
+ *    interleaved (re, im); spin 0,1 = P- (gamma5 = -1), spin 2,3 = P+
+ *    (Eq. 2.2);  phi = [x0][x1][x2][x3], shared by the batch;
+ *  - element type is complex64 (WZ_C64) or complex128 (WZ_C128), fixed per plan;
+ *  - every call is enqueued on the plan's stream and returns without
+ *    synchronising, except wz_cg_solve (see there);
+ *  - errors are returned, never thrown; there is no CPU fallback.
+ */
+#ifndef WZ_H_
+#define WZ_H_
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct wz_plan wz_plan; /* opaque */
+
+typedef enum { WZ_C64 = 0, WZ_C128 = 1 } wz_dtype;
+
+typedef enum {
+  WZ_OK = 0,
+  WZ_EINVAL = 1,        /* bad argument: null pointer, T odd, extent < 2, nbatch > max_batch,
+                           rho outside (0,2), tol <= 0, in == out where not allowed */
+  WZ_EUNSUPPORTED = 2,  /* lattice extents this build has no tile kernel for */
+  WZ_ENOMEM = 3,        /* device allocation of the plan workspace failed */
+  WZ_ECUDA = 4,         /* a CUDA call or launch failed (text via wz_last_error) */
+  WZ_ENOTCONVERGED = 5  /* wz_cg_solve: some source hit max_iter */
+} wz_status;
+
+const char *wz_status_string(wz_status s);
+/* Text of the last CUDA error seen by this thread's calls (empty string if none). */
+const char *wz_last_error(void);
+/* Library version, "major.minor". */
+const char *wz_version(void);
+
+/* Create a plan for a T x L1 x L2 x L3 lattice (T = extent of x0, the antiperiodic
+ * time direction; PAPER.md:234 requires T even).  `stream` is a cudaStream_t
+ * (0 = legacy default stream).  The plan owns: twiddle/momentum tables, the
+ * matvec temporaries (2 spinors per batch entry) and the CG vectors.  max_batch >= 1.
+ * Supported extents: (T,L1) and (L2,L3) pairs listed by wz_supported(). */
+wz_status wz_plan_create(wz_plan **plan, int T, int L1, int L2, int L3,
+                         wz_dtype dtype, int max_batch, void *stream);
+wz_status wz_plan_destroy(wz_plan *plan);
+/* 1 if this build has tile kernels for the lattice, else 0. */
+int wz_supported(int T, int L1, int L2, int L3, wz_dtype dtype);
+/* Bytes of device memory the plan holds. */
+unsigned long long wz_plan_workspace_bytes(const wz_plan *plan);
+
+/* 4D DFT of nbatch spinor fields (4 components each).
+ * direction +1: forward, kernel exp(-i p.x), unnormalised;
+ * direction -1: inverse, kernel exp(+i p.x), times 1/V.
+ * antiperiodic_time 0: p0 = 2 pi n0/T;  1: p0 = 2 pi (n0 + 1/2)/T, i.e. the field
+ * is multiplied by exp(-i pi x0/T) before the forward transform and by
+ * exp(+i pi x0/T) after the inverse one.
+ * in == out is allowed. */
+wz_status wz_fft4d(wz_plan *plan, int direction, int antiperiodic_time,
+                   const void *in, void *out, int nbatch);
+
+/* out = M in (dagger = 0) or M^dag in (dagger = 1), Eq. (2.19); m, g complex as
+ * {re, im}; 0 < rho < 2 is the overlap parameter (the paper has rho = 1).
+ * in == out is NOT allowed (in is re-read for the Yukawa term): WZ_EINVAL. */
+wz_status wz_apply_M(wz_plan *plan, int dagger, const void *phi,
+                     const double m[2], const double g[2], double rho,
+                     const void *in, void *out, int nbatch);
+
+/* out = M^dag M in. in == out is NOT allowed. */
+wz_status wz_apply_MdagM(wz_plan *plan, const void *phi,
+                         const double m[2], const double g[2], double rho,
+                         const void *in, void *out, int nbatch);
+
+typedef struct {
+  int iterations;       /* M^dag M applications inside the CG loop */
+  int reliable_updates; /* complex128 residual recomputations (WZ_C64 plans only) */
+  int converged;        /* 1 if the stop rule was met */
+  double rel_residual_recursive; /* sqrt(rho_k)/||b|| at exit */
+  double rel_residual_true;      /* ||b - M^dag M x|| / ||b||, recomputed at exit */
+} wz_cg_info;
+
+/* Conjugate gradient on M^dag M x = b, x0 = 0, one
+ * independent solve per source; stop when ||r||_2 <= tol ||b||_2.
+ *  - b: nbatch spinors of the plan's dtype (device).
+ *  - x: nbatch spinors, ALWAYS complex128 (device): WZ_C64 plans iterate in
+ *    complex64 with float64 reductions and accumulate the solution in complex128
+ *    by reliable updates (reading G9); rounding that solution to
+ *    complex64 would by itself lift the true residual above tol.
+ *  - info: HOST array of nbatch entries.
+ * Synchronises the plan's stream before returning.  Returns WZ_ENOTCONVERGED if
+ * any source hit max_iter; x then holds the last iterate. */
+wz_status wz_cg_solve(wz_plan *plan, const void *phi, const void *b, void *x,
+                      const double m[2], const double g[2], double rho,
+                      double tol, int max_iter, int nbatch, wz_cg_info *info);
+
+/* Number of kernel launches this plan has enqueued so far (for bench.py's
+ * gpu_launches), and a reset. */
+unsigned long long wz_plan_launch_count(const wz_plan *plan);
+void wz_plan_reset_launch_count(wz_plan *plan);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* WZ_H_ */

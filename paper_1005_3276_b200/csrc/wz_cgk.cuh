@@ -1,0 +1,163 @@
+// wz_cgk.cuh -- CG vector kernels:
+// fused AXPY pairs with float64 norm accumulation, the search-direction update,
+// and the complex128 reliable-update pieces for complex64 solves (G9).
+// Vectors are treated as flat real arrays of 2*4V entries, 16-byte accesses.
+#pragma once
+#include "wz_common.cuh"
+
+namespace wz {
+
+template <typename R>
+struct vec16;
+template <>
+struct vec16<float> {
+  typedef float4 T;
+  static constexpr int N = 4;
+};
+template <>
+struct vec16<double> {
+  typedef double2 T;
+  static constexpr int N = 2;
+};
+
+template <typename R>
+__device__ __forceinline__ void ld16(const R* p, R (&v)[vec16<R>::N]) {
+  typename vec16<R>::T t = *reinterpret_cast<const typename vec16<R>::T*>(p);
+  const R* q = reinterpret_cast<const R*>(&t);
+#pragma unroll
+  for (int i = 0; i < vec16<R>::N; ++i) v[i] = q[i];
+}
+template <typename R>
+__device__ __forceinline__ void st16(R* p, const R (&v)[vec16<R>::N]) {
+  typename vec16<R>::T t;
+  R* q = reinterpret_cast<R*>(&t);
+#pragma unroll
+  for (int i = 0; i < vec16<R>::N; ++i) q[i] = v[i];
+  *reinterpret_cast<typename vec16<R>::T*>(p) = t;
+}
+
+constexpr int CGK_NT = 256;
+
+// r = b, p = b, xs = 0 (if given), X = 0 (complex128, if given); ||b||^2 -> FIN_INIT
+template <typename R>
+__global__ void __launch_bounds__(CGK_NT)
+k_cg_init(const R* __restrict__ b, R* __restrict__ r, R* __restrict__ p, R* __restrict__ xs,
+          double* __restrict__ X, long n, RedArgs red) {
+  constexpr int N = vec16<R>::N;
+  __shared__ double sh[33];
+  double acc = 0.0;
+  for (long i = ((long)blockIdx.x * blockDim.x + threadIdx.x) * N; i < n;
+       i += (long)gridDim.x * blockDim.x * N) {
+    R v[N], z[N];
+    ld16<R>(b + i, v);
+#pragma unroll
+    for (int e = 0; e < N; ++e) {
+      acc += (double)v[e] * (double)v[e];
+      z[e] = R(0);
+    }
+    st16<R>(r + i, v);
+    st16<R>(p + i, v);
+    if (xs) st16<R>(xs + i, z);
+    if (X) {
+#pragma unroll
+      for (int e = 0; e < N; ++e) X[i + e] = 0.0;
+    }
+  }
+  grid_reduce<FIN_INIT>(acc, red, blockIdx.x, gridDim.x, sh);
+}
+
+// x += alpha p;  r -= alpha q;  ||r||^2 -> FIN_RR.   TX: type of x (R, or double for
+// complex128 solves writing straight into the caller's buffer).
+template <typename R, typename TX>
+__global__ void __launch_bounds__(CGK_NT)
+k_update_xr(TX* __restrict__ x, R* __restrict__ r, const R* __restrict__ p,
+            const R* __restrict__ q, long n, RedArgs red) {
+  constexpr int N = vec16<R>::N;
+  __shared__ double sh[33];
+  if (!cg_active(red.st)) return;
+  const R alpha = (R)red.st->alpha;
+  double acc = 0.0;
+  for (long i = ((long)blockIdx.x * blockDim.x + threadIdx.x) * N; i < n;
+       i += (long)gridDim.x * blockDim.x * N) {
+    R vp[N], vq[N], vr[N];
+    ld16<R>(p + i, vp);
+    ld16<R>(q + i, vq);
+    ld16<R>(r + i, vr);
+#pragma unroll
+    for (int e = 0; e < N; ++e) {
+      x[i + e] = (TX)((R)x[i + e] + alpha * vp[e]);
+      vr[e] = vr[e] - alpha * vq[e];
+      acc += (double)vr[e] * (double)vr[e];
+    }
+    st16<R>(r + i, vr);
+  }
+  grid_reduce<FIN_RR>(acc, red, blockIdx.x, gridDim.x, sh);
+}
+
+// p = r + beta p
+template <typename R>
+__global__ void __launch_bounds__(CGK_NT)
+k_update_p(R* __restrict__ p, const R* __restrict__ r, long n, const CGState* st) {
+  constexpr int N = vec16<R>::N;
+  if (!cg_active(st)) return;
+  const R beta = (R)st->beta;
+  for (long i = ((long)blockIdx.x * blockDim.x + threadIdx.x) * N; i < n;
+       i += (long)gridDim.x * blockDim.x * N) {
+    R vp[N], vr[N];
+    ld16<R>(p + i, vp);
+    ld16<R>(r + i, vr);
+#pragma unroll
+    for (int e = 0; e < N; ++e) vp[e] = vr[e] + beta * vp[e];
+    st16<R>(p + i, vp);
+  }
+}
+
+// Reliable update, part 1:  X += xs (complex128 += complex64);  xs = 0.
+__global__ void __launch_bounds__(CGK_NT)
+k_ru_accum(double* __restrict__ X, float* __restrict__ xs, long n) {
+  for (long i = ((long)blockIdx.x * blockDim.x + threadIdx.x) * 4; i < n;
+       i += (long)gridDim.x * blockDim.x * 4) {
+    float v[4], z[4] = {0.f, 0.f, 0.f, 0.f};
+    ld16<float>(xs + i, v);
+    double2 a = *reinterpret_cast<double2*>(X + i), c = *reinterpret_cast<double2*>(X + i + 2);
+    a.x += (double)v[0];
+    a.y += (double)v[1];
+    c.x += (double)v[2];
+    c.y += (double)v[3];
+    *reinterpret_cast<double2*>(X + i) = a;
+    *reinterpret_cast<double2*>(X + i + 2) = c;
+    st16<float>(xs + i, z);
+  }
+}
+
+// Residual in float64:  d = b - q;  sum |d|^2 -> FIN;  r = round(d) (if r given).
+// TB: storage type of b, TR: storage type of r.
+template <typename TB, typename TR, int FIN>
+__global__ void __launch_bounds__(CGK_NT)
+k_resid(const TB* __restrict__ b, const double* __restrict__ q, TR* __restrict__ r, long n,
+        RedArgs red) {
+  __shared__ double sh[33];
+  double acc = 0.0;
+  for (long i = ((long)blockIdx.x * blockDim.x + threadIdx.x) * 2; i < n;
+       i += (long)gridDim.x * blockDim.x * 2) {
+    double2 vq = *reinterpret_cast<const double2*>(q + i);
+    double d0 = (double)b[i] - vq.x, d1 = (double)b[i + 1] - vq.y;
+    acc += d0 * d0 + d1 * d1;
+    if (r) {
+      r[i] = (TR)d0;
+      r[i + 1] = (TR)d1;
+    }
+  }
+  grid_reduce<FIN>(acc, red, blockIdx.x, gridDim.x, sh);
+}
+
+// dst (double) = src (float), element-wise (phi for the complex128 operator of a
+// complex64 plan: the float-rounded values, exactly what the oracle consumes).
+__global__ void __launch_bounds__(CGK_NT)
+k_f2d(double* __restrict__ dst, const float* __restrict__ src, long n) {
+  for (long i = (long)blockIdx.x * blockDim.x + threadIdx.x; i < n;
+       i += (long)gridDim.x * blockDim.x)
+    dst[i] = (double)src[i];
+}
+
+}  // namespace wz

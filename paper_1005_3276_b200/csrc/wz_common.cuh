@@ -1,0 +1,150 @@
+// wz_common.cuh -- shared device-side types of the wz kernels: operator
+// parameters, the device-resident CG state, and the fixed-order block/grid
+// reduction with a "last block finalises" step (no host round trip, results
+// independent of block scheduling order).
+#pragma once
+#include <cuda_runtime.h>
+
+#include "wz_regfft.cuh"
+
+namespace wz {
+
+// Yukawa/mass and overlap parameters of Eq. (2.19).
+template <typename R>
+struct OpParams {
+  R m_re, m_im;    // m
+  R g2_re, g2_im;  // 2 g
+  R rho;           // overlap parameter (paper: 1)
+  int dagger;      // 0: M, 1: M^dag
+};
+
+// Device-resident scalars of one CG solve.
+struct CGState {
+  double bnorm2, bnorm;  // ||b||^2, ||b||
+  double rr;             // rho_{k-1} = <r,r>
+  double rr_new;         // rho_k candidate
+  double pq;             // <p, M^dag M p> = ||M p||^2
+  double alpha, beta;
+  double rmax;           // max ||r|| since the last reliable update (G9)
+  double tol, delta;
+  double true_rr;        // ||b - A x||^2 recomputed
+  int iter, max_iter;
+  int n_ru;
+  int converged;  // stop rule met
+  int need_ru;    // reliable update requested; iteration kernels idle until served
+  int stop;       // max_iter reached
+  int use_ru;     // 1: complex64 vectors + reliable updates; 0: plain CG
+  int pad_;
+};
+
+__device__ __forceinline__ bool cg_active(const CGState* st) {
+  return !(st->converged | st->need_ru | st->stop);
+}
+
+// What the last block of a reduction does with the total.
+enum { FIN_STORE = 0, FIN_PQ = 1, FIN_RR = 2, FIN_RU = 3, FIN_INIT = 4, FIN_TRUE = 5 };
+
+template <int FIN>
+__device__ __forceinline__ void cg_finalize(double total, CGState* st, double* store) {
+  if (FIN == FIN_STORE) {
+    *store = total;
+  } else if (FIN == FIN_PQ) {  // alpha = rho_{k-1} / <p, A p>
+    st->pq = total;
+    st->alpha = st->rr / total;
+  } else if (FIN == FIN_INIT) {  // r0 = p0 = b
+    st->bnorm2 = total;
+    st->bnorm = sqrt(total);
+    st->rr = total;
+    st->rmax = sqrt(total);
+    if (total == 0.0) st->converged = 1;
+  } else if (FIN == FIN_RR) {  // after x += alpha p, r -= alpha q
+    const double rn = sqrt(total);
+    st->iter += 1;
+    if (st->use_ru) {
+      if (rn > st->rmax) st->rmax = rn;
+      if (rn < st->delta * st->rmax || rn <= st->tol * st->bnorm) {
+        st->rr_new = total;
+        st->need_ru = 1;
+      } else {
+        st->beta = total / st->rr;
+        st->rr = total;
+      }
+    } else {
+      if (rn <= st->tol * st->bnorm) {
+        st->converged = 1;
+      } else {
+        st->beta = total / st->rr;
+      }
+      st->rr = total;
+    }
+    if (!st->converged && !st->need_ru && st->iter >= st->max_iter) st->stop = 1;
+  } else if (FIN == FIN_RU) {  // r = b - A X recomputed in complex128
+    const double rn = sqrt(total);
+    st->n_ru += 1;
+    st->rmax = rn;
+    st->true_rr = total;
+    if (rn <= st->tol * st->bnorm) st->converged = 1;
+    st->beta = total / st->rr;
+    st->rr = total;
+    st->need_ru = 0;
+    if (!st->converged && st->iter >= st->max_iter) st->stop = 1;
+  } else if (FIN == FIN_TRUE) {
+    st->true_rr = total;
+  }
+}
+
+// Reduction workspace: one partial per block, a ticket counter, and the target.
+struct RedArgs {
+  double* partials;   // [nblocks]
+  unsigned* counter;  // zero before first use; left zero after each use
+  CGState* st;
+  double* store;      // FIN_STORE target
+};
+
+// Sum `v` over the block in a fixed order; returns the total in thread 0.
+__device__ __forceinline__ double block_sum(double v, double* sh /* >= 32 doubles */) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  const int nw = (blockDim.x + 31) >> 5;
+  __syncthreads();
+  if (lane == 0) sh[wid] = v;
+  __syncthreads();
+  double t = 0.0;
+  if (wid == 0) {
+    t = (lane < nw) ? sh[lane] : 0.0;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) t += __shfl_down_sync(0xffffffffu, t, o);
+  }
+  return t;
+}
+
+// Each block contributes `v` (per thread); the last block to arrive sums all
+// partials in index order and runs cg_finalize<FIN>.  `blk`/`nblk`: linear block id
+// and count.  All threads of the block must call this.
+template <int FIN>
+__device__ __forceinline__ void grid_reduce(double v, const RedArgs& ra, int blk, int nblk,
+                                            double* sh /* >= 33 doubles */) {
+  double t = block_sum(v, sh);
+  __shared__ int s_last;
+  if (threadIdx.x == 0) {
+    ra.partials[blk] = t;
+    __threadfence();
+    unsigned ticket = atomicAdd(ra.counter, 1u);
+    s_last = (ticket == (unsigned)(nblk - 1));
+  }
+  __syncthreads();
+  if (s_last) {
+    __threadfence();
+    double acc = 0.0;
+    for (int i = threadIdx.x; i < nblk; i += blockDim.x) acc += __ldcg(ra.partials + i);
+    double tot = block_sum(acc, sh);
+    if (threadIdx.x == 0) {
+      cg_finalize<FIN>(tot, ra.st, ra.store);
+      *ra.counter = 0u;
+      __threadfence();
+    }
+  }
+}
+
+}  // namespace wz

@@ -1,0 +1,646 @@
+// wz_lib.cu -- host side of the C-ABI in include/wz.h: plans, tables, kernel
+// dispatch, the matvec pass schedule and the CG driver.  sm_100a only; there is no
+// CPU path: every entry point either enqueues kernels or returns an error.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "../../include/wz.h"
+#include "wz_cgk.cuh"
+#include "wz_p01.cuh"
+#include "wz_p23.cuh"
+
+using namespace wz;
+
+namespace {
+
+thread_local char g_err[512] = "";
+
+bool cuda_ok(cudaError_t e, const char* what) {
+  if (e == cudaSuccess) return true;
+  snprintf(g_err, sizeof(g_err), "%s: %s", what, cudaGetErrorString(e));
+  return false;
+}
+#define WZ_CUDA(call)                                   \
+  do {                                                  \
+    if (!cuda_ok((call), #call)) return WZ_ECUDA;       \
+  } while (0)
+
+// ---- kernel dispatch tables ---------------------------------------------------
+template <typename R>
+struct P01Entry {
+  int L0, L1, nseg, nt;
+  size_t smem;
+  void (*fwd)(const P01Args<R>);
+  void (*inv)(const P01Args<R>);
+  void (*mid)(const P01Args<R>);      // no reduction
+  void (*mid_pq)(const P01Args<R>);   // ||chi||^2 -> alpha
+  void (*end)(const P01Args<R>);
+};
+template <typename R>
+struct P23Entry {
+  int L2, L3, nt;
+  size_t smem;
+  void (*fwd)(const P23Args<R>);
+  void (*inv)(const P23Args<R>);
+  void (*mult)(const P23Args<R>);
+};
+
+template <typename R, int L0, int L1, int NSEG>
+P01Entry<R> make_p01() {
+  using C = P01Cfg<R, L0, L1, NSEG>;
+  P01Entry<R> e;
+  e.L0 = L0; e.L1 = L1; e.nseg = NSEG; e.nt = C::NT; e.smem = C::SMEM;
+  e.fwd = k_p01<R, L0, L1, NSEG, P01_FWD, FIN_STORE>;
+  e.inv = k_p01<R, L0, L1, NSEG, P01_INV, FIN_STORE>;
+  e.mid = k_p01<R, L0, L1, NSEG, P01_MID, FIN_STORE>;
+  e.mid_pq = k_p01<R, L0, L1, NSEG, P01_MID, FIN_PQ>;
+  e.end = k_p01<R, L0, L1, NSEG, P01_END, FIN_STORE>;
+  return e;
+}
+template <typename R, int L2, int L3>
+P23Entry<R> make_p23() {
+  using C = P23Cfg<R, L2, L3>;
+  P23Entry<R> e;
+  e.L2 = L2; e.L3 = L3; e.nt = C::NT; e.smem = C::SMEM;
+  e.fwd = k_p23<R, L2, L3, P23_FFT, +1>;
+  e.inv = k_p23<R, L2, L3, P23_FFT, -1>;
+  e.mult = k_p23<R, L2, L3, P23_MULT, +1>;
+  return e;
+}
+
+// NSEG: consecutive (x2,x3) sites per strided tile; chosen so that the tile
+// L0 x L1 x NSEG stays <= 128 KB and each contiguous run is >= 32 bytes.
+template <typename R> struct nseg_for {
+  static constexpr int small = (sizeof(R) == 4) ? 8 : 4;
+  static constexpr int big = (sizeof(R) == 4) ? 4 : 2;
+};
+
+template <typename R>
+const std::vector<P01Entry<R>>& p01_table() {
+  static const std::vector<P01Entry<R>> t = {
+      make_p01<R, 4, 4, nseg_for<R>::small>(),   make_p01<R, 8, 8, nseg_for<R>::small>(),
+      make_p01<R, 8, 4, nseg_for<R>::small>(),   make_p01<R, 16, 16, nseg_for<R>::small>(),
+      make_p01<R, 32, 32, nseg_for<R>::small>(), make_p01<R, 48, 24, nseg_for<R>::small>(),
+      make_p01<R, 64, 64, nseg_for<R>::big>(),
+  };
+  return t;
+}
+template <typename R>
+const std::vector<P23Entry<R>>& p23_table() {
+  static const std::vector<P23Entry<R>> t = [] {
+    std::vector<P23Entry<R>> v = {
+        make_p23<R, 4, 4>(),   make_p23<R, 8, 8>(),   make_p23<R, 16, 8>(), make_p23<R, 16, 16>(),
+        make_p23<R, 32, 32>(), make_p23<R, 24, 24>(),
+    };
+    // four 64x64 complex128 planes (266 KB) exceed one SM's shared memory
+    if constexpr (sizeof(R) == 4) v.push_back(make_p23<R, 64, 64>());
+    return v;
+  }();
+  return t;
+}
+template <typename R>
+const P01Entry<R>* find_p01(int L0, int L1) {
+  for (const auto& e : p01_table<R>())
+    if (e.L0 == L0 && e.L1 == L1) return &e;
+  return nullptr;
+}
+template <typename R>
+const P23Entry<R>* find_p23(int L2, int L3) {
+  for (const auto& e : p23_table<R>())
+    if (e.L2 == L2 && e.L3 == L3) return &e;
+  return nullptr;
+}
+
+template <typename K>
+bool set_smem(K kernel, size_t bytes) {
+  if (bytes <= 48 * 1024) return true;
+  return cuda_ok(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes),
+                 "cudaFuncSetAttribute(MaxDynamicSharedMemorySize)");
+}
+
+// ---- per-precision operator workspace -------------------------------------------
+template <typename R>
+struct OpWS {
+  const P01Entry<R>* p01 = nullptr;
+  const P23Entry<R>* p23 = nullptr;
+  R* tab = nullptr;        // momentum tables [2][4][64]
+  cpx<R>* t = nullptr;     // FFT temporary, max_batch spinors
+  cpx<R>* chi = nullptr;   // chi = M psi,   max_batch spinors
+};
+
+}  // namespace
+
+struct wz_plan {
+  int L[4];
+  long V, I;
+  wz_dtype dtype;
+  int max_batch;
+  cudaStream_t stream;
+  unsigned long long bytes = 0, launches = 0;
+  double rho_tab = -1.0;  // rho the momentum tables do not depend on; kept for clarity
+  OpWS<float> wsf;
+  OpWS<double> wsd;        // always present: complex128 operator (plans of both dtypes)
+  // CG vectors
+  void *r = nullptr, *p = nullptr, *q = nullptr, *xs = nullptr;  // plan dtype, one spinor each
+  cpx<double>* q128 = nullptr;    // C64 plans: A X in complex128
+  cpx<double>* phi128 = nullptr;  // C64 plans: phi widened
+  double* partials = nullptr;
+  unsigned* counter = nullptr;
+  CGState* d_state = nullptr;
+  CGState* h_state = nullptr;  // pinned, 2 slots
+  cudaEvent_t ev[2] = {nullptr, nullptr};
+  int npartials = 0;
+  std::vector<void*> allocs;
+};
+
+namespace {
+
+const double kPi = 3.14159265358979323846264338327950288;
+
+// exp(-2 pi i j/TWN) in both precisions; written once per process.
+bool init_twiddles() {
+  static bool done = false;
+  if (done) return true;
+  std::vector<float2> tf(TWN);
+  std::vector<double2> td(TWN);
+  for (int j = 0; j < TWN; ++j) {
+    // exact values on the axes and diagonals, symmetric elsewhere (octant reduction)
+    int o = j % TWN;
+    double ang = 2.0 * kPi * (double)o / (double)TWN;
+    double c = std::cos(ang), s = std::sin(ang);
+    if (o % (TWN / 4) == 0) {
+      const int qd = o / (TWN / 4);
+      c = (qd == 0) ? 1.0 : (qd == 2) ? -1.0 : 0.0;
+      s = (qd == 1) ? 1.0 : (qd == 3) ? -1.0 : 0.0;
+    }
+    td[j] = make_double2(c, -s);
+    tf[j] = make_float2((float)c, (float)-s);
+  }
+  if (!cuda_ok(cudaMemcpyToSymbol(c_twf, tf.data(), sizeof(float2) * TWN), "cudaMemcpyToSymbol(c_twf)")) return false;
+  if (!cuda_ok(cudaMemcpyToSymbol(c_twd, td.data(), sizeof(double2) * TWN), "cudaMemcpyToSymbol(c_twd)")) return false;
+  done = true;
+  return true;
+}
+
+template <typename T>
+bool dev_alloc(wz_plan* pl, T** ptr, size_t count) {
+  void* p = nullptr;
+  size_t bytes = count * sizeof(T);
+  if (bytes == 0) bytes = sizeof(T);
+  cudaError_t e = cudaMalloc(&p, bytes);
+  if (e != cudaSuccess) {
+    snprintf(g_err, sizeof(g_err), "cudaMalloc(%zu bytes): %s", bytes, cudaGetErrorString(e));
+    cudaGetLastError();
+    return false;
+  }
+  pl->allocs.push_back(p);
+  pl->bytes += bytes;
+  *ptr = reinterpret_cast<T*>(p);
+  return true;
+}
+
+// Momentum tables (p0 = 2 pi (n0 + 1/2)/T, p_i = 2 pi n_i/L_i),
+// computed in double on the host: tab[0][mu][n] = sin p_mu, tab[1][mu][n] = sin^2(p_mu/2).
+template <typename R>
+wz_status setup_ws(wz_plan* pl, OpWS<R>& ws, int nbatch_t) {
+  ws.p01 = find_p01<R>(pl->L[0], pl->L[1]);
+  ws.p23 = find_p23<R>(pl->L[2], pl->L[3]);
+  if (!ws.p01 || !ws.p23) return WZ_EUNSUPPORTED;
+  if (pl->I % ws.p01->nseg != 0) return WZ_EUNSUPPORTED;
+  const auto* a = ws.p01;
+  if (!set_smem(a->fwd, a->smem) || !set_smem(a->inv, a->smem) || !set_smem(a->mid, a->smem) ||
+      !set_smem(a->mid_pq, a->smem) || !set_smem(a->end, a->smem))
+    return WZ_ECUDA;
+  const auto* b = ws.p23;
+  if (!set_smem(b->fwd, b->smem) || !set_smem(b->inv, b->smem) || !set_smem(b->mult, b->smem))
+    return WZ_ECUDA;
+  std::vector<R> h(2 * 4 * 64, R(0));
+  for (int mu = 0; mu < 4; ++mu)
+    for (int n = 0; n < pl->L[mu]; ++n) {
+      const double p = 2.0 * kPi * ((double)n + (mu == 0 ? 0.5 : 0.0)) / (double)pl->L[mu];
+      const double sh = std::sin(0.5 * p);
+      h[(0 * 4 + mu) * 64 + n] = (R)std::sin(p);
+      h[(1 * 4 + mu) * 64 + n] = (R)(sh * sh);
+    }
+  if (!dev_alloc(pl, &ws.tab, h.size())) return WZ_ENOMEM;
+  WZ_CUDA(cudaMemcpyAsync(ws.tab, h.data(), sizeof(R) * h.size(), cudaMemcpyHostToDevice, pl->stream));
+  WZ_CUDA(cudaStreamSynchronize(pl->stream));
+  const size_t n = (size_t)nbatch_t * 4 * pl->V;
+  if (!dev_alloc(pl, &ws.t, n) || !dev_alloc(pl, &ws.chi, n)) return WZ_ENOMEM;
+  return WZ_OK;
+}
+
+template <typename R, typename A>
+wz_status launch(wz_plan* pl, void (*k)(const A), dim3 grid, int nt, size_t smem, const A& args) {
+  k<<<grid, nt, smem, pl->stream>>>(args);
+  pl->launches++;
+  WZ_CUDA(cudaGetLastError());
+  return WZ_OK;
+}
+
+template <typename R>
+OpWS<R>& ws_of(wz_plan* pl);
+template <>
+OpWS<float>& ws_of<float>(wz_plan* pl) { return pl->wsf; }
+template <>
+OpWS<double>& ws_of<double>(wz_plan* pl) { return pl->wsd; }
+
+template <typename R>
+OpParams<R> make_op(const double m[2], const double g[2], double rho, int dagger) {
+  OpParams<R> op;
+  op.m_re = (R)m[0]; op.m_im = (R)m[1];
+  op.g2_re = (R)(2.0 * g[0]); op.g2_im = (R)(2.0 * g[1]);
+  op.rho = (R)rho; op.dagger = dagger;
+  return op;
+}
+
+// ---- 4D FFT (steps a1, a2 / a4, a5) ---------------------------------------------
+template <typename R>
+wz_status fft4d_impl(wz_plan* pl, int direction, int apbc, const cpx<R>* in, cpx<R>* out, int nb) {
+  OpWS<R>& ws = ws_of<R>(pl);
+  const dim3 g01((unsigned)(pl->I / ws.p01->nseg), (unsigned)(nb * 4));
+  const dim3 g23((unsigned)(pl->L[0] * pl->L[1]), (unsigned)nb);
+  P01Args<R> a{};
+  a.I = pl->I; a.apbc = apbc; a.scale = R(1);
+  P23Args<R> b{};
+  b.nplanes = pl->L[0] * pl->L[1]; b.L1 = pl->L[1]; b.scale = R(1); b.tab = ws.tab;
+  b.rho = R(1); b.sign = R(1);
+  if (direction > 0) {
+    a.in = in; a.out = out;
+    wz_status s = launch<R>(pl, ws.p01->fwd, g01, ws.p01->nt, ws.p01->smem, a);
+    if (s != WZ_OK) return s;
+    b.in = out; b.out = out;
+    return launch<R>(pl, ws.p23->fwd, g23, ws.p23->nt, ws.p23->smem, b);
+  }
+  b.in = in; b.out = out;
+  wz_status s = launch<R>(pl, ws.p23->inv, g23, ws.p23->nt, ws.p23->smem, b);
+  if (s != WZ_OK) return s;
+  a.in = out; a.out = out; a.scale = (R)(1.0 / (double)pl->V);
+  return launch<R>(pl, ws.p01->inv, g01, ws.p01->nt, ws.p01->smem, a);
+}
+
+// ---- out = M in or M^dag in: passes A, B, E --------------------------
+template <typename R>
+wz_status apply_M_impl(wz_plan* pl, int dagger, const cpx<R>* phi, const double m[2], const double g[2],
+                       double rho, const cpx<R>* in, cpx<R>* out, int nb) {
+  OpWS<R>& ws = ws_of<R>(pl);
+  const dim3 g01((unsigned)(pl->I / ws.p01->nseg), (unsigned)(nb * 4));
+  const dim3 g23((unsigned)(pl->L[0] * pl->L[1]), (unsigned)nb);
+  P01Args<R> a{};
+  a.I = pl->I; a.apbc = 1; a.scale = R(1);
+  a.in = in; a.out = ws.t;
+  wz_status s = launch<R>(pl, ws.p01->fwd, g01, ws.p01->nt, ws.p01->smem, a);
+  if (s != WZ_OK) return s;
+  P23Args<R> b{};
+  b.in = ws.t; b.out = ws.t; b.nplanes = pl->L[0] * pl->L[1]; b.L1 = pl->L[1]; b.scale = R(1);
+  b.tab = ws.tab; b.rho = (R)rho; b.sign = dagger ? R(-1) : R(1);
+  s = launch<R>(pl, ws.p23->mult, g23, ws.p23->nt, ws.p23->smem, b);
+  if (s != WZ_OK) return s;
+  a.in = ws.t; a.out = ws.t; a.scale = (R)(1.0 / (double)pl->V);
+  a.psi = in; a.phi = phi; a.site_out = out; a.op = make_op<R>(m, g, rho, dagger);
+  return launch<R>(pl, ws.p01->end, g01, ws.p01->nt, ws.p01->smem, a);
+}
+
+// ---- out = M^dag M in: passes A-E.  With `cg` set (nb = 1) the kernels are gated on
+// the solve being active and pass C leaves alpha = rho/<p, A p> in the CG state. -----
+template <typename R>
+wz_status apply_MdagM_impl(wz_plan* pl, const cpx<R>* phi, const double m[2], const double g[2],
+                           double rho, const cpx<R>* in, cpx<R>* out, int nb, bool cg) {
+  OpWS<R>& ws = ws_of<R>(pl);
+  const dim3 g01((unsigned)(pl->I / ws.p01->nseg), (unsigned)(nb * 4));
+  const dim3 g23((unsigned)(pl->L[0] * pl->L[1]), (unsigned)nb);
+  const CGState* gate = cg ? pl->d_state : nullptr;
+  const R invV = (R)(1.0 / (double)pl->V);
+  wz_status s;
+  P01Args<R> a{};
+  a.I = pl->I; a.apbc = 1; a.scale = R(1); a.gate = gate;
+  a.in = in; a.out = ws.t;
+  if ((s = launch<R>(pl, ws.p01->fwd, g01, ws.p01->nt, ws.p01->smem, a)) != WZ_OK) return s;  // A
+  P23Args<R> b{};
+  b.in = ws.t; b.out = ws.t; b.nplanes = pl->L[0] * pl->L[1]; b.L1 = pl->L[1]; b.scale = R(1);
+  b.tab = ws.tab; b.rho = (R)rho; b.sign = R(1); b.gate = gate;
+  if ((s = launch<R>(pl, ws.p23->mult, g23, ws.p23->nt, ws.p23->smem, b)) != WZ_OK) return s;  // B
+  a.in = ws.t; a.out = ws.t; a.scale = invV;
+  a.psi = in; a.phi = phi; a.site_out = ws.chi; a.op = make_op<R>(m, g, rho, 0);
+  if (cg) {
+    a.red.partials = pl->partials; a.red.counter = pl->counter; a.red.st = pl->d_state; a.red.store = nullptr;
+    if ((int)(g01.x * g01.y) > pl->npartials) return WZ_EINVAL;
+    s = launch<R>(pl, ws.p01->mid_pq, g01, ws.p01->nt, ws.p01->smem, a);  // C
+  } else {
+    s = launch<R>(pl, ws.p01->mid, g01, ws.p01->nt, ws.p01->smem, a);
+  }
+  if (s != WZ_OK) return s;
+  b.sign = R(-1);
+  if ((s = launch<R>(pl, ws.p23->mult, g23, ws.p23->nt, ws.p23->smem, b)) != WZ_OK) return s;  // D
+  a.red = RedArgs{};
+  a.psi = ws.chi; a.site_out = out; a.op = make_op<R>(m, g, rho, 1);
+  return launch<R>(pl, ws.p01->end, g01, ws.p01->nt, ws.p01->smem, a);  // E
+}
+
+}  // namespace
+
+// =============================== C ABI =========================================
+extern "C" {
+
+const char* wz_status_string(wz_status s) {
+  switch (s) {
+    case WZ_OK: return "ok";
+    case WZ_EINVAL: return "invalid argument";
+    case WZ_EUNSUPPORTED: return "unsupported lattice extents";
+    case WZ_ENOMEM: return "out of device memory";
+    case WZ_ECUDA: return "CUDA error";
+    case WZ_ENOTCONVERGED: return "CG did not converge within max_iter";
+  }
+  return "unknown status";
+}
+const char* wz_last_error(void) { return g_err; }
+const char* wz_version(void) { return "0.1"; }
+
+int wz_supported(int T, int L1, int L2, int L3, wz_dtype dtype) {
+  if (T < 2 || (T & 1)) return 0;
+  const long I = (long)L2 * L3;
+  // every plan needs the complex128 operator (reliable updates, true residual)
+  const auto* ad = find_p01<double>(T, L1);
+  const auto* bd = find_p23<double>(L2, L3);
+  if (!ad || !bd || I % ad->nseg) return 0;
+  if (dtype == WZ_C64) {
+    const auto* af = find_p01<float>(T, L1);
+    const auto* bf = find_p23<float>(L2, L3);
+    if (!af || !bf || I % af->nseg) return 0;
+  }
+  return 1;
+}
+
+wz_status wz_plan_destroy(wz_plan* pl) {
+  if (!pl) return WZ_EINVAL;
+  for (void* p : pl->allocs) cudaFree(p);
+  if (pl->h_state) cudaFreeHost(pl->h_state);
+  for (int i = 0; i < 2; ++i)
+    if (pl->ev[i]) cudaEventDestroy(pl->ev[i]);
+  delete pl;
+  return WZ_OK;
+}
+
+wz_status wz_plan_create(wz_plan** plan, int T, int L1, int L2, int L3, wz_dtype dtype,
+                         int max_batch, void* stream) {
+  g_err[0] = 0;
+  if (!plan) return WZ_EINVAL;
+  *plan = nullptr;
+  if (T < 2 || L1 < 2 || L2 < 2 || L3 < 2 || (T & 1) || max_batch < 1) return WZ_EINVAL;
+  if (dtype != WZ_C64 && dtype != WZ_C128) return WZ_EINVAL;
+  if (!wz_supported(T, L1, L2, L3, dtype)) return WZ_EUNSUPPORTED;
+  if (!init_twiddles()) return WZ_ECUDA;
+  wz_plan* pl = new (std::nothrow) wz_plan();
+  if (!pl) return WZ_ENOMEM;
+  pl->L[0] = T; pl->L[1] = L1; pl->L[2] = L2; pl->L[3] = L3;
+  pl->I = (long)L2 * L3;
+  pl->V = (long)T * L1 * pl->I;
+  pl->dtype = dtype;
+  pl->max_batch = max_batch;
+  pl->stream = (cudaStream_t)stream;
+  wz_status s = WZ_OK;
+  const size_t n1 = (size_t)4 * pl->V;
+  do {
+    if (dtype == WZ_C64) {
+      if ((s = setup_ws<float>(pl, pl->wsf, max_batch)) != WZ_OK) break;
+      if ((s = setup_ws<double>(pl, pl->wsd, 1)) != WZ_OK) break;
+      float *r, *p, *q, *xs;
+      if (!dev_alloc(pl, &r, 2 * n1) || !dev_alloc(pl, &p, 2 * n1) || !dev_alloc(pl, &q, 2 * n1) ||
+          !dev_alloc(pl, &xs, 2 * n1) || !dev_alloc(pl, &pl->q128, n1) ||
+          !dev_alloc(pl, &pl->phi128, (size_t)pl->V)) { s = WZ_ENOMEM; break; }
+      pl->r = r; pl->p = p; pl->q = q; pl->xs = xs;
+    } else {
+      if ((s = setup_ws<double>(pl, pl->wsd, max_batch)) != WZ_OK) break;
+      double *r, *p, *q;
+      if (!dev_alloc(pl, &r, 2 * n1) || !dev_alloc(pl, &p, 2 * n1) || !dev_alloc(pl, &q, 2 * n1)) {
+        s = WZ_ENOMEM; break;
+      }
+      pl->r = r; pl->p = p; pl->q = q;
+    }
+    // reduction workspace: enough partials for the widest grid used in a solve
+    const int nseg_min = 2;
+    long np = (pl->I / nseg_min) * 4;
+    if (np < 4096) np = 4096;
+    pl->npartials = (int)np;
+    if (!dev_alloc(pl, &pl->partials, (size_t)np) || !dev_alloc(pl, &pl->counter, 4) ||
+        !dev_alloc(pl, &pl->d_state, 1)) { s = WZ_ENOMEM; break; }
+    if (!cuda_ok(cudaMemsetAsync(pl->counter, 0, 4 * sizeof(unsigned), pl->stream), "cudaMemsetAsync") ||
+        !cuda_ok(cudaMemsetAsync(pl->d_state, 0, sizeof(CGState), pl->stream), "cudaMemsetAsync") ||
+        !cuda_ok(cudaMallocHost((void**)&pl->h_state, 2 * sizeof(CGState)), "cudaMallocHost") ||
+        !cuda_ok(cudaEventCreateWithFlags(&pl->ev[0], cudaEventDisableTiming), "cudaEventCreate") ||
+        !cuda_ok(cudaEventCreateWithFlags(&pl->ev[1], cudaEventDisableTiming), "cudaEventCreate") ||
+        !cuda_ok(cudaStreamSynchronize(pl->stream), "cudaStreamSynchronize")) { s = WZ_ECUDA; break; }
+  } while (0);
+  if (s != WZ_OK) {
+    wz_plan_destroy(pl);
+    return s;
+  }
+  *plan = pl;
+  return WZ_OK;
+}
+
+unsigned long long wz_plan_workspace_bytes(const wz_plan* pl) { return pl ? pl->bytes : 0ull; }
+unsigned long long wz_plan_launch_count(const wz_plan* pl) { return pl ? pl->launches : 0ull; }
+void wz_plan_reset_launch_count(wz_plan* pl) { if (pl) pl->launches = 0; }
+
+wz_status wz_fft4d(wz_plan* pl, int direction, int antiperiodic_time, const void* in, void* out,
+                   int nbatch) {
+  g_err[0] = 0;
+  if (!pl || !in || !out || (direction != 1 && direction != -1)) return WZ_EINVAL;
+  if (nbatch < 0 || nbatch > pl->max_batch) return WZ_EINVAL;
+  if (nbatch == 0) return WZ_OK;
+  const int ap = antiperiodic_time ? 1 : 0;
+  if (pl->dtype == WZ_C64)
+    return fft4d_impl<float>(pl, direction, ap, (const cpx<float>*)in, (cpx<float>*)out, nbatch);
+  return fft4d_impl<double>(pl, direction, ap, (const cpx<double>*)in, (cpx<double>*)out, nbatch);
+}
+
+static wz_status check_op(const wz_plan* pl, const void* phi, const double* m, const double* g,
+                          double rho, const void* in, const void* out, int nbatch) {
+  if (!pl || !phi || !m || !g || !in || !out) return WZ_EINVAL;
+  if (in == out) return WZ_EINVAL;
+  if (!(rho > 0.0 && rho < 2.0)) return WZ_EINVAL;
+  if (nbatch < 0 || nbatch > pl->max_batch) return WZ_EINVAL;
+  return WZ_OK;
+}
+
+wz_status wz_apply_M(wz_plan* pl, int dagger, const void* phi, const double m[2], const double g[2],
+                     double rho, const void* in, void* out, int nbatch) {
+  g_err[0] = 0;
+  wz_status s = check_op(pl, phi, m, g, rho, in, out, nbatch);
+  if (s != WZ_OK) return s;
+  if (nbatch == 0) return WZ_OK;
+  const int dg = dagger ? 1 : 0;
+  if (pl->dtype == WZ_C64)
+    return apply_M_impl<float>(pl, dg, (const cpx<float>*)phi, m, g, rho, (const cpx<float>*)in,
+                               (cpx<float>*)out, nbatch);
+  return apply_M_impl<double>(pl, dg, (const cpx<double>*)phi, m, g, rho, (const cpx<double>*)in,
+                              (cpx<double>*)out, nbatch);
+}
+
+wz_status wz_apply_MdagM(wz_plan* pl, const void* phi, const double m[2], const double g[2],
+                         double rho, const void* in, void* out, int nbatch) {
+  g_err[0] = 0;
+  wz_status s = check_op(pl, phi, m, g, rho, in, out, nbatch);
+  if (s != WZ_OK) return s;
+  if (nbatch == 0) return WZ_OK;
+  if (pl->dtype == WZ_C64)
+    return apply_MdagM_impl<float>(pl, (const cpx<float>*)phi, m, g, rho, (const cpx<float>*)in,
+                                   (cpx<float>*)out, nbatch, false);
+  return apply_MdagM_impl<double>(pl, (const cpx<double>*)phi, m, g, rho, (const cpx<double>*)in,
+                                  (cpx<double>*)out, nbatch, false);
+}
+
+}  // extern "C"
+
+// =============================== CG driver ======================================
+namespace {
+
+constexpr int kCheckEvery = 8;  // iterations enqueued between two looks at the device state
+constexpr double kDelta = 0.1;  // reliable-update threshold (G9)
+
+int vec_grid(long n_real, int per_thread) {
+  long nb = (n_real / per_thread + CGK_NT - 1) / CGK_NT;
+  const long cap = 148L * 8;
+  if (nb > cap) nb = cap;
+  if (nb < 1) nb = 1;
+  return (int)nb;
+}
+
+RedArgs red_of(wz_plan* pl) {
+  RedArgs r;
+  r.partials = pl->partials; r.counter = pl->counter; r.st = pl->d_state; r.store = nullptr;
+  return r;
+}
+
+// One source.  R = iteration precision.  X: caller's complex128 solution buffer.
+template <typename R>
+wz_status cg_one(wz_plan* pl, const cpx<R>* phi, const cpx<R>* b, cpx<double>* X, const double m[2],
+                 const double g[2], double rho, double tol, int max_iter, wz_cg_info* info) {
+  constexpr bool kRU = (sizeof(R) == 4);
+  constexpr int N = vec16<R>::N;
+  const long n = 8 * pl->V;  // real entries of one spinor
+  cudaStream_t st = pl->stream;
+  R* r = (R*)pl->r; R* p = (R*)pl->p; R* q = (R*)pl->q; R* xs = (R*)pl->xs;
+  const int gv = vec_grid(n, N), gv2 = vec_grid(n, 2), gv4 = vec_grid(n, 4);
+  wz_status s;
+
+  CGState h;
+  memset(&h, 0, sizeof(h));
+  h.tol = tol; h.delta = kDelta; h.max_iter = max_iter; h.use_ru = kRU ? 1 : 0;
+  h.true_rr = -1.0;
+  WZ_CUDA(cudaMemcpyAsync(pl->d_state, &h, sizeof(h), cudaMemcpyHostToDevice, st));
+  WZ_CUDA(cudaStreamSynchronize(st));  // h is a stack variable
+  k_cg_init<R><<<gv, CGK_NT, 0, st>>>((const R*)b, r, p, kRU ? xs : nullptr, (double*)X, n, red_of(pl));
+  pl->launches++;
+  WZ_CUDA(cudaGetLastError());
+
+  auto reliable_update = [&](bool final_only) -> wz_status {
+    // X += xs; xs = 0; q128 = A X (complex128); r = b - q128
+    if constexpr (kRU) {
+      k_ru_accum<<<gv4, CGK_NT, 0, st>>>((double*)X, (float*)xs, n);
+      pl->launches++;
+      wz_status s2 = apply_MdagM_impl<double>(pl, pl->phi128, m, g, rho, X, pl->q128, 1, false);
+      if (s2 != WZ_OK) return s2;
+      if (final_only)
+        k_resid<float, float, FIN_TRUE><<<gv2, CGK_NT, 0, st>>>((const float*)b, (const double*)pl->q128,
+                                                                 nullptr, n, red_of(pl));
+      else
+        k_resid<float, float, FIN_RU><<<gv2, CGK_NT, 0, st>>>((const float*)b, (const double*)pl->q128,
+                                                               (float*)r, n, red_of(pl));
+      pl->launches++;
+      WZ_CUDA(cudaGetLastError());
+    }
+    return WZ_OK;
+  };
+
+  int slot_w = 0, slot_r = 0, inflight = 0, ru_served = 0;
+  CGState fin;
+  for (;;) {
+    while (inflight < 2) {
+      for (int it = 0; it < kCheckEvery; ++it) {
+        if ((s = apply_MdagM_impl<R>(pl, phi, m, g, rho, (const cpx<R>*)p, (cpx<R>*)q, 1, true)) != WZ_OK)
+          return s;
+        if constexpr (kRU)
+          k_update_xr<R, R><<<gv, CGK_NT, 0, st>>>(xs, r, p, q, n, red_of(pl));
+        else
+          k_update_xr<R, double><<<gv, CGK_NT, 0, st>>>((double*)X, r, p, q, n, red_of(pl));
+        k_update_p<R><<<gv, CGK_NT, 0, st>>>(p, r, n, pl->d_state);
+        pl->launches += 2;
+      }
+      WZ_CUDA(cudaGetLastError());
+      WZ_CUDA(cudaMemcpyAsync(&pl->h_state[slot_w], pl->d_state, sizeof(CGState), cudaMemcpyDeviceToHost, st));
+      WZ_CUDA(cudaEventRecord(pl->ev[slot_w], st));
+      slot_w ^= 1;
+      ++inflight;
+    }
+    WZ_CUDA(cudaEventSynchronize(pl->ev[slot_r]));
+    fin = pl->h_state[slot_r];
+    slot_r ^= 1;
+    --inflight;
+    if (fin.converged || fin.stop) break;
+    if (fin.need_ru && fin.n_ru == ru_served) {
+      if ((s = reliable_update(false)) != WZ_OK) return s;
+      k_update_p<R><<<gv, CGK_NT, 0, st>>>(p, r, n, pl->d_state);
+      pl->launches++;
+      ++ru_served;
+    }
+  }
+  // true residual at exit
+  if constexpr (kRU) {
+    WZ_CUDA(cudaStreamSynchronize(st));
+    WZ_CUDA(cudaMemcpy(&fin, pl->d_state, sizeof(CGState), cudaMemcpyDeviceToHost));
+    if (!fin.converged && fin.bnorm2 > 0.0) {
+      if ((s = reliable_update(true)) != WZ_OK) return s;
+    }
+  } else {
+    if ((s = apply_MdagM_impl<double>(pl, (const cpx<double>*)phi, m, g, rho, X, (cpx<double>*)q, 1, false)) != WZ_OK)
+      return s;
+    k_resid<double, double, FIN_TRUE><<<gv2, CGK_NT, 0, st>>>((const double*)b, (const double*)q, nullptr, n,
+                                                               red_of(pl));
+    pl->launches++;
+    WZ_CUDA(cudaGetLastError());
+  }
+  WZ_CUDA(cudaStreamSynchronize(st));
+  WZ_CUDA(cudaMemcpy(&fin, pl->d_state, sizeof(CGState), cudaMemcpyDeviceToHost));
+  info->iterations = fin.iter;
+  info->reliable_updates = fin.n_ru;
+  info->converged = fin.converged;
+  info->rel_residual_recursive = fin.bnorm > 0 ? std::sqrt(fin.rr) / fin.bnorm : 0.0;
+  info->rel_residual_true = fin.bnorm > 0 ? std::sqrt(fin.true_rr < 0 ? 0.0 : fin.true_rr) / fin.bnorm : 0.0;
+  return WZ_OK;
+}
+
+}  // namespace
+
+extern "C" wz_status wz_cg_solve(wz_plan* pl, const void* phi, const void* b, void* x,
+                                 const double m[2], const double g[2], double rho, double tol,
+                                 int max_iter, int nbatch, wz_cg_info* info) {
+  g_err[0] = 0;
+  if (!pl || !phi || !b || !x || !m || !g || !info) return WZ_EINVAL;
+  if (!(rho > 0.0 && rho < 2.0) || !(tol > 0.0) || max_iter < 0) return WZ_EINVAL;
+  if (nbatch < 0 || nbatch > pl->max_batch) return WZ_EINVAL;
+  const size_t n1 = (size_t)4 * pl->V;
+  bool all = true;
+  if (pl->dtype == WZ_C64) {
+    const long nphi = 2 * pl->V;
+    k_f2d<<<vec_grid(nphi, 1), CGK_NT, 0, pl->stream>>>((double*)pl->phi128, (const float*)phi, nphi);
+    pl->launches++;
+    WZ_CUDA(cudaGetLastError());
+  }
+  for (int j = 0; j < nbatch; ++j) {
+    wz_status s;
+    if (pl->dtype == WZ_C64)
+      s = cg_one<float>(pl, (const cpx<float>*)phi, (const cpx<float>*)b + j * n1,
+                        (cpx<double>*)x + j * n1, m, g, rho, tol, max_iter, &info[j]);
+    else
+      s = cg_one<double>(pl, (const cpx<double>*)phi, (const cpx<double>*)b + j * n1,
+                         (cpx<double>*)x + j * n1, m, g, rho, tol, max_iter, &info[j]);
+    if (s != WZ_OK) return s;
+    all = all && info[j].converged;
+  }
+  return all ? WZ_OK : WZ_ENOTCONVERGED;
+}

@@ -1,0 +1,218 @@
+// wz_p01.cuh -- the strided two-axis pass: DFTs over axes (x0, x1) of one spin
+// component, for a tile of NSEG consecutive values of the flattened (x2,x3) index.
+//
+// Modes (SURVEY 7.2 passes A, C, E; steps a1, a2, a4, a5, a6 of SURVEY 8(a)):
+//   P01_FWD : [time pre-twist] -> DFT axis 0 -> DFT axis 1                   (pass A)
+//   P01_INV : inverse DFT axis 1 -> inverse DFT axis 0 -> [post-twist] * scale
+//   P01_MID : P01_INV, then  chi = t + W psi  (Yukawa + mass, Eq. 2.19), store chi,
+//             [accumulate ||chi||^2], then P01_FWD on chi                    (pass C)
+//   P01_END : P01_INV, then  out = t + W psi, store out                      (pass E)
+// Each thread (or lane pair) owns one lattice line in registers; the only shared
+// memory traffic is one write + one read per element per axis change.
+#pragma once
+#include "wz_common.cuh"
+
+namespace wz {
+
+enum { P01_FWD = 0, P01_INV = 1, P01_MID = 2, P01_END = 3 };
+
+template <typename R>
+struct P01Args {
+  const cpx<R>* in;   // [nf][L0][L1][I]
+  cpx<R>* out;        // same shape (may alias in)
+  long I;             // L2*L3
+  int apbc;           // antiperiodic time twist on/off
+  R scale;            // 1/V for the inverse modes
+  // MID / END only:
+  const cpx<R>* psi;  // operand of the site-local term (psi for MID, chi for END)
+  const cpx<R>* phi;  // [L0][L1][I]
+  cpx<R>* site_out;   // chi (MID) or the matvec result (END)
+  OpParams<R> op;
+  RedArgs red;        // MID: ||chi||^2 (partials == nullptr: skip)
+  const CGState* gate;  // if set and the solve is idle, the kernel returns at once
+};
+
+template <typename R, int L0, int L1, int NSEG>
+struct P01Cfg {
+  static constexpr int TPL0 = line_tpl<R, L0>::v, TPL1 = line_tpl<R, L1>::v;
+  static constexpr int NR0 = L0 / TPL0, NR1 = L1 / TPL1;
+  static constexpr int NT_A = L1 * NSEG * TPL0;  // threads when lines run along axis 0
+  static constexpr int NT_B = L0 * NSEG * TPL1;  // threads when lines run along axis 1
+  static constexpr int NT_RAW = NT_A > NT_B ? NT_A : NT_B;
+  static constexpr int NT = (NT_RAW + 31) / 32 * 32;
+  static constexpr int PITCH0 = L1 * NSEG + NSEG;  // padded x0 stride (elements)
+  static constexpr size_t SMEM = sizeof(cpx<R>) * (size_t)L0 * PITCH0;
+};
+
+template <typename R, int L0, int L1, int NSEG, int MODE, int FIN>
+__global__ void __launch_bounds__(P01Cfg<R, L0, L1, NSEG>::NT)
+k_p01(const P01Args<R> a) {
+  using Cfg = P01Cfg<R, L0, L1, NSEG>;
+  constexpr int TPL0 = Cfg::TPL0, TPL1 = Cfg::TPL1, NR0 = Cfg::NR0, NR1 = Cfg::NR1;
+  constexpr int PITCH0 = Cfg::PITCH0;
+  constexpr int TWSTEP = TWN / 2 / L0;  // twist exp(-i pi x0/L0) = table[x0 * TWSTEP]
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  cpx<R>* sm = reinterpret_cast<cpx<R>*>(smem_raw);
+  __shared__ double red_sh[33];
+
+  if (a.gate && !cg_active(a.gate)) return;
+
+  const int tid = threadIdx.x;
+  const int f = blockIdx.y;            // field = batch*4 + spin
+  const int comp = f & 3;
+  const long i0 = (long)blockIdx.x * NSEG;
+  const long V = (long)L0 * L1 * a.I;
+  const cpx<R>* gin = a.in + (long)f * V + i0;
+  cpx<R>* gout = a.out + (long)f * V + i0;
+
+  // thread roles: A = line along axis 0 at (x1, s); B = line along axis 1 at (x0, s)
+  const int lineA = tid / TPL0, jA = tid % TPL0;
+  const bool actA = lineA < L1 * NSEG;
+  const int x1A = lineA / NSEG, sA = lineA % NSEG;
+  const int lineB = tid / TPL1, jB = tid % TPL1;
+  const bool actB = lineB < L0 * NSEG;
+  const int x0B = lineB / NSEG, sB = lineB % NSEG;
+
+  if constexpr (MODE == P01_FWD) {
+    using F0 = LineFFT<R, L0, +1, VAR_DIT>;
+    using F1 = LineFFT<R, L1, +1, VAR_DIT>;
+    cpx<R> x[NR0];
+#pragma unroll
+    for (int k = 0; k < NR0; ++k) {
+      const int x0 = F0::in_pos(k, jA);
+      cpx<R> v = {R(0), R(0)};
+      if (actA) v = gin[((long)x0 * L1 + x1A) * a.I + sA];
+      if (a.apbc) v = mul_tw_rt<R, +1>(v, x0 * TWSTEP);
+      x[k] = v;
+    }
+    F0::run(x, jA);
+    if (actA) {
+#pragma unroll
+      for (int k = 0; k < NR0; ++k) {
+        const int n0 = F0::out_pos(k, jA);
+        sm[n0 * PITCH0 + x1A * NSEG + sA] = x[k];
+      }
+    }
+    __syncthreads();
+    cpx<R> y[NR1];
+#pragma unroll
+    for (int k = 0; k < NR1; ++k) {
+      cpx<R> v = {R(0), R(0)};
+      if (actB) v = sm[x0B * PITCH0 + F1::in_pos(k, jB) * NSEG + sB];
+      y[k] = v;
+    }
+    F1::run(y, jB);
+    if (actB) {
+#pragma unroll
+      for (int k = 0; k < NR1; ++k)
+        gout[((long)x0B * L1 + F1::out_pos(k, jB)) * a.I + sB] = y[k];
+    }
+  } else {
+    // ---- inverse half: axis 1 first (from HBM), then axis 0 ----
+    using G1 = LineFFT<R, L1, -1, VAR_DIT>;
+    using G0 = LineFFT<R, L0, -1, VAR_DIT>;
+    {
+      cpx<R> y[NR1];
+#pragma unroll
+      for (int k = 0; k < NR1; ++k) {
+        cpx<R> v = {R(0), R(0)};
+        if (actB) v = gin[((long)x0B * L1 + G1::in_pos(k, jB)) * a.I + sB];
+        y[k] = v;
+      }
+      G1::run(y, jB);
+      if (actB) {
+#pragma unroll
+        for (int k = 0; k < NR1; ++k) sm[x0B * PITCH0 + G1::out_pos(k, jB) * NSEG + sB] = y[k];
+      }
+    }
+    __syncthreads();
+    cpx<R> x[NR0];
+#pragma unroll
+    for (int k = 0; k < NR0; ++k) {
+      cpx<R> v = {R(0), R(0)};
+      if (actA) v = sm[G0::in_pos(k, jA) * PITCH0 + x1A * NSEG + sA];
+      x[k] = v;
+    }
+    G0::run(x, jA);
+    // post-twist exp(+i pi x0/T) and 1/V
+#pragma unroll
+    for (int k = 0; k < NR0; ++k) {
+      const int x0 = G0::out_pos(k, jA);
+      cpx<R> v = x[k];
+      if (a.apbc) v = mul_tw_rt<R, -1>(v, x0 * TWSTEP);
+      x[k] = cscale(v, a.scale);
+    }
+    if constexpr (MODE == P01_INV) {
+      if (actA) {
+#pragma unroll
+        for (int k = 0; k < NR0; ++k)
+          gout[((long)G0::out_pos(k, jA) * L1 + x1A) * a.I + sA] = x[k];
+      }
+    } else {
+      // ---- site-local term of Eq. (2.19): + (m + 2 g phi) P+ psi + (m + 2 g phi)^* P- psi,
+      //      spin 0,1 = P-, spin 2,3 = P+; M^dag swaps w and w^* ----
+      const bool use_conj = (comp < 2) != (a.op.dagger != 0);
+      const cpx<R>* gpsi = a.psi + (long)f * V + i0;
+      const cpx<R>* gphi = a.phi + i0;
+      cpx<R>* gso = a.site_out + (long)f * V + i0;
+      double acc = 0.0;
+      if (actA) {
+#pragma unroll
+        for (int k = 0; k < NR0; ++k) {
+          const long off = ((long)G0::out_pos(k, jA) * L1 + x1A) * a.I + sA;
+          const cpx<R> ph = gphi[off];
+          const cpx<R> ps = gpsi[off];
+          cpx<R> w = {a.op.m_re + a.op.g2_re * ph.re - a.op.g2_im * ph.im,
+                      a.op.m_im + a.op.g2_re * ph.im + a.op.g2_im * ph.re};
+          if (use_conj) w.im = -w.im;
+          cpx<R> v = x[k];
+          v.re += w.re * ps.re - w.im * ps.im;
+          v.im += w.re * ps.im + w.im * ps.re;
+          x[k] = v;
+          gso[off] = v;
+          if (FIN != FIN_STORE || a.red.partials)
+            acc += (double)v.re * (double)v.re + (double)v.im * (double)v.im;
+        }
+      }
+      if constexpr (MODE == P01_MID) {
+        // forward again: pre-twist, DFT axis 0 (halves in -> DIF variant), DFT axis 1
+        using F0 = LineFFT<R, L0, +1, VAR_DIF>;
+        using F1 = LineFFT<R, L1, +1, VAR_DIT>;
+        cpx<R> z[NR0];
+#pragma unroll
+        for (int k = 0; k < NR0; ++k) {
+          const int x0 = G0::out_pos(k, jA);  // = out_index<NR0>(k) + jA*NR0 = F0::in_pos(oi(k), jA)
+          cpx<R> v = x[k];
+          if (a.apbc) v = mul_tw_rt<R, +1>(v, x0 * TWSTEP);
+          z[out_index<NR0>(k)] = v;
+        }
+        F0::run(z, jA);
+        __syncthreads();  // every axis-0 read of the tile is done
+        if (actA) {
+#pragma unroll
+          for (int k = 0; k < NR0; ++k) sm[F0::out_pos(k, jA) * PITCH0 + x1A * NSEG + sA] = z[k];
+        }
+        __syncthreads();
+        cpx<R> y[NR1];
+#pragma unroll
+        for (int k = 0; k < NR1; ++k) {
+          cpx<R> v = {R(0), R(0)};
+          if (actB) v = sm[x0B * PITCH0 + F1::in_pos(k, jB) * NSEG + sB];
+          y[k] = v;
+        }
+        F1::run(y, jB);
+        if (actB) {
+#pragma unroll
+          for (int k = 0; k < NR1; ++k)
+            gout[((long)x0B * L1 + F1::out_pos(k, jB)) * a.I + sB] = y[k];
+        }
+      }
+      if (a.red.partials) {
+        const int blk = blockIdx.y * gridDim.x + blockIdx.x;
+        grid_reduce<FIN>(acc, a.red, blk, gridDim.x * gridDim.y, red_sh);
+      }
+    }
+  }
+}
+
+}  // namespace wz

@@ -1,0 +1,186 @@
+// wz_p23.cuh -- the contiguous two-axis pass: DFTs over axes (x2, x3) of the four
+// spin components of one (n0, n1) plane, with the momentum-diagonal overlap
+// multiply between the forward and the inverse half (SURVEY 7.2 passes B, D;
+// step a3 of SURVEY 8(a)).
+//
+// Momentum-space operator (Eq. 2.19-2.20; 210-225 Eq. 3.1, 3.3;
+// 382-390 Eq. 4.1-4.2; readings G1-G3 of DESIGN.md):
+//   Dslash(p) = i c(p) sum_mu gamma_mu sin p_mu,   c = 2 rho / (s + Mw),
+//   Mw = rho - 2 sum_mu sin^2(p_mu/2),  s = sqrt(Mw^2 + sum_mu sin^2 p_mu),
+// with the gammas of Eq. (2.2), i.e. in 2x2 blocks
+//   Dslash = i c [[0, B], [B^dag, 0]],  B = sin p0 + i sigma_k sin p_k.
+// For Mw < 0 the cancellation-free form c = 2 rho (s - Mw) / sum sin^2 is used.
+#pragma once
+#include "wz_common.cuh"
+
+namespace wz {
+
+enum { P23_FFT = 0, P23_MULT = 1 };
+
+template <typename R>
+struct P23Args {
+  const cpx<R>* in;   // [nb][4][L0*L1][L2][L3]
+  cpx<R>* out;        // may alias in
+  int nplanes;        // L0*L1
+  int L1;             // to split the plane index into (n0, n1)
+  R scale;            // applied at the final store
+  const R* tab;       // momentum tables [2][4][64]: sin p_mu(n), sin^2(p_mu(n)/2)
+  R rho;
+  R sign;             // +1: Dslash, -1: Dslash^dag = -Dslash
+  const CGState* gate;
+};
+
+template <typename R, int L2, int L3>
+struct P23Cfg {
+  static constexpr int TPL2 = line_tpl<R, L2>::v, TPL3 = line_tpl<R, L3>::v;
+  static constexpr int NR2 = L2 / TPL2, NR3 = L3 / TPL3;
+  static constexpr int NTC_A = L3 * TPL2;  // threads per component, lines along axis 2
+  static constexpr int NTC_B = L2 * TPL3;  // lines along axis 3
+  static constexpr int NTC = NTC_A > NTC_B ? NTC_A : NTC_B;
+  static constexpr int NT = (4 * NTC + 31) / 32 * 32;
+  static constexpr int PITCH = L3 + 1;            // row pitch (elements)
+  static constexpr int CPITCH = L2 * PITCH + 4;   // component pitch
+  static constexpr size_t SMEM = sizeof(cpx<R>) * 4 * (size_t)CPITCH;
+};
+
+template <typename R, int L2, int L3, int MODE, int DIR>
+__global__ void __launch_bounds__(P23Cfg<R, L2, L3>::NT)
+k_p23(const P23Args<R> a) {
+  using Cfg = P23Cfg<R, L2, L3>;
+  constexpr int TPL2 = Cfg::TPL2, TPL3 = Cfg::TPL3, NR2 = Cfg::NR2, NR3 = Cfg::NR3;
+  constexpr int NTC = Cfg::NTC, PITCH = Cfg::PITCH, CPITCH = Cfg::CPITCH;
+  constexpr int D1 = (MODE == P23_MULT) ? +1 : DIR;  // direction of the first half
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  cpx<R>* sm = reinterpret_cast<cpx<R>*>(smem_raw);
+  __shared__ R tb[2 * 4 * 64];
+
+  if (a.gate && !cg_active(a.gate)) return;
+
+  const int tid = threadIdx.x;
+  const int plane = blockIdx.x;
+  const long PL = (long)L2 * L3;
+  const long fbase = (long)blockIdx.y * 4 * a.nplanes;  // first field of this batch entry
+
+  if constexpr (MODE == P23_MULT) {
+    for (int i = tid; i < 2 * 4 * 64; i += blockDim.x) tb[i] = a.tab[i];
+  }
+
+  const int c = tid / NTC;      // spin component (>= 4: idle thread)
+  const int tc = tid % NTC;
+  const bool actC = c < 4;
+  // role A: line along axis 2 at x3;  role B: line along axis 3 at n2
+  const int jA = tc % TPL2, x3A = tc / TPL2;
+  const bool actA = actC && (tc < L3 * TPL2);
+  const int jB = tc % TPL3, n2B = tc / TPL3;
+  const bool actB = actC && (tc < L2 * TPL3);
+  const int cc = actC ? c : 0;
+  const cpx<R>* gin = a.in + (fbase + (long)cc * a.nplanes + plane) * PL;
+  cpx<R>* gout = a.out + (fbase + (long)cc * a.nplanes + plane) * PL;
+  cpx<R>* smc = sm + cc * CPITCH;
+
+  // ---- half 1, axis 2 (lanes run along x3: coalesced HBM reads) ----
+  {
+    using F2 = LineFFT<R, L2, D1, VAR_DIT>;
+    cpx<R> x[NR2];
+#pragma unroll
+    for (int k = 0; k < NR2; ++k) {
+      cpx<R> v = {R(0), R(0)};
+      if (actA) v = gin[(long)F2::in_pos(k, jA) * L3 + x3A];
+      x[k] = v;
+    }
+    F2::run(x, jA);
+    if (actA) {
+#pragma unroll
+      for (int k = 0; k < NR2; ++k) smc[F2::out_pos(k, jA) * PITCH + x3A] = x[k];
+    }
+  }
+  __syncthreads();
+  // ---- half 1, axis 3 ----
+  {
+    using F3 = LineFFT<R, L3, D1, VAR_DIT>;
+    cpx<R> y[NR3];
+#pragma unroll
+    for (int k = 0; k < NR3; ++k) {
+      cpx<R> v = {R(0), R(0)};
+      if (actB) v = smc[n2B * PITCH + F3::in_pos(k, jB)];
+      y[k] = v;
+    }
+    F3::run(y, jB);
+    __syncthreads();  // pair partners have read their half of the row
+    if (actB) {
+#pragma unroll
+      for (int k = 0; k < NR3; ++k) smc[n2B * PITCH + F3::out_pos(k, jB)] = y[k];
+    }
+  }
+  __syncthreads();
+
+  if constexpr (MODE == P23_FFT) {
+    // coalesced copy-out of the four planes
+    for (int i = tid; i < 4 * L2 * L3; i += blockDim.x) {
+      const int ci = i / (L2 * L3), r = i % (L2 * L3);
+      const int n2 = r / L3, n3 = r % L3;
+      cpx<R> v = sm[ci * CPITCH + n2 * PITCH + n3];
+      a.out[(fbase + (long)ci * a.nplanes + plane) * PL + r] = cscale(v, a.scale);
+    }
+  } else {
+    // ---- momentum-diagonal multiply, then inverse axis 3 ----
+    using G3 = LineFFT<R, L3, -1, VAR_DIF>;
+    using G2 = LineFFT<R, L2, -1, VAR_DIT>;
+    cpx<R> y[NR3];
+    {
+      const int n0 = plane / a.L1, n1 = plane % a.L1;
+      const R* sn = tb;             // sin p_mu
+      const R* sh = tb + 4 * 64;    // sin^2(p_mu/2)
+      const int n2 = actB ? n2B : 0;
+      const R s0 = sn[0 * 64 + n0], s1 = sn[1 * 64 + n1], s2 = sn[2 * 64 + n2];
+      const R S012 = s0 * s0 + s1 * s1 + s2 * s2;
+      const R Mw012 = a.rho - R(2) * (sh[0 * 64 + n0] + sh[1 * 64 + n1] + sh[2 * 64 + n2]);
+      // out_c = i c(p) sign (Ca psi_ca + Cb psi_cb),  Ca = (A0, A1 + A3 s3), Cb = (B0, B1 + B3 s3)
+      R A0, A1, A3, B0, B1, B3;
+      if (cc == 0)      { A0 = s0;  A1 = R(0); A3 = R(1);  B0 = s2;  B1 = s1;   B3 = R(0); }
+      else if (cc == 1) { A0 = -s2; A1 = s1;   A3 = R(0);  B0 = s0;  B1 = R(0); B3 = R(-1); }
+      else if (cc == 2) { A0 = s0;  A1 = R(0); A3 = R(-1); B0 = -s2; B1 = -s1;  B3 = R(0); }
+      else              { A0 = s2;  A1 = -s1;  A3 = R(0);  B0 = s0;  B1 = R(0); B3 = R(1); }
+      const cpx<R>* sa = sm + ((cc < 2) ? 2 : 0) * CPITCH + n2 * PITCH;
+      const cpx<R>* sb = sa + CPITCH;
+      const R two_rho_sign = R(2) * a.rho * a.sign;
+#pragma unroll
+      for (int k = 0; k < NR3; ++k) {
+        const int n3 = G3::in_pos(k, jB);
+        const R s3 = sn[3 * 64 + n3];
+        const R S2 = S012 + s3 * s3;
+        const R Mw = Mw012 - R(2) * sh[3 * 64 + n3];
+        const R s = sqrt(Mw * Mw + S2);
+        const R cf = (Mw >= R(0)) ? two_rho_sign / (s + Mw) : two_rho_sign * (s - Mw) / S2;
+        const cpx<R> pa = sa[n3], pb = sb[n3];
+        const R Ai = A1 + A3 * s3, Bi = B1 + B3 * s3;
+        const R tr = A0 * pa.re - Ai * pa.im + B0 * pb.re - Bi * pb.im;
+        const R ti = A0 * pa.im + Ai * pa.re + B0 * pb.im + Bi * pb.re;
+        y[k] = {-cf * ti, cf * tr};  // times i
+      }
+    }
+    G3::run(y, jB);
+    __syncthreads();  // all momentum-space reads done
+    if (actB) {
+#pragma unroll
+      for (int k = 0; k < NR3; ++k) smc[n2B * PITCH + G3::out_pos(k, jB)] = y[k];
+    }
+    __syncthreads();
+    // ---- inverse axis 2, coalesced HBM writes ----
+    cpx<R> x[NR2];
+#pragma unroll
+    for (int k = 0; k < NR2; ++k) {
+      cpx<R> v = {R(0), R(0)};
+      if (actA) v = smc[G2::in_pos(k, jA) * PITCH + x3A];
+      x[k] = v;
+    }
+    G2::run(x, jA);
+    if (actA) {
+#pragma unroll
+      for (int k = 0; k < NR2; ++k)
+        gout[(long)G2::out_pos(k, jA) * L3 + x3A] = cscale(x[k], a.scale);
+    }
+  }
+}
+
+}  // namespace wz

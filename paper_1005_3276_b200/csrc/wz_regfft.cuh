@@ -1,0 +1,209 @@
+// wz_regfft.cuh -- 1D DFTs of compile-time length held in registers.
+//
+// Building block of the 4D FFT of PAPER.md:896-898 ("the crucial operation").
+// One lattice line of length L (L = 2^a 3^b, L <= 64) is transformed by ONE thread
+// (L/TPL = NR complex numbers in registers, TPL = 1) or by a PAIR of adjacent lanes
+// (TPL = 2, one radix-2 step across the pair by warp shuffle).  Everything is fully
+// unrolled: register indices, twiddle-table indices and the digit-reversed output
+// order are compile-time constants, so the "bit reversal" costs nothing (the caller
+// stores register k at position out_pos(k, j)).
+//
+// Transform convention (include/wz.h): DIR = +1 uses exp(-2 pi i n x / L)
+// (forward), DIR = -1 uses exp(+2 pi i n x / L) (inverse, unnormalised here).
+#pragma once
+#include <cuda_runtime.h>
+
+namespace wz {
+
+template <typename R>
+struct alignas(2 * sizeof(R)) cpx {
+  R re, im;
+};
+
+// exp(-2 pi i j / TWN), j = 0..TWN-1.  384 = 2^7 * 3 covers every twiddle of the
+// supported line lengths and the antiperiodic twist exp(-i pi x0 / T) (T | 192).
+constexpr int TWN = 384;
+__constant__ float2 c_twf[TWN];
+__constant__ double2 c_twd[TWN];
+
+template <typename R>
+__device__ __forceinline__ cpx<R> tw_load(int idx);
+template <>
+__device__ __forceinline__ cpx<float> tw_load<float>(int idx) {
+  float2 t = c_twf[idx];
+  return {t.x, t.y};
+}
+template <>
+__device__ __forceinline__ cpx<double> tw_load<double>(int idx) {
+  double2 t = c_twd[idx];
+  return {t.x, t.y};
+}
+
+template <typename R>
+__device__ __forceinline__ cpx<R> cadd(cpx<R> a, cpx<R> b) { return {a.re + b.re, a.im + b.im}; }
+template <typename R>
+__device__ __forceinline__ cpx<R> csub(cpx<R> a, cpx<R> b) { return {a.re - b.re, a.im - b.im}; }
+template <typename R>
+__device__ __forceinline__ cpx<R> cmul(cpx<R> a, cpx<R> b) {
+  return {a.re * b.re - a.im * b.im, a.re * b.im + a.im * b.re};
+}
+template <typename R>
+__device__ __forceinline__ cpx<R> cconj(cpx<R> a) { return {a.re, -a.im}; }
+template <typename R>
+__device__ __forceinline__ cpx<R> cscale(cpx<R> a, R s) { return {a.re * s, a.im * s}; }
+// multiply by -i*DIR  (DIR=+1: -i;  DIR=-1: +i)
+template <typename R, int DIR>
+__device__ __forceinline__ cpx<R> mul_mi(cpx<R> a) {
+  if (DIR > 0) return {a.im, -a.re};
+  return {-a.im, a.re};
+}
+
+// a * exp(-DIR 2 pi i num/den).  num, den are compile-time after unrolling, so the
+// branches fold and the table index becomes a constant-bank immediate.
+template <typename R, int DIR>
+__device__ __forceinline__ cpx<R> mul_tw(cpx<R> a, int num, int den) {
+  const int idx = (num % den) * (TWN / den);
+  if (idx == 0) return a;
+  if (idx == TWN / 4) return mul_mi<R, DIR>(a);
+  if (idx == TWN / 2) return {-a.re, -a.im};
+  if (idx == 3 * TWN / 4) return mul_mi<R, -DIR>(a);
+  cpx<R> w = tw_load<R>(idx);
+  if (DIR < 0) w.im = -w.im;
+  return cmul(a, w);
+}
+// same with a run-time index (pair twiddles, twist)
+template <typename R, int DIR>
+__device__ __forceinline__ cpx<R> mul_tw_rt(cpx<R> a, int idx) {
+  cpx<R> w = tw_load<R>(idx);
+  if (DIR < 0) w.im = -w.im;
+  return cmul(a, w);
+}
+
+// ---- small butterflies -------------------------------------------------------
+template <typename R>
+__device__ __forceinline__ void bf2(cpx<R>& a, cpx<R>& b) {
+  cpx<R> t = csub(a, b);
+  a = cadd(a, b);
+  b = t;
+}
+template <typename R, int DIR>
+__device__ __forceinline__ void bf4(cpx<R>& a, cpx<R>& b, cpx<R>& c, cpx<R>& d) {
+  cpx<R> t0 = cadd(a, c), t1 = csub(a, c), t2 = cadd(b, d), t3 = mul_mi<R, DIR>(csub(b, d));
+  a = cadd(t0, t2);
+  c = csub(t0, t2);
+  b = cadd(t1, t3);
+  d = csub(t1, t3);
+}
+template <typename R, int DIR>
+__device__ __forceinline__ void bf3(cpx<R>& a, cpx<R>& b, cpx<R>& c) {
+  const R h = R(0.86602540378443864676372317075294);  // sqrt(3)/2
+  cpx<R> t = cadd(b, c);
+  cpx<R> u = cscale(mul_mi<R, DIR>(csub(b, c)), h);
+  cpx<R> mm = {a.re - R(0.5) * t.re, a.im - R(0.5) * t.im};
+  a = cadd(a, t);
+  b = cadd(mm, u);
+  c = csub(mm, u);
+}
+
+template <int N>
+struct radix_of {
+  static constexpr int v = (N % 4 == 0) ? 4 : ((N % 2 == 0) ? 2 : 3);
+};
+
+// Position p of the in-place decimation-in-frequency result holds output index
+// out_index<N>(p).
+template <int N>
+__host__ __device__ constexpr int out_index(int p) {
+  if constexpr (N == 1) {
+    return 0;
+  } else {
+    constexpr int r = radix_of<N>::v, m = N / r;
+    return p / m + r * out_index<m>(p % m);
+  }
+}
+
+// In-place DIF FFT of x[0..N-1] (registers).
+template <typename R, int N, int DIR>
+struct RegFFT {
+  static __device__ __forceinline__ void run(cpx<R>* x) {
+    if constexpr (N > 1) {
+      constexpr int r = radix_of<N>::v, m = N / r;
+#pragma unroll
+      for (int k = 0; k < m; ++k) {
+        if constexpr (r == 4) {
+          bf4<R, DIR>(x[k], x[k + m], x[k + 2 * m], x[k + 3 * m]);
+          x[k + m] = mul_tw<R, DIR>(x[k + m], k, N);
+          x[k + 2 * m] = mul_tw<R, DIR>(x[k + 2 * m], 2 * k, N);
+          x[k + 3 * m] = mul_tw<R, DIR>(x[k + 3 * m], 3 * k, N);
+        } else if constexpr (r == 2) {
+          bf2<R>(x[k], x[k + m]);
+          x[k + m] = mul_tw<R, DIR>(x[k + m], k, N);
+        } else {
+          bf3<R, DIR>(x[k], x[k + m], x[k + 2 * m]);
+          x[k + m] = mul_tw<R, DIR>(x[k + m], k, N);
+          x[k + 2 * m] = mul_tw<R, DIR>(x[k + 2 * m], 2 * k, N);
+        }
+      }
+#pragma unroll
+      for (int q = 0; q < r; ++q) RegFFT<R, m, DIR>::run(x + q * m);
+    }
+  }
+};
+
+template <typename R>
+__device__ __forceinline__ cpx<R> shfl_xor1(cpx<R> v) {
+  cpx<R> o;
+  o.re = __shfl_xor_sync(0xffffffffu, v.re, 1);
+  o.im = __shfl_xor_sync(0xffffffffu, v.im, 1);
+  return o;
+}
+
+// Threads per line: keep at most 32 complex64 / 16 complex128 values per thread.
+template <typename R, int L>
+struct line_tpl {
+  static constexpr int v = (L * (int)sizeof(R) > 128) ? 2 : 1;
+};
+
+enum { VAR_DIT = 0, VAR_DIF = 1 };
+
+// One lattice line of length L handled by TPL adjacent lanes; lane sub-index j.
+//  VAR_DIT: register k holds input position TPL*k + j, output index oi(k) + j*NR.
+//  VAR_DIF: register k holds input position k + j*NR,  output index TPL*oi(k) + j.
+// (TPL = 1: both are input k, output oi(k).)  All lanes of the warp must call run().
+template <typename R, int L, int DIR, int VAR>
+struct LineFFT {
+  static constexpr int TPL = line_tpl<R, L>::v;
+  static constexpr int NR = L / TPL;
+  static __host__ __device__ constexpr int in_pos(int k, int j) {
+    return (VAR == VAR_DIT) ? (TPL * k + j) : (k + j * NR);
+  }
+  static __host__ __device__ constexpr int out_pos(int k, int j) {
+    return (VAR == VAR_DIT) ? (out_index<NR>(k) + j * NR) : (TPL * out_index<NR>(k) + j);
+  }
+  static __device__ __forceinline__ void run(cpx<R>* x, int j) {
+    if constexpr (TPL == 1) {
+      RegFFT<R, L, DIR>::run(x);
+    } else if constexpr (VAR == VAR_DIT) {
+      RegFFT<R, NR, DIR>::run(x);
+#pragma unroll
+      for (int k = 0; k < NR; ++k) {
+        cpx<R> v = x[k];
+        if (j) v = mul_tw<R, DIR>(v, out_index<NR>(k), L);  // O[n] w_L^n
+        cpx<R> o = shfl_xor1(v);
+        x[k] = j ? csub(o, v) : cadd(v, o);  // E + O' | E - O'
+      }
+    } else {
+#pragma unroll
+      for (int k = 0; k < NR; ++k) {
+        cpx<R> v = x[k];
+        cpx<R> o = shfl_xor1(v);
+        cpx<R> t = j ? csub(o, v) : cadd(v, o);  // lo - hi | lo + hi
+        if (j) t = mul_tw<R, DIR>(t, k, L);
+        x[k] = t;
+      }
+      RegFFT<R, NR, DIR>::run(x);
+    }
+  }
+};
+
+}  // namespace wz

@@ -1,0 +1,223 @@
+"""ctypes binding of libwz.so (include/wz.h).  Argument marshalling only: every
+step of the path runs in the CUDA kernels behind the C ABI.  PyTorch is used for
+device memory and streams.  There is no CPU fallback: a missing library or a
+missing GPU raises.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from dataclasses import dataclass
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libwz.so")
+_lib = None
+
+WZ_C64, WZ_C128 = 0, 1
+WZ_OK, WZ_EINVAL, WZ_EUNSUPPORTED, WZ_ENOMEM, WZ_ECUDA, WZ_ENOTCONVERGED = range(6)
+
+EXPORTS = [
+    "wz_status_string", "wz_last_error", "wz_version", "wz_plan_create", "wz_plan_destroy",
+    "wz_supported", "wz_plan_workspace_bytes", "wz_fft4d", "wz_apply_M", "wz_apply_MdagM",
+    "wz_cg_solve", "wz_plan_launch_count", "wz_plan_reset_launch_count",
+]
+
+
+class WZError(RuntimeError):
+    def __init__(self, status: int, text: str):
+        super().__init__(text)
+        self.status = status
+
+
+class _CGInfo(ctypes.Structure):
+    _fields_ = [("iterations", ctypes.c_int), ("reliable_updates", ctypes.c_int),
+                ("converged", ctypes.c_int), ("rel_residual_recursive", ctypes.c_double),
+                ("rel_residual_true", ctypes.c_double)]
+
+
+@dataclass
+class CGInfo:
+    iterations: int
+    reliable_updates: int
+    converged: bool
+    rel_residual_recursive: float
+    rel_residual_true: float
+
+
+def lib() -> ctypes.CDLL:
+    """Load libwz.so (built by paper_1005_3276_b200.build); fail loudly if absent."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise WZError(-1, "libwz.so not found at %s: run `python -m paper_1005_3276_b200.build` "
+                              "(there is no CPU fallback)" % LIB_PATH)
+        L = ctypes.CDLL(LIB_PATH)
+        vp, ci, cd = ctypes.c_void_p, ctypes.c_int, ctypes.c_double
+        d2 = ctypes.POINTER(ctypes.c_double)
+        L.wz_status_string.restype = ctypes.c_char_p
+        L.wz_status_string.argtypes = [ci]
+        L.wz_last_error.restype = ctypes.c_char_p
+        L.wz_version.restype = ctypes.c_char_p
+        L.wz_plan_create.argtypes = [ctypes.POINTER(vp), ci, ci, ci, ci, ci, ci, vp]
+        L.wz_plan_destroy.argtypes = [vp]
+        L.wz_supported.argtypes = [ci, ci, ci, ci, ci]
+        L.wz_plan_workspace_bytes.restype = ctypes.c_ulonglong
+        L.wz_plan_workspace_bytes.argtypes = [vp]
+        L.wz_plan_launch_count.restype = ctypes.c_ulonglong
+        L.wz_plan_launch_count.argtypes = [vp]
+        L.wz_plan_reset_launch_count.restype = None
+        L.wz_plan_reset_launch_count.argtypes = [vp]
+        L.wz_fft4d.argtypes = [vp, ci, ci, vp, vp, ci]
+        L.wz_apply_M.argtypes = [vp, ci, vp, d2, d2, cd, vp, vp, ci]
+        L.wz_apply_MdagM.argtypes = [vp, vp, d2, d2, cd, vp, vp, ci]
+        L.wz_cg_solve.argtypes = [vp, vp, vp, vp, d2, d2, cd, cd, ci, ci, ctypes.POINTER(_CGInfo)]
+        _lib = L
+    return _lib
+
+
+def _check(status: int):
+    if status != WZ_OK:
+        L = lib()
+        text = L.wz_status_string(status).decode()
+        extra = L.wz_last_error().decode()
+        raise WZError(status, "wz: %s%s" % (text, (" [" + extra + "]") if extra else ""))
+
+
+def _c2(z):
+    z = complex(z)
+    return (ctypes.c_double * 2)(z.real, z.imag)
+
+
+def supported(dims, dtype="c64") -> bool:
+    T, L1, L2, L3 = [int(d) for d in dims]
+    return bool(lib().wz_supported(T, L1, L2, L3, WZ_C64 if dtype == "c64" else WZ_C128))
+
+
+class Plan:
+    """wz_plan for a T x L1 x L2 x L3 lattice; dtype 'c64' or 'c128'."""
+
+    def __init__(self, dims, dtype: str = "c64", max_batch: int = 1, device="cuda:0", stream=None):
+        if not torch.cuda.is_available():
+            raise WZError(-1, "wz needs a CUDA device (no CPU fallback)")
+        self.dims = tuple(int(d) for d in dims)
+        self.dtype = dtype
+        self.tdtype = torch.complex64 if dtype == "c64" else torch.complex128
+        self.device = torch.device(device)
+        self.max_batch = int(max_batch)
+        torch.cuda.set_device(self.device)
+        self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+        h = ctypes.c_void_p()
+        T, L1, L2, L3 = self.dims
+        _check(lib().wz_plan_create(ctypes.byref(h), T, L1, L2, L3,
+                                    WZ_C64 if dtype == "c64" else WZ_C128, self.max_batch,
+                                    ctypes.c_void_p(self.stream.cuda_stream)))
+        self._h = h
+
+    def close(self):
+        if getattr(self, "_h", None):
+            lib().wz_plan_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # -- helpers --
+    def _spinor(self, t: torch.Tensor, dtype=None):
+        dtype = dtype or self.tdtype
+        shape = (4,) + self.dims
+        if t.dtype != dtype or not t.is_cuda or not t.is_contiguous():
+            raise ValueError("expected a contiguous CUDA tensor of dtype %s" % dtype)
+        if tuple(t.shape) == shape:
+            return 1
+        if t.dim() == 6 and tuple(t.shape[1:]) == shape:
+            return int(t.shape[0])
+        raise ValueError("expected shape [nbatch,]4,T,L1,L2,L3 = %s, got %s" % (shape, tuple(t.shape)))
+
+    def _phi(self, phi: torch.Tensor):
+        if phi.dtype != self.tdtype or not phi.is_cuda or not phi.is_contiguous() or \
+                tuple(phi.shape) != self.dims:
+            raise ValueError("phi must be a contiguous CUDA tensor of shape %s, dtype %s" % (self.dims, self.tdtype))
+
+    @property
+    def workspace_bytes(self) -> int:
+        return int(lib().wz_plan_workspace_bytes(self._h))
+
+    @property
+    def launch_count(self) -> int:
+        return int(lib().wz_plan_launch_count(self._h))
+
+    def reset_launch_count(self):
+        lib().wz_plan_reset_launch_count(self._h)
+
+    # -- the calls of include/wz.h --
+    def fft4d(self, inp, direction: int, antiperiodic_time: bool = True, out=None):
+        nb = self._spinor(inp)
+        if out is None:
+            out = torch.empty_like(inp)
+        self._spinor(out)
+        _check(lib().wz_fft4d(self._h, int(direction), int(bool(antiperiodic_time)),
+                              inp.data_ptr(), out.data_ptr(), nb))
+        return out
+
+    def apply_M(self, phi, psi, m, g, rho: float = 1.0, dagger: bool = False, out=None):
+        nb = self._spinor(psi)
+        self._phi(phi)
+        if out is None:
+            out = torch.empty_like(psi)
+        self._spinor(out)
+        _check(lib().wz_apply_M(self._h, int(bool(dagger)), phi.data_ptr(), _c2(m), _c2(g), float(rho),
+                                psi.data_ptr(), out.data_ptr(), nb))
+        return out
+
+    def apply_MdagM(self, phi, psi, m, g, rho: float = 1.0, out=None):
+        nb = self._spinor(psi)
+        self._phi(phi)
+        if out is None:
+            out = torch.empty_like(psi)
+        self._spinor(out)
+        _check(lib().wz_apply_MdagM(self._h, phi.data_ptr(), _c2(m), _c2(g), float(rho),
+                                    psi.data_ptr(), out.data_ptr(), nb))
+        return out
+
+    def cg_solve(self, phi, b, m, g, rho: float = 1.0, tol: float = 1e-6, max_iter: int = 100000,
+                 out=None, raise_on_fail: bool = True):
+        """Solve M^dag M x = b per source.  Returns (x complex128, [CGInfo])."""
+        nb = self._spinor(b)
+        self._phi(phi)
+        if out is None:
+            out = torch.empty(b.shape, dtype=torch.complex128, device=b.device)
+        self._spinor(out, torch.complex128)
+        infos = (_CGInfo * nb)()
+        st = lib().wz_cg_solve(self._h, phi.data_ptr(), b.data_ptr(), out.data_ptr(), _c2(m), _c2(g),
+                               float(rho), float(tol), int(max_iter), nb, infos)
+        if st != WZ_OK and not (st == WZ_ENOTCONVERGED and not raise_on_fail):
+            _check(st)
+        res = [CGInfo(i.iterations, i.reliable_updates, bool(i.converged), i.rel_residual_recursive,
+                      i.rel_residual_true) for i in infos]
+        return out, res
+
+
+# module-level aliases with the C names
+def wz_plan_create(dims, dtype="c64", max_batch=1, device="cuda:0", stream=None) -> Plan:
+    return Plan(dims, dtype, max_batch, device, stream)
+
+
+def wz_fft4d(plan: Plan, direction, antiperiodic_time, inp, out=None):
+    return plan.fft4d(inp, direction, antiperiodic_time, out)
+
+
+def wz_apply_M(plan: Plan, dagger, phi, m, g, rho, inp, out=None):
+    return plan.apply_M(phi, inp, m, g, rho, dagger, out)
+
+
+def wz_apply_MdagM(plan: Plan, phi, m, g, rho, inp, out=None):
+    return plan.apply_MdagM(phi, inp, m, g, rho, out)
+
+
+def wz_cg_solve(plan: Plan, phi, b, m, g, rho, tol, max_iter=100000, out=None):
+    return plan.cg_solve(phi, b, m, g, rho, tol, max_iter, out)

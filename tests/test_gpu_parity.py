@@ -1,0 +1,216 @@
+"""GPU parity: the CUDA path (through the C ABI, include/wz.h) against the CPU oracle,
+element by element on the same seeded inputs (SURVEY 8(d) thresholds):
+  FFT / matvec: relative L2 error <= 1e-12 (complex128), <= 2e-5 (complex64);
+  CG: true residual (recomputed by the ORACLE's M^dag M on the GPU's x) <= tol,
+      iterations within +-2 of the oracle for complex128.
+"""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+TOL = {"c128": 1e-12, "c64": 2e-5}
+NPDT = {"c128": np.complex128, "c64": np.complex64}
+
+# lattices small enough for the oracle: several tiles, ragged/asymmetric extents
+LATTICES = [(4, 4, 4, 4), (8, 8, 8, 8), (8, 4, 16, 8), (16, 16, 16, 16), (48, 24, 24, 24)]
+
+
+def rel(a, ref):
+    return float(np.linalg.norm((a - ref).ravel()) / np.linalg.norm(ref.ravel()))
+
+
+@pytest.fixture(scope="module")
+def wz():
+    if not torch.cuda.is_available():
+        pytest.fail("gpu tests need a CUDA device")
+    from paper_1005_3276_b200 import wz as _wz
+
+    _wz.lib()  # must load: no fallback
+    return _wz
+
+
+@pytest.fixture(scope="module")
+def inp():
+    from paper_1005_3276_b200 import inputs
+
+    return inputs
+
+
+def _fields(inp, dims, dtype, seed=7, sigma=0.4, nsrc=1):
+    phi = inp.make_phi(seed, dims, sigma, NPDT[dtype])
+    b = inp.make_sources(seed, nsrc, dims, NPDT[dtype])
+    return phi, b
+
+
+@pytest.mark.parametrize("dims", LATTICES)
+@pytest.mark.parametrize("dtype", ["c128", "c64"])
+@pytest.mark.parametrize("apbc", [True, False])
+def test_fft4d_vs_oracle(wz, orc, inp, dims, dtype, apbc):
+    if not wz.supported(dims, dtype):
+        pytest.skip("no tile kernel")
+    _, b = _fields(inp, dims, dtype, nsrc=2)
+    plan = wz.Plan(dims, dtype, 2)
+    d_b = torch.from_numpy(b).cuda()
+    f = plan.fft4d(d_b, +1, apbc)
+    ref = np.stack([orc.dft4d(b[j].astype(np.complex128), +1, apbc) for j in range(2)])
+    assert rel(f.cpu().numpy(), ref) <= TOL[dtype]
+    # inverse of the oracle's transform gives back b; also in place
+    d_f = torch.from_numpy(ref.astype(NPDT[dtype])).cuda()
+    plan.fft4d(d_f, -1, apbc, out=d_f)
+    back = np.stack([orc.dft4d(ref[j].astype(NPDT[dtype]).astype(np.complex128), -1, apbc) for j in range(2)])
+    assert rel(d_f.cpu().numpy(), back) <= TOL[dtype]
+    # GPU round trip
+    rt = plan.fft4d(f, -1, apbc)
+    assert rel(rt.cpu().numpy(), b.astype(np.complex128)) <= 2 * TOL[dtype]
+
+
+@pytest.mark.parametrize("dims", LATTICES)
+@pytest.mark.parametrize("dtype", ["c128", "c64"])
+@pytest.mark.parametrize("dagger", [False, True])
+def test_apply_M_vs_oracle(wz, orc, inp, dims, dtype, dagger):
+    if not wz.supported(dims, dtype):
+        pytest.skip("no tile kernel")
+    phi, b = _fields(inp, dims, dtype, nsrc=2)
+    m, g, rho = 0.1 + 0.05j, 0.5 - 0.2j, 1.0  # complex m, g exercise the conjugations of Eq. 2.19
+    plan = wz.Plan(dims, dtype, 2)
+    out = plan.apply_M(torch.from_numpy(phi).cuda(), torch.from_numpy(b).cuda(), m, g, rho, dagger)
+    ref = np.stack([orc.apply_M(phi.astype(np.complex128), b[j].astype(np.complex128), m, g, rho, dagger)
+                    for j in range(2)])
+    assert rel(out.cpu().numpy(), ref) <= TOL[dtype]
+
+
+@pytest.mark.parametrize("dims", LATTICES)
+@pytest.mark.parametrize("dtype", ["c128", "c64"])
+@pytest.mark.parametrize("rho", [1.0, 0.7, 1.4])
+def test_apply_MdagM_vs_oracle(wz, orc, inp, dims, dtype, rho):
+    if not wz.supported(dims, dtype):
+        pytest.skip("no tile kernel")
+    if rho != 1.0 and dims[0] > 8:
+        pytest.skip("rho sweep on the small lattices only")
+    phi, b = _fields(inp, dims, dtype, nsrc=1)
+    m, g = 0.05, 1.0
+    plan = wz.Plan(dims, dtype, 1)
+    out = plan.apply_MdagM(torch.from_numpy(phi).cuda(), torch.from_numpy(b).cuda(), m, g, rho)
+    ref = orc.apply_MdagM(phi.astype(np.complex128), b[0].astype(np.complex128), m, g, rho)[None]
+    assert rel(out.cpu().numpy(), ref) <= TOL[dtype]
+
+
+def _solve_and_check(wz, orc, inp, cfg, nsrc=None, max_iter=50000):
+    dims, dtype = cfg["dims"], cfg["dtype"]
+    nsrc = nsrc or cfg["nsrc"]
+    phi = inp.make_phi(cfg["seed"], dims, cfg["sigma"], NPDT[dtype])
+    b = inp.make_sources(cfg["seed"], nsrc, dims, NPDT[dtype])
+    plan = wz.Plan(dims, dtype, nsrc)
+    x, infos = plan.cg_solve(torch.from_numpy(phi).cuda(), torch.from_numpy(b).cuda(), cfg["m"], cfg["g"],
+                             cfg["rho"], cfg["tol"], max_iter)
+    x = x.cpu().numpy()
+    phi128 = phi.astype(np.complex128)
+    out = []
+    for j in range(nsrc):
+        bj = b[j].astype(np.complex128)
+        true_res = rel(orc.apply_MdagM(phi128, x[j], cfg["m"], cfg["g"], cfg["rho"]), bj)
+        assert infos[j].converged
+        assert true_res <= cfg["tol"], (j, true_res, infos[j])
+        assert abs(infos[j].rel_residual_true - true_res) <= 0.05 * cfg["tol"]
+        out.append((infos[j], true_res, phi128, bj))
+    return out
+
+
+@pytest.mark.parametrize("cfg_id", [1, 2])
+def test_cg_complex128_configs(wz, orc, inp, cfg_id):
+    cfg = inp.CONFIGS[cfg_id]
+    (info, true_res, phi, b), = _solve_and_check(wz, orc, inp, cfg)
+    xo, io = orc.cg(phi, b, cfg["m"], cfg["g"], cfg["rho"], cfg["tol"], 50000)
+    assert io.converged
+    assert abs(info.iterations - io.iterations) <= 2, (info.iterations, io.iterations)
+    assert info.reliable_updates == 0
+
+
+def test_cg_complex64_config3_first_source(wz, orc, inp):
+    """complex64 vectors + reliable updates (G9): bind on the true residual; the
+    iteration count is compared with the oracle's O4' and must not be below the
+    complex128 count by more than rounding noise (G10: report, +-2 is not expected)."""
+    cfg = inp.CONFIGS[3]
+    (info, true_res, phi, b), = _solve_and_check(wz, orc, inp, cfg, nsrc=1)
+    Xo, io = orc.cg_c64ru(phi, b, cfg["m"], cfg["g"], cfg["rho"], cfg["tol"], 50000)
+    print("config 3 source 0: iters gpu=%d oracle(O4')=%d  RU gpu=%d oracle=%d  true residual %.3e"
+          % (info.iterations, io.iterations, info.reliable_updates, io.reliable_updates, true_res))
+    assert io.converged
+    assert info.reliable_updates >= 1
+    assert abs(info.iterations - io.iterations) <= 0.05 * io.iterations
+
+
+def test_cg_batch_of_sources_c64(wz, orc, inp):
+    cfg = dict(inp.CONFIGS[3])
+    cfg.update(dims=(8, 8, 8, 8), nsrc=3, m=0.05)
+    res = _solve_and_check(wz, orc, inp, cfg)
+    its = [r[0].iterations for r in res]
+    assert len(set(its)) >= 1 and min(its) > 10
+
+
+def test_cg_max_iter_and_zero_source(wz, inp):
+    cfg = inp.CONFIGS[2]
+    dims = cfg["dims"]
+    phi = torch.from_numpy(inp.make_phi(2, dims, 0.3)).cuda()
+    b = torch.from_numpy(inp.make_source(2, 0, dims)).cuda()
+    plan = wz.Plan(dims, "c128", 1)
+    with pytest.raises(wz.WZError) as e:
+        plan.cg_solve(phi, b, cfg["m"], cfg["g"], 1.0, 1e-10, 5)
+    assert e.value.status == wz.WZ_ENOTCONVERGED
+    x, infos = plan.cg_solve(phi, b, cfg["m"], cfg["g"], 1.0, 1e-10, 5, raise_on_fail=False)
+    assert infos[0].iterations == 5 and not infos[0].converged and infos[0].rel_residual_true > 1e-10
+    x, infos = plan.cg_solve(phi, torch.zeros_like(b), cfg["m"], cfg["g"], 1.0, 1e-10, 100)
+    assert infos[0].converged and infos[0].iterations == 0 and float(x.abs().max()) == 0.0
+
+
+def test_errors(wz, inp):
+    dims = (4, 4, 4, 4)
+    plan = wz.Plan(dims, "c128", 1)
+    phi = torch.from_numpy(inp.make_phi(1, dims, 0.3)).cuda()
+    b = torch.from_numpy(inp.make_source(1, 0, dims)).cuda()
+    with pytest.raises(wz.WZError) as e:
+        plan.apply_M(phi, b, 0.1, 0.5, 1.0, False, out=b)  # in == out
+    assert e.value.status == wz.WZ_EINVAL
+    with pytest.raises(wz.WZError) as e:
+        plan.apply_MdagM(phi, b, 0.1, 0.5, 2.5)  # rho outside (0, 2)
+    assert e.value.status == wz.WZ_EINVAL
+    with pytest.raises(wz.WZError) as e:
+        plan.fft4d(torch.stack([b, b]), +1, True)  # nbatch > max_batch
+    assert e.value.status == wz.WZ_EINVAL
+    with pytest.raises(wz.WZError) as e:
+        wz.Plan((5, 4, 4, 4), "c128", 1)  # T odd
+    assert e.value.status == wz.WZ_EINVAL
+    with pytest.raises(wz.WZError) as e:
+        wz.Plan((10, 4, 4, 4), "c128", 1)
+    assert e.value.status == wz.WZ_EUNSUPPORTED
+
+
+def test_fft_constant_phi_closed_form(wz, inp):
+    """P5 on the GPU at a size the oracle does not run: constant phi = phi0 gives
+    M^dag M = (d^2(p) + |w|^2) 1 in momentum space, so
+    F[M^dag M psi] = (d^2 + |w|^2) F[psi]; checked with the GPU FFT on 32^4 complex64
+    against d^2 computed here in numpy from Eq. (3.1)/(4.2)."""
+    dims = (32, 32, 32, 32)
+    if not wz.supported(dims, "c64"):
+        pytest.skip("no tile kernel")
+    m, g, rho, phi0 = 0.01, 1.5, 1.0, 0.3 - 0.2j
+    b = inp.make_source(4, 0, dims, np.complex64)
+    plan = wz.Plan(dims, "c64", 1)
+    d_b = torch.from_numpy(b).cuda()
+    d_phi = torch.full(dims, phi0, dtype=torch.complex64, device="cuda")
+    q = plan.apply_MdagM(d_phi, d_b, m, g, rho)
+    fq = plan.fft4d(q, +1, True).cpu().numpy().astype(np.complex128)
+    fb = plan.fft4d(d_b, +1, True).cpu().numpy().astype(np.complex128)
+    p = [2 * np.pi * (np.arange(L) + (0.5 if mu == 0 else 0.0)) / L for mu, L in enumerate(dims)]
+    P = np.meshgrid(*p, indexing="ij")
+    S2 = sum(np.sin(x) ** 2 for x in P)
+    Mw = rho - 2 * sum(np.sin(x / 2) ** 2 for x in P)
+    s = np.sqrt(Mw ** 2 + S2)
+    c = np.where(Mw >= 0, 2 * rho / (s + Mw + (Mw < 0)), 2 * rho * (s - Mw) / S2)
+    d2 = c ** 2 * S2
+    w = m + 2 * g * np.complex128(np.complex64(phi0))
+    ref = (d2 + abs(w) ** 2)[None] * fb
+    assert rel(fq, ref) <= 2e-5
