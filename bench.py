@@ -1,0 +1,380 @@
+#!/usr/bin/env python
+"""bench.py -- BASELINE.json's metric on its config: CG iterations/s (and FFT / matvec
+HBM GB/s) for the 32^4 complex64 lattice, batch of 12 Gaussian sources solved to 1e-6.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl wz|reference]
+
+One "step" = one pass of the whole hot path over one batch: wz_cg_solve of all sources
+of config 4 (every solve runs to the stop rule; nothing is skipped or cached).
+Prints ONE JSON line (rank 0).  Multi-GPU: sources are independent, so
+every rank solves its own batch with phi replicated and no data-path collective
+("weak" scaling); time = max over ranks.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "CG iterations/s at 32^4 (complex64, 12 sources to 1e-6)"
+UNIT = "CG iterations/s"
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=2)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="wz", choices=["wz", "reference"])
+    ap.add_argument("--config", default="4", help="inputs.CONFIGS key (4 = the metric's workload)")
+    ap.add_argument("--sources", type=int, default=0, help="override the number of sources (0 = config's)")
+    ap.add_argument("--max-iter", type=int, default=200000,
+                    help="CG iteration cap; lower it ONLY for profiler runs (the line then says so)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-extras", action="store_true", help="skip the separate FFT / matvec timings")
+    return ap.parse_args()
+
+
+def get_cfg(key):
+    from paper_1005_3276_b200 import inputs
+
+    k = int(key) if key.isdigit() else key
+    return dict(inputs.CONFIGS[k]), k
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index = index
+        self.proc = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q, "--format=csv,noheader,nounits",
+                 "-lms", "200"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            self.proc = None
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            out, _ = self.proc.communicate(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+            out, _ = self.proc.communicate()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in out.splitlines():
+            f = [x.strip() for x in line.split(",")]
+            if len(f) < 6:
+                continue
+            try:
+                sm.append(float(f[0]))
+                mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for n, v in zip(names, f[2:6]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def oracle_sample(cfg, n_iter):
+    """The oracle as it stands (O4', complex64-rounded CG with reliable updates) on
+    source 0 of the workload for n_iter iterations; returns (iterations/s, threads, text)."""
+    import numpy as np
+
+    from oracle import wz_oracle as orc
+    from paper_1005_3276_b200 import inputs
+
+    orc.build()
+    dims = cfg["dims"]
+    phi = inputs.make_phi(cfg["seed"], dims, cfg["sigma"], np.complex64).astype(np.complex128)
+    b = inputs.make_source(cfg["seed"], 0, dims, np.complex64).astype(np.complex128)
+    threads = orc.set_threads(0)
+    fn = orc.cg_c64ru if cfg["dtype"] == "c64" else orc.cg
+    t0 = time.perf_counter()
+    _, info = fn(phi, b, cfg["m"], cfg["g"], cfg["rho"], cfg["tol"], n_iter)
+    dt = time.perf_counter() - t0
+    its = max(info.iterations, 1)
+    text = "source 0 of the workload, first %d CG iterations of the oracle (%s), %.1f s" % (
+        its, "O4' complex64+reliable updates" if cfg["dtype"] == "c64" else "O4 complex128", dt)
+    return its / dt, threads, text, dt
+
+
+def oracle_iters_for(cfg):
+    V = 1
+    for d in cfg["dims"]:
+        V *= d
+    return max(6, min(4000, int(24 * (1 << 20) / V)))
+
+
+def run_reference(args):
+    """--impl reference: the oracle (test infrastructure, never tuned) on the host cores,
+    each step a bounded sample of the same workload.  Rank 0 only."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    cfg, key = get_cfg(args.config)
+    n_iter = oracle_iters_for(cfg)
+    for _ in range(args.warmup):
+        oracle_sample(cfg, max(2, n_iter // 4))
+    tot_it, tot_t, threads, text = 0.0, 0.0, 0, ""
+    for _ in range(args.steps):
+        ips, threads, text, dt = oracle_sample(cfg, n_iter)
+        tot_it += ips * dt
+        tot_t += dt
+    value = tot_it / tot_t
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot_t / max(args.steps, 1),
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "config %s: %s lattice, %s" % (key, "x".join(map(str, cfg["dims"])), cfg["dtype"])},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": text},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+
+
+# algorithmic HBM bytes per launch in units of u (one spinor), nbatch = 1
+ALGO_U = {"p01_fwd": 2.0, "p23_mult": 2.0, "p01_mid": 4.25, "p01_end": 3.25, "p23_fft": 2.0, "p01_inv": 2.0,
+          "update_xr": 6.0, "update_p": 3.0}
+
+
+def load_traffic():
+    p = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            return json.load(f)
+    return {}
+
+
+def run_wz(args):
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+
+    from paper_1005_3276_b200 import inputs, wz
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    dev = torch.device("cuda", local)
+    torch.cuda.set_device(dev)
+    wz.lib()  # fail loudly if the extension is missing
+
+    cfg, key = get_cfg(args.config)
+    dims = cfg["dims"]
+    nsrc = args.sources or cfg["nsrc"]
+    npdt = np.complex64 if cfg["dtype"] == "c64" else np.complex128
+    m, g, rho, tol = cfg["m"], cfg["g"], cfg["rho"], cfg["tol"]
+    # host inputs (pinned); rank r takes sources r*nsrc .. (r+1)*nsrc-1, phi replicated
+    h_phi = torch.from_numpy(inputs.make_phi(cfg["seed"], dims, cfg["sigma"], npdt)).pin_memory()
+    h_b = torch.from_numpy(np.stack([inputs.make_source(cfg["seed"], rank * nsrc + j, dims, npdt)
+                                     for j in range(nsrc)])).pin_memory()
+    d_phi, d_b = h_phi.to(dev), h_b.to(dev)
+    d_x = torch.empty(h_b.shape, dtype=torch.complex128, device=dev)
+    h_x = torch.empty(h_b.shape, dtype=torch.complex128).pin_memory()
+    plan = wz.Plan(dims, cfg["dtype"], nsrc, dev)
+    u = 4 * int(np.prod(dims)) * (8 if cfg["dtype"] == "c64" else 16)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def step():
+        _, infos = plan.cg_solve(d_phi, d_b, m, g, rho, tol, args.max_iter, out=d_x, raise_on_fail=False)
+        return infos
+
+    for _ in range(args.warmup):
+        infos = step()
+    sampler = ClockSampler(local)
+    barrier()
+    sampler.start()
+    plan.reset_launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    iters = 0
+    for _ in range(args.steps):
+        infos = step()
+        iters += sum(i.iterations for i in infos)
+    e1.record()
+    barrier()
+    clocks = sampler.stop()
+    launches = plan.launch_count
+    secs = e0.elapsed_time(e1) * 1e-3
+    conv = all(i.converged for i in infos)
+    worst_true = max(i.rel_residual_true for i in infos)
+    if world > 1:
+        t = torch.tensor([secs], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        secs = float(t.item())
+        c = torch.tensor([iters, launches], device=dev, dtype=torch.float64)
+        dist.all_reduce(c, op=dist.ReduceOp.SUM)
+        iters, launches = int(c[0].item()), int(c[1].item())
+    value = iters / secs
+
+    # ---- end to end through the public API with HOST buffers (pinned), every step ----
+    barrier()
+    t0 = torch.cuda.Event(enable_timing=True)
+    t1 = torch.cuda.Event(enable_timing=True)
+    t0.record()
+    d_phi.copy_(h_phi, non_blocking=True)
+    d_b.copy_(h_b, non_blocking=True)
+    infos_e = step()
+    h_x.copy_(d_x, non_blocking=True)
+    t1.record()
+    barrier()
+    e_secs = t0.elapsed_time(t1) * 1e-3
+    e_iters = sum(i.iterations for i in infos_e)
+    if world > 1:
+        t = torch.tensor([e_secs], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e_secs = float(t.item())
+        c = torch.tensor([e_iters], device=dev, dtype=torch.float64)
+        dist.all_reduce(c, op=dist.ReduceOp.SUM)
+        e_iters = int(c.item())
+    e2e = {"value": e_iters / e_secs, "unit": UNIT,
+           "h2d_bytes_per_step": int(h_phi.numel() * h_phi.element_size() + h_b.numel() * h_b.element_size()),
+           "d2h_bytes_per_step": int(h_x.numel() * h_x.element_size())}
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    # ---- per-kernel durations, live, CUDA events on the plan's stream (one source) ----
+    peak, peak_src = measured_peaks()
+    plan.profile(True)
+    plan.cg_solve(d_phi, d_b[:1], m, g, rho, tol, 1000, out=d_x[:1], raise_on_fail=False)
+    prof = plan.profile_read()
+    plan.profile(False)
+    kinds = {k: {"us": 1e3 * ms / n, "launches": n, "share": 0.0} for k, (ms, n) in prof.items() if k in ALGO_U}
+    tot = sum(v["us"] * v["launches"] for v in kinds.values()) or 1.0
+    for k, v in kinds.items():
+        v["share"] = v["us"] * v["launches"] / tot
+        v["algo_bytes"] = ALGO_U[k] * u
+        v["gbs"] = v["algo_bytes"] / (v["us"] * 1e-6) / 1e9
+        v["frac"] = v["gbs"] / peak
+    dom = max(kinds, key=lambda k: kinds[k]["share"])
+    traffic = load_traffic().get(dom)
+    roofline = {"bound": "hbm", "kernel": dom, "achieved": kinds[dom]["gbs"], "peak": peak, "unit": "GB/s",
+                "frac": kinds[dom]["frac"], "traffic": traffic, "peak_source": peak_src,
+                "algo_bytes_per_launch": kinds[dom]["algo_bytes"], "us_per_launch": kinds[dom]["us"],
+                "share_of_step": kinds[dom]["share"],
+                "all_kernels": {k: {"us": round(v["us"], 2), "GB/s": round(v["gbs"], 1), "frac": round(v["frac"], 3),
+                                    "share": round(v["share"], 3)} for k, v in kinds.items()}}
+
+    extras = {}
+    if not args.no_extras:
+        extras = time_pieces(plan, d_phi, d_b[:1], m, g, rho, u, peak)
+    per_iter_us = 1e6 * secs * world / max(iters, 1)
+    extras.update({"cg_us_per_iteration": per_iter_us, "iterations_per_source": [i.iterations for i in infos],
+                   "reliable_updates_per_source": [i.reliable_updates for i in infos],
+                   "time_to_solution_s_per_source": secs / args.steps / nsrc,
+                   "all_converged": conv, "worst_true_residual": worst_true,
+                   "cg_algorithmic_GBs": 18.5 * u / (per_iter_us * 1e-6) / 1e9})
+
+    cpu = None
+    if not args.no_cpu_baseline and world == 1:
+        ips, threads, text, _ = oracle_sample(cfg, oracle_iters_for(cfg))
+        cpu = {"value": ips, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": text}
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * secs / args.steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f32 (complex64 vectors, f64 reductions, complex128 reliable updates)"
+        if cfg["dtype"] == "c64" else "f64",
+        "data": "synthetic",
+        "config": {"workload": "config %s: %s lattice, %s, %d Gaussian sources per GPU to tol %g, m=%g g=%g rho=%g, seed %d"
+                   % (key, "x".join(map(str, dims)), cfg["dtype"], nsrc, tol, m, g, rho, cfg["seed"]),
+                   "l2": "no flush: working set of one solve (8 vectors, %.0f MB) exceeds the 126 MB L2" % (8.25 * u / 1e6),
+                   "sources": "independent, solved one after another; sharded across ranks, phi replicated"},
+        "max_iter": args.max_iter, "valid": bool(conv),
+        "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
+        "cpu_baseline": cpu, "extras": extras,
+    }
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def time_pieces(plan, d_phi, d_b1, m, g, rho, u, peak):
+    """FFT and matvec timed separately (config 4), warm and with an L2 flush between
+    repetitions (cold), CUDA events on the plan's stream."""
+    import torch
+
+    out = torch.empty_like(d_b1)
+    scratch = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device=d_b1.device)
+
+    def timed(fn, reps=20, cold=False):
+        ts = []
+        for i in range(reps + 3):
+            if cold:
+                scratch.fill_(i & 0xFF)
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            fn()
+            b.record()
+            b.synchronize()
+            if i >= 3:
+                ts.append(a.elapsed_time(b) * 1e-3)
+        return statistics.median(ts), min(ts)
+
+    V4 = d_b1.numel()
+    import math
+    flops_fft = 5.0 * V4 * math.log2(V4 / 4)
+    res = {}
+    for name, fn, nu in [
+        ("fft4d_forward", lambda: plan.fft4d(d_b1, +1, True, out=out), 4.0),
+        ("fft4d_inverse", lambda: plan.fft4d(d_b1, -1, True, out=out), 4.0),
+        ("apply_M", lambda: plan.apply_M(d_phi, d_b1, m, g, rho, False, out=out), 7.25),
+        ("apply_MdagM", lambda: plan.apply_MdagM(d_phi, d_b1, m, g, rho, out=out), 13.5),
+    ]:
+        for cold in (False, True):
+            med, mn = timed(fn, cold=cold)
+            key = name + ("_cold" if cold else "_warm")
+            res[key] = {"us_median": 1e6 * med, "us_min": 1e6 * mn, "algo_GBs": nu * u / med / 1e9,
+                        "frac_of_peak": nu * u / med / 1e9 / peak}
+            if name.startswith("fft4d"):
+                res[key]["gflops_5NlogN"] = flops_fft / med / 1e9
+    res["matvecs_per_s_warm"] = 1.0 / (res["apply_MdagM_warm"]["us_median"] * 1e-6)
+    return res
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_wz(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -110,6 +110,28 @@ wz_status wz_cg_solve(wz_plan *plan, const void *phi, const void *b, void *x,
 unsigned long long wz_plan_launch_count(const wz_plan *plan);
 void wz_plan_reset_launch_count(wz_plan *plan);
 
+/* Optional per-kernel timing for measurement (bench.py's roofline): while enabled,
+ * up to 8192 launches are bracketed by CUDA events on the plan's stream.
+ * wz_plan_profile_read synchronises the stream, adds the recorded durations to the
+ * per-kind totals, and copies them out: ms[k] = summed milliseconds and count[k] =
+ * launches of kind k (arrays of WZ_NKINDS entries, host).  wz_plan_profile(plan, 0)
+ * stops recording; wz_plan_profile(plan, 1) clears the totals and starts. */
+enum {
+  WZ_K_P01_FWD = 0,  /* pass A: twist + DFT axes 0,1 */
+  WZ_K_P23_MULT = 1, /* passes B, D: DFT axes 2,3, overlap multiply, inverse DFT axes 2,3 */
+  WZ_K_P01_MID = 2,  /* pass C: inverse 0,1 + Yukawa + ||chi||^2 + forward 0,1 */
+  WZ_K_P01_END = 3,  /* pass E: inverse 0,1 + Yukawa */
+  WZ_K_P23_FFT = 4,  /* stand-alone DFT axes 2,3 */
+  WZ_K_P01_INV = 5,  /* stand-alone inverse DFT axes 0,1 */
+  WZ_K_UPDATE_XR = 6,
+  WZ_K_UPDATE_P = 7,
+  WZ_K_OTHER = 8,
+  WZ_NKINDS = 9
+};
+wz_status wz_plan_profile(wz_plan *plan, int enable);
+wz_status wz_plan_profile_read(wz_plan *plan, double *ms, unsigned long long *count);
+const char *wz_kind_name(int kind);
+
 #ifdef __cplusplus
 }
 #endif

@@ -154,6 +154,12 @@ struct wz_plan {
   cudaEvent_t ev[2] = {nullptr, nullptr};
   int npartials = 0;
   std::vector<void*> allocs;
+  // optional per-kernel timing (wz_plan_profile): event pairs around sampled launches
+  int profile = 0;
+  std::vector<cudaEvent_t> prof_ev;      // 2 per recorded launch
+  std::vector<int> prof_kind;
+  double prof_ms[WZ_NKINDS] = {0};
+  unsigned long long prof_n[WZ_NKINDS] = {0};
 };
 
 namespace {
@@ -233,10 +239,29 @@ wz_status setup_ws(wz_plan* pl, OpWS<R>& ws, int nbatch_t) {
   return WZ_OK;
 }
 
+constexpr size_t kProfMaxPairs = 8192;
+// Bracket the next launch with events when profiling (bounded number of samples).
+struct ProfScope {
+  wz_plan* pl; int kind; bool on = false;
+  ProfScope(wz_plan* p, int k) : pl(p), kind(k) {
+    if (pl->profile && pl->prof_kind.size() < kProfMaxPairs) {
+      cudaEvent_t a, b;
+      if (cudaEventCreate(&a) == cudaSuccess && cudaEventCreate(&b) == cudaSuccess) {
+        cudaEventRecord(a, pl->stream);
+        pl->prof_ev.push_back(a); pl->prof_ev.push_back(b); pl->prof_kind.push_back(kind);
+        on = true;
+      }
+    }
+  }
+  ~ProfScope() { if (on) cudaEventRecord(pl->prof_ev.back(), pl->stream); pl->launches++; }
+};
+
 template <typename R, typename A>
-wz_status launch(wz_plan* pl, void (*k)(const A), dim3 grid, int nt, size_t smem, const A& args) {
-  k<<<grid, nt, smem, pl->stream>>>(args);
-  pl->launches++;
+wz_status launch(wz_plan* pl, int kind, void (*k)(const A), dim3 grid, int nt, size_t smem, const A& args) {
+  {
+    ProfScope ps(pl, kind);
+    k<<<grid, nt, smem, pl->stream>>>(args);
+  }
   WZ_CUDA(cudaGetLastError());
   return WZ_OK;
 }
@@ -270,16 +295,16 @@ wz_status fft4d_impl(wz_plan* pl, int direction, int apbc, const cpx<R>* in, cpx
   b.rho = R(1); b.sign = R(1);
   if (direction > 0) {
     a.in = in; a.out = out;
-    wz_status s = launch<R>(pl, ws.p01->fwd, g01, ws.p01->nt, ws.p01->smem, a);
+    wz_status s = launch<R>(pl, WZ_K_P01_FWD, ws.p01->fwd, g01, ws.p01->nt, ws.p01->smem, a);
     if (s != WZ_OK) return s;
     b.in = out; b.out = out;
-    return launch<R>(pl, ws.p23->fwd, g23, ws.p23->nt, ws.p23->smem, b);
+    return launch<R>(pl, WZ_K_P23_FFT, ws.p23->fwd, g23, ws.p23->nt, ws.p23->smem, b);
   }
   b.in = in; b.out = out;
-  wz_status s = launch<R>(pl, ws.p23->inv, g23, ws.p23->nt, ws.p23->smem, b);
+  wz_status s = launch<R>(pl, WZ_K_P23_FFT, ws.p23->inv, g23, ws.p23->nt, ws.p23->smem, b);
   if (s != WZ_OK) return s;
   a.in = out; a.out = out; a.scale = (R)(1.0 / (double)pl->V);
-  return launch<R>(pl, ws.p01->inv, g01, ws.p01->nt, ws.p01->smem, a);
+  return launch<R>(pl, WZ_K_P01_INV, ws.p01->inv, g01, ws.p01->nt, ws.p01->smem, a);
 }
 
 // ---- out = M in or M^dag in: passes A, B, E --------------------------
@@ -292,16 +317,16 @@ wz_status apply_M_impl(wz_plan* pl, int dagger, const cpx<R>* phi, const double 
   P01Args<R> a{};
   a.I = pl->I; a.apbc = 1; a.scale = R(1);
   a.in = in; a.out = ws.t;
-  wz_status s = launch<R>(pl, ws.p01->fwd, g01, ws.p01->nt, ws.p01->smem, a);
+  wz_status s = launch<R>(pl, WZ_K_P01_FWD, ws.p01->fwd, g01, ws.p01->nt, ws.p01->smem, a);
   if (s != WZ_OK) return s;
   P23Args<R> b{};
   b.in = ws.t; b.out = ws.t; b.nplanes = pl->L[0] * pl->L[1]; b.L1 = pl->L[1]; b.scale = R(1);
   b.tab = ws.tab; b.rho = (R)rho; b.sign = dagger ? R(-1) : R(1);
-  s = launch<R>(pl, ws.p23->mult, g23, ws.p23->nt, ws.p23->smem, b);
+  s = launch<R>(pl, WZ_K_P23_MULT, ws.p23->mult, g23, ws.p23->nt, ws.p23->smem, b);
   if (s != WZ_OK) return s;
   a.in = ws.t; a.out = ws.t; a.scale = (R)(1.0 / (double)pl->V);
   a.psi = in; a.phi = phi; a.site_out = out; a.op = make_op<R>(m, g, rho, dagger);
-  return launch<R>(pl, ws.p01->end, g01, ws.p01->nt, ws.p01->smem, a);
+  return launch<R>(pl, WZ_K_P01_END, ws.p01->end, g01, ws.p01->nt, ws.p01->smem, a);
 }
 
 // ---- out = M^dag M in: passes A-E.  With `cg` set (nb = 1) the kernels are gated on
@@ -318,26 +343,26 @@ wz_status apply_MdagM_impl(wz_plan* pl, const cpx<R>* phi, const double m[2], co
   P01Args<R> a{};
   a.I = pl->I; a.apbc = 1; a.scale = R(1); a.gate = gate;
   a.in = in; a.out = ws.t;
-  if ((s = launch<R>(pl, ws.p01->fwd, g01, ws.p01->nt, ws.p01->smem, a)) != WZ_OK) return s;  // A
+  if ((s = launch<R>(pl, WZ_K_P01_FWD, ws.p01->fwd, g01, ws.p01->nt, ws.p01->smem, a)) != WZ_OK) return s;  // A
   P23Args<R> b{};
   b.in = ws.t; b.out = ws.t; b.nplanes = pl->L[0] * pl->L[1]; b.L1 = pl->L[1]; b.scale = R(1);
   b.tab = ws.tab; b.rho = (R)rho; b.sign = R(1); b.gate = gate;
-  if ((s = launch<R>(pl, ws.p23->mult, g23, ws.p23->nt, ws.p23->smem, b)) != WZ_OK) return s;  // B
+  if ((s = launch<R>(pl, WZ_K_P23_MULT, ws.p23->mult, g23, ws.p23->nt, ws.p23->smem, b)) != WZ_OK) return s;  // B
   a.in = ws.t; a.out = ws.t; a.scale = invV;
   a.psi = in; a.phi = phi; a.site_out = ws.chi; a.op = make_op<R>(m, g, rho, 0);
   if (cg) {
     a.red.partials = pl->partials; a.red.counter = pl->counter; a.red.st = pl->d_state; a.red.store = nullptr;
     if ((int)(g01.x * g01.y) > pl->npartials) return WZ_EINVAL;
-    s = launch<R>(pl, ws.p01->mid_pq, g01, ws.p01->nt, ws.p01->smem, a);  // C
+    s = launch<R>(pl, WZ_K_P01_MID, ws.p01->mid_pq, g01, ws.p01->nt, ws.p01->smem, a);  // C
   } else {
-    s = launch<R>(pl, ws.p01->mid, g01, ws.p01->nt, ws.p01->smem, a);
+    s = launch<R>(pl, WZ_K_P01_MID, ws.p01->mid, g01, ws.p01->nt, ws.p01->smem, a);
   }
   if (s != WZ_OK) return s;
   b.sign = R(-1);
-  if ((s = launch<R>(pl, ws.p23->mult, g23, ws.p23->nt, ws.p23->smem, b)) != WZ_OK) return s;  // D
+  if ((s = launch<R>(pl, WZ_K_P23_MULT, ws.p23->mult, g23, ws.p23->nt, ws.p23->smem, b)) != WZ_OK) return s;  // D
   a.red = RedArgs{};
   a.psi = ws.chi; a.site_out = out; a.op = make_op<R>(m, g, rho, 1);
-  return launch<R>(pl, ws.p01->end, g01, ws.p01->nt, ws.p01->smem, a);  // E
+  return launch<R>(pl, WZ_K_P01_END, ws.p01->end, g01, ws.p01->nt, ws.p01->smem, a);  // E
 }
 
 }  // namespace
@@ -374,8 +399,25 @@ int wz_supported(int T, int L1, int L2, int L3, wz_dtype dtype) {
   return 1;
 }
 
+static void prof_collect(wz_plan* pl) {
+  cudaStreamSynchronize(pl->stream);
+  for (size_t i = 0; i < pl->prof_kind.size(); ++i) {
+    float ms = 0.f;
+    if (cudaEventElapsedTime(&ms, pl->prof_ev[2 * i], pl->prof_ev[2 * i + 1]) == cudaSuccess) {
+      pl->prof_ms[pl->prof_kind[i]] += ms;
+      pl->prof_n[pl->prof_kind[i]] += 1;
+    }
+    cudaEventDestroy(pl->prof_ev[2 * i]);
+    cudaEventDestroy(pl->prof_ev[2 * i + 1]);
+  }
+  cudaGetLastError();
+  pl->prof_ev.clear();
+  pl->prof_kind.clear();
+}
+
 wz_status wz_plan_destroy(wz_plan* pl) {
   if (!pl) return WZ_EINVAL;
+  prof_collect(pl);
   for (void* p : pl->allocs) cudaFree(p);
   if (pl->h_state) cudaFreeHost(pl->h_state);
   for (int i = 0; i < 2; ++i)
@@ -439,6 +481,29 @@ wz_status wz_plan_create(wz_plan** plan, int T, int L1, int L2, int L3, wz_dtype
     return s;
   }
   *plan = pl;
+  return WZ_OK;
+}
+
+const char* wz_kind_name(int k) {
+  static const char* names[WZ_NKINDS] = {"p01_fwd", "p23_mult", "p01_mid", "p01_end", "p23_fft",
+                                         "p01_inv", "update_xr", "update_p", "other"};
+  return (k >= 0 && k < WZ_NKINDS) ? names[k] : "?";
+}
+
+wz_status wz_plan_profile(wz_plan* pl, int enable) {
+  if (!pl) return WZ_EINVAL;
+  prof_collect(pl);
+  if (enable) {
+    for (int k = 0; k < WZ_NKINDS; ++k) { pl->prof_ms[k] = 0.0; pl->prof_n[k] = 0; }
+  }
+  pl->profile = enable ? 1 : 0;
+  return WZ_OK;
+}
+
+wz_status wz_plan_profile_read(wz_plan* pl, double* ms, unsigned long long* count) {
+  if (!pl || !ms || !count) return WZ_EINVAL;
+  prof_collect(pl);
+  for (int k = 0; k < WZ_NKINDS; ++k) { ms[k] = pl->prof_ms[k]; count[k] = pl->prof_n[k]; }
   return WZ_OK;
 }
 
@@ -564,12 +629,17 @@ wz_status cg_one(wz_plan* pl, const cpx<R>* phi, const cpx<R>* b, cpx<double>* X
       for (int it = 0; it < kCheckEvery; ++it) {
         if ((s = apply_MdagM_impl<R>(pl, phi, m, g, rho, (const cpx<R>*)p, (cpx<R>*)q, 1, true)) != WZ_OK)
           return s;
-        if constexpr (kRU)
-          k_update_xr<R, R><<<gv, CGK_NT, 0, st>>>(xs, r, p, q, n, red_of(pl));
-        else
-          k_update_xr<R, double><<<gv, CGK_NT, 0, st>>>((double*)X, r, p, q, n, red_of(pl));
-        k_update_p<R><<<gv, CGK_NT, 0, st>>>(p, r, n, pl->d_state);
-        pl->launches += 2;
+        {
+          ProfScope ps(pl, WZ_K_UPDATE_XR);
+          if constexpr (kRU)
+            k_update_xr<R, R><<<gv, CGK_NT, 0, st>>>(xs, r, p, q, n, red_of(pl));
+          else
+            k_update_xr<R, double><<<gv, CGK_NT, 0, st>>>((double*)X, r, p, q, n, red_of(pl));
+        }
+        {
+          ProfScope ps(pl, WZ_K_UPDATE_P);
+          k_update_p<R><<<gv, CGK_NT, 0, st>>>(p, r, n, pl->d_state);
+        }
       }
       WZ_CUDA(cudaGetLastError());
       WZ_CUDA(cudaMemcpyAsync(&pl->h_state[slot_w], pl->d_state, sizeof(CGState), cudaMemcpyDeviceToHost, st));

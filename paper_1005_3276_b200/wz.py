@@ -16,12 +16,14 @@ LIB_PATH = os.path.join(_HERE, "libwz.so")
 _lib = None
 
 WZ_C64, WZ_C128 = 0, 1
+WZ_NKINDS = 9
 WZ_OK, WZ_EINVAL, WZ_EUNSUPPORTED, WZ_ENOMEM, WZ_ECUDA, WZ_ENOTCONVERGED = range(6)
 
 EXPORTS = [
     "wz_status_string", "wz_last_error", "wz_version", "wz_plan_create", "wz_plan_destroy",
     "wz_supported", "wz_plan_workspace_bytes", "wz_fft4d", "wz_apply_M", "wz_apply_MdagM",
     "wz_cg_solve", "wz_plan_launch_count", "wz_plan_reset_launch_count",
+    "wz_plan_profile", "wz_plan_profile_read", "wz_kind_name",
 ]
 
 
@@ -73,6 +75,10 @@ def lib() -> ctypes.CDLL:
         L.wz_apply_M.argtypes = [vp, ci, vp, d2, d2, cd, vp, vp, ci]
         L.wz_apply_MdagM.argtypes = [vp, vp, d2, d2, cd, vp, vp, ci]
         L.wz_cg_solve.argtypes = [vp, vp, vp, vp, d2, d2, cd, cd, ci, ci, ctypes.POINTER(_CGInfo)]
+        L.wz_plan_profile.argtypes = [vp, ci]
+        L.wz_plan_profile_read.argtypes = [vp, d2, ctypes.POINTER(ctypes.c_ulonglong)]
+        L.wz_kind_name.restype = ctypes.c_char_p
+        L.wz_kind_name.argtypes = [ci]
         _lib = L
     return _lib
 
@@ -153,6 +159,16 @@ class Plan:
 
     def reset_launch_count(self):
         lib().wz_plan_reset_launch_count(self._h)
+
+    def profile(self, enable: bool):
+        _check(lib().wz_plan_profile(self._h, int(bool(enable))))
+
+    def profile_read(self) -> dict:
+        """{kind: (total_ms, launches)} of the launches recorded since profile(True)."""
+        ms = (ctypes.c_double * WZ_NKINDS)()
+        cnt = (ctypes.c_ulonglong * WZ_NKINDS)()
+        _check(lib().wz_plan_profile_read(self._h, ms, cnt))
+        return {lib().wz_kind_name(k).decode(): (ms[k], int(cnt[k])) for k in range(WZ_NKINDS) if cnt[k]}
 
     # -- the calls of include/wz.h --
     def fft4d(self, inp, direction: int, antiperiodic_time: bool = True, out=None):
