@@ -272,7 +272,7 @@ def run_wz(args):
     # ---- per-kernel durations, live, CUDA events on the plan's stream (one source) ----
     peak, peak_src = measured_peaks()
     plan.profile(True)
-    plan.cg_solve(d_phi, d_b[:1], m, g, rho, tol, 1000, out=d_x[:1], raise_on_fail=False)
+    plan.cg_solve(d_phi, d_b[:1], m, g, rho, tol, min(1000, args.max_iter), out=d_x[:1], raise_on_fail=False)
     prof = plan.profile_read()
     plan.profile(False)
     kinds = {k: {"us": 1e3 * ms / n, "launches": n, "share": 0.0} for k, (ms, n) in prof.items() if k in ALGO_U}
