@@ -38,6 +38,8 @@ struct P01Entry {
   void (*mid)(const P01Args<R>);      // no reduction
   void (*mid_pq)(const P01Args<R>);   // ||chi||^2 -> alpha
   void (*end)(const P01Args<R>);
+  void (*fwdcg)(const P01Args<R>);    // pass A with p <- r + beta p
+  void (*endcg)(const P01Args<R>);    // pass E with x, r updates and ||r||^2
 };
 template <typename R>
 struct P23Entry {
@@ -58,6 +60,8 @@ P01Entry<R> make_p01() {
   e.mid = k_p01<R, L0, L1, NSEG, P01_MID, FIN_STORE>;
   e.mid_pq = k_p01<R, L0, L1, NSEG, P01_MID, FIN_PQ>;
   e.end = k_p01<R, L0, L1, NSEG, P01_END, FIN_STORE>;
+  e.fwdcg = k_p01<R, L0, L1, NSEG, P01_FWDCG, FIN_STORE>;
+  e.endcg = k_p01<R, L0, L1, NSEG, P01_ENDCG, FIN_RR>;
   return e;
 }
 template <typename R, int L2, int L3>
@@ -218,7 +222,8 @@ wz_status setup_ws(wz_plan* pl, OpWS<R>& ws, int nbatch_t) {
   if (pl->I % ws.p01->nseg != 0) return WZ_EUNSUPPORTED;
   const auto* a = ws.p01;
   if (!set_smem(a->fwd, a->smem) || !set_smem(a->inv, a->smem) || !set_smem(a->mid, a->smem) ||
-      !set_smem(a->mid_pq, a->smem) || !set_smem(a->end, a->smem))
+      !set_smem(a->mid_pq, a->smem) || !set_smem(a->end, a->smem) || !set_smem(a->fwdcg, a->smem) ||
+      !set_smem(a->endcg, a->smem))
     return WZ_ECUDA;
   const auto* b = ws.p23;
   if (!set_smem(b->fwd, b->smem) || !set_smem(b->inv, b->smem) || !set_smem(b->mult, b->smem))
@@ -363,6 +368,38 @@ wz_status apply_MdagM_impl(wz_plan* pl, const cpx<R>* phi, const double m[2], co
   a.red = RedArgs{};
   a.psi = ws.chi; a.site_out = out; a.op = make_op<R>(m, g, rho, 1);
   return launch<R>(pl, WZ_K_P01_END, ws.p01->end, g01, ws.p01->nt, ws.p01->smem, a);  // E
+}
+
+// ---- one CG iteration = five kernels: A' (p <- r + beta p, pass A),
+// B, C (chi = M p, alpha = rho/||chi||^2), D, E' (q = M^dag chi in registers,
+// x += alpha p, r -= alpha q, ||r||^2 -> stop rule / beta / reliable-update request).
+// All scalars live in the device CG state; every kernel is gated on it. ------------
+template <typename R>
+wz_status cg_iteration(wz_plan* pl, const cpx<R>* phi, const double m[2], const double g[2], double rho,
+                       cpx<R>* r, cpx<R>* p, cpx<R>* x) {
+  OpWS<R>& ws = ws_of<R>(pl);
+  const dim3 g01((unsigned)(pl->I / ws.p01->nseg), 4u);
+  const dim3 g23((unsigned)(pl->L[0] * pl->L[1]), 1u);
+  if ((int)(g01.x * g01.y) > pl->npartials) return WZ_EINVAL;
+  const R invV = (R)(1.0 / (double)pl->V);
+  wz_status s;
+  P01Args<R> a{};
+  a.I = pl->I; a.apbc = 1; a.scale = R(1); a.gate = pl->d_state;
+  a.in = p; a.out = ws.t; a.cg_r = r; a.cg_p = p;
+  if ((s = launch<R>(pl, WZ_K_P01_FWD, ws.p01->fwdcg, g01, ws.p01->nt, ws.p01->smem, a)) != WZ_OK) return s;
+  P23Args<R> b{};
+  b.in = ws.t; b.out = ws.t; b.nplanes = pl->L[0] * pl->L[1]; b.L1 = pl->L[1]; b.scale = R(1);
+  b.tab = ws.tab; b.rho = (R)rho; b.sign = R(1); b.gate = pl->d_state;
+  if ((s = launch<R>(pl, WZ_K_P23_MULT, ws.p23->mult, g23, ws.p23->nt, ws.p23->smem, b)) != WZ_OK) return s;
+  a.in = ws.t; a.out = ws.t; a.scale = invV;
+  a.psi = p; a.phi = phi; a.site_out = ws.chi; a.op = make_op<R>(m, g, rho, 0);
+  a.red.partials = pl->partials; a.red.counter = pl->counter; a.red.st = pl->d_state; a.red.store = nullptr;
+  if ((s = launch<R>(pl, WZ_K_P01_MID, ws.p01->mid_pq, g01, ws.p01->nt, ws.p01->smem, a)) != WZ_OK) return s;
+  b.sign = R(-1);
+  if ((s = launch<R>(pl, WZ_K_P23_MULT, ws.p23->mult, g23, ws.p23->nt, ws.p23->smem, b)) != WZ_OK) return s;
+  a.psi = ws.chi; a.site_out = nullptr; a.op = make_op<R>(m, g, rho, 1);
+  a.cg_r = r; a.cg_p = p; a.cg_x = x;
+  return launch<R>(pl, WZ_K_P01_END, ws.p01->endcg, g01, ws.p01->nt, ws.p01->smem, a);
 }
 
 }  // namespace
@@ -627,19 +664,11 @@ wz_status cg_one(wz_plan* pl, const cpx<R>* phi, const cpx<R>* b, cpx<double>* X
   for (;;) {
     while (inflight < 2) {
       for (int it = 0; it < kCheckEvery; ++it) {
-        if ((s = apply_MdagM_impl<R>(pl, phi, m, g, rho, (const cpx<R>*)p, (cpx<R>*)q, 1, true)) != WZ_OK)
-          return s;
-        {
-          ProfScope ps(pl, WZ_K_UPDATE_XR);
-          if constexpr (kRU)
-            k_update_xr<R, R><<<gv, CGK_NT, 0, st>>>(xs, r, p, q, n, red_of(pl));
-          else
-            k_update_xr<R, double><<<gv, CGK_NT, 0, st>>>((double*)X, r, p, q, n, red_of(pl));
-        }
-        {
-          ProfScope ps(pl, WZ_K_UPDATE_P);
-          k_update_p<R><<<gv, CGK_NT, 0, st>>>(p, r, n, pl->d_state);
-        }
+        if constexpr (kRU)
+          s = cg_iteration<R>(pl, phi, m, g, rho, (cpx<R>*)r, (cpx<R>*)p, (cpx<R>*)xs);
+        else
+          s = cg_iteration<R>(pl, phi, m, g, rho, (cpx<R>*)r, (cpx<R>*)p, (cpx<R>*)X);
+        if (s != WZ_OK) return s;
       }
       WZ_CUDA(cudaGetLastError());
       WZ_CUDA(cudaMemcpyAsync(&pl->h_state[slot_w], pl->d_state, sizeof(CGState), cudaMemcpyDeviceToHost, st));
@@ -653,9 +682,7 @@ wz_status cg_one(wz_plan* pl, const cpx<R>* phi, const cpx<R>* b, cpx<double>* X
     --inflight;
     if (fin.converged || fin.stop) break;
     if (fin.need_ru && fin.n_ru == ru_served) {
-      if ((s = reliable_update(false)) != WZ_OK) return s;
-      k_update_p<R><<<gv, CGK_NT, 0, st>>>(p, r, n, pl->d_state);
-      pl->launches++;
+      if ((s = reliable_update(false)) != WZ_OK) return s;  // sets beta; the next pass A' applies it
       ++ru_served;
     }
   }

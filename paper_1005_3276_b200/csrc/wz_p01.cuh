@@ -14,7 +14,20 @@
 
 namespace wz {
 
-enum { P01_FWD = 0, P01_INV = 1, P01_MID = 2, P01_END = 3 };
+enum { P01_FWD = 0, P01_INV = 1, P01_MID = 2, P01_END = 3, P01_FWDCG = 4, P01_ENDCG = 5 };
+// CG-fused variants (SURVEY 7.2 "CG fusion"; steps a8-a10 of SURVEY 8(a)):
+//   P01_FWDCG : p <- r + beta p on load (p stored back), then P01_FWD on p
+//   P01_ENDCG : P01_INV, q = t + W chi (never stored);  x += alpha p;  r -= alpha q;
+//               ||r||^2 -> FIN_RR (stop rule, beta, reliable-update request)
+
+__device__ __forceinline__ cpx<float> ldg_c(const cpx<float>* p) {
+  float2 t = __ldg(reinterpret_cast<const float2*>(p));
+  return {t.x, t.y};
+}
+__device__ __forceinline__ cpx<double> ldg_c(const cpx<double>* p) {
+  double2 t = __ldg(reinterpret_cast<const double2*>(p));
+  return {t.x, t.y};
+}
 
 template <typename R>
 struct P01Args {
@@ -28,7 +41,10 @@ struct P01Args {
   const cpx<R>* phi;  // [L0][L1][I]
   cpx<R>* site_out;   // chi (MID) or the matvec result (END)
   OpParams<R> op;
-  RedArgs red;        // MID: ||chi||^2 (partials == nullptr: skip)
+  RedArgs red;        // MID: ||chi||^2 (partials == nullptr: skip);  ENDCG: ||r||^2
+  cpx<R>* cg_r;       // FWDCG (read), ENDCG (read+write)
+  cpx<R>* cg_p;       // FWDCG (read+write), ENDCG (read)
+  cpx<R>* cg_x;       // ENDCG (read+write)
   const CGState* gate;  // if set and the solve is idle, the kernel returns at once
 };
 
@@ -73,17 +89,43 @@ k_p01(const P01Args<R> a) {
   const bool actB = lineB < L0 * NSEG;
   const int x0B = lineB / NSEG, sB = lineB % NSEG;
 
-  if constexpr (MODE == P01_FWD) {
+  if constexpr (MODE == P01_FWD || MODE == P01_FWDCG) {
     using F0 = LineFFT<R, L0, +1, VAR_DIT>;
     using F1 = LineFFT<R, L1, +1, VAR_DIT>;
     cpx<R> x[NR0];
+    if constexpr (MODE == P01_FWDCG) {
+      // p <- r + beta p (PAPER.md:896 CG), all p loads first, r through the
+      // read-only path so that nothing waits behind the p stores
+      const long fo = (long)f * V + i0;
 #pragma unroll
-    for (int k = 0; k < NR0; ++k) {
-      const int x0 = F0::in_pos(k, jA);
-      cpx<R> v = {R(0), R(0)};
-      if (actA) v = gin[((long)x0 * L1 + x1A) * a.I + sA];
-      if (a.apbc) v = mul_tw_rt<R, +1>(v, x0 * TWSTEP);
-      x[k] = v;
+      for (int k = 0; k < NR0; ++k) {
+        cpx<R> v = {R(0), R(0)};
+        if (actA) v = a.cg_p[fo + ((long)F0::in_pos(k, jA) * L1 + x1A) * a.I + sA];
+        x[k] = v;
+      }
+      const R beta = (R)a.gate->beta;
+#pragma unroll
+      for (int k = 0; k < NR0; ++k) {
+        const int x0 = F0::in_pos(k, jA);
+        cpx<R> v = x[k];
+        if (actA) {
+          const long off = fo + ((long)x0 * L1 + x1A) * a.I + sA;
+          const cpx<R> vr = ldg_c(a.cg_r + off);
+          v = {vr.re + beta * v.re, vr.im + beta * v.im};
+          a.cg_p[off] = v;
+        }
+        if (a.apbc) v = mul_tw_rt<R, +1>(v, x0 * TWSTEP);
+        x[k] = v;
+      }
+    } else {
+#pragma unroll
+      for (int k = 0; k < NR0; ++k) {
+        const int x0 = F0::in_pos(k, jA);
+        cpx<R> v = {R(0), R(0)};
+        if (actA) v = gin[((long)x0 * L1 + x1A) * a.I + sA];
+        if (a.apbc) v = mul_tw_rt<R, +1>(v, x0 * TWSTEP);
+        x[k] = v;
+      }
     }
     F0::run(x, jA);
     if (actA) {
@@ -156,22 +198,60 @@ k_p01(const P01Args<R> a) {
       const cpx<R>* gphi = a.phi + i0;
       cpx<R>* gso = a.site_out + (long)f * V + i0;
       double acc = 0.0;
+      constexpr int CH = 4;  // sites whose operands are fetched together (independent loads)
+      static_assert(NR0 % CH == 0, "chunking");
       if (actA) {
 #pragma unroll
-        for (int k = 0; k < NR0; ++k) {
-          const long off = ((long)G0::out_pos(k, jA) * L1 + x1A) * a.I + sA;
-          const cpx<R> ph = gphi[off];
-          const cpx<R> ps = gpsi[off];
-          cpx<R> w = {a.op.m_re + a.op.g2_re * ph.re - a.op.g2_im * ph.im,
-                      a.op.m_im + a.op.g2_re * ph.im + a.op.g2_im * ph.re};
-          if (use_conj) w.im = -w.im;
-          cpx<R> v = x[k];
-          v.re += w.re * ps.re - w.im * ps.im;
-          v.im += w.re * ps.im + w.im * ps.re;
-          x[k] = v;
-          gso[off] = v;
-          if (FIN != FIN_STORE || a.red.partials)
-            acc += (double)v.re * (double)v.re + (double)v.im * (double)v.im;
+        for (int k0 = 0; k0 < NR0; k0 += CH) {
+          long off[CH];
+          cpx<R> ph[CH], ps[CH];
+#pragma unroll
+          for (int c = 0; c < CH; ++c) {
+            off[c] = ((long)G0::out_pos(k0 + c, jA) * L1 + x1A) * a.I + sA;
+            ph[c] = ldg_c(gphi + off[c]);
+            ps[c] = ldg_c(gpsi + off[c]);
+          }
+          if constexpr (MODE == P01_ENDCG) {
+            cpx<R> vr[CH], vp[CH], vx[CH];
+            cpx<R>* gr = a.cg_r + (long)f * V + i0;
+            const cpx<R>* gp = a.cg_p + (long)f * V + i0;
+            cpx<R>* gx = a.cg_x + (long)f * V + i0;
+#pragma unroll
+            for (int c = 0; c < CH; ++c) {
+              vr[c] = gr[off[c]];
+              vp[c] = ldg_c(gp + off[c]);
+              vx[c] = gx[off[c]];
+            }
+            const R alpha = (R)a.red.st->alpha;
+#pragma unroll
+            for (int c = 0; c < CH; ++c) {
+              cpx<R> w = {a.op.m_re + a.op.g2_re * ph[c].re - a.op.g2_im * ph[c].im,
+                          a.op.m_im + a.op.g2_re * ph[c].im + a.op.g2_im * ph[c].re};
+              if (use_conj) w.im = -w.im;
+              cpx<R> q = x[k0 + c];
+              q.re += w.re * ps[c].re - w.im * ps[c].im;
+              q.im += w.re * ps[c].im + w.im * ps[c].re;
+              cpx<R> rn = {vr[c].re - alpha * q.re, vr[c].im - alpha * q.im};
+              cpx<R> xn = {vx[c].re + alpha * vp[c].re, vx[c].im + alpha * vp[c].im};
+              gr[off[c]] = rn;
+              gx[off[c]] = xn;
+              acc += (double)rn.re * (double)rn.re + (double)rn.im * (double)rn.im;
+            }
+          } else {
+#pragma unroll
+            for (int c = 0; c < CH; ++c) {
+              cpx<R> w = {a.op.m_re + a.op.g2_re * ph[c].re - a.op.g2_im * ph[c].im,
+                          a.op.m_im + a.op.g2_re * ph[c].im + a.op.g2_im * ph[c].re};
+              if (use_conj) w.im = -w.im;
+              cpx<R> v = x[k0 + c];
+              v.re += w.re * ps[c].re - w.im * ps[c].im;
+              v.im += w.re * ps[c].im + w.im * ps[c].re;
+              x[k0 + c] = v;
+              gso[off[c]] = v;
+              if (FIN != FIN_STORE || a.red.partials)
+                acc += (double)v.re * (double)v.re + (double)v.im * (double)v.im;
+            }
+          }
         }
       }
       if constexpr (MODE == P01_MID) {
