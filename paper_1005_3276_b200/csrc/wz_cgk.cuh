@@ -94,6 +94,26 @@ k_update_xr(TX* __restrict__ x, R* __restrict__ r, const R* __restrict__ p,
   grid_reduce<FIN_RR>(acc, red, blockIdx.x, gridDim.x, sh);
 }
 
+// x += alpha p with the alpha still pending in the CG state (the fused pass A' applies
+// it one iteration late); not gated.  k_clear_alpha then marks it as applied.
+template <typename R>
+__global__ void __launch_bounds__(CGK_NT)
+k_flush_x(R* __restrict__ x, const R* __restrict__ p, long n, const CGState* st) {
+  constexpr int N = vec16<R>::N;
+  const R alpha = (R)st->alpha;
+  if (alpha == R(0)) return;
+  for (long i = ((long)blockIdx.x * blockDim.x + threadIdx.x) * N; i < n;
+       i += (long)gridDim.x * blockDim.x * N) {
+    R vx[N], vp[N];
+    ld16<R>(x + i, vx);
+    ld16<R>(p + i, vp);
+#pragma unroll
+    for (int e = 0; e < N; ++e) vx[e] = vx[e] + alpha * vp[e];
+    st16<R>(x + i, vx);
+  }
+}
+__global__ void k_clear_alpha(CGState* st) { st->alpha = 0.0; }
+
 // p = r + beta p
 template <typename R>
 __global__ void __launch_bounds__(CGK_NT)

@@ -10,6 +10,7 @@
 #include "../../include/wz.h"
 #include "wz_cgk.cuh"
 #include "wz_p01.cuh"
+#include "wz_p01p.cuh"
 #include "wz_p23.cuh"
 
 using namespace wz;
@@ -29,17 +30,30 @@ bool cuda_ok(cudaError_t e, const char* what) {
   } while (0)
 
 // ---- kernel dispatch tables ---------------------------------------------------
+// One (x0,x1)-pass kernel: the plain version (one tile per CTA) or the persistent
+// pipelined version (wz_p01p.cuh), with its launch shape.
+template <typename R>
+struct P01Kern {
+  void (*fn)(const P01Args<R>) = nullptr;
+  void (*fnp)(const P01Args<R>, int, int) = nullptr;  // persistent: (args, nseg_tiles, ntiles)
+  int nt = 0, nseg = 0;
+  size_t smem = 0;
+};
 template <typename R>
 struct P01Entry {
-  int L0, L1, nseg, nt;
-  size_t smem;
-  void (*fwd)(const P01Args<R>);
-  void (*inv)(const P01Args<R>);
-  void (*mid)(const P01Args<R>);      // no reduction
-  void (*mid_pq)(const P01Args<R>);   // ||chi||^2 -> alpha
-  void (*end)(const P01Args<R>);
-  void (*fwdcg)(const P01Args<R>);    // pass A with p <- r + beta p
-  void (*endcg)(const P01Args<R>);    // pass E with x, r updates and ||r||^2
+  int L0, L1;
+  P01Kern<R> fwd, inv, mid, mid_pq, end, fwdcg, endcg;
+  int max_nseg_tiles(long I) const {  // widest grid any kernel of this entry uses (per field)
+    int m = 1;
+    for (const P01Kern<R>* k : {&fwd, &inv, &mid, &mid_pq, &end, &fwdcg, &endcg})
+      if ((int)(I / k->nseg) > m) m = (int)(I / k->nseg);
+    return m;
+  }
+  bool divides(long I) const {
+    for (const P01Kern<R>* k : {&fwd, &inv, &mid, &mid_pq, &end, &fwdcg, &endcg})
+      if (I % k->nseg) return false;
+    return true;
+  }
 };
 template <typename R>
 struct P23Entry {
@@ -50,45 +64,94 @@ struct P23Entry {
   void (*mult)(const P23Args<R>);
 };
 
-template <typename R, int L0, int L1, int NSEG>
+// ---- tuning: lanes per lattice line (TPL) and tile width (NSEG) -------------------
+// More lanes per line = fewer registers per thread and more resident warps (the
+// passes are latency-bound otherwise: profiles/r01_*); one radix-2 shuffle step per
+// doubling.  Compile-time overrides for sweeps: -DWZ_TPL32F=.. -DWZ_NSEG32F=..
+#ifndef WZ_TPL32F
+#define WZ_TPL32F 2
+#endif
+#ifndef WZ_TPL32F_P23
+#define WZ_TPL32F_P23 2
+#endif
+#ifndef WZ_NSEG32F
+#define WZ_NSEG32F 8
+#endif
+template <typename R, int L> struct tune_tpl {   // axes 0,1
+  static constexpr int v = (sizeof(R) == 4) ? (L >= 48 ? 2 : (L == 32 ? WZ_TPL32F : 1))
+                                            : (L >= 48 ? 4 : (L >= 24 ? 2 : 1));
+};
+template <typename R, int L> struct tune_tpl23 {  // axes 2,3
+  static constexpr int v = (sizeof(R) == 4) ? (L >= 48 ? 2 : (L == 32 ? WZ_TPL32F_P23 : 1))
+                                            : (L >= 48 ? 4 : (L >= 24 ? 2 : 1));
+};
+// NSEG: consecutive (x2,x3) sites per strided tile: tile L0 x L1 x NSEG <= 128 KB,
+// contiguous runs >= 32 bytes.
+template <typename R, int L0, int L1> struct tune_nseg {
+  static constexpr int v = (sizeof(R) == 4) ? (L0 * L1 > 2048 ? 4 : (L0 * L1 == 1024 ? WZ_NSEG32F : 8))
+                                            : (L0 * L1 > 2048 ? 2 : 4);
+};
+
+#ifndef WZ_TPLP32F
+#define WZ_TPLP32F 2
+#endif
+#ifndef WZ_PIPELINE
+#define WZ_PIPELINE 1
+#endif
+// which lattices use the persistent pipelined (x0,x1) pass, and its tile shape
+template <typename R, int L0, int L1> struct tune_pipe {
+  static constexpr bool on = WZ_PIPELINE && sizeof(R) == 4 && L0 == 32 && L1 == 32;
+};
+template <typename R, int L0, int L1> struct tune_pipe_shape {
+  static constexpr int nseg = 4, t0 = WZ_TPLP32F, t1 = WZ_TPLP32F;
+};
+
+template <typename R, int L0, int L1, int MODE, int FIN>
+P01Kern<R> make_p01_kern() {
+  P01Kern<R> k;
+  if constexpr (tune_pipe<R, L0, L1>::on) {
+    using TP = tune_pipe_shape<R, L0, L1>;
+    using C = P01PCfg<R, L0, L1, TP::nseg, TP::t0, TP::t1, MODE>;
+    k.fnp = k_p01p<R, L0, L1, TP::nseg, TP::t0, TP::t1, MODE, FIN>;
+    k.nt = C::NT; k.nseg = TP::nseg; k.smem = C::SMEM;
+  } else {
+    constexpr int NSEG = tune_nseg<R, L0, L1>::v, T0 = tune_tpl<R, L0>::v, T1 = tune_tpl<R, L1>::v;
+    using C = P01Cfg<R, L0, L1, NSEG, T0, T1>;
+    k.fn = k_p01<R, L0, L1, NSEG, T0, T1, MODE, FIN>;
+    k.nt = C::NT; k.nseg = NSEG; k.smem = C::SMEM;
+  }
+  return k;
+}
+template <typename R, int L0, int L1>
 P01Entry<R> make_p01() {
-  using C = P01Cfg<R, L0, L1, NSEG>;
   P01Entry<R> e;
-  e.L0 = L0; e.L1 = L1; e.nseg = NSEG; e.nt = C::NT; e.smem = C::SMEM;
-  e.fwd = k_p01<R, L0, L1, NSEG, P01_FWD, FIN_STORE>;
-  e.inv = k_p01<R, L0, L1, NSEG, P01_INV, FIN_STORE>;
-  e.mid = k_p01<R, L0, L1, NSEG, P01_MID, FIN_STORE>;
-  e.mid_pq = k_p01<R, L0, L1, NSEG, P01_MID, FIN_PQ>;
-  e.end = k_p01<R, L0, L1, NSEG, P01_END, FIN_STORE>;
-  e.fwdcg = k_p01<R, L0, L1, NSEG, P01_FWDCG, FIN_STORE>;
-  e.endcg = k_p01<R, L0, L1, NSEG, P01_ENDCG, FIN_RR>;
+  e.L0 = L0; e.L1 = L1;
+  e.fwd = make_p01_kern<R, L0, L1, P01_FWD, FIN_STORE>();
+  e.inv = make_p01_kern<R, L0, L1, P01_INV, FIN_STORE>();
+  e.mid = make_p01_kern<R, L0, L1, P01_MID, FIN_STORE>();
+  e.mid_pq = make_p01_kern<R, L0, L1, P01_MID, FIN_PQ>();
+  e.end = make_p01_kern<R, L0, L1, P01_END, FIN_STORE>();
+  e.fwdcg = make_p01_kern<R, L0, L1, P01_FWDCG, FIN_STORE>();
+  e.endcg = make_p01_kern<R, L0, L1, P01_ENDCG, FIN_RR>();
   return e;
 }
 template <typename R, int L2, int L3>
 P23Entry<R> make_p23() {
-  using C = P23Cfg<R, L2, L3>;
+  constexpr int T2 = tune_tpl23<R, L2>::v, T3 = tune_tpl23<R, L3>::v;
+  using C = P23Cfg<R, L2, L3, T2, T3>;
   P23Entry<R> e;
   e.L2 = L2; e.L3 = L3; e.nt = C::NT; e.smem = C::SMEM;
-  e.fwd = k_p23<R, L2, L3, P23_FFT, +1>;
-  e.inv = k_p23<R, L2, L3, P23_FFT, -1>;
-  e.mult = k_p23<R, L2, L3, P23_MULT, +1>;
+  e.fwd = k_p23<R, L2, L3, T2, T3, P23_FFT, +1>;
+  e.inv = k_p23<R, L2, L3, T2, T3, P23_FFT, -1>;
+  e.mult = k_p23<R, L2, L3, T2, T3, P23_MULT, +1>;
   return e;
 }
-
-// NSEG: consecutive (x2,x3) sites per strided tile; chosen so that the tile
-// L0 x L1 x NSEG stays <= 128 KB and each contiguous run is >= 32 bytes.
-template <typename R> struct nseg_for {
-  static constexpr int small = (sizeof(R) == 4) ? 8 : 4;
-  static constexpr int big = (sizeof(R) == 4) ? 4 : 2;
-};
 
 template <typename R>
 const std::vector<P01Entry<R>>& p01_table() {
   static const std::vector<P01Entry<R>> t = {
-      make_p01<R, 4, 4, nseg_for<R>::small>(),   make_p01<R, 8, 8, nseg_for<R>::small>(),
-      make_p01<R, 8, 4, nseg_for<R>::small>(),   make_p01<R, 16, 16, nseg_for<R>::small>(),
-      make_p01<R, 32, 32, nseg_for<R>::small>(), make_p01<R, 48, 24, nseg_for<R>::small>(),
-      make_p01<R, 64, 64, nseg_for<R>::big>(),
+      make_p01<R, 4, 4>(),   make_p01<R, 8, 8>(),   make_p01<R, 8, 4>(),   make_p01<R, 16, 16>(),
+      make_p01<R, 32, 32>(), make_p01<R, 48, 24>(), make_p01<R, 64, 64>(),
   };
   return t;
 }
@@ -118,6 +181,12 @@ const P23Entry<R>* find_p23(int L2, int L3) {
   return nullptr;
 }
 
+template <typename K>
+bool set_smem(K kernel, size_t bytes);
+template <typename R>
+bool set_smem_kern(const P01Kern<R>& k) {
+  return k.fn ? set_smem(k.fn, k.smem) : set_smem(k.fnp, k.smem);
+}
 template <typename K>
 bool set_smem(K kernel, size_t bytes) {
   if (bytes <= 48 * 1024) return true;
@@ -157,6 +226,7 @@ struct wz_plan {
   CGState* h_state = nullptr;  // pinned, 2 slots
   cudaEvent_t ev[2] = {nullptr, nullptr};
   int npartials = 0;
+  int num_sms = 148;
   std::vector<void*> allocs;
   // optional per-kernel timing (wz_plan_profile): event pairs around sampled launches
   int profile = 0;
@@ -219,11 +289,11 @@ wz_status setup_ws(wz_plan* pl, OpWS<R>& ws, int nbatch_t) {
   ws.p01 = find_p01<R>(pl->L[0], pl->L[1]);
   ws.p23 = find_p23<R>(pl->L[2], pl->L[3]);
   if (!ws.p01 || !ws.p23) return WZ_EUNSUPPORTED;
-  if (pl->I % ws.p01->nseg != 0) return WZ_EUNSUPPORTED;
+  if (!ws.p01->divides(pl->I)) return WZ_EUNSUPPORTED;
   const auto* a = ws.p01;
-  if (!set_smem(a->fwd, a->smem) || !set_smem(a->inv, a->smem) || !set_smem(a->mid, a->smem) ||
-      !set_smem(a->mid_pq, a->smem) || !set_smem(a->end, a->smem) || !set_smem(a->fwdcg, a->smem) ||
-      !set_smem(a->endcg, a->smem))
+  if (!set_smem_kern(a->fwd) || !set_smem_kern(a->inv) || !set_smem_kern(a->mid) ||
+      !set_smem_kern(a->mid_pq) || !set_smem_kern(a->end) || !set_smem_kern(a->fwdcg) ||
+      !set_smem_kern(a->endcg))
     return WZ_ECUDA;
   const auto* b = ws.p23;
   if (!set_smem(b->fwd, b->smem) || !set_smem(b->inv, b->smem) || !set_smem(b->mult, b->smem))
@@ -271,6 +341,24 @@ wz_status launch(wz_plan* pl, int kind, void (*k)(const A), dim3 grid, int nt, s
   return WZ_OK;
 }
 
+// (x0,x1) pass over nf = 4*nbatch fields
+template <typename R>
+wz_status launch_p01(wz_plan* pl, int kind, const P01Kern<R>& k, const P01Args<R>& args, int nb) {
+  const int nseg_tiles = (int)(pl->I / k.nseg), nf = 4 * nb;
+  {
+    ProfScope ps(pl, kind);
+    if (k.fnp) {
+      const int ntiles = nseg_tiles * nf;
+      const int grid = ntiles < pl->num_sms ? ntiles : pl->num_sms;
+      k.fnp<<<grid, k.nt, k.smem, pl->stream>>>(args, nseg_tiles, ntiles);
+    } else {
+      k.fn<<<dim3((unsigned)nseg_tiles, (unsigned)nf), k.nt, k.smem, pl->stream>>>(args);
+    }
+  }
+  WZ_CUDA(cudaGetLastError());
+  return WZ_OK;
+}
+
 template <typename R>
 OpWS<R>& ws_of(wz_plan* pl);
 template <>
@@ -291,7 +379,6 @@ OpParams<R> make_op(const double m[2], const double g[2], double rho, int dagger
 template <typename R>
 wz_status fft4d_impl(wz_plan* pl, int direction, int apbc, const cpx<R>* in, cpx<R>* out, int nb) {
   OpWS<R>& ws = ws_of<R>(pl);
-  const dim3 g01((unsigned)(pl->I / ws.p01->nseg), (unsigned)(nb * 4));
   const dim3 g23((unsigned)(pl->L[0] * pl->L[1]), (unsigned)nb);
   P01Args<R> a{};
   a.I = pl->I; a.apbc = apbc; a.scale = R(1);
@@ -300,7 +387,7 @@ wz_status fft4d_impl(wz_plan* pl, int direction, int apbc, const cpx<R>* in, cpx
   b.rho = R(1); b.sign = R(1);
   if (direction > 0) {
     a.in = in; a.out = out;
-    wz_status s = launch<R>(pl, WZ_K_P01_FWD, ws.p01->fwd, g01, ws.p01->nt, ws.p01->smem, a);
+    wz_status s = launch_p01<R>(pl, WZ_K_P01_FWD, ws.p01->fwd, a, nb);
     if (s != WZ_OK) return s;
     b.in = out; b.out = out;
     return launch<R>(pl, WZ_K_P23_FFT, ws.p23->fwd, g23, ws.p23->nt, ws.p23->smem, b);
@@ -309,7 +396,7 @@ wz_status fft4d_impl(wz_plan* pl, int direction, int apbc, const cpx<R>* in, cpx
   wz_status s = launch<R>(pl, WZ_K_P23_FFT, ws.p23->inv, g23, ws.p23->nt, ws.p23->smem, b);
   if (s != WZ_OK) return s;
   a.in = out; a.out = out; a.scale = (R)(1.0 / (double)pl->V);
-  return launch<R>(pl, WZ_K_P01_INV, ws.p01->inv, g01, ws.p01->nt, ws.p01->smem, a);
+  return launch_p01<R>(pl, WZ_K_P01_INV, ws.p01->inv, a, nb);
 }
 
 // ---- out = M in or M^dag in: passes A, B, E --------------------------
@@ -317,12 +404,11 @@ template <typename R>
 wz_status apply_M_impl(wz_plan* pl, int dagger, const cpx<R>* phi, const double m[2], const double g[2],
                        double rho, const cpx<R>* in, cpx<R>* out, int nb) {
   OpWS<R>& ws = ws_of<R>(pl);
-  const dim3 g01((unsigned)(pl->I / ws.p01->nseg), (unsigned)(nb * 4));
   const dim3 g23((unsigned)(pl->L[0] * pl->L[1]), (unsigned)nb);
   P01Args<R> a{};
   a.I = pl->I; a.apbc = 1; a.scale = R(1);
   a.in = in; a.out = ws.t;
-  wz_status s = launch<R>(pl, WZ_K_P01_FWD, ws.p01->fwd, g01, ws.p01->nt, ws.p01->smem, a);
+  wz_status s = launch_p01<R>(pl, WZ_K_P01_FWD, ws.p01->fwd, a, nb);
   if (s != WZ_OK) return s;
   P23Args<R> b{};
   b.in = ws.t; b.out = ws.t; b.nplanes = pl->L[0] * pl->L[1]; b.L1 = pl->L[1]; b.scale = R(1);
@@ -331,7 +417,7 @@ wz_status apply_M_impl(wz_plan* pl, int dagger, const cpx<R>* phi, const double 
   if (s != WZ_OK) return s;
   a.in = ws.t; a.out = ws.t; a.scale = (R)(1.0 / (double)pl->V);
   a.psi = in; a.phi = phi; a.site_out = out; a.op = make_op<R>(m, g, rho, dagger);
-  return launch<R>(pl, WZ_K_P01_END, ws.p01->end, g01, ws.p01->nt, ws.p01->smem, a);
+  return launch_p01<R>(pl, WZ_K_P01_END, ws.p01->end, a, nb);
 }
 
 // ---- out = M^dag M in: passes A-E.  With `cg` set (nb = 1) the kernels are gated on
@@ -340,7 +426,6 @@ template <typename R>
 wz_status apply_MdagM_impl(wz_plan* pl, const cpx<R>* phi, const double m[2], const double g[2],
                            double rho, const cpx<R>* in, cpx<R>* out, int nb, bool cg) {
   OpWS<R>& ws = ws_of<R>(pl);
-  const dim3 g01((unsigned)(pl->I / ws.p01->nseg), (unsigned)(nb * 4));
   const dim3 g23((unsigned)(pl->L[0] * pl->L[1]), (unsigned)nb);
   const CGState* gate = cg ? pl->d_state : nullptr;
   const R invV = (R)(1.0 / (double)pl->V);
@@ -348,7 +433,7 @@ wz_status apply_MdagM_impl(wz_plan* pl, const cpx<R>* phi, const double m[2], co
   P01Args<R> a{};
   a.I = pl->I; a.apbc = 1; a.scale = R(1); a.gate = gate;
   a.in = in; a.out = ws.t;
-  if ((s = launch<R>(pl, WZ_K_P01_FWD, ws.p01->fwd, g01, ws.p01->nt, ws.p01->smem, a)) != WZ_OK) return s;  // A
+  if ((s = launch_p01<R>(pl, WZ_K_P01_FWD, ws.p01->fwd, a, nb)) != WZ_OK) return s;  // A
   P23Args<R> b{};
   b.in = ws.t; b.out = ws.t; b.nplanes = pl->L[0] * pl->L[1]; b.L1 = pl->L[1]; b.scale = R(1);
   b.tab = ws.tab; b.rho = (R)rho; b.sign = R(1); b.gate = gate;
@@ -357,36 +442,37 @@ wz_status apply_MdagM_impl(wz_plan* pl, const cpx<R>* phi, const double m[2], co
   a.psi = in; a.phi = phi; a.site_out = ws.chi; a.op = make_op<R>(m, g, rho, 0);
   if (cg) {
     a.red.partials = pl->partials; a.red.counter = pl->counter; a.red.st = pl->d_state; a.red.store = nullptr;
-    if ((int)(g01.x * g01.y) > pl->npartials) return WZ_EINVAL;
-    s = launch<R>(pl, WZ_K_P01_MID, ws.p01->mid_pq, g01, ws.p01->nt, ws.p01->smem, a);  // C
+    if (ws.p01->max_nseg_tiles(pl->I) * 4 * nb > pl->npartials) return WZ_EINVAL;
+    s = launch_p01<R>(pl, WZ_K_P01_MID, ws.p01->mid_pq, a, nb);  // C
   } else {
-    s = launch<R>(pl, WZ_K_P01_MID, ws.p01->mid, g01, ws.p01->nt, ws.p01->smem, a);
+    s = launch_p01<R>(pl, WZ_K_P01_MID, ws.p01->mid, a, nb);
   }
   if (s != WZ_OK) return s;
   b.sign = R(-1);
   if ((s = launch<R>(pl, WZ_K_P23_MULT, ws.p23->mult, g23, ws.p23->nt, ws.p23->smem, b)) != WZ_OK) return s;  // D
   a.red = RedArgs{};
   a.psi = ws.chi; a.site_out = out; a.op = make_op<R>(m, g, rho, 1);
-  return launch<R>(pl, WZ_K_P01_END, ws.p01->end, g01, ws.p01->nt, ws.p01->smem, a);  // E
+  return launch_p01<R>(pl, WZ_K_P01_END, ws.p01->end, a, nb);  // E
 }
 
-// ---- one CG iteration = five kernels: A' (p <- r + beta p, pass A),
-// B, C (chi = M p, alpha = rho/||chi||^2), D, E' (q = M^dag chi in registers,
-// x += alpha p, r -= alpha q, ||r||^2 -> stop rule / beta / reliable-update request).
-// All scalars live in the device CG state; every kernel is gated on it. ------------
+// ---- one CG iteration = five kernels: A' (x += alpha p pending from the
+// previous iteration, p <- r + beta p, pass A), B, C (chi = M p, alpha = rho/||chi||^2),
+// D, E' (q = M^dag chi in registers, r -= alpha q, ||r||^2 -> stop rule / beta /
+// reliable-update request) = 18.5 u of traffic.  All scalars live in the device CG
+// state; every kernel is gated on it.  x lags one update: flush_x() before x is used. --
 template <typename R>
 wz_status cg_iteration(wz_plan* pl, const cpx<R>* phi, const double m[2], const double g[2], double rho,
                        cpx<R>* r, cpx<R>* p, cpx<R>* x) {
   OpWS<R>& ws = ws_of<R>(pl);
-  const dim3 g01((unsigned)(pl->I / ws.p01->nseg), 4u);
+  const int nb = 1;
   const dim3 g23((unsigned)(pl->L[0] * pl->L[1]), 1u);
-  if ((int)(g01.x * g01.y) > pl->npartials) return WZ_EINVAL;
+  if (ws.p01->max_nseg_tiles(pl->I) * 4 > pl->npartials) return WZ_EINVAL;
   const R invV = (R)(1.0 / (double)pl->V);
   wz_status s;
   P01Args<R> a{};
   a.I = pl->I; a.apbc = 1; a.scale = R(1); a.gate = pl->d_state;
-  a.in = p; a.out = ws.t; a.cg_r = r; a.cg_p = p;
-  if ((s = launch<R>(pl, WZ_K_P01_FWD, ws.p01->fwdcg, g01, ws.p01->nt, ws.p01->smem, a)) != WZ_OK) return s;
+  a.in = p; a.out = ws.t; a.cg_r = r; a.cg_p = p; a.cg_x = x;
+  if ((s = launch_p01<R>(pl, WZ_K_P01_FWD, ws.p01->fwdcg, a, nb)) != WZ_OK) return s;
   P23Args<R> b{};
   b.in = ws.t; b.out = ws.t; b.nplanes = pl->L[0] * pl->L[1]; b.L1 = pl->L[1]; b.scale = R(1);
   b.tab = ws.tab; b.rho = (R)rho; b.sign = R(1); b.gate = pl->d_state;
@@ -394,12 +480,12 @@ wz_status cg_iteration(wz_plan* pl, const cpx<R>* phi, const double m[2], const 
   a.in = ws.t; a.out = ws.t; a.scale = invV;
   a.psi = p; a.phi = phi; a.site_out = ws.chi; a.op = make_op<R>(m, g, rho, 0);
   a.red.partials = pl->partials; a.red.counter = pl->counter; a.red.st = pl->d_state; a.red.store = nullptr;
-  if ((s = launch<R>(pl, WZ_K_P01_MID, ws.p01->mid_pq, g01, ws.p01->nt, ws.p01->smem, a)) != WZ_OK) return s;
+  if ((s = launch_p01<R>(pl, WZ_K_P01_MID, ws.p01->mid_pq, a, nb)) != WZ_OK) return s;
   b.sign = R(-1);
   if ((s = launch<R>(pl, WZ_K_P23_MULT, ws.p23->mult, g23, ws.p23->nt, ws.p23->smem, b)) != WZ_OK) return s;
   a.psi = ws.chi; a.site_out = nullptr; a.op = make_op<R>(m, g, rho, 1);
   a.cg_r = r; a.cg_p = p; a.cg_x = x;
-  return launch<R>(pl, WZ_K_P01_END, ws.p01->endcg, g01, ws.p01->nt, ws.p01->smem, a);
+  return launch_p01<R>(pl, WZ_K_P01_END, ws.p01->endcg, a, nb);
 }
 
 }  // namespace
@@ -427,11 +513,11 @@ int wz_supported(int T, int L1, int L2, int L3, wz_dtype dtype) {
   // every plan needs the complex128 operator (reliable updates, true residual)
   const auto* ad = find_p01<double>(T, L1);
   const auto* bd = find_p23<double>(L2, L3);
-  if (!ad || !bd || I % ad->nseg) return 0;
+  if (!ad || !bd || !ad->divides(I)) return 0;
   if (dtype == WZ_C64) {
     const auto* af = find_p01<float>(T, L1);
     const auto* bf = find_p23<float>(L2, L3);
-    if (!af || !bf || I % af->nseg) return 0;
+    if (!af || !bf || !af->divides(I)) return 0;
   }
   return 1;
 }
@@ -480,6 +566,13 @@ wz_status wz_plan_create(wz_plan** plan, int T, int L1, int L2, int L3, wz_dtype
   pl->dtype = dtype;
   pl->max_batch = max_batch;
   pl->stream = (cudaStream_t)stream;
+  {
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) == cudaSuccess &&
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && sms > 0)
+      pl->num_sms = sms;
+    cudaGetLastError();
+  }
   wz_status s = WZ_OK;
   const size_t n1 = (size_t)4 * pl->V;
   do {
@@ -640,6 +733,20 @@ wz_status cg_one(wz_plan* pl, const cpx<R>* phi, const cpx<R>* b, cpx<double>* X
   pl->launches++;
   WZ_CUDA(cudaGetLastError());
 
+  // x += alpha p still pending from the last active iteration (the iteration kernels are idle)
+  auto flush_x = [&]() -> wz_status {
+    {
+      ProfScope ps(pl, WZ_K_OTHER);
+      if constexpr (kRU) k_flush_x<R><<<gv, CGK_NT, 0, st>>>(xs, p, n, pl->d_state);
+      else k_flush_x<R><<<gv, CGK_NT, 0, st>>>((R*)X, p, n, pl->d_state);
+    }
+    {
+      ProfScope ps(pl, WZ_K_OTHER);
+      k_clear_alpha<<<1, 1, 0, st>>>(pl->d_state);
+    }
+    WZ_CUDA(cudaGetLastError());
+    return WZ_OK;
+  };
   auto reliable_update = [&](bool final_only) -> wz_status {
     // X += xs; xs = 0; q128 = A X (complex128); r = b - q128
     if constexpr (kRU) {
@@ -682,10 +789,12 @@ wz_status cg_one(wz_plan* pl, const cpx<R>* phi, const cpx<R>* b, cpx<double>* X
     --inflight;
     if (fin.converged || fin.stop) break;
     if (fin.need_ru && fin.n_ru == ru_served) {
+      if ((s = flush_x()) != WZ_OK) return s;
       if ((s = reliable_update(false)) != WZ_OK) return s;  // sets beta; the next pass A' applies it
       ++ru_served;
     }
   }
+  if ((s = flush_x()) != WZ_OK) return s;
   // true residual at exit
   if constexpr (kRU) {
     WZ_CUDA(cudaStreamSynchronize(st));

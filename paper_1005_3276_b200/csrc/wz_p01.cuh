@@ -16,9 +16,11 @@ namespace wz {
 
 enum { P01_FWD = 0, P01_INV = 1, P01_MID = 2, P01_END = 3, P01_FWDCG = 4, P01_ENDCG = 5 };
 // CG-fused variants (SURVEY 7.2 "CG fusion"; steps a8-a10 of SURVEY 8(a)):
-//   P01_FWDCG : p <- r + beta p on load (p stored back), then P01_FWD on p
-//   P01_ENDCG : P01_INV, q = t + W chi (never stored);  x += alpha p;  r -= alpha q;
+//   P01_FWDCG : on load  x += alpha p (the update left pending by the previous iteration),
+//               p <- r + beta p (both stored back), then P01_FWD on p
+//   P01_ENDCG : P01_INV, q = t + W chi (never stored);  r -= alpha q;
 //               ||r||^2 -> FIN_RR (stop rule, beta, reliable-update request)
+// x lags by one update: wz_lib.cu flushes it (k_flush_x) before x is used.
 
 __device__ __forceinline__ cpx<float> ldg_c(const cpx<float>* p) {
   float2 t = __ldg(reinterpret_cast<const float2*>(p));
@@ -44,13 +46,13 @@ struct P01Args {
   RedArgs red;        // MID: ||chi||^2 (partials == nullptr: skip);  ENDCG: ||r||^2
   cpx<R>* cg_r;       // FWDCG (read), ENDCG (read+write)
   cpx<R>* cg_p;       // FWDCG (read+write), ENDCG (read)
-  cpx<R>* cg_x;       // ENDCG (read+write)
+  cpx<R>* cg_x;       // FWDCG (read+write)
   const CGState* gate;  // if set and the solve is idle, the kernel returns at once
 };
 
-template <typename R, int L0, int L1, int NSEG>
+template <typename R, int L0, int L1, int NSEG, int T0, int T1>
 struct P01Cfg {
-  static constexpr int TPL0 = line_tpl<R, L0>::v, TPL1 = line_tpl<R, L1>::v;
+  static constexpr int TPL0 = T0, TPL1 = T1;  // lanes per line along axis 0 / axis 1
   static constexpr int NR0 = L0 / TPL0, NR1 = L1 / TPL1;
   static constexpr int NT_A = L1 * NSEG * TPL0;  // threads when lines run along axis 0
   static constexpr int NT_B = L0 * NSEG * TPL1;  // threads when lines run along axis 1
@@ -60,10 +62,10 @@ struct P01Cfg {
   static constexpr size_t SMEM = sizeof(cpx<R>) * (size_t)L0 * PITCH0;
 };
 
-template <typename R, int L0, int L1, int NSEG, int MODE, int FIN>
-__global__ void __launch_bounds__(P01Cfg<R, L0, L1, NSEG>::NT)
+template <typename R, int L0, int L1, int NSEG, int T0, int T1, int MODE, int FIN>
+__global__ void __launch_bounds__(P01Cfg<R, L0, L1, NSEG, T0, T1>::NT)
 k_p01(const P01Args<R> a) {
-  using Cfg = P01Cfg<R, L0, L1, NSEG>;
+  using Cfg = P01Cfg<R, L0, L1, NSEG, T0, T1>;
   constexpr int TPL0 = Cfg::TPL0, TPL1 = Cfg::TPL1, NR0 = Cfg::NR0, NR1 = Cfg::NR1;
   constexpr int PITCH0 = Cfg::PITCH0;
   constexpr int TWSTEP = TWN / 2 / L0;  // twist exp(-i pi x0/L0) = table[x0 * TWSTEP]
@@ -82,16 +84,17 @@ k_p01(const P01Args<R> a) {
   cpx<R>* gout = a.out + (long)f * V + i0;
 
   // thread roles: A = line along axis 0 at (x1, s); B = line along axis 1 at (x0, s)
-  const int lineA = tid / TPL0, jA = tid % TPL0;
+  int lineA, jA, lineB, jB;
+  lane_split<TPL0>(tid, lineA, jA);
+  lane_split<TPL1>(tid, lineB, jB);
   const bool actA = lineA < L1 * NSEG;
   const int x1A = lineA / NSEG, sA = lineA % NSEG;
-  const int lineB = tid / TPL1, jB = tid % TPL1;
   const bool actB = lineB < L0 * NSEG;
   const int x0B = lineB / NSEG, sB = lineB % NSEG;
 
   if constexpr (MODE == P01_FWD || MODE == P01_FWDCG) {
-    using F0 = LineFFT<R, L0, +1, VAR_DIT>;
-    using F1 = LineFFT<R, L1, +1, VAR_DIT>;
+    using F0 = LineFFT<R, L0, +1, VAR_DIT, TPL0>;
+    using F1 = LineFFT<R, L1, +1, VAR_DIT, TPL1>;
     cpx<R> x[NR0];
     if constexpr (MODE == P01_FWDCG) {
       // p <- r + beta p (PAPER.md:896 CG), all p loads first, r through the
@@ -103,7 +106,7 @@ k_p01(const P01Args<R> a) {
         if (actA) v = a.cg_p[fo + ((long)F0::in_pos(k, jA) * L1 + x1A) * a.I + sA];
         x[k] = v;
       }
-      const R beta = (R)a.gate->beta;
+      const R beta = (R)a.gate->beta, alpha = (R)a.gate->alpha;
 #pragma unroll
       for (int k = 0; k < NR0; ++k) {
         const int x0 = F0::in_pos(k, jA);
@@ -111,6 +114,8 @@ k_p01(const P01Args<R> a) {
         if (actA) {
           const long off = fo + ((long)x0 * L1 + x1A) * a.I + sA;
           const cpx<R> vr = ldg_c(a.cg_r + off);
+          const cpx<R> vx = a.cg_x[off];  // each x element is read, then written, by this thread only
+          a.cg_x[off] = {vx.re + alpha * v.re, vx.im + alpha * v.im};  // pending x += alpha_{k-1} p_{k-1}
           v = {vr.re + beta * v.re, vr.im + beta * v.im};
           a.cg_p[off] = v;
         }
@@ -151,8 +156,8 @@ k_p01(const P01Args<R> a) {
     }
   } else {
     // ---- inverse half: axis 1 first (from HBM), then axis 0 ----
-    using G1 = LineFFT<R, L1, -1, VAR_DIT>;
-    using G0 = LineFFT<R, L0, -1, VAR_DIT>;
+    using G1 = LineFFT<R, L1, -1, VAR_DIT, TPL1>;
+    using G0 = LineFFT<R, L0, -1, VAR_DIT, TPL0>;
     {
       cpx<R> y[NR1];
 #pragma unroll
@@ -198,7 +203,7 @@ k_p01(const P01Args<R> a) {
       const cpx<R>* gphi = a.phi + i0;
       cpx<R>* gso = a.site_out + (long)f * V + i0;
       double acc = 0.0;
-      constexpr int CH = 4;  // sites whose operands are fetched together (independent loads)
+      constexpr int CH = (NR0 % 8 == 0) ? 8 : 4;  // sites whose operands are fetched together
       static_assert(NR0 % CH == 0, "chunking");
       if (actA) {
 #pragma unroll
@@ -208,20 +213,22 @@ k_p01(const P01Args<R> a) {
 #pragma unroll
           for (int c = 0; c < CH; ++c) {
             off[c] = ((long)G0::out_pos(k0 + c, jA) * L1 + x1A) * a.I + sA;
+#if defined(WZ_DBG_SITE) && (WZ_DBG_SITE & 1)
+            ph[c] = {R(0.25), R(0.5)};
+#else
             ph[c] = ldg_c(gphi + off[c]);
+#endif
+#if defined(WZ_DBG_SITE) && (WZ_DBG_SITE & 2)
+            ps[c] = {R(0.25), R(0.5)};
+#else
             ps[c] = ldg_c(gpsi + off[c]);
+#endif
           }
           if constexpr (MODE == P01_ENDCG) {
-            cpx<R> vr[CH], vp[CH], vx[CH];
+            cpx<R> vr[CH];
             cpx<R>* gr = a.cg_r + (long)f * V + i0;
-            const cpx<R>* gp = a.cg_p + (long)f * V + i0;
-            cpx<R>* gx = a.cg_x + (long)f * V + i0;
 #pragma unroll
-            for (int c = 0; c < CH; ++c) {
-              vr[c] = gr[off[c]];
-              vp[c] = ldg_c(gp + off[c]);
-              vx[c] = gx[off[c]];
-            }
+            for (int c = 0; c < CH; ++c) vr[c] = gr[off[c]];
             const R alpha = (R)a.red.st->alpha;
 #pragma unroll
             for (int c = 0; c < CH; ++c) {
@@ -232,9 +239,7 @@ k_p01(const P01Args<R> a) {
               q.re += w.re * ps[c].re - w.im * ps[c].im;
               q.im += w.re * ps[c].im + w.im * ps[c].re;
               cpx<R> rn = {vr[c].re - alpha * q.re, vr[c].im - alpha * q.im};
-              cpx<R> xn = {vx[c].re + alpha * vp[c].re, vx[c].im + alpha * vp[c].im};
               gr[off[c]] = rn;
-              gx[off[c]] = xn;
               acc += (double)rn.re * (double)rn.re + (double)rn.im * (double)rn.im;
             }
           } else {
@@ -247,7 +252,11 @@ k_p01(const P01Args<R> a) {
               v.re += w.re * ps[c].re - w.im * ps[c].im;
               v.im += w.re * ps[c].im + w.im * ps[c].re;
               x[k0 + c] = v;
+#if defined(WZ_DBG_SITE) && (WZ_DBG_SITE & 4)
+              if (a.scale == R(12345)) gso[off[c]] = v;
+#else
               gso[off[c]] = v;
+#endif
               if (FIN != FIN_STORE || a.red.partials)
                 acc += (double)v.re * (double)v.re + (double)v.im * (double)v.im;
             }
@@ -256,8 +265,8 @@ k_p01(const P01Args<R> a) {
       }
       if constexpr (MODE == P01_MID) {
         // forward again: pre-twist, DFT axis 0 (halves in -> DIF variant), DFT axis 1
-        using F0 = LineFFT<R, L0, +1, VAR_DIF>;
-        using F1 = LineFFT<R, L1, +1, VAR_DIT>;
+        using F0 = LineFFT<R, L0, +1, VAR_DIF, TPL0>;
+        using F1 = LineFFT<R, L1, +1, VAR_DIT, TPL1>;
         cpx<R> z[NR0];
 #pragma unroll
         for (int k = 0; k < NR0; ++k) {

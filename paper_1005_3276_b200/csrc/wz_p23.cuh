@@ -30,23 +30,24 @@ struct P23Args {
   const CGState* gate;
 };
 
-template <typename R, int L2, int L3>
+template <typename R, int L2, int L3, int T2, int T3>
 struct P23Cfg {
-  static constexpr int TPL2 = line_tpl<R, L2>::v, TPL3 = line_tpl<R, L3>::v;
+  static constexpr int TPL2 = T2, TPL3 = T3;  // lanes per line along axis 2 / axis 3
   static constexpr int NR2 = L2 / TPL2, NR3 = L3 / TPL3;
   static constexpr int NTC_A = L3 * TPL2;  // threads per component, lines along axis 2
   static constexpr int NTC_B = L2 * TPL3;  // lines along axis 3
-  static constexpr int NTC = NTC_A > NTC_B ? NTC_A : NTC_B;
-  static constexpr int NT = (4 * NTC + 31) / 32 * 32;
+  static constexpr int NTC_RAW = NTC_A > NTC_B ? NTC_A : NTC_B;
+  static constexpr int NTC = (NTC_RAW + 31) / 32 * 32;  // whole warps per spin component
+  static constexpr int NT = 4 * NTC;
   static constexpr int PITCH = L3 + 1;            // row pitch (elements)
   static constexpr int CPITCH = L2 * PITCH + 4;   // component pitch
   static constexpr size_t SMEM = sizeof(cpx<R>) * 4 * (size_t)CPITCH;
 };
 
-template <typename R, int L2, int L3, int MODE, int DIR>
-__global__ void __launch_bounds__(P23Cfg<R, L2, L3>::NT)
+template <typename R, int L2, int L3, int T2, int T3, int MODE, int DIR>
+__global__ void __launch_bounds__(P23Cfg<R, L2, L3, T2, T3>::NT)
 k_p23(const P23Args<R> a) {
-  using Cfg = P23Cfg<R, L2, L3>;
+  using Cfg = P23Cfg<R, L2, L3, T2, T3>;
   constexpr int TPL2 = Cfg::TPL2, TPL3 = Cfg::TPL3, NR2 = Cfg::NR2, NR3 = Cfg::NR3;
   constexpr int NTC = Cfg::NTC, PITCH = Cfg::PITCH, CPITCH = Cfg::CPITCH;
   constexpr int D1 = (MODE == P23_MULT) ? +1 : DIR;  // direction of the first half
@@ -65,22 +66,21 @@ k_p23(const P23Args<R> a) {
     for (int i = tid; i < 2 * 4 * 64; i += blockDim.x) tb[i] = a.tab[i];
   }
 
-  const int c = tid / NTC;      // spin component (>= 4: idle thread)
+  const int cc = tid / NTC;     // spin component (NTC is a multiple of 32)
   const int tc = tid % NTC;
-  const bool actC = c < 4;
   // role A: line along axis 2 at x3;  role B: line along axis 3 at n2
-  const int jA = tc % TPL2, x3A = tc / TPL2;
-  const bool actA = actC && (tc < L3 * TPL2);
-  const int jB = tc % TPL3, n2B = tc / TPL3;
-  const bool actB = actC && (tc < L2 * TPL3);
-  const int cc = actC ? c : 0;
+  int x3A, jA, n2B, jB;
+  lane_split<TPL2>(tc, x3A, jA);
+  lane_split<TPL3>(tc, n2B, jB);
+  const bool actA = x3A < L3;
+  const bool actB = n2B < L2;
   const cpx<R>* gin = a.in + (fbase + (long)cc * a.nplanes + plane) * PL;
   cpx<R>* gout = a.out + (fbase + (long)cc * a.nplanes + plane) * PL;
   cpx<R>* smc = sm + cc * CPITCH;
 
   // ---- half 1, axis 2 (lanes run along x3: coalesced HBM reads) ----
   {
-    using F2 = LineFFT<R, L2, D1, VAR_DIT>;
+    using F2 = LineFFT<R, L2, D1, VAR_DIT, TPL2>;
     cpx<R> x[NR2];
 #pragma unroll
     for (int k = 0; k < NR2; ++k) {
@@ -97,7 +97,7 @@ k_p23(const P23Args<R> a) {
   __syncthreads();
   // ---- half 1, axis 3 ----
   {
-    using F3 = LineFFT<R, L3, D1, VAR_DIT>;
+    using F3 = LineFFT<R, L3, D1, VAR_DIT, TPL3>;
     cpx<R> y[NR3];
 #pragma unroll
     for (int k = 0; k < NR3; ++k) {
@@ -124,8 +124,8 @@ k_p23(const P23Args<R> a) {
     }
   } else {
     // ---- momentum-diagonal multiply, then inverse axis 3 ----
-    using G3 = LineFFT<R, L3, -1, VAR_DIF>;
-    using G2 = LineFFT<R, L2, -1, VAR_DIT>;
+    using G3 = LineFFT<R, L3, -1, VAR_DIF, TPL3>;
+    using G2 = LineFFT<R, L2, -1, VAR_DIT, TPL2>;
     cpx<R> y[NR3];
     {
       const int n0 = plane / a.L1, n1 = plane % a.L1;

@@ -151,59 +151,90 @@ struct RegFFT {
 };
 
 template <typename R>
-__device__ __forceinline__ cpx<R> shfl_xor1(cpx<R> v) {
+__device__ __forceinline__ cpx<R> shfl_xor_c(cpx<R> v, int dist) {
   cpx<R> o;
-  o.re = __shfl_xor_sync(0xffffffffu, v.re, 1);
-  o.im = __shfl_xor_sync(0xffffffffu, v.im, 1);
+  o.re = __shfl_xor_sync(0xffffffffu, v.re, dist);
+  o.im = __shfl_xor_sync(0xffffffffu, v.im, dist);
   return o;
 }
 
-// Threads per line: keep at most 32 complex64 / 16 complex128 values per thread.
+// Default lanes per line: at most 32 complex64 / 16 complex128 values per thread.
+// (Kernels pick TPL per pass; more lanes per line = fewer registers, more warps.)
 template <typename R, int L>
 struct line_tpl {
   static constexpr int v = (L * (int)sizeof(R) > 128) ? 2 : 1;
 };
 
+// Thread -> (line, j) inside a group of threads working on lines with TPL lanes each:
+// the G = 32/TPL lines of a warp sit in consecutive lanes (coalescing, bank-conflict
+// free tiles), the lane sub-index j in the HIGH lane bits (shuffle distances G, 2G).
+template <int TPL>
+__device__ __forceinline__ void lane_split(int t, int& line, int& j) {
+  constexpr int G = 32 / TPL;
+  const int w = t >> 5, l = t & 31;
+  line = w * G + (l % G);
+  j = l / G;
+}
+
 enum { VAR_DIT = 0, VAR_DIF = 1 };
 
-// One lattice line of length L handled by TPL adjacent lanes; lane sub-index j.
-//  VAR_DIT: register k holds input position TPL*k + j, output index oi(k) + j*NR.
-//  VAR_DIF: register k holds input position k + j*NR,  output index TPL*oi(k) + j.
-// (TPL = 1: both are input k, output oi(k).)  All lanes of the warp must call run().
-template <typename R, int L, int DIR, int VAR>
+// One lattice line of length L handled by TPL lanes (1, 2 or 4); lane sub-index j,
+// bit b of j <-> lane xor distance XD << b.  NR = L/TPL values per lane.
+//  VAR_DIT: radix-2 steps across lanes AFTER the register FFT:
+//           input  position of register k: 2*sub_in(k, j>>1) + (j&1)   (interleaved),
+//           output index    of register k: sub_out(k, j>>1) + (j&1)*L/2 (blocks).
+//  VAR_DIF: radix-2 steps across lanes BEFORE the register FFT: input in blocks,
+//           output interleaved.  A DIT inverse feeds a DIF forward of the same TPL
+//           without any cross-lane traffic (register k -> register out_index<NR>(k)).
+// All 32 lanes of the warp must call run().
+template <typename R, int L, int DIR, int VAR, int TPL, int XD = 32 / TPL>
 struct LineFFT {
-  static constexpr int TPL = line_tpl<R, L>::v;
   static constexpr int NR = L / TPL;
+  using Sub = LineFFT<R, L / 2, DIR, VAR, TPL / 2, XD * 2>;
   static __host__ __device__ constexpr int in_pos(int k, int j) {
-    return (VAR == VAR_DIT) ? (TPL * k + j) : (k + j * NR);
+    return (VAR == VAR_DIT) ? (2 * Sub::in_pos(k, j >> 1) + (j & 1)) : (Sub::in_pos(k, j >> 1) + (j & 1) * (L / 2));
   }
   static __host__ __device__ constexpr int out_pos(int k, int j) {
-    return (VAR == VAR_DIT) ? (out_index<NR>(k) + j * NR) : (TPL * out_index<NR>(k) + j);
+    return (VAR == VAR_DIT) ? (Sub::out_pos(k, j >> 1) + (j & 1) * (L / 2)) : (2 * Sub::out_pos(k, j >> 1) + (j & 1));
   }
   static __device__ __forceinline__ void run(cpx<R>* x, int j) {
-    if constexpr (TPL == 1) {
-      RegFFT<R, L, DIR>::run(x);
-    } else if constexpr (VAR == VAR_DIT) {
-      RegFFT<R, NR, DIR>::run(x);
+    const bool odd = (j & 1) != 0;
+    if constexpr (VAR == VAR_DIT) {
+      Sub::run(x, j >> 1);
+      // twiddle w_L^n, n = Sub::out_pos(k, j>>1) = out_pos(k, 0) + lane part; the lane part
+      // (TPL = 4 only) is L/4, i.e. a factor -i (forward) on the lanes with bit 1 of j set
 #pragma unroll
       for (int k = 0; k < NR; ++k) {
         cpx<R> v = x[k];
-        if (j) v = mul_tw<R, DIR>(v, out_index<NR>(k), L);  // O[n] w_L^n
-        cpx<R> o = shfl_xor1(v);
-        x[k] = j ? csub(o, v) : cadd(v, o);  // E + O' | E - O'
+        if (odd) {
+          v = mul_tw<R, DIR>(v, Sub::out_pos(k, 0), L);
+          if (TPL >= 4 && (j & 2)) v = mul_mi<R, DIR>(v);
+        }
+        cpx<R> o = shfl_xor_c(v, XD);
+        x[k] = odd ? csub(o, v) : cadd(v, o);  // E + O' | E - O'
       }
     } else {
 #pragma unroll
       for (int k = 0; k < NR; ++k) {
         cpx<R> v = x[k];
-        cpx<R> o = shfl_xor1(v);
-        cpx<R> t = j ? csub(o, v) : cadd(v, o);  // lo - hi | lo + hi
-        if (j) t = mul_tw<R, DIR>(t, k, L);
+        cpx<R> o = shfl_xor_c(v, XD);
+        cpx<R> t = odd ? csub(o, v) : cadd(v, o);  // lo - hi | lo + hi
+        if (odd) {
+          t = mul_tw<R, DIR>(t, Sub::in_pos(k, 0), L);
+          if (TPL >= 4 && (j & 2)) t = mul_mi<R, DIR>(t);
+        }
         x[k] = t;
       }
-      RegFFT<R, NR, DIR>::run(x);
+      Sub::run(x, j >> 1);
     }
   }
+};
+template <typename R, int L, int DIR, int VAR, int XD>
+struct LineFFT<R, L, DIR, VAR, 1, XD> {
+  static constexpr int NR = L;
+  static __host__ __device__ constexpr int in_pos(int k, int) { return k; }
+  static __host__ __device__ constexpr int out_pos(int k, int) { return out_index<L>(k); }
+  static __device__ __forceinline__ void run(cpx<R>* x, int) { RegFFT<R, L, DIR>::run(x); }
 };
 
 }  // namespace wz

@@ -12,7 +12,7 @@ from dataclasses import dataclass
 import torch
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libwz.so")
+LIB_PATH = os.environ.get("WZ_LIB", os.path.join(_HERE, "libwz.so"))  # WZ_LIB: alternative build (tuning sweeps)
 _lib = None
 
 WZ_C64, WZ_C128 = 0, 1
