@@ -161,7 +161,7 @@ def run_reference(args):
 
 # algorithmic HBM bytes per launch in units of u (one spinor), nbatch = 1
 ALGO_U = {"p01_fwd": 2.0, "p23_mult": 2.0, "p01_mid": 4.25, "p01_end": 3.25, "p23_fft": 2.0, "p01_inv": 2.0,
-          "update_xr": 6.0, "update_p": 3.0}
+          "p01_fwdcg": 6.0, "p01_endcg": 4.25}
 
 
 def load_traffic():
@@ -272,14 +272,15 @@ def run_wz(args):
     # ---- per-kernel durations, live, CUDA events on the plan's stream (one source) ----
     peak, peak_src = measured_peaks()
     plan.profile(True)
-    plan.cg_solve(d_phi, d_b[:1], m, g, rho, tol, min(1000, args.max_iter), out=d_x[:1], raise_on_fail=False)
+    # the same batched solve as the timed steps, first iterations only (all sources active)
+    plan.cg_solve(d_phi, d_b, m, g, rho, tol, min(400, args.max_iter), out=d_x, raise_on_fail=False)
     prof = plan.profile_read()
     plan.profile(False)
     kinds = {k: {"us": 1e3 * ms / n, "launches": n, "share": 0.0} for k, (ms, n) in prof.items() if k in ALGO_U}
     tot = sum(v["us"] * v["launches"] for v in kinds.values()) or 1.0
     for k, v in kinds.items():
         v["share"] = v["us"] * v["launches"] / tot
-        v["algo_bytes"] = ALGO_U[k] * u
+        v["algo_bytes"] = ALGO_U[k] * u * nsrc
         v["gbs"] = v["algo_bytes"] / (v["us"] * 1e-6) / 1e9
         v["frac"] = v["gbs"] / peak
     dom = max(kinds, key=lambda k: kinds[k]["share"])

@@ -123,8 +123,8 @@ enum {
   WZ_K_P01_END = 3,  /* pass E: inverse 0,1 + Yukawa */
   WZ_K_P23_FFT = 4,  /* stand-alone DFT axes 2,3 */
   WZ_K_P01_INV = 5,  /* stand-alone inverse DFT axes 0,1 */
-  WZ_K_UPDATE_XR = 6,
-  WZ_K_UPDATE_P = 7,
+  WZ_K_P01_FWDCG = 6, /* pass A': x += alpha p, p <- r + beta p, twist + DFT axes 0,1 */
+  WZ_K_P01_ENDCG = 7, /* pass E': inverse 0,1 + Yukawa, r -= alpha q, ||r||^2, stop rule */
   WZ_K_OTHER = 8,
   WZ_NKINDS = 9
 };

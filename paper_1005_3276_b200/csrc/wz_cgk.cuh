@@ -1,6 +1,5 @@
 // wz_cgk.cuh -- CG vector kernels:
-// fused AXPY pairs with float64 norm accumulation, the search-direction update,
-// and the complex128 reliable-update pieces for complex64 solves (G9).
+// initialisation, the deferred x update, and the complex128 reliable-update pieces for complex64 solves (G9).
 // Vectors are treated as flat real arrays of 2*4V entries, 16-byte accesses.
 #pragma once
 #include "wz_common.cuh"
@@ -43,6 +42,11 @@ template <typename R>
 __global__ void __launch_bounds__(CGK_NT)
 k_cg_init(const R* __restrict__ b, R* __restrict__ r, R* __restrict__ p, R* __restrict__ xs,
           double* __restrict__ X, long n, RedArgs red) {
+  const int src = blockIdx.y;  // one source per grid row
+  b += src * n; r += src * n; p += src * n;
+  if (xs) xs += src * n;
+  if (X) X += src * n;
+  red = red.for_source(src);
   constexpr int N = vec16<R>::N;
   __shared__ double sh[33];
   double acc = 0.0;
@@ -66,39 +70,13 @@ k_cg_init(const R* __restrict__ b, R* __restrict__ r, R* __restrict__ p, R* __re
   grid_reduce<FIN_INIT>(acc, red, blockIdx.x, gridDim.x, sh);
 }
 
-// x += alpha p;  r -= alpha q;  ||r||^2 -> FIN_RR.   TX: type of x (R, or double for
-// complex128 solves writing straight into the caller's buffer).
-template <typename R, typename TX>
-__global__ void __launch_bounds__(CGK_NT)
-k_update_xr(TX* __restrict__ x, R* __restrict__ r, const R* __restrict__ p,
-            const R* __restrict__ q, long n, RedArgs red) {
-  constexpr int N = vec16<R>::N;
-  __shared__ double sh[33];
-  if (!cg_active(red.st)) return;
-  const R alpha = (R)red.st->alpha;
-  double acc = 0.0;
-  for (long i = ((long)blockIdx.x * blockDim.x + threadIdx.x) * N; i < n;
-       i += (long)gridDim.x * blockDim.x * N) {
-    R vp[N], vq[N], vr[N];
-    ld16<R>(p + i, vp);
-    ld16<R>(q + i, vq);
-    ld16<R>(r + i, vr);
-#pragma unroll
-    for (int e = 0; e < N; ++e) {
-      x[i + e] = (TX)((R)x[i + e] + alpha * vp[e]);
-      vr[e] = vr[e] - alpha * vq[e];
-      acc += (double)vr[e] * (double)vr[e];
-    }
-    st16<R>(r + i, vr);
-  }
-  grid_reduce<FIN_RR>(acc, red, blockIdx.x, gridDim.x, sh);
-}
-
 // x += alpha p with the alpha still pending in the CG state (the fused pass A' applies
 // it one iteration late); not gated.  k_clear_alpha then marks it as applied.
 template <typename R>
 __global__ void __launch_bounds__(CGK_NT)
 k_flush_x(R* __restrict__ x, const R* __restrict__ p, long n, const CGState* st) {
+  const int src = blockIdx.y;
+  x += src * n; p += src * n; st += src;
   constexpr int N = vec16<R>::N;
   const R alpha = (R)st->alpha;
   if (alpha == R(0)) return;
@@ -112,29 +90,12 @@ k_flush_x(R* __restrict__ x, const R* __restrict__ p, long n, const CGState* st)
     st16<R>(x + i, vx);
   }
 }
-__global__ void k_clear_alpha(CGState* st) { st->alpha = 0.0; }
-
-// p = r + beta p
-template <typename R>
-__global__ void __launch_bounds__(CGK_NT)
-k_update_p(R* __restrict__ p, const R* __restrict__ r, long n, const CGState* st) {
-  constexpr int N = vec16<R>::N;
-  if (!cg_active(st)) return;
-  const R beta = (R)st->beta;
-  for (long i = ((long)blockIdx.x * blockDim.x + threadIdx.x) * N; i < n;
-       i += (long)gridDim.x * blockDim.x * N) {
-    R vp[N], vr[N];
-    ld16<R>(p + i, vp);
-    ld16<R>(r + i, vr);
-#pragma unroll
-    for (int e = 0; e < N; ++e) vp[e] = vr[e] + beta * vp[e];
-    st16<R>(p + i, vp);
-  }
-}
+__global__ void k_clear_alpha(CGState* st) { st[blockIdx.x].alpha = 0.0; }
 
 // Reliable update, part 1:  X += xs (complex128 += complex64);  xs = 0.
 __global__ void __launch_bounds__(CGK_NT)
 k_ru_accum(double* __restrict__ X, float* __restrict__ xs, long n) {
+  X += blockIdx.y * n; xs += blockIdx.y * n;
   for (long i = ((long)blockIdx.x * blockDim.x + threadIdx.x) * 4; i < n;
        i += (long)gridDim.x * blockDim.x * 4) {
     float v[4], z[4] = {0.f, 0.f, 0.f, 0.f};
@@ -156,6 +117,10 @@ template <typename TB, typename TR, int FIN>
 __global__ void __launch_bounds__(CGK_NT)
 k_resid(const TB* __restrict__ b, const double* __restrict__ q, TR* __restrict__ r, long n,
         RedArgs red) {
+  const int src = blockIdx.y;
+  b += src * n; q += src * n;
+  if (r) r += src * n;
+  red = red.for_source(src);
   __shared__ double sh[33];
   double acc = 0.0;
   for (long i = ((long)blockIdx.x * blockDim.x + threadIdx.x) * 2; i < n;

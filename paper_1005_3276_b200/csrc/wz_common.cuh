@@ -94,11 +94,22 @@ __device__ __forceinline__ void cg_finalize(double total, CGState* st, double* s
 }
 
 // Reduction workspace: one partial per block, a ticket counter, and the target.
+// Batched solves keep one CGState, one counter and one row of partials PER SOURCE; a
+// kernel working on source `src` uses for_source(src).
 struct RedArgs {
-  double* partials;   // [nblocks]
-  unsigned* counter;  // zero before first use; left zero after each use
-  CGState* st;
-  double* store;      // FIN_STORE target
+  double* partials;   // [nsources][pstride]
+  unsigned* counter;  // [nsources]; zero before first use; left zero after each use
+  CGState* st;        // [nsources]
+  double* store;      // FIN_STORE target, [nsources]
+  int pstride;
+  __host__ __device__ RedArgs for_source(int src) const {
+    RedArgs r = *this;
+    r.partials = partials ? partials + (long)src * pstride : nullptr;
+    r.counter = counter ? counter + src : nullptr;
+    r.st = st ? st + src : nullptr;
+    r.store = store ? store + src : nullptr;
+    return r;
+  }
 };
 
 // Sum `v` over the block in a fixed order; returns the total in thread 0.

@@ -10,7 +10,6 @@
 #include "../../include/wz.h"
 #include "wz_cgk.cuh"
 #include "wz_p01.cuh"
-#include "wz_p01p.cuh"
 #include "wz_p23.cuh"
 
 using namespace wz;
@@ -30,12 +29,10 @@ bool cuda_ok(cudaError_t e, const char* what) {
   } while (0)
 
 // ---- kernel dispatch tables ---------------------------------------------------
-// One (x0,x1)-pass kernel: the plain version (one tile per CTA) or the persistent
-// pipelined version (wz_p01p.cuh), with its launch shape.
+// One (x0,x1)-pass kernel with its launch shape.
 template <typename R>
 struct P01Kern {
   void (*fn)(const P01Args<R>) = nullptr;
-  void (*fnp)(const P01Args<R>, int, int) = nullptr;  // persistent: (args, nseg_tiles, ntiles)
   int nt = 0, nseg = 0;
   size_t smem = 0;
 };
@@ -43,17 +40,7 @@ template <typename R>
 struct P01Entry {
   int L0, L1;
   P01Kern<R> fwd, inv, mid, mid_pq, end, fwdcg, endcg;
-  int max_nseg_tiles(long I) const {  // widest grid any kernel of this entry uses (per field)
-    int m = 1;
-    for (const P01Kern<R>* k : {&fwd, &inv, &mid, &mid_pq, &end, &fwdcg, &endcg})
-      if ((int)(I / k->nseg) > m) m = (int)(I / k->nseg);
-    return m;
-  }
-  bool divides(long I) const {
-    for (const P01Kern<R>* k : {&fwd, &inv, &mid, &mid_pq, &end, &fwdcg, &endcg})
-      if (I % k->nseg) return false;
-    return true;
-  }
+  int nseg() const { return fwd.nseg; }
 };
 template <typename R>
 struct P23Entry {
@@ -75,7 +62,7 @@ struct P23Entry {
 #define WZ_TPL32F_P23 2
 #endif
 #ifndef WZ_NSEG32F
-#define WZ_NSEG32F 8
+#define WZ_NSEG32F 4
 #endif
 template <typename R, int L> struct tune_tpl {   // axes 0,1
   static constexpr int v = (sizeof(R) == 4) ? (L >= 48 ? 2 : (L == 32 ? WZ_TPL32F : 1))
@@ -92,34 +79,13 @@ template <typename R, int L0, int L1> struct tune_nseg {
                                             : (L0 * L1 > 2048 ? 2 : 4);
 };
 
-#ifndef WZ_TPLP32F
-#define WZ_TPLP32F 2
-#endif
-#ifndef WZ_PIPELINE
-#define WZ_PIPELINE 1
-#endif
-// which lattices use the persistent pipelined (x0,x1) pass, and its tile shape
-template <typename R, int L0, int L1> struct tune_pipe {
-  static constexpr bool on = WZ_PIPELINE && sizeof(R) == 4 && L0 == 32 && L1 == 32;
-};
-template <typename R, int L0, int L1> struct tune_pipe_shape {
-  static constexpr int nseg = 4, t0 = WZ_TPLP32F, t1 = WZ_TPLP32F;
-};
-
 template <typename R, int L0, int L1, int MODE, int FIN>
 P01Kern<R> make_p01_kern() {
+  constexpr int NSEG = tune_nseg<R, L0, L1>::v, T0 = tune_tpl<R, L0>::v, T1 = tune_tpl<R, L1>::v;
+  using C = P01Cfg<R, L0, L1, NSEG, T0, T1>;
   P01Kern<R> k;
-  if constexpr (tune_pipe<R, L0, L1>::on) {
-    using TP = tune_pipe_shape<R, L0, L1>;
-    using C = P01PCfg<R, L0, L1, TP::nseg, TP::t0, TP::t1, MODE>;
-    k.fnp = k_p01p<R, L0, L1, TP::nseg, TP::t0, TP::t1, MODE, FIN>;
-    k.nt = C::NT; k.nseg = TP::nseg; k.smem = C::SMEM;
-  } else {
-    constexpr int NSEG = tune_nseg<R, L0, L1>::v, T0 = tune_tpl<R, L0>::v, T1 = tune_tpl<R, L1>::v;
-    using C = P01Cfg<R, L0, L1, NSEG, T0, T1>;
-    k.fn = k_p01<R, L0, L1, NSEG, T0, T1, MODE, FIN>;
-    k.nt = C::NT; k.nseg = NSEG; k.smem = C::SMEM;
-  }
+  k.fn = k_p01<R, L0, L1, NSEG, T0, T1, MODE, FIN>;
+  k.nt = C::NT; k.nseg = NSEG; k.smem = C::SMEM;
   return k;
 }
 template <typename R, int L0, int L1>
@@ -185,7 +151,7 @@ template <typename K>
 bool set_smem(K kernel, size_t bytes);
 template <typename R>
 bool set_smem_kern(const P01Kern<R>& k) {
-  return k.fn ? set_smem(k.fn, k.smem) : set_smem(k.fnp, k.smem);
+  return set_smem(k.fn, k.smem);
 }
 template <typename K>
 bool set_smem(K kernel, size_t bytes) {
@@ -217,8 +183,8 @@ struct wz_plan {
   OpWS<float> wsf;
   OpWS<double> wsd;        // always present: complex128 operator (plans of both dtypes)
   // CG vectors
-  void *r = nullptr, *p = nullptr, *q = nullptr, *xs = nullptr;  // plan dtype, one spinor each
-  cpx<double>* q128 = nullptr;    // C64 plans: A X in complex128
+  void *r = nullptr, *p = nullptr, *xs = nullptr;  // plan dtype, max_batch spinors each
+  cpx<double>* q128 = nullptr;    // A X in complex128 (reliable updates, true residual), one spinor
   cpx<double>* phi128 = nullptr;  // C64 plans: phi widened
   double* partials = nullptr;
   unsigned* counter = nullptr;
@@ -230,6 +196,7 @@ struct wz_plan {
   std::vector<void*> allocs;
   // optional per-kernel timing (wz_plan_profile): event pairs around sampled launches
   int profile = 0;
+  int prof_override = -1;  // >= 0: record launches under this kind (reliable-update matvecs -> other)
   std::vector<cudaEvent_t> prof_ev;      // 2 per recorded launch
   std::vector<int> prof_kind;
   double prof_ms[WZ_NKINDS] = {0};
@@ -289,7 +256,7 @@ wz_status setup_ws(wz_plan* pl, OpWS<R>& ws, int nbatch_t) {
   ws.p01 = find_p01<R>(pl->L[0], pl->L[1]);
   ws.p23 = find_p23<R>(pl->L[2], pl->L[3]);
   if (!ws.p01 || !ws.p23) return WZ_EUNSUPPORTED;
-  if (!ws.p01->divides(pl->I)) return WZ_EUNSUPPORTED;
+  if (pl->I % ws.p01->nseg()) return WZ_EUNSUPPORTED;
   const auto* a = ws.p01;
   if (!set_smem_kern(a->fwd) || !set_smem_kern(a->inv) || !set_smem_kern(a->mid) ||
       !set_smem_kern(a->mid_pq) || !set_smem_kern(a->end) || !set_smem_kern(a->fwdcg) ||
@@ -318,7 +285,7 @@ constexpr size_t kProfMaxPairs = 8192;
 // Bracket the next launch with events when profiling (bounded number of samples).
 struct ProfScope {
   wz_plan* pl; int kind; bool on = false;
-  ProfScope(wz_plan* p, int k) : pl(p), kind(k) {
+  ProfScope(wz_plan* p, int k) : pl(p), kind(p->prof_override >= 0 ? p->prof_override : k) {
     if (pl->profile && pl->prof_kind.size() < kProfMaxPairs) {
       cudaEvent_t a, b;
       if (cudaEventCreate(&a) == cudaSuccess && cudaEventCreate(&b) == cudaSuccess) {
@@ -347,16 +314,17 @@ wz_status launch_p01(wz_plan* pl, int kind, const P01Kern<R>& k, const P01Args<R
   const int nseg_tiles = (int)(pl->I / k.nseg), nf = 4 * nb;
   {
     ProfScope ps(pl, kind);
-    if (k.fnp) {
-      const int ntiles = nseg_tiles * nf;
-      const int grid = ntiles < pl->num_sms ? ntiles : pl->num_sms;
-      k.fnp<<<grid, k.nt, k.smem, pl->stream>>>(args, nseg_tiles, ntiles);
-    } else {
-      k.fn<<<dim3((unsigned)nseg_tiles, (unsigned)nf), k.nt, k.smem, pl->stream>>>(args);
-    }
+    k.fn<<<dim3((unsigned)nseg_tiles, (unsigned)nf), k.nt, k.smem, pl->stream>>>(args);
   }
   WZ_CUDA(cudaGetLastError());
   return WZ_OK;
+}
+
+RedArgs red_of(wz_plan* pl) {
+  RedArgs r;
+  r.partials = pl->partials; r.counter = pl->counter; r.st = pl->d_state; r.store = nullptr;
+  r.pstride = pl->npartials;
+  return r;
 }
 
 template <typename R>
@@ -441,8 +409,8 @@ wz_status apply_MdagM_impl(wz_plan* pl, const cpx<R>* phi, const double m[2], co
   a.in = ws.t; a.out = ws.t; a.scale = invV;
   a.psi = in; a.phi = phi; a.site_out = ws.chi; a.op = make_op<R>(m, g, rho, 0);
   if (cg) {
-    a.red.partials = pl->partials; a.red.counter = pl->counter; a.red.st = pl->d_state; a.red.store = nullptr;
-    if (ws.p01->max_nseg_tiles(pl->I) * 4 * nb > pl->npartials) return WZ_EINVAL;
+    a.red = red_of(pl);
+    if ((int)(pl->I / ws.p01->nseg()) * 4 > pl->npartials) return WZ_EINVAL;
     s = launch_p01<R>(pl, WZ_K_P01_MID, ws.p01->mid_pq, a, nb);  // C
   } else {
     s = launch_p01<R>(pl, WZ_K_P01_MID, ws.p01->mid, a, nb);
@@ -462,30 +430,29 @@ wz_status apply_MdagM_impl(wz_plan* pl, const cpx<R>* phi, const double m[2], co
 // state; every kernel is gated on it.  x lags one update: flush_x() before x is used. --
 template <typename R>
 wz_status cg_iteration(wz_plan* pl, const cpx<R>* phi, const double m[2], const double g[2], double rho,
-                       cpx<R>* r, cpx<R>* p, cpx<R>* x) {
+                       cpx<R>* r, cpx<R>* p, cpx<R>* x, int nb) {
   OpWS<R>& ws = ws_of<R>(pl);
-  const int nb = 1;
-  const dim3 g23((unsigned)(pl->L[0] * pl->L[1]), 1u);
-  if (ws.p01->max_nseg_tiles(pl->I) * 4 > pl->npartials) return WZ_EINVAL;
+  const dim3 g23((unsigned)(pl->L[0] * pl->L[1]), (unsigned)nb);
+  if ((int)(pl->I / ws.p01->nseg()) * 4 > pl->npartials) return WZ_EINVAL;
   const R invV = (R)(1.0 / (double)pl->V);
   wz_status s;
   P01Args<R> a{};
   a.I = pl->I; a.apbc = 1; a.scale = R(1); a.gate = pl->d_state;
   a.in = p; a.out = ws.t; a.cg_r = r; a.cg_p = p; a.cg_x = x;
-  if ((s = launch_p01<R>(pl, WZ_K_P01_FWD, ws.p01->fwdcg, a, nb)) != WZ_OK) return s;
+  if ((s = launch_p01<R>(pl, WZ_K_P01_FWDCG, ws.p01->fwdcg, a, nb)) != WZ_OK) return s;
   P23Args<R> b{};
   b.in = ws.t; b.out = ws.t; b.nplanes = pl->L[0] * pl->L[1]; b.L1 = pl->L[1]; b.scale = R(1);
   b.tab = ws.tab; b.rho = (R)rho; b.sign = R(1); b.gate = pl->d_state;
   if ((s = launch<R>(pl, WZ_K_P23_MULT, ws.p23->mult, g23, ws.p23->nt, ws.p23->smem, b)) != WZ_OK) return s;
   a.in = ws.t; a.out = ws.t; a.scale = invV;
   a.psi = p; a.phi = phi; a.site_out = ws.chi; a.op = make_op<R>(m, g, rho, 0);
-  a.red.partials = pl->partials; a.red.counter = pl->counter; a.red.st = pl->d_state; a.red.store = nullptr;
+  a.red = red_of(pl);
   if ((s = launch_p01<R>(pl, WZ_K_P01_MID, ws.p01->mid_pq, a, nb)) != WZ_OK) return s;
   b.sign = R(-1);
   if ((s = launch<R>(pl, WZ_K_P23_MULT, ws.p23->mult, g23, ws.p23->nt, ws.p23->smem, b)) != WZ_OK) return s;
   a.psi = ws.chi; a.site_out = nullptr; a.op = make_op<R>(m, g, rho, 1);
   a.cg_r = r; a.cg_p = p; a.cg_x = x;
-  return launch_p01<R>(pl, WZ_K_P01_END, ws.p01->endcg, a, nb);
+  return launch_p01<R>(pl, WZ_K_P01_ENDCG, ws.p01->endcg, a, nb);
 }
 
 }  // namespace
@@ -513,11 +480,11 @@ int wz_supported(int T, int L1, int L2, int L3, wz_dtype dtype) {
   // every plan needs the complex128 operator (reliable updates, true residual)
   const auto* ad = find_p01<double>(T, L1);
   const auto* bd = find_p23<double>(L2, L3);
-  if (!ad || !bd || !ad->divides(I)) return 0;
+  if (!ad || !bd || I % ad->nseg()) return 0;
   if (dtype == WZ_C64) {
     const auto* af = find_p01<float>(T, L1);
     const auto* bf = find_p23<float>(L2, L3);
-    if (!af || !bf || !af->divides(I)) return 0;
+    if (!af || !bf || I % af->nseg()) return 0;
   }
   return 1;
 }
@@ -576,32 +543,31 @@ wz_status wz_plan_create(wz_plan** plan, int T, int L1, int L2, int L3, wz_dtype
   wz_status s = WZ_OK;
   const size_t n1 = (size_t)4 * pl->V;
   do {
+    const size_t nbv = (size_t)max_batch * n1;  // CG vectors: one spinor per source
     if (dtype == WZ_C64) {
       if ((s = setup_ws<float>(pl, pl->wsf, max_batch)) != WZ_OK) break;
       if ((s = setup_ws<double>(pl, pl->wsd, 1)) != WZ_OK) break;
-      float *r, *p, *q, *xs;
-      if (!dev_alloc(pl, &r, 2 * n1) || !dev_alloc(pl, &p, 2 * n1) || !dev_alloc(pl, &q, 2 * n1) ||
-          !dev_alloc(pl, &xs, 2 * n1) || !dev_alloc(pl, &pl->q128, n1) ||
-          !dev_alloc(pl, &pl->phi128, (size_t)pl->V)) { s = WZ_ENOMEM; break; }
-      pl->r = r; pl->p = p; pl->q = q; pl->xs = xs;
+      float *r, *p, *xs;
+      if (!dev_alloc(pl, &r, 2 * nbv) || !dev_alloc(pl, &p, 2 * nbv) || !dev_alloc(pl, &xs, 2 * nbv) ||
+          !dev_alloc(pl, &pl->q128, n1) || !dev_alloc(pl, &pl->phi128, (size_t)pl->V)) { s = WZ_ENOMEM; break; }
+      pl->r = r; pl->p = p; pl->xs = xs;
     } else {
       if ((s = setup_ws<double>(pl, pl->wsd, max_batch)) != WZ_OK) break;
-      double *r, *p, *q;
-      if (!dev_alloc(pl, &r, 2 * n1) || !dev_alloc(pl, &p, 2 * n1) || !dev_alloc(pl, &q, 2 * n1)) {
+      double *r, *p;
+      if (!dev_alloc(pl, &r, 2 * nbv) || !dev_alloc(pl, &p, 2 * nbv) || !dev_alloc(pl, &pl->q128, n1)) {
         s = WZ_ENOMEM; break;
       }
-      pl->r = r; pl->p = p; pl->q = q;
+      pl->r = r; pl->p = p;
     }
-    // reduction workspace: enough partials for the widest grid used in a solve
-    const int nseg_min = 2;
-    long np = (pl->I / nseg_min) * 4;
+    // reduction workspace per source: a row of partials wide enough for every grid used
+    long np = (pl->I / 2) * 4;
     if (np < 4096) np = 4096;
     pl->npartials = (int)np;
-    if (!dev_alloc(pl, &pl->partials, (size_t)np) || !dev_alloc(pl, &pl->counter, 4) ||
-        !dev_alloc(pl, &pl->d_state, 1)) { s = WZ_ENOMEM; break; }
-    if (!cuda_ok(cudaMemsetAsync(pl->counter, 0, 4 * sizeof(unsigned), pl->stream), "cudaMemsetAsync") ||
-        !cuda_ok(cudaMemsetAsync(pl->d_state, 0, sizeof(CGState), pl->stream), "cudaMemsetAsync") ||
-        !cuda_ok(cudaMallocHost((void**)&pl->h_state, 2 * sizeof(CGState)), "cudaMallocHost") ||
+    if (!dev_alloc(pl, &pl->partials, (size_t)np * max_batch) || !dev_alloc(pl, &pl->counter, (size_t)max_batch) ||
+        !dev_alloc(pl, &pl->d_state, (size_t)max_batch)) { s = WZ_ENOMEM; break; }
+    if (!cuda_ok(cudaMemsetAsync(pl->counter, 0, max_batch * sizeof(unsigned), pl->stream), "cudaMemsetAsync") ||
+        !cuda_ok(cudaMemsetAsync(pl->d_state, 0, max_batch * sizeof(CGState), pl->stream), "cudaMemsetAsync") ||
+        !cuda_ok(cudaMallocHost((void**)&pl->h_state, 2 * max_batch * sizeof(CGState)), "cudaMallocHost") ||
         !cuda_ok(cudaEventCreateWithFlags(&pl->ev[0], cudaEventDisableTiming), "cudaEventCreate") ||
         !cuda_ok(cudaEventCreateWithFlags(&pl->ev[1], cudaEventDisableTiming), "cudaEventCreate") ||
         !cuda_ok(cudaStreamSynchronize(pl->stream), "cudaStreamSynchronize")) { s = WZ_ECUDA; break; }
@@ -616,7 +582,7 @@ wz_status wz_plan_create(wz_plan** plan, int T, int L1, int L2, int L3, wz_dtype
 
 const char* wz_kind_name(int k) {
   static const char* names[WZ_NKINDS] = {"p01_fwd", "p23_mult", "p01_mid", "p01_end", "p23_fft",
-                                         "p01_inv", "update_xr", "update_p", "other"};
+                                         "p01_inv", "p01_fwdcg", "p01_endcg", "other"};
   return (k >= 0 && k < WZ_NKINDS) ? names[k] : "?";
 }
 
@@ -705,118 +671,141 @@ int vec_grid(long n_real, int per_thread) {
   return (int)nb;
 }
 
-RedArgs red_of(wz_plan* pl) {
-  RedArgs r;
-  r.partials = pl->partials; r.counter = pl->counter; r.st = pl->d_state; r.store = nullptr;
-  return r;
-}
-
-// One source.  R = iteration precision.  X: caller's complex128 solution buffer.
+// All nb sources advance in lock step through the same five kernels per iteration
+// (grid rows = sources), each with its own device-resident CG state: a source that
+// has converged, hit max_iter or waits for a reliable update simply idles (its CTAs
+// return at once).  The host looks at the states every kCheckEvery iterations, one
+// chunk behind the GPU, and serves reliable updates source by source.
+// R = iteration precision.  X: caller's complex128 solution buffer.
 template <typename R>
-wz_status cg_one(wz_plan* pl, const cpx<R>* phi, const cpx<R>* b, cpx<double>* X, const double m[2],
-                 const double g[2], double rho, double tol, int max_iter, wz_cg_info* info) {
+wz_status cg_batch(wz_plan* pl, const cpx<R>* phi, const cpx<R>* b, cpx<double>* X, const double m[2],
+                   const double g[2], double rho, double tol, int max_iter, int nb, wz_cg_info* info) {
   constexpr bool kRU = (sizeof(R) == 4);
   constexpr int N = vec16<R>::N;
-  const long n = 8 * pl->V;  // real entries of one spinor
+  const long n = 8 * pl->V;       // real entries of one spinor
+  const size_t n1 = (size_t)4 * pl->V;  // complex entries of one spinor
   cudaStream_t st = pl->stream;
-  R* r = (R*)pl->r; R* p = (R*)pl->p; R* q = (R*)pl->q; R* xs = (R*)pl->xs;
+  R* r = (R*)pl->r; R* p = (R*)pl->p; R* xs = (R*)pl->xs;
   const int gv = vec_grid(n, N), gv2 = vec_grid(n, 2), gv4 = vec_grid(n, 4);
   wz_status s;
 
-  CGState h;
-  memset(&h, 0, sizeof(h));
-  h.tol = tol; h.delta = kDelta; h.max_iter = max_iter; h.use_ru = kRU ? 1 : 0;
-  h.true_rr = -1.0;
-  WZ_CUDA(cudaMemcpyAsync(pl->d_state, &h, sizeof(h), cudaMemcpyHostToDevice, st));
-  WZ_CUDA(cudaStreamSynchronize(st));  // h is a stack variable
-  k_cg_init<R><<<gv, CGK_NT, 0, st>>>((const R*)b, r, p, kRU ? xs : nullptr, (double*)X, n, red_of(pl));
-  pl->launches++;
+  std::vector<CGState> h(nb);
+  memset(h.data(), 0, sizeof(CGState) * nb);
+  for (int j = 0; j < nb; ++j) {
+    h[j].tol = tol; h[j].delta = kDelta; h[j].max_iter = max_iter; h[j].use_ru = kRU ? 1 : 0;
+    h[j].true_rr = -1.0;
+    if (max_iter == 0) h[j].stop = 1;
+  }
+  WZ_CUDA(cudaMemcpyAsync(pl->d_state, h.data(), sizeof(CGState) * nb, cudaMemcpyHostToDevice, st));
+  WZ_CUDA(cudaStreamSynchronize(st));  // h is pageable host memory
+  {
+    ProfScope ps(pl, WZ_K_OTHER);
+    k_cg_init<R><<<dim3(gv, nb), CGK_NT, 0, st>>>((const R*)b, r, p, kRU ? xs : nullptr, (double*)X, n, red_of(pl));
+  }
   WZ_CUDA(cudaGetLastError());
 
-  // x += alpha p still pending from the last active iteration (the iteration kernels are idle)
-  auto flush_x = [&]() -> wz_status {
+  // x += alpha p still pending from the last active iteration of source j (its kernels idle)
+  auto flush_x = [&](int j) -> wz_status {
     {
       ProfScope ps(pl, WZ_K_OTHER);
-      if constexpr (kRU) k_flush_x<R><<<gv, CGK_NT, 0, st>>>(xs, p, n, pl->d_state);
-      else k_flush_x<R><<<gv, CGK_NT, 0, st>>>((R*)X, p, n, pl->d_state);
+      if constexpr (kRU) k_flush_x<R><<<dim3(gv, 1), CGK_NT, 0, st>>>(xs + j * n, p + j * n, n, pl->d_state + j);
+      else k_flush_x<R><<<dim3(gv, 1), CGK_NT, 0, st>>>((R*)X + j * n, p + j * n, n, pl->d_state + j);
     }
     {
       ProfScope ps(pl, WZ_K_OTHER);
-      k_clear_alpha<<<1, 1, 0, st>>>(pl->d_state);
+      k_clear_alpha<<<1, 1, 0, st>>>(pl->d_state + j);
     }
     WZ_CUDA(cudaGetLastError());
     return WZ_OK;
   };
-  auto reliable_update = [&](bool final_only) -> wz_status {
-    // X += xs; xs = 0; q128 = A X (complex128); r = b - q128
+  // residual of source j recomputed in complex128:  q128 = A X_j;  d = b_j - q128
+  auto residual128 = [&](int j, bool update_r) -> wz_status {
+    RedArgs ra = red_of(pl).for_source(j);
+    struct Override {  // the one-source complex128 matvec is not part of the batched iteration
+      wz_plan* p;
+      explicit Override(wz_plan* q) : p(q) { p->prof_override = WZ_K_OTHER; }
+      ~Override() { p->prof_override = -1; }
+    } ov(pl);
     if constexpr (kRU) {
-      k_ru_accum<<<gv4, CGK_NT, 0, st>>>((double*)X, (float*)xs, n);
-      pl->launches++;
-      wz_status s2 = apply_MdagM_impl<double>(pl, pl->phi128, m, g, rho, X, pl->q128, 1, false);
+      if (update_r) {  // X += xs; xs = 0
+        ProfScope ps(pl, WZ_K_OTHER);
+        k_ru_accum<<<dim3(gv4, 1), CGK_NT, 0, st>>>((double*)(X + j * n1), (float*)(xs + j * n), n);
+      }
+      wz_status s2 = apply_MdagM_impl<double>(pl, pl->phi128, m, g, rho, X + j * n1, pl->q128, 1, false);
       if (s2 != WZ_OK) return s2;
-      if (final_only)
-        k_resid<float, float, FIN_TRUE><<<gv2, CGK_NT, 0, st>>>((const float*)b, (const double*)pl->q128,
-                                                                 nullptr, n, red_of(pl));
+      ProfScope ps(pl, WZ_K_OTHER);
+      if (update_r)
+        k_resid<float, float, FIN_RU><<<dim3(gv2, 1), CGK_NT, 0, st>>>(
+            (const float*)(b + j * n1), (const double*)pl->q128, (float*)(r + j * n), n, ra);
       else
-        k_resid<float, float, FIN_RU><<<gv2, CGK_NT, 0, st>>>((const float*)b, (const double*)pl->q128,
-                                                               (float*)r, n, red_of(pl));
-      pl->launches++;
-      WZ_CUDA(cudaGetLastError());
+        k_resid<float, float, FIN_TRUE><<<dim3(gv2, 1), CGK_NT, 0, st>>>(
+            (const float*)(b + j * n1), (const double*)pl->q128, nullptr, n, ra);
+    } else {
+      wz_status s2 = apply_MdagM_impl<double>(pl, (const cpx<double>*)phi, m, g, rho, X + j * n1, pl->q128, 1, false);
+      if (s2 != WZ_OK) return s2;
+      ProfScope ps(pl, WZ_K_OTHER);
+      k_resid<double, double, FIN_TRUE><<<dim3(gv2, 1), CGK_NT, 0, st>>>(
+          (const double*)(b + j * n1), (const double*)pl->q128, nullptr, n, ra);
     }
+    WZ_CUDA(cudaGetLastError());
     return WZ_OK;
   };
 
-  int slot_w = 0, slot_r = 0, inflight = 0, ru_served = 0;
-  CGState fin;
+  int slot_w = 0, slot_r = 0, inflight = 0;
+  std::vector<int> ru_served(nb, 0);
+  const CGState* snap = nullptr;
   for (;;) {
     while (inflight < 2) {
       for (int it = 0; it < kCheckEvery; ++it) {
         if constexpr (kRU)
-          s = cg_iteration<R>(pl, phi, m, g, rho, (cpx<R>*)r, (cpx<R>*)p, (cpx<R>*)xs);
+          s = cg_iteration<R>(pl, phi, m, g, rho, (cpx<R>*)r, (cpx<R>*)p, (cpx<R>*)xs, nb);
         else
-          s = cg_iteration<R>(pl, phi, m, g, rho, (cpx<R>*)r, (cpx<R>*)p, (cpx<R>*)X);
+          s = cg_iteration<R>(pl, phi, m, g, rho, (cpx<R>*)r, (cpx<R>*)p, (cpx<R>*)X, nb);
         if (s != WZ_OK) return s;
       }
-      WZ_CUDA(cudaGetLastError());
-      WZ_CUDA(cudaMemcpyAsync(&pl->h_state[slot_w], pl->d_state, sizeof(CGState), cudaMemcpyDeviceToHost, st));
+      WZ_CUDA(cudaMemcpyAsync(pl->h_state + slot_w * pl->max_batch, pl->d_state, sizeof(CGState) * nb,
+                              cudaMemcpyDeviceToHost, st));
       WZ_CUDA(cudaEventRecord(pl->ev[slot_w], st));
       slot_w ^= 1;
       ++inflight;
     }
     WZ_CUDA(cudaEventSynchronize(pl->ev[slot_r]));
-    fin = pl->h_state[slot_r];
+    snap = pl->h_state + slot_r * pl->max_batch;
     slot_r ^= 1;
     --inflight;
-    if (fin.converged || fin.stop) break;
-    if (fin.need_ru && fin.n_ru == ru_served) {
-      if ((s = flush_x()) != WZ_OK) return s;
-      if ((s = reliable_update(false)) != WZ_OK) return s;  // sets beta; the next pass A' applies it
-      ++ru_served;
+    bool all_done = true;
+    for (int j = 0; j < nb; ++j) {
+      if (snap[j].converged || snap[j].stop) continue;
+      all_done = false;
+      if (snap[j].need_ru && snap[j].n_ru == ru_served[j]) {
+        if ((s = flush_x(j)) != WZ_OK) return s;
+        if ((s = residual128(j, true)) != WZ_OK) return s;  // sets beta; the next pass A' applies it
+        ++ru_served[j];
+      }
     }
-  }
-  if ((s = flush_x()) != WZ_OK) return s;
-  // true residual at exit
-  if constexpr (kRU) {
-    WZ_CUDA(cudaStreamSynchronize(st));
-    WZ_CUDA(cudaMemcpy(&fin, pl->d_state, sizeof(CGState), cudaMemcpyDeviceToHost));
-    if (!fin.converged && fin.bnorm2 > 0.0) {
-      if ((s = reliable_update(true)) != WZ_OK) return s;
-    }
-  } else {
-    if ((s = apply_MdagM_impl<double>(pl, (const cpx<double>*)phi, m, g, rho, X, (cpx<double>*)q, 1, false)) != WZ_OK)
-      return s;
-    k_resid<double, double, FIN_TRUE><<<gv2, CGK_NT, 0, st>>>((const double*)b, (const double*)q, nullptr, n,
-                                                               red_of(pl));
-    pl->launches++;
-    WZ_CUDA(cudaGetLastError());
+    if (all_done) break;
   }
   WZ_CUDA(cudaStreamSynchronize(st));
-  WZ_CUDA(cudaMemcpy(&fin, pl->d_state, sizeof(CGState), cudaMemcpyDeviceToHost));
-  info->iterations = fin.iter;
-  info->reliable_updates = fin.n_ru;
-  info->converged = fin.converged;
-  info->rel_residual_recursive = fin.bnorm > 0 ? std::sqrt(fin.rr) / fin.bnorm : 0.0;
-  info->rel_residual_true = fin.bnorm > 0 ? std::sqrt(fin.true_rr < 0 ? 0.0 : fin.true_rr) / fin.bnorm : 0.0;
+  std::vector<CGState> fin(nb);
+  WZ_CUDA(cudaMemcpy(fin.data(), pl->d_state, sizeof(CGState) * nb, cudaMemcpyDeviceToHost));
+  for (int j = 0; j < nb; ++j) {
+    if ((s = flush_x(j)) != WZ_OK) return s;
+    // true residual at exit: complex64 solves that converged carry it from their last
+    // reliable update; everything else recomputes it now
+    if (kRU && fin[j].converged) continue;
+    if (fin[j].bnorm2 == 0.0) continue;
+    if ((s = residual128(j, kRU)) != WZ_OK) return s;  // C64, not converged: fold xs into X first
+  }
+  WZ_CUDA(cudaStreamSynchronize(st));
+  WZ_CUDA(cudaMemcpy(fin.data(), pl->d_state, sizeof(CGState) * nb, cudaMemcpyDeviceToHost));
+  for (int j = 0; j < nb; ++j) {
+    info[j].iterations = fin[j].iter;
+    info[j].reliable_updates = ru_served[j];
+    info[j].converged = fin[j].converged;
+    info[j].rel_residual_recursive = fin[j].bnorm > 0 ? std::sqrt(fin[j].rr) / fin[j].bnorm : 0.0;
+    info[j].rel_residual_true =
+        fin[j].bnorm > 0 ? std::sqrt(fin[j].true_rr < 0 ? 0.0 : fin[j].true_rr) / fin[j].bnorm : 0.0;
+  }
   return WZ_OK;
 }
 
@@ -829,24 +818,23 @@ extern "C" wz_status wz_cg_solve(wz_plan* pl, const void* phi, const void* b, vo
   if (!pl || !phi || !b || !x || !m || !g || !info) return WZ_EINVAL;
   if (!(rho > 0.0 && rho < 2.0) || !(tol > 0.0) || max_iter < 0) return WZ_EINVAL;
   if (nbatch < 0 || nbatch > pl->max_batch) return WZ_EINVAL;
-  const size_t n1 = (size_t)4 * pl->V;
-  bool all = true;
+  if (nbatch == 0) return WZ_OK;
+  wz_status s;
   if (pl->dtype == WZ_C64) {
     const long nphi = 2 * pl->V;
-    k_f2d<<<vec_grid(nphi, 1), CGK_NT, 0, pl->stream>>>((double*)pl->phi128, (const float*)phi, nphi);
-    pl->launches++;
+    {
+      ProfScope ps(pl, WZ_K_OTHER);
+      k_f2d<<<vec_grid(nphi, 1), CGK_NT, 0, pl->stream>>>((double*)pl->phi128, (const float*)phi, nphi);
+    }
     WZ_CUDA(cudaGetLastError());
+    s = cg_batch<float>(pl, (const cpx<float>*)phi, (const cpx<float>*)b, (cpx<double>*)x, m, g, rho, tol,
+                        max_iter, nbatch, info);
+  } else {
+    s = cg_batch<double>(pl, (const cpx<double>*)phi, (const cpx<double>*)b, (cpx<double>*)x, m, g, rho, tol,
+                         max_iter, nbatch, info);
   }
-  for (int j = 0; j < nbatch; ++j) {
-    wz_status s;
-    if (pl->dtype == WZ_C64)
-      s = cg_one<float>(pl, (const cpx<float>*)phi, (const cpx<float>*)b + j * n1,
-                        (cpx<double>*)x + j * n1, m, g, rho, tol, max_iter, &info[j]);
-    else
-      s = cg_one<double>(pl, (const cpx<double>*)phi, (const cpx<double>*)b + j * n1,
-                         (cpx<double>*)x + j * n1, m, g, rho, tol, max_iter, &info[j]);
-    if (s != WZ_OK) return s;
-    all = all && info[j].converged;
-  }
-  return all ? WZ_OK : WZ_ENOTCONVERGED;
+  if (s != WZ_OK) return s;
+  for (int j = 0; j < nbatch; ++j)
+    if (!info[j].converged) return WZ_ENOTCONVERGED;
+  return WZ_OK;
 }

@@ -31,6 +31,12 @@ __device__ __forceinline__ cpx<double> ldg_c(const cpx<double>* p) {
   return {t.x, t.y};
 }
 
+// L2 prefetch hint: no register, no scoreboard; the later load then pays L2 latency
+// instead of HBM latency (the passes are latency-bound on their operand streams).
+__device__ __forceinline__ void prefetch_l2(const void* p) {
+  asm volatile("prefetch.global.L2 [%0];" ::"l"(p));
+}
+
 template <typename R>
 struct P01Args {
   const cpx<R>* in;   // [nf][L0][L1][I]
@@ -47,7 +53,7 @@ struct P01Args {
   cpx<R>* cg_r;       // FWDCG (read), ENDCG (read+write)
   cpx<R>* cg_p;       // FWDCG (read+write), ENDCG (read)
   cpx<R>* cg_x;       // FWDCG (read+write)
-  const CGState* gate;  // if set and the solve is idle, the kernel returns at once
+  const CGState* gate;  // [nbatch]; if set and this source's solve is idle, the CTA returns at once
 };
 
 template <typename R, int L0, int L1, int NSEG, int T0, int T1>
@@ -73,11 +79,10 @@ k_p01(const P01Args<R> a) {
   cpx<R>* sm = reinterpret_cast<cpx<R>*>(smem_raw);
   __shared__ double red_sh[33];
 
-  if (a.gate && !cg_active(a.gate)) return;
-
   const int tid = threadIdx.x;
-  const int f = blockIdx.y;            // field = batch*4 + spin
-  const int comp = f & 3;
+  const int f = blockIdx.y;            // field = source*4 + spin
+  const int comp = f & 3, src = f >> 2;
+  if (a.gate && !cg_active(a.gate + src)) return;
   const long i0 = (long)blockIdx.x * NSEG;
   const long V = (long)L0 * L1 * a.I;
   const cpx<R>* gin = a.in + (long)f * V + i0;
@@ -100,27 +105,48 @@ k_p01(const P01Args<R> a) {
       // p <- r + beta p (PAPER.md:896 CG), all p loads first, r through the
       // read-only path so that nothing waits behind the p stores
       const long fo = (long)f * V + i0;
+      if (actA && (sA * (int)sizeof(cpx<R>)) % 32 == 0) {
+#pragma unroll
+        for (int k = 0; k < NR0; ++k) {
+          const long off = fo + ((long)F0::in_pos(k, jA) * L1 + x1A) * a.I + sA;
+          prefetch_l2(a.cg_r + off);
+          prefetch_l2(a.cg_x + off);
+        }
+      }
 #pragma unroll
       for (int k = 0; k < NR0; ++k) {
         cpx<R> v = {R(0), R(0)};
         if (actA) v = a.cg_p[fo + ((long)F0::in_pos(k, jA) * L1 + x1A) * a.I + sA];
         x[k] = v;
       }
-      const R beta = (R)a.gate->beta, alpha = (R)a.gate->alpha;
+      const R beta = (R)a.gate[src].beta, alpha = (R)a.gate[src].alpha;
+      constexpr int CHF = (NR0 % 8 == 0) ? 8 : 4;
 #pragma unroll
-      for (int k = 0; k < NR0; ++k) {
-        const int x0 = F0::in_pos(k, jA);
-        cpx<R> v = x[k];
-        if (actA) {
-          const long off = fo + ((long)x0 * L1 + x1A) * a.I + sA;
-          const cpx<R> vr = ldg_c(a.cg_r + off);
-          const cpx<R> vx = a.cg_x[off];  // each x element is read, then written, by this thread only
-          a.cg_x[off] = {vx.re + alpha * v.re, vx.im + alpha * v.im};  // pending x += alpha_{k-1} p_{k-1}
-          v = {vr.re + beta * v.re, vr.im + beta * v.im};
-          a.cg_p[off] = v;
+      for (int k0 = 0; k0 < NR0; k0 += CHF) {
+        cpx<R> vr[CHF], vx[CHF];
+        long off[CHF];
+#pragma unroll
+        for (int c = 0; c < CHF; ++c) {
+          off[c] = fo + ((long)F0::in_pos(k0 + c, jA) * L1 + x1A) * a.I + sA;
+          vr[c] = {R(0), R(0)};
+          vx[c] = {R(0), R(0)};
+          if (actA) {
+            vr[c] = ldg_c(a.cg_r + off[c]);
+            vx[c] = a.cg_x[off[c]];  // read, then written, by this thread only
+          }
         }
-        if (a.apbc) v = mul_tw_rt<R, +1>(v, x0 * TWSTEP);
-        x[k] = v;
+#pragma unroll
+        for (int c = 0; c < CHF; ++c) {
+          const int x0 = F0::in_pos(k0 + c, jA);
+          cpx<R> v = x[k0 + c];
+          if (actA) {
+            a.cg_x[off[c]] = {vx[c].re + alpha * v.re, vx[c].im + alpha * v.im};  // pending x += alpha p
+            v = {vr[c].re + beta * v.re, vr[c].im + beta * v.im};
+            a.cg_p[off[c]] = v;
+          }
+          if (a.apbc) v = mul_tw_rt<R, +1>(v, x0 * TWSTEP);
+          x[k0 + c] = v;
+        }
       }
     } else {
 #pragma unroll
@@ -165,6 +191,19 @@ k_p01(const P01Args<R> a) {
         cpx<R> v = {R(0), R(0)};
         if (actB) v = gin[((long)x0B * L1 + G1::in_pos(k, jB)) * a.I + sB];
         y[k] = v;
+      }
+      if constexpr (MODE != P01_INV) {
+        // operands of the site-local step (this thread's axis-0 line), one hint per 32-byte sector
+        if (actA && (sA * (int)sizeof(cpx<R>)) % 32 == 0) {
+          const long fo = (long)f * V + i0;
+#pragma unroll
+          for (int k = 0; k < NR0; ++k) {
+            const long off = ((long)G0::out_pos(k, jA) * L1 + x1A) * a.I + sA;
+            prefetch_l2(a.psi + fo + off);
+            prefetch_l2(a.phi + i0 + off);
+            if constexpr (MODE == P01_ENDCG) prefetch_l2(a.cg_r + fo + off);
+          }
+        }
       }
       G1::run(y, jB);
       if (actB) {
@@ -229,7 +268,7 @@ k_p01(const P01Args<R> a) {
             cpx<R>* gr = a.cg_r + (long)f * V + i0;
 #pragma unroll
             for (int c = 0; c < CH; ++c) vr[c] = gr[off[c]];
-            const R alpha = (R)a.red.st->alpha;
+            const R alpha = (R)a.red.st[src].alpha;
 #pragma unroll
             for (int c = 0; c < CH; ++c) {
               cpx<R> w = {a.op.m_re + a.op.g2_re * ph[c].re - a.op.g2_im * ph[c].im,
@@ -296,9 +335,9 @@ k_p01(const P01Args<R> a) {
             gout[((long)x0B * L1 + F1::out_pos(k, jB)) * a.I + sB] = y[k];
         }
       }
-      if (a.red.partials) {
-        const int blk = blockIdx.y * gridDim.x + blockIdx.x;
-        grid_reduce<FIN>(acc, a.red, blk, gridDim.x * gridDim.y, red_sh);
+      if (a.red.partials) {  // one reduction per source: its 4 spin components x all segments
+        const int blk = comp * gridDim.x + blockIdx.x;
+        grid_reduce<FIN>(acc, a.red.for_source(src), blk, 4 * gridDim.x, red_sh);
       }
     }
   }

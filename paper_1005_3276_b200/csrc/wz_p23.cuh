@@ -27,7 +27,7 @@ struct P23Args {
   const R* tab;       // momentum tables [2][4][64]: sin p_mu(n), sin^2(p_mu(n)/2)
   R rho;
   R sign;             // +1: Dslash, -1: Dslash^dag = -Dslash
-  const CGState* gate;
+  const CGState* gate;  // [nbatch], indexed by blockIdx.y
 };
 
 template <typename R, int L2, int L3, int T2, int T3>
@@ -55,7 +55,7 @@ k_p23(const P23Args<R> a) {
   cpx<R>* sm = reinterpret_cast<cpx<R>*>(smem_raw);
   __shared__ R tb[2 * 4 * 64];
 
-  if (a.gate && !cg_active(a.gate)) return;
+  if (a.gate && !cg_active(a.gate + blockIdx.y)) return;
 
   const int tid = threadIdx.x;
   const int plane = blockIdx.x;
