@@ -44,7 +44,7 @@ struct P01Entry {
 };
 template <typename R>
 struct P23Entry {
-  int L2, L3, nt;
+  int L2, L3, nt, nhalf;  // nhalf = 2: two components per CTA, grid.z = 2, multiply needs in != out
   size_t smem;
   void (*fwd)(const P23Args<R>);
   void (*inv)(const P23Args<R>);
@@ -101,15 +101,15 @@ P01Entry<R> make_p01() {
   e.endcg = make_p01_kern<R, L0, L1, P01_ENDCG, FIN_RR>();
   return e;
 }
-template <typename R, int L2, int L3>
+template <typename R, int L2, int L3, int NC = 4>
 P23Entry<R> make_p23() {
   constexpr int T2 = tune_tpl23<R, L2>::v, T3 = tune_tpl23<R, L3>::v;
-  using C = P23Cfg<R, L2, L3, T2, T3>;
+  using C = P23Cfg<R, L2, L3, T2, T3, NC>;
   P23Entry<R> e;
-  e.L2 = L2; e.L3 = L3; e.nt = C::NT; e.smem = C::SMEM;
-  e.fwd = k_p23<R, L2, L3, T2, T3, P23_FFT, +1>;
-  e.inv = k_p23<R, L2, L3, T2, T3, P23_FFT, -1>;
-  e.mult = k_p23<R, L2, L3, T2, T3, P23_MULT, +1>;
+  e.L2 = L2; e.L3 = L3; e.nt = C::NT; e.smem = C::SMEM; e.nhalf = 4 / NC;
+  e.fwd = k_p23<R, L2, L3, T2, T3, P23_FFT, +1, NC>;
+  e.inv = k_p23<R, L2, L3, T2, T3, P23_FFT, -1, NC>;
+  e.mult = k_p23<R, L2, L3, T2, T3, P23_MULT, +1, NC>;
   return e;
 }
 
@@ -128,8 +128,9 @@ const std::vector<P23Entry<R>>& p23_table() {
         make_p23<R, 4, 4>(),   make_p23<R, 8, 8>(),   make_p23<R, 16, 8>(), make_p23<R, 16, 16>(),
         make_p23<R, 32, 32>(), make_p23<R, 24, 24>(),
     };
-    // four 64x64 complex128 planes (266 KB) exceed one SM's shared memory
+    // four 64x64 complex128 planes (266 KB) exceed one SM's shared memory: two per CTA there
     if constexpr (sizeof(R) == 4) v.push_back(make_p23<R, 64, 64>());
+    else v.push_back(make_p23<R, 64, 64, 2>());
     return v;
   }();
   return t;
@@ -167,6 +168,7 @@ struct OpWS {
   const P23Entry<R>* p23 = nullptr;
   R* tab = nullptr;        // momentum tables [2][4][64]
   cpx<R>* t = nullptr;     // FFT temporary, max_batch spinors
+  cpx<R>* t2 = nullptr;    // second FFT temporary (only where the multiply pass is out of place)
   cpx<R>* chi = nullptr;   // chi = M psi,   max_batch spinors
 };
 
@@ -278,6 +280,7 @@ wz_status setup_ws(wz_plan* pl, OpWS<R>& ws, int nbatch_t) {
   WZ_CUDA(cudaStreamSynchronize(pl->stream));
   const size_t n = (size_t)nbatch_t * 4 * pl->V;
   if (!dev_alloc(pl, &ws.t, n) || !dev_alloc(pl, &ws.chi, n)) return WZ_ENOMEM;
+  if (ws.p23->nhalf == 2 && !dev_alloc(pl, &ws.t2, n)) return WZ_ENOMEM;
   return WZ_OK;
 }
 
@@ -320,6 +323,24 @@ wz_status launch_p01(wz_plan* pl, int kind, const P01Kern<R>& k, const P01Args<R
   return WZ_OK;
 }
 
+// (x2,x3) pass over nb sources
+template <typename R>
+wz_status launch_p23(wz_plan* pl, int kind, const P23Entry<R>& e, void (*k)(const P23Args<R>),
+                     const P23Args<R>& args, int nb) {
+  const dim3 grid((unsigned)(pl->L[0] * pl->L[1]), (unsigned)nb, (unsigned)e.nhalf);
+  return launch<R>(pl, kind, k, grid, e.nt, e.smem, args);
+}
+// Momentum-space multiply pass on the FFT temporary `cur`; in place, or into the other
+// temporary where the kernel works on half the spin components per CTA.  `cur` follows.
+template <typename R>
+wz_status mult_pass(wz_plan* pl, OpWS<R>& ws, P23Args<R>& b, cpx<R>*& cur, int nb) {
+  cpx<R>* dst = (ws.p23->nhalf == 2) ? ((cur == ws.t) ? ws.t2 : ws.t) : cur;
+  b.in = cur; b.out = dst;
+  wz_status s = launch_p23<R>(pl, WZ_K_P23_MULT, *ws.p23, ws.p23->mult, b, nb);
+  cur = dst;
+  return s;
+}
+
 RedArgs red_of(wz_plan* pl) {
   RedArgs r;
   r.partials = pl->partials; r.counter = pl->counter; r.st = pl->d_state; r.store = nullptr;
@@ -347,7 +368,6 @@ OpParams<R> make_op(const double m[2], const double g[2], double rho, int dagger
 template <typename R>
 wz_status fft4d_impl(wz_plan* pl, int direction, int apbc, const cpx<R>* in, cpx<R>* out, int nb) {
   OpWS<R>& ws = ws_of<R>(pl);
-  const dim3 g23((unsigned)(pl->L[0] * pl->L[1]), (unsigned)nb);
   P01Args<R> a{};
   a.I = pl->I; a.apbc = apbc; a.scale = R(1);
   P23Args<R> b{};
@@ -358,10 +378,10 @@ wz_status fft4d_impl(wz_plan* pl, int direction, int apbc, const cpx<R>* in, cpx
     wz_status s = launch_p01<R>(pl, WZ_K_P01_FWD, ws.p01->fwd, a, nb);
     if (s != WZ_OK) return s;
     b.in = out; b.out = out;
-    return launch<R>(pl, WZ_K_P23_FFT, ws.p23->fwd, g23, ws.p23->nt, ws.p23->smem, b);
+    return launch_p23<R>(pl, WZ_K_P23_FFT, *ws.p23, ws.p23->fwd, b, nb);
   }
   b.in = in; b.out = out;
-  wz_status s = launch<R>(pl, WZ_K_P23_FFT, ws.p23->inv, g23, ws.p23->nt, ws.p23->smem, b);
+  wz_status s = launch_p23<R>(pl, WZ_K_P23_FFT, *ws.p23, ws.p23->inv, b, nb);
   if (s != WZ_OK) return s;
   a.in = out; a.out = out; a.scale = (R)(1.0 / (double)pl->V);
   return launch_p01<R>(pl, WZ_K_P01_INV, ws.p01->inv, a, nb);
@@ -372,18 +392,17 @@ template <typename R>
 wz_status apply_M_impl(wz_plan* pl, int dagger, const cpx<R>* phi, const double m[2], const double g[2],
                        double rho, const cpx<R>* in, cpx<R>* out, int nb) {
   OpWS<R>& ws = ws_of<R>(pl);
-  const dim3 g23((unsigned)(pl->L[0] * pl->L[1]), (unsigned)nb);
   P01Args<R> a{};
   a.I = pl->I; a.apbc = 1; a.scale = R(1);
   a.in = in; a.out = ws.t;
   wz_status s = launch_p01<R>(pl, WZ_K_P01_FWD, ws.p01->fwd, a, nb);
   if (s != WZ_OK) return s;
   P23Args<R> b{};
-  b.in = ws.t; b.out = ws.t; b.nplanes = pl->L[0] * pl->L[1]; b.L1 = pl->L[1]; b.scale = R(1);
+  b.nplanes = pl->L[0] * pl->L[1]; b.L1 = pl->L[1]; b.scale = R(1);
   b.tab = ws.tab; b.rho = (R)rho; b.sign = dagger ? R(-1) : R(1);
-  s = launch<R>(pl, WZ_K_P23_MULT, ws.p23->mult, g23, ws.p23->nt, ws.p23->smem, b);
-  if (s != WZ_OK) return s;
-  a.in = ws.t; a.out = ws.t; a.scale = (R)(1.0 / (double)pl->V);
+  cpx<R>* cur = ws.t;
+  if ((s = mult_pass<R>(pl, ws, b, cur, nb)) != WZ_OK) return s;
+  a.in = cur; a.out = cur; a.scale = (R)(1.0 / (double)pl->V);
   a.psi = in; a.phi = phi; a.site_out = out; a.op = make_op<R>(m, g, rho, dagger);
   return launch_p01<R>(pl, WZ_K_P01_END, ws.p01->end, a, nb);
 }
@@ -394,7 +413,6 @@ template <typename R>
 wz_status apply_MdagM_impl(wz_plan* pl, const cpx<R>* phi, const double m[2], const double g[2],
                            double rho, const cpx<R>* in, cpx<R>* out, int nb, bool cg) {
   OpWS<R>& ws = ws_of<R>(pl);
-  const dim3 g23((unsigned)(pl->L[0] * pl->L[1]), (unsigned)nb);
   const CGState* gate = cg ? pl->d_state : nullptr;
   const R invV = (R)(1.0 / (double)pl->V);
   wz_status s;
@@ -403,10 +421,11 @@ wz_status apply_MdagM_impl(wz_plan* pl, const cpx<R>* phi, const double m[2], co
   a.in = in; a.out = ws.t;
   if ((s = launch_p01<R>(pl, WZ_K_P01_FWD, ws.p01->fwd, a, nb)) != WZ_OK) return s;  // A
   P23Args<R> b{};
-  b.in = ws.t; b.out = ws.t; b.nplanes = pl->L[0] * pl->L[1]; b.L1 = pl->L[1]; b.scale = R(1);
+  b.nplanes = pl->L[0] * pl->L[1]; b.L1 = pl->L[1]; b.scale = R(1);
   b.tab = ws.tab; b.rho = (R)rho; b.sign = R(1); b.gate = gate;
-  if ((s = launch<R>(pl, WZ_K_P23_MULT, ws.p23->mult, g23, ws.p23->nt, ws.p23->smem, b)) != WZ_OK) return s;  // B
-  a.in = ws.t; a.out = ws.t; a.scale = invV;
+  cpx<R>* cur = ws.t;
+  if ((s = mult_pass<R>(pl, ws, b, cur, nb)) != WZ_OK) return s;  // B
+  a.in = cur; a.out = cur; a.scale = invV;
   a.psi = in; a.phi = phi; a.site_out = ws.chi; a.op = make_op<R>(m, g, rho, 0);
   if (cg) {
     a.red = red_of(pl);
@@ -417,7 +436,8 @@ wz_status apply_MdagM_impl(wz_plan* pl, const cpx<R>* phi, const double m[2], co
   }
   if (s != WZ_OK) return s;
   b.sign = R(-1);
-  if ((s = launch<R>(pl, WZ_K_P23_MULT, ws.p23->mult, g23, ws.p23->nt, ws.p23->smem, b)) != WZ_OK) return s;  // D
+  if ((s = mult_pass<R>(pl, ws, b, cur, nb)) != WZ_OK) return s;  // D
+  a.in = cur; a.out = cur;
   a.red = RedArgs{};
   a.psi = ws.chi; a.site_out = out; a.op = make_op<R>(m, g, rho, 1);
   return launch_p01<R>(pl, WZ_K_P01_END, ws.p01->end, a, nb);  // E
@@ -432,7 +452,6 @@ template <typename R>
 wz_status cg_iteration(wz_plan* pl, const cpx<R>* phi, const double m[2], const double g[2], double rho,
                        cpx<R>* r, cpx<R>* p, cpx<R>* x, int nb) {
   OpWS<R>& ws = ws_of<R>(pl);
-  const dim3 g23((unsigned)(pl->L[0] * pl->L[1]), (unsigned)nb);
   if ((int)(pl->I / ws.p01->nseg()) * 4 > pl->npartials) return WZ_EINVAL;
   const R invV = (R)(1.0 / (double)pl->V);
   wz_status s;
@@ -441,15 +460,17 @@ wz_status cg_iteration(wz_plan* pl, const cpx<R>* phi, const double m[2], const 
   a.in = p; a.out = ws.t; a.cg_r = r; a.cg_p = p; a.cg_x = x;
   if ((s = launch_p01<R>(pl, WZ_K_P01_FWDCG, ws.p01->fwdcg, a, nb)) != WZ_OK) return s;
   P23Args<R> b{};
-  b.in = ws.t; b.out = ws.t; b.nplanes = pl->L[0] * pl->L[1]; b.L1 = pl->L[1]; b.scale = R(1);
+  b.nplanes = pl->L[0] * pl->L[1]; b.L1 = pl->L[1]; b.scale = R(1);
   b.tab = ws.tab; b.rho = (R)rho; b.sign = R(1); b.gate = pl->d_state;
-  if ((s = launch<R>(pl, WZ_K_P23_MULT, ws.p23->mult, g23, ws.p23->nt, ws.p23->smem, b)) != WZ_OK) return s;
-  a.in = ws.t; a.out = ws.t; a.scale = invV;
+  cpx<R>* cur = ws.t;
+  if ((s = mult_pass<R>(pl, ws, b, cur, nb)) != WZ_OK) return s;
+  a.in = cur; a.out = cur; a.scale = invV;
   a.psi = p; a.phi = phi; a.site_out = ws.chi; a.op = make_op<R>(m, g, rho, 0);
   a.red = red_of(pl);
   if ((s = launch_p01<R>(pl, WZ_K_P01_MID, ws.p01->mid_pq, a, nb)) != WZ_OK) return s;
   b.sign = R(-1);
-  if ((s = launch<R>(pl, WZ_K_P23_MULT, ws.p23->mult, g23, ws.p23->nt, ws.p23->smem, b)) != WZ_OK) return s;
+  if ((s = mult_pass<R>(pl, ws, b, cur, nb)) != WZ_OK) return s;
+  a.in = cur; a.out = cur;
   a.psi = ws.chi; a.site_out = nullptr; a.op = make_op<R>(m, g, rho, 1);
   a.cg_r = r; a.cg_p = p; a.cg_x = x;
   return launch_p01<R>(pl, WZ_K_P01_ENDCG, ws.p01->endcg, a, nb);

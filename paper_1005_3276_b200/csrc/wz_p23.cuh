@@ -30,7 +30,11 @@ struct P23Args {
   const CGState* gate;  // [nbatch], indexed by blockIdx.y
 };
 
-template <typename R, int L2, int L3, int T2, int T3>
+// NC = spin components per CTA: 4 (whole plane quad, in place), or 2 when four planes
+// do not fit in shared memory (64x64 complex128).  With NC = 2 the CTA with
+// blockIdx.z = h reads components (2,3) [h = 0] or (0,1) [h = 1] and, for the multiply,
+// writes the OTHER pair -- so in != out is required there (ping-pong buffers).
+template <typename R, int L2, int L3, int T2, int T3, int NC = 4>
 struct P23Cfg {
   static constexpr int TPL2 = T2, TPL3 = T3;  // lanes per line along axis 2 / axis 3
   static constexpr int NR2 = L2 / TPL2, NR3 = L3 / TPL3;
@@ -38,16 +42,16 @@ struct P23Cfg {
   static constexpr int NTC_B = L2 * TPL3;  // lines along axis 3
   static constexpr int NTC_RAW = NTC_A > NTC_B ? NTC_A : NTC_B;
   static constexpr int NTC = (NTC_RAW + 31) / 32 * 32;  // whole warps per spin component
-  static constexpr int NT = 4 * NTC;
+  static constexpr int NT = NC * NTC;
   static constexpr int PITCH = L3 + 1;            // row pitch (elements)
   static constexpr int CPITCH = L2 * PITCH + 4;   // component pitch
-  static constexpr size_t SMEM = sizeof(cpx<R>) * 4 * (size_t)CPITCH;
+  static constexpr size_t SMEM = sizeof(cpx<R>) * NC * (size_t)CPITCH;
 };
 
-template <typename R, int L2, int L3, int T2, int T3, int MODE, int DIR>
-__global__ void __launch_bounds__(P23Cfg<R, L2, L3, T2, T3>::NT)
+template <typename R, int L2, int L3, int T2, int T3, int MODE, int DIR, int NC = 4>
+__global__ void __launch_bounds__(P23Cfg<R, L2, L3, T2, T3, NC>::NT)
 k_p23(const P23Args<R> a) {
-  using Cfg = P23Cfg<R, L2, L3, T2, T3>;
+  using Cfg = P23Cfg<R, L2, L3, T2, T3, NC>;
   constexpr int TPL2 = Cfg::TPL2, TPL3 = Cfg::TPL3, NR2 = Cfg::NR2, NR3 = Cfg::NR3;
   constexpr int NTC = Cfg::NTC, PITCH = Cfg::PITCH, CPITCH = Cfg::CPITCH;
   constexpr int D1 = (MODE == P23_MULT) ? +1 : DIR;  // direction of the first half
@@ -66,17 +70,21 @@ k_p23(const P23Args<R> a) {
     for (int i = tid; i < 2 * 4 * 64; i += blockDim.x) tb[i] = a.tab[i];
   }
 
-  const int cc = tid / NTC;     // spin component (NTC is a multiple of 32)
+  const int cl = tid / NTC;     // component slot in this CTA (NTC is a multiple of 32)
   const int tc = tid % NTC;
+  // global spin component read (cin) and written (cc) by this thread
+  const int half = (NC == 4) ? 0 : (int)blockIdx.z;
+  const int cin = (NC == 4) ? cl : ((MODE == P23_MULT) ? (half ? cl : 2 + cl) : 2 * half + cl);
+  const int cc = (NC == 4) ? cl : ((MODE == P23_MULT) ? (half ? 2 + cl : cl) : 2 * half + cl);
   // role A: line along axis 2 at x3;  role B: line along axis 3 at n2
   int x3A, jA, n2B, jB;
   lane_split<TPL2>(tc, x3A, jA);
   lane_split<TPL3>(tc, n2B, jB);
   const bool actA = x3A < L3;
   const bool actB = n2B < L2;
-  const cpx<R>* gin = a.in + (fbase + (long)cc * a.nplanes + plane) * PL;
+  const cpx<R>* gin = a.in + (fbase + (long)cin * a.nplanes + plane) * PL;
   cpx<R>* gout = a.out + (fbase + (long)cc * a.nplanes + plane) * PL;
-  cpx<R>* smc = sm + cc * CPITCH;
+  cpx<R>* smc = sm + cl * CPITCH;
 
   // ---- half 1, axis 2 (lanes run along x3: coalesced HBM reads) ----
   {
@@ -116,11 +124,12 @@ k_p23(const P23Args<R> a) {
 
   if constexpr (MODE == P23_FFT) {
     // coalesced copy-out of the four planes
-    for (int i = tid; i < 4 * L2 * L3; i += blockDim.x) {
+    for (int i = tid; i < NC * L2 * L3; i += blockDim.x) {
       const int ci = i / (L2 * L3), r = i % (L2 * L3);
       const int n2 = r / L3, n3 = r % L3;
       cpx<R> v = sm[ci * CPITCH + n2 * PITCH + n3];
-      a.out[(fbase + (long)ci * a.nplanes + plane) * PL + r] = cscale(v, a.scale);
+      const int cg = (NC == 4) ? ci : 2 * half + ci;
+      a.out[(fbase + (long)cg * a.nplanes + plane) * PL + r] = cscale(v, a.scale);
     }
   } else {
     // ---- momentum-diagonal multiply, then inverse axis 3 ----
@@ -141,7 +150,9 @@ k_p23(const P23Args<R> a) {
       else if (cc == 1) { A0 = -s2; A1 = s1;   A3 = R(0);  B0 = s0;  B1 = R(0); B3 = R(-1); }
       else if (cc == 2) { A0 = s0;  A1 = R(0); A3 = R(-1); B0 = -s2; B1 = -s1;  B3 = R(0); }
       else              { A0 = s2;  A1 = -s1;  A3 = R(0);  B0 = s0;  B1 = R(0); B3 = R(1); }
-      const cpx<R>* sa = sm + ((cc < 2) ? 2 : 0) * CPITCH + n2 * PITCH;
+      // inputs of output component cc: (psi_2, psi_3) for cc < 2, (psi_0, psi_1) otherwise;
+      // with NC = 2 those are the two planes this CTA holds
+      const cpx<R>* sa = sm + ((NC == 4) ? ((cc < 2) ? 2 : 0) : 0) * CPITCH + n2 * PITCH;
       const cpx<R>* sb = sa + CPITCH;
       const R two_rho_sign = R(2) * a.rho * a.sign;
 #pragma unroll

@@ -222,3 +222,62 @@ def test_fft_constant_phi_closed_form(wz, inp):
     w = m + 2 * g * np.complex128(np.complex64(phi0))
     ref = (d2 + abs(w) ** 2)[None] * fb
     assert rel(fq, ref) <= 2e-5
+
+
+# ---- full-size checks (BASELINE.json configs 4 and 5), in the launch configuration bench.py times ----
+
+@pytest.mark.parametrize("dims,dtype", [((32, 32, 32, 32), "c64"), ((32, 32, 32, 32), "c128"),
+                                        ((64, 64, 64, 64), "c64"), ((64, 64, 64, 64), "c128")])
+def test_full_size_MdagM_vs_oracle(wz, orc, inp, dims, dtype):
+    """One M^dag M at 32^4 / 64^4 against the oracle (radix-2 route), element by element."""
+    if not wz.supported(dims, dtype):
+        pytest.fail("configs 4 and 5b must be supported")
+    cfg = inp.CONFIGS[4 if dims[0] == 32 else "5b"]
+    phi = inp.make_phi(cfg["seed"], dims, cfg["sigma"], NPDT[dtype])
+    b = inp.make_source(cfg["seed"], 0, dims, NPDT[dtype])
+    plan = wz.Plan(dims, dtype, 1)
+    out = plan.apply_MdagM(torch.from_numpy(phi).cuda(), torch.from_numpy(b).cuda(), cfg["m"], cfg["g"], cfg["rho"])
+    out = out.cpu().numpy()
+    del plan
+    ref = orc.apply_MdagM(phi.astype(np.complex128), b.astype(np.complex128), cfg["m"], cfg["g"], cfg["rho"])
+    assert rel(out, ref) <= TOL[dtype]
+
+
+def test_config4_batched_solve_true_residual(wz, orc, inp):
+    """Config 4 as bench.py runs it: 12 sources in lock step to 1e-6.  Every source must
+    converge; for a sample of sources the ORACLE recomputes the true residual of the GPU's x."""
+    cfg = inp.CONFIGS[4]
+    dims, nsrc = cfg["dims"], cfg["nsrc"]
+    phi = inp.make_phi(cfg["seed"], dims, cfg["sigma"], np.complex64)
+    b = inp.make_sources(cfg["seed"], nsrc, dims, np.complex64)
+    plan = wz.Plan(dims, "c64", nsrc)
+    x, infos = plan.cg_solve(torch.from_numpy(phi).cuda(), torch.from_numpy(b).cuda(), cfg["m"], cfg["g"],
+                             cfg["rho"], cfg["tol"], 100000)
+    assert all(i.converged for i in infos)
+    assert all(i.rel_residual_true <= cfg["tol"] for i in infos)
+    its = [i.iterations for i in infos]
+    print("config 4 iterations per source:", its, "reliable updates:", [i.reliable_updates for i in infos])
+    assert max(its) < 1.2 * min(its)  # same operator, same spectrum: counts differ by a few per cent
+    phi128 = phi.astype(np.complex128)
+    for j in (0, nsrc - 1):
+        xj = x[j].cpu().numpy()
+        res = rel(orc.apply_MdagM(phi128, xj, cfg["m"], cfg["g"], cfg["rho"]), b[j].astype(np.complex128))
+        assert res <= cfg["tol"], (j, res)
+        assert abs(res - infos[j].rel_residual_true) <= 0.02 * cfg["tol"]
+
+
+def test_batched_solve_equals_single_solves(wz, inp):
+    """Lock-step batching does not couple the sources: same iteration counts and the same x,
+    bit for bit, as solving each source alone (fixed-order reductions per source)."""
+    cfg = inp.CONFIGS[3]
+    dims = cfg["dims"]
+    phi = torch.from_numpy(inp.make_phi(cfg["seed"], dims, cfg["sigma"], np.complex64)).cuda()
+    b = torch.from_numpy(inp.make_sources(cfg["seed"], 3, dims, np.complex64)).cuda()
+    plan = wz.Plan(dims, "c64", 3)
+    xb, ib = plan.cg_solve(phi, b, cfg["m"], cfg["g"], cfg["rho"], cfg["tol"], 400, raise_on_fail=False)
+    for j in range(3):
+        xs, i1 = plan.cg_solve(phi, b[j:j + 1].contiguous(), cfg["m"], cfg["g"], cfg["rho"], cfg["tol"], 400,
+                               raise_on_fail=False)
+        assert i1[0].iterations == ib[j].iterations == 400
+        assert i1[0].reliable_updates == ib[j].reliable_updates
+        assert torch.equal(xs[0], xb[j])
