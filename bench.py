@@ -164,6 +164,28 @@ ALGO_U = {"p01_fwd": 2.0, "p23_mult": 2.0, "p01_mid": 4.25, "p01_end": 3.25, "p2
           "p01_fwdcg": 6.0, "p01_endcg": 4.25}
 
 
+def rank_sources(rank: int, nsrc: int):
+    """Source ids (generator streams 1 + id) of rank `rank`: every rank solves its own nsrc
+    sources, disjoint across ranks, phi replicated (replicas only, no data-path collective)."""
+    return list(range(rank * nsrc, (rank + 1) * nsrc))
+
+
+def reduce_over_ranks(secs: float, counts, device=None):
+    """Job time = MAX over ranks of the device-timed seconds; counts (iterations, launches, ...)
+    = SUM over ranks.  Works with any initialised torch.distributed backend (NCCL on the GPUs,
+    gloo in the CPU tests); single process: identity."""
+    import torch
+    import torch.distributed as dist
+
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return secs, list(counts)
+    t = torch.tensor([secs], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    c = torch.tensor(list(counts), dtype=torch.float64, device=device)
+    dist.all_reduce(c, op=dist.ReduceOp.SUM)
+    return float(t.item()), [int(round(v)) for v in c.tolist()]
+
+
 def load_traffic():
     p = os.path.join(ROOT, "profiles", "traffic.json")
     if os.path.exists(p):
@@ -195,8 +217,8 @@ def run_wz(args):
     m, g, rho, tol = cfg["m"], cfg["g"], cfg["rho"], cfg["tol"]
     # host inputs (pinned); rank r takes sources r*nsrc .. (r+1)*nsrc-1, phi replicated
     h_phi = torch.from_numpy(inputs.make_phi(cfg["seed"], dims, cfg["sigma"], npdt)).pin_memory()
-    h_b = torch.from_numpy(np.stack([inputs.make_source(cfg["seed"], rank * nsrc + j, dims, npdt)
-                                     for j in range(nsrc)])).pin_memory()
+    h_b = torch.from_numpy(np.stack([inputs.make_source(cfg["seed"], j, dims, npdt)
+                                     for j in rank_sources(rank, nsrc)])).pin_memory()
     d_phi, d_b = h_phi.to(dev), h_b.to(dev)
     d_x = torch.empty(h_b.shape, dtype=torch.complex128, device=dev)
     h_x = torch.empty(h_b.shape, dtype=torch.complex128).pin_memory()
@@ -231,13 +253,7 @@ def run_wz(args):
     secs = e0.elapsed_time(e1) * 1e-3
     conv = all(i.converged for i in infos)
     worst_true = max(i.rel_residual_true for i in infos)
-    if world > 1:
-        t = torch.tensor([secs], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        secs = float(t.item())
-        c = torch.tensor([iters, launches], device=dev, dtype=torch.float64)
-        dist.all_reduce(c, op=dist.ReduceOp.SUM)
-        iters, launches = int(c[0].item()), int(c[1].item())
+    secs, (iters, launches) = reduce_over_ranks(secs, [iters, launches], dev)
     value = iters / secs
 
     # ---- end to end through the public API with HOST buffers (pinned), every step ----
@@ -253,13 +269,7 @@ def run_wz(args):
     barrier()
     e_secs = t0.elapsed_time(t1) * 1e-3
     e_iters = sum(i.iterations for i in infos_e)
-    if world > 1:
-        t = torch.tensor([e_secs], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e_secs = float(t.item())
-        c = torch.tensor([e_iters], device=dev, dtype=torch.float64)
-        dist.all_reduce(c, op=dist.ReduceOp.SUM)
-        e_iters = int(c.item())
+    e_secs, (e_iters,) = reduce_over_ranks(e_secs, [e_iters], dev)
     e2e = {"value": e_iters / e_secs, "unit": UNIT,
            "h2d_bytes_per_step": int(h_phi.numel() * h_phi.element_size() + h_b.numel() * h_b.element_size()),
            "d2h_bytes_per_step": int(h_x.numel() * h_x.element_size())}
@@ -316,7 +326,7 @@ def run_wz(args):
         "config": {"workload": "config %s: %s lattice, %s, %d Gaussian sources per GPU to tol %g, m=%g g=%g rho=%g, seed %d"
                    % (key, "x".join(map(str, dims)), cfg["dtype"], nsrc, tol, m, g, rho, cfg["seed"]),
                    "l2": "no flush: working set of one solve (8 vectors, %.0f MB) exceeds the 126 MB L2" % (8.25 * u / 1e6),
-                   "sources": "independent, solved one after another; sharded across ranks, phi replicated"},
+                   "sources": "independent, advanced in lock step through shared launches; sharded across ranks, phi replicated"},
         "max_iter": args.max_iter, "valid": bool(conv),
         "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
         "cpu_baseline": cpu, "extras": extras,
