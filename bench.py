@@ -283,10 +283,16 @@ def run_wz(args):
     peak, peak_src = measured_peaks()
     plan.profile(True)
     # the same batched solve as the timed steps, first iterations only (all sources active)
-    plan.cg_solve(d_phi, d_b, m, g, rho, tol, min(400, args.max_iter), out=d_x, raise_on_fail=False)
+    _, pinfo = plan.cg_solve(d_phi, d_b, m, g, rho, tol, min(400, args.max_iter), out=d_x, raise_on_fail=False)
     prof = plan.profile_read()
     plan.profile(False)
-    kinds = {k: {"us": 1e3 * ms / n, "launches": n, "share": 0.0} for k, (ms, n) in prof.items() if k in ALGO_U}
+    # mean duration of an ACTIVE launch: the solve also enqueues a few idle launches (chunks already
+    # in flight when the last source stops; ~3 us each, they return at once), so divide the summed
+    # time by the launches that did work = iterations x launches per iteration of that kind
+    piters = max(i.iterations for i in pinfo)
+    per_iter = {"p23_mult": 2}
+    kinds = {k: {"us": 1e3 * ms / (piters * per_iter.get(k, 1)), "launches": piters * per_iter.get(k, 1), "share": 0.0}
+             for k, (ms, n) in prof.items() if k in ("p01_fwdcg", "p23_mult", "p01_mid", "p01_endcg")}
     tot = sum(v["us"] * v["launches"] for v in kinds.values()) or 1.0
     for k, v in kinds.items():
         v["share"] = v["us"] * v["launches"] / tot

@@ -39,6 +39,7 @@ struct P01Kern {
 template <typename R>
 struct P01Entry {
   int L0, L1;
+  long I;  // (x2,x3) volume the kernels were specialised for; 0 = any (run-time)
   P01Kern<R> fwd, inv, mid, mid_pq, end, fwdcg, endcg;
   int nseg() const { return fwd.nseg; }
 };
@@ -59,7 +60,7 @@ struct P23Entry {
 #define WZ_TPL32F 2
 #endif
 #ifndef WZ_TPL32F_P23
-#define WZ_TPL32F_P23 2
+#define WZ_TPL32F_P23 1
 #endif
 #ifndef WZ_NSEG32F
 #define WZ_NSEG32F 4
@@ -79,26 +80,26 @@ template <typename R, int L0, int L1> struct tune_nseg {
                                             : (L0 * L1 > 2048 ? 2 : 4);
 };
 
-template <typename R, int L0, int L1, int MODE, int FIN>
+template <typename R, int L0, int L1, int MODE, int FIN, int IC>
 P01Kern<R> make_p01_kern() {
   constexpr int NSEG = tune_nseg<R, L0, L1>::v, T0 = tune_tpl<R, L0>::v, T1 = tune_tpl<R, L1>::v;
   using C = P01Cfg<R, L0, L1, NSEG, T0, T1>;
   P01Kern<R> k;
-  k.fn = k_p01<R, L0, L1, NSEG, T0, T1, MODE, FIN>;
+  k.fn = k_p01<R, L0, L1, NSEG, T0, T1, MODE, FIN, IC>;
   k.nt = C::NT; k.nseg = NSEG; k.smem = C::SMEM;
   return k;
 }
-template <typename R, int L0, int L1>
+template <typename R, int L0, int L1, int IC = 0>
 P01Entry<R> make_p01() {
   P01Entry<R> e;
-  e.L0 = L0; e.L1 = L1;
-  e.fwd = make_p01_kern<R, L0, L1, P01_FWD, FIN_STORE>();
-  e.inv = make_p01_kern<R, L0, L1, P01_INV, FIN_STORE>();
-  e.mid = make_p01_kern<R, L0, L1, P01_MID, FIN_STORE>();
-  e.mid_pq = make_p01_kern<R, L0, L1, P01_MID, FIN_PQ>();
-  e.end = make_p01_kern<R, L0, L1, P01_END, FIN_STORE>();
-  e.fwdcg = make_p01_kern<R, L0, L1, P01_FWDCG, FIN_STORE>();
-  e.endcg = make_p01_kern<R, L0, L1, P01_ENDCG, FIN_RR>();
+  e.L0 = L0; e.L1 = L1; e.I = IC;
+  e.fwd = make_p01_kern<R, L0, L1, P01_FWD, FIN_STORE, IC>();
+  e.inv = make_p01_kern<R, L0, L1, P01_INV, FIN_STORE, IC>();
+  e.mid = make_p01_kern<R, L0, L1, P01_MID, FIN_STORE, IC>();
+  e.mid_pq = make_p01_kern<R, L0, L1, P01_MID, FIN_PQ, IC>();
+  e.end = make_p01_kern<R, L0, L1, P01_END, FIN_STORE, IC>();
+  e.fwdcg = make_p01_kern<R, L0, L1, P01_FWDCG, FIN_STORE, IC>();
+  e.endcg = make_p01_kern<R, L0, L1, P01_ENDCG, FIN_RR, IC>();
   return e;
 }
 template <typename R, int L2, int L3, int NC = 4>
@@ -116,6 +117,9 @@ P23Entry<R> make_p23() {
 template <typename R>
 const std::vector<P01Entry<R>>& p01_table() {
   static const std::vector<P01Entry<R>> t = {
+      // specialised for the (x2,x3) volume of the benchmark lattices (32^4, 48x24^3, 64^4) ...
+      make_p01<R, 32, 32, 1024>(), make_p01<R, 48, 24, 576>(), make_p01<R, 64, 64, 4096>(),
+      // ... and generic in it
       make_p01<R, 4, 4>(),   make_p01<R, 8, 8>(),   make_p01<R, 8, 4>(),   make_p01<R, 16, 16>(),
       make_p01<R, 32, 32>(), make_p01<R, 48, 24>(), make_p01<R, 64, 64>(),
   };
@@ -136,9 +140,9 @@ const std::vector<P23Entry<R>>& p23_table() {
   return t;
 }
 template <typename R>
-const P01Entry<R>* find_p01(int L0, int L1) {
-  for (const auto& e : p01_table<R>())
-    if (e.L0 == L0 && e.L1 == L1) return &e;
+const P01Entry<R>* find_p01(int L0, int L1, long I) {
+  for (const auto& e : p01_table<R>())  // specialised entries come first
+    if (e.L0 == L0 && e.L1 == L1 && (e.I == 0 || e.I == I)) return &e;
   return nullptr;
 }
 template <typename R>
@@ -255,7 +259,7 @@ bool dev_alloc(wz_plan* pl, T** ptr, size_t count) {
 // computed in double on the host: tab[0][mu][n] = sin p_mu, tab[1][mu][n] = sin^2(p_mu/2).
 template <typename R>
 wz_status setup_ws(wz_plan* pl, OpWS<R>& ws, int nbatch_t) {
-  ws.p01 = find_p01<R>(pl->L[0], pl->L[1]);
+  ws.p01 = find_p01<R>(pl->L[0], pl->L[1], pl->I);
   ws.p23 = find_p23<R>(pl->L[2], pl->L[3]);
   if (!ws.p01 || !ws.p23) return WZ_EUNSUPPORTED;
   if (pl->I % ws.p01->nseg()) return WZ_EUNSUPPORTED;
@@ -398,11 +402,11 @@ wz_status apply_M_impl(wz_plan* pl, int dagger, const cpx<R>* phi, const double 
   wz_status s = launch_p01<R>(pl, WZ_K_P01_FWD, ws.p01->fwd, a, nb);
   if (s != WZ_OK) return s;
   P23Args<R> b{};
-  b.nplanes = pl->L[0] * pl->L[1]; b.L1 = pl->L[1]; b.scale = R(1);
+  b.nplanes = pl->L[0] * pl->L[1]; b.L1 = pl->L[1]; b.scale = (R)(1.0 / (double)pl->V);
   b.tab = ws.tab; b.rho = (R)rho; b.sign = dagger ? R(-1) : R(1);
   cpx<R>* cur = ws.t;
   if ((s = mult_pass<R>(pl, ws, b, cur, nb)) != WZ_OK) return s;
-  a.in = cur; a.out = cur; a.scale = (R)(1.0 / (double)pl->V);
+  a.in = cur; a.out = cur;
   a.psi = in; a.phi = phi; a.site_out = out; a.op = make_op<R>(m, g, rho, dagger);
   return launch_p01<R>(pl, WZ_K_P01_END, ws.p01->end, a, nb);
 }
@@ -421,11 +425,11 @@ wz_status apply_MdagM_impl(wz_plan* pl, const cpx<R>* phi, const double m[2], co
   a.in = in; a.out = ws.t;
   if ((s = launch_p01<R>(pl, WZ_K_P01_FWD, ws.p01->fwd, a, nb)) != WZ_OK) return s;  // A
   P23Args<R> b{};
-  b.nplanes = pl->L[0] * pl->L[1]; b.L1 = pl->L[1]; b.scale = R(1);
+  b.nplanes = pl->L[0] * pl->L[1]; b.L1 = pl->L[1]; b.scale = invV;
   b.tab = ws.tab; b.rho = (R)rho; b.sign = R(1); b.gate = gate;
   cpx<R>* cur = ws.t;
   if ((s = mult_pass<R>(pl, ws, b, cur, nb)) != WZ_OK) return s;  // B
-  a.in = cur; a.out = cur; a.scale = invV;
+  a.in = cur; a.out = cur;
   a.psi = in; a.phi = phi; a.site_out = ws.chi; a.op = make_op<R>(m, g, rho, 0);
   if (cg) {
     a.red = red_of(pl);
@@ -460,11 +464,11 @@ wz_status cg_iteration(wz_plan* pl, const cpx<R>* phi, const double m[2], const 
   a.in = p; a.out = ws.t; a.cg_r = r; a.cg_p = p; a.cg_x = x;
   if ((s = launch_p01<R>(pl, WZ_K_P01_FWDCG, ws.p01->fwdcg, a, nb)) != WZ_OK) return s;
   P23Args<R> b{};
-  b.nplanes = pl->L[0] * pl->L[1]; b.L1 = pl->L[1]; b.scale = R(1);
+  b.nplanes = pl->L[0] * pl->L[1]; b.L1 = pl->L[1]; b.scale = invV;
   b.tab = ws.tab; b.rho = (R)rho; b.sign = R(1); b.gate = pl->d_state;
   cpx<R>* cur = ws.t;
   if ((s = mult_pass<R>(pl, ws, b, cur, nb)) != WZ_OK) return s;
-  a.in = cur; a.out = cur; a.scale = invV;
+  a.in = cur; a.out = cur;
   a.psi = p; a.phi = phi; a.site_out = ws.chi; a.op = make_op<R>(m, g, rho, 0);
   a.red = red_of(pl);
   if ((s = launch_p01<R>(pl, WZ_K_P01_MID, ws.p01->mid_pq, a, nb)) != WZ_OK) return s;
@@ -499,11 +503,11 @@ int wz_supported(int T, int L1, int L2, int L3, wz_dtype dtype) {
   if (T < 2 || (T & 1)) return 0;
   const long I = (long)L2 * L3;
   // every plan needs the complex128 operator (reliable updates, true residual)
-  const auto* ad = find_p01<double>(T, L1);
+  const auto* ad = find_p01<double>(T, L1, I);
   const auto* bd = find_p23<double>(L2, L3);
   if (!ad || !bd || I % ad->nseg()) return 0;
   if (dtype == WZ_C64) {
-    const auto* af = find_p01<float>(T, L1);
+    const auto* af = find_p01<float>(T, L1, I);
     const auto* bf = find_p23<float>(L2, L3);
     if (!af || !bf || I % af->nseg()) return 0;
   }

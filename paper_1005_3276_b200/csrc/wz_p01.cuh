@@ -68,8 +68,20 @@ struct P01Cfg {
   static constexpr size_t SMEM = sizeof(cpx<R>) * (size_t)L0 * PITCH0;
 };
 
-template <typename R, int L0, int L1, int NSEG, int T0, int T1, int MODE, int FIN>
-__global__ void __launch_bounds__(P01Cfg<R, L0, L1, NSEG, T0, T1>::NT)
+// Resident CTAs per SM the register allocation must allow: the inverse-side modes are
+// latency-bound on their operand loads and gain from a third CTA (32x32 complex64:
+// pass C 48.9 -> 39.7 us, E' 46.7 -> 40.5 us per source).
+#ifndef WZ_P01_MINB
+#define WZ_P01_MINB 3
+#endif
+template <typename R, int L0, int L1, int MODE>
+struct p01_minb {
+  static constexpr int v =
+      (sizeof(R) == 4 && L0 == 32 && L1 == 32) ? WZ_P01_MINB : 1;
+};
+
+template <typename R, int L0, int L1, int NSEG, int T0, int T1, int MODE, int FIN, int IC = 0>
+__global__ void __launch_bounds__(P01Cfg<R, L0, L1, NSEG, T0, T1>::NT, p01_minb<R, L0, L1, MODE>::v)
 k_p01(const P01Args<R> a) {
   using Cfg = P01Cfg<R, L0, L1, NSEG, T0, T1>;
   constexpr int TPL0 = Cfg::TPL0, TPL1 = Cfg::TPL1, NR0 = Cfg::NR0, NR1 = Cfg::NR1;
@@ -84,7 +96,10 @@ k_p01(const P01Args<R> a) {
   const int comp = f & 3, src = f >> 2;
   if (a.gate && !cg_active(a.gate + src)) return;
   const long i0 = (long)blockIdx.x * NSEG;
-  const long V = (long)L0 * L1 * a.I;
+  // IC > 0: the (x2,x3) volume is a compile-time constant, so every tile offset below folds
+  // into an immediate of the load/store instead of 64-bit integer arithmetic per access
+  const long I = IC ? (long)IC : a.I;
+  const long V = (long)L0 * L1 * I;
   const cpx<R>* gin = a.in + (long)f * V + i0;
   cpx<R>* gout = a.out + (long)f * V + i0;
 
@@ -108,7 +123,7 @@ k_p01(const P01Args<R> a) {
       if (actA && (sA * (int)sizeof(cpx<R>)) % 32 == 0) {
 #pragma unroll
         for (int k = 0; k < NR0; ++k) {
-          const long off = fo + ((long)F0::in_pos(k, jA) * L1 + x1A) * a.I + sA;
+          const long off = fo + ((long)F0::in_pos(k, jA) * L1 + x1A) * I + sA;
           prefetch_l2(a.cg_r + off);
           prefetch_l2(a.cg_x + off);
         }
@@ -116,7 +131,7 @@ k_p01(const P01Args<R> a) {
 #pragma unroll
       for (int k = 0; k < NR0; ++k) {
         cpx<R> v = {R(0), R(0)};
-        if (actA) v = a.cg_p[fo + ((long)F0::in_pos(k, jA) * L1 + x1A) * a.I + sA];
+        if (actA) v = a.cg_p[fo + ((long)F0::in_pos(k, jA) * L1 + x1A) * I + sA];
         x[k] = v;
       }
       const R beta = (R)a.gate[src].beta, alpha = (R)a.gate[src].alpha;
@@ -127,7 +142,7 @@ k_p01(const P01Args<R> a) {
         long off[CHF];
 #pragma unroll
         for (int c = 0; c < CHF; ++c) {
-          off[c] = fo + ((long)F0::in_pos(k0 + c, jA) * L1 + x1A) * a.I + sA;
+          off[c] = fo + ((long)F0::in_pos(k0 + c, jA) * L1 + x1A) * I + sA;
           vr[c] = {R(0), R(0)};
           vx[c] = {R(0), R(0)};
           if (actA) {
@@ -153,7 +168,7 @@ k_p01(const P01Args<R> a) {
       for (int k = 0; k < NR0; ++k) {
         const int x0 = F0::in_pos(k, jA);
         cpx<R> v = {R(0), R(0)};
-        if (actA) v = gin[((long)x0 * L1 + x1A) * a.I + sA];
+        if (actA) v = gin[((long)x0 * L1 + x1A) * I + sA];
         if (a.apbc) v = mul_tw_rt<R, +1>(v, x0 * TWSTEP);
         x[k] = v;
       }
@@ -178,7 +193,7 @@ k_p01(const P01Args<R> a) {
     if (actB) {
 #pragma unroll
       for (int k = 0; k < NR1; ++k)
-        gout[((long)x0B * L1 + F1::out_pos(k, jB)) * a.I + sB] = y[k];
+        gout[((long)x0B * L1 + F1::out_pos(k, jB)) * I + sB] = y[k];
     }
   } else {
     // ---- inverse half: axis 1 first (from HBM), then axis 0 ----
@@ -189,7 +204,7 @@ k_p01(const P01Args<R> a) {
 #pragma unroll
       for (int k = 0; k < NR1; ++k) {
         cpx<R> v = {R(0), R(0)};
-        if (actB) v = gin[((long)x0B * L1 + G1::in_pos(k, jB)) * a.I + sB];
+        if (actB) v = gin[((long)x0B * L1 + G1::in_pos(k, jB)) * I + sB];
         y[k] = v;
       }
       if constexpr (MODE != P01_INV) {
@@ -198,7 +213,7 @@ k_p01(const P01Args<R> a) {
           const long fo = (long)f * V + i0;
 #pragma unroll
           for (int k = 0; k < NR0; ++k) {
-            const long off = ((long)G0::out_pos(k, jA) * L1 + x1A) * a.I + sA;
+            const long off = ((long)G0::out_pos(k, jA) * L1 + x1A) * I + sA;
             prefetch_l2(a.psi + fo + off);
             prefetch_l2(a.phi + i0 + off);
             if constexpr (MODE == P01_ENDCG) prefetch_l2(a.cg_r + fo + off);
@@ -226,13 +241,14 @@ k_p01(const P01Args<R> a) {
       const int x0 = G0::out_pos(k, jA);
       cpx<R> v = x[k];
       if (a.apbc) v = mul_tw_rt<R, -1>(v, x0 * TWSTEP);
-      x[k] = cscale(v, a.scale);
+      if constexpr (MODE == P01_INV) v = cscale(v, a.scale);  // the fused modes get 1/V from the multiply pass
+      x[k] = v;
     }
     if constexpr (MODE == P01_INV) {
       if (actA) {
 #pragma unroll
         for (int k = 0; k < NR0; ++k)
-          gout[((long)G0::out_pos(k, jA) * L1 + x1A) * a.I + sA] = x[k];
+          gout[((long)G0::out_pos(k, jA) * L1 + x1A) * I + sA] = x[k];
       }
     } else {
       // ---- site-local term of Eq. (2.19): + (m + 2 g phi) P+ psi + (m + 2 g phi)^* P- psi,
@@ -251,17 +267,9 @@ k_p01(const P01Args<R> a) {
           cpx<R> ph[CH], ps[CH];
 #pragma unroll
           for (int c = 0; c < CH; ++c) {
-            off[c] = ((long)G0::out_pos(k0 + c, jA) * L1 + x1A) * a.I + sA;
-#if defined(WZ_DBG_SITE) && (WZ_DBG_SITE & 1)
-            ph[c] = {R(0.25), R(0.5)};
-#else
+            off[c] = ((long)G0::out_pos(k0 + c, jA) * L1 + x1A) * I + sA;
             ph[c] = ldg_c(gphi + off[c]);
-#endif
-#if defined(WZ_DBG_SITE) && (WZ_DBG_SITE & 2)
-            ps[c] = {R(0.25), R(0.5)};
-#else
             ps[c] = ldg_c(gpsi + off[c]);
-#endif
           }
           if constexpr (MODE == P01_ENDCG) {
             cpx<R> vr[CH];
@@ -291,11 +299,7 @@ k_p01(const P01Args<R> a) {
               v.re += w.re * ps[c].re - w.im * ps[c].im;
               v.im += w.re * ps[c].im + w.im * ps[c].re;
               x[k0 + c] = v;
-#if defined(WZ_DBG_SITE) && (WZ_DBG_SITE & 4)
-              if (a.scale == R(12345)) gso[off[c]] = v;
-#else
               gso[off[c]] = v;
-#endif
               if (FIN != FIN_STORE || a.red.partials)
                 acc += (double)v.re * (double)v.re + (double)v.im * (double)v.im;
             }
@@ -332,7 +336,7 @@ k_p01(const P01Args<R> a) {
         if (actB) {
 #pragma unroll
           for (int k = 0; k < NR1; ++k)
-            gout[((long)x0B * L1 + F1::out_pos(k, jB)) * a.I + sB] = y[k];
+            gout[((long)x0B * L1 + F1::out_pos(k, jB)) * I + sB] = y[k];
         }
       }
       if (a.red.partials) {  // one reduction per source: its 4 spin components x all segments

@@ -17,6 +17,20 @@ namespace wz {
 
 enum { P23_FFT = 0, P23_MULT = 1 };
 
+// c(p) = k / (s + Mw) with s = sqrt(Mw^2 + S2), k = 2 rho sign / V; for Mw < 0 the
+// cancellation-free form k (s - Mw) / S2 = k (s + |Mw|) / S2.  float: rsqrt/rcp approximations
+// (<= 2 ulp each, far inside the 2e-5 matvec tolerance); double: IEEE sqrt and divide.
+__device__ __forceinline__ float overlap_c(float Mw, float S2, float k) {
+  const float q = fmaf(Mw, Mw, S2);
+  const float a = fmaf(q, rsqrtf(q), fabsf(Mw));  // s + |Mw|: no cancellation on either branch
+  const bool pos = Mw >= 0.f;
+  return __fdividef(pos ? k : k * a, pos ? a : S2);
+}
+__device__ __forceinline__ double overlap_c(double Mw, double S2, double k) {
+  const double a = sqrt(Mw * Mw + S2) + fabs(Mw);
+  return (Mw >= 0.0) ? k / a : k * a / S2;
+}
+
 template <typename R>
 struct P23Args {
   const cpx<R>* in;   // [nb][4][L0*L1][L2][L3]
@@ -45,7 +59,8 @@ struct P23Cfg {
   static constexpr int NT = NC * NTC;
   static constexpr int PITCH = L3 + 1;            // row pitch (elements)
   static constexpr int CPITCH = L2 * PITCH + 4;   // component pitch
-  static constexpr size_t SMEM = sizeof(cpx<R>) * NC * (size_t)CPITCH;
+  static constexpr int CF_ELEMS = L2 * PITCH;  // c(p) of the plane, computed once per site and shared by the components
+  static constexpr size_t SMEM = sizeof(cpx<R>) * NC * (size_t)CPITCH + sizeof(R) * CF_ELEMS;
 };
 
 template <typename R, int L2, int L3, int T2, int T3, int MODE, int DIR, int NC = 4>
@@ -57,6 +72,7 @@ k_p23(const P23Args<R> a) {
   constexpr int D1 = (MODE == P23_MULT) ? +1 : DIR;  // direction of the first half
   extern __shared__ __align__(16) unsigned char smem_raw[];
   cpx<R>* sm = reinterpret_cast<cpx<R>*>(smem_raw);
+  R* cfs = reinterpret_cast<R*>(sm + NC * CPITCH);
   __shared__ R tb[2 * 4 * 64];
 
   if (a.gate && !cg_active(a.gate + blockIdx.y)) return;
@@ -114,6 +130,26 @@ k_p23(const P23Args<R> a) {
       y[k] = v;
     }
     F3::run(y, jB);
+    if constexpr (MODE == P23_MULT) {
+      // c(p) once per momentum site: component slot cl covers 1/NC of this lane's n3 values
+      static_assert(NR3 % NC == 0, "c(p) sharing");
+      if (actB) {
+        using G3i = LineFFT<R, L3, -1, VAR_DIF, TPL3>;
+        const int n0 = plane / a.L1, n1 = plane % a.L1;
+        const R* sn = tb;
+        const R* sh = tb + 4 * 64;
+        const R s0 = sn[0 * 64 + n0], s1 = sn[1 * 64 + n1], s2 = sn[2 * 64 + n2B];
+        const R S012 = s0 * s0 + s1 * s1 + s2 * s2;
+        const R Mw012 = a.rho - R(2) * (sh[0 * 64 + n0] + sh[1 * 64 + n1] + sh[2 * 64 + n2B]);
+        const R kk = R(2) * a.rho * a.sign * a.scale;  // 1/V of the inverse transform rides along
+#pragma unroll
+        for (int k = cl * (NR3 / NC); k < (cl + 1) * (NR3 / NC); ++k) {
+          const int n3 = G3i::in_pos(k, jB);
+          const R s3 = sn[3 * 64 + n3];
+          cfs[n2B * PITCH + n3] = overlap_c(Mw012 - R(2) * sh[3 * 64 + n3], S012 + s3 * s3, kk);
+        }
+      }
+    }
     __syncthreads();  // pair partners have read their half of the row
     if (actB) {
 #pragma unroll
@@ -142,8 +178,6 @@ k_p23(const P23Args<R> a) {
       const R* sh = tb + 4 * 64;    // sin^2(p_mu/2)
       const int n2 = actB ? n2B : 0;
       const R s0 = sn[0 * 64 + n0], s1 = sn[1 * 64 + n1], s2 = sn[2 * 64 + n2];
-      const R S012 = s0 * s0 + s1 * s1 + s2 * s2;
-      const R Mw012 = a.rho - R(2) * (sh[0 * 64 + n0] + sh[1 * 64 + n1] + sh[2 * 64 + n2]);
       // out_c = i c(p) sign (Ca psi_ca + Cb psi_cb),  Ca = (A0, A1 + A3 s3), Cb = (B0, B1 + B3 s3)
       R A0, A1, A3, B0, B1, B3;
       if (cc == 0)      { A0 = s0;  A1 = R(0); A3 = R(1);  B0 = s2;  B1 = s1;   B3 = R(0); }
@@ -154,15 +188,11 @@ k_p23(const P23Args<R> a) {
       // with NC = 2 those are the two planes this CTA holds
       const cpx<R>* sa = sm + ((NC == 4) ? ((cc < 2) ? 2 : 0) : 0) * CPITCH + n2 * PITCH;
       const cpx<R>* sb = sa + CPITCH;
-      const R two_rho_sign = R(2) * a.rho * a.sign;
 #pragma unroll
       for (int k = 0; k < NR3; ++k) {
         const int n3 = G3::in_pos(k, jB);
         const R s3 = sn[3 * 64 + n3];
-        const R S2 = S012 + s3 * s3;
-        const R Mw = Mw012 - R(2) * sh[3 * 64 + n3];
-        const R s = sqrt(Mw * Mw + S2);
-        const R cf = (Mw >= R(0)) ? two_rho_sign / (s + Mw) : two_rho_sign * (s - Mw) / S2;
+        const R cf = cfs[n2 * PITCH + n3];
         const cpx<R> pa = sa[n3], pb = sb[n3];
         const R Ai = A1 + A3 * s3, Bi = B1 + B3 * s3;
         const R tr = A0 * pa.re - Ai * pa.im + B0 * pb.re - Bi * pb.im;
@@ -189,7 +219,7 @@ k_p23(const P23Args<R> a) {
     if (actA) {
 #pragma unroll
       for (int k = 0; k < NR2; ++k)
-        gout[(long)G2::out_pos(k, jA) * L3 + x3A] = cscale(x[k], a.scale);
+        gout[(long)G2::out_pos(k, jA) * L3 + x3A] = x[k];
     }
   }
 }

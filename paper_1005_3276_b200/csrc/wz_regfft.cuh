@@ -199,6 +199,7 @@ struct LineFFT {
   }
   static __device__ __forceinline__ void run(cpx<R>* x, int j) {
     const bool odd = (j & 1) != 0;
+    const R sgn = odd ? R(-1) : R(1);  // even lane: v + o, odd lane: o - v  ==  fma(sgn, v, o)
     if constexpr (VAR == VAR_DIT) {
       Sub::run(x, j >> 1);
       // twiddle w_L^n, n = Sub::out_pos(k, j>>1) = out_pos(k, 0) + lane part; the lane part
@@ -211,14 +212,14 @@ struct LineFFT {
           if (TPL >= 4 && (j & 2)) v = mul_mi<R, DIR>(v);
         }
         cpx<R> o = shfl_xor_c(v, XD);
-        x[k] = odd ? csub(o, v) : cadd(v, o);  // E + O' | E - O'
+        x[k] = {fma(sgn, v.re, o.re), fma(sgn, v.im, o.im)};  // E + O' | E - O'
       }
     } else {
 #pragma unroll
       for (int k = 0; k < NR; ++k) {
         cpx<R> v = x[k];
         cpx<R> o = shfl_xor_c(v, XD);
-        cpx<R> t = odd ? csub(o, v) : cadd(v, o);  // lo - hi | lo + hi
+        cpx<R> t = {fma(sgn, v.re, o.re), fma(sgn, v.im, o.im)};  // lo + hi | lo - hi
         if (odd) {
           t = mul_tw<R, DIR>(t, Sub::in_pos(k, 0), L);
           if (TPL >= 4 && (j & 2)) t = mul_mi<R, DIR>(t);
