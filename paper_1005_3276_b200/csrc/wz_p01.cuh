@@ -94,7 +94,13 @@ k_p01(const P01Args<R> a) {
   const int tid = threadIdx.x;
   const int f = blockIdx.y;            // field = source*4 + spin
   const int comp = f & 3, src = f >> 2;
-  if (a.gate && !cg_active(a.gate + src)) return;
+  // forward modes: the idle test of this source is issued now but consumed only after the
+  // first loads are in flight (measured: pays there, not in the inverse modes)
+  int idle = 0;
+  if (a.gate) idle = a.gate[src].converged | a.gate[src].need_ru | a.gate[src].stop;
+  if constexpr (MODE != P01_FWD && MODE != P01_FWDCG) {
+    if (idle) return;
+  }
   const long i0 = (long)blockIdx.x * NSEG;
   // IC > 0: the (x2,x3) volume is a compile-time constant, so every tile offset below folds
   // into an immediate of the load/store instead of 64-bit integer arithmetic per access
@@ -135,6 +141,7 @@ k_p01(const P01Args<R> a) {
         x[k] = v;
       }
       const R beta = (R)a.gate[src].beta, alpha = (R)a.gate[src].alpha;
+      if (idle) return;
       constexpr int CHF = (NR0 % 8 == 0) ? 8 : 4;
 #pragma unroll
       for (int k0 = 0; k0 < NR0; k0 += CHF) {
@@ -172,6 +179,7 @@ k_p01(const P01Args<R> a) {
         if (a.apbc) v = mul_tw_rt<R, +1>(v, x0 * TWSTEP);
         x[k] = v;
       }
+      if (idle) return;
     }
     F0::run(x, jA);
     if (actA) {
