@@ -41,7 +41,16 @@ struct P01Entry {
   int L0, L1;
   long I;  // (x2,x3) volume the kernels were specialised for; 0 = any (run-time)
   P01Kern<R> fwd, inv, mid, mid_pq, end, fwdcg, endcg;
-  int nseg() const { return fwd.nseg; }
+  int nseg() const {  // largest tile width of the entry: the (x2,x3) volume must be a multiple
+    int m = 1;
+    for (const P01Kern<R>* k : {&fwd, &inv, &mid, &mid_pq, &end, &fwdcg, &endcg}) m = k->nseg > m ? k->nseg : m;
+    return m;
+  }
+  int min_nseg() const {
+    int m = 1 << 30;
+    for (const P01Kern<R>* k : {&fwd, &inv, &mid, &mid_pq, &end, &fwdcg, &endcg}) m = k->nseg < m ? k->nseg : m;
+    return m;
+  }
 };
 template <typename R>
 struct P23Entry {
@@ -55,15 +64,12 @@ struct P23Entry {
 // ---- tuning: lanes per lattice line (TPL) and tile width (NSEG) -------------------
 // More lanes per line = fewer registers per thread and more resident warps (the
 // passes are latency-bound otherwise: profiles/r01_*); one radix-2 shuffle step per
-// doubling.  Compile-time overrides for sweeps: -DWZ_TPL32F=.. -DWZ_NSEG32F=..
+// doubling.  Compile-time overrides for sweeps: -DWZ_TPL32F=.. -DWZ_NSEG32F_FWD=.. -DWZ_NSEG32F_INV=..
 #ifndef WZ_TPL32F
 #define WZ_TPL32F 2
 #endif
 #ifndef WZ_TPL32F_P23
 #define WZ_TPL32F_P23 1
-#endif
-#ifndef WZ_NSEG32F
-#define WZ_NSEG32F 4
 #endif
 template <typename R, int L> struct tune_tpl {   // axes 0,1
   static constexpr int v = (sizeof(R) == 4) ? (L >= 48 ? 2 : (L == 32 ? WZ_TPL32F : 1))
@@ -73,16 +79,27 @@ template <typename R, int L> struct tune_tpl23 {  // axes 2,3
   static constexpr int v = (sizeof(R) == 4) ? (L >= 48 ? 2 : (L == 32 ? WZ_TPL32F_P23 : 1))
                                             : (L >= 48 ? 4 : (L >= 24 ? 2 : 1));
 };
-// NSEG: consecutive (x2,x3) sites per strided tile: tile L0 x L1 x NSEG <= 128 KB,
-// contiguous runs >= 32 bytes.
-template <typename R, int L0, int L1> struct tune_nseg {
-  static constexpr int v = (sizeof(R) == 4) ? (L0 * L1 > 2048 ? 4 : (L0 * L1 == 1024 ? WZ_NSEG32F : 8))
+// NSEG: consecutive (x2,x3) sites per strided tile: tile L0 x L1 x NSEG <= 136 KB.  The
+// Each (x0,x1) row contributes one run of NSEG*8 bytes, and every
+// run costs one L1 tag lookup per access: at 32^4 complex64 going from 32-byte to 64-/128-byte
+// runs (with 1024 resident threads per SM at 64 registers) took the iteration from 173 to
+// 141 us per source (profiles/r01_notes.md).  Forward modes: 64-byte runs, two 512-thread
+// CTAs per SM; inverse modes: 128-byte runs, one 1024-thread CTA per SM.
+#ifndef WZ_NSEG32F_FWD
+#define WZ_NSEG32F_FWD 8
+#endif
+#ifndef WZ_NSEG32F_INV
+#define WZ_NSEG32F_INV 16
+#endif
+template <typename R, int L0, int L1, int MODE> struct tune_nseg {
+  static constexpr bool fwd = (MODE == P01_FWD || MODE == P01_FWDCG);
+  static constexpr int v = (sizeof(R) == 4) ? (L0 * L1 > 2048 ? 4 : (L0 * L1 == 1024 ? (fwd ? WZ_NSEG32F_FWD : WZ_NSEG32F_INV) : 8))
                                             : (L0 * L1 > 2048 ? 2 : 4);
 };
 
 template <typename R, int L0, int L1, int MODE, int FIN, int IC>
 P01Kern<R> make_p01_kern() {
-  constexpr int NSEG = tune_nseg<R, L0, L1>::v, T0 = tune_tpl<R, L0>::v, T1 = tune_tpl<R, L1>::v;
+  constexpr int NSEG = tune_nseg<R, L0, L1, MODE>::v, T0 = tune_tpl<R, L0>::v, T1 = tune_tpl<R, L1>::v;
   using C = P01Cfg<R, L0, L1, NSEG, T0, T1>;
   P01Kern<R> k;
   k.fn = k_p01<R, L0, L1, NSEG, T0, T1, MODE, FIN, IC>;
@@ -433,7 +450,7 @@ wz_status apply_MdagM_impl(wz_plan* pl, const cpx<R>* phi, const double m[2], co
   a.psi = in; a.phi = phi; a.site_out = ws.chi; a.op = make_op<R>(m, g, rho, 0);
   if (cg) {
     a.red = red_of(pl);
-    if ((int)(pl->I / ws.p01->nseg()) * 4 > pl->npartials) return WZ_EINVAL;
+    if ((int)(pl->I / ws.p01->min_nseg()) * 4 > pl->npartials) return WZ_EINVAL;
     s = launch_p01<R>(pl, WZ_K_P01_MID, ws.p01->mid_pq, a, nb);  // C
   } else {
     s = launch_p01<R>(pl, WZ_K_P01_MID, ws.p01->mid, a, nb);
@@ -456,7 +473,7 @@ template <typename R>
 wz_status cg_iteration(wz_plan* pl, const cpx<R>* phi, const double m[2], const double g[2], double rho,
                        cpx<R>* r, cpx<R>* p, cpx<R>* x, int nb) {
   OpWS<R>& ws = ws_of<R>(pl);
-  if ((int)(pl->I / ws.p01->nseg()) * 4 > pl->npartials) return WZ_EINVAL;
+  if ((int)(pl->I / ws.p01->min_nseg()) * 4 > pl->npartials) return WZ_EINVAL;
   const R invV = (R)(1.0 / (double)pl->V);
   wz_status s;
   P01Args<R> a{};

@@ -68,20 +68,15 @@ struct P01Cfg {
   static constexpr size_t SMEM = sizeof(cpx<R>) * (size_t)L0 * PITCH0;
 };
 
-// Resident CTAs per SM the register allocation must allow: the inverse-side modes are
-// latency-bound on their operand loads and gain from a third CTA (32x32 complex64:
-// pass C 48.9 -> 39.7 us, E' 46.7 -> 40.5 us per source).
-#ifndef WZ_P01_MINB
-#define WZ_P01_MINB 3
-#endif
-template <typename R, int L0, int L1, int MODE>
+// Resident CTAs per SM the register allocation must allow: 32x32 complex64 tiles aim at
+// 1024 resident threads per SM (64 registers each); everything else takes what it needs.
+template <typename R, int L0, int L1, int NT>
 struct p01_minb {
-  static constexpr int v =
-      (sizeof(R) == 4 && L0 == 32 && L1 == 32) ? WZ_P01_MINB : 1;
+  static constexpr int v = (sizeof(R) == 4 && L0 == 32 && L1 == 32 && NT <= 1024) ? (1024 / NT) : 1;
 };
 
 template <typename R, int L0, int L1, int NSEG, int T0, int T1, int MODE, int FIN, int IC = 0>
-__global__ void __launch_bounds__(P01Cfg<R, L0, L1, NSEG, T0, T1>::NT, p01_minb<R, L0, L1, MODE>::v)
+__global__ void __launch_bounds__(P01Cfg<R, L0, L1, NSEG, T0, T1>::NT, p01_minb<R, L0, L1, P01Cfg<R, L0, L1, NSEG, T0, T1>::NT>::v)
 k_p01(const P01Args<R> a) {
   using Cfg = P01Cfg<R, L0, L1, NSEG, T0, T1>;
   constexpr int TPL0 = Cfg::TPL0, TPL1 = Cfg::TPL1, NR0 = Cfg::NR0, NR1 = Cfg::NR1;

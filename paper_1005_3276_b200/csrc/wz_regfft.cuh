@@ -79,6 +79,45 @@ __device__ __forceinline__ cpx<R> mul_tw_rt(cpx<R> a, int idx) {
   return cmul(a, w);
 }
 
+// ---- packed FP32x2 (Blackwell FADD2/FFMA2): one instruction per complex add ----------
+// A complex64 value is an aligned register pair, so a complex add/sub is ONE add.f32x2 /
+// sub.f32x2 issue slot instead of two (same FP-pipe time, half the issue slots; the
+// passes are issue-bound, profiles/r01_*).  Multiplications by twiddles stay scalar.
+#ifndef WZ_PACKED
+#define WZ_PACKED 1
+#endif
+__device__ __forceinline__ unsigned long long pk(cpx<float> a) {
+  unsigned long long r;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(a.re), "f"(a.im));
+  return r;
+}
+__device__ __forceinline__ cpx<float> upk(unsigned long long v) {
+  cpx<float> a;
+  asm("mov.b64 {%0, %1}, %2;" : "=f"(a.re), "=f"(a.im) : "l"(v));
+  return a;
+}
+#if WZ_PACKED
+template <>
+__device__ __forceinline__ cpx<float> cadd<float>(cpx<float> a, cpx<float> b) {
+  unsigned long long r;
+  asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(pk(a)), "l"(pk(b)));
+  return upk(r);
+}
+template <>
+__device__ __forceinline__ cpx<float> csub<float>(cpx<float> a, cpx<float> b) {
+  unsigned long long r;
+  asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(pk(a)), "l"(pk(b)));
+  return upk(r);
+}
+#endif
+// a + s * (b.im, -b.re) for s = +1 (a - i b) and the mirrored a + i b: one FFMA2 each
+__device__ __forceinline__ cpx<float> fma_pm(cpx<float> bs /* (b.im, b.re) */, float c0, float c1, cpx<float> a) {
+  unsigned long long r;
+  cpx<float> c = {c0, c1};
+  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(pk(bs)), "l"(pk(c)), "l"(pk(a)));
+  return upk(r);
+}
+
 // ---- small butterflies -------------------------------------------------------
 template <typename R>
 __device__ __forceinline__ void bf2(cpx<R>& a, cpx<R>& b) {
@@ -94,6 +133,19 @@ __device__ __forceinline__ void bf4(cpx<R>& a, cpx<R>& b, cpx<R>& c, cpx<R>& d) 
   b = cadd(t1, t3);
   d = csub(t1, t3);
 }
+#if WZ_PACKED
+template <int DIR>
+__device__ __forceinline__ void bf4_packed(cpx<float>& a, cpx<float>& b, cpx<float>& c, cpx<float>& d) {
+  const cpx<float> t0 = cadd(a, c), t1 = csub(a, c), t2 = cadd(b, d), u = csub(b, d);
+  const cpx<float> us = {u.im, u.re};
+  // forward: -i u = (u.im, -u.re);  inverse: +i u = (-u.im, u.re)
+  const float s = (DIR > 0) ? 1.f : -1.f;
+  a = cadd(t0, t2);
+  c = csub(t0, t2);
+  b = fma_pm(us, s, -s, t1);
+  d = fma_pm(us, -s, s, t1);
+}
+#endif
 template <typename R, int DIR>
 __device__ __forceinline__ void bf3(cpx<R>& a, cpx<R>& b, cpx<R>& c) {
   const R h = R(0.86602540378443864676372317075294);  // sqrt(3)/2
@@ -131,7 +183,11 @@ struct RegFFT {
 #pragma unroll
       for (int k = 0; k < m; ++k) {
         if constexpr (r == 4) {
-          bf4<R, DIR>(x[k], x[k + m], x[k + 2 * m], x[k + 3 * m]);
+#if WZ_PACKED
+          if constexpr (sizeof(R) == 4) bf4_packed<DIR>(x[k], x[k + m], x[k + 2 * m], x[k + 3 * m]);
+          else
+#endif
+            bf4<R, DIR>(x[k], x[k + m], x[k + 2 * m], x[k + 3 * m]);
           x[k + m] = mul_tw<R, DIR>(x[k + m], k, N);
           x[k + 2 * m] = mul_tw<R, DIR>(x[k + 2 * m], 2 * k, N);
           x[k + 3 * m] = mul_tw<R, DIR>(x[k + 3 * m], 3 * k, N);
