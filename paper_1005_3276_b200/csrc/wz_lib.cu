@@ -71,8 +71,11 @@ struct P23Entry {
 #ifndef WZ_TPL32F_P23
 #define WZ_TPL32F_P23 1
 #endif
-template <typename R, int L> struct tune_tpl {   // axes 0,1
-  static constexpr int v = (sizeof(R) == 4) ? (L >= 48 ? 2 : (L == 32 ? WZ_TPL32F : 1))
+#ifndef WZ_TPL32F_MID
+#define WZ_TPL32F_MID 1
+#endif
+template <typename R, int L, int MODE> struct tune_tpl {   // axes 0,1; pass C does best with whole lines per thread
+  static constexpr int v = (sizeof(R) == 4) ? (L >= 48 ? 2 : (L == 32 ? (MODE == P01_MID ? WZ_TPL32F_MID : WZ_TPL32F) : 1))
                                             : (L >= 48 ? 4 : (L >= 24 ? 2 : 1));
 };
 template <typename R, int L> struct tune_tpl23 {  // axes 2,3
@@ -99,7 +102,7 @@ template <typename R, int L0, int L1, int MODE> struct tune_nseg {
 
 template <typename R, int L0, int L1, int MODE, int FIN, int IC>
 P01Kern<R> make_p01_kern() {
-  constexpr int NSEG = tune_nseg<R, L0, L1, MODE>::v, T0 = tune_tpl<R, L0>::v, T1 = tune_tpl<R, L1>::v;
+  constexpr int NSEG = tune_nseg<R, L0, L1, MODE>::v, T0 = tune_tpl<R, L0, MODE>::v, T1 = tune_tpl<R, L1, MODE>::v;
   using C = P01Cfg<R, L0, L1, NSEG, T0, T1>;
   P01Kern<R> k;
   k.fn = k_p01<R, L0, L1, NSEG, T0, T1, MODE, FIN, IC>;

@@ -70,13 +70,14 @@ struct P01Cfg {
 
 // Resident CTAs per SM the register allocation must allow: 32x32 complex64 tiles aim at
 // 1024 resident threads per SM (64 registers each); everything else takes what it needs.
-template <typename R, int L0, int L1, int NT>
-struct p01_minb {
-  static constexpr int v = (sizeof(R) == 4 && L0 == 32 && L1 == 32 && NT <= 1024) ? (1024 / NT) : 1;
+template <typename R, int L0, int L1, int NT, int TPL>
+struct p01_minb {  // TPL = 2: 16 values per thread, 64 registers; TPL = 1: 32 values, 128 registers
+  static constexpr int want = 512 * TPL;
+  static constexpr int v = (sizeof(R) == 4 && L0 == 32 && L1 == 32 && NT <= want) ? (want / NT) : 1;
 };
 
 template <typename R, int L0, int L1, int NSEG, int T0, int T1, int MODE, int FIN, int IC = 0>
-__global__ void __launch_bounds__(P01Cfg<R, L0, L1, NSEG, T0, T1>::NT, p01_minb<R, L0, L1, P01Cfg<R, L0, L1, NSEG, T0, T1>::NT>::v)
+__global__ void __launch_bounds__(P01Cfg<R, L0, L1, NSEG, T0, T1>::NT, p01_minb<R, L0, L1, P01Cfg<R, L0, L1, NSEG, T0, T1>::NT, T0>::v)
 k_p01(const P01Args<R> a) {
   using Cfg = P01Cfg<R, L0, L1, NSEG, T0, T1>;
   constexpr int TPL0 = Cfg::TPL0, TPL1 = Cfg::TPL1, NR0 = Cfg::NR0, NR1 = Cfg::NR1;
