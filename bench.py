@@ -311,6 +311,7 @@ def run_wz(args):
     extras = {}
     if not args.no_extras:
         extras = time_pieces(plan, d_phi, d_b[:1], m, g, rho, u, peak)
+        extras.update(time_pieces_batched(plan, d_phi, d_b, m, g, rho, u, peak))
     per_iter_us = 1e6 * secs * world / max(iters, 1)
     extras.update({"cg_us_per_iteration": per_iter_us, "iterations_per_source": [i.iterations for i in infos],
                    "reliable_updates_per_source": [i.reliable_updates for i in infos],
@@ -382,6 +383,36 @@ def time_pieces(plan, d_phi, d_b1, m, g, rho, u, peak):
             if name.startswith("fft4d"):
                 res[key]["gflops_5NlogN"] = flops_fft / med / 1e9
     res["matvecs_per_s_warm"] = 1.0 / (res["apply_MdagM_warm"]["us_median"] * 1e-6)
+    return res
+
+
+def time_pieces_batched(plan, d_phi, d_b, m, g, rho, u, peak):
+    """The same calls on the whole batch of sources (steady state: ~20 waves per launch, working
+    set far beyond L2); times are per source."""
+    import torch
+
+    nb = d_b.shape[0]
+    out = torch.empty_like(d_b)
+    res = {}
+    for name, fn, nu in [
+        ("fft4d_forward", lambda: plan.fft4d(d_b, +1, True, out=out), 4.0),
+        ("fft4d_inverse", lambda: plan.fft4d(d_b, -1, True, out=out), 4.0),
+        ("apply_M", lambda: plan.apply_M(d_phi, d_b, m, g, rho, False, out=out), 7.25),
+        ("apply_MdagM", lambda: plan.apply_MdagM(d_phi, d_b, m, g, rho, out=out), 13.5),
+    ]:
+        ts = []
+        for i in range(13):
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            fn()
+            b.record()
+            b.synchronize()
+            if i >= 3:
+                ts.append(a.elapsed_time(b) * 1e-3 / nb)
+        med = statistics.median(ts)
+        res[name + "_batched"] = {"us_median_per_source": 1e6 * med, "algo_GBs": nu * u / med / 1e9,
+                                  "frac_of_peak": nu * u / med / 1e9 / peak, "sources": nb}
+    res["matvecs_per_s_batched"] = 1.0 / (res["apply_MdagM_batched"]["us_median_per_source"] * 1e-6)
     return res
 
 
