@@ -71,11 +71,14 @@ struct P23Entry {
 #ifndef WZ_TPL32F_P23
 #define WZ_TPL32F_P23 1
 #endif
+#ifndef WZ_TPL64F
+#define WZ_TPL64F 2
+#endif
 #ifndef WZ_TPL32F_MID
 #define WZ_TPL32F_MID 1
 #endif
 template <typename R, int L, int MODE> struct tune_tpl {   // axes 0,1; pass C does best with whole lines per thread
-  static constexpr int v = (sizeof(R) == 4) ? (L >= 48 ? 2 : (L == 32 ? (MODE == P01_MID ? WZ_TPL32F_MID : WZ_TPL32F) : 1))
+  static constexpr int v = (sizeof(R) == 4) ? (L == 64 ? WZ_TPL64F : (L >= 48 ? 2 : (L == 32 ? (MODE == P01_MID ? WZ_TPL32F_MID : WZ_TPL32F) : 1)))
                                             : (L >= 48 ? 4 : (L >= 24 ? 2 : 1));
 };
 template <typename R, int L> struct tune_tpl23 {  // axes 2,3

@@ -281,3 +281,27 @@ def test_batched_solve_equals_single_solves(wz, inp):
         assert i1[0].iterations == ib[j].iterations == 400
         assert i1[0].reliable_updates == ib[j].reliable_updates
         assert torch.equal(xs[0], xb[j])
+
+
+@pytest.mark.parametrize("key", ["5a", "5b"])
+def test_config5_solve_true_residual(wz, orc, inp, key):
+    """Config 5 (48x24^3 mixed radix 2/3, and 64^4): one Gaussian source solved to 1e-6 in
+    complex64 with reliable updates; the ORACLE recomputes the true residual of the GPU's x
+    (naive-DFT route at 48x24^3, radix-2 route at 64^4)."""
+    cfg = inp.CONFIGS[key]
+    dims = cfg["dims"]
+    phi = inp.make_phi(cfg["seed"], dims, cfg["sigma"], np.complex64)
+    b = inp.make_source(cfg["seed"], 0, dims, np.complex64)
+    plan = wz.Plan(dims, "c64", 1)
+    x, infos = plan.cg_solve(torch.from_numpy(phi).cuda(), torch.from_numpy(b).cuda(), cfg["m"], cfg["g"],
+                             cfg["rho"], cfg["tol"], 200000)
+    info = infos[0]
+    print("config %s: iterations %d, reliable updates %d, true residual %.3e"
+          % (key, info.iterations, info.reliable_updates, info.rel_residual_true))
+    assert info.converged and info.rel_residual_true <= cfg["tol"] and info.reliable_updates >= 1
+    xh = x.cpu().numpy()
+    del plan, x
+    res = rel(orc.apply_MdagM(phi.astype(np.complex128), xh, cfg["m"], cfg["g"], cfg["rho"]),
+              b.astype(np.complex128))
+    assert res <= cfg["tol"], res
+    assert abs(res - info.rel_residual_true) <= 0.02 * cfg["tol"]
