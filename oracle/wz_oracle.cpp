@@ -583,4 +583,147 @@ int orc_cg_c64ru(int method, const int* L, const double* phi, const double* b_, 
   return 0;
 }
 
+// ----------------------------------------------------------------------------
+// O5 (NEXT-1). Preconditioning by the free fermion matrix.
+//   M0 = Dslash + m P+ + m^* P-          (Eq. 2.19 at g = 0)
+//   M0^-1 = M0^dag / (D_mu^dag D_mu + |m|^2)                      (Eq. 7.11)
+// with D_mu^dag D_mu = d^2(p) = c(p)^2 sum_mu sin^2 p_mu in momentum space.
+// Applied as the paper applies Dslash: forward DFT, the explicit 4x4 matrix at
+// every momentum, inverse DFT.  dagger = 1 applies (M0^-1)^dag = M0 / (d^2 + |m|^2),
+// written as the conjugate transpose of the same 4x4 matrix.
+// ----------------------------------------------------------------------------
+int orc_apply_M0inv(int method, const int* L, const double* m_, double rho, int dagger,
+                    const double* in_, double* out_) {
+  const cd* in = reinterpret_cast<const cd*>(in_);
+  cd* out = reinterpret_cast<cd*>(out_);
+  const cd m(m_[0], m_[1]);
+  const cd I(0.0, 1.0);
+  const long V = (long)L[0] * L[1] * L[2] * L[3];
+  std::vector<cd> f(in, in + 4 * V);
+  int rc = orc_dft4d(method, +1, 1, L, reinterpret_cast<double*>(f.data()), 4);
+  if (rc) return rc;
+  cd gam[4][4][4];
+  for (int mu = 0; mu < 4; ++mu) gamma_matrix(mu, gam[mu]);
+  std::vector<double> sn[4], sh2[4];
+  for (int mu = 0; mu < 4; ++mu) {
+    sn[mu].resize(L[mu]);
+    sh2[mu].resize(L[mu]);
+    for (int n = 0; n < L[mu]; ++n) {
+      double p = momentum(n, L[mu], mu == 0);
+      sn[mu][n] = std::sin(p);
+      double h = std::sin(0.5 * p);
+      sh2[mu][n] = h * h;
+    }
+  }
+#pragma omp parallel for collapse(2) schedule(static)
+  for (int n0 = 0; n0 < L[0]; ++n0)
+    for (int n1 = 0; n1 < L[1]; ++n1)
+      for (int n2 = 0; n2 < L[2]; ++n2)
+        for (int n3 = 0; n3 < L[3]; ++n3) {
+          long site = (((long)n0 * L[1] + n1) * L[2] + n2) * L[3] + n3;
+          double s4[4] = {sn[0][n0], sn[1][n1], sn[2][n2], sn[3][n3]};
+          double h4[4] = {sh2[0][n0], sh2[1][n1], sh2[2][n2], sh2[3][n3]};
+          double d2 = 0.0;
+          double c = dslash_c(s4, h4, rho, &d2);
+          // M0(p) = i c gamma.sin p + m P+ + m^* P-   (P- = spin 0,1; P+ = spin 2,3)
+          cd M0[4][4];
+          for (int a = 0; a < 4; ++a)
+            for (int b = 0; b < 4; ++b) {
+              cd acc = 0.0;
+              for (int mu = 0; mu < 4; ++mu) acc += I * c * s4[mu] * gam[mu][a][b];
+              M0[a][b] = acc;
+            }
+          M0[0][0] += std::conj(m); M0[1][1] += std::conj(m);
+          M0[2][2] += m;            M0[3][3] += m;
+          const double den = d2 + std::norm(m);
+          // Minv = M0^dag / den
+          cd Minv[4][4];
+          for (int a = 0; a < 4; ++a)
+            for (int b = 0; b < 4; ++b) Minv[a][b] = std::conj(M0[b][a]) / den;
+          cd v[4], r[4];
+          for (int a = 0; a < 4; ++a) v[a] = f[a * V + site];
+          for (int a = 0; a < 4; ++a) {
+            cd acc = 0.0;
+            for (int b = 0; b < 4; ++b) acc += (dagger ? std::conj(Minv[b][a]) : Minv[a][b]) * v[b];
+            r[a] = acc;
+          }
+          for (int a = 0; a < 4; ++a) f[a * V + site] = r[a];
+        }
+  rc = orc_dft4d(method, -1, 1, L, reinterpret_cast<double*>(f.data()), 4);
+  if (rc) return rc;
+  for (long i = 0; i < 4 * V; ++i) out[i] = f[i];
+  return 0;
+}
+
+// Mtilde = M M0^-1 (dagger = 0),  Mtilde^dag = (M0^-1)^dag M^dag (dagger = 1); Eq. 7.10,
+// composed literally from the two operators above.
+int orc_apply_Mtilde(int method, const int* L, const double* phi, const double* m, const double* g,
+                     double rho, int dagger, const double* in, double* out) {
+  const long V = (long)L[0] * L[1] * L[2] * L[3];
+  std::vector<double> tmp(8 * V);
+  int rc;
+  if (!dagger) {
+    if ((rc = orc_apply_M0inv(method, L, m, rho, 0, in, tmp.data()))) return rc;
+    return orc_apply_M(method, L, phi, m, g, rho, 0, tmp.data(), out);
+  }
+  if ((rc = orc_apply_M(method, L, phi, m, g, rho, 1, in, tmp.data()))) return rc;
+  return orc_apply_M0inv(method, L, m, rho, 1, tmp.data(), out);
+}
+
+// Preconditioned solve, Eq. 7.8-7.10:  btilde = (M0^-1)^dag b;  CG on
+// Mtilde^dag Mtilde xtilde = btilde (same textbook loop as orc_cg, xtilde0 = 0, stop when
+// ||rtilde|| <= tol ||btilde||: DESIGN.md reading G15);  x = M0^-1 xtilde.
+// info->rel_residual_recursive is the preconditioned system's; rel_residual_true is
+// ||b - M^dag M x|| / ||b|| of the ORIGINAL system, recomputed at exit.
+int orc_cg_pc(int method, const int* L, const double* phi, const double* b_, double* x_,
+              const double* m, const double* g, double rho, double tol, int max_iter,
+              orc_cg_info* info, double* history) {
+  const long V = (long)L[0] * L[1] * L[2] * L[3];
+  const long n = 4 * V;
+  const cd* b = reinterpret_cast<const cd*>(b_);
+  std::vector<cd> bt(n), xt(n, 0.0), r(n), p(n), q(n), w(n);
+  int rc = orc_apply_M0inv(method, L, m, rho, 1, b_, reinterpret_cast<double*>(bt.data()));
+  if (rc) return rc;
+  r = bt;
+  p = bt;
+  double btnorm = std::sqrt(dot_re(bt.data(), bt.data(), n));
+  double rr = btnorm * btnorm;
+  if (history) history[0] = 1.0;
+  int k = 0, converged = (btnorm == 0.0);
+  while (!converged && k < max_iter) {
+    ++k;
+    if ((rc = orc_apply_Mtilde(method, L, phi, m, g, rho, 0, reinterpret_cast<double*>(p.data()),
+                               reinterpret_cast<double*>(w.data())))) return rc;
+    if ((rc = orc_apply_Mtilde(method, L, phi, m, g, rho, 1, reinterpret_cast<double*>(w.data()),
+                               reinterpret_cast<double*>(q.data())))) return rc;
+    double alpha = rr / dot_re(p.data(), q.data(), n);
+#pragma omp parallel for schedule(static)
+    for (long i = 0; i < n; ++i) {
+      xt[i] += alpha * p[i];
+      r[i] -= alpha * q[i];
+    }
+    double rr_new = dot_re(r.data(), r.data(), n);
+    if (history) history[k] = std::sqrt(rr_new) / btnorm;
+    if (std::sqrt(rr_new) <= tol * btnorm) {
+      rr = rr_new;
+      converged = 1;
+      break;
+    }
+    double beta = rr_new / rr;
+    rr = rr_new;
+#pragma omp parallel for schedule(static)
+    for (long i = 0; i < n; ++i) p[i] = r[i] + beta * p[i];
+  }
+  if ((rc = orc_apply_M0inv(method, L, m, rho, 0, reinterpret_cast<double*>(xt.data()), x_))) return rc;
+  orc_apply_MdagM(method, L, phi, m, g, rho, x_, reinterpret_cast<double*>(q.data()));
+  double tr = 0.0, bb = 0.0;
+  for (long i = 0; i < n; ++i) { tr += std::norm(b[i] - q[i]); bb += std::norm(b[i]); }
+  info->iterations = k;
+  info->reliable_updates = 0;
+  info->converged = converged;
+  info->rel_residual_recursive = btnorm > 0 ? std::sqrt(rr) / btnorm : 0.0;
+  info->rel_residual_true = bb > 0 ? std::sqrt(tr / bb) : 0.0;
+  return 0;
+}
+
 }  // extern "C"

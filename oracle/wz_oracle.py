@@ -177,3 +177,45 @@ def cg_c64ru(phi, b, m, g, rho=1.0, tol=1e-6, max_iter=100000, delta=0.1, method
         raise ValueError("oracle cg_c64ru failed")
     return X, CGInfo(info.iterations, info.reliable_updates, bool(info.converged),
                      info.rel_residual_recursive, info.rel_residual_true, hist[: info.iterations + 1].copy())
+
+
+def apply_M0inv(dims, psi, m, rho=1.0, dagger=False, method="auto") -> np.ndarray:
+    """M0^-1 psi (Eq. 7.11) or its conjugate transpose; M0 = free (g = 0) fermion matrix."""
+    psi = np.ascontiguousarray(psi, dtype=np.complex128)
+    dims = tuple(int(d) for d in dims)
+    assert psi.shape == (4,) + dims
+    out = np.empty_like(psi)
+    rc = lib().orc_apply_M0inv(_method(dims, method), _dims(dims), _c2(m), ctypes.c_double(rho),
+                               int(bool(dagger)), _dp(psi), _dp(out))
+    if rc:
+        raise ValueError("oracle apply_M0inv failed")
+    return out
+
+
+def apply_Mtilde(phi, psi, m, g, rho=1.0, dagger=False, method="auto") -> np.ndarray:
+    """Mtilde = M M0^-1 (Eq. 7.10) or its conjugate transpose."""
+    phi = np.ascontiguousarray(phi, dtype=np.complex128)
+    psi = np.ascontiguousarray(psi, dtype=np.complex128)
+    dims = phi.shape
+    out = np.empty_like(psi)
+    rc = lib().orc_apply_Mtilde(_method(dims, method), _dims(dims), _dp(phi), _c2(m), _c2(g),
+                                ctypes.c_double(rho), int(bool(dagger)), _dp(psi), _dp(out))
+    if rc:
+        raise ValueError("oracle apply_Mtilde failed")
+    return out
+
+
+def cg_pc(phi, b, m, g, rho=1.0, tol=1e-10, max_iter=100000, method="auto"):
+    """Preconditioned CG (Eq. 7.8-7.11) in complex128.  Returns (x, CGInfo)."""
+    phi = np.ascontiguousarray(phi, dtype=np.complex128)
+    b = np.ascontiguousarray(b, dtype=np.complex128)
+    dims = phi.shape
+    x = np.zeros_like(b)
+    hist = np.zeros(max_iter + 1, dtype=np.float64)
+    info = _Info()
+    rc = lib().orc_cg_pc(_method(dims, method), _dims(dims), _dp(phi), _dp(b), _dp(x), _c2(m), _c2(g),
+                         ctypes.c_double(rho), ctypes.c_double(tol), int(max_iter), ctypes.byref(info), _dp(hist))
+    if rc:
+        raise ValueError("oracle cg_pc failed")
+    return x, CGInfo(info.iterations, info.reliable_updates, bool(info.converged),
+                     info.rel_residual_recursive, info.rel_residual_true, hist[: info.iterations + 1].copy())

@@ -1,0 +1,75 @@
+"""Pins of the oracle's preconditioned solve (Eq. 7.8-7.11).
+None of these re-types the oracle's formula: they use the unpreconditioned operator, the
+dense position-space route and the paper's Table VI as references."""
+import numpy as np
+import pytest
+
+from paper_1005_3276_b200 import inputs
+
+
+def rel(a, ref):
+    return float(np.linalg.norm((a - ref).ravel()) / np.linalg.norm(ref.ravel()))
+
+
+@pytest.mark.parametrize("dims", [(4, 4, 4, 4), (8, 4, 6, 4)])
+@pytest.mark.parametrize("m", [0.3, 0.2 + 0.1j])
+def test_M0inv_inverts_the_free_matrix(orc, dims, m):
+    """M0^-1 M0 = M0 M0^-1 = 1, with M0 = the oracle's M at g = 0 (independent code path: Eq. 2.19)."""
+    psi = inputs.make_source(11, 0, dims)
+    phi = inputs.make_phi(11, dims, 0.4)  # irrelevant at g = 0
+    for rho in (1.0, 0.7):
+        M0psi = orc.apply_M(phi, psi, m, 0.0, rho)
+        assert rel(orc.apply_M0inv(dims, M0psi, m, rho), psi) < 1e-12
+        assert rel(orc.apply_M(phi, orc.apply_M0inv(dims, psi, m, rho), m, 0.0, rho), psi) < 1e-12
+        # dagger: (M0^-1)^dag M0^dag = 1
+        M0dpsi = orc.apply_M(phi, psi, m, 0.0, rho, dagger=True)
+        assert rel(orc.apply_M0inv(dims, M0dpsi, m, rho, dagger=True), psi) < 1e-12
+
+
+def test_M0inv_adjoint_and_Mtilde_identity_at_g0(orc):
+    dims = (4, 4, 4, 4)
+    u, v = inputs.make_source(3, 0, dims), inputs.make_source(3, 1, dims)
+    m = 0.25 - 0.1j
+    lhs = np.vdot(u, orc.apply_M0inv(dims, v, m))
+    rhs = np.vdot(orc.apply_M0inv(dims, u, m, dagger=True), v)
+    assert abs(lhs - rhs) < 1e-12 * abs(lhs)
+    phi = inputs.make_phi(3, dims, 0.3)
+    assert rel(orc.apply_Mtilde(phi, v, m, 0.0), v) < 1e-12  # Mtilde = 1 in the free theory
+    # <u, Mtilde v> = <Mtilde^dag u, v> at g != 0
+    g = 0.4 + 0.2j
+    lhs = np.vdot(u, orc.apply_Mtilde(phi, v, m, g))
+    rhs = np.vdot(orc.apply_Mtilde(phi, u, m, g, dagger=True), v)
+    assert abs(lhs - rhs) < 1e-12 * abs(lhs)
+
+
+def test_pc_solution_equals_direct_solution(orc):
+    """x from the preconditioned CG = the Cholesky solution of the DENSE position-space M^dag M."""
+    from oracle import dense_route
+
+    dims = (4, 4, 4, 4)
+    cfg = inputs.CONFIGS[1]
+    phi = inputs.make_phi(1, dims, cfg["sigma"])
+    b = inputs.make_source(1, 0, dims)
+    x, info = orc.cg_pc(phi, b, cfg["m"], cfg["g"], 1.0, 1e-12, 5000)
+    assert info.converged and info.rel_residual_true < 1e-9
+    M = dense_route.fermion_matrix_dense(dims, phi, cfg["m"], cfg["g"], 1.0)
+    xd = np.linalg.solve(M.conj().T @ M, b.reshape(-1)).reshape(b.shape)
+    assert rel(x, xd) < 1e-8
+    x2, info2 = orc.cg(phi, b, cfg["m"], cfg["g"], 1.0, 1e-12, 5000)
+    assert rel(x, x2) < 1e-8
+
+
+def test_weak_coupling_iteration_counts_like_table_VI(orc):
+    """Table VI: at m = 1, g = 1/5 the preconditioned solve needs 8 (1e-6) to 15
+    (1e-12) iterations, the plain one hundreds to thousands.  phi of the paper's ensembles is not
+    available; with phi ~ N(0, 0.5^2) at the same m, g the counts must land in the same regime."""
+    dims = (8, 4, 4, 4)
+    phi = inputs.make_phi(5, dims, 0.5)
+    b = inputs.make_source(5, 0, dims)
+    _, plain = orc.cg(phi, b, 1.0, 0.2, 1.0, 1e-6, 5000)
+    _, pc6 = orc.cg_pc(phi, b, 1.0, 0.2, 1.0, 1e-6, 5000)
+    _, pc12 = orc.cg_pc(phi, b, 1.0, 0.2, 1.0, 1e-12, 5000)
+    assert pc6.converged and pc12.converged and plain.converged
+    assert pc6.iterations <= 12 and pc12.iterations <= 25
+    assert plain.iterations >= 3 * pc6.iterations
+    assert pc6.rel_residual_true < 1e-5
