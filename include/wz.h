@@ -105,6 +105,24 @@ wz_status wz_cg_solve(wz_plan *plan, const void *phi, const void *b, void *x,
                       const double m[2], const double g[2], double rho,
                       double tol, int max_iter, int nbatch, wz_cg_info *info);
 
+/* ---- Free-inverse preconditioning (Eq. 7.8-7.11) ----
+ * M0 = Dslash + m P+ + m* P- is the fermion matrix at g = 0;  M0^-1 = M0^dag / (D_mu^dag D_mu + |m|^2)
+ * is diagonal in momentum space (4x4 per momentum).  m != 0 is required.
+ * wz_apply_M0inv:   out = M0^-1 in (dagger = 0) or (M0^-1)^dag in (dagger = 1); in == out allowed.
+ * wz_apply_MtdagMt: out = Mtilde^dag Mtilde in with Mtilde = M M0^-1 (Eq. 7.10); in != out.
+ * wz_cg_solve_pc:   btilde = (M0^-1)^dag b;  CG on Mtilde^dag Mtilde xtilde = btilde from xtilde0 = 0,
+ *   stop when ||rtilde|| <= tol ||btilde|| (the preconditioned system's residual; G15);
+ *   x = M0^-1 xtilde.  Arguments as wz_cg_solve (x always complex128).  In info,
+ *   rel_residual_recursive refers to the preconditioned system, rel_residual_true is
+ *   ||b - M^dag M x|| / ||b|| of the ORIGINAL system recomputed at exit. */
+wz_status wz_apply_M0inv(wz_plan *plan, int dagger, const double m[2], double rho,
+                         const void *in, void *out, int nbatch);
+wz_status wz_apply_MtdagMt(wz_plan *plan, const void *phi, const double m[2], const double g[2],
+                           double rho, const void *in, void *out, int nbatch);
+wz_status wz_cg_solve_pc(wz_plan *plan, const void *phi, const void *b, void *x,
+                         const double m[2], const double g[2], double rho,
+                         double tol, int max_iter, int nbatch, wz_cg_info *info);
+
 /* Number of kernel launches this plan has enqueued so far (for bench.py's
  * gpu_launches), and a reset. */
 unsigned long long wz_plan_launch_count(const wz_plan *plan);

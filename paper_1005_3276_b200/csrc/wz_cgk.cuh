@@ -37,37 +37,42 @@ __device__ __forceinline__ void st16(R* p, const R (&v)[vec16<R>::N]) {
 
 constexpr int CGK_NT = 256;
 
-// r = b, p = b, xs = 0 (if given), X = 0 (complex128, if given); ||b||^2 -> FIN_INIT
-template <typename R>
+// r = b, p = b (rounded to R if b is wider), xs = 0 (if given), X = 0 (complex128, if given);
+// ||b||^2 (of the values as given) -> FIN_INIT.  TB: storage type of b.
+template <typename R, typename TB>
 __global__ void __launch_bounds__(CGK_NT)
-k_cg_init(const R* __restrict__ b, R* __restrict__ r, R* __restrict__ p, R* __restrict__ xs,
+k_cg_init(const TB* b, R* r, R* p /* b may alias r or p */, R* __restrict__ xs,
           double* __restrict__ X, long n, RedArgs red) {
   const int src = blockIdx.y;  // one source per grid row
   b += src * n; r += src * n; p += src * n;
   if (xs) xs += src * n;
   if (X) X += src * n;
   red = red.for_source(src);
-  constexpr int N = vec16<R>::N;
   __shared__ double sh[33];
   double acc = 0.0;
-  for (long i = ((long)blockIdx.x * blockDim.x + threadIdx.x) * N; i < n;
-       i += (long)gridDim.x * blockDim.x * N) {
-    R v[N], z[N];
-    ld16<R>(b + i, v);
-#pragma unroll
-    for (int e = 0; e < N; ++e) {
-      acc += (double)v[e] * (double)v[e];
-      z[e] = R(0);
-    }
-    st16<R>(r + i, v);
-    st16<R>(p + i, v);
-    if (xs) st16<R>(xs + i, z);
-    if (X) {
-#pragma unroll
-      for (int e = 0; e < N; ++e) X[i + e] = 0.0;
-    }
+  for (long i = ((long)blockIdx.x * blockDim.x + threadIdx.x) * 2; i < n;
+       i += (long)gridDim.x * blockDim.x * 2) {
+    const TB b0 = b[i], b1 = b[i + 1];
+    acc += (double)b0 * (double)b0 + (double)b1 * (double)b1;
+    r[i] = (R)b0; r[i + 1] = (R)b1;
+    p[i] = (R)b0; p[i + 1] = (R)b1;
+    if (xs) { xs[i] = R(0); xs[i + 1] = R(0); }
+    if (X) { X[i] = 0.0; X[i + 1] = 0.0; }
   }
   grid_reduce<FIN_INIT>(acc, red, blockIdx.x, gridDim.x, sh);
+}
+
+// sum |v|^2 -> FIN (one source per grid row)
+template <typename TB, int FIN>
+__global__ void __launch_bounds__(CGK_NT)
+k_norm2(const TB* __restrict__ v, long n, RedArgs red) {
+  v += blockIdx.y * n;
+  red = red.for_source(blockIdx.y);
+  __shared__ double sh[33];
+  double acc = 0.0;
+  for (long i = (long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long)gridDim.x * blockDim.x)
+    acc += (double)v[i] * (double)v[i];
+  grid_reduce<FIN>(acc, red, blockIdx.x, gridDim.x, sh);
 }
 
 // x += alpha p with the alpha still pending in the CG state (the fused pass A' applies

@@ -16,6 +16,7 @@ struct OpParams {
   R g2_re, g2_im;  // 2 g
   R rho;           // overlap parameter (paper: 1)
   int dagger;      // 0: M, 1: M^dag
+  int pc;          // 1: site-local steps of the preconditioned operator Mtilde = 1 + Y M0^-1 (wz_p01.cuh)
 };
 
 // Device-resident scalars of one CG solve.
@@ -28,6 +29,7 @@ struct CGState {
   double rmax;           // max ||r|| since the last reliable update (G9)
   double tol, delta;
   double true_rr;        // ||b - A x||^2 recomputed
+  double aux;            // scratch norm (||b||^2 of the original system in preconditioned solves)
   int iter, max_iter;
   int n_ru;
   int converged;  // stop rule met
@@ -42,7 +44,7 @@ __device__ __forceinline__ bool cg_active(const CGState* st) {
 }
 
 // What the last block of a reduction does with the total.
-enum { FIN_STORE = 0, FIN_PQ = 1, FIN_RR = 2, FIN_RU = 3, FIN_INIT = 4, FIN_TRUE = 5 };
+enum { FIN_STORE = 0, FIN_PQ = 1, FIN_RR = 2, FIN_RU = 3, FIN_INIT = 4, FIN_TRUE = 5, FIN_AUX = 6 };
 
 template <int FIN>
 __device__ __forceinline__ void cg_finalize(double total, CGState* st, double* store) {
@@ -90,6 +92,8 @@ __device__ __forceinline__ void cg_finalize(double total, CGState* st, double* s
     if (!st->converged && st->iter >= st->max_iter) st->stop = 1;
   } else if (FIN == FIN_TRUE) {
     st->true_rr = total;
+  } else if (FIN == FIN_AUX) {
+    st->aux = total;
   }
 }
 

@@ -55,7 +55,7 @@ struct P01Entry {
 template <typename R>
 struct P23Entry {
   int L2, L3, nt, nhalf;  // nhalf = 2: two components per CTA, grid.z = 2, multiply needs in != out
-  size_t smem;
+  size_t smem, smem_pc;
   void (*fwd)(const P23Args<R>);
   void (*inv)(const P23Args<R>);
   void (*mult)(const P23Args<R>);
@@ -130,7 +130,7 @@ P23Entry<R> make_p23() {
   constexpr int T2 = tune_tpl23<R, L2>::v, T3 = tune_tpl23<R, L3>::v;
   using C = P23Cfg<R, L2, L3, T2, T3, NC>;
   P23Entry<R> e;
-  e.L2 = L2; e.L3 = L3; e.nt = C::NT; e.smem = C::SMEM; e.nhalf = 4 / NC;
+  e.L2 = L2; e.L3 = L3; e.nt = C::NT; e.smem = C::SMEM; e.smem_pc = C::SMEM_PC; e.nhalf = 4 / NC;
   e.fwd = k_p23<R, L2, L3, T2, T3, P23_FFT, +1, NC>;
   e.inv = k_p23<R, L2, L3, T2, T3, P23_FFT, -1, NC>;
   e.mult = k_p23<R, L2, L3, T2, T3, P23_MULT, +1, NC>;
@@ -183,7 +183,7 @@ bool set_smem_kern(const P01Kern<R>& k) {
 }
 template <typename K>
 bool set_smem(K kernel, size_t bytes) {
-  if (bytes <= 48 * 1024) return true;
+  if (bytes <= 32 * 1024) return true;  // static shared memory (tables, reduction scratch) counts against the 48 KB default too
   return cuda_ok(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes),
                  "cudaFuncSetAttribute(MaxDynamicSharedMemorySize)");
 }
@@ -215,6 +215,7 @@ struct wz_plan {
   void *r = nullptr, *p = nullptr, *xs = nullptr;  // plan dtype, max_batch spinors each
   cpx<double>* q128 = nullptr;    // A X in complex128 (reliable updates, true residual), one spinor
   cpx<double>* phi128 = nullptr;  // C64 plans: phi widened
+  cpx<double>* btilde128 = nullptr;  // C64 plans, preconditioned solves: (M0^-1)^dag b in complex128, per source
   double* partials = nullptr;
   unsigned* counter = nullptr;
   CGState* d_state = nullptr;
@@ -292,7 +293,7 @@ wz_status setup_ws(wz_plan* pl, OpWS<R>& ws, int nbatch_t) {
       !set_smem_kern(a->endcg))
     return WZ_ECUDA;
   const auto* b = ws.p23;
-  if (!set_smem(b->fwd, b->smem) || !set_smem(b->inv, b->smem) || !set_smem(b->mult, b->smem))
+  if (!set_smem(b->fwd, b->smem) || !set_smem(b->inv, b->smem) || !set_smem(b->mult, b->smem_pc))
     return WZ_ECUDA;
   std::vector<R> h(2 * 4 * 64, R(0));
   for (int mu = 0; mu < 4; ++mu)
@@ -355,7 +356,7 @@ template <typename R>
 wz_status launch_p23(wz_plan* pl, int kind, const P23Entry<R>& e, void (*k)(const P23Args<R>),
                      const P23Args<R>& args, int nb) {
   const dim3 grid((unsigned)(pl->L[0] * pl->L[1]), (unsigned)nb, (unsigned)e.nhalf);
-  return launch<R>(pl, kind, k, grid, e.nt, e.smem, args);
+  return launch<R>(pl, kind, k, grid, e.nt, args.pc ? e.smem_pc : e.smem, args);
 }
 // Momentum-space multiply pass on the FFT temporary `cur`; in place, or into the other
 // temporary where the kernel works on half the spin components per CTA.  `cur` follows.
@@ -383,11 +384,11 @@ template <>
 OpWS<double>& ws_of<double>(wz_plan* pl) { return pl->wsd; }
 
 template <typename R>
-OpParams<R> make_op(const double m[2], const double g[2], double rho, int dagger) {
+OpParams<R> make_op(const double m[2], const double g[2], double rho, int dagger, int pc = 0) {
   OpParams<R> op;
   op.m_re = (R)m[0]; op.m_im = (R)m[1];
   op.g2_re = (R)(2.0 * g[0]); op.g2_im = (R)(2.0 * g[1]);
-  op.rho = (R)rho; op.dagger = dagger;
+  op.rho = (R)rho; op.dagger = dagger; op.pc = pc;
   return op;
 }
 
@@ -438,7 +439,9 @@ wz_status apply_M_impl(wz_plan* pl, int dagger, const cpx<R>* phi, const double 
 // the solve being active and pass C leaves alpha = rho/<p, A p> in the CG state. -----
 template <typename R>
 wz_status apply_MdagM_impl(wz_plan* pl, const cpx<R>* phi, const double m[2], const double g[2],
-                           double rho, const cpx<R>* in, cpx<R>* out, int nb, bool cg) {
+                           double rho, const cpx<R>* in, cpx<R>* out, int nb, bool cg, bool pc = false) {
+  // pc: Mtilde^dag Mtilde with Mtilde = M M0^-1 = 1 + Y M0^-1: same five passes,
+  // the multiply passes apply M0^-1 / (M0^-1)^dag, the site-local steps use Y alone
   OpWS<R>& ws = ws_of<R>(pl);
   const CGState* gate = cg ? pl->d_state : nullptr;
   const R invV = (R)(1.0 / (double)pl->V);
@@ -449,11 +452,12 @@ wz_status apply_MdagM_impl(wz_plan* pl, const cpx<R>* phi, const double m[2], co
   if ((s = launch_p01<R>(pl, WZ_K_P01_FWD, ws.p01->fwd, a, nb)) != WZ_OK) return s;  // A
   P23Args<R> b{};
   b.nplanes = pl->L[0] * pl->L[1]; b.L1 = pl->L[1]; b.scale = invV;
-  b.tab = ws.tab; b.rho = (R)rho; b.sign = R(1); b.gate = gate;
+  b.tab = ws.tab; b.rho = (R)rho; b.sign = pc ? R(-1) : R(1); b.gate = gate;
+  b.pc = pc ? 1 : 0; b.m_re = (R)m[0]; b.m_im = (R)m[1];
   cpx<R>* cur = ws.t;
   if ((s = mult_pass<R>(pl, ws, b, cur, nb)) != WZ_OK) return s;  // B
   a.in = cur; a.out = cur;
-  a.psi = in; a.phi = phi; a.site_out = ws.chi; a.op = make_op<R>(m, g, rho, 0);
+  a.psi = in; a.phi = phi; a.site_out = ws.chi; a.op = make_op<R>(m, g, rho, 0, pc);
   if (cg) {
     a.red = red_of(pl);
     if ((int)(pl->I / ws.p01->min_nseg()) * 4 > pl->npartials) return WZ_EINVAL;
@@ -462,12 +466,34 @@ wz_status apply_MdagM_impl(wz_plan* pl, const cpx<R>* phi, const double m[2], co
     s = launch_p01<R>(pl, WZ_K_P01_MID, ws.p01->mid, a, nb);
   }
   if (s != WZ_OK) return s;
-  b.sign = R(-1);
+  b.sign = pc ? R(1) : R(-1);
+  b.pc = pc ? 2 : 0;
   if ((s = mult_pass<R>(pl, ws, b, cur, nb)) != WZ_OK) return s;  // D
   a.in = cur; a.out = cur;
   a.red = RedArgs{};
-  a.psi = ws.chi; a.site_out = out; a.op = make_op<R>(m, g, rho, 1);
+  a.psi = ws.chi; a.site_out = out; a.op = make_op<R>(m, g, rho, 1, pc);
   return launch_p01<R>(pl, WZ_K_P01_END, ws.p01->end, a, nb);  // E
+}
+
+// ---- out = M0^-1 in (dagger = 0) or (M0^-1)^dag in, Eq. (7.11): forward FFT, the 4x4 free
+// inverse at every momentum (multiply pass with pc), inverse FFT.  in == out allowed. -------
+template <typename R>
+wz_status apply_M0inv_impl(wz_plan* pl, int dagger, const double m[2], double rho, const cpx<R>* in,
+                           cpx<R>* out, int nb) {
+  OpWS<R>& ws = ws_of<R>(pl);
+  wz_status s;
+  P01Args<R> a{};
+  a.I = pl->I; a.apbc = 1; a.scale = R(1);
+  a.in = in; a.out = ws.t;
+  if ((s = launch_p01<R>(pl, WZ_K_P01_FWD, ws.p01->fwd, a, nb)) != WZ_OK) return s;
+  P23Args<R> b{};
+  b.nplanes = pl->L[0] * pl->L[1]; b.L1 = pl->L[1]; b.scale = (R)(1.0 / (double)pl->V);
+  b.tab = ws.tab; b.rho = (R)rho; b.sign = dagger ? R(1) : R(-1);
+  b.pc = dagger ? 2 : 1; b.m_re = (R)m[0]; b.m_im = (R)m[1];
+  cpx<R>* cur = ws.t;
+  if ((s = mult_pass<R>(pl, ws, b, cur, nb)) != WZ_OK) return s;
+  a.in = cur; a.out = out;  // 1/V already applied by the multiply pass
+  return launch_p01<R>(pl, WZ_K_P01_INV, ws.p01->inv, a, nb);
 }
 
 // ---- one CG iteration = five kernels: A' (x += alpha p pending from the
@@ -477,7 +503,7 @@ wz_status apply_MdagM_impl(wz_plan* pl, const cpx<R>* phi, const double m[2], co
 // state; every kernel is gated on it.  x lags one update: flush_x() before x is used. --
 template <typename R>
 wz_status cg_iteration(wz_plan* pl, const cpx<R>* phi, const double m[2], const double g[2], double rho,
-                       cpx<R>* r, cpx<R>* p, cpx<R>* x, int nb) {
+                       cpx<R>* r, cpx<R>* p, cpx<R>* x, int nb, bool pc) {
   OpWS<R>& ws = ws_of<R>(pl);
   if ((int)(pl->I / ws.p01->min_nseg()) * 4 > pl->npartials) return WZ_EINVAL;
   const R invV = (R)(1.0 / (double)pl->V);
@@ -488,17 +514,19 @@ wz_status cg_iteration(wz_plan* pl, const cpx<R>* phi, const double m[2], const 
   if ((s = launch_p01<R>(pl, WZ_K_P01_FWDCG, ws.p01->fwdcg, a, nb)) != WZ_OK) return s;
   P23Args<R> b{};
   b.nplanes = pl->L[0] * pl->L[1]; b.L1 = pl->L[1]; b.scale = invV;
-  b.tab = ws.tab; b.rho = (R)rho; b.sign = R(1); b.gate = pl->d_state;
+  b.tab = ws.tab; b.rho = (R)rho; b.sign = pc ? R(-1) : R(1); b.gate = pl->d_state;
+  b.pc = pc ? 1 : 0; b.m_re = (R)m[0]; b.m_im = (R)m[1];
   cpx<R>* cur = ws.t;
   if ((s = mult_pass<R>(pl, ws, b, cur, nb)) != WZ_OK) return s;
   a.in = cur; a.out = cur;
-  a.psi = p; a.phi = phi; a.site_out = ws.chi; a.op = make_op<R>(m, g, rho, 0);
+  a.psi = p; a.phi = phi; a.site_out = ws.chi; a.op = make_op<R>(m, g, rho, 0, pc);
   a.red = red_of(pl);
   if ((s = launch_p01<R>(pl, WZ_K_P01_MID, ws.p01->mid_pq, a, nb)) != WZ_OK) return s;
-  b.sign = R(-1);
+  b.sign = pc ? R(1) : R(-1);
+  b.pc = pc ? 2 : 0;
   if ((s = mult_pass<R>(pl, ws, b, cur, nb)) != WZ_OK) return s;
   a.in = cur; a.out = cur;
-  a.psi = ws.chi; a.site_out = nullptr; a.op = make_op<R>(m, g, rho, 1);
+  a.psi = ws.chi; a.site_out = nullptr; a.op = make_op<R>(m, g, rho, 1, pc);
   a.cg_r = r; a.cg_p = p; a.cg_x = x;
   return launch_p01<R>(pl, WZ_K_P01_ENDCG, ws.p01->endcg, a, nb);
 }
@@ -725,9 +753,13 @@ int vec_grid(long n_real, int per_thread) {
 // return at once).  The host looks at the states every kCheckEvery iterations, one
 // chunk behind the GPU, and serves reliable updates source by source.
 // R = iteration precision.  X: caller's complex128 solution buffer.
+// pc: the preconditioned system of PAPER.md:900-921 (Eq. 7.8-7.10): btilde = (M0^-1)^dag b, CG on
+// Mtilde^dag Mtilde xtilde = btilde with the stop rule on ITS residual (reading G15), x = M0^-1 xtilde;
+// info.rel_residual_true is then ||b - M^dag M x|| / ||b|| of the original system.
 template <typename R>
 wz_status cg_batch(wz_plan* pl, const cpx<R>* phi, const cpx<R>* b, cpx<double>* X, const double m[2],
-                   const double g[2], double rho, double tol, int max_iter, int nb, wz_cg_info* info) {
+                   const double g[2], double rho, double tol, int max_iter, int nb, wz_cg_info* info,
+                   bool pc) {
   constexpr bool kRU = (sizeof(R) == 4);
   constexpr int N = vec16<R>::N;
   const long n = 8 * pl->V;       // real entries of one spinor
@@ -746,9 +778,25 @@ wz_status cg_batch(wz_plan* pl, const cpx<R>* phi, const cpx<R>* b, cpx<double>*
   }
   WZ_CUDA(cudaMemcpyAsync(pl->d_state, h.data(), sizeof(CGState) * nb, cudaMemcpyHostToDevice, st));
   WZ_CUDA(cudaStreamSynchronize(st));  // h is pageable host memory
-  {
+  if (!pc) {
     ProfScope ps(pl, WZ_K_OTHER);
-    k_cg_init<R><<<dim3(gv, nb), CGK_NT, 0, st>>>((const R*)b, r, p, kRU ? xs : nullptr, (double*)X, n, red_of(pl));
+    k_cg_init<R, R><<<dim3(gv2, nb), CGK_NT, 0, st>>>((const R*)b, r, p, kRU ? xs : nullptr, (double*)X, n, red_of(pl));
+  } else if constexpr (kRU) {
+    // btilde in complex128, source by source (the complex128 workspace holds one spinor)
+    if (!pl->btilde128 && !dev_alloc(pl, &pl->btilde128, (size_t)pl->max_batch * n1)) return WZ_ENOMEM;
+    for (int j = 0; j < nb; ++j) {
+      {
+        ProfScope ps(pl, WZ_K_OTHER);
+        k_f2d<<<vec_grid(n, 1), CGK_NT, 0, st>>>((double*)pl->q128, (const float*)(b + j * n1), n);
+      }
+      if ((s = apply_M0inv_impl<double>(pl, 1, m, rho, pl->q128, pl->btilde128 + j * n1, 1)) != WZ_OK) return s;
+    }
+    ProfScope ps(pl, WZ_K_OTHER);
+    k_cg_init<R, double><<<dim3(gv2, nb), CGK_NT, 0, st>>>((const double*)pl->btilde128, r, p, xs, (double*)X, n, red_of(pl));
+  } else {
+    if ((s = apply_M0inv_impl<R>(pl, 1, m, rho, b, (cpx<R>*)p, nb)) != WZ_OK) return s;  // btilde -> p
+    ProfScope ps(pl, WZ_K_OTHER);
+    k_cg_init<R, R><<<dim3(gv2, nb), CGK_NT, 0, st>>>((const R*)p, r, p, nullptr, (double*)X, n, red_of(pl));
   }
   WZ_CUDA(cudaGetLastError());
 
@@ -779,10 +827,16 @@ wz_status cg_batch(wz_plan* pl, const cpx<R>* phi, const cpx<R>* b, cpx<double>*
         ProfScope ps(pl, WZ_K_OTHER);
         k_ru_accum<<<dim3(gv4, 1), CGK_NT, 0, st>>>((double*)(X + j * n1), (float*)(xs + j * n), n);
       }
-      wz_status s2 = apply_MdagM_impl<double>(pl, pl->phi128, m, g, rho, X + j * n1, pl->q128, 1, false);
+      wz_status s2 = apply_MdagM_impl<double>(pl, pl->phi128, m, g, rho, X + j * n1, pl->q128, 1, false, pc);
       if (s2 != WZ_OK) return s2;
       ProfScope ps(pl, WZ_K_OTHER);
-      if (update_r)
+      if (pc) {  // rhs of the preconditioned system: btilde, kept in complex128
+        const double* bt = (const double*)(pl->btilde128 + j * n1);
+        if (update_r)
+          k_resid<double, float, FIN_RU><<<dim3(gv2, 1), CGK_NT, 0, st>>>(bt, (const double*)pl->q128, (float*)(r + j * n), n, ra);
+        else
+          k_resid<double, float, FIN_TRUE><<<dim3(gv2, 1), CGK_NT, 0, st>>>(bt, (const double*)pl->q128, nullptr, n, ra);
+      } else if (update_r)
         k_resid<float, float, FIN_RU><<<dim3(gv2, 1), CGK_NT, 0, st>>>(
             (const float*)(b + j * n1), (const double*)pl->q128, (float*)(r + j * n), n, ra);
       else
@@ -806,9 +860,9 @@ wz_status cg_batch(wz_plan* pl, const cpx<R>* phi, const cpx<R>* b, cpx<double>*
     while (inflight < 2) {
       for (int it = 0; it < kCheckEvery; ++it) {
         if constexpr (kRU)
-          s = cg_iteration<R>(pl, phi, m, g, rho, (cpx<R>*)r, (cpx<R>*)p, (cpx<R>*)xs, nb);
+          s = cg_iteration<R>(pl, phi, m, g, rho, (cpx<R>*)r, (cpx<R>*)p, (cpx<R>*)xs, nb, pc);
         else
-          s = cg_iteration<R>(pl, phi, m, g, rho, (cpx<R>*)r, (cpx<R>*)p, (cpx<R>*)X, nb);
+          s = cg_iteration<R>(pl, phi, m, g, rho, (cpx<R>*)r, (cpx<R>*)p, (cpx<R>*)X, nb, pc);
         if (s != WZ_OK) return s;
       }
       WZ_CUDA(cudaMemcpyAsync(pl->h_state + slot_w * pl->max_batch, pl->d_state, sizeof(CGState) * nb,
@@ -838,11 +892,39 @@ wz_status cg_batch(wz_plan* pl, const cpx<R>* phi, const cpx<R>* b, cpx<double>*
   WZ_CUDA(cudaMemcpy(fin.data(), pl->d_state, sizeof(CGState) * nb, cudaMemcpyDeviceToHost));
   for (int j = 0; j < nb; ++j) {
     if ((s = flush_x(j)) != WZ_OK) return s;
-    // true residual at exit: complex64 solves that converged carry it from their last
-    // reliable update; everything else recomputes it now
-    if (kRU && fin[j].converged) continue;
     if (fin[j].bnorm2 == 0.0) continue;
-    if ((s = residual128(j, kRU)) != WZ_OK) return s;  // C64, not converged: fold xs into X first
+    if (!pc) {
+      // true residual at exit: complex64 solves that converged carry it from their last
+      // reliable update; everything else recomputes it now
+      if (kRU && fin[j].converged) continue;
+      if ((s = residual128(j, kRU)) != WZ_OK) return s;  // C64, not converged: fold xs into X first
+      continue;
+    }
+    // preconditioned solve: X_j holds xtilde (+ xs still to be folded in for C64 solves that stopped)
+    if constexpr (kRU) {
+      if (!fin[j].converged) {
+        ProfScope ps(pl, WZ_K_OTHER);
+        k_ru_accum<<<dim3(gv4, 1), CGK_NT, 0, st>>>((double*)(X + j * n1), (float*)(xs + j * n), n);
+      }
+    }
+    // x = M0^-1 xtilde in complex128, then the residual of the ORIGINAL system against b
+    RedArgs ra = red_of(pl).for_source(j);
+    if constexpr (kRU) {
+      if ((s = apply_M0inv_impl<double>(pl, 0, m, rho, X + j * n1, X + j * n1, 1)) != WZ_OK) return s;
+      if ((s = apply_MdagM_impl<double>(pl, pl->phi128, m, g, rho, X + j * n1, pl->q128, 1, false)) != WZ_OK) return s;
+      ProfScope ps(pl, WZ_K_OTHER);
+      k_resid<float, float, FIN_TRUE><<<dim3(gv2, 1), CGK_NT, 0, st>>>((const float*)(b + j * n1), (const double*)pl->q128, nullptr, n, ra);
+      k_norm2<float, FIN_AUX><<<dim3(gv2, 1), CGK_NT, 0, st>>>((const float*)(b + j * n1), n, ra);
+      pl->launches++;
+    } else {
+      if ((s = apply_M0inv_impl<double>(pl, 0, m, rho, X + j * n1, X + j * n1, 1)) != WZ_OK) return s;
+      if ((s = apply_MdagM_impl<double>(pl, (const cpx<double>*)phi, m, g, rho, X + j * n1, pl->q128, 1, false)) != WZ_OK) return s;
+      ProfScope ps(pl, WZ_K_OTHER);
+      k_resid<double, double, FIN_TRUE><<<dim3(gv2, 1), CGK_NT, 0, st>>>((const double*)(b + j * n1), (const double*)pl->q128, nullptr, n, ra);
+      k_norm2<double, FIN_AUX><<<dim3(gv2, 1), CGK_NT, 0, st>>>((const double*)(b + j * n1), n, ra);
+      pl->launches++;
+    }
+    WZ_CUDA(cudaGetLastError());
   }
   WZ_CUDA(cudaStreamSynchronize(st));
   WZ_CUDA(cudaMemcpy(fin.data(), pl->d_state, sizeof(CGState) * nb, cudaMemcpyDeviceToHost));
@@ -851,21 +933,22 @@ wz_status cg_batch(wz_plan* pl, const cpx<R>* phi, const cpx<R>* b, cpx<double>*
     info[j].reliable_updates = ru_served[j];
     info[j].converged = fin[j].converged;
     info[j].rel_residual_recursive = fin[j].bnorm > 0 ? std::sqrt(fin[j].rr) / fin[j].bnorm : 0.0;
-    info[j].rel_residual_true =
-        fin[j].bnorm > 0 ? std::sqrt(fin[j].true_rr < 0 ? 0.0 : fin[j].true_rr) / fin[j].bnorm : 0.0;
+    const double bref = pc ? std::sqrt(fin[j].aux) : fin[j].bnorm;  // ||b|| of the system true_rr refers to
+    info[j].rel_residual_true = bref > 0 ? std::sqrt(fin[j].true_rr < 0 ? 0.0 : fin[j].true_rr) / bref : 0.0;
   }
   return WZ_OK;
 }
 
 }  // namespace
 
-extern "C" wz_status wz_cg_solve(wz_plan* pl, const void* phi, const void* b, void* x,
-                                 const double m[2], const double g[2], double rho, double tol,
-                                 int max_iter, int nbatch, wz_cg_info* info) {
+static wz_status cg_solve_any(wz_plan* pl, const void* phi, const void* b, void* x, const double m[2],
+                              const double g[2], double rho, double tol, int max_iter, int nbatch,
+                              wz_cg_info* info, bool pc) {
   g_err[0] = 0;
   if (!pl || !phi || !b || !x || !m || !g || !info) return WZ_EINVAL;
   if (!(rho > 0.0 && rho < 2.0) || !(tol > 0.0) || max_iter < 0) return WZ_EINVAL;
   if (nbatch < 0 || nbatch > pl->max_batch) return WZ_EINVAL;
+  if (pc && m[0] == 0.0 && m[1] == 0.0) return WZ_EINVAL;  // M0 must be invertible at every momentum
   if (nbatch == 0) return WZ_OK;
   wz_status s;
   if (pl->dtype == WZ_C64) {
@@ -876,13 +959,53 @@ extern "C" wz_status wz_cg_solve(wz_plan* pl, const void* phi, const void* b, vo
     }
     WZ_CUDA(cudaGetLastError());
     s = cg_batch<float>(pl, (const cpx<float>*)phi, (const cpx<float>*)b, (cpx<double>*)x, m, g, rho, tol,
-                        max_iter, nbatch, info);
+                        max_iter, nbatch, info, pc);
   } else {
     s = cg_batch<double>(pl, (const cpx<double>*)phi, (const cpx<double>*)b, (cpx<double>*)x, m, g, rho, tol,
-                         max_iter, nbatch, info);
+                         max_iter, nbatch, info, pc);
   }
   if (s != WZ_OK) return s;
   for (int j = 0; j < nbatch; ++j)
     if (!info[j].converged) return WZ_ENOTCONVERGED;
   return WZ_OK;
 }
+
+extern "C" {
+
+wz_status wz_cg_solve(wz_plan* pl, const void* phi, const void* b, void* x, const double m[2],
+                      const double g[2], double rho, double tol, int max_iter, int nbatch, wz_cg_info* info) {
+  return cg_solve_any(pl, phi, b, x, m, g, rho, tol, max_iter, nbatch, info, false);
+}
+
+wz_status wz_cg_solve_pc(wz_plan* pl, const void* phi, const void* b, void* x, const double m[2],
+                         const double g[2], double rho, double tol, int max_iter, int nbatch, wz_cg_info* info) {
+  return cg_solve_any(pl, phi, b, x, m, g, rho, tol, max_iter, nbatch, info, true);
+}
+
+wz_status wz_apply_M0inv(wz_plan* pl, int dagger, const double m[2], double rho, const void* in, void* out,
+                         int nbatch) {
+  g_err[0] = 0;
+  if (!pl || !m || !in || !out) return WZ_EINVAL;
+  if (!(rho > 0.0 && rho < 2.0) || (m[0] == 0.0 && m[1] == 0.0)) return WZ_EINVAL;
+  if (nbatch < 0 || nbatch > pl->max_batch) return WZ_EINVAL;
+  if (nbatch == 0) return WZ_OK;
+  if (pl->dtype == WZ_C64)
+    return apply_M0inv_impl<float>(pl, dagger ? 1 : 0, m, rho, (const cpx<float>*)in, (cpx<float>*)out, nbatch);
+  return apply_M0inv_impl<double>(pl, dagger ? 1 : 0, m, rho, (const cpx<double>*)in, (cpx<double>*)out, nbatch);
+}
+
+wz_status wz_apply_MtdagMt(wz_plan* pl, const void* phi, const double m[2], const double g[2], double rho,
+                           const void* in, void* out, int nbatch) {
+  g_err[0] = 0;
+  wz_status s = check_op(pl, phi, m, g, rho, in, out, nbatch);
+  if (s != WZ_OK) return s;
+  if (m[0] == 0.0 && m[1] == 0.0) return WZ_EINVAL;
+  if (nbatch == 0) return WZ_OK;
+  if (pl->dtype == WZ_C64)
+    return apply_MdagM_impl<float>(pl, (const cpx<float>*)phi, m, g, rho, (const cpx<float>*)in,
+                                   (cpx<float>*)out, nbatch, false, true);
+  return apply_MdagM_impl<double>(pl, (const cpx<double>*)phi, m, g, rho, (const cpx<double>*)in,
+                                  (cpx<double>*)out, nbatch, false, true);
+}
+
+}  // extern "C"

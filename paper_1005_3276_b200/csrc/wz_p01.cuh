@@ -257,7 +257,15 @@ k_p01(const P01Args<R> a) {
     } else {
       // ---- site-local term of Eq. (2.19): + (m + 2 g phi) P+ psi + (m + 2 g phi)^* P- psi,
       //      spin 0,1 = P-, spin 2,3 = P+; M^dag swaps w and w^* ----
+      // Preconditioned operator (op.pc): Mtilde = M M0^-1 = 1 + Y M0^-1 with
+      // Y = 2 g phi P+ + 2 g^* phi^* P-, so the same passes serve with other site-local formulas:
+      //   MID:  w = psi + Y t  (stored, ||w||^2),  then the forward half transforms Y^dag w;
+      //   END / ENDCG:  q = t + w  (no phi).
       const bool use_conj = (comp < 2) != (a.op.dagger != 0);
+      const bool pc = a.op.pc != 0;
+      const bool pc_swap = pc && MODE == P01_MID;   // base = psi, multiplied = t
+      const bool pc_unit = pc && MODE != P01_MID;   // coefficient 1
+      const R m_re = pc ? R(0) : a.op.m_re, m_im = pc ? R(0) : a.op.m_im;
       const cpx<R>* gpsi = a.psi + (long)f * V + i0;
       const cpx<R>* gphi = a.phi + i0;
       cpx<R>* gso = a.site_out + (long)f * V + i0;
@@ -283,9 +291,10 @@ k_p01(const P01Args<R> a) {
             const R alpha = (R)a.red.st[src].alpha;
 #pragma unroll
             for (int c = 0; c < CH; ++c) {
-              cpx<R> w = {a.op.m_re + a.op.g2_re * ph[c].re - a.op.g2_im * ph[c].im,
-                          a.op.m_im + a.op.g2_re * ph[c].im + a.op.g2_im * ph[c].re};
+              cpx<R> w = {m_re + a.op.g2_re * ph[c].re - a.op.g2_im * ph[c].im,
+                          m_im + a.op.g2_re * ph[c].im + a.op.g2_im * ph[c].re};
               if (use_conj) w.im = -w.im;
+              if (pc_unit) w = {R(1), R(0)};
               cpx<R> q = x[k0 + c];
               q.re += w.re * ps[c].re - w.im * ps[c].im;
               q.im += w.re * ps[c].im + w.im * ps[c].re;
@@ -296,13 +305,17 @@ k_p01(const P01Args<R> a) {
           } else {
 #pragma unroll
             for (int c = 0; c < CH; ++c) {
-              cpx<R> w = {a.op.m_re + a.op.g2_re * ph[c].re - a.op.g2_im * ph[c].im,
-                          a.op.m_im + a.op.g2_re * ph[c].im + a.op.g2_im * ph[c].re};
+              cpx<R> w = {m_re + a.op.g2_re * ph[c].re - a.op.g2_im * ph[c].im,
+                          m_im + a.op.g2_re * ph[c].im + a.op.g2_im * ph[c].re};
               if (use_conj) w.im = -w.im;
-              cpx<R> v = x[k0 + c];
-              v.re += w.re * ps[c].re - w.im * ps[c].im;
-              v.im += w.re * ps[c].im + w.im * ps[c].re;
-              x[k0 + c] = v;
+              if (pc_unit) w = {R(1), R(0)};
+              const cpx<R> base = pc_swap ? ps[c] : x[k0 + c];
+              const cpx<R> mul = pc_swap ? x[k0 + c] : ps[c];
+              cpx<R> v = base;
+              v.re += w.re * mul.re - w.im * mul.im;
+              v.im += w.re * mul.im + w.im * mul.re;
+              // value that enters the forward half (MID): v, or Y^dag v for the preconditioned operator
+              x[k0 + c] = pc_swap ? cpx<R>{w.re * v.re + w.im * v.im, w.re * v.im - w.im * v.re} : v;
               gso[off[c]] = v;
               if (FIN != FIN_STORE || a.red.partials)
                 acc += (double)v.re * (double)v.re + (double)v.im * (double)v.im;

@@ -16,6 +16,10 @@
 namespace wz {
 
 enum { P23_FFT = 0, P23_MULT = 1 };
+// Preconditioner (Eq. 7.11): with args.pc set, the multiply applies the free
+// inverse  M0^-1(p) = (-i c gamma.sin p + m^* P+ + m P-) / (c^2 sum sin^2 p + |m|^2)  (pc = 1) or its
+// conjugate transpose M0(p) / (...) (pc = 2) instead of +-Dslash(p): same off-diagonal 2x2 blocks
+// scaled by -+c/D, plus the diagonal m/D, m^*/D on the thread's own component.
 
 // c(p) = k / (s + Mw) with s = sqrt(Mw^2 + S2), k = 2 rho sign / V; for Mw < 0 the
 // cancellation-free form k (s - Mw) / S2 = k (s + |Mw|) / S2.  float: rsqrt/rcp approximations
@@ -41,6 +45,8 @@ struct P23Args {
   const R* tab;       // momentum tables [2][4][64]: sin p_mu(n), sin^2(p_mu(n)/2)
   R rho;
   R sign;             // +1: Dslash, -1: Dslash^dag = -Dslash
+  int pc;             // 0: Dslash;  1: M0^-1;  2: (M0^-1)^dag
+  R m_re, m_im;       // m (pc only)
   const CGState* gate;  // [nbatch], indexed by blockIdx.y
 };
 
@@ -59,8 +65,9 @@ struct P23Cfg {
   static constexpr int NT = NC * NTC;
   static constexpr int PITCH = L3 + 1;            // row pitch (elements)
   static constexpr int CPITCH = L2 * PITCH + 4;   // component pitch
-  static constexpr int CF_ELEMS = L2 * PITCH;  // c(p) of the plane, computed once per site and shared by the components
+  static constexpr int CF_ELEMS = L2 * PITCH;  // per-site factor(s) of the multiply, computed once, shared by the components
   static constexpr size_t SMEM = sizeof(cpx<R>) * NC * (size_t)CPITCH + sizeof(R) * CF_ELEMS;
+  static constexpr size_t SMEM_PC = SMEM + sizeof(R) * CF_ELEMS;  // + the diagonal factor (launches with args.pc)
 };
 
 template <typename R, int L2, int L3, int T2, int T3, int MODE, int DIR, int NC = 4>
@@ -72,7 +79,8 @@ k_p23(const P23Args<R> a) {
   constexpr int D1 = (MODE == P23_MULT) ? +1 : DIR;  // direction of the first half
   extern __shared__ __align__(16) unsigned char smem_raw[];
   cpx<R>* sm = reinterpret_cast<cpx<R>*>(smem_raw);
-  R* cfs = reinterpret_cast<R*>(sm + NC * CPITCH);
+  R* cfs = reinterpret_cast<R*>(sm + NC * CPITCH);  // off-diagonal factor
+  R* dgs = cfs + Cfg::CF_ELEMS;                     // diagonal factor (pc launches only)
   __shared__ R tb[2 * 4 * 64];
 
   if (a.gate && !cg_active(a.gate + blockIdx.y)) return;
@@ -146,7 +154,16 @@ k_p23(const P23Args<R> a) {
         for (int k = cl * (NR3 / NC); k < (cl + 1) * (NR3 / NC); ++k) {
           const int n3 = G3i::in_pos(k, jB);
           const R s3 = sn[3 * 64 + n3];
-          cfs[n2B * PITCH + n3] = overlap_c(Mw012 - R(2) * sh[3 * 64 + n3], S012 + s3 * s3, kk);
+          const R S2 = S012 + s3 * s3;
+          const R cf = overlap_c(Mw012 - R(2) * sh[3 * 64 + n3], S2, kk);
+          if (a.pc) {  // cf carries rho-scaling and 1/V; c = cf / a.scale;  D = c^2 S2 + |m|^2
+            const R c = cf / a.scale;
+            const R invD = R(1) / (c * c * S2 + a.m_re * a.m_re + a.m_im * a.m_im);
+            cfs[n2B * PITCH + n3] = cf * invD;
+            dgs[n2B * PITCH + n3] = a.scale * invD;
+          } else {
+            cfs[n2B * PITCH + n3] = cf;
+          }
         }
       }
     }
@@ -184,6 +201,9 @@ k_p23(const P23Args<R> a) {
       else if (cc == 1) { A0 = -s2; A1 = s1;   A3 = R(0);  B0 = s0;  B1 = R(0); B3 = R(-1); }
       else if (cc == 2) { A0 = s0;  A1 = R(0); A3 = R(-1); B0 = -s2; B1 = -s1;  B3 = R(0); }
       else              { A0 = s2;  A1 = -s1;  A3 = R(0);  B0 = s0;  B1 = R(0); B3 = R(1); }
+      // pc = 1 (M0^-1): upper components carry m, lower m^*;  pc = 2 (dagger): the other way round
+      const R dm_re = a.m_re;
+      const R dm_im = ((cc < 2) == (a.pc == 1)) ? a.m_im : -a.m_im;
       // inputs of output component cc: (psi_2, psi_3) for cc < 2, (psi_0, psi_1) otherwise;
       // with NC = 2 those are the two planes this CTA holds
       const cpx<R>* sa = sm + ((NC == 4) ? ((cc < 2) ? 2 : 0) : 0) * CPITCH + n2 * PITCH;
@@ -197,7 +217,15 @@ k_p23(const P23Args<R> a) {
         const R Ai = A1 + A3 * s3, Bi = B1 + B3 * s3;
         const R tr = A0 * pa.re - Ai * pa.im + B0 * pb.re - Bi * pb.im;
         const R ti = A0 * pa.im + Ai * pa.re + B0 * pb.im + Bi * pb.re;
-        y[k] = {-cf * ti, cf * tr};  // times i
+        cpx<R> o = {-cf * ti, cf * tr};  // times i
+        if (a.pc) {  // + (m or m^*) / D on the own component
+          const cpx<R> own = smc[n2 * PITCH + n3];
+          const R dg = dgs[n2 * PITCH + n3];
+          const R dr = dm_re * dg, di = dm_im * dg;
+          o.re += dr * own.re - di * own.im;
+          o.im += dr * own.im + di * own.re;
+        }
+        y[k] = o;
       }
     }
     G3::run(y, jB);

@@ -24,6 +24,7 @@ EXPORTS = [
     "wz_supported", "wz_plan_workspace_bytes", "wz_fft4d", "wz_apply_M", "wz_apply_MdagM",
     "wz_cg_solve", "wz_plan_launch_count", "wz_plan_reset_launch_count",
     "wz_plan_profile", "wz_plan_profile_read", "wz_kind_name",
+    "wz_apply_M0inv", "wz_apply_MtdagMt", "wz_cg_solve_pc",
 ]
 
 
@@ -75,6 +76,9 @@ def lib() -> ctypes.CDLL:
         L.wz_apply_M.argtypes = [vp, ci, vp, d2, d2, cd, vp, vp, ci]
         L.wz_apply_MdagM.argtypes = [vp, vp, d2, d2, cd, vp, vp, ci]
         L.wz_cg_solve.argtypes = [vp, vp, vp, vp, d2, d2, cd, cd, ci, ci, ctypes.POINTER(_CGInfo)]
+        L.wz_cg_solve_pc.argtypes = L.wz_cg_solve.argtypes
+        L.wz_apply_M0inv.argtypes = [vp, ci, d2, cd, vp, vp, ci]
+        L.wz_apply_MtdagMt.argtypes = [vp, vp, d2, d2, cd, vp, vp, ci]
         L.wz_plan_profile.argtypes = [vp, ci]
         L.wz_plan_profile_read.argtypes = [vp, d2, ctypes.POINTER(ctypes.c_ulonglong)]
         L.wz_kind_name.restype = ctypes.c_char_p
@@ -200,16 +204,37 @@ class Plan:
                                     psi.data_ptr(), out.data_ptr(), nb))
         return out
 
+    def apply_M0inv(self, psi, m, rho: float = 1.0, dagger: bool = False, out=None):
+        nb = self._spinor(psi)
+        if out is None:
+            out = torch.empty_like(psi)
+        self._spinor(out)
+        _check(lib().wz_apply_M0inv(self._h, int(bool(dagger)), _c2(m), float(rho), psi.data_ptr(),
+                                    out.data_ptr(), nb))
+        return out
+
+    def apply_MtdagMt(self, phi, psi, m, g, rho: float = 1.0, out=None):
+        nb = self._spinor(psi)
+        self._phi(phi)
+        if out is None:
+            out = torch.empty_like(psi)
+        self._spinor(out)
+        _check(lib().wz_apply_MtdagMt(self._h, phi.data_ptr(), _c2(m), _c2(g), float(rho),
+                                      psi.data_ptr(), out.data_ptr(), nb))
+        return out
+
     def cg_solve(self, phi, b, m, g, rho: float = 1.0, tol: float = 1e-6, max_iter: int = 100000,
-                 out=None, raise_on_fail: bool = True):
-        """Solve M^dag M x = b per source.  Returns (x complex128, [CGInfo])."""
+                 out=None, raise_on_fail: bool = True, precondition: bool = False):
+        """Solve M^dag M x = b per source (precondition=True: through the free-inverse
+        preconditioned system, wz_cg_solve_pc).  Returns (x complex128, [CGInfo])."""
         nb = self._spinor(b)
         self._phi(phi)
         if out is None:
             out = torch.empty(b.shape, dtype=torch.complex128, device=b.device)
         self._spinor(out, torch.complex128)
         infos = (_CGInfo * nb)()
-        st = lib().wz_cg_solve(self._h, phi.data_ptr(), b.data_ptr(), out.data_ptr(), _c2(m), _c2(g),
+        fn = lib().wz_cg_solve_pc if precondition else lib().wz_cg_solve
+        st = fn(self._h, phi.data_ptr(), b.data_ptr(), out.data_ptr(), _c2(m), _c2(g),
                                float(rho), float(tol), int(max_iter), nb, infos)
         if st != WZ_OK and not (st == WZ_ENOTCONVERGED and not raise_on_fail):
             _check(st)

@@ -305,3 +305,67 @@ def test_config5_solve_true_residual(wz, orc, inp, key):
               b.astype(np.complex128))
     assert res <= cfg["tol"], res
     assert abs(res - info.rel_residual_true) <= 0.02 * cfg["tol"]
+
+
+# ---- NEXT-1: free-inverse preconditioning ----
+
+@pytest.mark.parametrize("dims", [(4, 4, 4, 4), (8, 4, 16, 8), (16, 16, 16, 16), (48, 24, 24, 24)])
+@pytest.mark.parametrize("dtype", ["c128", "c64"])
+def test_M0inv_and_MtdagMt_vs_oracle(wz, orc, inp, dims, dtype):
+    phi, b = _fields(inp, dims, dtype, nsrc=2)
+    m, g, rho = 0.3 + 0.1j, 0.4 - 0.2j, 1.0
+    plan = wz.Plan(dims, dtype, 2)
+    d_b, d_phi = torch.from_numpy(b).cuda(), torch.from_numpy(phi).cuda()
+    b128, phi128 = b.astype(np.complex128), phi.astype(np.complex128)
+    for dagger in (False, True):
+        out = plan.apply_M0inv(d_b, m, rho, dagger).cpu().numpy()
+        ref = np.stack([orc.apply_M0inv(dims, b128[j], m, rho, dagger) for j in range(2)])
+        assert rel(out, ref) <= TOL[dtype]
+    out = plan.apply_MtdagMt(d_phi, d_b, m, g, rho).cpu().numpy()
+    ref = np.stack([orc.apply_Mtilde(phi128, orc.apply_Mtilde(phi128, b128[j], m, g, rho), m, g, rho, dagger=True)
+                    for j in range(2)])
+    assert rel(out, ref) <= TOL[dtype]
+
+
+@pytest.mark.parametrize("dims,dtype,tol", [((8, 8, 8, 8), "c128", 1e-12), ((8, 8, 8, 8), "c64", 1e-6),
+                                            ((16, 16, 16, 16), "c64", 1e-6)])
+def test_cg_pc_weak_coupling_like_table_VI(wz, orc, inp, dims, dtype, tol):
+    """Table VI regime (m = 1, g = 1/5): the preconditioned solve converges in 8 (1e-6) to 15 (1e-12)
+    iterations; counts within +-2 of the oracle's, true residual of the ORIGINAL system recomputed
+    by the oracle."""
+    m, g, rho = 1.0, 0.2, 1.0
+    phi = inp.make_phi(5, dims, 0.5, NPDT[dtype])
+    b = inp.make_sources(5, 2, dims, NPDT[dtype])
+    plan = wz.Plan(dims, dtype, 2)
+    x, infos = plan.cg_solve(torch.from_numpy(phi).cuda(), torch.from_numpy(b).cuda(), m, g, rho, tol, 2000,
+                             precondition=True)
+    x = x.cpu().numpy()
+    phi128 = phi.astype(np.complex128)
+    for j in range(2):
+        bj = b[j].astype(np.complex128)
+        xo, io = orc.cg_pc(phi128, bj, m, g, rho, tol, 2000)
+        true_res = rel(orc.apply_MdagM(phi128, x[j], m, g, rho), bj)
+        print("pc %s %s: iterations gpu=%d oracle=%d true residual %.2e (oracle %.2e)"
+              % (dims, dtype, infos[j].iterations, io.iterations, true_res, io.rel_residual_true))
+        assert infos[j].converged and io.converged
+        assert abs(infos[j].iterations - io.iterations) <= 2
+        assert infos[j].iterations <= 25
+        assert abs(true_res - infos[j].rel_residual_true) <= 0.05 * max(true_res, tol)
+        assert true_res <= 20 * tol  # original-system residual: same order as the preconditioned one
+        assert rel(x[j], xo) <= (1e-9 if dtype == "c128" else 1e-4)
+
+
+def test_cg_pc_strong_coupling_config2(wz, orc, inp):
+    """Config 2 parameters (g sigma = 0.3, m = 0.05): preconditioning still has to give the same x."""
+    cfg = inp.CONFIGS[2]
+    dims = cfg["dims"]
+    phi = inp.make_phi(cfg["seed"], dims, cfg["sigma"])
+    b = inp.make_source(cfg["seed"], 0, dims)
+    plan = wz.Plan(dims, "c128", 1)
+    d_phi, d_b = torch.from_numpy(phi).cuda(), torch.from_numpy(b).cuda()
+    x0, i0 = plan.cg_solve(d_phi, d_b, cfg["m"], cfg["g"], 1.0, 1e-10, 20000)
+    x1, i1 = plan.cg_solve(d_phi, d_b, cfg["m"], cfg["g"], 1.0, 1e-10, 20000, precondition=True)
+    print("config 2: plain %d iterations, preconditioned %d" % (i0[0].iterations, i1[0].iterations))
+    res = rel(orc.apply_MdagM(phi, x1.cpu().numpy(), cfg["m"], cfg["g"], 1.0), b)
+    assert i1[0].converged and res <= 1e-7
+    assert rel(x1.cpu().numpy(), x0.cpu().numpy()) <= 1e-6

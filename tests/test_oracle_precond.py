@@ -70,6 +70,14 @@ def test_weak_coupling_iteration_counts_like_table_VI(orc):
     _, pc6 = orc.cg_pc(phi, b, 1.0, 0.2, 1.0, 1e-6, 5000)
     _, pc12 = orc.cg_pc(phi, b, 1.0, 0.2, 1.0, 1e-12, 5000)
     assert pc6.converged and pc12.converged and plain.converged
-    assert pc6.iterations <= 12 and pc12.iterations <= 25
+    import os
+    gold = {}
+    for line in open(os.path.join(os.path.dirname(__file__), "golden", "table_VI_pc_iterations.txt")):
+        if line.strip() and not line.startswith("#"):
+            t, it = line.split()
+            gold[float(t)] = int(it)
+    # the paper prints 8 and 15, independent of the lattice size; phi differs (synthetic), so +-2 / +-3
+    assert abs(pc6.iterations - gold[1e-6]) <= 2, pc6.iterations
+    assert abs(pc12.iterations - gold[1e-12]) <= 3, pc12.iterations
     assert plain.iterations >= 3 * pc6.iterations
     assert pc6.rel_residual_true < 1e-5
