@@ -319,6 +319,9 @@ def run_wz(args):
                    "all_converged": conv, "worst_true_residual": worst_true,
                    "cg_algorithmic_GBs": 18.5 * u / (per_iter_us * 1e-6) / 1e9})
 
+    if not args.no_extras:
+        extras["preconditioned"] = time_preconditioned(plan, d_phi, d_b, d_x, cfg, secs / args.steps)
+
     cpu = None
     if not args.no_cpu_baseline and world == 1:
         ips, threads, text, _ = oracle_sample(cfg, oracle_iters_for(cfg))
@@ -414,6 +417,35 @@ def time_pieces_batched(plan, d_phi, d_b, m, g, rho, u, peak):
                                   "frac_of_peak": nu * u / med / 1e9 / peak, "sources": nb}
     res["matvecs_per_s_batched"] = 1.0 / (res["apply_MdagM_batched"]["us_median_per_source"] * 1e-6)
     return res
+
+
+def time_preconditioned(plan, d_phi, d_b, d_x, cfg, plain_secs):
+    """NEXT-1 (Table VI): the same batch through wz_cg_solve_pc, at the
+    workload's own (strong) coupling and at the paper's Table VI parameters m = 1, g = 1/5."""
+    import torch
+
+    def solve(m, g, pc):
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        _, infos = plan.cg_solve(d_phi, d_b, m, g, cfg["rho"], cfg["tol"], 200000, out=d_x,
+                                 raise_on_fail=False, precondition=pc)
+        b.record()
+        b.synchronize()
+        return a.elapsed_time(b) * 1e-3, infos
+
+    t_pc, i_pc = solve(cfg["m"], cfg["g"], True)
+    t_w0, i_w0 = solve(1.0, 0.2, False)
+    t_w1, i_w1 = solve(1.0, 0.2, True)
+    return {
+        "workload_coupling": {"plain_s": plain_secs, "pc_s": t_pc, "speedup": plain_secs / t_pc,
+                              "pc_iterations": [i.iterations for i in i_pc],
+                              "pc_worst_true_residual": max(i.rel_residual_true for i in i_pc),
+                              "pc_all_converged": all(i.converged for i in i_pc)},
+        "table_VI_parameters_m1_g0.2": {"plain_s": t_w0, "pc_s": t_w1, "speedup": t_w0 / t_w1,
+                                        "plain_iterations": [i.iterations for i in i_w0],
+                                        "pc_iterations": [i.iterations for i in i_w1],
+                                        "paper": "Table VI, GTX 285: 8 iterations (single), speed-up 34-62"},
+    }
 
 
 def main():
