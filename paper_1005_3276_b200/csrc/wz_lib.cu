@@ -59,6 +59,7 @@ struct P23Entry {
   void (*fwd)(const P23Args<R>);
   void (*inv)(const P23Args<R>);
   void (*mult)(const P23Args<R>);
+  void (*multpc)(const P23Args<R>);  // multiply with the free inverse (preconditioner)
 };
 
 // ---- tuning: lanes per lattice line (TPL) and tile width (NSEG) -------------------
@@ -134,6 +135,7 @@ P23Entry<R> make_p23() {
   e.fwd = k_p23<R, L2, L3, T2, T3, P23_FFT, +1, NC>;
   e.inv = k_p23<R, L2, L3, T2, T3, P23_FFT, -1, NC>;
   e.mult = k_p23<R, L2, L3, T2, T3, P23_MULT, +1, NC>;
+  e.multpc = k_p23<R, L2, L3, T2, T3, P23_MULTPC, +1, NC>;
   return e;
 }
 
@@ -293,7 +295,8 @@ wz_status setup_ws(wz_plan* pl, OpWS<R>& ws, int nbatch_t) {
       !set_smem_kern(a->endcg))
     return WZ_ECUDA;
   const auto* b = ws.p23;
-  if (!set_smem(b->fwd, b->smem) || !set_smem(b->inv, b->smem) || !set_smem(b->mult, b->smem_pc))
+  if (!set_smem(b->fwd, b->smem) || !set_smem(b->inv, b->smem) || !set_smem(b->mult, b->smem) ||
+      !set_smem(b->multpc, b->smem_pc))
     return WZ_ECUDA;
   std::vector<R> h(2 * 4 * 64, R(0));
   for (int mu = 0; mu < 4; ++mu)
@@ -364,7 +367,7 @@ template <typename R>
 wz_status mult_pass(wz_plan* pl, OpWS<R>& ws, P23Args<R>& b, cpx<R>*& cur, int nb) {
   cpx<R>* dst = (ws.p23->nhalf == 2) ? ((cur == ws.t) ? ws.t2 : ws.t) : cur;
   b.in = cur; b.out = dst;
-  wz_status s = launch_p23<R>(pl, WZ_K_P23_MULT, *ws.p23, ws.p23->mult, b, nb);
+  wz_status s = launch_p23<R>(pl, WZ_K_P23_MULT, *ws.p23, b.pc ? ws.p23->multpc : ws.p23->mult, b, nb);
   cur = dst;
   return s;
 }

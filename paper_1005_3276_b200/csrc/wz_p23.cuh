@@ -15,7 +15,7 @@
 
 namespace wz {
 
-enum { P23_FFT = 0, P23_MULT = 1 };
+enum { P23_FFT = 0, P23_MULT = 1, P23_MULTPC = 2 };  // MULTPC: the multiply with args.pc = 1 or 2
 // Preconditioner (Eq. 7.11): with args.pc set, the multiply applies the free
 // inverse  M0^-1(p) = (-i c gamma.sin p + m^* P+ + m P-) / (c^2 sum sin^2 p + |m|^2)  (pc = 1) or its
 // conjugate transpose M0(p) / (...) (pc = 2) instead of +-Dslash(p): same off-diagonal 2x2 blocks
@@ -76,7 +76,9 @@ k_p23(const P23Args<R> a) {
   using Cfg = P23Cfg<R, L2, L3, T2, T3, NC>;
   constexpr int TPL2 = Cfg::TPL2, TPL3 = Cfg::TPL3, NR2 = Cfg::NR2, NR3 = Cfg::NR3;
   constexpr int NTC = Cfg::NTC, PITCH = Cfg::PITCH, CPITCH = Cfg::CPITCH;
-  constexpr int D1 = (MODE == P23_MULT) ? +1 : DIR;  // direction of the first half
+  constexpr bool kMult = (MODE == P23_MULT || MODE == P23_MULTPC);
+  constexpr bool kPC = (MODE == P23_MULTPC);
+  constexpr int D1 = kMult ? +1 : DIR;  // direction of the first half
   extern __shared__ __align__(16) unsigned char smem_raw[];
   cpx<R>* sm = reinterpret_cast<cpx<R>*>(smem_raw);
   R* cfs = reinterpret_cast<R*>(sm + NC * CPITCH);  // off-diagonal factor
@@ -90,7 +92,7 @@ k_p23(const P23Args<R> a) {
   const long PL = (long)L2 * L3;
   const long fbase = (long)blockIdx.y * 4 * a.nplanes;  // first field of this batch entry
 
-  if constexpr (MODE == P23_MULT) {
+  if constexpr (kMult) {
     for (int i = tid; i < 2 * 4 * 64; i += blockDim.x) tb[i] = a.tab[i];
   }
 
@@ -98,8 +100,8 @@ k_p23(const P23Args<R> a) {
   const int tc = tid % NTC;
   // global spin component read (cin) and written (cc) by this thread
   const int half = (NC == 4) ? 0 : (int)blockIdx.z;
-  const int cin = (NC == 4) ? cl : ((MODE == P23_MULT) ? (half ? cl : 2 + cl) : 2 * half + cl);
-  const int cc = (NC == 4) ? cl : ((MODE == P23_MULT) ? (half ? 2 + cl : cl) : 2 * half + cl);
+  const int cin = (NC == 4) ? cl : (kMult ? (half ? cl : 2 + cl) : 2 * half + cl);
+  const int cc = (NC == 4) ? cl : (kMult ? (half ? 2 + cl : cl) : 2 * half + cl);
   // role A: line along axis 2 at x3;  role B: line along axis 3 at n2
   int x3A, jA, n2B, jB;
   lane_split<TPL2>(tc, x3A, jA);
@@ -138,7 +140,7 @@ k_p23(const P23Args<R> a) {
       y[k] = v;
     }
     F3::run(y, jB);
-    if constexpr (MODE == P23_MULT) {
+    if constexpr (kMult) {
       // c(p) once per momentum site: component slot cl covers 1/NC of this lane's n3 values
       static_assert(NR3 % NC == 0, "c(p) sharing");
       if (actB) {
@@ -156,7 +158,7 @@ k_p23(const P23Args<R> a) {
           const R s3 = sn[3 * 64 + n3];
           const R S2 = S012 + s3 * s3;
           const R cf = overlap_c(Mw012 - R(2) * sh[3 * 64 + n3], S2, kk);
-          if (a.pc) {  // cf carries rho-scaling and 1/V; c = cf / a.scale;  D = c^2 S2 + |m|^2
+          if constexpr (kPC) {  // cf carries rho-scaling and 1/V; c = cf / a.scale;  D = c^2 S2 + |m|^2
             const R c = cf / a.scale;
             const R invD = R(1) / (c * c * S2 + a.m_re * a.m_re + a.m_im * a.m_im);
             cfs[n2B * PITCH + n3] = cf * invD;
@@ -218,7 +220,7 @@ k_p23(const P23Args<R> a) {
         const R tr = A0 * pa.re - Ai * pa.im + B0 * pb.re - Bi * pb.im;
         const R ti = A0 * pa.im + Ai * pa.re + B0 * pb.im + Bi * pb.re;
         cpx<R> o = {-cf * ti, cf * tr};  // times i
-        if (a.pc) {  // + (m or m^*) / D on the own component
+        if constexpr (kPC) {  // + (m or m^*) / D on the own component
           const cpx<R> own = smc[n2 * PITCH + n3];
           const R dg = dgs[n2 * PITCH + n3];
           const R dr = dm_re * dg, di = dm_im * dg;
