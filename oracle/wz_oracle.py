@@ -219,3 +219,33 @@ def cg_pc(phi, b, m, g, rho=1.0, tol=1e-10, max_iter=100000, method="auto"):
         raise ValueError("oracle cg_pc failed")
     return x, CGInfo(info.iterations, info.reliable_updates, bool(info.converged),
                      info.rel_residual_recursive, info.rel_residual_true, hist[: info.iterations + 1].copy())
+
+
+def apply_Dslash(dims, psi, rho=1.0, method="auto") -> np.ndarray:
+    """Dslash psi = (1 - D2/2)^-1 D1 psi: the fermion matrix of Eq. (2.19) at m = 0, g = 0."""
+    dims = tuple(int(d) for d in dims)
+    return apply_M(np.zeros(dims, dtype=np.complex128), psi, 0.0, 0.0, rho, False, method)
+
+
+def locality_profile(dims, spin=0, rho=1.0, method="auto"):
+    """PAPER.md:262-282, Eq. (3.9)-(3.11): psi = Dslash eta for a unit point source eta at the
+    origin (spin component `spin`), f(r) = max{ ||psi(x)|| : ||x||_1 = r } with the taxi-driver
+    distance of Eq. (3.10) and ||.|| the norm over the spinor index.  Returns (f, psi)."""
+    dims = tuple(int(d) for d in dims)
+    eta = np.zeros((4,) + dims, dtype=np.complex128)
+    eta[(spin, 0, 0, 0, 0)] = 1.0
+    psi = apply_Dslash(dims, eta, rho, method)
+    nrm = np.sqrt((np.abs(psi) ** 2).sum(axis=0))
+    dist = np.zeros(dims, dtype=np.int64)
+    for mu, L in enumerate(dims):
+        x = np.arange(L)
+        d = np.minimum(x, L - x)                      # |x_mu| or |L_mu - x_mu|, the shorter one
+        shape = [1, 1, 1, 1]
+        shape[mu] = L
+        dist = dist + d.reshape(shape)
+    rmax = int(sum(L // 2 for L in dims))
+    f = np.zeros(rmax + 1)
+    for r in range(rmax + 1):
+        sel = nrm[dist == r]
+        f[r] = sel.max() if sel.size else 0.0
+    return f, psi
