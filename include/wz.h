@@ -123,6 +123,15 @@ wz_status wz_cg_solve_pc(wz_plan *plan, const void *phi, const void *b, void *x,
                          const double m[2], const double g[2], double rho,
                          double tol, int max_iter, int nbatch, wz_cg_info *info);
 
+/* ---- Locality probe (Eq. 3.9-3.11, Fig. 1) ----
+ * wz_apply_Dslash: out = Dslash in = (1 - D2/2)^-1 D1 in (the fermion matrix at m = g = 0); in != out.
+ * wz_locality_profile: psi = Dslash eta for a unit point source at the origin in spin component
+ *   `spin`; f[r] = max{ ||psi(x)|| over the spinor index : ||x||_1 = r }, taxi-driver distance with the
+ *   shorter way round each axis.  f is a HOST array of nf = 1 + sum_mu floor(L_mu / 2) doubles.
+ *   Uses plan temporaries; synchronises the stream. */
+wz_status wz_apply_Dslash(wz_plan *plan, double rho, const void *in, void *out, int nbatch);
+wz_status wz_locality_profile(wz_plan *plan, double rho, int spin, double *f_host, int nf);
+
 /* Number of kernel launches this plan has enqueued so far (for bench.py's
  * gpu_launches), and a reset. */
 unsigned long long wz_plan_launch_count(const wz_plan *plan);

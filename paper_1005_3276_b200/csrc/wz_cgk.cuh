@@ -141,6 +141,31 @@ k_resid(const TB* __restrict__ b, const double* __restrict__ q, TR* __restrict__
   grid_reduce<FIN>(acc, red, blockIdx.x, gridDim.x, sh);
 }
 
+// Locality probe, Eq. (3.10)-(3.11):  f(r) = max{ ||psi(x)|| : ||x||_1 = r } with
+// the taxi-driver distance to the origin (shorter way round each axis) and ||.|| the norm over
+// the four spin components.  f holds ||.||^2 as the bit pattern of a non-negative double, so
+// an unsigned 64-bit atomicMax orders it; the host takes the square root.
+template <typename R>
+__global__ void __launch_bounds__(CGK_NT)
+k_locality(const cpx<R>* __restrict__ psi, unsigned long long* __restrict__ f, int L0, int L1, int L2, int L3) {
+  const long V = (long)L0 * L1 * L2 * L3;
+  for (long x = (long)blockIdx.x * blockDim.x + threadIdx.x; x < V; x += (long)gridDim.x * blockDim.x) {
+    double n2 = 0.0;
+#pragma unroll
+    for (int c = 0; c < 4; ++c) {
+      const cpx<R> v = psi[c * V + x];
+      n2 += (double)v.re * (double)v.re + (double)v.im * (double)v.im;
+    }
+    long t = x;
+    const int x3 = (int)(t % L3); t /= L3;
+    const int x2 = (int)(t % L2); t /= L2;
+    const int x1 = (int)(t % L1); t /= L1;
+    const int x0 = (int)t;
+    const int r = min(x0, L0 - x0) + min(x1, L1 - x1) + min(x2, L2 - x2) + min(x3, L3 - x3);
+    atomicMax(f + r, (unsigned long long)__double_as_longlong(n2));
+  }
+}
+
 // dst (double) = src (float), element-wise (phi for the complex128 operator of a
 // complex64 plan: the float-rounded values, exactly what the oracle consumes).
 __global__ void __launch_bounds__(CGK_NT)

@@ -997,6 +997,58 @@ wz_status wz_apply_M0inv(wz_plan* pl, int dagger, const double m[2], double rho,
   return apply_M0inv_impl<double>(pl, dagger ? 1 : 0, m, rho, (const cpx<double>*)in, (cpx<double>*)out, nbatch);
 }
 
+// Dslash = the fermion matrix at m = 0, g = 0 (Eq. 2.19): passes A, B, E with a zero site-local term.
+wz_status wz_apply_Dslash(wz_plan* pl, double rho, const void* in, void* out, int nbatch) {
+  g_err[0] = 0;
+  if (!pl || !in || !out || in == out) return WZ_EINVAL;
+  if (!(rho > 0.0 && rho < 2.0) || nbatch < 0 || nbatch > pl->max_batch) return WZ_EINVAL;
+  if (nbatch == 0) return WZ_OK;
+  const double zero[2] = {0.0, 0.0};
+  // the site-local coefficient m + 2 g phi vanishes identically; `in` (finite values) stands in for phi
+  if (pl->dtype == WZ_C64)
+    return apply_M_impl<float>(pl, 0, (const cpx<float>*)in, zero, zero, rho, (const cpx<float>*)in,
+                               (cpx<float>*)out, nbatch);
+  return apply_M_impl<double>(pl, 0, (const cpx<double>*)in, zero, zero, rho, (const cpx<double>*)in,
+                              (cpx<double>*)out, nbatch);
+}
+
+wz_status wz_locality_profile(wz_plan* pl, double rho, int spin, double* f_host, int nf) {
+  g_err[0] = 0;
+  int rmax = 0;
+  if (pl) for (int mu = 0; mu < 4; ++mu) rmax += pl->L[mu] / 2;
+  if (!pl || !f_host || spin < 0 || spin > 3 || nf != rmax + 1 || !(rho > 0.0 && rho < 2.0)) return WZ_EINVAL;
+  const size_t n1 = (size_t)4 * pl->V;
+  const bool f32 = pl->dtype == WZ_C64;
+  const size_t esz = f32 ? sizeof(cpx<float>) : sizeof(cpx<double>);
+  void* eta = f32 ? (void*)pl->wsf.chi : (void*)pl->wsd.chi;  // plan temporaries: eta -> chi, psi -> r
+  void* psi = pl->r;
+  unsigned long long* d_f = reinterpret_cast<unsigned long long*>(pl->partials);  // >= 4096 doubles
+  if (nf > pl->npartials) return WZ_EINVAL;
+  WZ_CUDA(cudaMemsetAsync(eta, 0, n1 * esz, pl->stream));
+  WZ_CUDA(cudaMemsetAsync(d_f, 0, sizeof(double) * nf, pl->stream));
+  if (f32) {
+    const cpx<float> one = {1.f, 0.f};
+    WZ_CUDA(cudaMemcpyAsync((cpx<float>*)eta + (size_t)spin * pl->V, &one, sizeof(one), cudaMemcpyHostToDevice, pl->stream));
+  } else {
+    const cpx<double> one = {1.0, 0.0};
+    WZ_CUDA(cudaMemcpyAsync((cpx<double>*)eta + (size_t)spin * pl->V, &one, sizeof(one), cudaMemcpyHostToDevice, pl->stream));
+  }
+  WZ_CUDA(cudaStreamSynchronize(pl->stream));  // `one` lives on this stack frame
+  wz_status s = wz_apply_Dslash(pl, rho, eta, psi, 1);
+  if (s != WZ_OK) return s;
+  {
+    ProfScope ps(pl, WZ_K_OTHER);
+    const int grid = vec_grid(pl->V, 1);
+    if (f32) k_locality<float><<<grid, CGK_NT, 0, pl->stream>>>((const cpx<float>*)psi, d_f, pl->L[0], pl->L[1], pl->L[2], pl->L[3]);
+    else k_locality<double><<<grid, CGK_NT, 0, pl->stream>>>((const cpx<double>*)psi, d_f, pl->L[0], pl->L[1], pl->L[2], pl->L[3]);
+  }
+  WZ_CUDA(cudaGetLastError());
+  WZ_CUDA(cudaMemcpyAsync(f_host, d_f, sizeof(double) * nf, cudaMemcpyDeviceToHost, pl->stream));
+  WZ_CUDA(cudaStreamSynchronize(pl->stream));
+  for (int r = 0; r < nf; ++r) f_host[r] = std::sqrt(f_host[r]);
+  return WZ_OK;
+}
+
 wz_status wz_apply_MtdagMt(wz_plan* pl, const void* phi, const double m[2], const double g[2], double rho,
                            const void* in, void* out, int nbatch) {
   g_err[0] = 0;

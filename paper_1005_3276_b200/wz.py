@@ -24,7 +24,7 @@ EXPORTS = [
     "wz_supported", "wz_plan_workspace_bytes", "wz_fft4d", "wz_apply_M", "wz_apply_MdagM",
     "wz_cg_solve", "wz_plan_launch_count", "wz_plan_reset_launch_count",
     "wz_plan_profile", "wz_plan_profile_read", "wz_kind_name",
-    "wz_apply_M0inv", "wz_apply_MtdagMt", "wz_cg_solve_pc",
+    "wz_apply_M0inv", "wz_apply_MtdagMt", "wz_cg_solve_pc", "wz_apply_Dslash", "wz_locality_profile",
 ]
 
 
@@ -79,6 +79,8 @@ def lib() -> ctypes.CDLL:
         L.wz_cg_solve_pc.argtypes = L.wz_cg_solve.argtypes
         L.wz_apply_M0inv.argtypes = [vp, ci, d2, cd, vp, vp, ci]
         L.wz_apply_MtdagMt.argtypes = [vp, vp, d2, d2, cd, vp, vp, ci]
+        L.wz_apply_Dslash.argtypes = [vp, cd, vp, vp, ci]
+        L.wz_locality_profile.argtypes = [vp, cd, ci, d2, ci]
         L.wz_plan_profile.argtypes = [vp, ci]
         L.wz_plan_profile_read.argtypes = [vp, d2, ctypes.POINTER(ctypes.c_ulonglong)]
         L.wz_kind_name.restype = ctypes.c_char_p
@@ -203,6 +205,21 @@ class Plan:
         _check(lib().wz_apply_MdagM(self._h, phi.data_ptr(), _c2(m), _c2(g), float(rho),
                                     psi.data_ptr(), out.data_ptr(), nb))
         return out
+
+    def apply_Dslash(self, psi, rho: float = 1.0, out=None):
+        nb = self._spinor(psi)
+        if out is None:
+            out = torch.empty_like(psi)
+        self._spinor(out)
+        _check(lib().wz_apply_Dslash(self._h, float(rho), psi.data_ptr(), out.data_ptr(), nb))
+        return out
+
+    def locality_profile(self, spin: int = 0, rho: float = 1.0):
+        """f(r) of Eq. (3.11) as a list of floats, r = 0 .. sum(L_mu // 2)."""
+        nf = 1 + sum(d // 2 for d in self.dims)
+        f = (ctypes.c_double * nf)()
+        _check(lib().wz_locality_profile(self._h, float(rho), int(spin), f, nf))
+        return list(f)
 
     def apply_M0inv(self, psi, m, rho: float = 1.0, dagger: bool = False, out=None):
         nb = self._spinor(psi)

@@ -369,3 +369,20 @@ def test_cg_pc_strong_coupling_config2(wz, orc, inp):
     res = rel(orc.apply_MdagM(phi, x1.cpu().numpy(), cfg["m"], cfg["g"], 1.0), b)
     assert i1[0].converged and res <= 1e-7
     assert rel(x1.cpu().numpy(), x0.cpu().numpy()) <= 1e-6
+
+
+# ---- NEXT-4: locality probe ----
+
+@pytest.mark.parametrize("dims,dtype", [((16, 16, 16, 16), "c128"), ((16, 16, 16, 16), "c64"), ((8, 4, 16, 8), "c128")])
+def test_locality_profile_vs_oracle(wz, orc, dims, dtype):
+    plan = wz.Plan(dims, dtype, 1)
+    for spin in (0, 3):
+        f = np.array(plan.locality_profile(spin))
+        fo, psio = orc.locality_profile(dims, spin)
+        assert f.shape == fo.shape
+        assert f[0] <= (1e-12 if dtype == "c128" else 1e-5)          # Fig. 1: f(0) = 0
+        assert np.max(np.abs(f[1:] - fo[1:]) / fo[1:]) <= (1e-11 if dtype == "c128" else 1e-4)
+    eta = torch.zeros((4,) + tuple(dims), dtype=plan.tdtype, device="cuda")
+    eta[2, 0, 0, 0, 0] = 1.0
+    psi = plan.apply_Dslash(eta).cpu().numpy()
+    assert rel(psi, orc.locality_profile(dims, 2)[1]) <= TOL[dtype]
