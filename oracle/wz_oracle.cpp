@@ -726,4 +726,56 @@ int orc_cg_pc(int method, const int* L, const double* phi, const double* b_, dou
   return 0;
 }
 
+// ----------------------------------------------------------------------------
+// O6 (NEXT-2, first step). Shifted system (M^dag M + sigma) x = b, sigma >= 0
+// (Eq. 7.13: the systems of the rational approximation).  The
+// textbook loop of orc_cg with A = M^dag M + sigma; the true residual at exit is
+// that of the shifted system.
+// ----------------------------------------------------------------------------
+int orc_cg_shift(int method, const int* L, const double* phi, const double* b_, double* x_,
+                 const double* m, const double* g, double rho, double sigma, double tol, int max_iter,
+                 orc_cg_info* info, double* history) {
+  const long V = (long)L[0] * L[1] * L[2] * L[3];
+  const long n = 4 * V;
+  const cd* b = reinterpret_cast<const cd*>(b_);
+  cd* x = reinterpret_cast<cd*>(x_);
+  std::vector<cd> r(b, b + n), p(b, b + n), q(n);
+  for (long i = 0; i < n; ++i) x[i] = 0.0;
+  double bnorm = std::sqrt(dot_re(b, b, n));
+  double rr = bnorm * bnorm;
+  if (history) history[0] = 1.0;
+  int k = 0, converged = (bnorm == 0.0);
+  while (!converged && k < max_iter) {
+    ++k;
+    int rc = orc_apply_MdagM(method, L, phi, m, g, rho, reinterpret_cast<double*>(p.data()),
+                             reinterpret_cast<double*>(q.data()));
+    if (rc) return rc;
+    for (long i = 0; i < n; ++i) q[i] += sigma * p[i];
+    double alpha = rr / dot_re(p.data(), q.data(), n);
+    for (long i = 0; i < n; ++i) {
+      x[i] += alpha * p[i];
+      r[i] -= alpha * q[i];
+    }
+    double rr_new = dot_re(r.data(), r.data(), n);
+    if (history) history[k] = std::sqrt(rr_new) / bnorm;
+    if (std::sqrt(rr_new) <= tol * bnorm) {
+      rr = rr_new;
+      converged = 1;
+      break;
+    }
+    double beta = rr_new / rr;
+    rr = rr_new;
+    for (long i = 0; i < n; ++i) p[i] = r[i] + beta * p[i];
+  }
+  orc_apply_MdagM(method, L, phi, m, g, rho, x_, reinterpret_cast<double*>(q.data()));
+  double tr = 0.0;
+  for (long i = 0; i < n; ++i) tr += std::norm(b[i] - q[i] - sigma * x[i]);
+  info->iterations = k;
+  info->reliable_updates = 0;
+  info->converged = converged;
+  info->rel_residual_recursive = bnorm > 0 ? std::sqrt(rr) / bnorm : 0.0;
+  info->rel_residual_true = bnorm > 0 ? std::sqrt(tr) / bnorm : 0.0;
+  return 0;
+}
+
 }  // extern "C"

@@ -249,3 +249,20 @@ def locality_profile(dims, spin=0, rho=1.0, method="auto"):
         sel = nrm[dist == r]
         f[r] = sel.max() if sel.size else 0.0
     return f, psi
+
+
+def cg_shift(phi, b, m, g, sigma, rho=1.0, tol=1e-10, max_iter=100000, method="auto"):
+    """Textbook CG on (M^dag M + sigma) x = b (Eq. 7.13) in complex128.  Returns (x, CGInfo)."""
+    phi = np.ascontiguousarray(phi, dtype=np.complex128)
+    b = np.ascontiguousarray(b, dtype=np.complex128)
+    dims = phi.shape
+    x = np.zeros_like(b)
+    hist = np.zeros(max_iter + 1, dtype=np.float64)
+    info = _Info()
+    rc = lib().orc_cg_shift(_method(dims, method), _dims(dims), _dp(phi), _dp(b), _dp(x), _c2(m), _c2(g),
+                            ctypes.c_double(rho), ctypes.c_double(sigma), ctypes.c_double(tol), int(max_iter),
+                            ctypes.byref(info), _dp(hist))
+    if rc:
+        raise ValueError("oracle cg_shift failed")
+    return x, CGInfo(info.iterations, info.reliable_updates, bool(info.converged),
+                     info.rel_residual_recursive, info.rel_residual_true, hist[: info.iterations + 1].copy())
