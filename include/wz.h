@@ -123,6 +123,17 @@ wz_status wz_cg_solve_pc(wz_plan *plan, const void *phi, const void *b, void *x,
                          const double m[2], const double g[2], double rho,
                          double tol, int max_iter, int nbatch, wz_cg_info *info);
 
+/* ---- Shifted system (Eq. 7.6-7.7; 927-931, Eq. 7.13) ----
+ * The partial-fraction terms of the rational approximation need (M^dag M + beta_i) X_i = eta, one
+ * conjugate-gradient solve per shift ("solved one at a time").
+ * wz_cg_solve_shift: CG on (M^dag M + sigma) x = b, sigma >= 0 real, x0 = 0, stop when
+ *   ||b - (M^dag M + sigma) x|| <= tol ||b||.  sigma = 0 is wz_cg_solve.  All other arguments, the
+ *   complex128 solution buffer and info as in wz_cg_solve; residuals refer to the shifted system.
+ *   sigma < 0 or NaN: WZ_EINVAL. */
+wz_status wz_cg_solve_shift(wz_plan *plan, const void *phi, const void *b, void *x,
+                            const double m[2], const double g[2], double rho, double sigma,
+                            double tol, int max_iter, int nbatch, wz_cg_info *info);
+
 /* ---- Locality probe (Eq. 3.9-3.11, Fig. 1) ----
  * wz_apply_Dslash: out = Dslash in = (1 - D2/2)^-1 D1 in (the fermion matrix at m = g = 0); in != out.
  * wz_locality_profile: psi = Dslash eta for a unit point source at the origin in spin component

@@ -116,15 +116,16 @@ k_ru_accum(double* __restrict__ X, float* __restrict__ xs, long n) {
   }
 }
 
-// Residual in float64:  d = b - q;  sum |d|^2 -> FIN;  r = round(d) (if r given).
-// TB: storage type of b, TR: storage type of r.
+// Residual in float64:  d = b - q - sigma x  (sigma x only if xshift is given);  sum |d|^2 -> FIN;
+// r = round(d) (if r given).  TB: storage type of b, TR: storage type of r.
 template <typename TB, typename TR, int FIN>
 __global__ void __launch_bounds__(CGK_NT)
 k_resid(const TB* __restrict__ b, const double* __restrict__ q, TR* __restrict__ r, long n,
-        RedArgs red) {
+        RedArgs red, const double* __restrict__ xshift = nullptr, double sigma = 0.0) {
   const int src = blockIdx.y;
   b += src * n; q += src * n;
   if (r) r += src * n;
+  if (xshift) xshift += src * n;
   red = red.for_source(src);
   __shared__ double sh[33];
   double acc = 0.0;
@@ -132,6 +133,10 @@ k_resid(const TB* __restrict__ b, const double* __restrict__ q, TR* __restrict__
        i += (long)gridDim.x * blockDim.x * 2) {
     double2 vq = *reinterpret_cast<const double2*>(q + i);
     double d0 = (double)b[i] - vq.x, d1 = (double)b[i + 1] - vq.y;
+    if (xshift) {
+      d0 -= sigma * xshift[i];
+      d1 -= sigma * xshift[i + 1];
+    }
     acc += d0 * d0 + d1 * d1;
     if (r) {
       r[i] = (TR)d0;

@@ -16,6 +16,7 @@ struct OpParams {
   R g2_re, g2_im;  // 2 g
   R rho;           // overlap parameter (paper: 1)
   int dagger;      // 0: M, 1: M^dag
+  R shift;         // sigma: pass E' subtracts alpha (q + sigma p) (wz_cg_solve_shift)
   int pc;          // 1: site-local steps of the preconditioned operator Mtilde = 1 + Y M0^-1 (wz_p01.cuh)
 };
 
@@ -29,6 +30,8 @@ struct CGState {
   double rmax;           // max ||r|| since the last reliable update (G9)
   double tol, delta;
   double true_rr;        // ||b - A x||^2 recomputed
+  double shift;          // sigma of the shifted system (M^dag M + sigma) x = b (0: plain)
+  double pp;             // <p,p> of the current search direction (shifted solves)
   double aux;            // scratch norm (||b||^2 of the original system in preconditioned solves)
   int iter, max_iter;
   int n_ru;
@@ -44,22 +47,24 @@ __device__ __forceinline__ bool cg_active(const CGState* st) {
 }
 
 // What the last block of a reduction does with the total.
-enum { FIN_STORE = 0, FIN_PQ = 1, FIN_RR = 2, FIN_RU = 3, FIN_INIT = 4, FIN_TRUE = 5, FIN_AUX = 6 };
+enum { FIN_STORE = 0, FIN_PQ = 1, FIN_RR = 2, FIN_RU = 3, FIN_INIT = 4, FIN_TRUE = 5, FIN_AUX = 6, FIN_PP = 7, FIN_RRS = 8 };
+// FIN_PP / FIN_RRS select the shifted-system variants of passes A' / E' (wz_cg_solve_shift); FIN_RRS
+// finalises like FIN_RR.
 
 template <int FIN>
 __device__ __forceinline__ void cg_finalize(double total, CGState* st, double* store) {
   if (FIN == FIN_STORE) {
     *store = total;
   } else if (FIN == FIN_PQ) {  // alpha = rho_{k-1} / <p, A p>
-    st->pq = total;
-    st->alpha = st->rr / total;
+    st->pq = total + st->shift * st->pp;  // <p, (A + sigma) p> = ||M p||^2 + sigma <p,p>
+    st->alpha = st->rr / st->pq;
   } else if (FIN == FIN_INIT) {  // r0 = p0 = b
     st->bnorm2 = total;
     st->bnorm = sqrt(total);
     st->rr = total;
     st->rmax = sqrt(total);
     if (total == 0.0) st->converged = 1;
-  } else if (FIN == FIN_RR) {  // after x += alpha p, r -= alpha q
+  } else if (FIN == FIN_RR || FIN == FIN_RRS) {  // after x += alpha p, r -= alpha q
     const double rn = sqrt(total);
     st->iter += 1;
     if (st->use_ru) {
@@ -94,6 +99,8 @@ __device__ __forceinline__ void cg_finalize(double total, CGState* st, double* s
     st->true_rr = total;
   } else if (FIN == FIN_AUX) {
     st->aux = total;
+  } else if (FIN == FIN_PP) {
+    st->pp = total;
   }
 }
 

@@ -41,14 +41,15 @@ struct P01Entry {
   int L0, L1;
   long I;  // (x2,x3) volume the kernels were specialised for; 0 = any (run-time)
   P01Kern<R> fwd, inv, mid, mid_pq, end, fwdcg, endcg;
+  P01Kern<R> fwdcg_s, endcg_s;  // shifted system (M^dag M + sigma): A' also reduces <p,p>, E' adds sigma p to q
   int nseg() const {  // largest tile width of the entry: the (x2,x3) volume must be a multiple
     int m = 1;
-    for (const P01Kern<R>* k : {&fwd, &inv, &mid, &mid_pq, &end, &fwdcg, &endcg}) m = k->nseg > m ? k->nseg : m;
+    for (const P01Kern<R>* k : {&fwd, &inv, &mid, &mid_pq, &end, &fwdcg, &endcg, &fwdcg_s, &endcg_s}) m = k->nseg > m ? k->nseg : m;
     return m;
   }
   int min_nseg() const {
     int m = 1 << 30;
-    for (const P01Kern<R>* k : {&fwd, &inv, &mid, &mid_pq, &end, &fwdcg, &endcg}) m = k->nseg < m ? k->nseg : m;
+    for (const P01Kern<R>* k : {&fwd, &inv, &mid, &mid_pq, &end, &fwdcg, &endcg, &fwdcg_s, &endcg_s}) m = k->nseg < m ? k->nseg : m;
     return m;
   }
 };
@@ -124,6 +125,8 @@ P01Entry<R> make_p01() {
   e.end = make_p01_kern<R, L0, L1, P01_END, FIN_STORE, IC>();
   e.fwdcg = make_p01_kern<R, L0, L1, P01_FWDCG, FIN_STORE, IC>();
   e.endcg = make_p01_kern<R, L0, L1, P01_ENDCG, FIN_RR, IC>();
+  e.fwdcg_s = make_p01_kern<R, L0, L1, P01_FWDCG, FIN_PP, IC>();
+  e.endcg_s = make_p01_kern<R, L0, L1, P01_ENDCG, FIN_RRS, IC>();
   return e;
 }
 template <typename R, int L2, int L3, int NC = 4>
@@ -290,6 +293,7 @@ wz_status setup_ws(wz_plan* pl, OpWS<R>& ws, int nbatch_t) {
   if (!ws.p01 || !ws.p23) return WZ_EUNSUPPORTED;
   if (pl->I % ws.p01->nseg()) return WZ_EUNSUPPORTED;
   const auto* a = ws.p01;
+  if (!set_smem_kern(a->fwdcg_s) || !set_smem_kern(a->endcg_s)) return WZ_ECUDA;
   if (!set_smem_kern(a->fwd) || !set_smem_kern(a->inv) || !set_smem_kern(a->mid) ||
       !set_smem_kern(a->mid_pq) || !set_smem_kern(a->end) || !set_smem_kern(a->fwdcg) ||
       !set_smem_kern(a->endcg))
@@ -391,7 +395,7 @@ OpParams<R> make_op(const double m[2], const double g[2], double rho, int dagger
   OpParams<R> op;
   op.m_re = (R)m[0]; op.m_im = (R)m[1];
   op.g2_re = (R)(2.0 * g[0]); op.g2_im = (R)(2.0 * g[1]);
-  op.rho = (R)rho; op.dagger = dagger; op.pc = pc;
+  op.rho = (R)rho; op.dagger = dagger; op.pc = pc; op.shift = R(0);
   return op;
 }
 
@@ -506,7 +510,10 @@ wz_status apply_M0inv_impl(wz_plan* pl, int dagger, const double m[2], double rh
 // state; every kernel is gated on it.  x lags one update: flush_x() before x is used. --
 template <typename R>
 wz_status cg_iteration(wz_plan* pl, const cpx<R>* phi, const double m[2], const double g[2], double rho,
-                       cpx<R>* r, cpx<R>* p, cpx<R>* x, int nb, bool pc) {
+                       cpx<R>* r, cpx<R>* p, cpx<R>* x, int nb, bool pc, double sigma = 0.0) {
+  // sigma != 0: the shifted system (M^dag M + sigma) x = b (Eq. 7.13): pass A' also
+  // reduces <p,p> (alpha = rho / (||M p||^2 + sigma <p,p>)), pass E' uses q + sigma p
+  const bool sh = sigma != 0.0;
   OpWS<R>& ws = ws_of<R>(pl);
   if ((int)(pl->I / ws.p01->min_nseg()) * 4 > pl->npartials) return WZ_EINVAL;
   const R invV = (R)(1.0 / (double)pl->V);
@@ -514,7 +521,8 @@ wz_status cg_iteration(wz_plan* pl, const cpx<R>* phi, const double m[2], const 
   P01Args<R> a{};
   a.I = pl->I; a.apbc = 1; a.scale = R(1); a.gate = pl->d_state;
   a.in = p; a.out = ws.t; a.cg_r = r; a.cg_p = p; a.cg_x = x;
-  if ((s = launch_p01<R>(pl, WZ_K_P01_FWDCG, ws.p01->fwdcg, a, nb)) != WZ_OK) return s;
+  if (sh) a.red = red_of(pl);
+  if ((s = launch_p01<R>(pl, WZ_K_P01_FWDCG, sh ? ws.p01->fwdcg_s : ws.p01->fwdcg, a, nb)) != WZ_OK) return s;
   P23Args<R> b{};
   b.nplanes = pl->L[0] * pl->L[1]; b.L1 = pl->L[1]; b.scale = invV;
   b.tab = ws.tab; b.rho = (R)rho; b.sign = pc ? R(-1) : R(1); b.gate = pl->d_state;
@@ -530,8 +538,8 @@ wz_status cg_iteration(wz_plan* pl, const cpx<R>* phi, const double m[2], const 
   if ((s = mult_pass<R>(pl, ws, b, cur, nb)) != WZ_OK) return s;
   a.in = cur; a.out = cur;
   a.psi = ws.chi; a.site_out = nullptr; a.op = make_op<R>(m, g, rho, 1, pc);
-  a.cg_r = r; a.cg_p = p; a.cg_x = x;
-  return launch_p01<R>(pl, WZ_K_P01_ENDCG, ws.p01->endcg, a, nb);
+  a.cg_r = r; a.cg_p = p; a.cg_x = x; a.op.shift = (R)sigma;
+  return launch_p01<R>(pl, WZ_K_P01_ENDCG, sh ? ws.p01->endcg_s : ws.p01->endcg, a, nb);
 }
 
 }  // namespace
@@ -762,7 +770,8 @@ int vec_grid(long n_real, int per_thread) {
 template <typename R>
 wz_status cg_batch(wz_plan* pl, const cpx<R>* phi, const cpx<R>* b, cpx<double>* X, const double m[2],
                    const double g[2], double rho, double tol, int max_iter, int nb, wz_cg_info* info,
-                   bool pc) {
+                   bool pc, double sigma = 0.0) {
+  // sigma: shift of the system (M^dag M + sigma) x = b (Eq. 7.13); not combined with pc
   constexpr bool kRU = (sizeof(R) == 4);
   constexpr int N = vec16<R>::N;
   const long n = 8 * pl->V;       // real entries of one spinor
@@ -776,7 +785,7 @@ wz_status cg_batch(wz_plan* pl, const cpx<R>* phi, const cpx<R>* b, cpx<double>*
   memset(h.data(), 0, sizeof(CGState) * nb);
   for (int j = 0; j < nb; ++j) {
     h[j].tol = tol; h[j].delta = kDelta; h[j].max_iter = max_iter; h[j].use_ru = kRU ? 1 : 0;
-    h[j].true_rr = -1.0;
+    h[j].true_rr = -1.0; h[j].shift = sigma;
     if (max_iter == 0) h[j].stop = 1;
   }
   WZ_CUDA(cudaMemcpyAsync(pl->d_state, h.data(), sizeof(CGState) * nb, cudaMemcpyHostToDevice, st));
@@ -818,6 +827,7 @@ wz_status cg_batch(wz_plan* pl, const cpx<R>* phi, const cpx<R>* b, cpx<double>*
     return WZ_OK;
   };
   // residual of source j recomputed in complex128:  q128 = A X_j;  d = b_j - q128
+  auto xsh = [&](int j) -> const double* { return sigma != 0.0 ? (const double*)(X + j * n1) : nullptr; };
   auto residual128 = [&](int j, bool update_r) -> wz_status {
     RedArgs ra = red_of(pl).for_source(j);
     struct Override {  // the one-source complex128 matvec is not part of the batched iteration
@@ -841,16 +851,16 @@ wz_status cg_batch(wz_plan* pl, const cpx<R>* phi, const cpx<R>* b, cpx<double>*
           k_resid<double, float, FIN_TRUE><<<dim3(gv2, 1), CGK_NT, 0, st>>>(bt, (const double*)pl->q128, nullptr, n, ra);
       } else if (update_r)
         k_resid<float, float, FIN_RU><<<dim3(gv2, 1), CGK_NT, 0, st>>>(
-            (const float*)(b + j * n1), (const double*)pl->q128, (float*)(r + j * n), n, ra);
+            (const float*)(b + j * n1), (const double*)pl->q128, (float*)(r + j * n), n, ra, xsh(j), sigma);
       else
         k_resid<float, float, FIN_TRUE><<<dim3(gv2, 1), CGK_NT, 0, st>>>(
-            (const float*)(b + j * n1), (const double*)pl->q128, nullptr, n, ra);
+            (const float*)(b + j * n1), (const double*)pl->q128, nullptr, n, ra, xsh(j), sigma);
     } else {
       wz_status s2 = apply_MdagM_impl<double>(pl, (const cpx<double>*)phi, m, g, rho, X + j * n1, pl->q128, 1, false);
       if (s2 != WZ_OK) return s2;
       ProfScope ps(pl, WZ_K_OTHER);
       k_resid<double, double, FIN_TRUE><<<dim3(gv2, 1), CGK_NT, 0, st>>>(
-          (const double*)(b + j * n1), (const double*)pl->q128, nullptr, n, ra);
+          (const double*)(b + j * n1), (const double*)pl->q128, nullptr, n, ra, xsh(j), sigma);
     }
     WZ_CUDA(cudaGetLastError());
     return WZ_OK;
@@ -863,9 +873,9 @@ wz_status cg_batch(wz_plan* pl, const cpx<R>* phi, const cpx<R>* b, cpx<double>*
     while (inflight < 2) {
       for (int it = 0; it < kCheckEvery; ++it) {
         if constexpr (kRU)
-          s = cg_iteration<R>(pl, phi, m, g, rho, (cpx<R>*)r, (cpx<R>*)p, (cpx<R>*)xs, nb, pc);
+          s = cg_iteration<R>(pl, phi, m, g, rho, (cpx<R>*)r, (cpx<R>*)p, (cpx<R>*)xs, nb, pc, sigma);
         else
-          s = cg_iteration<R>(pl, phi, m, g, rho, (cpx<R>*)r, (cpx<R>*)p, (cpx<R>*)X, nb, pc);
+          s = cg_iteration<R>(pl, phi, m, g, rho, (cpx<R>*)r, (cpx<R>*)p, (cpx<R>*)X, nb, pc, sigma);
         if (s != WZ_OK) return s;
       }
       WZ_CUDA(cudaMemcpyAsync(pl->h_state + slot_w * pl->max_batch, pl->d_state, sizeof(CGState) * nb,
@@ -946,8 +956,9 @@ wz_status cg_batch(wz_plan* pl, const cpx<R>* phi, const cpx<R>* b, cpx<double>*
 
 static wz_status cg_solve_any(wz_plan* pl, const void* phi, const void* b, void* x, const double m[2],
                               const double g[2], double rho, double tol, int max_iter, int nbatch,
-                              wz_cg_info* info, bool pc) {
+                              wz_cg_info* info, bool pc, double sigma = 0.0) {
   g_err[0] = 0;
+  if (!(sigma >= 0.0) || (pc && sigma != 0.0)) return WZ_EINVAL;
   if (!pl || !phi || !b || !x || !m || !g || !info) return WZ_EINVAL;
   if (!(rho > 0.0 && rho < 2.0) || !(tol > 0.0) || max_iter < 0) return WZ_EINVAL;
   if (nbatch < 0 || nbatch > pl->max_batch) return WZ_EINVAL;
@@ -962,10 +973,10 @@ static wz_status cg_solve_any(wz_plan* pl, const void* phi, const void* b, void*
     }
     WZ_CUDA(cudaGetLastError());
     s = cg_batch<float>(pl, (const cpx<float>*)phi, (const cpx<float>*)b, (cpx<double>*)x, m, g, rho, tol,
-                        max_iter, nbatch, info, pc);
+                        max_iter, nbatch, info, pc, sigma);
   } else {
     s = cg_batch<double>(pl, (const cpx<double>*)phi, (const cpx<double>*)b, (cpx<double>*)x, m, g, rho, tol,
-                         max_iter, nbatch, info, pc);
+                         max_iter, nbatch, info, pc, sigma);
   }
   if (s != WZ_OK) return s;
   for (int j = 0; j < nbatch; ++j)
@@ -978,6 +989,12 @@ extern "C" {
 wz_status wz_cg_solve(wz_plan* pl, const void* phi, const void* b, void* x, const double m[2],
                       const double g[2], double rho, double tol, int max_iter, int nbatch, wz_cg_info* info) {
   return cg_solve_any(pl, phi, b, x, m, g, rho, tol, max_iter, nbatch, info, false);
+}
+
+wz_status wz_cg_solve_shift(wz_plan* pl, const void* phi, const void* b, void* x, const double m[2],
+                            const double g[2], double rho, double sigma, double tol, int max_iter, int nbatch,
+                            wz_cg_info* info) {
+  return cg_solve_any(pl, phi, b, x, m, g, rho, tol, max_iter, nbatch, info, false, sigma);
 }
 
 wz_status wz_cg_solve_pc(wz_plan* pl, const void* phi, const void* b, void* x, const double m[2],

@@ -118,6 +118,7 @@ k_p01(const P01Args<R> a) {
     using F0 = LineFFT<R, L0, +1, VAR_DIT, TPL0>;
     using F1 = LineFFT<R, L1, +1, VAR_DIT, TPL1>;
     cpx<R> x[NR0];
+    [[maybe_unused]] double accp = 0.0;  // ||p||^2 of the new search direction (FIN_PP: shifted solves)
     if constexpr (MODE == P01_FWDCG) {
       // p <- r + beta p (PAPER.md:896 CG), all p loads first, r through the
       // read-only path so that nothing waits behind the p stores
@@ -161,6 +162,7 @@ k_p01(const P01Args<R> a) {
             a.cg_x[off[c]] = {vx[c].re + alpha * v.re, vx[c].im + alpha * v.im};  // pending x += alpha p
             v = {vr[c].re + beta * v.re, vr[c].im + beta * v.im};
             a.cg_p[off[c]] = v;
+            if constexpr (FIN == FIN_PP) accp += (double)v.re * (double)v.re + (double)v.im * (double)v.im;
           }
           if (a.apbc) v = mul_tw_rt<R, +1>(v, x0 * TWSTEP);
           x[k0 + c] = v;
@@ -198,6 +200,11 @@ k_p01(const P01Args<R> a) {
 #pragma unroll
       for (int k = 0; k < NR1; ++k)
         gout[((long)x0B * L1 + F1::out_pos(k, jB)) * I + sB] = y[k];
+    }
+    if constexpr (MODE == P01_FWDCG && FIN == FIN_PP) {
+      // shifted solves: <p,p> of this source for alpha = rho / (||M p||^2 + sigma <p,p>)
+      const int blk = comp * gridDim.x + blockIdx.x;
+      grid_reduce<FIN_PP>(accp, a.red.for_source(src), blk, 4 * gridDim.x, red_sh);
     }
   } else {
     // ---- inverse half: axis 1 first (from HBM), then axis 0 ----
@@ -298,6 +305,11 @@ k_p01(const P01Args<R> a) {
               cpx<R> q = x[k0 + c];
               q.re += w.re * ps[c].re - w.im * ps[c].im;
               q.im += w.re * ps[c].im + w.im * ps[c].re;
+              if constexpr (FIN == FIN_RRS) {  // shifted system: q <- q + sigma p
+                const cpx<R> vp = ldg_c(a.cg_p + (long)f * V + i0 + off[c]);
+                q.re += a.op.shift * vp.re;
+                q.im += a.op.shift * vp.im;
+              }
               cpx<R> rn = {vr[c].re - alpha * q.re, vr[c].im - alpha * q.im};
               gr[off[c]] = rn;
               acc += (double)rn.re * (double)rn.re + (double)rn.im * (double)rn.im;

