@@ -778,4 +778,66 @@ int orc_cg_shift(int method, const int* L, const double* phi, const double* b_, 
   return 0;
 }
 
+// ----------------------------------------------------------------------------
+// O7 (NEXT-2, second step). Preconditioned shifted system, Eq. 7.14:
+//   (Mtilde^dag Mtilde + sigma (M0^-1)^dag M0^-1) xtilde = btilde,
+//   btilde = (M0^-1)^dag b,  x = M0^-1 xtilde,
+// i.e. Eq. 7.13 with x = M0^-1 xtilde multiplied from the left by (M0^-1)^dag.  The
+// operator is composed literally: Mtilde, Mtilde^dag, and M0^-1 followed by (M0^-1)^dag
+// for the sigma term (no closed form for (M0^-1)^dag M0^-1 is used).  Textbook CG as
+// in orc_cg_pc; stop rule on the residual of the system iterated on (reading G15).
+// info->rel_residual_true is ||b - (M^dag M + sigma) x|| / ||b|| of Eq. 7.13.
+// ----------------------------------------------------------------------------
+int orc_cg_shift_pc(int method, const int* L, const double* phi, const double* b_, double* x_,
+                    const double* m, const double* g, double rho, double sigma, double tol, int max_iter,
+                    orc_cg_info* info, double* history) {
+  const long V = (long)L[0] * L[1] * L[2] * L[3];
+  const long n = 4 * V;
+  const cd* b = reinterpret_cast<const cd*>(b_);
+  cd* x = reinterpret_cast<cd*>(x_);
+  std::vector<cd> bt(n), xt(n, 0.0), r(n), p(n), q(n), w(n), u(n), z(n);
+  auto D = [](std::vector<cd>& v) { return reinterpret_cast<double*>(v.data()); };
+  int rc = orc_apply_M0inv(method, L, m, rho, 1, b_, D(bt));
+  if (rc) return rc;
+  r = bt;
+  p = bt;
+  double btnorm = std::sqrt(dot_re(bt.data(), bt.data(), n));
+  double rr = btnorm * btnorm;
+  if (history) history[0] = 1.0;
+  int k = 0, converged = (btnorm == 0.0);
+  while (!converged && k < max_iter) {
+    ++k;
+    if ((rc = orc_apply_Mtilde(method, L, phi, m, g, rho, 0, D(p), D(w)))) return rc;
+    if ((rc = orc_apply_Mtilde(method, L, phi, m, g, rho, 1, D(w), D(q)))) return rc;
+    if ((rc = orc_apply_M0inv(method, L, m, rho, 0, D(p), D(u)))) return rc;
+    if ((rc = orc_apply_M0inv(method, L, m, rho, 1, D(u), D(z)))) return rc;
+    for (long i = 0; i < n; ++i) q[i] += sigma * z[i];
+    double alpha = rr / dot_re(p.data(), q.data(), n);
+    for (long i = 0; i < n; ++i) {
+      xt[i] += alpha * p[i];
+      r[i] -= alpha * q[i];
+    }
+    double rr_new = dot_re(r.data(), r.data(), n);
+    if (history) history[k] = std::sqrt(rr_new) / btnorm;
+    if (std::sqrt(rr_new) <= tol * btnorm) {
+      rr = rr_new;
+      converged = 1;
+      break;
+    }
+    double beta = rr_new / rr;
+    rr = rr_new;
+    for (long i = 0; i < n; ++i) p[i] = r[i] + beta * p[i];
+  }
+  if ((rc = orc_apply_M0inv(method, L, m, rho, 0, D(xt), x_))) return rc;
+  orc_apply_MdagM(method, L, phi, m, g, rho, x_, D(q));
+  double tr = 0.0, bb = 0.0;
+  for (long i = 0; i < n; ++i) { tr += std::norm(b[i] - q[i] - sigma * x[i]); bb += std::norm(b[i]); }
+  info->iterations = k;
+  info->reliable_updates = 0;
+  info->converged = converged;
+  info->rel_residual_recursive = btnorm > 0 ? std::sqrt(rr) / btnorm : 0.0;
+  info->rel_residual_true = bb > 0 ? std::sqrt(tr / bb) : 0.0;
+  return 0;
+}
+
 }  // extern "C"

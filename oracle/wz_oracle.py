@@ -266,3 +266,41 @@ def cg_shift(phi, b, m, g, sigma, rho=1.0, tol=1e-10, max_iter=100000, method="a
         raise ValueError("oracle cg_shift failed")
     return x, CGInfo(info.iterations, info.reliable_updates, bool(info.converged),
                      info.rel_residual_recursive, info.rel_residual_true, hist[: info.iterations + 1].copy())
+
+
+def cg_shift_pc(phi, b, m, g, sigma, rho=1.0, tol=1e-10, max_iter=100000, method="auto"):
+    """Textbook CG on the preconditioned shifted system of Eq. (7.14),
+    (Mtilde^dag Mtilde + sigma (M0^-1)^dag M0^-1) xtilde = (M0^-1)^dag b, x = M0^-1 xtilde.
+    Returns (x, CGInfo); rel_residual_true refers to (M^dag M + sigma) x = b."""
+    phi = np.ascontiguousarray(phi, dtype=np.complex128)
+    b = np.ascontiguousarray(b, dtype=np.complex128)
+    dims = phi.shape
+    x = np.zeros_like(b)
+    hist = np.zeros(max_iter + 1, dtype=np.float64)
+    info = _Info()
+    rc = lib().orc_cg_shift_pc(_method(dims, method), _dims(dims), _dp(phi), _dp(b), _dp(x), _c2(m), _c2(g),
+                               ctypes.c_double(rho), ctypes.c_double(sigma), ctypes.c_double(tol), int(max_iter),
+                               ctypes.byref(info), _dp(hist))
+    if rc:
+        raise ValueError("oracle cg_shift_pc failed")
+    return x, CGInfo(info.iterations, info.reliable_updates, bool(info.converged),
+                     info.rel_residual_recursive, info.rel_residual_true, hist[: info.iterations + 1].copy())
+
+
+def rational_apply(phi, eta, m, g, alpha0, alphas, betas, rho=1.0, tol=1e-10, max_iter=100000,
+                   pc_cutoff=100.0, method="auto"):
+    """PAPER.md:877-892 Eq. (7.6)-(7.7) with the rule of PAPER.md:948: out = alpha_0 eta +
+    sum_i alpha_i X_i, (M^dag M + beta_i) X_i = eta solved one shift at a time by CG --
+    preconditioned (Eq. 7.14) for beta_i <= pc_cutoff, plain (Eq. 7.13) above it.
+    Returns (out, [CGInfo per shift])."""
+    eta = np.ascontiguousarray(eta, dtype=np.complex128)
+    out = alpha0 * eta
+    infos = []
+    for a_i, b_i in zip(alphas, betas):
+        if b_i <= pc_cutoff:
+            X, info = cg_shift_pc(phi, eta, m, g, float(b_i), rho, tol, max_iter, method)
+        else:
+            X, info = cg_shift(phi, eta, m, g, float(b_i), rho, tol, max_iter, method)
+        out = out + a_i * X
+        infos.append(info)
+    return out, infos

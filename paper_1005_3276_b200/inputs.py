@@ -76,3 +76,22 @@ CONFIGS = {
     "5a": dict(dims=(48, 24, 24, 24), dtype="c64", sigma=0.5, m=0.005, g=1.5, rho=1.0, nsrc=1, tol=1e-6, seed=5),
     "5b": dict(dims=(64, 64, 64, 64), dtype="c64", sigma=0.5, m=0.005, g=1.5, rho=1.0, nsrc=1, tol=1e-6, seed=5),
 }
+
+
+def rational_ladder(d: int = 20, lo: float = 1e-2, hi: float = 1e3, gamma: float = 0.25, pad: float = 4.0):
+    """Synthetic stand-in for the coefficients of Eq. (7.6), which the paper does not print
+    ("chosen to minimize errors over the range of eigenvalues"; d = 20 at
+    PAPER.md:931).  Returns (alpha_0, alpha[d], beta[d]) with
+        x^-gamma ~ alpha_0 + sum_i alpha_i / (x + beta_i)   for lo <= x <= hi,
+    from the trapezoid rule in u = ln t on  x^-gamma = sin(pi gamma)/pi * int_0^inf t^-gamma/(x+t) dt:
+    a geometric ladder of positive shifts beta_i from lo e^-pad to hi e^+pad (all alpha_i > 0),
+    alpha_0 = the tail beyond the last node.  Not Remez-optimal (about 1 % at d = 20, pad = 4 over
+    five decades); what matters here is the form of the input: d shifts spread over the spectrum.
+    These are INPUTS of the method, like phi and b; both sides consume the same arrays."""
+    u = np.linspace(np.log(lo) - pad, np.log(hi) + pad, d)
+    h = u[1] - u[0]
+    c = np.sin(np.pi * gamma) / np.pi
+    beta = np.exp(u)
+    alpha = c * h * np.exp((1.0 - gamma) * u)
+    alpha0 = c * np.exp(-gamma * (u[-1] + 0.5 * h)) / gamma
+    return float(alpha0), alpha, beta
