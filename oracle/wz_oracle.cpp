@@ -514,9 +514,10 @@ int orc_cg(int method, const int* L, const double* phi, const double* b_, double
 //   converged only when that recomputed (true) ||r|| <= tol ||b||.
 static inline cd round_c64(cd z) { return cd((double)(float)z.real(), (double)(float)z.imag()); }
 
-int orc_cg_c64ru(int method, const int* L, const double* phi, const double* b_, double* X_,
-                 const double* m, const double* g, double rho, double tol, int max_iter,
-                 double delta, orc_cg_info* info, double* history) {
+// sigma: the same loop on the shifted system (M^dag M + sigma) x = b of Eq. 7.13 (sigma = 0: Eq. 7.8).
+int orc_cg_c64ru_shift(int method, const int* L, const double* phi, const double* b_, double* X_,
+                       const double* m, const double* g, double rho, double sigma, double tol, int max_iter,
+                       double delta, orc_cg_info* info, double* history) {
   const long V = (long)L[0] * L[1] * L[2] * L[3];
   const long n = 4 * V;
   const cd* b = reinterpret_cast<const cd*>(b_);
@@ -535,7 +536,7 @@ int orc_cg_c64ru(int method, const int* L, const double* phi, const double* b_, 
     int rc = orc_apply_MdagM(method, L, phi, m, g, rho, reinterpret_cast<double*>(p.data()),
                              reinterpret_cast<double*>(q.data()));
     if (rc) return rc;
-    for (long i = 0; i < n; ++i) q[i] = round_c64(q[i]);
+    for (long i = 0; i < n; ++i) q[i] = round_c64(q[i] + sigma * p[i]);
     double alpha = rr / dot_re(p.data(), q.data(), n);
 #pragma omp parallel for schedule(static)
     for (long i = 0; i < n; ++i) {
@@ -551,7 +552,7 @@ int orc_cg_c64ru(int method, const int* L, const double* phi, const double* b_, 
       orc_apply_MdagM(method, L, phi, m, g, rho, X_, reinterpret_cast<double*>(q.data()));
       double tr = 0.0;
       for (long i = 0; i < n; ++i) {
-        cd d = b[i] - q[i];
+        cd d = b[i] - q[i] - sigma * X[i];
         tr += std::norm(d);
         r[i] = round_c64(d);
       }
@@ -572,7 +573,7 @@ int orc_cg_c64ru(int method, const int* L, const double* phi, const double* b_, 
     for (long i = 0; i < n; ++i) X[i] += x[i];
     orc_apply_MdagM(method, L, phi, m, g, rho, X_, reinterpret_cast<double*>(q.data()));
     double tr = 0.0;
-    for (long i = 0; i < n; ++i) tr += std::norm(b[i] - q[i]);
+    for (long i = 0; i < n; ++i) tr += std::norm(b[i] - q[i] - sigma * X[i]);
     true_rel = bnorm > 0 ? std::sqrt(tr) / bnorm : 0.0;
   }
   info->iterations = k;
@@ -581,6 +582,11 @@ int orc_cg_c64ru(int method, const int* L, const double* phi, const double* b_, 
   info->rel_residual_recursive = bnorm > 0 ? std::sqrt(rr) / bnorm : 0.0;
   info->rel_residual_true = true_rel;
   return 0;
+}
+int orc_cg_c64ru(int method, const int* L, const double* phi, const double* b_, double* X_,
+                 const double* m, const double* g, double rho, double tol, int max_iter,
+                 double delta, orc_cg_info* info, double* history) {
+  return orc_cg_c64ru_shift(method, L, phi, b_, X_, m, g, rho, 0.0, tol, max_iter, delta, info, history);
 }
 
 // ----------------------------------------------------------------------------

@@ -162,17 +162,18 @@ def cg(phi, b, m, g, rho=1.0, tol=1e-10, max_iter=100000, method="auto"):
                      info.rel_residual_recursive, info.rel_residual_true, hist[: info.iterations + 1].copy())
 
 
-def cg_c64ru(phi, b, m, g, rho=1.0, tol=1e-6, max_iter=100000, delta=0.1, method="auto"):
-    """complex64-vector CG with reliable updates (oracle variant O4').  Returns (X, CGInfo)."""
+def cg_c64ru(phi, b, m, g, rho=1.0, tol=1e-6, max_iter=100000, delta=0.1, method="auto", sigma=0.0):
+    """complex64-vector CG with reliable updates (oracle variant O4'); sigma: on the shifted
+    system (M^dag M + sigma) x = b of Eq. (7.13).  Returns (X, CGInfo)."""
     phi = np.ascontiguousarray(phi, dtype=np.complex128)
     b = np.ascontiguousarray(b, dtype=np.complex128)
     dims = phi.shape
     X = np.zeros_like(b)
     hist = np.zeros(max_iter + 1, dtype=np.float64)
     info = _Info()
-    rc = lib().orc_cg_c64ru(_method(dims, method), _dims(dims), _dp(phi), _dp(b), _dp(X), _c2(m), _c2(g),
-                            ctypes.c_double(rho), ctypes.c_double(tol), int(max_iter), ctypes.c_double(delta),
-                            ctypes.byref(info), _dp(hist))
+    rc = lib().orc_cg_c64ru_shift(_method(dims, method), _dims(dims), _dp(phi), _dp(b), _dp(X), _c2(m), _c2(g),
+                                  ctypes.c_double(rho), ctypes.c_double(sigma), ctypes.c_double(tol), int(max_iter),
+                                  ctypes.c_double(delta), ctypes.byref(info), _dp(hist))
     if rc:
         raise ValueError("oracle cg_c64ru failed")
     return X, CGInfo(info.iterations, info.reliable_updates, bool(info.converged),

@@ -412,12 +412,17 @@ def test_cg_shift_vs_oracle(wz, orc, inp, dims, dtype, tol):
         x = x.cpu().numpy()
         for j in range(2):
             bj = b[j].astype(np.complex128)
-            xo, io = orc.cg_shift(phi128, bj, m, g, sigma, rho, tol, 20000)
+            # complex64 plans follow reading G9: compare with the oracle's complex64 + reliable-update loop
+            if dtype == "c128":
+                xo, io = orc.cg_shift(phi128, bj, m, g, sigma, rho, tol, 20000)
+            else:
+                xo, io = orc.cg_c64ru(phi128, bj, m, g, rho, tol, 20000, sigma=sigma)
             true_res = rel(orc.apply_MdagM(phi128, x[j], m, g, rho) + sigma * x[j], bj)
             print("shift %g %s %s: iterations gpu=%d oracle=%d true residual %.2e"
                   % (sigma, dims, dtype, infos[j].iterations, io.iterations, true_res))
             assert infos[j].converged and io.converged
-            assert abs(infos[j].iterations - io.iterations) <= max(2, io.iterations // 100)
+            bound = max(2, io.iterations // 100) if dtype == "c128" else max(2, io.iterations // 20)  # G10
+            assert abs(infos[j].iterations - io.iterations) <= bound
             assert true_res <= tol * (1.0 + 1e-3)
             assert abs(true_res - infos[j].rel_residual_true) <= 0.05 * tol
             assert rel(x[j], xo) <= (1e-7 if dtype == "c128" else 5e-4)
