@@ -134,6 +134,29 @@ wz_status wz_cg_solve_shift(wz_plan *plan, const void *phi, const void *b, void 
                             const double m[2], const double g[2], double rho, double sigma,
                             double tol, int max_iter, int nbatch, wz_cg_info *info);
 
+/* ---- Preconditioned shifted system and the rational sum (Eq. 7.14; 877-892 Eq. 7.6-7.7;
+ *      948-950 cutoff rule; Table VII) ----
+ * wz_cg_solve_shift_pc: with x = M0^-1 xtilde, CG on
+ *     (Mtilde^dag Mtilde + sigma (M0^-1)^dag M0^-1) xtilde = btilde,  btilde = (M0^-1)^dag b      (Eq. 7.14)
+ *   from xtilde0 = 0, stop rule on THIS system's residual (G15), then x = M0^-1 xtilde.  The sigma
+ *   term rides through the same five passes as wz_cg_solve_pc (pass C adds sigma M0^-1 p to what pass D
+ *   multiplies by (M0^-1)^dag).  m != 0 and sigma >= 0 required (else WZ_EINVAL); sigma = 0 is
+ *   wz_cg_solve_pc.  x: complex128; info.rel_residual_true = ||b - (M^dag M + sigma) x|| / ||b||.
+ * wz_rational_apply: out = alpha0 eta + sum_{i < nshift} alphas[i] X_i with (M^dag M + betas[i]) X_i = eta
+ *   (Eq. 7.6-7.7), one solve per shift for the whole batch: wz_cg_solve_shift_pc when betas[i] <= pc_cutoff
+ *   (the paper uses 100) and m != 0, wz_cg_solve_shift otherwise.  alphas, betas: HOST arrays of nshift
+ *   doubles, betas[i] >= 0.  eta: nbatch spinors of the plan's dtype; out: nbatch spinors, ALWAYS
+ *   complex128 (device; must not alias eta).  info: HOST array of nshift * nbatch entries, [shift][source].
+ *   Returns WZ_ENOTCONVERGED if any solve hit max_iter (out then holds the sum of the last iterates).
+ *   Synchronises the stream. */
+wz_status wz_cg_solve_shift_pc(wz_plan *plan, const void *phi, const void *b, void *x,
+                               const double m[2], const double g[2], double rho, double sigma,
+                               double tol, int max_iter, int nbatch, wz_cg_info *info);
+wz_status wz_rational_apply(wz_plan *plan, const void *phi, const void *eta, void *out,
+                            const double m[2], const double g[2], double rho, double alpha0,
+                            const double *alphas, const double *betas, int nshift, double pc_cutoff,
+                            double tol, int max_iter, int nbatch, wz_cg_info *info);
+
 /* ---- Locality probe (Eq. 3.9-3.11, Fig. 1) ----
  * wz_apply_Dslash: out = Dslash in = (1 - D2/2)^-1 D1 in (the fermion matrix at m = g = 0); in != out.
  * wz_locality_profile: psi = Dslash eta for a unit point source at the origin in spin component

@@ -146,6 +146,21 @@ k_resid(const TB* __restrict__ b, const double* __restrict__ q, TR* __restrict__
   grid_reduce<FIN>(acc, red, blockIdx.x, gridDim.x, sh);
 }
 
+// Rational sum, Eq. (7.6):  out = alpha_0 eta  (first = 1)  or  out += alpha_i X_i,
+// complex128 accumulation; one source per grid row.  TB: storage type of the term.
+template <typename TB>
+__global__ void __launch_bounds__(CGK_NT)
+k_rat_term(double* __restrict__ out, const TB* __restrict__ v, double a, long n, int first) {
+  out += blockIdx.y * n; v += blockIdx.y * n;
+  for (long i = ((long)blockIdx.x * blockDim.x + threadIdx.x) * 2; i < n;
+       i += (long)gridDim.x * blockDim.x * 2) {
+    double2 o = first ? make_double2(0.0, 0.0) : *reinterpret_cast<double2*>(out + i);
+    o.x += a * (double)v[i];
+    o.y += a * (double)v[i + 1];
+    *reinterpret_cast<double2*>(out + i) = o;
+  }
+}
+
 // Locality probe, Eq. (3.10)-(3.11):  f(r) = max{ ||psi(x)|| : ||x||_1 = r } with
 // the taxi-driver distance to the origin (shorter way round each axis) and ||.|| the norm over
 // the four spin components.  f holds ||.||^2 as the bit pattern of a non-negative double, so

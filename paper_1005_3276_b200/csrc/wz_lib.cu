@@ -221,6 +221,7 @@ struct wz_plan {
   cpx<double>* q128 = nullptr;    // A X in complex128 (reliable updates, true residual), one spinor
   cpx<double>* phi128 = nullptr;  // C64 plans: phi widened
   cpx<double>* btilde128 = nullptr;  // C64 plans, preconditioned solves: (M0^-1)^dag b in complex128, per source
+  cpx<double>* ratX = nullptr;       // wz_rational_apply: the X_i of the current shift, max_batch spinors
   double* partials = nullptr;
   unsigned* counter = nullptr;
   CGState* d_state = nullptr;
@@ -446,7 +447,9 @@ wz_status apply_M_impl(wz_plan* pl, int dagger, const cpx<R>* phi, const double 
 // the solve being active and pass C leaves alpha = rho/<p, A p> in the CG state. -----
 template <typename R>
 wz_status apply_MdagM_impl(wz_plan* pl, const cpx<R>* phi, const double m[2], const double g[2],
-                           double rho, const cpx<R>* in, cpx<R>* out, int nb, bool cg, bool pc = false) {
+                           double rho, const cpx<R>* in, cpx<R>* out, int nb, bool cg, bool pc = false,
+                           double sigma_pc = 0.0) {
+  // sigma_pc (pc only): + sigma (M0^-1)^dag M0^-1, the operator of Eq. 7.14
   // pc: Mtilde^dag Mtilde with Mtilde = M M0^-1 = 1 + Y M0^-1: same five passes,
   // the multiply passes apply M0^-1 / (M0^-1)^dag, the site-local steps use Y alone
   OpWS<R>& ws = ws_of<R>(pl);
@@ -465,6 +468,7 @@ wz_status apply_MdagM_impl(wz_plan* pl, const cpx<R>* phi, const double m[2], co
   if ((s = mult_pass<R>(pl, ws, b, cur, nb)) != WZ_OK) return s;  // B
   a.in = cur; a.out = cur;
   a.psi = in; a.phi = phi; a.site_out = ws.chi; a.op = make_op<R>(m, g, rho, 0, pc);
+  if (pc) a.op.shift = (R)sigma_pc;
   if (cg) {
     a.red = red_of(pl);
     if ((int)(pl->I / ws.p01->min_nseg()) * 4 > pl->npartials) return WZ_EINVAL;
@@ -513,7 +517,8 @@ wz_status cg_iteration(wz_plan* pl, const cpx<R>* phi, const double m[2], const 
                        cpx<R>* r, cpx<R>* p, cpx<R>* x, int nb, bool pc, double sigma = 0.0) {
   // sigma != 0: the shifted system (M^dag M + sigma) x = b (Eq. 7.13): pass A' also
   // reduces <p,p> (alpha = rho / (||M p||^2 + sigma <p,p>)), pass E' uses q + sigma p
-  const bool sh = sigma != 0.0;
+  // with pc the shift enters pass C instead (Eq. 7.14: + sigma (M0^-1)^dag M0^-1, see wz_p01.cuh)
+  const bool sh = sigma != 0.0 && !pc;
   OpWS<R>& ws = ws_of<R>(pl);
   if ((int)(pl->I / ws.p01->min_nseg()) * 4 > pl->npartials) return WZ_EINVAL;
   const R invV = (R)(1.0 / (double)pl->V);
@@ -531,6 +536,7 @@ wz_status cg_iteration(wz_plan* pl, const cpx<R>* phi, const double m[2], const 
   if ((s = mult_pass<R>(pl, ws, b, cur, nb)) != WZ_OK) return s;
   a.in = cur; a.out = cur;
   a.psi = p; a.phi = phi; a.site_out = ws.chi; a.op = make_op<R>(m, g, rho, 0, pc);
+  if (pc) a.op.shift = (R)sigma;
   a.red = red_of(pl);
   if ((s = launch_p01<R>(pl, WZ_K_P01_MID, ws.p01->mid_pq, a, nb)) != WZ_OK) return s;
   b.sign = pc ? R(1) : R(-1);
@@ -538,7 +544,7 @@ wz_status cg_iteration(wz_plan* pl, const cpx<R>* phi, const double m[2], const 
   if ((s = mult_pass<R>(pl, ws, b, cur, nb)) != WZ_OK) return s;
   a.in = cur; a.out = cur;
   a.psi = ws.chi; a.site_out = nullptr; a.op = make_op<R>(m, g, rho, 1, pc);
-  a.cg_r = r; a.cg_p = p; a.cg_x = x; a.op.shift = (R)sigma;
+  a.cg_r = r; a.cg_p = p; a.cg_x = x; a.op.shift = sh ? (R)sigma : R(0);
   return launch_p01<R>(pl, WZ_K_P01_ENDCG, sh ? ws.p01->endcg_s : ws.p01->endcg, a, nb);
 }
 
@@ -771,7 +777,8 @@ template <typename R>
 wz_status cg_batch(wz_plan* pl, const cpx<R>* phi, const cpx<R>* b, cpx<double>* X, const double m[2],
                    const double g[2], double rho, double tol, int max_iter, int nb, wz_cg_info* info,
                    bool pc, double sigma = 0.0) {
-  // sigma: shift of the system (M^dag M + sigma) x = b (Eq. 7.13); not combined with pc
+  // sigma: shift of the system (M^dag M + sigma) x = b (Eq. 7.13); with pc the system
+  // iterated on is Eq. 7.14, (Mtilde^dag Mtilde + sigma (M0^-1)^dag M0^-1) xtilde = btilde
   constexpr bool kRU = (sizeof(R) == 4);
   constexpr int N = vec16<R>::N;
   const long n = 8 * pl->V;       // real entries of one spinor
@@ -785,7 +792,7 @@ wz_status cg_batch(wz_plan* pl, const cpx<R>* phi, const cpx<R>* b, cpx<double>*
   memset(h.data(), 0, sizeof(CGState) * nb);
   for (int j = 0; j < nb; ++j) {
     h[j].tol = tol; h[j].delta = kDelta; h[j].max_iter = max_iter; h[j].use_ru = kRU ? 1 : 0;
-    h[j].true_rr = -1.0; h[j].shift = sigma;
+    h[j].true_rr = -1.0; h[j].shift = pc ? 0.0 : sigma;  // pc: the shift is inside pass C's reduction
     if (max_iter == 0) h[j].stop = 1;
   }
   WZ_CUDA(cudaMemcpyAsync(pl->d_state, h.data(), sizeof(CGState) * nb, cudaMemcpyHostToDevice, st));
@@ -827,7 +834,7 @@ wz_status cg_batch(wz_plan* pl, const cpx<R>* phi, const cpx<R>* b, cpx<double>*
     return WZ_OK;
   };
   // residual of source j recomputed in complex128:  q128 = A X_j;  d = b_j - q128
-  auto xsh = [&](int j) -> const double* { return sigma != 0.0 ? (const double*)(X + j * n1) : nullptr; };
+  auto xsh = [&](int j) -> const double* { return (sigma != 0.0 && !pc) ? (const double*)(X + j * n1) : nullptr; };
   auto residual128 = [&](int j, bool update_r) -> wz_status {
     RedArgs ra = red_of(pl).for_source(j);
     struct Override {  // the one-source complex128 matvec is not part of the batched iteration
@@ -840,7 +847,7 @@ wz_status cg_batch(wz_plan* pl, const cpx<R>* phi, const cpx<R>* b, cpx<double>*
         ProfScope ps(pl, WZ_K_OTHER);
         k_ru_accum<<<dim3(gv4, 1), CGK_NT, 0, st>>>((double*)(X + j * n1), (float*)(xs + j * n), n);
       }
-      wz_status s2 = apply_MdagM_impl<double>(pl, pl->phi128, m, g, rho, X + j * n1, pl->q128, 1, false, pc);
+      wz_status s2 = apply_MdagM_impl<double>(pl, pl->phi128, m, g, rho, X + j * n1, pl->q128, 1, false, pc, sigma);
       if (s2 != WZ_OK) return s2;
       ProfScope ps(pl, WZ_K_OTHER);
       if (pc) {  // rhs of the preconditioned system: btilde, kept in complex128
@@ -926,14 +933,16 @@ wz_status cg_batch(wz_plan* pl, const cpx<R>* phi, const cpx<R>* b, cpx<double>*
       if ((s = apply_M0inv_impl<double>(pl, 0, m, rho, X + j * n1, X + j * n1, 1)) != WZ_OK) return s;
       if ((s = apply_MdagM_impl<double>(pl, pl->phi128, m, g, rho, X + j * n1, pl->q128, 1, false)) != WZ_OK) return s;
       ProfScope ps(pl, WZ_K_OTHER);
-      k_resid<float, float, FIN_TRUE><<<dim3(gv2, 1), CGK_NT, 0, st>>>((const float*)(b + j * n1), (const double*)pl->q128, nullptr, n, ra);
+      k_resid<float, float, FIN_TRUE><<<dim3(gv2, 1), CGK_NT, 0, st>>>((const float*)(b + j * n1), (const double*)pl->q128, nullptr, n, ra,
+                                                                       sigma != 0.0 ? (const double*)(X + j * n1) : nullptr, sigma);
       k_norm2<float, FIN_AUX><<<dim3(gv2, 1), CGK_NT, 0, st>>>((const float*)(b + j * n1), n, ra);
       pl->launches++;
     } else {
       if ((s = apply_M0inv_impl<double>(pl, 0, m, rho, X + j * n1, X + j * n1, 1)) != WZ_OK) return s;
       if ((s = apply_MdagM_impl<double>(pl, (const cpx<double>*)phi, m, g, rho, X + j * n1, pl->q128, 1, false)) != WZ_OK) return s;
       ProfScope ps(pl, WZ_K_OTHER);
-      k_resid<double, double, FIN_TRUE><<<dim3(gv2, 1), CGK_NT, 0, st>>>((const double*)(b + j * n1), (const double*)pl->q128, nullptr, n, ra);
+      k_resid<double, double, FIN_TRUE><<<dim3(gv2, 1), CGK_NT, 0, st>>>((const double*)(b + j * n1), (const double*)pl->q128, nullptr, n, ra,
+                                                                         sigma != 0.0 ? (const double*)(X + j * n1) : nullptr, sigma);
       k_norm2<double, FIN_AUX><<<dim3(gv2, 1), CGK_NT, 0, st>>>((const double*)(b + j * n1), n, ra);
       pl->launches++;
     }
@@ -958,7 +967,7 @@ static wz_status cg_solve_any(wz_plan* pl, const void* phi, const void* b, void*
                               const double g[2], double rho, double tol, int max_iter, int nbatch,
                               wz_cg_info* info, bool pc, double sigma = 0.0) {
   g_err[0] = 0;
-  if (!(sigma >= 0.0) || (pc && sigma != 0.0)) return WZ_EINVAL;
+  if (!(sigma >= 0.0)) return WZ_EINVAL;
   if (!pl || !phi || !b || !x || !m || !g || !info) return WZ_EINVAL;
   if (!(rho > 0.0 && rho < 2.0) || !(tol > 0.0) || max_iter < 0) return WZ_EINVAL;
   if (nbatch < 0 || nbatch > pl->max_batch) return WZ_EINVAL;
@@ -1000,6 +1009,52 @@ wz_status wz_cg_solve_shift(wz_plan* pl, const void* phi, const void* b, void* x
 wz_status wz_cg_solve_pc(wz_plan* pl, const void* phi, const void* b, void* x, const double m[2],
                          const double g[2], double rho, double tol, int max_iter, int nbatch, wz_cg_info* info) {
   return cg_solve_any(pl, phi, b, x, m, g, rho, tol, max_iter, nbatch, info, true);
+}
+
+wz_status wz_cg_solve_shift_pc(wz_plan* pl, const void* phi, const void* b, void* x, const double m[2],
+                               const double g[2], double rho, double sigma, double tol, int max_iter, int nbatch,
+                               wz_cg_info* info) {
+  return cg_solve_any(pl, phi, b, x, m, g, rho, tol, max_iter, nbatch, info, true, sigma);
+}
+
+// Eq. (7.6)-(7.7) with the cutoff rule of PAPER.md:948: one CG solve per shift ("for each i"),
+// preconditioned (Eq. 7.14) up to pc_cutoff, plain (Eq. 7.13) above; terms summed in complex128.
+wz_status wz_rational_apply(wz_plan* pl, const void* phi, const void* eta, void* out, const double m[2],
+                            const double g[2], double rho, double alpha0, const double* alphas,
+                            const double* betas, int nshift, double pc_cutoff, double tol, int max_iter,
+                            int nbatch, wz_cg_info* info) {
+  g_err[0] = 0;
+  if (!pl || !phi || !eta || !out || !m || !g || !info || nshift < 0 || (nshift > 0 && (!alphas || !betas)))
+    return WZ_EINVAL;
+  if (nbatch < 0 || nbatch > pl->max_batch) return WZ_EINVAL;
+  for (int i = 0; i < nshift; ++i)
+    if (!(betas[i] >= 0.0)) return WZ_EINVAL;
+  if (nbatch == 0) return WZ_OK;
+  const size_t n1 = (size_t)4 * pl->V;
+  const long n = 8 * pl->V;
+  if (!pl->ratX && !dev_alloc(pl, &pl->ratX, (size_t)pl->max_batch * n1)) return WZ_ENOMEM;
+  const int gv2 = vec_grid(n, 2);
+  {
+    ProfScope ps(pl, WZ_K_OTHER);
+    if (pl->dtype == WZ_C64)
+      k_rat_term<float><<<dim3(gv2, nbatch), CGK_NT, 0, pl->stream>>>((double*)out, (const float*)eta, alpha0, n, 1);
+    else
+      k_rat_term<double><<<dim3(gv2, nbatch), CGK_NT, 0, pl->stream>>>((double*)out, (const double*)eta, alpha0, n, 1);
+  }
+  WZ_CUDA(cudaGetLastError());
+  bool all_ok = true;
+  for (int i = 0; i < nshift; ++i) {
+    const bool pc = betas[i] <= pc_cutoff && !(m[0] == 0.0 && m[1] == 0.0);
+    wz_status s = cg_solve_any(pl, phi, eta, pl->ratX, m, g, rho, tol, max_iter, nbatch, info + (size_t)i * nbatch,
+                               pc, betas[i]);
+    if (s == WZ_ENOTCONVERGED) all_ok = false;
+    else if (s != WZ_OK) return s;
+    ProfScope ps(pl, WZ_K_OTHER);
+    k_rat_term<double><<<dim3(gv2, nbatch), CGK_NT, 0, pl->stream>>>((double*)out, (const double*)pl->ratX, alphas[i], n, 0);
+    WZ_CUDA(cudaGetLastError());
+  }
+  WZ_CUDA(cudaStreamSynchronize(pl->stream));
+  return all_ok ? WZ_OK : WZ_ENOTCONVERGED;
 }
 
 wz_status wz_apply_M0inv(wz_plan* pl, int dagger, const double m[2], double rho, const void* in, void* out,

@@ -266,7 +266,7 @@ k_p01(const P01Args<R> a) {
       //      spin 0,1 = P-, spin 2,3 = P+; M^dag swaps w and w^* ----
       // Preconditioned operator (op.pc): Mtilde = M M0^-1 = 1 + Y M0^-1 with
       // Y = 2 g phi P+ + 2 g^* phi^* P-, so the same passes serve with other site-local formulas:
-      //   MID:  w = psi + Y t  (stored, ||w||^2),  then the forward half transforms Y^dag w;
+      //   MID:  w = psi + Y t  (stored, ||w||^2),  then the forward half transforms Y^dag w (+ sigma t, Eq. 7.14);
       //   END / ENDCG:  q = t + w  (no phi).
       const bool use_conj = (comp < 2) != (a.op.dagger != 0);
       const bool pc = a.op.pc != 0;
@@ -326,11 +326,17 @@ k_p01(const P01Args<R> a) {
               cpx<R> v = base;
               v.re += w.re * mul.re - w.im * mul.im;
               v.im += w.re * mul.im + w.im * mul.re;
-              // value that enters the forward half (MID): v, or Y^dag v for the preconditioned operator
-              x[k0 + c] = pc_swap ? cpx<R>{w.re * v.re + w.im * v.im, w.re * v.im - w.im * v.re} : v;
+              // value that enters the forward half (MID): v, or Y^dag v for the preconditioned operator;
+              // preconditioned shifted system (Eq. 7.14): + sigma t with t = M0^-1 p, which
+              // pass D turns into sigma (M0^-1)^dag M0^-1 p, and <p, A p> = ||w||^2 + sigma ||t||^2
+              const cpx<R> tin = x[k0 + c];
+              x[k0 + c] = pc_swap ? cpx<R>{w.re * v.re + w.im * v.im + a.op.shift * tin.re,
+                                           w.re * v.im - w.im * v.re + a.op.shift * tin.im} : v;
               gso[off[c]] = v;
-              if (FIN != FIN_STORE || a.red.partials)
+              if (FIN != FIN_STORE || a.red.partials) {
                 acc += (double)v.re * (double)v.re + (double)v.im * (double)v.im;
+                if (pc_swap) acc += (double)a.op.shift * ((double)tin.re * (double)tin.re + (double)tin.im * (double)tin.im);
+              }
             }
           }
         }

@@ -25,7 +25,7 @@ EXPORTS = [
     "wz_cg_solve", "wz_plan_launch_count", "wz_plan_reset_launch_count",
     "wz_plan_profile", "wz_plan_profile_read", "wz_kind_name",
     "wz_apply_M0inv", "wz_apply_MtdagMt", "wz_cg_solve_pc", "wz_apply_Dslash", "wz_locality_profile",
-    "wz_cg_solve_shift",
+    "wz_cg_solve_shift", "wz_cg_solve_shift_pc", "wz_rational_apply",
 ]
 
 
@@ -79,6 +79,9 @@ def lib() -> ctypes.CDLL:
         L.wz_cg_solve.argtypes = [vp, vp, vp, vp, d2, d2, cd, cd, ci, ci, ctypes.POINTER(_CGInfo)]
         L.wz_cg_solve_pc.argtypes = L.wz_cg_solve.argtypes
         L.wz_cg_solve_shift.argtypes = [vp, vp, vp, vp, d2, d2, cd, cd, cd, ci, ci, ctypes.POINTER(_CGInfo)]
+        L.wz_cg_solve_shift_pc.argtypes = L.wz_cg_solve_shift.argtypes
+        L.wz_rational_apply.argtypes = [vp, vp, vp, vp, d2, d2, cd, cd, d2, d2, ci, cd, cd, ci, ci,
+                                        ctypes.POINTER(_CGInfo)]
         L.wz_apply_M0inv.argtypes = [vp, ci, d2, cd, vp, vp, ci]
         L.wz_apply_MtdagMt.argtypes = [vp, vp, d2, d2, cd, vp, vp, ci]
         L.wz_apply_Dslash.argtypes = [vp, cd, vp, vp, ci]
@@ -246,7 +249,8 @@ class Plan:
                  out=None, raise_on_fail: bool = True, precondition: bool = False, sigma=None):
         """Solve M^dag M x = b per source (precondition=True: through the free-inverse
         preconditioned system, wz_cg_solve_pc; sigma given: the shifted system
-        (M^dag M + sigma) x = b, wz_cg_solve_shift).  Returns (x complex128, [CGInfo])."""
+        (M^dag M + sigma) x = b, wz_cg_solve_shift; both: Eq. 7.14, wz_cg_solve_shift_pc).
+        Returns (x complex128, [CGInfo])."""
         nb = self._spinor(b)
         self._phi(phi)
         if out is None:
@@ -254,10 +258,9 @@ class Plan:
         self._spinor(out, torch.complex128)
         infos = (_CGInfo * nb)()
         if sigma is not None:
-            if precondition:
-                raise ValueError("sigma and precondition cannot be combined")
-            st = lib().wz_cg_solve_shift(self._h, phi.data_ptr(), b.data_ptr(), out.data_ptr(), _c2(m), _c2(g),
-                                         float(rho), float(sigma), float(tol), int(max_iter), nb, infos)
+            fn = lib().wz_cg_solve_shift_pc if precondition else lib().wz_cg_solve_shift
+            st = fn(self._h, phi.data_ptr(), b.data_ptr(), out.data_ptr(), _c2(m), _c2(g),
+                    float(rho), float(sigma), float(tol), int(max_iter), nb, infos)
         else:
             fn = lib().wz_cg_solve_pc if precondition else lib().wz_cg_solve
             st = fn(self._h, phi.data_ptr(), b.data_ptr(), out.data_ptr(), _c2(m), _c2(g),
@@ -266,6 +269,31 @@ class Plan:
             _check(st)
         res = [CGInfo(i.iterations, i.reliable_updates, bool(i.converged), i.rel_residual_recursive,
                       i.rel_residual_true) for i in infos]
+        return out, res
+
+
+    def rational_apply(self, phi, eta, m, g, alpha0, alphas, betas, rho: float = 1.0, tol: float = 1e-6,
+                       max_iter: int = 100000, pc_cutoff: float = 100.0, out=None, raise_on_fail: bool = True):
+        """out = alpha0 eta + sum_i alphas[i] (M^dag M + betas[i])^-1 eta (wz_rational_apply, Eq. 7.6-7.7).
+        Returns (out complex128, infos[shift][source])."""
+        nb = self._spinor(eta)
+        self._phi(phi)
+        if out is None:
+            out = torch.empty(eta.shape, dtype=torch.complex128, device=eta.device)
+        self._spinor(out, torch.complex128)
+        d = len(alphas)
+        assert len(betas) == d
+        ca = (ctypes.c_double * max(d, 1))(*[float(a) for a in alphas])
+        cb = (ctypes.c_double * max(d, 1))(*[float(b) for b in betas])
+        infos = (_CGInfo * max(d * nb, 1))()
+        st = lib().wz_rational_apply(self._h, phi.data_ptr(), eta.data_ptr(), out.data_ptr(), _c2(m), _c2(g),
+                                     float(rho), float(alpha0), ca, cb, d, float(pc_cutoff), float(tol),
+                                     int(max_iter), nb, infos)
+        if st != WZ_OK and not (st == WZ_ENOTCONVERGED and not raise_on_fail):
+            _check(st)
+        res = [[CGInfo(infos[i * nb + j].iterations, infos[i * nb + j].reliable_updates,
+                       bool(infos[i * nb + j].converged), infos[i * nb + j].rel_residual_recursive,
+                       infos[i * nb + j].rel_residual_true) for j in range(nb)] for i in range(d)]
         return out, res
 
 

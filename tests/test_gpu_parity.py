@@ -442,3 +442,109 @@ def test_cg_shift_zero_is_plain_solve_and_errors(wz, inp):
     with pytest.raises(wz.WZError) as e:
         plan.cg_solve(d_phi, d_b, 0.05, 1.0, 1.0, 1e-10, 100, sigma=-1.0)
     assert e.value.status == wz.WZ_EINVAL
+
+
+# ---- NEXT-2 (second step): preconditioned shifted system and the rational sum
+#      (Eq. 7.14; 877-892 Eq. 7.6-7.7; 948-950 cutoff rule; Table VII) ----
+
+@pytest.mark.parametrize("dims,dtype,tol", [((8, 8, 8, 8), "c128", 1e-10), ((8, 4, 16, 8), "c128", 1e-12),
+                                            ((8, 8, 8, 8), "c64", 1e-6), ((16, 16, 16, 16), "c64", 1e-6),
+                                            ((48, 24, 24, 24), "c64", 1e-6)])
+def test_cg_shift_pc_vs_oracle(wz, orc, inp, dims, dtype, tol):
+    """Eq. 7.14 at weak coupling (m = 1, g = 1/5) over a ladder of shifts: iteration counts against the
+    oracle's literal composition (+-2; 5 % for complex64, G10), solution, and the true residual of the
+    shifted ORIGINAL system (M^dag M + sigma) x = b recomputed by the oracle."""
+    m, g, rho = 1.0, 0.2, 1.0
+    phi = inp.make_phi(8, dims, 0.5, NPDT[dtype])
+    b = inp.make_sources(8, 2, dims, NPDT[dtype])
+    plan = wz.Plan(dims, dtype, 2)
+    d_phi, d_b = torch.from_numpy(phi).cuda(), torch.from_numpy(b).cuda()
+    phi128 = phi.astype(np.complex128)
+    for sigma in (0.01, 1.0, 100.0):
+        x, infos = plan.cg_solve(d_phi, d_b, m, g, rho, tol, 2000, precondition=True, sigma=sigma)
+        x = x.cpu().numpy()
+        for j in range(2):
+            bj = b[j].astype(np.complex128)
+            xo, io = orc.cg_shift_pc(phi128, bj, m, g, sigma, rho, tol, 2000)
+            true_res = rel(orc.apply_MdagM(phi128, x[j], m, g, rho) + sigma * x[j], bj)
+            print("shift-pc %g %s %s: iterations gpu=%d oracle=%d true residual %.2e (oracle %.2e)"
+                  % (sigma, dims, dtype, infos[j].iterations, io.iterations, true_res, io.rel_residual_true))
+            assert infos[j].converged and io.converged
+            bound = 2 if dtype == "c128" else max(2, io.iterations // 20)
+            assert abs(infos[j].iterations - io.iterations) <= bound
+            assert abs(true_res - infos[j].rel_residual_true) <= 0.05 * max(true_res, tol)
+            assert true_res <= 20 * tol
+            assert rel(x[j], xo) <= (1e-8 if dtype == "c128" else 1e-4)
+
+
+def test_cg_shift_pc_special_cases_and_errors(wz, orc, inp):
+    cfg = inp.CONFIGS[2]
+    dims = cfg["dims"]
+    phi = inp.make_phi(cfg["seed"], dims, cfg["sigma"])
+    b = inp.make_sources(cfg["seed"], 1, dims)
+    plan = wz.Plan(dims, "c128", 1)
+    d_phi, d_b = torch.from_numpy(phi).cuda(), torch.from_numpy(b).cuda()
+    # sigma = 0 is the preconditioned solve, bit for bit
+    x0, i0 = plan.cg_solve(d_phi, d_b, 1.0, 0.2, 1.0, 1e-10, 2000, precondition=True)
+    x1, i1 = plan.cg_solve(d_phi, d_b, 1.0, 0.2, 1.0, 1e-10, 2000, precondition=True, sigma=0.0)
+    assert i0[0].iterations == i1[0].iterations and torch.equal(x0, x1)
+    # strong coupling (config 2): Eq. 7.14 and Eq. 7.13 have the same solution
+    xa, ia = plan.cg_solve(d_phi, d_b, cfg["m"], cfg["g"], 1.0, 1e-10, 20000, sigma=0.5)
+    xb, ib = plan.cg_solve(d_phi, d_b, cfg["m"], cfg["g"], 1.0, 1e-10, 20000, precondition=True, sigma=0.5)
+    print("config 2, sigma 0.5: plain %d iterations, preconditioned %d" % (ia[0].iterations, ib[0].iterations))
+    assert ib[0].converged and rel(xb.cpu().numpy(), xa.cpu().numpy()) <= 1e-7
+    # g = 0, sigma = 0: the operator is the identity, one iteration
+    _, i2 = plan.cg_solve(d_phi, d_b, 1.0, 0.0, 1.0, 1e-10, 100, precondition=True, sigma=0.0)
+    assert i2[0].iterations == 1
+    for kw in (dict(sigma=-1.0, precondition=True), dict(sigma=float("nan"), precondition=True)):
+        with pytest.raises(wz.WZError) as e:
+            plan.cg_solve(d_phi, d_b, 1.0, 0.2, 1.0, 1e-10, 100, **kw)
+        assert e.value.status == wz.WZ_EINVAL
+    with pytest.raises(wz.WZError) as e:  # M0 must be invertible
+        plan.cg_solve(d_phi, d_b, 0.0, 0.2, 1.0, 1e-10, 100, precondition=True, sigma=1.0)
+    assert e.value.status == wz.WZ_EINVAL
+
+
+@pytest.mark.parametrize("dims,dtype,tol", [((8, 8, 8, 8), "c128", 1e-12), ((16, 8, 8, 8), "c64", 1e-6)])
+def test_rational_apply_vs_oracle(wz, orc, inp, dims, dtype, tol):
+    """Eq. 7.6 with d = 20 shifts at Table VII's parameters (m = 1, g = 0.1), preconditioned up to
+    beta = 100: the sum against the oracle's, per-shift iteration counts against the oracle's, and the
+    paper's caps (under 100 iterations per problem in single, under 200 in double precision)."""
+    m, g, rho = 1.0, 0.1, 1.0
+    phi = inp.make_phi(9, dims, 0.5, NPDT[dtype])
+    eta = inp.make_sources(9, 2, dims, NPDT[dtype])
+    a0, al, be = inp.rational_ladder(20, 1e-2, 1e3)
+    plan = wz.Plan(dims, dtype, 2)
+    out, infos = plan.rational_apply(torch.from_numpy(phi).cuda(), torch.from_numpy(eta).cuda(), m, g, a0, al, be,
+                                     rho, tol, 1000)
+    out = out.cpu().numpy()
+    phi128 = phi.astype(np.complex128)
+    cap = 200 if dtype == "c128" else 100
+    total = 0
+    for j in range(2):
+        ref, oinfos = orc.rational_apply(phi128, eta[j].astype(np.complex128), m, g, a0, al, be, rho, tol, 1000)
+        assert rel(out[j], ref) <= (1e-10 if dtype == "c128" else 2e-6)
+        for i in range(20):
+            gi, oi = infos[i][j], oinfos[i]
+            assert gi.converged and oi.converged and gi.iterations < cap
+            if dtype == "c128" or be[i] <= 100.0:  # plain complex64 solves follow G9's loop, not this oracle's
+                assert abs(gi.iterations - oi.iterations) <= max(2, oi.iterations // 20), (i, gi.iterations, oi.iterations)
+            total += gi.iterations
+    print("rational sum %s %s: %d iterations over 20 shifts x 2 sources" % (dims, dtype, total))
+    # the plain branch alone and the preconditioned branch alone give the same sum
+    out_np, _ = plan.rational_apply(torch.from_numpy(phi).cuda(), torch.from_numpy(eta).cuda(), m, g, a0, al, be,
+                                    rho, tol, 5000, pc_cutoff=-1.0)
+    assert rel(out_np.cpu().numpy(), out) <= (1e-9 if dtype == "c128" else 1e-5)
+
+
+def test_rational_apply_edge_cases(wz, inp):
+    dims = (4, 4, 4, 4)
+    phi = inp.make_phi(9, dims, 0.5)
+    eta = inp.make_sources(9, 1, dims)
+    plan = wz.Plan(dims, "c128", 1)
+    d_phi, d_eta = torch.from_numpy(phi).cuda(), torch.from_numpy(eta).cuda()
+    out, infos = plan.rational_apply(d_phi, d_eta, 1.0, 0.1, 0.75, [], [], 1.0, 1e-10, 100)  # no shifts: alpha0 eta
+    assert infos == [] and rel(out.cpu().numpy(), 0.75 * eta) <= 1e-15
+    with pytest.raises(wz.WZError) as e:
+        plan.rational_apply(d_phi, d_eta, 1.0, 0.1, 0.0, [1.0], [-2.0], 1.0, 1e-10, 100)
+    assert e.value.status == wz.WZ_EINVAL
