@@ -3,8 +3,10 @@
 // CPU path: every entry point either enqueues kernels or returns an error.
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
+#include <map>
 #include <vector>
 
 #include "../../include/wz.h"
@@ -347,10 +349,28 @@ wz_status launch(wz_plan* pl, int kind, void (*k)(const A), dim3 grid, int nt, s
   return WZ_OK;
 }
 
+// Prefetch distance = CTAs resident on the whole GPU at once (one wave), times WZ_PFA (environment,
+// tuning; 0 = off).  Occupancy is queried once per kernel.
+int pf_mult() {
+  static const int v = [] { const char* e = getenv("WZ_PFA"); return e ? atoi(e) : 1; }();
+  return v;
+}
+int wave_ctas(wz_plan* pl, const void* fn, int nt, size_t smem) {
+  static std::map<const void*, int> cache;
+  auto it = cache.find(fn);
+  if (it != cache.end()) return it->second;
+  int occ = 0;
+  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, nt, smem) != cudaSuccess || occ < 1) occ = 1;
+  return cache[fn] = occ * pl->num_sms;
+}
+
 // (x0,x1) pass over nf = 4*nbatch fields
 template <typename R>
-wz_status launch_p01(wz_plan* pl, int kind, const P01Kern<R>& k, const P01Args<R>& args, int nb) {
+wz_status launch_p01(wz_plan* pl, int kind, const P01Kern<R>& k, const P01Args<R>& args_in, int nb) {
   const int nseg_tiles = (int)(pl->I / k.nseg), nf = 4 * nb;
+  P01Args<R> args = args_in;
+  args.pf_dist = pf_mult() * wave_ctas(pl, (const void*)k.fn, k.nt, k.smem);
+  if ((long)nseg_tiles * nf <= args.pf_dist) args.pf_dist = 0;  // a single wave: nothing to run ahead of
   {
     ProfScope ps(pl, kind);
     k.fn<<<dim3((unsigned)nseg_tiles, (unsigned)nf), k.nt, k.smem, pl->stream>>>(args);
@@ -364,7 +384,11 @@ template <typename R>
 wz_status launch_p23(wz_plan* pl, int kind, const P23Entry<R>& e, void (*k)(const P23Args<R>),
                      const P23Args<R>& args, int nb) {
   const dim3 grid((unsigned)(pl->L[0] * pl->L[1]), (unsigned)nb, (unsigned)e.nhalf);
-  return launch<R>(pl, kind, k, grid, e.nt, args.pc ? e.smem_pc : e.smem, args);
+  P23Args<R> a2 = args;
+  const size_t smem = args.pc ? e.smem_pc : e.smem;
+  a2.pf_dist = pf_mult() * wave_ctas(pl, (const void*)k, e.nt, smem);
+  if ((long)grid.x * grid.y <= a2.pf_dist) a2.pf_dist = 0;
+  return launch<R>(pl, kind, k, grid, e.nt, smem, a2);
 }
 // Momentum-space multiply pass on the FFT temporary `cur`; in place, or into the other
 // temporary where the kernel works on half the spin components per CTA.  `cur` follows.

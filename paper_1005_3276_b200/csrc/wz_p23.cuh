@@ -48,6 +48,7 @@ struct P23Args {
   int pc;             // 0: Dslash;  1: M0^-1;  2: (M0^-1)^dag
   R m_re, m_im;       // m (pc only)
   const CGState* gate;  // [nbatch], indexed by blockIdx.y
+  int pf_dist;          // > 0: L2-prefetch the planes of the CTA pf_dist launches-in-order ahead (one wave)
 };
 
 // NC = spin components per CTA: 4 (whole plane quad, in place), or 2 when four planes
@@ -121,6 +122,18 @@ k_p23(const P23Args<R> a) {
       cpx<R> v = {R(0), R(0)};
       if (actA) v = gin[(long)F2::in_pos(k, jA) * L3 + x3A];
       x[k] = v;
+    }
+    // next wave's planes -> L2 while this CTA computes (one bulk prefetch per spin plane): the CTA that
+    // takes them later pays L2 latency instead of HBM latency (the pass is latency-bound, profiles/r01_*)
+    if constexpr (NC == 4) {
+      if (a.pf_dist > 0 && tid < 4) {
+        const long lin = (long)blockIdx.y * gridDim.x + blockIdx.x + a.pf_dist;
+        if (lin < (long)gridDim.y * gridDim.x) {
+          const long by = lin / gridDim.x, bx = lin % gridDim.x;
+          const cpx<R>* pf = a.in + ((by * 4 + tid) * a.nplanes + bx) * PL;
+          asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(pf), "r"((unsigned)(PL * sizeof(cpx<R>))));
+        }
+      }
     }
     F2::run(x, jA);
     if (actA) {
