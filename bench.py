@@ -322,6 +322,7 @@ def run_wz(args):
     if not args.no_extras:
         extras["preconditioned"] = time_preconditioned(plan, d_phi, d_b, d_x, cfg, secs / args.steps)
         extras["heatbath_rational_sum"] = time_rational(plan, d_phi, d_b, d_x, cfg)
+        extras["mixed_precision_to_1e-10"] = time_mixed(plan, d_phi, d_b, cfg, dev)
 
     cpu = None
     if not args.no_cpu_baseline and world == 1:
@@ -472,6 +473,38 @@ def time_rational(plan, d_phi, d_b, d_x, cfg):
             "all_converged": all(i.converged for row in infos for i in row),
             "worst_true_residual": max(i.rel_residual_true for row in infos for i in row),
             "paper": "Table VII, GTX 285, single: 360-540 iterations in total over 20 shifts, 0.93-220 s"}
+
+
+def time_mixed(plan, d_phi, d_b, cfg, dev, nsrc=2):
+    """NEXT-3 (mixed-precision CG): the first `nsrc` sources of the workload solved to the
+    double-precision tolerance 1e-10, once by the complex64 plan (complex128 reliable updates, reading G9)
+    and once by a complex128 plan on the same values."""
+    import torch
+
+    from paper_1005_3276_b200 import wz
+
+    def solve(pl, phi, b):
+        a, e = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        _, infos = pl.cg_solve(phi, b, cfg["m"], cfg["g"], cfg["rho"], 1e-10, 200000, raise_on_fail=False)
+        e.record()
+        e.synchronize()
+        return a.elapsed_time(e) * 1e-3, infos
+
+    b = d_b[:nsrc].contiguous()
+    t32, i32 = solve(plan, d_phi, b)
+    plan128 = wz.Plan(cfg["dims"], "c128", nsrc, dev)
+    t64, i64 = solve(plan128, d_phi.to(torch.complex128), b.to(torch.complex128))
+    plan128.close()
+    return {"sources": nsrc, "tol": 1e-10,
+            "c64_plan": {"secs": t32, "iterations": [i.iterations for i in i32],
+                         "reliable_updates": [i.reliable_updates for i in i32],
+                         "worst_true_residual": max(i.rel_residual_true for i in i32),
+                         "all_converged": all(i.converged for i in i32)},
+            "c128_plan": {"secs": t64, "iterations": [i.iterations for i in i64],
+                          "worst_true_residual": max(i.rel_residual_true for i in i64),
+                          "all_converged": all(i.converged for i in i64)},
+            "speedup": t64 / t32}
 
 
 def main():

@@ -349,10 +349,13 @@ wz_status launch(wz_plan* pl, int kind, void (*k)(const A), dim3 grid, int nt, s
   return WZ_OK;
 }
 
-// Prefetch distance = CTAs resident on the whole GPU at once (one wave), times WZ_PFA (environment,
-// tuning; 0 = off).  Occupancy is queried once per kernel.
-int pf_mult() {
-  static const int v = [] { const char* e = getenv("WZ_PFA"); return e ? atoi(e) : 1; }();
+// Wave-ahead L2 prefetch of the contiguous pass (wz_p23.cuh): distance = the CTAs resident on the whole
+// GPU at once (one wave) x WZ_PFA percent (environment, tuning sweeps; 0 = off; default 50).
+// Measured at 32^4 complex64, 12 sources (profiles/r01_notes.md): k_p23 207.7 -> 190 us per launch at a
+// quarter to a half wave, 193 at one, 200 at 1.5; per-line hints for the strided pass cost more than
+// they bring (dropped).
+int pf_percent() {
+  static const int v = [] { const char* e = getenv("WZ_PFA"); return e ? atoi(e) : 50; }();
   return v;
 }
 int wave_ctas(wz_plan* pl, const void* fn, int nt, size_t smem) {
@@ -366,11 +369,8 @@ int wave_ctas(wz_plan* pl, const void* fn, int nt, size_t smem) {
 
 // (x0,x1) pass over nf = 4*nbatch fields
 template <typename R>
-wz_status launch_p01(wz_plan* pl, int kind, const P01Kern<R>& k, const P01Args<R>& args_in, int nb) {
+wz_status launch_p01(wz_plan* pl, int kind, const P01Kern<R>& k, const P01Args<R>& args, int nb) {
   const int nseg_tiles = (int)(pl->I / k.nseg), nf = 4 * nb;
-  P01Args<R> args = args_in;
-  args.pf_dist = pf_mult() * wave_ctas(pl, (const void*)k.fn, k.nt, k.smem);
-  if ((long)nseg_tiles * nf <= args.pf_dist) args.pf_dist = 0;  // a single wave: nothing to run ahead of
   {
     ProfScope ps(pl, kind);
     k.fn<<<dim3((unsigned)nseg_tiles, (unsigned)nf), k.nt, k.smem, pl->stream>>>(args);
@@ -386,8 +386,8 @@ wz_status launch_p23(wz_plan* pl, int kind, const P23Entry<R>& e, void (*k)(cons
   const dim3 grid((unsigned)(pl->L[0] * pl->L[1]), (unsigned)nb, (unsigned)e.nhalf);
   P23Args<R> a2 = args;
   const size_t smem = args.pc ? e.smem_pc : e.smem;
-  a2.pf_dist = pf_mult() * wave_ctas(pl, (const void*)k, e.nt, smem);
-  if ((long)grid.x * grid.y <= a2.pf_dist) a2.pf_dist = 0;
+  a2.pf_dist = (int)((long)pf_percent() * wave_ctas(pl, (const void*)k, e.nt, smem) / 100);
+  if ((long)grid.x * grid.y <= a2.pf_dist) a2.pf_dist = 0;  // a single wave: nothing to run ahead of
   return launch<R>(pl, kind, k, grid, e.nt, smem, a2);
 }
 // Momentum-space multiply pass on the FFT temporary `cur`; in place, or into the other

@@ -54,20 +54,7 @@ struct P01Args {
   cpx<R>* cg_p;       // FWDCG (read+write), ENDCG (read)
   cpx<R>* cg_x;       // FWDCG (read+write)
   const CGState* gate;  // [nbatch]; if set and this source's solve is idle, the CTA returns at once
-  int pf_dist;          // > 0: L2-prefetch the input tile of the CTA pf_dist launches-in-order ahead (one wave)
 };
-
-// Input tile of a later CTA -> L2 (one hint per 128-byte line of each (x0,x1) row).
-template <typename R, int L0, int L1, int NSEG, int NT>
-__device__ __forceinline__ void prefetch_tile_ahead(const cpx<R>* in, long V, long I, int dist, int tid) {
-  if (dist <= 0) return;
-  const long lin = (long)blockIdx.y * gridDim.x + blockIdx.x + dist;
-  if (lin >= (long)gridDim.y * gridDim.x) return;
-  const cpx<R>* pb = in + (lin / gridDim.x) * V + (lin % gridDim.x) * NSEG;
-  constexpr int EPL = 128 / (int)sizeof(cpx<R>);           // elements per 128-byte line
-  constexpr int LINES = (NSEG + EPL - 1) / EPL;            // lines per row
-  for (int i = tid; i < L0 * L1 * LINES; i += NT) prefetch_l2(pb + (long)(i / LINES) * I + (i % LINES) * EPL);
-}
 
 template <typename R, int L0, int L1, int NSEG, int T0, int T1>
 struct P01Cfg {
@@ -152,7 +139,6 @@ k_p01(const P01Args<R> a) {
       }
       const R beta = (R)a.gate[src].beta, alpha = (R)a.gate[src].alpha;
       if (idle) return;
-      prefetch_tile_ahead<R, L0, L1, NSEG, Cfg::NT>(a.cg_p, V, I, a.pf_dist, tid);
       constexpr int CHF = (NR0 % 8 == 0) ? 8 : 4;
 #pragma unroll
       for (int k0 = 0; k0 < NR0; k0 += CHF) {
@@ -192,7 +178,6 @@ k_p01(const P01Args<R> a) {
         x[k] = v;
       }
       if (idle) return;
-      prefetch_tile_ahead<R, L0, L1, NSEG, Cfg::NT>(a.in, V, I, a.pf_dist, tid);
     }
     F0::run(x, jA);
     if (actA) {
@@ -233,7 +218,6 @@ k_p01(const P01Args<R> a) {
         if (actB) v = gin[((long)x0B * L1 + G1::in_pos(k, jB)) * I + sB];
         y[k] = v;
       }
-      prefetch_tile_ahead<R, L0, L1, NSEG, Cfg::NT>(a.in, V, I, a.pf_dist, tid);
       if constexpr (MODE != P01_INV) {
         // operands of the site-local step (this thread's axis-0 line), one hint per 32-byte sector
         if (actA && (sA * (int)sizeof(cpx<R>)) % 32 == 0) {

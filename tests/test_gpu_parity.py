@@ -548,3 +548,29 @@ def test_rational_apply_edge_cases(wz, inp):
     with pytest.raises(wz.WZError) as e:
         plan.rational_apply(d_phi, d_eta, 1.0, 0.1, 0.0, [1.0], [-2.0], 1.0, 1e-10, 100)
     assert e.value.status == wz.WZ_EINVAL
+
+
+# ---- NEXT-3: mixed precision to double-precision tolerances ----
+
+@pytest.mark.parametrize("dims", [(8, 8, 8, 8), (16, 16, 16, 16)])
+def test_mixed_precision_solve_to_double_tolerance(wz, orc, inp, dims):
+    """single precision 'could however be used for a mixed precision conjugate gradient'.
+    A WZ_C64 plan iterates in complex64 and corrects with complex128 reliable updates (reading G9), so it
+    reaches the double-precision tolerance 1e-10: true residual recomputed by the oracle, solution against
+    the complex128 oracle, iteration count against the oracle's complex64 + reliable-update loop (5 %)."""
+    m, g, rho, tol = 0.05, 1.0, 1.0, 1e-10
+    phi = inp.make_phi(2, dims, 0.3, np.complex64)
+    b = inp.make_sources(2, 1, dims, np.complex64)
+    plan = wz.Plan(dims, "c64", 1)
+    x, infos = plan.cg_solve(torch.from_numpy(phi).cuda(), torch.from_numpy(b).cuda(), m, g, rho, tol, 50000)
+    x = x.cpu().numpy()[0]
+    phi128, b128 = phi.astype(np.complex128), b[0].astype(np.complex128)
+    Xo, io = orc.cg_c64ru(phi128, b128, m, g, rho, tol, 50000)
+    xd, idb = orc.cg(phi128, b128, m, g, rho, tol, 50000)
+    true_res = rel(orc.apply_MdagM(phi128, x, m, g, rho), b128)
+    print("mixed precision %s: iterations gpu=%d (reliable updates %d) oracle c64ru=%d (%d) oracle c128=%d true residual %.2e"
+          % (dims, infos[0].iterations, infos[0].reliable_updates, io.iterations, io.reliable_updates, idb.iterations, true_res))
+    assert infos[0].converged and io.converged
+    assert true_res <= tol * (1.0 + 1e-3)
+    assert abs(infos[0].iterations - io.iterations) <= max(2, io.iterations // 20)
+    assert rel(x, xd) <= 1e-8 and rel(x, Xo) <= 1e-8
