@@ -81,8 +81,11 @@ struct P23Entry {
 #ifndef WZ_TPL32F_MID
 #define WZ_TPL32F_MID 1
 #endif
+#ifndef WZ_TPL32F_END
+#define WZ_TPL32F_END WZ_TPL32F
+#endif
 template <typename R, int L, int MODE> struct tune_tpl {   // axes 0,1; pass C does best with whole lines per thread
-  static constexpr int v = (sizeof(R) == 4) ? (L == 64 ? WZ_TPL64F : (L >= 48 ? 2 : (L == 32 ? (MODE == P01_MID ? WZ_TPL32F_MID : WZ_TPL32F) : 1)))
+  static constexpr int v = (sizeof(R) == 4) ? (L == 64 ? WZ_TPL64F : (L >= 48 ? 2 : (L == 32 ? (MODE == P01_MID ? WZ_TPL32F_MID : ((MODE == P01_ENDCG || MODE == P01_END) ? WZ_TPL32F_END : WZ_TPL32F)) : 1)))
                                             : (L >= 48 ? 4 : (L >= 24 ? 2 : 1));
 };
 template <typename R, int L> struct tune_tpl23 {  // axes 2,3
@@ -101,9 +104,12 @@ template <typename R, int L> struct tune_tpl23 {  // axes 2,3
 #ifndef WZ_NSEG32F_INV
 #define WZ_NSEG32F_INV 16
 #endif
+#ifndef WZ_NSEG32F_MID
+#define WZ_NSEG32F_MID WZ_NSEG32F_INV
+#endif
 template <typename R, int L0, int L1, int MODE> struct tune_nseg {
   static constexpr bool fwd = (MODE == P01_FWD || MODE == P01_FWDCG);
-  static constexpr int v = (sizeof(R) == 4) ? (L0 * L1 > 2048 ? 4 : (L0 * L1 == 1024 ? (fwd ? WZ_NSEG32F_FWD : WZ_NSEG32F_INV) : 8))
+  static constexpr int v = (sizeof(R) == 4) ? (L0 * L1 > 2048 ? 4 : (L0 * L1 == 1024 ? (fwd ? WZ_NSEG32F_FWD : (MODE == P01_MID ? WZ_NSEG32F_MID : WZ_NSEG32F_INV)) : 8))
                                             : (L0 * L1 > 2048 ? 2 : 4);
 };
 
