@@ -70,7 +70,7 @@ struct P23Entry {
 // passes are latency-bound otherwise: profiles/r01_*); one radix-2 shuffle step per
 // doubling.  Compile-time overrides for sweeps: -DWZ_TPL32F=.. -DWZ_NSEG32F_FWD=.. -DWZ_NSEG32F_INV=..
 #ifndef WZ_TPL32F
-#define WZ_TPL32F 2
+#define WZ_TPL32F 1  // whole lines per thread in every (x0,x1) mode at 32^4 complex64 (pass A': 441 -> 427 us per launch)
 #endif
 #ifndef WZ_TPL32F_P23
 #define WZ_TPL32F_P23 1
@@ -82,7 +82,7 @@ struct P23Entry {
 #define WZ_TPL32F_MID 1
 #endif
 #ifndef WZ_TPL32F_END
-#define WZ_TPL32F_END WZ_TPL32F
+#define WZ_TPL32F_END 1  // pass E', E: whole lines per thread (measured 330 -> 317 us per launch at 12 sources)
 #endif
 template <typename R, int L, int MODE> struct tune_tpl {   // axes 0,1; pass C does best with whole lines per thread
   static constexpr int v = (sizeof(R) == 4) ? (L == 64 ? WZ_TPL64F : (L >= 48 ? 2 : (L == 32 ? (MODE == P01_MID ? WZ_TPL32F_MID : ((MODE == P01_ENDCG || MODE == P01_END) ? WZ_TPL32F_END : WZ_TPL32F)) : 1)))
@@ -237,6 +237,7 @@ struct wz_plan {
   cudaEvent_t ev[2] = {nullptr, nullptr};
   int npartials = 0;
   int num_sms = 148;
+  int sweep = 0;  // direction of the last pass launched (next_sweep)
   std::vector<void*> allocs;
   // optional per-kernel timing (wz_plan_profile): event pairs around sampled launches
   int profile = 0;
@@ -373,10 +374,23 @@ int wave_ctas(wz_plan* pl, const void* fn, int nt, size_t smem) {
   return cache[fn] = occ * pl->num_sms;
 }
 
+// Alternating sweep direction: consecutive passes run over the tiles in opposite orders, so the first CTAs
+// of a launch read what the previous launch wrote (or read) last and the 126 MB L2 still holds.  Every CTA's
+// work and every reduction slot is indexed by the tile, not by blockIdx, so results do not depend on it.
+// WZ_SWEEP=0 (environment) turns it off for A/B measurements.
+int next_sweep(wz_plan* pl) {
+  static const int on = [] { const char* e = getenv("WZ_SWEEP"); return e ? atoi(e) : 1; }();
+  if (!on) return 0;
+  pl->sweep ^= 1;
+  return pl->sweep;
+}
+
 // (x0,x1) pass over nf = 4*nbatch fields
 template <typename R>
-wz_status launch_p01(wz_plan* pl, int kind, const P01Kern<R>& k, const P01Args<R>& args, int nb) {
+wz_status launch_p01(wz_plan* pl, int kind, const P01Kern<R>& k, const P01Args<R>& args_in, int nb) {
   const int nseg_tiles = (int)(pl->I / k.nseg), nf = 4 * nb;
+  P01Args<R> args = args_in;
+  args.rev = next_sweep(pl);
   {
     ProfScope ps(pl, kind);
     k.fn<<<dim3((unsigned)nseg_tiles, (unsigned)nf), k.nt, k.smem, pl->stream>>>(args);
@@ -391,6 +405,7 @@ wz_status launch_p23(wz_plan* pl, int kind, const P23Entry<R>& e, void (*k)(cons
                      const P23Args<R>& args, int nb) {
   const dim3 grid((unsigned)(pl->L[0] * pl->L[1]), (unsigned)nb, (unsigned)e.nhalf);
   P23Args<R> a2 = args;
+  a2.rev = next_sweep(pl);
   const size_t smem = args.pc ? e.smem_pc : e.smem;
   a2.pf_dist = (int)((long)pf_percent() * wave_ctas(pl, (const void*)k, e.nt, smem) / 100);
   if ((long)grid.x * grid.y <= a2.pf_dist) a2.pf_dist = 0;  // a single wave: nothing to run ahead of

@@ -31,6 +31,74 @@ __device__ __forceinline__ cpx<double> ldg_c(const cpx<double>* p) {
   return {t.x, t.y};
 }
 
+// Streaming loads: chi in passes E / E' is read once and by no launch soon after; marking it evict-first
+// in L2 (createpolicy + .L2::cache_hint) leaves more of the 126 MB L2 to what the NEXT launch reads first
+// (the tail of r written here; see next_sweep() in wz_lib.cu).  Measured at 32^4 complex64, 12 sources:
+// pass E' 307.6 -> 291 us per launch.  The same hint on x / r in pass A' and on the chi store of pass C
+// made those passes slower (420 -> 599 us, 380 -> 406 us) and is not used (profiles/r01_notes.md).
+#ifndef WZ_EVICT
+#define WZ_EVICT 1
+#endif
+#ifndef WZ_EVICT_MID
+#define WZ_EVICT_MID 0
+#endif
+__device__ __forceinline__ unsigned long long l2_evict_first_policy() {
+  unsigned long long pol;
+  asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+  return pol;
+}
+__device__ __forceinline__ cpx<float> ld_stream(const cpx<float>* p, unsigned long long pol) {
+#if WZ_EVICT
+  cpx<float> v;
+  asm volatile("ld.global.L2::cache_hint.v2.f32 {%0, %1}, [%2], %3;" : "=f"(v.re), "=f"(v.im) : "l"(p), "l"(pol));
+  return v;
+#else
+  return *p;
+#endif
+}
+__device__ __forceinline__ cpx<double> ld_stream(const cpx<double>* p, unsigned long long pol) {
+#if WZ_EVICT
+  cpx<double> v;
+  asm volatile("ld.global.L2::cache_hint.v2.f64 {%0, %1}, [%2], %3;" : "=d"(v.re), "=d"(v.im) : "l"(p), "l"(pol));
+  return v;
+#else
+  return *p;
+#endif
+}
+// read-only data (non-coherent path, as ldg_c)
+__device__ __forceinline__ cpx<float> ld_stream_nc(const cpx<float>* p, unsigned long long pol) {
+#if WZ_EVICT
+  cpx<float> v;
+  asm volatile("ld.global.nc.L2::cache_hint.v2.f32 {%0, %1}, [%2], %3;" : "=f"(v.re), "=f"(v.im) : "l"(p), "l"(pol));
+  return v;
+#else
+  return ldg_c(p);
+#endif
+}
+__device__ __forceinline__ cpx<double> ld_stream_nc(const cpx<double>* p, unsigned long long pol) {
+#if WZ_EVICT
+  cpx<double> v;
+  asm volatile("ld.global.nc.L2::cache_hint.v2.f64 {%0, %1}, [%2], %3;" : "=d"(v.re), "=d"(v.im) : "l"(p), "l"(pol));
+  return v;
+#else
+  return ldg_c(p);
+#endif
+}
+__device__ __forceinline__ void st_stream(cpx<float>* p, cpx<float> v, unsigned long long pol) {
+#if WZ_EVICT
+  asm volatile("st.global.L2::cache_hint.v2.f32 [%0], {%1, %2}, %3;" ::"l"(p), "f"(v.re), "f"(v.im), "l"(pol));
+#else
+  *p = v;
+#endif
+}
+__device__ __forceinline__ void st_stream(cpx<double>* p, cpx<double> v, unsigned long long pol) {
+#if WZ_EVICT
+  asm volatile("st.global.L2::cache_hint.v2.f64 [%0], {%1, %2}, %3;" ::"l"(p), "d"(v.re), "d"(v.im), "l"(pol));
+#else
+  *p = v;
+#endif
+}
+
 // L2 prefetch hint: no register, no scoreboard; the later load then pays L2 latency
 // instead of HBM latency (the passes are latency-bound on their operand streams).
 __device__ __forceinline__ void prefetch_l2(const void* p) {
@@ -54,6 +122,7 @@ struct P01Args {
   cpx<R>* cg_p;       // FWDCG (read+write), ENDCG (read)
   cpx<R>* cg_x;       // FWDCG (read+write)
   const CGState* gate;  // [nbatch]; if set and this source's solve is idle, the CTA returns at once
+  int rev;              // 1: CTAs take the tiles in reverse order (see launch_p01: L2 reuse across launches)
 };
 
 template <typename R, int L0, int L1, int NSEG, int T0, int T1>
@@ -88,7 +157,10 @@ k_p01(const P01Args<R> a) {
   __shared__ double red_sh[33];
 
   const int tid = threadIdx.x;
-  const int f = blockIdx.y;            // field = source*4 + spin
+  [[maybe_unused]] const unsigned long long pol = l2_evict_first_policy();
+  // sweep direction: with rev the first CTAs of this launch take what the previous launch wrote last
+  const int bx = a.rev ? (int)(gridDim.x - 1 - blockIdx.x) : (int)blockIdx.x;
+  const int f = a.rev ? (int)(gridDim.y - 1 - blockIdx.y) : (int)blockIdx.y;  // field = source*4 + spin
   const int comp = f & 3, src = f >> 2;
   // forward modes: the idle test of this source is issued now but consumed only after the
   // first loads are in flight (measured: pays there, not in the inverse modes)
@@ -97,7 +169,7 @@ k_p01(const P01Args<R> a) {
   if constexpr (MODE != P01_FWD && MODE != P01_FWDCG) {
     if (idle) return;
   }
-  const long i0 = (long)blockIdx.x * NSEG;
+  const long i0 = (long)bx * NSEG;
   // IC > 0: the (x2,x3) volume is a compile-time constant, so every tile offset below folds
   // into an immediate of the load/store instead of 64-bit integer arithmetic per access
   const long I = IC ? (long)IC : a.I;
@@ -203,7 +275,7 @@ k_p01(const P01Args<R> a) {
     }
     if constexpr (MODE == P01_FWDCG && FIN == FIN_PP) {
       // shifted solves: <p,p> of this source for alpha = rho / (||M p||^2 + sigma <p,p>)
-      const int blk = comp * gridDim.x + blockIdx.x;
+      const int blk = comp * gridDim.x + bx;
       grid_reduce<FIN_PP>(accp, a.red.for_source(src), blk, 4 * gridDim.x, red_sh);
     }
   } else {
@@ -288,7 +360,8 @@ k_p01(const P01Args<R> a) {
           for (int c = 0; c < CH; ++c) {
             off[c] = ((long)G0::out_pos(k0 + c, jA) * L1 + x1A) * I + sA;
             ph[c] = ldg_c(gphi + off[c]);
-            ps[c] = ldg_c(gpsi + off[c]);
+            if constexpr (MODE == P01_MID && !WZ_EVICT_MID) ps[c] = ldg_c(gpsi + off[c]);
+            else ps[c] = ld_stream_nc(gpsi + off[c], pol);  // chi in pass E/E': read once, evict first
           }
           if constexpr (MODE == P01_ENDCG) {
             cpx<R> vr[CH];
@@ -375,7 +448,7 @@ k_p01(const P01Args<R> a) {
         }
       }
       if (a.red.partials) {  // one reduction per source: its 4 spin components x all segments
-        const int blk = comp * gridDim.x + blockIdx.x;
+        const int blk = comp * gridDim.x + bx;
         grid_reduce<FIN>(acc, a.red.for_source(src), blk, 4 * gridDim.x, red_sh);
       }
     }

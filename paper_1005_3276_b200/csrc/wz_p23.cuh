@@ -48,6 +48,7 @@ struct P23Args {
   int pc;             // 0: Dslash;  1: M0^-1;  2: (M0^-1)^dag
   R m_re, m_im;       // m (pc only)
   const CGState* gate;  // [nbatch], indexed by blockIdx.y
+  int rev;              // 1: CTAs take (plane, source) in reverse order (L2 reuse across launches)
   int pf_dist;          // > 0: L2-prefetch the planes of the CTA pf_dist launches-in-order ahead (one wave)
 };
 
@@ -86,12 +87,14 @@ k_p23(const P23Args<R> a) {
   R* dgs = cfs + Cfg::CF_ELEMS;                     // diagonal factor (pc launches only)
   __shared__ R tb[2 * 4 * 64];
 
-  if (a.gate && !cg_active(a.gate + blockIdx.y)) return;
+  const int bxr = a.rev ? (int)(gridDim.x - 1 - blockIdx.x) : (int)blockIdx.x;
+  const int byr = a.rev ? (int)(gridDim.y - 1 - blockIdx.y) : (int)blockIdx.y;
+  if (a.gate && !cg_active(a.gate + byr)) return;
 
   const int tid = threadIdx.x;
-  const int plane = blockIdx.x;
+  const int plane = bxr;
   const long PL = (long)L2 * L3;
-  const long fbase = (long)blockIdx.y * 4 * a.nplanes;  // first field of this batch entry
+  const long fbase = (long)byr * 4 * a.nplanes;  // first field of this batch entry
 
   if constexpr (kMult) {
     for (int i = tid; i < 2 * 4 * 64; i += blockDim.x) tb[i] = a.tab[i];
@@ -129,7 +132,8 @@ k_p23(const P23Args<R> a) {
       if (a.pf_dist > 0 && tid < 4) {
         const long lin = (long)blockIdx.y * gridDim.x + blockIdx.x + a.pf_dist;
         if (lin < (long)gridDim.y * gridDim.x) {
-          const long by = lin / gridDim.x, bx = lin % gridDim.x;
+          long by = lin / gridDim.x, bx = lin % gridDim.x;  // launch order -> data order
+          if (a.rev) { by = gridDim.y - 1 - by; bx = gridDim.x - 1 - bx; }
           const cpx<R>* pf = a.in + ((by * 4 + tid) * a.nplanes + bx) * PL;
           asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(pf), "r"((unsigned)(PL * sizeof(cpx<R>))));
         }
