@@ -421,8 +421,15 @@ def test_cg_shift_vs_oracle(wz, orc, inp, dims, dtype, tol):
             print("shift %g %s %s: iterations gpu=%d oracle=%d true residual %.2e"
                   % (sigma, dims, dtype, infos[j].iterations, io.iterations, true_res))
             assert infos[j].converged and io.converged
-            bound = max(2, io.iterations // 100) if dtype == "c128" else max(2, io.iterations // 20)  # G10
+            # G10: near the stop the oracle's residual hovers within +-30 % of tol for several iterations
+            # (measured here at sigma = 1: 1.31, 1.41, 1.28, 1.44, 0.93 x tol), and its own count moves with
+            # the OpenMP thread count (492 on one box, 491 on the next; GPU 496 on both): bind complex128 at
+            # max(2, 2 %) AND require the oracle to be at the threshold where the GPU stopped
+            bound = max(2, io.iterations // 50) if dtype == "c128" else max(2, io.iterations // 20)
             assert abs(infos[j].iterations - io.iterations) <= bound
+            if dtype == "c128":
+                k = min(infos[j].iterations, len(io.history) - 1)
+                assert min(io.history[max(0, k - 2):k + 3]) <= 2.0 * tol
             assert true_res <= tol * (1.0 + 1e-3)
             assert abs(true_res - infos[j].rel_residual_true) <= 0.05 * tol
             assert rel(x[j], xo) <= (1e-7 if dtype == "c128" else 5e-4)
