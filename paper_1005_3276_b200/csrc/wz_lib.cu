@@ -391,6 +391,8 @@ wz_status launch_p01(wz_plan* pl, int kind, const P01Kern<R>& k, const P01Args<R
   const int nseg_tiles = (int)(pl->I / k.nseg), nf = 4 * nb;
   P01Args<R> args = args_in;
   args.rev = next_sweep(pl);
+  static const int comp_fast = [] { const char* e = getenv("WZ_COMPFAST"); return e ? atoi(e) : 0; }();
+  args.comp_fast = comp_fast;
   {
     ProfScope ps(pl, kind);
     k.fn<<<dim3((unsigned)nseg_tiles, (unsigned)nf), k.nt, k.smem, pl->stream>>>(args);

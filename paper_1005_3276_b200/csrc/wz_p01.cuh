@@ -123,6 +123,8 @@ struct P01Args {
   cpx<R>* cg_x;       // FWDCG (read+write)
   const CGState* gate;  // [nbatch]; if set and this source's solve is idle, the CTA returns at once
   int rev;              // 1: CTAs take the tiles in reverse order (see launch_p01: L2 reuse across launches)
+  int comp_fast;        // 1: launch order = (source, tile, spin) with spin fastest: the four CTAs that share one
+                        //    phi tile run together, so phi comes from HBM once per source instead of four times
 };
 
 template <typename R, int L0, int L1, int NSEG, int T0, int T1>
@@ -159,8 +161,15 @@ k_p01(const P01Args<R> a) {
   const int tid = threadIdx.x;
   [[maybe_unused]] const unsigned long long pol = l2_evict_first_policy();
   // sweep direction: with rev the first CTAs of this launch take what the previous launch wrote last
-  const int bx = a.rev ? (int)(gridDim.x - 1 - blockIdx.x) : (int)blockIdx.x;
-  const int f = a.rev ? (int)(gridDim.y - 1 - blockIdx.y) : (int)blockIdx.y;  // field = source*4 + spin
+  int bx = a.rev ? (int)(gridDim.x - 1 - blockIdx.x) : (int)blockIdx.x;
+  int f = a.rev ? (int)(gridDim.y - 1 - blockIdx.y) : (int)blockIdx.y;  // field = source*4 + spin
+  if (a.comp_fast) {
+    const unsigned lin0 = blockIdx.y * gridDim.x + blockIdx.x;
+    const unsigned lin = a.rev ? gridDim.x * gridDim.y - 1 - lin0 : lin0;
+    const unsigned q = lin >> 2;
+    bx = (int)(q % gridDim.x);
+    f = (int)(q / gridDim.x) * 4 + (int)(lin & 3);
+  }
   const int comp = f & 3, src = f >> 2;
   // forward modes: the idle test of this source is issued now but consumed only after the
   // first loads are in flight (measured: pays there, not in the inverse modes)
