@@ -391,8 +391,10 @@ wz_status launch_p01(wz_plan* pl, int kind, const P01Kern<R>& k, const P01Args<R
   const int nseg_tiles = (int)(pl->I / k.nseg), nf = 4 * nb;
   P01Args<R> args = args_in;
   args.rev = next_sweep(pl);
-  static const int comp_fast = [] { const char* e = getenv("WZ_COMPFAST"); return e ? atoi(e) : 0; }();
-  args.comp_fast = comp_fast;
+  // spin-fastest launch order (bit 0: pass C, bit 1: passes E/E', bit 2: forward modes; WZ_COMPFAST, tuning)
+  static const int comp_fast = [] { const char* e = getenv("WZ_COMPFAST"); return e ? atoi(e) : 1; }();
+  const int cf_bit = (kind == WZ_K_P01_MID) ? 1 : ((kind == WZ_K_P01_END || kind == WZ_K_P01_ENDCG) ? 2 : 4);
+  args.comp_fast = (comp_fast & cf_bit) ? 1 : 0;
   {
     ProfScope ps(pl, kind);
     k.fn<<<dim3((unsigned)nseg_tiles, (unsigned)nf), k.nt, k.smem, pl->stream>>>(args);
