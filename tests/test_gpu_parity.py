@@ -581,3 +581,38 @@ def test_mixed_precision_solve_to_double_tolerance(wz, orc, inp, dims):
     assert true_res <= tol * (1.0 + 1e-3)
     assert abs(infos[0].iterations - io.iterations) <= max(2, io.iterations // 20)
     assert rel(x, xd) <= 1e-8 and rel(x, Xo) <= 1e-8
+
+
+def test_launch_order_knobs_do_not_change_results(wz):
+    """Prefetch distance, sweep direction and CTA order only permute or hint:
+    CTA work and reduction slots are indexed by tile, so a solve is bit-identical with all of them off."""
+    import hashlib
+    import os
+    import subprocess
+    import sys
+
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    code = (
+        "import hashlib, torch\n"
+        "from paper_1005_3276_b200 import inputs, wz\n"
+        "dims = (32, 32, 32, 32)\n"
+        "phi = torch.from_numpy(inputs.make_phi(11, dims, 0.5, 'complex64')).cuda()\n"
+        "b = torch.from_numpy(inputs.make_sources(11, 2, dims, 'complex64')).cuda()\n"
+        "plan = wz.Plan(dims, 'c64', 2)\n"
+        "x, info = plan.cg_solve(phi, b, 0.01, 1.5, 1.0, 1e-6, 60, raise_on_fail=False)\n"
+        "q = plan.apply_MdagM(phi, b, 0.01, 1.5, 1.0)\n"
+        "h = hashlib.sha256(x.cpu().numpy().tobytes() + q.cpu().numpy().tobytes()).hexdigest()\n"
+        "print('DIGEST', h, info[0].iterations, info[0].rel_residual_true)\n"
+    )
+
+    def run(env_extra):
+        env = dict(os.environ)
+        env.update(env_extra)
+        out = subprocess.run([sys.executable, "-c", code], cwd=root, env=env, capture_output=True, text=True, timeout=600)
+        assert out.returncode == 0, out.stderr[-2000:]
+        return [l for l in out.stdout.splitlines() if l.startswith("DIGEST")][0]
+
+    on = run({})
+    off = run({"WZ_PFA": "0", "WZ_SWEEP": "0", "WZ_COMPFAST": "0"})
+    alt = run({"WZ_PFA": "150", "WZ_SWEEP": "1", "WZ_COMPFAST": "7"})
+    assert on == off == alt, (on, off, alt)
