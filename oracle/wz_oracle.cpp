@@ -447,11 +447,24 @@ struct orc_cg_info {
   double rel_residual_true;
 };
 
+// Re <a, b>.  Fixed summation order, independent of the OpenMP thread count: blocks of
+// DOT_BLOCK consecutive elements are each summed left to right, then the block sums are
+// added left to right.  (An OpenMP reduction(+) would make the CG iteration count of
+// the oracle itself move with the number of threads: DESIGN.md reading G10.)
+static const long DOT_BLOCK = 4096;
 static double dot_re(const cd* a, const cd* b, long n) {
-  double acc = 0.0;
-#pragma omp parallel for reduction(+ : acc) schedule(static)
-  for (long i = 0; i < n; ++i) acc += a[i].real() * b[i].real() + a[i].imag() * b[i].imag();
-  return acc;
+  const long nblk = (n + DOT_BLOCK - 1) / DOT_BLOCK;
+  std::vector<double> part(nblk > 0 ? nblk : 1, 0.0);
+#pragma omp parallel for schedule(static)
+  for (long k = 0; k < nblk; ++k) {
+    const long i1 = (k + 1) * DOT_BLOCK < n ? (k + 1) * DOT_BLOCK : n;
+    double acc = 0.0;
+    for (long i = k * DOT_BLOCK; i < i1; ++i) acc += a[i].real() * b[i].real() + a[i].imag() * b[i].imag();
+    part[k] = acc;
+  }
+  double tot = 0.0;
+  for (long k = 0; k < nblk; ++k) tot += part[k];
+  return tot;
 }
 
 int orc_cg(int method, const int* L, const double* phi, const double* b_, double* x_,

@@ -32,7 +32,9 @@ def test_cg_residuals_and_energy_norm_config1(orc):
     assert info.rel_residual_recursive <= cfg["tol"]
     assert abs(info.rel_residual_true - info.rel_residual_recursive) <= 1e-3 * info.rel_residual_recursive
     res = np.linalg.norm(b.reshape(-1) - A @ x.reshape(-1)) / np.linalg.norm(b)
-    assert abs(res - info.rel_residual_true) <= 1e-3 * res
+    # the dense matrix A carries rounding of order eps * cond(A) (entries pinned to 1e-11 in test_oracle_operator):
+    # its residual of the same x agrees with the oracle's to that absolute floor (measured: 1.2e-13 on 7.2e-11)
+    assert abs(res - info.rel_residual_true) <= 1e-3 * res + 5e-13
     assert 100 <= info.iterations <= 300                     # survey estimate with numpy's RNG: 163
     errs = []
     for k in (10, 40, 80, 120):
