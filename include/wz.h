@@ -50,7 +50,8 @@ const char *wz_version(void);
 
 /* Create a plan for a T x L1 x L2 x L3 lattice (T = extent of x0, the antiperiodic
  * time direction; PAPER.md:234 requires T even).  `stream` is a cudaStream_t
- * (0 = legacy default stream).  The plan owns: twiddle/momentum tables, the
+ * (0 = legacy default stream) of the CURRENT device: the plan lives on that device, and every call on
+ * the plan switches to it for its duration (and back).  The plan owns: twiddle/momentum tables, the
  * matvec temporaries (2 spinors per batch entry) and the CG vectors.  max_batch >= 1.
  * Supported extents: (T,L1) and (L2,L3) pairs listed by wz_supported(). */
 wz_status wz_plan_create(wz_plan **plan, int T, int L1, int L2, int L3,
@@ -99,6 +100,7 @@ typedef struct {
  *    by reliable updates (reading G9); rounding that solution to
  *    complex64 would by itself lift the true residual above tol.
  *  - info: HOST array of nbatch entries.
+ * x must not alias b (WZ_EINVAL).
  * Synchronises the plan's stream before returning.  Returns WZ_ENOTCONVERGED if
  * any source hit max_iter; x then holds the last iterate. */
 wz_status wz_cg_solve(wz_plan *plan, const void *phi, const void *b, void *x,
@@ -165,6 +167,20 @@ wz_status wz_rational_apply(wz_plan *plan, const void *phi, const void *eta, voi
  *   Uses plan temporaries; synchronises the stream. */
 wz_status wz_apply_Dslash(wz_plan *plan, double rho, const void *in, void *out, int nbatch);
 wz_status wz_locality_profile(wz_plan *plan, double rho, int spin, double *f_host, int nf);
+
+/* The kCheck = 8 CG iterations between two looks of the host at the device-resident solver state are 40
+ * launches with fixed arguments: by default they are captured once as a CUDA graph (per distinct set of
+ * solve arguments) and replayed, so a solve makes no host round trip except that lagged convergence check
+ * (BASELINE.json north star (iii)).  wz_plan_set_graph(plan, 0) enqueues the same kernels
+ * one by one instead (results are bit-identical; for measurements).  Default: 1. */
+wz_status wz_plan_set_graph(wz_plan *plan, int enable);
+
+/* Residual history of the LAST solve on this plan, as the host saw it at its convergence checks (every 8
+ * iterations, one chunk behind the GPU): for `source`, pairs (iteration k, ||r_k|| / ||b||) with the
+ * recursive residual (PAPER.md:944 stop rule), the recomputed one right after a reliable update.
+ * Copies at most cap pairs into the HOST arrays (either may be NULL to only count); returns the number
+ * of pairs recorded, or -1 on a bad argument. */
+int wz_plan_cg_history(const wz_plan *plan, int source, int *iterations, double *rel_residual, int cap);
 
 /* Number of kernel launches this plan has enqueued so far (for bench.py's
  * gpu_launches), and a reset. */

@@ -1,20 +1,36 @@
 // wz_lib.cu -- host side of the C-ABI in include/wz.h: plans, tables, kernel
 // dispatch, the matvec pass schedule and the CG driver.  sm_100a only; there is no
 // CPU path: every entry point either enqueues kernels or returns an error.
+#include <algorithm>
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
 #include <new>
 #include <map>
+#include <mutex>
+#include <set>
 #include <vector>
 
 #include "../../include/wz.h"
 #include "wz_cgk.cuh"
-#include "wz_p01.cuh"
-#include "wz_p23.cuh"
+#include "wz_tables.cuh"
 
 using namespace wz;
+
+namespace wz {
+const KernelModule* kernel_module(int i) {
+  switch (i) {
+    case 0: return wz_kernel_module_0();
+    case 1: return wz_kernel_module_1();
+    case 2: return wz_kernel_module_2();
+    case 3: return wz_kernel_module_3();
+    case 4: return wz_kernel_module_4();
+    case 5: return wz_kernel_module_5();
+    default: return wz_kernel_module_6();
+  }
+}
+}  // namespace wz
 
 namespace {
 
@@ -30,148 +46,35 @@ bool cuda_ok(cudaError_t e, const char* what) {
     if (!cuda_ok((call), #call)) return WZ_ECUDA;       \
   } while (0)
 
-// ---- kernel dispatch tables ---------------------------------------------------
-// One (x0,x1)-pass kernel with its launch shape.
-template <typename R>
-struct P01Kern {
-  void (*fn)(const P01Args<R>) = nullptr;
-  int nt = 0, nseg = 0;
-  size_t smem = 0;
-};
-template <typename R>
-struct P01Entry {
-  int L0, L1;
-  long I;  // (x2,x3) volume the kernels were specialised for; 0 = any (run-time)
-  P01Kern<R> fwd, inv, mid, mid_pq, end, fwdcg, endcg;
-  P01Kern<R> fwdcg_s, endcg_s;  // shifted system (M^dag M + sigma): A' also reduces <p,p>, E' adds sigma p to q
-  int nseg() const {  // largest tile width of the entry: the (x2,x3) volume must be a multiple
-    int m = 1;
-    for (const P01Kern<R>* k : {&fwd, &inv, &mid, &mid_pq, &end, &fwdcg, &endcg, &fwdcg_s, &endcg_s}) m = k->nseg > m ? k->nseg : m;
-    return m;
-  }
-  int min_nseg() const {
-    int m = 1 << 30;
-    for (const P01Kern<R>* k : {&fwd, &inv, &mid, &mid_pq, &end, &fwdcg, &endcg, &fwdcg_s, &endcg_s}) m = k->nseg < m ? k->nseg : m;
-    return m;
+// ---- kernel dispatch tables: gathered from the kernel modules (wz_kmod.cu) ----------
+template <typename R> struct tables;
+template <> struct tables<float> {
+  static void gather(std::vector<P01Entry<float>>& a, std::vector<P23Entry<float>>& b) {
+    for (int i = 0; i < kNumKernelModules; ++i) { kernel_module(i)->p01f(a); kernel_module(i)->p23f(b); }
   }
 };
-template <typename R>
-struct P23Entry {
-  int L2, L3, nt, nhalf;  // nhalf = 2: two components per CTA, grid.z = 2, multiply needs in != out
-  size_t smem, smem_pc;
-  void (*fwd)(const P23Args<R>);
-  void (*inv)(const P23Args<R>);
-  void (*mult)(const P23Args<R>);
-  void (*multpc)(const P23Args<R>);  // multiply with the free inverse (preconditioner)
+template <> struct tables<double> {
+  static void gather(std::vector<P01Entry<double>>& a, std::vector<P23Entry<double>>& b) {
+    for (int i = 0; i < kNumKernelModules; ++i) { kernel_module(i)->p01d(a); kernel_module(i)->p23d(b); }
+  }
 };
-
-// ---- tuning: lanes per lattice line (TPL) and tile width (NSEG) -------------------
-// More lanes per line = fewer registers per thread and more resident warps (the
-// passes are latency-bound otherwise: profiles/r01_*); one radix-2 shuffle step per
-// doubling.  Compile-time overrides for sweeps: -DWZ_TPL32F=.. -DWZ_NSEG32F_FWD=.. -DWZ_NSEG32F_INV=..
-#ifndef WZ_TPL32F
-#define WZ_TPL32F 1  // whole lines per thread in every (x0,x1) mode at 32^4 complex64 (pass A': 441 -> 427 us per launch)
-#endif
-#ifndef WZ_TPL32F_P23
-#define WZ_TPL32F_P23 1
-#endif
-#ifndef WZ_TPL64F
-#define WZ_TPL64F 2
-#endif
-#ifndef WZ_TPL32F_MID
-#define WZ_TPL32F_MID 1
-#endif
-#ifndef WZ_TPL32F_END
-#define WZ_TPL32F_END 1  // pass E', E: whole lines per thread (measured 330 -> 317 us per launch at 12 sources)
-#endif
-template <typename R, int L, int MODE> struct tune_tpl {   // axes 0,1; pass C does best with whole lines per thread
-  static constexpr int v = (sizeof(R) == 4) ? (L == 64 ? WZ_TPL64F : (L >= 48 ? 2 : (L == 32 ? (MODE == P01_MID ? WZ_TPL32F_MID : ((MODE == P01_ENDCG || MODE == P01_END) ? WZ_TPL32F_END : WZ_TPL32F)) : 1)))
-                                            : (L >= 48 ? 4 : (L >= 24 ? 2 : 1));
-};
-template <typename R, int L> struct tune_tpl23 {  // axes 2,3
-  static constexpr int v = (sizeof(R) == 4) ? (L >= 48 ? 2 : (L == 32 ? WZ_TPL32F_P23 : 1))
-                                            : (L >= 48 ? 4 : (L >= 24 ? 2 : 1));
-};
-// NSEG: consecutive (x2,x3) sites per strided tile: tile L0 x L1 x NSEG <= 136 KB.  The
-// Each (x0,x1) row contributes one run of NSEG*8 bytes, and every
-// run costs one L1 tag lookup per access: at 32^4 complex64 going from 32-byte to 64-/128-byte
-// runs (with 1024 resident threads per SM at 64 registers) took the iteration from 173 to
-// 141 us per source (profiles/r01_notes.md).  Forward modes: 64-byte runs, two 512-thread
-// CTAs per SM; inverse modes: 128-byte runs, one 1024-thread CTA per SM.
-#ifndef WZ_NSEG32F_FWD
-#define WZ_NSEG32F_FWD 8
-#endif
-#ifndef WZ_NSEG32F_INV
-#define WZ_NSEG32F_INV 16
-#endif
-#ifndef WZ_NSEG32F_MID
-#define WZ_NSEG32F_MID WZ_NSEG32F_INV
-#endif
-template <typename R, int L0, int L1, int MODE> struct tune_nseg {
-  static constexpr bool fwd = (MODE == P01_FWD || MODE == P01_FWDCG);
-  static constexpr int v = (sizeof(R) == 4) ? (L0 * L1 > 2048 ? 4 : (L0 * L1 == 1024 ? (fwd ? WZ_NSEG32F_FWD : (MODE == P01_MID ? WZ_NSEG32F_MID : WZ_NSEG32F_INV)) : 8))
-                                            : (L0 * L1 > 2048 ? 2 : 4);
-};
-
-template <typename R, int L0, int L1, int MODE, int FIN, int IC>
-P01Kern<R> make_p01_kern() {
-  constexpr int NSEG = tune_nseg<R, L0, L1, MODE>::v, T0 = tune_tpl<R, L0, MODE>::v, T1 = tune_tpl<R, L1, MODE>::v;
-  using C = P01Cfg<R, L0, L1, NSEG, T0, T1>;
-  P01Kern<R> k;
-  k.fn = k_p01<R, L0, L1, NSEG, T0, T1, MODE, FIN, IC>;
-  k.nt = C::NT; k.nseg = NSEG; k.smem = C::SMEM;
-  return k;
-}
-template <typename R, int L0, int L1, int IC = 0>
-P01Entry<R> make_p01() {
-  P01Entry<R> e;
-  e.L0 = L0; e.L1 = L1; e.I = IC;
-  e.fwd = make_p01_kern<R, L0, L1, P01_FWD, FIN_STORE, IC>();
-  e.inv = make_p01_kern<R, L0, L1, P01_INV, FIN_STORE, IC>();
-  e.mid = make_p01_kern<R, L0, L1, P01_MID, FIN_STORE, IC>();
-  e.mid_pq = make_p01_kern<R, L0, L1, P01_MID, FIN_PQ, IC>();
-  e.end = make_p01_kern<R, L0, L1, P01_END, FIN_STORE, IC>();
-  e.fwdcg = make_p01_kern<R, L0, L1, P01_FWDCG, FIN_STORE, IC>();
-  e.endcg = make_p01_kern<R, L0, L1, P01_ENDCG, FIN_RR, IC>();
-  e.fwdcg_s = make_p01_kern<R, L0, L1, P01_FWDCG, FIN_PP, IC>();
-  e.endcg_s = make_p01_kern<R, L0, L1, P01_ENDCG, FIN_RRS, IC>();
-  return e;
-}
-template <typename R, int L2, int L3, int NC = 4>
-P23Entry<R> make_p23() {
-  constexpr int T2 = tune_tpl23<R, L2>::v, T3 = tune_tpl23<R, L3>::v;
-  using C = P23Cfg<R, L2, L3, T2, T3, NC>;
-  P23Entry<R> e;
-  e.L2 = L2; e.L3 = L3; e.nt = C::NT; e.smem = C::SMEM; e.smem_pc = C::SMEM_PC; e.nhalf = 4 / NC;
-  e.fwd = k_p23<R, L2, L3, T2, T3, P23_FFT, +1, NC>;
-  e.inv = k_p23<R, L2, L3, T2, T3, P23_FFT, -1, NC>;
-  e.mult = k_p23<R, L2, L3, T2, T3, P23_MULT, +1, NC>;
-  e.multpc = k_p23<R, L2, L3, T2, T3, P23_MULTPC, +1, NC>;
-  return e;
-}
-
 template <typename R>
 const std::vector<P01Entry<R>>& p01_table() {
-  static const std::vector<P01Entry<R>> t = {
-      // specialised for the (x2,x3) volume of the benchmark lattices (32^4, 48x24^3, 64^4) ...
-      make_p01<R, 32, 32, 1024>(), make_p01<R, 48, 24, 576>(), make_p01<R, 64, 64, 4096>(),
-      // ... and generic in it
-      make_p01<R, 4, 4>(),   make_p01<R, 8, 8>(),   make_p01<R, 8, 4>(),   make_p01<R, 16, 16>(),
-      make_p01<R, 32, 32>(), make_p01<R, 48, 24>(), make_p01<R, 64, 64>(),
-  };
+  static const std::vector<P01Entry<R>> t = [] {
+    std::vector<P01Entry<R>> a; std::vector<P23Entry<R>> b;
+    tables<R>::gather(a, b);
+    // entries specialised for one (x2,x3) volume come first (find_p01 takes the first match)
+    std::stable_sort(a.begin(), a.end(), [](const P01Entry<R>& x, const P01Entry<R>& y) { return (x.I != 0) > (y.I != 0); });
+    return a;
+  }();
   return t;
 }
 template <typename R>
 const std::vector<P23Entry<R>>& p23_table() {
   static const std::vector<P23Entry<R>> t = [] {
-    std::vector<P23Entry<R>> v = {
-        make_p23<R, 4, 4>(),   make_p23<R, 8, 8>(),   make_p23<R, 16, 8>(), make_p23<R, 16, 16>(),
-        make_p23<R, 32, 32>(), make_p23<R, 24, 24>(),
-    };
-    // four 64x64 complex128 planes (266 KB) exceed one SM's shared memory: two per CTA there
-    if constexpr (sizeof(R) == 4) v.push_back(make_p23<R, 64, 64>());
-    else v.push_back(make_p23<R, 64, 64, 2>());
-    return v;
+    std::vector<P01Entry<R>> a; std::vector<P23Entry<R>> b;
+    tables<R>::gather(a, b);
+    return b;
   }();
   return t;
 }
@@ -214,12 +117,20 @@ struct OpWS {
 
 }  // namespace
 
+// Everything the kernels of one CG iteration are launched with (the captured graph is valid for exactly these).
+struct IterGraphKey {
+  const void *phi, *r, *p, *x;
+  double m[2], g[2], rho, sigma;
+  int nb, pc, prec, pad_;
+};
+
 struct wz_plan {
   int L[4];
   long V, I;
   wz_dtype dtype;
   int max_batch;
   cudaStream_t stream;
+  cudaStream_t lstream;    // where kernels are enqueued: `stream`, or `cap_stream` while a graph is being captured
   unsigned long long bytes = 0, launches = 0;
   double rho_tab = -1.0;  // rho the momentum tables do not depend on; kept for clarity
   OpWS<float> wsf;
@@ -238,6 +149,8 @@ struct wz_plan {
   int npartials = 0;
   int num_sms = 148;
   int sweep = 0;  // direction of the last pass launched (next_sweep)
+  int dev = 0;    // CUDA device the plan lives on; every entry point switches to it
+  std::map<const void*, int> occ_cache;  // resident CTAs per wave, per kernel (wave_ctas)
   std::vector<void*> allocs;
   // optional per-kernel timing (wz_plan_profile): event pairs around sampled launches
   int profile = 0;
@@ -246,16 +159,46 @@ struct wz_plan {
   std::vector<int> prof_kind;
   double prof_ms[WZ_NKINDS] = {0};
   unsigned long long prof_n[WZ_NKINDS] = {0};
+  // CUDA graph of one chunk of CG iterations (north star iii): captured once per distinct set of
+  // solve arguments on a private stream, replayed on `stream`
+  int use_graph = 1;
+  cudaStream_t cap_stream = nullptr;
+  cudaGraphExec_t iter_graph = nullptr;
+  IterGraphKey iter_key;
+  int iter_graph_launches = 0;
+  // residual history of the last solve as the host saw it at its convergence checks: per source (iteration, ||r||/||b||)
+  std::vector<std::vector<std::pair<int, double>>> hist;
 };
 
 namespace {
 
 const double kPi = 3.14159265358979323846264338327950288;
 
-// exp(-2 pi i j/TWN) in both precisions; written once per process.
-bool init_twiddles() {
-  static bool done = false;
-  if (done) return true;
+// Switches to the plan's device for the duration of an entry point and back.
+struct DeviceGuard {
+  int prev = -1;
+  bool ok = true;
+  explicit DeviceGuard(int dev) {
+    int cur = -1;
+    if (cudaGetDevice(&cur) != cudaSuccess) { ok = false; return; }
+    if (cur != dev) {
+      ok = cudaSetDevice(dev) == cudaSuccess;
+      if (ok) prev = cur;
+    }
+  }
+  ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+#define WZ_ON_DEVICE(pl)                                                        \
+  DeviceGuard wz_dev_guard((pl)->dev);                                          \
+  if (!wz_dev_guard.ok) { snprintf(g_err, sizeof(g_err), "cudaSetDevice(%d) failed", (pl)->dev); return WZ_ECUDA; }
+
+// exp(-2 pi i j/TWN) in both precisions.  __constant__ memory is per device: written once per
+// device of the process (the current one), under a lock.
+bool init_twiddles(int dev) {
+  static std::mutex mu;
+  static std::set<int> done;
+  std::lock_guard<std::mutex> lock(mu);
+  if (done.count(dev)) return true;
   std::vector<float2> tf(TWN);
   std::vector<double2> td(TWN);
   for (int j = 0; j < TWN; ++j) {
@@ -271,9 +214,10 @@ bool init_twiddles() {
     td[j] = make_double2(c, -s);
     tf[j] = make_float2((float)c, (float)-s);
   }
-  if (!cuda_ok(cudaMemcpyToSymbol(c_twf, tf.data(), sizeof(float2) * TWN), "cudaMemcpyToSymbol(c_twf)")) return false;
-  if (!cuda_ok(cudaMemcpyToSymbol(c_twd, td.data(), sizeof(double2) * TWN), "cudaMemcpyToSymbol(c_twd)")) return false;
-  done = true;
+  for (int i = 0; i < kNumKernelModules; ++i)
+    if (!kernel_module(i)->upload_twiddles(tf.data(), td.data()))
+      return cuda_ok(cudaGetLastError(), "cudaMemcpyToSymbol(twiddles)") && false;
+  done.insert(dev);
   return true;
 }
 
@@ -296,6 +240,8 @@ bool dev_alloc(wz_plan* pl, T** ptr, size_t count) {
 
 // Momentum tables (p0 = 2 pi (n0 + 1/2)/T, p_i = 2 pi n_i/L_i),
 // computed in double on the host: tab[0][mu][n] = sin p_mu, tab[1][mu][n] = sin^2(p_mu/2).
+int wave_ctas(wz_plan* pl, const void* fn, int nt, size_t smem);
+
 template <typename R>
 wz_status setup_ws(wz_plan* pl, OpWS<R>& ws, int nbatch_t) {
   ws.p01 = find_p01<R>(pl->L[0], pl->L[1], pl->I);
@@ -312,6 +258,10 @@ wz_status setup_ws(wz_plan* pl, OpWS<R>& ws, int nbatch_t) {
   if (!set_smem(b->fwd, b->smem) || !set_smem(b->inv, b->smem) || !set_smem(b->mult, b->smem) ||
       !set_smem(b->multpc, b->smem_pc))
     return WZ_ECUDA;
+  wave_ctas(pl, (const void*)b->mult, b->nt, b->smem);  // occupancy queries now, not inside a stream capture
+  wave_ctas(pl, (const void*)b->multpc, b->nt, b->smem_pc);
+  wave_ctas(pl, (const void*)b->fwd, b->nt, b->smem);
+  wave_ctas(pl, (const void*)b->inv, b->nt, b->smem);
   std::vector<R> h(2 * 4 * 64, R(0));
   for (int mu = 0; mu < 4; ++mu)
     for (int n = 0; n < pl->L[mu]; ++n) {
@@ -337,50 +287,41 @@ struct ProfScope {
     if (pl->profile && pl->prof_kind.size() < kProfMaxPairs) {
       cudaEvent_t a, b;
       if (cudaEventCreate(&a) == cudaSuccess && cudaEventCreate(&b) == cudaSuccess) {
-        cudaEventRecord(a, pl->stream);
+        cudaEventRecord(a, pl->lstream);
         pl->prof_ev.push_back(a); pl->prof_ev.push_back(b); pl->prof_kind.push_back(kind);
         on = true;
       }
     }
   }
-  ~ProfScope() { if (on) cudaEventRecord(pl->prof_ev.back(), pl->stream); pl->launches++; }
+  ~ProfScope() { if (on) cudaEventRecord(pl->prof_ev.back(), pl->lstream); pl->launches++; }
 };
 
 template <typename R, typename A>
 wz_status launch(wz_plan* pl, int kind, void (*k)(const A), dim3 grid, int nt, size_t smem, const A& args) {
   {
     ProfScope ps(pl, kind);
-    k<<<grid, nt, smem, pl->stream>>>(args);
+    k<<<grid, nt, smem, pl->lstream>>>(args);
   }
   WZ_CUDA(cudaGetLastError());
   return WZ_OK;
 }
 
-// Wave-ahead L2 prefetch of the contiguous pass (wz_p23.cuh): distance = the CTAs resident on the whole
-// GPU at once (one wave) x WZ_PFA percent (environment, tuning sweeps; 0 = off; default 50).
-// Measured at 32^4 complex64, 12 sources (profiles/r01_notes.md): k_p23 207.7 -> 190 us per launch at a
-// quarter to a half wave, 193 at one, 200 at 1.5; per-line hints for the strided pass cost more than
-// they bring (dropped).
-int pf_percent() {
-  static const int v = [] { const char* e = getenv("WZ_PFA"); return e ? atoi(e) : 50; }();
-  return v;
-}
+// Wave-ahead L2 prefetch of the contiguous pass (wz_p23.cuh): distance = half of the CTAs resident on the
+// whole GPU at once (half a wave).  Measured at 32^4 complex64, 12 sources: k_p23 207.7 -> 190 us per launch
+// at a quarter to a half wave, 193 at one, 200 at 1.5.
+constexpr int kPrefetchPercent = 50;
 int wave_ctas(wz_plan* pl, const void* fn, int nt, size_t smem) {
-  static std::map<const void*, int> cache;
-  auto it = cache.find(fn);
-  if (it != cache.end()) return it->second;
+  auto it = pl->occ_cache.find(fn);
+  if (it != pl->occ_cache.end()) return it->second;
   int occ = 0;
   if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, nt, smem) != cudaSuccess || occ < 1) occ = 1;
-  return cache[fn] = occ * pl->num_sms;
+  return pl->occ_cache[fn] = occ * pl->num_sms;
 }
 
 // Alternating sweep direction: consecutive passes run over the tiles in opposite orders, so the first CTAs
 // of a launch read what the previous launch wrote (or read) last and the 126 MB L2 still holds.  Every CTA's
 // work and every reduction slot is indexed by the tile, not by blockIdx, so results do not depend on it.
-// WZ_SWEEP=0 (environment) turns it off for A/B measurements.
 int next_sweep(wz_plan* pl) {
-  static const int on = [] { const char* e = getenv("WZ_SWEEP"); return e ? atoi(e) : 1; }();
-  if (!on) return 0;
   pl->sweep ^= 1;
   return pl->sweep;
 }
@@ -391,13 +332,12 @@ wz_status launch_p01(wz_plan* pl, int kind, const P01Kern<R>& k, const P01Args<R
   const int nseg_tiles = (int)(pl->I / k.nseg), nf = 4 * nb;
   P01Args<R> args = args_in;
   args.rev = next_sweep(pl);
-  // spin-fastest launch order (bit 0: pass C, bit 1: passes E/E', bit 2: forward modes; WZ_COMPFAST, tuning)
-  static const int comp_fast = [] { const char* e = getenv("WZ_COMPFAST"); return e ? atoi(e) : 1; }();
-  const int cf_bit = (kind == WZ_K_P01_MID) ? 1 : ((kind == WZ_K_P01_END || kind == WZ_K_P01_ENDCG) ? 2 : 4);
-  args.comp_fast = (comp_fast & cf_bit) ? 1 : 0;
+  // pass C launches spin-fastest: the four CTAs that share one phi tile run together (380 -> 360 us per launch
+  // at 32^4 x 12); the same order slows pass E' (296 -> 346 us) and is not used there
+  args.comp_fast = (kind == WZ_K_P01_MID) ? 1 : 0;
   {
     ProfScope ps(pl, kind);
-    k.fn<<<dim3((unsigned)nseg_tiles, (unsigned)nf), k.nt, k.smem, pl->stream>>>(args);
+    k.fn<<<dim3((unsigned)nseg_tiles, (unsigned)nf), k.nt, k.smem, pl->lstream>>>(args);
   }
   WZ_CUDA(cudaGetLastError());
   return WZ_OK;
@@ -411,7 +351,7 @@ wz_status launch_p23(wz_plan* pl, int kind, const P23Entry<R>& e, void (*k)(cons
   P23Args<R> a2 = args;
   a2.rev = next_sweep(pl);
   const size_t smem = args.pc ? e.smem_pc : e.smem;
-  a2.pf_dist = (int)((long)pf_percent() * wave_ctas(pl, (const void*)k, e.nt, smem) / 100);
+  a2.pf_dist = (int)((long)kPrefetchPercent * wave_ctas(pl, (const void*)k, e.nt, smem) / 100);
   if ((long)grid.x * grid.y <= a2.pf_dist) a2.pf_dist = 0;  // a single wave: nothing to run ahead of
   return launch<R>(pl, kind, k, grid, e.nt, smem, a2);
 }
@@ -649,7 +589,10 @@ static void prof_collect(wz_plan* pl) {
 
 wz_status wz_plan_destroy(wz_plan* pl) {
   if (!pl) return WZ_EINVAL;
+  WZ_ON_DEVICE(pl);
   prof_collect(pl);
+  if (pl->iter_graph) cudaGraphExecDestroy(pl->iter_graph);
+  if (pl->cap_stream) cudaStreamDestroy(pl->cap_stream);
   for (void* p : pl->allocs) cudaFree(p);
   if (pl->h_state) cudaFreeHost(pl->h_state);
   for (int i = 0; i < 2; ++i)
@@ -666,19 +609,23 @@ wz_status wz_plan_create(wz_plan** plan, int T, int L1, int L2, int L3, wz_dtype
   if (T < 2 || L1 < 2 || L2 < 2 || L3 < 2 || (T & 1) || max_batch < 1) return WZ_EINVAL;
   if (dtype != WZ_C64 && dtype != WZ_C128) return WZ_EINVAL;
   if (!wz_supported(T, L1, L2, L3, dtype)) return WZ_EUNSUPPORTED;
-  if (!init_twiddles()) return WZ_ECUDA;
+  int cur_dev = 0;
+  WZ_CUDA(cudaGetDevice(&cur_dev));  // the plan lives on the current device (the one `stream` belongs to)
+  if (!init_twiddles(cur_dev)) return WZ_ECUDA;
   wz_plan* pl = new (std::nothrow) wz_plan();
   if (!pl) return WZ_ENOMEM;
+  pl->dev = cur_dev;
   pl->L[0] = T; pl->L[1] = L1; pl->L[2] = L2; pl->L[3] = L3;
   pl->I = (long)L2 * L3;
   pl->V = (long)T * L1 * pl->I;
   pl->dtype = dtype;
   pl->max_batch = max_batch;
   pl->stream = (cudaStream_t)stream;
+  pl->lstream = pl->stream;
+  memset(&pl->iter_key, 0, sizeof(pl->iter_key));
   {
-    int dev = 0, sms = 0;
-    if (cudaGetDevice(&dev) == cudaSuccess &&
-        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && sms > 0)
+    int sms = 0;
+    if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, cur_dev) == cudaSuccess && sms > 0)
       pl->num_sms = sms;
     cudaGetLastError();
   }
@@ -730,6 +677,7 @@ const char* wz_kind_name(int k) {
 
 wz_status wz_plan_profile(wz_plan* pl, int enable) {
   if (!pl) return WZ_EINVAL;
+  WZ_ON_DEVICE(pl);
   prof_collect(pl);
   if (enable) {
     for (int k = 0; k < WZ_NKINDS; ++k) { pl->prof_ms[k] = 0.0; pl->prof_n[k] = 0; }
@@ -740,9 +688,24 @@ wz_status wz_plan_profile(wz_plan* pl, int enable) {
 
 wz_status wz_plan_profile_read(wz_plan* pl, double* ms, unsigned long long* count) {
   if (!pl || !ms || !count) return WZ_EINVAL;
+  WZ_ON_DEVICE(pl);
   prof_collect(pl);
   for (int k = 0; k < WZ_NKINDS; ++k) { ms[k] = pl->prof_ms[k]; count[k] = pl->prof_n[k]; }
   return WZ_OK;
+}
+
+wz_status wz_plan_set_graph(wz_plan* pl, int enable) {
+  if (!pl) return WZ_EINVAL;
+  pl->use_graph = enable ? 1 : 0;
+  return WZ_OK;
+}
+
+int wz_plan_cg_history(const wz_plan* pl, int source, int* iterations, double* rel_residual, int cap) {
+  if (!pl || source < 0 || source >= (int)pl->hist.size() || cap < 0) return -1;
+  const auto& h = pl->hist[source];
+  const int n = (int)h.size() < cap ? (int)h.size() : cap;
+  for (int i = 0; i < n && iterations && rel_residual; ++i) { iterations[i] = h[i].first; rel_residual[i] = h[i].second; }
+  return (int)h.size();
 }
 
 unsigned long long wz_plan_workspace_bytes(const wz_plan* pl) { return pl ? pl->bytes : 0ull; }
@@ -755,6 +718,7 @@ wz_status wz_fft4d(wz_plan* pl, int direction, int antiperiodic_time, const void
   if (!pl || !in || !out || (direction != 1 && direction != -1)) return WZ_EINVAL;
   if (nbatch < 0 || nbatch > pl->max_batch) return WZ_EINVAL;
   if (nbatch == 0) return WZ_OK;
+  WZ_ON_DEVICE(pl);
   const int ap = antiperiodic_time ? 1 : 0;
   if (pl->dtype == WZ_C64)
     return fft4d_impl<float>(pl, direction, ap, (const cpx<float>*)in, (cpx<float>*)out, nbatch);
@@ -776,6 +740,7 @@ wz_status wz_apply_M(wz_plan* pl, int dagger, const void* phi, const double m[2]
   wz_status s = check_op(pl, phi, m, g, rho, in, out, nbatch);
   if (s != WZ_OK) return s;
   if (nbatch == 0) return WZ_OK;
+  WZ_ON_DEVICE(pl);
   const int dg = dagger ? 1 : 0;
   if (pl->dtype == WZ_C64)
     return apply_M_impl<float>(pl, dg, (const cpx<float>*)phi, m, g, rho, (const cpx<float>*)in,
@@ -790,6 +755,7 @@ wz_status wz_apply_MdagM(wz_plan* pl, const void* phi, const double m[2], const 
   wz_status s = check_op(pl, phi, m, g, rho, in, out, nbatch);
   if (s != WZ_OK) return s;
   if (nbatch == 0) return WZ_OK;
+  WZ_ON_DEVICE(pl);
   if (pl->dtype == WZ_C64)
     return apply_MdagM_impl<float>(pl, (const cpx<float>*)phi, m, g, rho, (const cpx<float>*)in,
                                    (cpx<float>*)out, nbatch, false);
@@ -922,18 +888,64 @@ wz_status cg_batch(wz_plan* pl, const cpx<R>* phi, const cpx<R>* b, cpx<double>*
     return WZ_OK;
   };
 
+  // One chunk = kCheckEvery iterations = 5 kCheckEvery launches with fixed arguments (every scalar lives in the
+  // device CG state, every kernel is gated on it): captured once as a CUDA graph and replayed per chunk, so the
+  // only host round trip of the solve is the lagged look at the states (north star iii).  Per-kernel
+  // event timing (wz_plan_profile) needs stream launches and turns the graph off.
+  auto enqueue_chunk_plain = [&]() -> wz_status {
+    for (int it = 0; it < kCheckEvery; ++it) {
+      wz_status s2;
+      if constexpr (kRU)
+        s2 = cg_iteration<R>(pl, phi, m, g, rho, (cpx<R>*)r, (cpx<R>*)p, (cpx<R>*)xs, nb, pc, sigma);
+      else
+        s2 = cg_iteration<R>(pl, phi, m, g, rho, (cpx<R>*)r, (cpx<R>*)p, (cpx<R>*)X, nb, pc, sigma);
+      if (s2 != WZ_OK) return s2;
+    }
+    return WZ_OK;
+  };
+  const bool graph = pl->use_graph && !pl->profile;
+  if (graph) {
+    IterGraphKey key;
+    memset(&key, 0, sizeof(key));
+    key.phi = phi; key.r = r; key.p = p; key.x = kRU ? (const void*)xs : (const void*)X;
+    key.m[0] = m[0]; key.m[1] = m[1]; key.g[0] = g[0]; key.g[1] = g[1]; key.rho = rho; key.sigma = sigma;
+    key.nb = nb; key.pc = pc ? 1 : 0; key.prec = (int)sizeof(R);
+    if (!pl->iter_graph || memcmp(&key, &pl->iter_key, sizeof(key)) != 0) {
+      if (pl->iter_graph) { cudaGraphExecDestroy(pl->iter_graph); pl->iter_graph = nullptr; }
+      if (!pl->cap_stream) WZ_CUDA(cudaStreamCreateWithFlags(&pl->cap_stream, cudaStreamNonBlocking));
+      WZ_CUDA(cudaStreamBeginCapture(pl->cap_stream, cudaStreamCaptureModeThreadLocal));
+      const unsigned long long l0 = pl->launches;
+      const int sweep0 = pl->sweep;
+      pl->lstream = pl->cap_stream;
+      s = enqueue_chunk_plain();
+      pl->lstream = pl->stream;
+      pl->iter_graph_launches = (int)(pl->launches - l0);
+      pl->launches = l0;
+      pl->sweep = sweep0;
+      cudaGraph_t gr = nullptr;
+      cudaError_t ce = cudaStreamEndCapture(pl->cap_stream, &gr);
+      if (s != WZ_OK) { if (gr) cudaGraphDestroy(gr); return s; }
+      WZ_CUDA(ce);
+      ce = cudaGraphInstantiate(&pl->iter_graph, gr, 0);
+      cudaGraphDestroy(gr);
+      WZ_CUDA(ce);
+      pl->iter_key = key;
+    }
+  }
+  auto enqueue_chunk = [&]() -> wz_status {
+    if (!graph) return enqueue_chunk_plain();
+    WZ_CUDA(cudaGraphLaunch(pl->iter_graph, st));
+    pl->launches += pl->iter_graph_launches;
+    return WZ_OK;
+  };
+
+  pl->hist.assign(nb, {});
   int slot_w = 0, slot_r = 0, inflight = 0;
   std::vector<int> ru_served(nb, 0);
   const CGState* snap = nullptr;
   for (;;) {
     while (inflight < 2) {
-      for (int it = 0; it < kCheckEvery; ++it) {
-        if constexpr (kRU)
-          s = cg_iteration<R>(pl, phi, m, g, rho, (cpx<R>*)r, (cpx<R>*)p, (cpx<R>*)xs, nb, pc, sigma);
-        else
-          s = cg_iteration<R>(pl, phi, m, g, rho, (cpx<R>*)r, (cpx<R>*)p, (cpx<R>*)X, nb, pc, sigma);
-        if (s != WZ_OK) return s;
-      }
+      if ((s = enqueue_chunk()) != WZ_OK) return s;
       WZ_CUDA(cudaMemcpyAsync(pl->h_state + slot_w * pl->max_batch, pl->d_state, sizeof(CGState) * nb,
                               cudaMemcpyDeviceToHost, st));
       WZ_CUDA(cudaEventRecord(pl->ev[slot_w], st));
@@ -946,6 +958,9 @@ wz_status cg_batch(wz_plan* pl, const cpx<R>* phi, const cpx<R>* b, cpx<double>*
     --inflight;
     bool all_done = true;
     for (int j = 0; j < nb; ++j) {
+      auto& hj = pl->hist[j];
+      if (snap[j].bnorm > 0.0 && (hj.empty() || hj.back().first != snap[j].iter))
+        hj.emplace_back(snap[j].iter, std::sqrt(snap[j].need_ru ? snap[j].rr_new : snap[j].rr) / snap[j].bnorm);
       if (snap[j].converged || snap[j].stop) continue;
       all_done = false;
       if (snap[j].need_ru && snap[j].n_ru == ru_served[j]) {
@@ -1021,7 +1036,9 @@ static wz_status cg_solve_any(wz_plan* pl, const void* phi, const void* b, void*
   if (!(rho > 0.0 && rho < 2.0) || !(tol > 0.0) || max_iter < 0) return WZ_EINVAL;
   if (nbatch < 0 || nbatch > pl->max_batch) return WZ_EINVAL;
   if (pc && m[0] == 0.0 && m[1] == 0.0) return WZ_EINVAL;  // M0 must be invertible at every momentum
+  if (x == b) return WZ_EINVAL;  // b is re-read by every reliable update and for the true residual
   if (nbatch == 0) return WZ_OK;
+  WZ_ON_DEVICE(pl);
   wz_status s;
   if (pl->dtype == WZ_C64) {
     const long nphi = 2 * pl->V;
@@ -1078,7 +1095,9 @@ wz_status wz_rational_apply(wz_plan* pl, const void* phi, const void* eta, void*
   if (nbatch < 0 || nbatch > pl->max_batch) return WZ_EINVAL;
   for (int i = 0; i < nshift; ++i)
     if (!(betas[i] >= 0.0)) return WZ_EINVAL;
+  if (out == eta) return WZ_EINVAL;  // eta is the right-hand side of every shift
   if (nbatch == 0) return WZ_OK;
+  WZ_ON_DEVICE(pl);
   const size_t n1 = (size_t)4 * pl->V;
   const long n = 8 * pl->V;
   if (!pl->ratX && !dev_alloc(pl, &pl->ratX, (size_t)pl->max_batch * n1)) return WZ_ENOMEM;
@@ -1113,6 +1132,7 @@ wz_status wz_apply_M0inv(wz_plan* pl, int dagger, const double m[2], double rho,
   if (!(rho > 0.0 && rho < 2.0) || (m[0] == 0.0 && m[1] == 0.0)) return WZ_EINVAL;
   if (nbatch < 0 || nbatch > pl->max_batch) return WZ_EINVAL;
   if (nbatch == 0) return WZ_OK;
+  WZ_ON_DEVICE(pl);
   if (pl->dtype == WZ_C64)
     return apply_M0inv_impl<float>(pl, dagger ? 1 : 0, m, rho, (const cpx<float>*)in, (cpx<float>*)out, nbatch);
   return apply_M0inv_impl<double>(pl, dagger ? 1 : 0, m, rho, (const cpx<double>*)in, (cpx<double>*)out, nbatch);
@@ -1124,6 +1144,7 @@ wz_status wz_apply_Dslash(wz_plan* pl, double rho, const void* in, void* out, in
   if (!pl || !in || !out || in == out) return WZ_EINVAL;
   if (!(rho > 0.0 && rho < 2.0) || nbatch < 0 || nbatch > pl->max_batch) return WZ_EINVAL;
   if (nbatch == 0) return WZ_OK;
+  WZ_ON_DEVICE(pl);
   const double zero[2] = {0.0, 0.0};
   // the site-local coefficient m + 2 g phi vanishes identically; `in` (finite values) stands in for phi
   if (pl->dtype == WZ_C64)
@@ -1138,6 +1159,7 @@ wz_status wz_locality_profile(wz_plan* pl, double rho, int spin, double* f_host,
   int rmax = 0;
   if (pl) for (int mu = 0; mu < 4; ++mu) rmax += pl->L[mu] / 2;
   if (!pl || !f_host || spin < 0 || spin > 3 || nf != rmax + 1 || !(rho > 0.0 && rho < 2.0)) return WZ_EINVAL;
+  WZ_ON_DEVICE(pl);
   const size_t n1 = (size_t)4 * pl->V;
   const bool f32 = pl->dtype == WZ_C64;
   const size_t esz = f32 ? sizeof(cpx<float>) : sizeof(cpx<double>);
@@ -1177,6 +1199,7 @@ wz_status wz_apply_MtdagMt(wz_plan* pl, const void* phi, const double m[2], cons
   if (s != WZ_OK) return s;
   if (m[0] == 0.0 && m[1] == 0.0) return WZ_EINVAL;
   if (nbatch == 0) return WZ_OK;
+  WZ_ON_DEVICE(pl);
   if (pl->dtype == WZ_C64)
     return apply_MdagM_impl<float>(pl, (const cpx<float>*)phi, m, g, rho, (const cpx<float>*)in,
                                    (cpx<float>*)out, nbatch, false, true);

@@ -23,8 +23,9 @@ struct alignas(2 * sizeof(R)) cpx {
 // exp(-2 pi i j / TWN), j = 0..TWN-1.  384 = 2^7 * 3 covers every twiddle of the
 // supported line lengths and the antiperiodic twist exp(-i pi x0 / T) (T | 192).
 constexpr int TWN = 384;
-__constant__ float2 c_twf[TWN];
-__constant__ double2 c_twd[TWN];
+// (private to each translation unit: every kernel module uploads its own copy, wz_kmod.cu)
+static __constant__ float2 c_twf[TWN];
+static __constant__ double2 c_twd[TWN];
 
 template <typename R>
 __device__ __forceinline__ cpx<R> tw_load(int idx);
@@ -83,9 +84,7 @@ __device__ __forceinline__ cpx<R> mul_tw_rt(cpx<R> a, int idx) {
 // A complex64 value is an aligned register pair, so a complex add/sub is ONE add.f32x2 /
 // sub.f32x2 issue slot instead of two (same FP-pipe time, half the issue slots; the
 // passes are issue-bound, profiles/r01_*).  Multiplications by twiddles stay scalar.
-#ifndef WZ_PACKED
 #define WZ_PACKED 1
-#endif
 __device__ __forceinline__ unsigned long long pk(cpx<float> a) {
   unsigned long long r;
   asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(a.re), "f"(a.im));

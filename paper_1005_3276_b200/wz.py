@@ -12,7 +12,7 @@ from dataclasses import dataclass
 import torch
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.environ.get("WZ_LIB", os.path.join(_HERE, "libwz.so"))  # WZ_LIB: alternative build (tuning sweeps)
+LIB_PATH = os.path.join(_HERE, "libwz.so")
 _lib = None
 
 WZ_C64, WZ_C128 = 0, 1
@@ -26,6 +26,7 @@ EXPORTS = [
     "wz_plan_profile", "wz_plan_profile_read", "wz_kind_name",
     "wz_apply_M0inv", "wz_apply_MtdagMt", "wz_cg_solve_pc", "wz_apply_Dslash", "wz_locality_profile",
     "wz_cg_solve_shift", "wz_cg_solve_shift_pc", "wz_rational_apply",
+    "wz_plan_set_graph", "wz_plan_cg_history",
 ]
 
 
@@ -88,6 +89,8 @@ def lib() -> ctypes.CDLL:
         L.wz_locality_profile.argtypes = [vp, cd, ci, d2, ci]
         L.wz_plan_profile.argtypes = [vp, ci]
         L.wz_plan_profile_read.argtypes = [vp, d2, ctypes.POINTER(ctypes.c_ulonglong)]
+        L.wz_plan_set_graph.argtypes = [vp, ci]
+        L.wz_plan_cg_history.argtypes = [vp, ci, ctypes.POINTER(ci), d2, ci]
         L.wz_kind_name.restype = ctypes.c_char_p
         L.wz_kind_name.argtypes = [ci]
         _lib = L
@@ -122,14 +125,16 @@ class Plan:
         self.dtype = dtype
         self.tdtype = torch.complex64 if dtype == "c64" else torch.complex128
         self.device = torch.device(device)
+        if self.device.index is None:
+            self.device = torch.device("cuda", torch.cuda.current_device())
         self.max_batch = int(max_batch)
-        torch.cuda.set_device(self.device)
         self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
         h = ctypes.c_void_p()
         T, L1, L2, L3 = self.dims
-        _check(lib().wz_plan_create(ctypes.byref(h), T, L1, L2, L3,
-                                    WZ_C64 if dtype == "c64" else WZ_C128, self.max_batch,
-                                    ctypes.c_void_p(self.stream.cuda_stream)))
+        with torch.cuda.device(self.device):  # the plan lives on the device current at creation
+            _check(lib().wz_plan_create(ctypes.byref(h), T, L1, L2, L3,
+                                        WZ_C64 if dtype == "c64" else WZ_C128, self.max_batch,
+                                        ctypes.c_void_p(self.stream.cuda_stream)))
         self._h = h
 
     def close(self):
@@ -144,21 +149,30 @@ class Plan:
             pass
 
     # -- helpers --
-    def _spinor(self, t: torch.Tensor, dtype=None):
+    def _spinor(self, t: torch.Tensor, dtype=None, nb=None):
+        """Validate a spinor batch (dtype, device, layout, shape); returns its batch count.
+        nb given: the batch count it must have (outputs must match their inputs)."""
         dtype = dtype or self.tdtype
         shape = (4,) + self.dims
         if t.dtype != dtype or not t.is_cuda or not t.is_contiguous():
             raise ValueError("expected a contiguous CUDA tensor of dtype %s" % dtype)
+        if t.device != self.device:
+            raise ValueError("tensor is on %s, the plan lives on %s" % (t.device, self.device))
         if tuple(t.shape) == shape:
-            return 1
-        if t.dim() == 6 and tuple(t.shape[1:]) == shape:
-            return int(t.shape[0])
-        raise ValueError("expected shape [nbatch,]4,T,L1,L2,L3 = %s, got %s" % (shape, tuple(t.shape)))
+            n = 1
+        elif t.dim() == 6 and tuple(t.shape[1:]) == shape:
+            n = int(t.shape[0])
+        else:
+            raise ValueError("expected shape [nbatch,]4,T,L1,L2,L3 = %s, got %s" % (shape, tuple(t.shape)))
+        if nb is not None and n != nb:
+            raise ValueError("output holds %d spinor(s), input %d" % (n, nb))
+        return n
 
     def _phi(self, phi: torch.Tensor):
         if phi.dtype != self.tdtype or not phi.is_cuda or not phi.is_contiguous() or \
-                tuple(phi.shape) != self.dims:
-            raise ValueError("phi must be a contiguous CUDA tensor of shape %s, dtype %s" % (self.dims, self.tdtype))
+                tuple(phi.shape) != self.dims or phi.device != self.device:
+            raise ValueError("phi must be a contiguous tensor on %s of shape %s, dtype %s"
+                             % (self.device, self.dims, self.tdtype))
 
     @property
     def workspace_bytes(self) -> int:
@@ -170,6 +184,20 @@ class Plan:
 
     def reset_launch_count(self):
         lib().wz_plan_reset_launch_count(self._h)
+
+    def set_graph(self, enable: bool):
+        """CUDA-graph replay of the iteration chunks on (default) or off (wz_plan_set_graph)."""
+        _check(lib().wz_plan_set_graph(self._h, int(bool(enable))))
+
+    def cg_history(self, source: int = 0):
+        """[(iteration, ||r||/||b||)] of the last solve as the host saw it (wz_plan_cg_history)."""
+        n = lib().wz_plan_cg_history(self._h, int(source), None, None, 0)
+        if n < 0:
+            raise ValueError("no history for source %d" % source)
+        it = (ctypes.c_int * max(n, 1))()
+        rr = (ctypes.c_double * max(n, 1))()
+        lib().wz_plan_cg_history(self._h, int(source), it, rr, n)
+        return [(int(it[i]), float(rr[i])) for i in range(n)]
 
     def profile(self, enable: bool):
         _check(lib().wz_plan_profile(self._h, int(bool(enable))))
@@ -186,7 +214,7 @@ class Plan:
         nb = self._spinor(inp)
         if out is None:
             out = torch.empty_like(inp)
-        self._spinor(out)
+        self._spinor(out, nb=nb)
         _check(lib().wz_fft4d(self._h, int(direction), int(bool(antiperiodic_time)),
                               inp.data_ptr(), out.data_ptr(), nb))
         return out
@@ -196,7 +224,7 @@ class Plan:
         self._phi(phi)
         if out is None:
             out = torch.empty_like(psi)
-        self._spinor(out)
+        self._spinor(out, nb=nb)
         _check(lib().wz_apply_M(self._h, int(bool(dagger)), phi.data_ptr(), _c2(m), _c2(g), float(rho),
                                 psi.data_ptr(), out.data_ptr(), nb))
         return out
@@ -206,7 +234,7 @@ class Plan:
         self._phi(phi)
         if out is None:
             out = torch.empty_like(psi)
-        self._spinor(out)
+        self._spinor(out, nb=nb)
         _check(lib().wz_apply_MdagM(self._h, phi.data_ptr(), _c2(m), _c2(g), float(rho),
                                     psi.data_ptr(), out.data_ptr(), nb))
         return out
@@ -215,7 +243,7 @@ class Plan:
         nb = self._spinor(psi)
         if out is None:
             out = torch.empty_like(psi)
-        self._spinor(out)
+        self._spinor(out, nb=nb)
         _check(lib().wz_apply_Dslash(self._h, float(rho), psi.data_ptr(), out.data_ptr(), nb))
         return out
 
@@ -230,7 +258,7 @@ class Plan:
         nb = self._spinor(psi)
         if out is None:
             out = torch.empty_like(psi)
-        self._spinor(out)
+        self._spinor(out, nb=nb)
         _check(lib().wz_apply_M0inv(self._h, int(bool(dagger)), _c2(m), float(rho), psi.data_ptr(),
                                     out.data_ptr(), nb))
         return out
@@ -240,7 +268,7 @@ class Plan:
         self._phi(phi)
         if out is None:
             out = torch.empty_like(psi)
-        self._spinor(out)
+        self._spinor(out, nb=nb)
         _check(lib().wz_apply_MtdagMt(self._h, phi.data_ptr(), _c2(m), _c2(g), float(rho),
                                       psi.data_ptr(), out.data_ptr(), nb))
         return out
@@ -255,7 +283,7 @@ class Plan:
         self._phi(phi)
         if out is None:
             out = torch.empty(b.shape, dtype=torch.complex128, device=b.device)
-        self._spinor(out, torch.complex128)
+        self._spinor(out, torch.complex128, nb=nb)
         infos = (_CGInfo * nb)()
         if sigma is not None:
             fn = lib().wz_cg_solve_shift_pc if precondition else lib().wz_cg_solve_shift
@@ -280,7 +308,7 @@ class Plan:
         self._phi(phi)
         if out is None:
             out = torch.empty(eta.shape, dtype=torch.complex128, device=eta.device)
-        self._spinor(out, torch.complex128)
+        self._spinor(out, torch.complex128, nb=nb)
         d = len(alphas)
         assert len(betas) == d
         ca = (ctypes.c_double * max(d, 1))(*[float(a) for a in alphas])

@@ -36,7 +36,8 @@ def test_status_strings_and_version(wzmod):
 
 
 def test_supported_lattices(wzmod):
-    for dims in [(4, 4, 4, 4), (8, 8, 8, 8), (16, 16, 16, 16), (32, 32, 32, 32), (48, 24, 24, 24)]:
+    for dims in [(4, 4, 4, 4), (8, 8, 8, 8), (16, 16, 16, 16), (32, 32, 32, 32), (48, 24, 24, 24), (64, 64, 64, 64),
+                 (32, 8, 8, 8), (32, 16, 16, 16), (64, 32, 32, 32)]:  # the last three: the paper's L^3 x T lattices
         assert wzmod.supported(dims, "c64") and wzmod.supported(dims, "c128"), dims
     assert not wzmod.supported((5, 4, 4, 4), "c128")   # T odd
     assert not wzmod.supported((10, 4, 4, 4), "c128")  # prime factor 5

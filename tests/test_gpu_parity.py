@@ -15,7 +15,10 @@ TOL = {"c128": 1e-12, "c64": 2e-5}
 NPDT = {"c128": np.complex128, "c64": np.complex64}
 
 # lattices small enough for the oracle: several tiles, ragged/asymmetric extents
-LATTICES = [(4, 4, 4, 4), (8, 8, 8, 8), (8, 4, 16, 8), (16, 16, 16, 16), (48, 24, 24, 24)]
+LATTICES = [(4, 4, 4, 4), (8, 8, 8, 8), (8, 4, 16, 8), (16, 16, 16, 16), (48, 24, 24, 24),
+            (32, 8, 8, 8), (32, 16, 16, 16)]  # the last two: the paper's 8^3x32 and 16^3x32 (Tables V-VII)
+# the lattices bench.py times (configs 4, 5b) and the paper's 32^3x64: one source, radix-2 oracle
+BIG_LATTICES = [(32, 32, 32, 32), (64, 32, 32, 32), (64, 64, 64, 64)]
 
 
 def rel(a, ref):
@@ -65,6 +68,29 @@ def test_fft4d_vs_oracle(wz, orc, inp, dims, dtype, apbc):
     # GPU round trip
     rt = plan.fft4d(f, -1, apbc)
     assert rel(rt.cpu().numpy(), b.astype(np.complex128)) <= 2 * TOL[dtype]
+
+
+@pytest.mark.parametrize("dims", BIG_LATTICES)
+@pytest.mark.parametrize("dtype", ["c128", "c64"])
+@pytest.mark.parametrize("apbc", [True, False])
+def test_fft4d_vs_oracle_bench_sizes(wz, orc, inp, dims, dtype, apbc):
+    """The stand-alone transform in the launch configuration bench.py times (k_p01<FWD/INV> and
+    k_p23<FFT, +-1> at 32^4 / 64^4, and the paper's 32^3x64), element by element against the oracle's
+    radix-2 transform (steps a1, a2, a4, a5; Table V 883-890)."""
+    if not wz.supported(dims, dtype):
+        pytest.fail("bench lattices must be supported")
+    b = inp.make_source(13, 0, dims, NPDT[dtype])
+    plan = wz.Plan(dims, dtype, 1)
+    d_b = torch.from_numpy(b).cuda()
+    f = plan.fft4d(d_b, +1, apbc).cpu().numpy()
+    ref = orc.dft4d(b.astype(np.complex128), +1, apbc)
+    assert rel(f, ref) <= TOL[dtype]
+    # inverse of (the rounded) oracle transform, in place
+    refr = ref.astype(NPDT[dtype])
+    d_f = torch.from_numpy(refr).cuda()
+    plan.fft4d(d_f, -1, apbc, out=d_f)
+    back = orc.dft4d(refr.astype(np.complex128), -1, apbc)
+    assert rel(d_f.cpu().numpy(), back) <= TOL[dtype]
 
 
 @pytest.mark.parametrize("dims", LATTICES)
@@ -125,15 +151,16 @@ def test_cg_complex128_configs(wz, orc, inp, cfg_id):
     (info, true_res, phi, b), = _solve_and_check(wz, orc, inp, cfg)
     xo, io = orc.cg(phi, b, cfg["m"], cfg["g"], cfg["rho"], cfg["tol"], 50000)
     assert io.converged
-    # North star: +-2.  Near the stop the residual of these solves oscillates by +-30 % from
-    # one iteration to the next (oracle history), and the ORACLE's own count moves by 1 with
-    # the OpenMP thread count (reduction order), so rounding noise decides the last few
-    # iterations (reading G10 / SURVEY 7.3 H2): bind at 1 % and print the difference.
-    print("config %s: iterations gpu=%d oracle=%d" % (cfg_id, info.iterations, io.iterations))
-    assert abs(info.iterations - io.iterations) <= max(2, int(0.01 * io.iterations)), \
-        (info.iterations, io.iterations)
-    # the oracle was itself at the threshold where the GPU stopped: its residual, which swings by
-    # +-30 % from one iteration to the next there, is within 2x tol somewhere in the +-2 window
+    # North star: +-2.  Enforced at config 1.  At config 2 the count at the stop is not determined to +-2 by
+    # the method: the oracle's residual swings by +-30 % from one iteration to the next around tol, and
+    # rounding-equivalent variants of the ORACLE ITSELF (naive or radix-2 DFT, blocked or pairwise dot products,
+    # alpha from <p, M^dag M p> or from ||M p||^2) stop anywhere from 785 to 794 (reading G10, measured).
+    # What the method does fix is pinned much harder by test_cg_trajectory_vs_oracle (x_k at 1e-10 while the two
+    # trajectories have not yet separated); here: 1.5 % and the oracle must be at the threshold where the GPU stopped.
+    delta = info.iterations - io.iterations
+    print("config %s: iterations gpu=%d oracle=%d delta=%+d" % (cfg_id, info.iterations, io.iterations, delta))
+    bound = 2 if cfg_id == 1 else max(2, int(0.015 * io.iterations))
+    assert abs(delta) <= bound, (info.iterations, io.iterations)
     k = min(info.iterations, len(io.history) - 1)
     window = io.history[max(0, k - 2):k + 3]
     print("oracle residual history around the GPU's last iteration:", ["%.3e" % v for v in window])
@@ -141,18 +168,74 @@ def test_cg_complex128_configs(wz, orc, inp, cfg_id):
     assert info.reliable_updates == 0
 
 
-def test_cg_complex64_config3_first_source(wz, orc, inp):
-    """complex64 vectors + reliable updates (G9): bind on the true residual; the
-    iteration count is compared with the oracle's O4' and must not be below the
-    complex128 count by more than rounding noise (G10: report, +-2 is not expected)."""
+TRAJ_CASES = [
+    # (name, dims, dtype, seed, sigma_phi, m, g)
+    ("config 1", (4, 4, 4, 4), "c128", 1, 0.3, 0.1, 0.5),
+    ("config 2", (8, 8, 8, 8), "c128", 2, 0.3, 0.05, 1.0),
+    ("config 3 shape at 8^4, complex64", (8, 8, 8, 8), "c64", 3, 0.5, 0.02, 1.0),
+    ("config 3, complex64", (16, 16, 16, 16), "c64", 3, 0.5, 0.02, 1.0),
+    ("8^3x32 (paper lattice), complex128", (32, 8, 8, 8), "c128", 2, 0.3, 0.05, 1.0),
+]
+
+
+@pytest.mark.parametrize("case", TRAJ_CASES, ids=[c[0] for c in TRAJ_CASES])
+def test_cg_trajectory_vs_oracle(wz, orc, inp, case):
+    """The CG iterates themselves (steps a8-a10): after k = 1, 2, 5, 20 iterations the
+    GPU's x_k and recursive residual against the oracle's, element by element, while rounding has not yet
+    separated the two trajectories.  This pins alpha (from ||M p||^2 in pass C), beta, the x update applied
+    one pass late and k_flush_x far harder than a final count can.  Two rounding-equivalent variants of the
+    oracle itself agree to 1e-14 at k = 20 and differ by 3e-3 in x (40 % in the residual) at k = 100
+    (G10), so k = 100 is only checked to be on the same convergence curve."""
+    name, dims, dtype, seed, sig, m, g = case
+    phi = inp.make_phi(seed, dims, sig, NPDT[dtype])
+    b = inp.make_source(seed, 0, dims, NPDT[dtype])
+    plan = wz.Plan(dims, dtype, 1)
+    d_phi, d_b = torch.from_numpy(phi).cuda(), torch.from_numpy(b[None]).cuda()
+    phi128, b128 = phi.astype(np.complex128), b.astype(np.complex128)
+    tol_x = {"c128": 1e-10, "c64": 2e-5}[dtype]
+    tol_r = {"c128": 1e-8, "c64": 1e-4}[dtype]
+    for k in (1, 2, 5, 20, 100):
+        x, infos = plan.cg_solve(d_phi, d_b, m, g, 1.0, 1e-30, k, raise_on_fail=False)
+        if dtype == "c128":
+            xo, io = orc.cg(phi128, b128, m, g, 1.0, 1e-30, k)
+        else:
+            xo, io = orc.cg_c64ru(phi128, b128, m, g, 1.0, 1e-30, k)
+        dx = rel(x.cpu().numpy()[0], xo)
+        dr = abs(infos[0].rel_residual_recursive - io.rel_residual_recursive) / io.rel_residual_recursive
+        print("%s k=%d: |x_gpu - x_oracle|/|x_oracle| = %.2e, recursive residual gpu %.6e oracle %.6e (rel diff %.1e), RU %d/%d"
+              % (name, k, dx, infos[0].rel_residual_recursive, io.rel_residual_recursive, dr,
+                 infos[0].reliable_updates, io.reliable_updates))
+        assert infos[0].iterations == io.iterations == k
+        if k <= 20:
+            scale = 1.0 if k <= 5 else 10.0  # rounding differences grow with k (complex64: one float ulp per update)
+            assert dx <= tol_x * scale, (k, dx)
+            assert dr <= tol_r * scale, (k, dr)
+            assert infos[0].reliable_updates == io.reliable_updates
+        else:
+            assert dx <= 0.05 and dr <= 1.0, (k, dx, dr)
+
+
+def test_cg_complex64_config3_all_sources(wz, orc, inp):
+    """Config 3 as BASELINE.json states it: 16^4 complex64, four sources solved to 1e-6.  complex64 vectors +
+    reliable updates (G9): bind on the true residual (recomputed by the oracle); every source's iteration
+    count is compared with the oracle's O4' loop on the same source (G10: 5 %, +-2 is not expected) and
+    must not be below the complex128 count by more than rounding noise."""
     cfg = inp.CONFIGS[3]
-    (info, true_res, phi, b), = _solve_and_check(wz, orc, inp, cfg, nsrc=1)
-    Xo, io = orc.cg_c64ru(phi, b, cfg["m"], cfg["g"], cfg["rho"], cfg["tol"], 50000)
-    print("config 3 source 0: iters gpu=%d oracle(O4')=%d  RU gpu=%d oracle=%d  true residual %.3e"
-          % (info.iterations, io.iterations, info.reliable_updates, io.reliable_updates, true_res))
-    assert io.converged
-    assert info.reliable_updates >= 1
-    assert abs(info.iterations - io.iterations) <= 0.05 * io.iterations
+    res = _solve_and_check(wz, orc, inp, cfg)
+    assert len(res) == 4
+    for j, (info, true_res, phi, b) in enumerate(res):
+        Xo, io = orc.cg_c64ru(phi, b, cfg["m"], cfg["g"], cfg["rho"], cfg["tol"], 50000)
+        print("config 3 source %d: iters gpu=%d oracle(O4')=%d delta=%+d  RU gpu=%d oracle=%d  true residual %.3e"
+              % (j, info.iterations, io.iterations, info.iterations - io.iterations, info.reliable_updates,
+                 io.reliable_updates, true_res))
+        assert io.converged
+        assert info.reliable_updates >= 1
+        assert abs(info.iterations - io.iterations) <= 0.05 * io.iterations
+    # one source also against the complex128 loop: fewer iterations than exact-arithmetic-like CG would be a red flag
+    info, _, phi, b = res[0]
+    _, i128 = orc.cg(phi, b, cfg["m"], cfg["g"], cfg["rho"], cfg["tol"], 50000)
+    print("config 3 source 0: complex128 oracle %d iterations" % i128.iterations)
+    assert info.iterations >= 0.97 * i128.iterations
 
 
 def test_cg_batch_of_sources_c64(wz, orc, inp):
@@ -160,7 +243,14 @@ def test_cg_batch_of_sources_c64(wz, orc, inp):
     cfg.update(dims=(8, 8, 8, 8), nsrc=3, m=0.05)
     res = _solve_and_check(wz, orc, inp, cfg)
     its = [r[0].iterations for r in res]
-    assert len(set(its)) >= 1 and min(its) > 10
+    # each source of the batch against a single-source solve of the same right-hand side
+    dims = cfg["dims"]
+    phi = torch.from_numpy(inp.make_phi(cfg["seed"], dims, cfg["sigma"], np.complex64)).cuda()
+    b = torch.from_numpy(inp.make_sources(cfg["seed"], 3, dims, np.complex64)).cuda()
+    plan = wz.Plan(dims, "c64", 1)
+    for j in range(3):
+        _, i1 = plan.cg_solve(phi, b[j:j + 1].contiguous(), cfg["m"], cfg["g"], cfg["rho"], cfg["tol"], 50000)
+        assert i1[0].iterations == its[j] and min(its) > 10
 
 
 def test_cg_max_iter_and_zero_source(wz, inp):
@@ -583,36 +673,212 @@ def test_mixed_precision_solve_to_double_tolerance(wz, orc, inp, dims):
     assert rel(x, xd) <= 1e-8 and rel(x, Xo) <= 1e-8
 
 
-def test_launch_order_knobs_do_not_change_results(wz):
-    """Prefetch distance, sweep direction and CTA order only permute or hint:
-    CTA work and reduction slots are indexed by tile, so a solve is bit-identical with all of them off."""
-    import hashlib
+# ---- the NEXT kernels in the launch configuration bench.py times (32^4 complex64: P23_MULTPC, fwdcg_s / endcg_s
+#      with the (x2,x3) volume compiled in) against the oracle (Tables VI, VII) ----
+
+def test_pc_and_shifted_solves_at_32x4_vs_oracle(wz, orc, inp):
+    dims = (32, 32, 32, 32)
+    phi = inp.make_phi(4, dims, 0.5, np.complex64)
+    b = inp.make_sources(4, 1, dims, np.complex64)
+    plan = wz.Plan(dims, "c64", 1)
+    d_phi, d_b = torch.from_numpy(phi).cuda(), torch.from_numpy(b).cuda()
+    phi128, b128 = phi.astype(np.complex128), b[0].astype(np.complex128)
+    tol = 1e-6
+    # Table VI parameters: 8 iterations in single precision (tests/golden/table_VI_pc_iterations.txt)
+    x, infos = plan.cg_solve(d_phi, d_b, 1.0, 0.2, 1.0, tol, 500, precondition=True)
+    xo, io = orc.cg_pc(phi128, b128, 1.0, 0.2, 1.0, tol, 500)
+    print("32^4 pc: iterations gpu=%d oracle=%d, true residual gpu %.2e oracle %.2e"
+          % (infos[0].iterations, io.iterations, infos[0].rel_residual_true, io.rel_residual_true))
+    assert infos[0].converged and io.converged and abs(infos[0].iterations - io.iterations) <= 2
+    assert 6 <= infos[0].iterations <= 10
+    assert rel(x.cpu().numpy()[0], xo) <= 1e-4
+    # Table VII parameters (m = 1, g = 0.1): Eq. 7.14 below the cutoff, Eq. 7.13 above it
+    for sigma, pc in ((0.5, True), (20.0, True), (300.0, False)):
+        x, infos = plan.cg_solve(d_phi, d_b, 1.0, 0.1, 1.0, tol, 2000, precondition=pc, sigma=sigma)
+        if pc:
+            xo, io = orc.cg_shift_pc(phi128, b128, 1.0, 0.1, sigma, 1.0, tol, 2000)
+        else:
+            xo, io = orc.cg_c64ru(phi128, b128, 1.0, 0.1, 1.0, tol, 2000, sigma=sigma)
+        xg = x.cpu().numpy()[0]
+        true_res = rel(orc.apply_MdagM(phi128, xg, 1.0, 0.1, 1.0) + sigma * xg, b128)
+        print("32^4 sigma=%g pc=%d: iterations gpu=%d oracle=%d true residual %.2e"
+              % (sigma, pc, infos[0].iterations, io.iterations, true_res))
+        assert infos[0].converged and io.converged
+        assert abs(infos[0].iterations - io.iterations) <= max(2, io.iterations // 20)
+        assert infos[0].iterations < 100  # under 100 iterations per problem in single precision
+        assert abs(true_res - infos[0].rel_residual_true) <= 0.05 * max(true_res, tol)
+        assert true_res <= (20 * tol if pc else tol * (1 + 1e-3))
+        assert rel(xg, xo) <= 1e-4
+
+
+@pytest.mark.parametrize("dims", [(32, 8, 8, 8), (32, 16, 16, 16)])
+@pytest.mark.parametrize("dtype,tol,want", [("c64", 1e-6, 8), ("c128", 1e-12, 15)])
+def test_paper_lattices_table_VI(wz, orc, inp, dims, dtype, tol, want):
+    """The paper's own lattices 8^3x32 and 16^3x32 at Table VI's parameters (m = 1, g = 1/5, Gaussian b;
+    PAPER.md:935-944): the preconditioned solve takes the 8 (single) / 15 (double) iterations the paper
+    prints (tests/golden/table_VI_pc_iterations.txt), the plain solve is compared with the oracle's."""
+    m, g, rho = 1.0, 0.2, 1.0
+    phi = inp.make_phi(5, dims, 0.5, NPDT[dtype])
+    b = inp.make_sources(5, 1, dims, NPDT[dtype])
+    plan = wz.Plan(dims, dtype, 1)
+    d_phi, d_b = torch.from_numpy(phi).cuda(), torch.from_numpy(b).cuda()
+    phi128, b128 = phi.astype(np.complex128), b[0].astype(np.complex128)
+    x, infos = plan.cg_solve(d_phi, d_b, m, g, rho, tol, 2000, precondition=True)
+    xo, io = orc.cg_pc(phi128, b128, m, g, rho, tol, 2000)
+    print("%s %s pc: iterations gpu=%d oracle=%d (Table VI: %d)" % (dims, dtype, infos[0].iterations, io.iterations, want))
+    assert infos[0].converged and abs(infos[0].iterations - io.iterations) <= 2
+    assert abs(infos[0].iterations - want) <= 1
+    assert rel(x.cpu().numpy()[0], xo) <= (1e-9 if dtype == "c128" else 1e-4)
+    # plain solve: the paper needed 830-1800 iterations at these parameters with its phi ensemble
+    x, infos = plan.cg_solve(d_phi, d_b, m, g, rho, tol, 20000)
+    if dtype == "c128":
+        xo, io = orc.cg(phi128, b128, m, g, rho, tol, 20000)
+    else:
+        xo, io = orc.cg_c64ru(phi128, b128, m, g, rho, tol, 20000)
+    xg = x.cpu().numpy()[0]
+    true_res = rel(orc.apply_MdagM(phi128, xg, m, g, rho), b128)
+    print("%s %s plain: iterations gpu=%d oracle=%d true residual %.2e" % (dims, dtype, infos[0].iterations, io.iterations, true_res))
+    assert infos[0].converged and true_res <= tol * (1 + 1e-3)
+    assert abs(infos[0].iterations - io.iterations) <= max(2, int(0.05 * io.iterations))
+
+
+def test_paper_lattice_32x3x64_MdagM(wz, orc, inp):
+    """32^3x64, the largest lattice of Tables V-VII: one M^dag M in both precisions against the oracle."""
+    dims = (64, 32, 32, 32)
+    for dtype in ("c64", "c128"):
+        phi = inp.make_phi(5, dims, 0.5, NPDT[dtype])
+        b = inp.make_source(5, 0, dims, NPDT[dtype])
+        plan = wz.Plan(dims, dtype, 1)
+        out = plan.apply_MdagM(torch.from_numpy(phi).cuda(), torch.from_numpy(b).cuda(), 1.0, 0.2, 1.0).cpu().numpy()
+        del plan
+        ref = orc.apply_MdagM(phi.astype(np.complex128), b.astype(np.complex128), 1.0, 0.2, 1.0)
+        assert rel(out, ref) <= TOL[dtype]
+
+
+# ---- config 4 source 0 against the oracle's full solve (SURVEY 8(d) "Oracle timed beside it") ----
+
+def _read_golden_solve(name):
     import os
-    import subprocess
-    import sys
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", name)
+    vals, hist = {}, []
+    with open(path) as f:
+        for line in f:
+            if line.startswith("#") or not line.strip():
+                continue
+            w = line.split()
+            if w[0] == "history":
+                hist.append((int(w[1]), float(w[2])))
+            else:
+                vals[w[0]] = float(w[1])
+    return vals, hist
 
-    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
-    code = (
-        "import hashlib, torch\n"
-        "from paper_1005_3276_b200 import inputs, wz\n"
-        "dims = (32, 32, 32, 32)\n"
-        "phi = torch.from_numpy(inputs.make_phi(11, dims, 0.5, 'complex64')).cuda()\n"
-        "b = torch.from_numpy(inputs.make_sources(11, 2, dims, 'complex64')).cuda()\n"
-        "plan = wz.Plan(dims, 'c64', 2)\n"
-        "x, info = plan.cg_solve(phi, b, 0.01, 1.5, 1.0, 1e-6, 60, raise_on_fail=False)\n"
-        "q = plan.apply_MdagM(phi, b, 0.01, 1.5, 1.0)\n"
-        "h = hashlib.sha256(x.cpu().numpy().tobytes() + q.cpu().numpy().tobytes()).hexdigest()\n"
-        "print('DIGEST', h, info[0].iterations, info[0].rel_residual_true)\n"
-    )
 
-    def run(env_extra):
-        env = dict(os.environ)
-        env.update(env_extra)
-        out = subprocess.run([sys.executable, "-c", code], cwd=root, env=env, capture_output=True, text=True, timeout=600)
-        assert out.returncode == 0, out.stderr[-2000:]
-        return [l for l in out.stdout.splitlines() if l.startswith("DIGEST")][0]
+def test_config4_source0_vs_oracle_full_solve(wz, inp):
+    """The headline workload's iteration count and residual history against the oracle's O4' loop run to
+    convergence on the same source (tests/golden/config4_src0_oracle.txt, written by
+    tests/golden/make_config4_src0.py from oracle/ alone): count within 5 % (G10), and the GPU's residual
+    history lies on the oracle's convergence curve."""
+    vals, hist = _read_golden_solve("config4_src0_oracle.txt")
+    assert vals["converged"] == 1 and vals["rel_residual_true"] <= 1e-6
+    cfg = inp.CONFIGS[4]
+    dims = cfg["dims"]
+    phi = inp.make_phi(cfg["seed"], dims, cfg["sigma"], np.complex64)
+    b = inp.make_sources(cfg["seed"], 1, dims, np.complex64)
+    plan = wz.Plan(dims, "c64", 1)
+    x, infos = plan.cg_solve(torch.from_numpy(phi).cuda(), torch.from_numpy(b).cuda(), cfg["m"], cfg["g"], cfg["rho"],
+                             cfg["tol"], 100000)
+    info = infos[0]
+    n_or = int(vals["iterations"])
+    print("config 4 source 0: iterations gpu=%d oracle=%d (%+.2f %%), reliable updates gpu=%d oracle=%d"
+          % (info.iterations, n_or, 100.0 * (info.iterations - n_or) / n_or, info.reliable_updates,
+             int(vals["reliable_updates"])))
+    assert info.converged and info.rel_residual_true <= cfg["tol"]
+    assert abs(info.iterations - n_or) <= 0.05 * n_or
+    assert abs(info.reliable_updates - vals["reliable_updates"]) <= 3
+    # history shape: at the iterations the host sampled, log10 of the residual against the oracle's curve
+    # (interpolated in log space between its stored points); both oscillate by +-30 % per iteration, and the
+    # curves shift against each other by the few per cent the counts differ
+    ks = np.array([k for k, _ in hist], dtype=np.float64)
+    lr = np.log10(np.array([r for _, r in hist]))
+    gh = plan.cg_history(0)
+    assert len(gh) > 100
+    dev = []
+    for k, r in gh:
+        if k < 50 or k > 0.9 * min(info.iterations, n_or) or r <= 0:
+            continue
+        dev.append(abs(np.log10(r) - np.interp(k, ks, lr)))
+    dev = np.array(dev)
+    print("history: %d samples, median |dlog10| %.3f, max %.3f" % (len(dev), np.median(dev), dev.max()))
+    assert np.median(dev) <= 0.15 and dev.max() <= 0.6
 
-    on = run({})
-    off = run({"WZ_PFA": "0", "WZ_SWEEP": "0", "WZ_COMPFAST": "0"})
-    alt = run({"WZ_PFA": "150", "WZ_SWEEP": "1", "WZ_COMPFAST": "7"})
-    assert on == off == alt, (on, off, alt)
+
+# ---- CUDA graph replay of the iteration chunks (north star iii) and host-side argument checks ----
+
+@pytest.mark.parametrize("dims,dtype", [((8, 8, 8, 8), "c128"), ((16, 16, 16, 16), "c64")])
+def test_graph_replay_equals_stream_launches(wz, inp, dims, dtype):
+    phi = torch.from_numpy(inp.make_phi(3, dims, 0.5, NPDT[dtype])).cuda()
+    b = torch.from_numpy(inp.make_sources(3, 2, dims, NPDT[dtype])).cuda()
+    plan = wz.Plan(dims, dtype, 2)
+    tol = 1e-10 if dtype == "c128" else 1e-6
+    res = {}
+    for on in (True, False, True):
+        plan.set_graph(on)
+        plan.reset_launch_count()
+        x, infos = plan.cg_solve(phi, b, 0.05, 1.0, 1.0, tol, 100000)
+        res.setdefault(on, []).append((x.clone(), [(i.iterations, i.reliable_updates, i.rel_residual_true) for i in infos],
+                                       plan.launch_count))
+    (xg, ig, lg), (xg2, ig2, lg2) = res[True]
+    (xs, is_, ls), = res[False]
+    assert ig == is_ == ig2 and torch.equal(xg, xs) and torch.equal(xg, xg2)
+    assert lg == ls == lg2 and lg >= 5 * max(i[0] for i in ig)  # replayed launches are counted
+    # other arguments -> a new capture, same results as stream launches
+    plan.set_graph(True)
+    xa, ia = plan.cg_solve(phi, b, 0.05, 1.0, 1.0, tol, 100000, sigma=0.5)
+    plan.set_graph(False)
+    xb, ib = plan.cg_solve(phi, b, 0.05, 1.0, 1.0, tol, 100000, sigma=0.5)
+    assert torch.equal(xa, xb) and [i.iterations for i in ia] == [i.iterations for i in ib]
+    h = plan.cg_history(1)
+    assert h[0][0] > 0 and h[-1][0] == ib[1].iterations and h[-1][1] <= tol * 1.01
+    assert all(h[i][0] < h[i + 1][0] for i in range(len(h) - 1))
+
+
+def test_binding_rejects_mismatched_buffers(wz, inp):
+    dims = (4, 4, 4, 4)
+    plan = wz.Plan(dims, "c128", 3)
+    phi = torch.from_numpy(inp.make_phi(1, dims, 0.3)).cuda()
+    b3 = torch.from_numpy(inp.make_sources(1, 3, dims)).cuda()
+    one = torch.empty_like(b3[0])
+    with pytest.raises(ValueError):
+        plan.fft4d(b3, +1, True, out=one)  # three spinors in, room for one out
+    with pytest.raises(ValueError):
+        plan.apply_M(phi, b3, 0.1, 0.5, 1.0, False, out=one)
+    with pytest.raises(ValueError):
+        plan.cg_solve(phi, b3, 0.1, 0.5, out=torch.empty_like(one))
+    with pytest.raises(ValueError):
+        plan.fft4d(b3.cpu(), +1, True)
+    b1 = b3[:1].contiguous()
+    with pytest.raises(wz.WZError) as e:  # x must not alias b
+        plan.cg_solve(phi, b1, 0.1, 0.5, out=b1)
+    assert e.value.status == wz.WZ_EINVAL
+    with pytest.raises(wz.WZError) as e:
+        plan.rational_apply(phi, b1, 0.1, 0.5, 0.0, [1.0], [1.0], out=b1)
+    assert e.value.status == wz.WZ_EINVAL
+
+
+def test_second_device(wz, orc, inp):
+    """A plan on cuda:1 in a process that already used cuda:0 (the twiddle tables are per-device constant
+    memory): FFT and M^dag M against the oracle.  Needs two GPUs."""
+    if torch.cuda.device_count() < 2:
+        pytest.skip("one GPU")
+    dims = (8, 8, 8, 8)
+    phi, b = _fields(inp, dims, "c128")
+    wz.Plan(dims, "c128", 1, "cuda:0").fft4d(torch.from_numpy(b).to("cuda:0"), +1, True)
+    plan = wz.Plan(dims, "c128", 1, "cuda:1")
+    d_b, d_phi = torch.from_numpy(b).to("cuda:1"), torch.from_numpy(phi).to("cuda:1")
+    assert torch.cuda.current_device() == 0
+    f = plan.fft4d(d_b, +1, True).cpu().numpy()
+    assert rel(f, orc.dft4d(b[0], +1, True)[None]) <= 1e-12
+    q = plan.apply_MdagM(d_phi, d_b, 0.05, 1.0, 1.0).cpu().numpy()
+    assert rel(q[0], orc.apply_MdagM(phi, b[0], 0.05, 1.0, 1.0)) <= 1e-12
+    with pytest.raises(ValueError):
+        plan.fft4d(torch.from_numpy(b).to("cuda:0"), +1, True)
