@@ -175,6 +175,12 @@ wz_status wz_locality_profile(wz_plan *plan, double rho, int spin, double *f_hos
  * one by one instead (results are bit-identical; for measurements).  Default: 1. */
 wz_status wz_plan_set_graph(wz_plan *plan, int enable);
 
+/* Sources per block of a batched solve.  The sources of a batch are independent solves (one CG state, one
+ * set of reductions each): they advance block by block, each block running its 8 iterations between two
+ * convergence checks back to back, so that a block's vectors stay in the L2 cache from one pass to the next.
+ * 0 = the whole batch in lock step through shared launches.  Results do not depend on it, bit for bit. */
+wz_status wz_plan_set_block(wz_plan *plan, int sources_per_block);
+
 /* Residual history of the LAST solve on this plan, as the host saw it at its convergence checks (every 8
  * iterations, one chunk behind the GPU): for `source`, pairs (iteration k, ||r_k|| / ||b||) with the
  * recursive residual (PAPER.md:944 stop rule), the recomputed one right after a reliable update.

@@ -859,4 +859,92 @@ int orc_cg_shift_pc(int method, const int* L, const double* phi, const double* b
   return 0;
 }
 
+// ----------------------------------------------------------------------------
+// O8 (NEXT-2, third step). Multi-shift CG: all systems (M^dag M + sigma_i) X_i = b,
+// i = 1..d (Eq. 7.6-7.7; 927-931 Eq. 7.13), from ONE Krylov space.
+// Not in the paper (it solves one shift at a time); SURVEY 8(f) NEXT-2 asks
+// for it.  Textbook algorithm (B. Jegerlehner, hep-lat/9612014, restated in the usual CG
+// notation): run CG on A = M^dag M itself,
+//   r_0 = p_0 = b;  alpha_n = <r_n,r_n>/<p_n, A p_n>;  r_{n+1} = r_n - alpha_n A p_n;
+//   beta_n = <r_{n+1},r_{n+1}>/<r_n,r_n>;  p_{n+1} = r_{n+1} + beta_n p_n,
+// and use that the residual of the CG iteration for A + sigma started from the same b is
+// collinear with r_n:  r^sigma_n = zeta^sigma_n r_n,  zeta_{-1} = zeta_0 = 1, with (alpha_{-1} = 1, beta_{-1} = 0)
+//   zeta_{n+1} = zeta_n zeta_{n-1} alpha_{n-1} /
+//                ( alpha_n beta_{n-1} (zeta_{n-1} - zeta_n) + zeta_{n-1} alpha_{n-1} (1 + sigma alpha_n) ),
+//   alpha^sigma_n = alpha_n zeta_{n+1}/zeta_n,   beta^sigma_n = beta_n (zeta_{n+1}/zeta_n)^2,
+//   x^sigma_{n+1} = x^sigma_n + alpha^sigma_n p^sigma_n,   p^sigma_{n+1} = zeta_{n+1} r_{n+1} + beta^sigma_n p^sigma_n.
+// Stop rule per shift (reading G8 applied to each system): frozen once |zeta_n| ||r_n|| <= tol ||b||;
+// the loop ends when every shift is frozen.  info[i].iterations = the iteration at which shift i froze
+// (= the number of M^dag M applications it took part in).  True residuals recomputed at exit.
+// ----------------------------------------------------------------------------
+int orc_cg_multishift(int method, const int* L, const double* phi, const double* b_, int nshift,
+                      const double* sigmas, double* X_ /* [nshift][4V] complex128 */,
+                      const double* m, const double* g, double rho, double tol, int max_iter,
+                      orc_cg_info* info /* [nshift] */, int* matvecs) {
+  const long V = (long)L[0] * L[1] * L[2] * L[3];
+  const long n = 4 * V;
+  const cd* b = reinterpret_cast<const cd*>(b_);
+  cd* X = reinterpret_cast<cd*>(X_);
+  std::vector<cd> r(b, b + n), p(b, b + n), q(n);
+  std::vector<std::vector<cd>> ps(nshift, std::vector<cd>(b, b + n));
+  std::vector<double> zeta(nshift, 1.0), zeta_prev(nshift, 1.0);
+  std::vector<int> frozen(nshift, 0), its(nshift, 0);
+  std::vector<double> rec(nshift, 1.0);  // |zeta| ||r|| / ||b|| of each shift at its last update
+  for (long i = 0; i < (long)nshift * n; ++i) X[i] = 0.0;
+  const double bnorm = std::sqrt(dot_re(b, b, n));
+  double rr = bnorm * bnorm;
+  double alpha_prev = 1.0, beta_prev = 0.0;
+  int k = 0, nfrozen = 0;
+  if (bnorm == 0.0) {
+    for (int i = 0; i < nshift; ++i) frozen[i] = 1;
+    nfrozen = nshift;
+  }
+  while (nfrozen < nshift && k < max_iter) {
+    ++k;
+    int rc = orc_apply_MdagM(method, L, phi, m, g, rho, reinterpret_cast<double*>(p.data()),
+                             reinterpret_cast<double*>(q.data()));
+    if (rc) return rc;
+    const double alpha = rr / dot_re(p.data(), q.data(), n);
+    for (long j = 0; j < n; ++j) r[j] -= alpha * q[j];
+    const double rr_new = dot_re(r.data(), r.data(), n);
+    const double beta = rr_new / rr;
+    for (int i = 0; i < nshift; ++i) {
+      if (frozen[i]) continue;
+      const double zn = zeta[i], zp = zeta_prev[i];
+      const double znew = zn * zp * alpha_prev /
+                          (alpha * beta_prev * (zp - zn) + zp * alpha_prev * (1.0 + sigmas[i] * alpha));
+      const double alpha_s = alpha * znew / zn;
+      const double beta_s = beta * (znew / zn) * (znew / zn);
+      cd* x = X + (long)i * n;
+      std::vector<cd>& pi = ps[i];
+      for (long j = 0; j < n; ++j) {
+        x[j] += alpha_s * pi[j];
+        pi[j] = znew * r[j] + beta_s * pi[j];
+      }
+      zeta_prev[i] = zn;
+      zeta[i] = znew;
+      its[i] = k;
+      rec[i] = std::fabs(znew) * std::sqrt(rr_new) / bnorm;
+      if (std::fabs(znew) * std::sqrt(rr_new) <= tol * bnorm) { frozen[i] = 1; ++nfrozen; }
+    }
+    for (long j = 0; j < n; ++j) p[j] = r[j] + beta * p[j];
+    alpha_prev = alpha;
+    beta_prev = beta;
+    rr = rr_new;
+  }
+  for (int i = 0; i < nshift; ++i) {
+    cd* x = X + (long)i * n;
+    orc_apply_MdagM(method, L, phi, m, g, rho, reinterpret_cast<double*>(x), reinterpret_cast<double*>(q.data()));
+    double tr = 0.0;
+    for (long j = 0; j < n; ++j) tr += std::norm(b[j] - q[j] - sigmas[i] * x[j]);
+    info[i].iterations = its[i];
+    info[i].reliable_updates = 0;
+    info[i].converged = frozen[i];
+    info[i].rel_residual_recursive = bnorm > 0 ? rec[i] : 0.0;
+    info[i].rel_residual_true = bnorm > 0 ? std::sqrt(tr) / bnorm : 0.0;
+  }
+  if (matvecs) *matvecs = k;
+  return 0;
+}
+
 }  // extern "C"

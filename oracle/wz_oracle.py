@@ -305,3 +305,24 @@ def rational_apply(phi, eta, m, g, alpha0, alphas, betas, rho=1.0, tol=1e-10, ma
         out = out + a_i * X
         infos.append(info)
     return out, infos
+
+
+def cg_multishift(phi, b, m, g, sigmas, rho=1.0, tol=1e-10, max_iter=100000, method="auto"):
+    """Multi-shift CG (oracle O8): all (M^dag M + sigma_i) X_i = b from one Krylov space, complex128.
+    Returns (X[nshift, 4, T, L1, L2, L3], [CGInfo per shift], matvecs)."""
+    phi = np.ascontiguousarray(phi, dtype=np.complex128)
+    b = np.ascontiguousarray(b, dtype=np.complex128)
+    sig = np.ascontiguousarray(sigmas, dtype=np.float64)
+    d = int(sig.size)
+    dims = phi.shape
+    X = np.zeros((d,) + b.shape, dtype=np.complex128)
+    infos = (_Info * max(d, 1))()
+    mv = ctypes.c_int(0)
+    rc = lib().orc_cg_multishift(_method(dims, method), _dims(dims), _dp(phi), _dp(b), d, _dp(sig), _dp(X),
+                                 _c2(m), _c2(g), ctypes.c_double(rho), ctypes.c_double(tol), int(max_iter),
+                                 infos, ctypes.byref(mv))
+    if rc:
+        raise ValueError("oracle cg_multishift failed")
+    out = [CGInfo(i.iterations, i.reliable_updates, bool(i.converged), i.rel_residual_recursive,
+                  i.rel_residual_true, np.zeros(0)) for i in infos[:d]]
+    return X, out, int(mv.value)

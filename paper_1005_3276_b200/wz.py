@@ -26,7 +26,7 @@ EXPORTS = [
     "wz_plan_profile", "wz_plan_profile_read", "wz_kind_name",
     "wz_apply_M0inv", "wz_apply_MtdagMt", "wz_cg_solve_pc", "wz_apply_Dslash", "wz_locality_profile",
     "wz_cg_solve_shift", "wz_cg_solve_shift_pc", "wz_rational_apply",
-    "wz_plan_set_graph", "wz_plan_cg_history",
+    "wz_plan_set_graph", "wz_plan_cg_history", "wz_plan_set_block",
 ]
 
 
@@ -90,6 +90,7 @@ def lib() -> ctypes.CDLL:
         L.wz_plan_profile.argtypes = [vp, ci]
         L.wz_plan_profile_read.argtypes = [vp, d2, ctypes.POINTER(ctypes.c_ulonglong)]
         L.wz_plan_set_graph.argtypes = [vp, ci]
+        L.wz_plan_set_block.argtypes = [vp, ci]
         L.wz_plan_cg_history.argtypes = [vp, ci, ctypes.POINTER(ci), d2, ci]
         L.wz_kind_name.restype = ctypes.c_char_p
         L.wz_kind_name.argtypes = [ci]
@@ -188,6 +189,10 @@ class Plan:
     def set_graph(self, enable: bool):
         """CUDA-graph replay of the iteration chunks on (default) or off (wz_plan_set_graph)."""
         _check(lib().wz_plan_set_graph(self._h, int(bool(enable))))
+
+    def set_block(self, sources_per_block: int):
+        """Sources per block of a batched solve (wz_plan_set_block); 0 = whole batch in lock step."""
+        _check(lib().wz_plan_set_block(self._h, int(sources_per_block)))
 
     def cg_history(self, source: int = 0):
         """[(iteration, ||r||/||b||)] of the last solve as the host saw it (wz_plan_cg_history)."""
