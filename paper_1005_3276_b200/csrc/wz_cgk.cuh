@@ -186,6 +186,122 @@ k_locality(const cpx<R>* __restrict__ psi, unsigned long long* __restrict__ f, i
   }
 }
 
+
+// ---- multi-shift CG (Eq. 7.6-7.7, 927-931 Eq. 7.13) ----------------
+// All systems (A + sigma_i) x_i = b from the Krylov space of ONE CG iteration (the base system, the smallest
+// shift): the residual of shift i stays collinear with the base residual, r_i = zeta_i r (B. Jegerlehner,
+// hep-lat/9612014).  Per base iteration n (alpha_n, beta_n the base CG coefficients, s_i = sigma_i - sigma_base):
+//   zeta_{n+1} = zeta_n zeta_{n-1} alpha_{n-1} / (alpha_n beta_{n-1} (zeta_{n-1} - zeta_n) + zeta_{n-1} alpha_{n-1} (1 + s_i alpha_n))
+//   x_i += alpha_n (zeta_{n+1}/zeta_n) p_i;   p_i = zeta_{n+1} r_{n+1} + beta_n (zeta_{n+1}/zeta_n)^2 p_i
+// A shift is frozen once |zeta| ||r|| <= tol ||b||.
+constexpr int WZ_MAX_SHIFTS = 32;
+struct MSState {  // per source
+  double zeta[WZ_MAX_SHIFTS], zeta_prev[WZ_MAX_SHIFTS];
+  double ax[WZ_MAX_SHIFTS];    // coefficient of p_i in this iteration's x_i update
+  double zr[WZ_MAX_SHIFTS];    // coefficient of r in this iteration's p_i update
+  double bp[WZ_MAX_SHIFTS];    // coefficient of p_i in this iteration's p_i update
+  double rec[WZ_MAX_SHIFTS];   // |zeta| ||r|| / ||b|| at the shift's last update
+  double srel[WZ_MAX_SHIFTS];  // sigma_i - sigma_base
+  double alpha_prev, beta_prev;
+  int upd[WZ_MAX_SHIFTS];      // 1: the vectors of shift i take part in this iteration's update
+  int frozen[WZ_MAX_SHIFTS];
+  int its[WZ_MAX_SHIFTS];      // base iteration of the shift's last update
+  int nshift, last_iter;
+};
+
+// One thread per source, after pass E' of the base iteration: the scalar recurrences.
+__global__ void k_ms_scalars(MSState* ms_, const CGState* st_) {
+  MSState* ms = ms_ + blockIdx.x;
+  const CGState* st = st_ + blockIdx.x;
+  const int i = threadIdx.x;
+  if (i >= ms->nshift) return;
+  const bool advanced = st->iter != ms->last_iter;  // the base took a step since the last call
+  int upd = 0;
+  if (advanced && !ms->frozen[i]) {
+    const double alpha = st->alpha, beta = st->beta;
+    const double zn = ms->zeta[i], zp = ms->zeta_prev[i];
+    const double znew = zn * zp * ms->alpha_prev /
+                        (alpha * ms->beta_prev * (zp - zn) + zp * ms->alpha_prev * (1.0 + ms->srel[i] * alpha));
+    const double ratio = znew / zn;
+    ms->ax[i] = alpha * ratio;
+    ms->zr[i] = znew;
+    ms->bp[i] = beta * ratio * ratio;
+    ms->zeta_prev[i] = zn;
+    ms->zeta[i] = znew;
+    ms->its[i] = st->iter;
+    const double rn = fabs(znew) * sqrt(st->rr);
+    ms->rec[i] = st->bnorm > 0.0 ? rn / st->bnorm : 0.0;
+    if (rn <= st->tol * st->bnorm) ms->frozen[i] = 1;
+    upd = 1;
+  }
+  ms->upd[i] = upd;
+  __syncthreads();
+  if (i == 0 && advanced) {
+    ms->alpha_prev = st->alpha;
+    ms->beta_prev = st->beta;
+    ms->last_iter = st->iter;
+  }
+}
+
+// x_i += ax_i p_i;  p_i = zr_i r + bp_i p_i  for every shift that takes part (upd), r read once per element.
+// Vectors: [shift][source][n] for ps and xsh; r: [source][n].  TX: storage type of the x_i.
+template <typename R, typename TX>
+__global__ void __launch_bounds__(CGK_NT)
+k_ms_update(const R* __restrict__ r, R* __restrict__ ps, TX* __restrict__ xsh, long n, int nb, int base,
+            const MSState* __restrict__ ms_) {
+  const int src = blockIdx.y;
+  const MSState* ms = ms_ + src;
+  __shared__ double s_ax[WZ_MAX_SHIFTS], s_zr[WZ_MAX_SHIFTS], s_bp[WZ_MAX_SHIFTS];
+  __shared__ int s_upd[WZ_MAX_SHIFTS];
+  const int ns = ms->nshift;
+  if (threadIdx.x < ns) {
+    s_ax[threadIdx.x] = ms->ax[threadIdx.x]; s_zr[threadIdx.x] = ms->zr[threadIdx.x];
+    s_bp[threadIdx.x] = ms->bp[threadIdx.x];
+    s_upd[threadIdx.x] = (threadIdx.x == base) ? 0 : ms->upd[threadIdx.x];  // the base system is advanced by passes A'/E'
+  }
+  __syncthreads();
+  bool any = false;
+  for (int i = 0; i < ns; ++i) any |= (s_upd[i] != 0);
+  if (!any) return;
+  r += src * n;
+  for (long e = ((long)blockIdx.x * blockDim.x + threadIdx.x) * 2; e < n; e += (long)gridDim.x * blockDim.x * 2) {
+    const R r0 = r[e], r1 = r[e + 1];
+    for (int i = 0; i < ns; ++i) {
+      if (!s_upd[i]) continue;
+      const size_t o = ((size_t)i * nb + src) * n + e;
+      const R p0 = ps[o], p1 = ps[o + 1];
+      xsh[o] = (TX)((double)xsh[o] + s_ax[i] * (double)p0);
+      xsh[o + 1] = (TX)((double)xsh[o + 1] + s_ax[i] * (double)p1);
+      ps[o] = (R)(s_zr[i] * (double)r0 + s_bp[i] * (double)p0);
+      ps[o + 1] = (R)(s_zr[i] * (double)r1 + s_bp[i] * (double)p1);
+    }
+  }
+}
+
+// ps_i = b, x_i = 0 for every shift (one source per grid row, all shifts).  TB: storage type of b.
+template <typename R, typename TX, typename TB>
+__global__ void __launch_bounds__(CGK_NT)
+k_ms_init(const TB* __restrict__ b, R* __restrict__ ps, TX* __restrict__ xsh, long n, int nb, int ns) {
+  const int src = blockIdx.y;
+  b += src * n;
+  for (long e = (long)blockIdx.x * blockDim.x + threadIdx.x; e < n; e += (long)gridDim.x * blockDim.x) {
+    const R v = (R)b[e];
+    for (int i = 0; i < ns; ++i) {
+      const size_t o = ((size_t)i * nb + src) * n + e;
+      ps[o] = v;
+      xsh[o] = TX(0);
+    }
+  }
+}
+
+// dst (double) = src (TX) element-wise, or dst += src
+template <typename TX>
+__global__ void __launch_bounds__(CGK_NT)
+k_to_double(double* __restrict__ dst, const TX* __restrict__ src, long n, int accumulate) {
+  for (long i = (long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long)gridDim.x * blockDim.x)
+    dst[i] = (accumulate ? dst[i] : 0.0) + (double)src[i];
+}
+
 // dst (double) = src (float), element-wise (phi for the complex128 operator of a
 // complex64 plan: the float-rounded values, exactly what the oracle consumes).
 __global__ void __launch_bounds__(CGK_NT)

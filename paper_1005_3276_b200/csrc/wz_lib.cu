@@ -257,10 +257,11 @@ wz_status setup_ws(wz_plan* pl, OpWS<R>& ws, int nbatch_t) {
     return WZ_ECUDA;
   const auto* b = ws.p23;
   if (!set_smem(b->fwd, b->smem) || !set_smem(b->inv, b->smem) || !set_smem(b->mult, b->smem) ||
-      !set_smem(b->multpc, b->smem_pc))
+      !set_smem(b->multpc, b->smem_pc) || (b->diagpc && !set_smem(b->diagpc, b->smem_pc)))
     return WZ_ECUDA;
   wave_ctas(pl, (const void*)b->mult, b->nt, b->smem);  // occupancy queries now, not inside a stream capture
   wave_ctas(pl, (const void*)b->multpc, b->nt, b->smem_pc);
+  if (b->diagpc) wave_ctas(pl, (const void*)b->diagpc, b->nt, b->smem_pc);
   wave_ctas(pl, (const void*)b->fwd, b->nt, b->smem);
   wave_ctas(pl, (const void*)b->inv, b->nt, b->smem);
   std::vector<R> h(2 * 4 * 64, R(0));
@@ -364,6 +365,8 @@ wz_status mult_pass(wz_plan* pl, OpWS<R>& ws, P23Args<R>& b, cpx<R>*& cur, int n
   cpx<R>* dst = (ws.p23->nhalf == 2) ? ((cur == t) ? t2 : t) : cur;
   b.in = cur; b.out = dst;
   wz_status s = launch_p23<R>(pl, WZ_K_P23_MULT, *ws.p23, b.pc ? ws.p23->multpc : ws.p23->mult, b, nb);
+  // two components per CTA: the diagonal term of M0^-1 needs the pair the CTA does not hold -> second launch
+  if (s == WZ_OK && b.pc && ws.p23->diagpc) s = launch_p23<R>(pl, WZ_K_P23_MULT, *ws.p23, ws.p23->diagpc, b, nb);
   cur = dst;
   return s;
 }
