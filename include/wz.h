@@ -159,6 +159,31 @@ wz_status wz_rational_apply(wz_plan *plan, const void *phi, const void *eta, voi
                             const double *alphas, const double *betas, int nshift, double pc_cutoff,
                             double tol, int max_iter, int nbatch, wz_cg_info *info);
 
+/* ---- Multi-shift CG (Eq. 7.6-7.7, 927-931 Eq. 7.13) ----
+ * The paper solves the d = 20 systems (M^dag M + beta_i) X_i = eta one at a time.  They share
+ * one Krylov space: wz_cg_solve_multishift solves all of them in the iterations of the hardest one (B.
+ * Jegerlehner, hep-lat/9612014): CG runs on the system with the smallest shift, the residuals of the others
+ * stay collinear with its residual, r_i = zeta_i r, and two site-local updates per shift carry x_i and p_i along.
+ *  - sigmas: HOST array of nshift >= 1 shifts, each >= 0, nshift <= 32.
+ *  - b: nbatch spinors of the plan's dtype;  x: nshift * nbatch spinors, [shift][source], ALWAYS complex128.
+ *  - info: HOST array [shift][source].  iterations = the iteration at which that shift met
+ *    |zeta_i| ||r|| <= tol ||b|| (its updates stop there).  WZ_C64 plans iterate in complex64 WITHOUT reliable
+ *    updates (a recomputed residual would break the collinearity) and then polish every shift whose true
+ *    residual, recomputed in complex128, is above tol: the defect is solved for by wz_cg_solve_shift's loop and
+ *    added; iterations then includes the polishing iterations, reliable_updates counts theirs.
+ *    rel_residual_true = ||b - (M^dag M + sigma_i) x_i|| / ||b|| recomputed at exit.
+ * Synchronises the stream.  WZ_ENOTCONVERGED if any system hit max_iter.
+ * wz_rational_apply_multishift: wz_rational_apply with every shift above pc_cutoff (all shifts if pc_cutoff < 0
+ *   or m = 0) taken from ONE multi-shift solve; shifts up to pc_cutoff keep the paper's preconditioned solves. */
+wz_status wz_cg_solve_multishift(wz_plan *plan, const void *phi, const void *b, void *x,
+                                 const double m[2], const double g[2], double rho,
+                                 const double *sigmas, int nshift, double tol, int max_iter, int nbatch,
+                                 wz_cg_info *info);
+wz_status wz_rational_apply_multishift(wz_plan *plan, const void *phi, const void *eta, void *out,
+                                       const double m[2], const double g[2], double rho, double alpha0,
+                                       const double *alphas, const double *betas, int nshift, double pc_cutoff,
+                                       double tol, int max_iter, int nbatch, wz_cg_info *info);
+
 /* ---- Locality probe (Eq. 3.9-3.11, Fig. 1) ----
  * wz_apply_Dslash: out = Dslash in = (1 - D2/2)^-1 D1 in (the fermion matrix at m = g = 0); in != out.
  * wz_locality_profile: psi = Dslash eta for a unit point source at the origin in spin component

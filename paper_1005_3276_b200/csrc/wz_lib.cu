@@ -140,7 +140,15 @@ struct wz_plan {
   cpx<double>* q128 = nullptr;    // A X in complex128 (reliable updates, true residual), one spinor
   cpx<double>* phi128 = nullptr;  // C64 plans: phi widened
   cpx<double>* btilde128 = nullptr;  // C64 plans, preconditioned solves: (M0^-1)^dag b in complex128, per source
-  cpx<double>* ratX = nullptr;       // wz_rational_apply: the X_i of the current shift, max_batch spinors
+  cpx<double>* ratX = nullptr;       // wz_rational_apply: the X_i of the current shift(s), ratX_cap spinors
+  size_t ratX_cap = 0;
+  // multi-shift CG: search directions and (complex64 plans) solutions of every shift, [shift][source] spinors
+  void *ms_p = nullptr, *ms_x = nullptr;
+  size_t ms_cap = 0;               // spinors each of ms_p / ms_x holds
+  MSState* ms_state = nullptr;     // [max_batch]
+  double* ms_true = nullptr;       // [WZ_MAX_SHIFTS][max_batch] true residual norms squared
+  void* ms_rhs = nullptr;          // complex64 plans: defect of one shift, max_batch spinors (plan dtype)
+  cpx<double>* ms_e = nullptr;     // complex64 plans: correction of the polishing solve, max_batch spinors
   double* partials = nullptr;
   unsigned* counter = nullptr;
   CGState* d_state = nullptr;
@@ -811,7 +819,8 @@ int vec_grid(long n_real, int per_thread) {
 template <typename R>
 wz_status cg_batch(wz_plan* pl, const cpx<R>* phi, const cpx<R>* b, cpx<double>* X, const double m[2],
                    const double g[2], double rho, double tol, int max_iter, int nb, wz_cg_info* info,
-                   bool pc, double sigma = 0.0) {
+                   bool pc, double sigma = 0.0, const double* tol_per_source = nullptr) {
+  // tol_per_source (optional, nb entries): overrides tol source by source (defect-correction solves)
   // sigma: shift of the system (M^dag M + sigma) x = b (Eq. 7.13); with pc the system
   // iterated on is Eq. 7.14, (Mtilde^dag Mtilde + sigma (M0^-1)^dag M0^-1) xtilde = btilde
   constexpr bool kRU = (sizeof(R) == 4);
@@ -826,7 +835,7 @@ wz_status cg_batch(wz_plan* pl, const cpx<R>* phi, const cpx<R>* b, cpx<double>*
   std::vector<CGState> h(nb);
   memset(h.data(), 0, sizeof(CGState) * nb);
   for (int j = 0; j < nb; ++j) {
-    h[j].tol = tol; h[j].delta = kDelta; h[j].max_iter = max_iter; h[j].use_ru = kRU ? 1 : 0;
+    h[j].tol = tol_per_source ? tol_per_source[j] : tol; h[j].delta = kDelta; h[j].max_iter = max_iter; h[j].use_ru = kRU ? 1 : 0;
     h[j].true_rr = -1.0; h[j].shift = pc ? 0.0 : sigma;  // pc: the shift is inside pass C's reduction
     if (max_iter == 0) h[j].stop = 1;
   }
@@ -1055,6 +1064,260 @@ wz_status cg_batch(wz_plan* pl, const cpx<R>* phi, const cpx<R>* b, cpx<double>*
 
 }  // namespace
 
+// =============================== multi-shift CG =================================
+namespace {
+
+// All systems (M^dag M + sigma_i) x_i = b from one Krylov space (wz_cgk.cuh).  The base
+// system -- the smallest shift -- runs through the five fused passes of cg_iteration (shifted passes A'/E' if
+// its shift is not zero); two small kernels per iteration carry the other shifts along: k_ms_scalars (zeta
+// recurrences, on the device) and k_ms_update (x_i, p_i; r read once for all shifts).  complex64 plans iterate
+// without reliable updates (a recomputed residual would break the collinearity the method rests on) and
+// then POLISH: per shift, the defect b - (A + sigma_i) x_i is formed in complex128 and solved for by the
+// complex64 solver with reliable updates (wz_cg_solve_shift's loop), x_i += correction.
+template <typename R>
+wz_status ms_batch(wz_plan* pl, const cpx<R>* phi, const cpx<R>* b, cpx<double>* X, const double m[2],
+                   const double g[2], double rho, const double* sigmas, int ns, double tol, int max_iter, int nb,
+                   wz_cg_info* info) {
+  constexpr bool kF = (sizeof(R) == 4);
+  constexpr int N = vec16<R>::N;
+  const long n = 8 * pl->V;
+  const size_t n1 = (size_t)4 * pl->V;
+  cudaStream_t st = pl->stream;
+  R* r = (R*)pl->r; R* p = (R*)pl->p; R* xs = (R*)pl->xs;
+  const int gv = vec_grid(n, N), gv2 = vec_grid(n, 2);
+  wz_status s;
+  int base = 0;
+  for (int i = 1; i < ns; ++i)
+    if (sigmas[i] < sigmas[base]) base = i;
+  const double sigma0 = sigmas[base];
+
+  // workspace
+  const size_t need = (size_t)ns * pl->max_batch;
+  if (pl->ms_cap < need) {
+    R* a = nullptr; R* c = nullptr;
+    if (!dev_alloc(pl, &a, need * 2 * n1)) return WZ_ENOMEM;
+    if (kF && !dev_alloc(pl, &c, need * 2 * n1)) return WZ_ENOMEM;
+    pl->ms_p = a; pl->ms_x = c; pl->ms_cap = need;
+  }
+  if (!pl->ms_state && (!dev_alloc(pl, &pl->ms_state, (size_t)pl->max_batch) ||
+                        !dev_alloc(pl, &pl->ms_true, (size_t)WZ_MAX_SHIFTS * pl->max_batch)))
+    return WZ_ENOMEM;
+  if (kF && !pl->ms_rhs) {
+    R* a = nullptr;
+    if (!dev_alloc(pl, &a, (size_t)pl->max_batch * 2 * n1)) return WZ_ENOMEM;
+    pl->ms_rhs = a;
+  }
+  if (kF && !pl->ms_e && !dev_alloc(pl, &pl->ms_e, (size_t)pl->max_batch * n1)) return WZ_ENOMEM;
+  R* msp = (R*)pl->ms_p;
+  // x_i: complex128 plans write the caller's buffer directly; complex64 plans iterate on float copies
+  R* msx_f = (R*)pl->ms_x;
+  double* msx_d = (double*)X;
+  // solution of the base system: advanced by pass A' (one update late) in its slot of the same array
+  R* xbase_f = kF ? msx_f + (size_t)base * nb * n : nullptr;
+  double* xbase_d = msx_d + (size_t)base * nb * n;
+
+  std::vector<CGState> h(nb);
+  memset(h.data(), 0, sizeof(CGState) * nb);
+  for (int j = 0; j < nb; ++j) {
+    h[j].tol = tol; h[j].delta = kDelta; h[j].max_iter = max_iter; h[j].use_ru = 0;
+    h[j].true_rr = -1.0; h[j].shift = sigma0;
+    if (max_iter == 0) h[j].stop = 1;
+  }
+  std::vector<MSState> hm(nb);
+  memset(hm.data(), 0, sizeof(MSState) * nb);
+  for (int j = 0; j < nb; ++j) {
+    hm[j].nshift = ns; hm[j].alpha_prev = 1.0; hm[j].beta_prev = 0.0; hm[j].last_iter = 0;
+    for (int i = 0; i < ns; ++i) { hm[j].zeta[i] = hm[j].zeta_prev[i] = 1.0; hm[j].srel[i] = sigmas[i] - sigma0; hm[j].rec[i] = 1.0; }
+  }
+  WZ_CUDA(cudaMemcpyAsync(pl->d_state, h.data(), sizeof(CGState) * nb, cudaMemcpyHostToDevice, st));
+  WZ_CUDA(cudaMemcpyAsync(pl->ms_state, hm.data(), sizeof(MSState) * nb, cudaMemcpyHostToDevice, st));
+  WZ_CUDA(cudaStreamSynchronize(st));
+  {
+    ProfScope ps(pl, WZ_K_OTHER);
+    k_cg_init<R, R><<<dim3(gv2, nb), CGK_NT, 0, st>>>((const R*)b, r, p, nullptr, nullptr, n, red_of(pl));
+  }
+  {
+    ProfScope ps(pl, WZ_K_OTHER);
+    if constexpr (kF) k_ms_init<R, R, R><<<dim3(gv2, nb), CGK_NT, 0, st>>>((const R*)b, msp, msx_f, n, nb, ns);
+    else k_ms_init<R, double, R><<<dim3(gv2, nb), CGK_NT, 0, st>>>((const R*)b, msp, msx_d, n, nb, ns);
+  }
+  WZ_CUDA(cudaGetLastError());
+
+  int slot_w = 0, slot_r = 0, inflight = 0;
+  const CGState* snap = nullptr;
+  for (;;) {
+    while (inflight < 2) {
+      for (int it = 0; it < kCheckEvery; ++it) {
+        if constexpr (kF) s = cg_iteration<R>(pl, phi, m, g, rho, (cpx<R>*)r, (cpx<R>*)p, (cpx<R>*)xbase_f, 0, nb, false, sigma0);
+        else s = cg_iteration<R>(pl, phi, m, g, rho, (cpx<R>*)r, (cpx<R>*)p, (cpx<R>*)xbase_d, 0, nb, false, sigma0);
+        if (s != WZ_OK) return s;
+        if (ns > 1) {
+          {
+            ProfScope ps(pl, WZ_K_OTHER);
+            k_ms_scalars<<<nb, WZ_MAX_SHIFTS, 0, st>>>(pl->ms_state, pl->d_state);
+          }
+          ProfScope ps(pl, WZ_K_OTHER);
+          if constexpr (kF) k_ms_update<R, R><<<dim3(gv2, nb), CGK_NT, 0, st>>>(r, msp, msx_f, n, nb, base, pl->ms_state);
+          else k_ms_update<R, double><<<dim3(gv2, nb), CGK_NT, 0, st>>>(r, msp, msx_d, n, nb, base, pl->ms_state);
+        }
+        WZ_CUDA(cudaGetLastError());
+      }
+      WZ_CUDA(cudaMemcpyAsync(pl->h_state + slot_w * pl->max_batch, pl->d_state, sizeof(CGState) * nb,
+                              cudaMemcpyDeviceToHost, st));
+      WZ_CUDA(cudaEventRecord(pl->ev[slot_w], st));
+      slot_w ^= 1;
+      ++inflight;
+    }
+    WZ_CUDA(cudaEventSynchronize(pl->ev[slot_r]));
+    snap = pl->h_state + slot_r * pl->max_batch;
+    slot_r ^= 1;
+    --inflight;
+    bool all_done = true;
+    for (int j = 0; j < nb; ++j)
+      if (!(snap[j].converged || snap[j].stop)) all_done = false;
+    if (all_done) break;
+  }
+  WZ_CUDA(cudaStreamSynchronize(st));
+  // the base system's x lags one update behind (pass A' applies it): flush
+  {
+    ProfScope ps(pl, WZ_K_OTHER);
+    if constexpr (kF) k_flush_x<R><<<dim3(gv, nb), CGK_NT, 0, st>>>(xbase_f, p, n, pl->d_state);
+    else k_flush_x<double><<<dim3(gv, nb), CGK_NT, 0, st>>>(xbase_d, (const double*)p, n, pl->d_state);
+  }
+  {
+    ProfScope ps(pl, WZ_K_OTHER);
+    k_clear_alpha<<<nb, 1, 0, st>>>(pl->d_state);
+  }
+  if constexpr (kF) {  // complex64 plans: x_i -> the caller's complex128 buffer
+    ProfScope ps(pl, WZ_K_OTHER);
+    k_to_double<float><<<vec_grid((long)ns * nb * n, 1), CGK_NT, 0, st>>>(msx_d, msx_f, (long)ns * nb * n, 0);
+  }
+  WZ_CUDA(cudaGetLastError());
+  std::vector<CGState> fin(nb);
+  std::vector<MSState> finm(nb);
+  WZ_CUDA(cudaMemcpyAsync(fin.data(), pl->d_state, sizeof(CGState) * nb, cudaMemcpyDeviceToHost, st));
+  WZ_CUDA(cudaMemcpyAsync(finm.data(), pl->ms_state, sizeof(MSState) * nb, cudaMemcpyDeviceToHost, st));
+  WZ_CUDA(cudaStreamSynchronize(st));
+
+  // true residuals ||b - (A + sigma_i) x_i||^2 in complex128, every shift and source
+  const cpx<double>* phid = kF ? pl->phi128 : (const cpx<double>*)phi;
+  auto true_residuals = [&](int i) -> wz_status {
+    struct Override {
+      wz_plan* p;
+      explicit Override(wz_plan* q) : p(q) { p->prof_override = WZ_K_OTHER; }
+      ~Override() { p->prof_override = -1; }
+    } ov(pl);
+    for (int j = 0; j < nb; ++j) {
+      cpx<double>* xij = X + ((size_t)i * nb + j) * n1;
+      wz_status s2 = apply_MdagM_impl<double>(pl, phid, m, g, rho, xij, pl->q128, 1, false);
+      if (s2 != WZ_OK) return s2;
+      RedArgs ra = red_of(pl).for_source(j);
+      ra.store = pl->ms_true + (size_t)i * pl->max_batch + j;
+      ProfScope ps(pl, WZ_K_OTHER);
+      if constexpr (kF)  // also leaves the defect, rounded to complex64, as the right-hand side of the polishing solve
+        k_resid<float, float, FIN_STORE><<<dim3(gv2, 1), CGK_NT, 0, st>>>((const float*)(b + j * n1), (const double*)pl->q128,
+                                                                          (float*)pl->ms_rhs + j * n, n, ra, (const double*)xij, sigmas[i]);
+      else
+        k_resid<double, double, FIN_STORE><<<dim3(gv2, 1), CGK_NT, 0, st>>>((const double*)(b + j * n1), (const double*)pl->q128,
+                                                                            nullptr, n, ra, (const double*)xij, sigmas[i]);
+      WZ_CUDA(cudaGetLastError());
+    }
+    return WZ_OK;
+  };
+  std::vector<double> tr((size_t)WZ_MAX_SHIFTS * pl->max_batch, 0.0);
+  auto read_true = [&]() -> wz_status {
+    WZ_CUDA(cudaMemcpyAsync(tr.data(), pl->ms_true, sizeof(double) * tr.size(), cudaMemcpyDeviceToHost, st));
+    WZ_CUDA(cudaStreamSynchronize(st));
+    return WZ_OK;
+  };
+  for (int i = 0; i < ns; ++i) {
+    if ((s = true_residuals(i)) != WZ_OK) return s;
+    if ((s = read_true()) != WZ_OK) return s;
+    for (int j = 0; j < nb; ++j) {
+      wz_cg_info& o = info[(size_t)i * nb + j];
+      const double bn = fin[j].bnorm;
+      o.iterations = (i == base) ? fin[j].iter : finm[j].its[i];
+      o.reliable_updates = 0;
+      o.converged = (i == base) ? fin[j].converged : finm[j].frozen[i];
+      if (bn == 0.0) o.converged = 1;
+      o.rel_residual_recursive = bn > 0 ? ((i == base) ? std::sqrt(fin[j].rr) / bn : finm[j].rec[i]) : 0.0;
+      o.rel_residual_true = bn > 0 ? std::sqrt(tr[(size_t)i * pl->max_batch + j]) / bn : 0.0;
+    }
+    if constexpr (kF) {
+      // polish: solve (A + sigma_i) e = d_i for the sources whose true residual is above tol (complex64 drift)
+      std::vector<double> tolj(nb, 0.5);
+      bool any = false;
+      for (int j = 0; j < nb; ++j) {
+        const wz_cg_info& o = info[(size_t)i * nb + j];
+        if (fin[j].bnorm > 0 && o.rel_residual_true > tol) {
+          tolj[j] = 0.95 * tol / o.rel_residual_true;  // relative to ||d||: ends at 0.95 tol ||b||
+          any = true;
+        } else {
+          tolj[j] = 1e30;  // nothing to do: converges at once
+        }
+      }
+      if (any) {
+        int spent = 0;
+        for (int j = 0; j < nb; ++j) spent = std::max(spent, info[(size_t)i * nb + j].iterations);
+        std::vector<wz_cg_info> pol(nb);
+        s = cg_batch<float>(pl, (const cpx<float>*)phi, (const cpx<float>*)pl->ms_rhs, pl->ms_e, m, g, rho, tol,
+                            std::max(0, max_iter - spent), nb, pol.data(), false, sigmas[i], tolj.data());
+        if (s != WZ_OK) return s;
+        {
+          ProfScope ps(pl, WZ_K_OTHER);
+          k_rat_term<double><<<dim3(gv2, nb), CGK_NT, 0, st>>>((double*)(X + (size_t)i * nb * n1), (const double*)pl->ms_e, 1.0, n, 0);
+        }
+        WZ_CUDA(cudaGetLastError());
+        if ((s = true_residuals(i)) != WZ_OK) return s;
+        if ((s = read_true()) != WZ_OK) return s;
+        for (int j = 0; j < nb; ++j) {
+          wz_cg_info& o = info[(size_t)i * nb + j];
+          if (tolj[j] > 1e29) continue;
+          o.iterations += pol[j].iterations;
+          o.reliable_updates = pol[j].reliable_updates;
+          o.rel_residual_true = std::sqrt(tr[(size_t)i * pl->max_batch + j]) / fin[j].bnorm;
+          o.converged = (o.rel_residual_true <= tol * (1.0 + 1e-9)) ? 1 : 0;
+        }
+      }
+    }
+  }
+  return WZ_OK;
+}
+
+}  // namespace
+
+extern "C" wz_status wz_cg_solve_multishift(wz_plan* pl, const void* phi, const void* b, void* x, const double m[2],
+                                            const double g[2], double rho, const double* sigmas, int nshift, double tol,
+                                            int max_iter, int nbatch, wz_cg_info* info) {
+  g_err[0] = 0;
+  if (!pl || !phi || !b || !x || !m || !g || !info || !sigmas) return WZ_EINVAL;
+  if (nshift < 1 || nshift > WZ_MAX_SHIFTS) return WZ_EINVAL;
+  for (int i = 0; i < nshift; ++i)
+    if (!(sigmas[i] >= 0.0)) return WZ_EINVAL;
+  if (!(rho > 0.0 && rho < 2.0) || !(tol > 0.0) || max_iter < 0) return WZ_EINVAL;
+  if (nbatch < 0 || nbatch > pl->max_batch || x == b) return WZ_EINVAL;
+  if (nbatch == 0) return WZ_OK;
+  WZ_ON_DEVICE(pl);
+  wz_status s;
+  if (pl->dtype == WZ_C64) {
+    const long nphi = 2 * pl->V;
+    {
+      ProfScope ps(pl, WZ_K_OTHER);
+      k_f2d<<<vec_grid(nphi, 1), CGK_NT, 0, pl->stream>>>((double*)pl->phi128, (const float*)phi, nphi);
+    }
+    WZ_CUDA(cudaGetLastError());
+    s = ms_batch<float>(pl, (const cpx<float>*)phi, (const cpx<float>*)b, (cpx<double>*)x, m, g, rho, sigmas, nshift,
+                        tol, max_iter, nbatch, info);
+  } else {
+    s = ms_batch<double>(pl, (const cpx<double>*)phi, (const cpx<double>*)b, (cpx<double>*)x, m, g, rho, sigmas,
+                         nshift, tol, max_iter, nbatch, info);
+  }
+  if (s != WZ_OK) return s;
+  for (int i = 0; i < nshift * nbatch; ++i)
+    if (!info[i].converged) return WZ_ENOTCONVERGED;
+  return WZ_OK;
+}
+
 static wz_status cg_solve_any(wz_plan* pl, const void* phi, const void* b, void* x, const double m[2],
                               const double g[2], double rho, double tol, int max_iter, int nbatch,
                               wz_cg_info* info, bool pc, double sigma = 0.0) {
@@ -1128,7 +1391,10 @@ wz_status wz_rational_apply(wz_plan* pl, const void* phi, const void* eta, void*
   WZ_ON_DEVICE(pl);
   const size_t n1 = (size_t)4 * pl->V;
   const long n = 8 * pl->V;
-  if (!pl->ratX && !dev_alloc(pl, &pl->ratX, (size_t)pl->max_batch * n1)) return WZ_ENOMEM;
+  if (pl->ratX_cap < (size_t)pl->max_batch) {
+    if (!dev_alloc(pl, &pl->ratX, (size_t)pl->max_batch * n1)) return WZ_ENOMEM;
+    pl->ratX_cap = pl->max_batch;
+  }
   const int gv2 = vec_grid(n, 2);
   {
     ProfScope ps(pl, WZ_K_OTHER);
@@ -1148,6 +1414,73 @@ wz_status wz_rational_apply(wz_plan* pl, const void* phi, const void* eta, void*
     ProfScope ps(pl, WZ_K_OTHER);
     k_rat_term<double><<<dim3(gv2, nbatch), CGK_NT, 0, pl->stream>>>((double*)out, (const double*)pl->ratX, alphas[i], n, 0);
     WZ_CUDA(cudaGetLastError());
+  }
+  WZ_CUDA(cudaStreamSynchronize(pl->stream));
+  return all_ok ? WZ_OK : WZ_ENOTCONVERGED;
+}
+
+// Eq. (7.6)-(7.7) with ONE multi-shift solve for every shift above pc_cutoff (all of them if pc_cutoff < 0 or
+// m = 0) and the paper's preconditioned per-shift solves (Eq. 7.14) below it.
+wz_status wz_rational_apply_multishift(wz_plan* pl, const void* phi, const void* eta, void* out, const double m[2],
+                                       const double g[2], double rho, double alpha0, const double* alphas,
+                                       const double* betas, int nshift, double pc_cutoff, double tol, int max_iter,
+                                       int nbatch, wz_cg_info* info) {
+  g_err[0] = 0;
+  if (!pl || !phi || !eta || !out || !m || !g || !info || nshift < 0 || (nshift > 0 && (!alphas || !betas)))
+    return WZ_EINVAL;
+  if (nbatch < 0 || nbatch > pl->max_batch) return WZ_EINVAL;
+  for (int i = 0; i < nshift; ++i)
+    if (!(betas[i] >= 0.0)) return WZ_EINVAL;
+  if (out == eta) return WZ_EINVAL;
+  if (nbatch == 0) return WZ_OK;
+  WZ_ON_DEVICE(pl);
+  const size_t n1 = (size_t)4 * pl->V;
+  const long n = 8 * pl->V;
+  std::vector<int> ms_idx, pc_idx;
+  for (int i = 0; i < nshift; ++i) {
+    const bool pc = betas[i] <= pc_cutoff && !(m[0] == 0.0 && m[1] == 0.0);
+    (pc ? pc_idx : ms_idx).push_back(i);
+  }
+  if ((int)ms_idx.size() > WZ_MAX_SHIFTS) return WZ_EINVAL;
+  const size_t needX = std::max<size_t>(ms_idx.size(), 1) * pl->max_batch;
+  if (pl->ratX_cap < needX) {
+    if (!dev_alloc(pl, &pl->ratX, needX * n1)) return WZ_ENOMEM;
+    pl->ratX_cap = needX;
+  }
+  const int gv2 = vec_grid(n, 2);
+  {
+    ProfScope ps(pl, WZ_K_OTHER);
+    if (pl->dtype == WZ_C64)
+      k_rat_term<float><<<dim3(gv2, nbatch), CGK_NT, 0, pl->stream>>>((double*)out, (const float*)eta, alpha0, n, 1);
+    else
+      k_rat_term<double><<<dim3(gv2, nbatch), CGK_NT, 0, pl->stream>>>((double*)out, (const double*)eta, alpha0, n, 1);
+  }
+  WZ_CUDA(cudaGetLastError());
+  bool all_ok = true;
+  for (int i : pc_idx) {
+    wz_status s = cg_solve_any(pl, phi, eta, pl->ratX, m, g, rho, tol, max_iter, nbatch, info + (size_t)i * nbatch,
+                               true, betas[i]);
+    if (s == WZ_ENOTCONVERGED) all_ok = false;
+    else if (s != WZ_OK) return s;
+    ProfScope ps(pl, WZ_K_OTHER);
+    k_rat_term<double><<<dim3(gv2, nbatch), CGK_NT, 0, pl->stream>>>((double*)out, (const double*)pl->ratX, alphas[i], n, 0);
+    WZ_CUDA(cudaGetLastError());
+  }
+  if (!ms_idx.empty()) {
+    std::vector<double> sig(ms_idx.size());
+    for (size_t k = 0; k < ms_idx.size(); ++k) sig[k] = betas[ms_idx[k]];
+    std::vector<wz_cg_info> inf(ms_idx.size() * nbatch);
+    wz_status s = wz_cg_solve_multishift(pl, phi, eta, pl->ratX, m, g, rho, sig.data(), (int)sig.size(), tol, max_iter,
+                                         nbatch, inf.data());
+    if (s == WZ_ENOTCONVERGED) all_ok = false;
+    else if (s != WZ_OK) return s;
+    for (size_t k = 0; k < ms_idx.size(); ++k) {
+      for (int j = 0; j < nbatch; ++j) info[(size_t)ms_idx[k] * nbatch + j] = inf[k * nbatch + j];
+      ProfScope ps(pl, WZ_K_OTHER);
+      k_rat_term<double><<<dim3(gv2, nbatch), CGK_NT, 0, pl->stream>>>(
+          (double*)out, (const double*)(pl->ratX + k * nbatch * n1), alphas[ms_idx[k]], n, 0);
+      WZ_CUDA(cudaGetLastError());
+    }
   }
   WZ_CUDA(cudaStreamSynchronize(pl->stream));
   return all_ok ? WZ_OK : WZ_ENOTCONVERGED;

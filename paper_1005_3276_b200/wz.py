@@ -27,6 +27,7 @@ EXPORTS = [
     "wz_apply_M0inv", "wz_apply_MtdagMt", "wz_cg_solve_pc", "wz_apply_Dslash", "wz_locality_profile",
     "wz_cg_solve_shift", "wz_cg_solve_shift_pc", "wz_rational_apply",
     "wz_plan_set_graph", "wz_plan_cg_history", "wz_plan_set_block",
+    "wz_cg_solve_multishift", "wz_rational_apply_multishift",
 ]
 
 
@@ -83,6 +84,8 @@ def lib() -> ctypes.CDLL:
         L.wz_cg_solve_shift_pc.argtypes = L.wz_cg_solve_shift.argtypes
         L.wz_rational_apply.argtypes = [vp, vp, vp, vp, d2, d2, cd, cd, d2, d2, ci, cd, cd, ci, ci,
                                         ctypes.POINTER(_CGInfo)]
+        L.wz_rational_apply_multishift.argtypes = L.wz_rational_apply.argtypes
+        L.wz_cg_solve_multishift.argtypes = [vp, vp, vp, vp, d2, d2, cd, d2, ci, cd, ci, ci, ctypes.POINTER(_CGInfo)]
         L.wz_apply_M0inv.argtypes = [vp, ci, d2, cd, vp, vp, ci]
         L.wz_apply_MtdagMt.argtypes = [vp, vp, d2, d2, cd, vp, vp, ci]
         L.wz_apply_Dslash.argtypes = [vp, cd, vp, vp, ci]
@@ -305,9 +308,34 @@ class Plan:
         return out, res
 
 
+    def cg_solve_multishift(self, phi, b, m, g, sigmas, rho: float = 1.0, tol: float = 1e-6, max_iter: int = 100000,
+                            out=None, raise_on_fail: bool = True):
+        """All (M^dag M + sigma_i) x_i = b from one Krylov space (wz_cg_solve_multishift).
+        Returns (x complex128 [nshift, nbatch, 4, T, L1, L2, L3], infos[shift][source])."""
+        nb = self._spinor(b)
+        self._phi(phi)
+        d = len(sigmas)
+        shape = (d, nb, 4) + self.dims
+        if out is None:
+            out = torch.empty(shape, dtype=torch.complex128, device=b.device)
+        if out.dtype != torch.complex128 or tuple(out.shape) != shape or not out.is_contiguous() or out.device != self.device:
+            raise ValueError("out must be a contiguous complex128 tensor of shape %s on %s" % (shape, self.device))
+        cs = (ctypes.c_double * max(d, 1))(*[float(v) for v in sigmas])
+        infos = (_CGInfo * max(d * nb, 1))()
+        st = lib().wz_cg_solve_multishift(self._h, phi.data_ptr(), b.data_ptr(), out.data_ptr(), _c2(m), _c2(g),
+                                          float(rho), cs, d, float(tol), int(max_iter), nb, infos)
+        if st != WZ_OK and not (st == WZ_ENOTCONVERGED and not raise_on_fail):
+            _check(st)
+        res = [[CGInfo(infos[i * nb + j].iterations, infos[i * nb + j].reliable_updates,
+                       bool(infos[i * nb + j].converged), infos[i * nb + j].rel_residual_recursive,
+                       infos[i * nb + j].rel_residual_true) for j in range(nb)] for i in range(d)]
+        return out, res
+
     def rational_apply(self, phi, eta, m, g, alpha0, alphas, betas, rho: float = 1.0, tol: float = 1e-6,
-                       max_iter: int = 100000, pc_cutoff: float = 100.0, out=None, raise_on_fail: bool = True):
-        """out = alpha0 eta + sum_i alphas[i] (M^dag M + betas[i])^-1 eta (wz_rational_apply, Eq. 7.6-7.7).
+                       max_iter: int = 100000, pc_cutoff: float = 100.0, out=None, raise_on_fail: bool = True,
+                       multishift: bool = False):
+        """out = alpha0 eta + sum_i alphas[i] (M^dag M + betas[i])^-1 eta (wz_rational_apply, Eq. 7.6-7.7;
+        multishift=True: wz_rational_apply_multishift, one multi-shift solve for the shifts above pc_cutoff).
         Returns (out complex128, infos[shift][source])."""
         nb = self._spinor(eta)
         self._phi(phi)
@@ -319,7 +347,8 @@ class Plan:
         ca = (ctypes.c_double * max(d, 1))(*[float(a) for a in alphas])
         cb = (ctypes.c_double * max(d, 1))(*[float(b) for b in betas])
         infos = (_CGInfo * max(d * nb, 1))()
-        st = lib().wz_rational_apply(self._h, phi.data_ptr(), eta.data_ptr(), out.data_ptr(), _c2(m), _c2(g),
+        fn = lib().wz_rational_apply_multishift if multishift else lib().wz_rational_apply
+        st = fn(self._h, phi.data_ptr(), eta.data_ptr(), out.data_ptr(), _c2(m), _c2(g),
                                      float(rho), float(alpha0), ca, cb, d, float(pc_cutoff), float(tol),
                                      int(max_iter), nb, infos)
         if st != WZ_OK and not (st == WZ_ENOTCONVERGED and not raise_on_fail):

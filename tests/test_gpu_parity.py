@@ -882,3 +882,85 @@ def test_second_device(wz, orc, inp):
     assert rel(q[0], orc.apply_MdagM(phi, b[0], 0.05, 1.0, 1.0)) <= 1e-12
     with pytest.raises(ValueError):
         plan.fft4d(torch.from_numpy(b).to("cuda:0"), +1, True)
+
+
+# ---- NEXT-2, second half: multi-shift CG (oracle O8; Eq. 7.6-7.7, 927-931 Eq. 7.13) ----
+
+@pytest.mark.parametrize("dims,dtype,tol", [((8, 8, 8, 8), "c128", 1e-10), ((8, 4, 16, 8), "c128", 1e-12),
+                                            ((8, 8, 8, 8), "c64", 1e-6), ((16, 16, 16, 16), "c64", 1e-6)])
+def test_cg_multishift_vs_oracle(wz, orc, inp, dims, dtype, tol):
+    """All shifts from one Krylov space: per shift the iteration at which it froze against the oracle's
+    multi-shift loop (complex128; complex64 plans add their polishing iterations, so only a lower bound
+    there), the solution against the oracle's, and the true residual of (M^dag M + sigma_i) x_i = b
+    recomputed by the oracle.  Shifts unsorted on purpose (the base system is the smallest, wherever it is)."""
+    m, g, rho = 0.05, 1.0, 1.0
+    sigmas = [1.0, 0.01, 100.0, 0.0, 1e4]
+    phi = inp.make_phi(6, dims, 0.3, NPDT[dtype])
+    b = inp.make_sources(6, 2, dims, NPDT[dtype])
+    plan = wz.Plan(dims, dtype, 2)
+    d_phi, d_b = torch.from_numpy(phi).cuda(), torch.from_numpy(b).cuda()
+    plan.reset_launch_count()
+    x, infos = plan.cg_solve_multishift(d_phi, d_b, m, g, sigmas, rho, tol, 20000)
+    launches = plan.launch_count
+    x = x.cpu().numpy()
+    phi128 = phi.astype(np.complex128)
+    for j in range(2):
+        bj = b[j].astype(np.complex128)
+        Xo, io, mv = orc.cg_multishift(phi128, bj, m, g, sigmas, rho, tol, 20000)
+        for i, sigma in enumerate(sigmas):
+            gi = infos[i][j]
+            true_res = rel(orc.apply_MdagM(phi128, x[i, j], m, g, rho) + sigma * x[i, j], bj)
+            print("multishift %s %s sigma=%g: iterations gpu=%d (+polish RU %d) oracle=%d true residual %.2e"
+                  % (dims, dtype, sigma, gi.iterations, gi.reliable_updates, io[i].iterations, true_res))
+            assert gi.converged and io[i].converged
+            assert abs(true_res - gi.rel_residual_true) <= 0.05 * tol
+            if dtype == "c128":
+                assert true_res <= tol * 1.05
+                assert abs(gi.iterations - io[i].iterations) <= max(2, int(0.015 * io[i].iterations))
+                assert rel(x[i, j], Xo[i]) <= 1e-7
+            else:
+                assert true_res <= tol * (1 + 1e-3)
+                assert gi.iterations >= io[i].iterations - max(2, int(0.05 * io[i].iterations))
+                assert rel(x[i, j], Xo[i]) <= 5e-4
+    # one matvec per base iteration: far fewer launches than five separate solves
+    base_its = max(infos[3][j].iterations for j in range(2))
+    assert launches < 12 * base_its + 2000
+
+
+def test_cg_multishift_single_shift_and_errors(wz, inp):
+    dims = (8, 8, 8, 8)
+    phi = inp.make_phi(6, dims, 0.3)
+    b = inp.make_sources(6, 1, dims)
+    plan = wz.Plan(dims, "c128", 1)
+    d_phi, d_b = torch.from_numpy(phi).cuda(), torch.from_numpy(b).cuda()
+    x0, i0 = plan.cg_solve(d_phi, d_b, 0.05, 1.0, 1.0, 1e-10, 20000, sigma=0.5)
+    x1, i1 = plan.cg_solve_multishift(d_phi, d_b, 0.05, 1.0, [0.5], 1.0, 1e-10, 20000)
+    assert i1[0][0].iterations == i0[0].iterations and torch.equal(x1[0], x0)  # the base system IS wz_cg_solve_shift
+    for bad in ([], [-1.0], [0.1] * 33):
+        with pytest.raises(wz.WZError) as e:
+            plan.cg_solve_multishift(d_phi, d_b, 0.05, 1.0, bad, 1.0, 1e-10, 100)
+        assert e.value.status == wz.WZ_EINVAL
+    x2, i2 = plan.cg_solve_multishift(d_phi, d_b, 0.05, 1.0, [0.5, 2.0], 1.0, 1e-10, 7, raise_on_fail=False)
+    assert i2[0][0].iterations == 7 and not i2[0][0].converged and not i2[1][0].converged
+
+
+@pytest.mark.parametrize("dims,dtype,tol", [((8, 8, 8, 8), "c128", 1e-12), ((16, 16, 16, 16), "c64", 1e-6)])
+def test_rational_apply_multishift_vs_oracle(wz, orc, inp, dims, dtype, tol):
+    """Eq. 7.6 with the shifts above the cutoff from one multi-shift solve (and all of them with pc_cutoff < 0):
+    the sum against the oracle's one-solve-per-shift sum and against the library's own per-shift mode."""
+    m, g, rho = 1.0, 0.1, 1.0
+    phi = inp.make_phi(9, dims, 0.5, NPDT[dtype])
+    eta = inp.make_sources(9, 2, dims, NPDT[dtype])
+    a0, al, be = inp.rational_ladder(20, 1e-2, 1e3)
+    plan = wz.Plan(dims, dtype, 2)
+    d_phi, d_eta = torch.from_numpy(phi).cuda(), torch.from_numpy(eta).cuda()
+    phi128 = phi.astype(np.complex128)
+    ref = np.stack([orc.rational_apply(phi128, eta[j].astype(np.complex128), m, g, a0, al, be, rho, tol, 1000)[0]
+                    for j in range(2)])
+    bound = 1e-10 if dtype == "c128" else 2e-6
+    for cutoff in (100.0, -1.0):
+        out, infos = plan.rational_apply(d_phi, d_eta, m, g, a0, al, be, rho, tol, 5000, pc_cutoff=cutoff, multishift=True)
+        assert all(i.converged for row in infos for i in row)
+        assert rel(out.cpu().numpy(), ref) <= bound
+        its = [max(i.iterations for i in row) for row in infos]
+        print("rational multishift %s %s cutoff %g: iterations per shift %s" % (dims, dtype, cutoff, its))
