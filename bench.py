@@ -25,6 +25,7 @@ if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
 METRIC = "CG iterations/s at 32^4 (complex64, 12 sources to 1e-6)"
+NOMINAL_HBM_GBS = 8000.0  # the "~8 TB/s" BASELINE.json's north star quotes; the roofline uses the MEASURED peak
 UNIT = "CG iterations/s"
 
 
@@ -40,7 +41,16 @@ def parse_args():
                     help="CG iteration cap; lower it ONLY for profiler runs (the line then says so)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-extras", action="store_true", help="skip the separate FFT / matvec timings")
+    ap.add_argument("--full-table", action="store_true",
+                    help="also solve config 5b (64^4; about two minutes) in the table of the other configs")
     return ap.parse_args()
+
+
+def workload_string(key, cfg, nsrc):
+    """One description of the workload for both arms (the driver compares the strings)."""
+    return ("config %s: %s lattice, %s, %d Gaussian sources per GPU to tol %g, m=%g g=%g rho=%g, seed %d"
+            % (key, "x".join(map(str, cfg["dims"])), cfg["dtype"], nsrc, cfg["tol"], cfg["m"], cfg["g"], cfg["rho"],
+               cfg["seed"]))
 
 
 def get_cfg(key):
@@ -102,9 +112,9 @@ class ClockSampler:
                 "samples": len(sm), "reasons": sorted(reasons)}
 
 
-def oracle_sample(cfg, n_iter):
+def oracle_sample(cfg, n_iter, threads=0):
     """The oracle as it stands (O4', complex64-rounded CG with reliable updates) on
-    source 0 of the workload for n_iter iterations; returns (iterations/s, threads, text)."""
+    source 0 of the workload for n_iter iterations; returns (iterations/s, threads, text, seconds)."""
     import numpy as np
 
     from oracle import wz_oracle as orc
@@ -112,17 +122,116 @@ def oracle_sample(cfg, n_iter):
 
     orc.build()
     dims = cfg["dims"]
-    phi = inputs.make_phi(cfg["seed"], dims, cfg["sigma"], np.complex64).astype(np.complex128)
-    b = inputs.make_source(cfg["seed"], 0, dims, np.complex64).astype(np.complex128)
-    threads = orc.set_threads(0)
+    npdt = np.complex64 if cfg["dtype"] == "c64" else np.complex128
+    phi = inputs.make_phi(cfg["seed"], dims, cfg["sigma"], npdt).astype(np.complex128)
+    b = inputs.make_source(cfg["seed"], 0, dims, npdt).astype(np.complex128)
+    all_threads = orc.set_threads(0)
+    threads = orc.set_threads(threads) if threads > 0 else all_threads
     fn = orc.cg_c64ru if cfg["dtype"] == "c64" else orc.cg
     t0 = time.perf_counter()
     _, info = fn(phi, b, cfg["m"], cfg["g"], cfg["rho"], cfg["tol"], n_iter)
     dt = time.perf_counter() - t0
+    orc.set_threads(all_threads)
     its = max(info.iterations, 1)
-    text = "source 0 of the workload, first %d CG iterations of the oracle (%s), %.1f s" % (
-        its, "O4' complex64+reliable updates" if cfg["dtype"] == "c64" else "O4 complex128", dt)
+    text = "source 0 of the workload, first %d CG iterations of the oracle (%s), %.1f s on %d threads" % (
+        its, "O4' complex64+reliable updates" if cfg["dtype"] == "c64" else "O4 complex128", dt, threads)
     return its / dt, threads, text, dt
+
+
+def oracle_pieces(cfg, threads):
+    """Oracle timings beside the GPU's (SURVEY 8(d) "Oracle timed beside it"): one 4-spinor 4D FFT, one
+    M^dag M, and CG seconds per iteration, on `threads` OpenMP threads (0 = all)."""
+    import numpy as np
+
+    from oracle import wz_oracle as orc
+    from paper_1005_3276_b200 import inputs
+
+    orc.build()
+    dims = cfg["dims"]
+    npdt = np.complex64 if cfg["dtype"] == "c64" else np.complex128
+    phi = inputs.make_phi(cfg["seed"], dims, cfg["sigma"], npdt).astype(np.complex128)
+    b = inputs.make_source(cfg["seed"], 0, dims, npdt).astype(np.complex128)
+    all_threads = orc.set_threads(0)
+    used = orc.set_threads(threads) if threads > 0 else all_threads
+    t0 = time.perf_counter()
+    orc.dft4d(b, +1, True)
+    t_fft = time.perf_counter() - t0
+    t0 = time.perf_counter()
+    orc.apply_MdagM(phi, b, cfg["m"], cfg["g"], cfg["rho"])
+    t_mv = time.perf_counter() - t0
+    n_it = 2 if used == 1 else 6
+    fn = orc.cg_c64ru if cfg["dtype"] == "c64" else orc.cg
+    t0 = time.perf_counter()
+    _, info = fn(phi, b, cfg["m"], cfg["g"], cfg["rho"], cfg["tol"], n_it)
+    t_cg = (time.perf_counter() - t0) / max(info.iterations, 1)
+    orc.set_threads(all_threads)
+    return {"threads": used, "fft4d_4spinor_s": t_fft, "MdagM_s": t_mv, "cg_s_per_iteration": t_cg,
+            "cg_iterations_per_s": 1.0 / t_cg, "cg_sample_iterations": n_it}
+
+
+def small_config_table(dev, full=False):
+    """Time to solution and CG iterations/s at the configs other than the metric's (BASELINE.json configs 1, 2,
+    3, 5a, [5b], and config 4 with a single source), each with the iteration chunks replayed as a CUDA graph
+    and enqueued kernel by kernel, next to the oracle's time on the host cores: full solve for configs 1, 2,
+    per-iteration sample x the GPU's iteration count (labelled extrapolated) for config 3
+    ("Small configs (1-3) ... report absolute times")."""
+    import numpy as np
+    import torch
+
+    from oracle import wz_oracle as orc
+    from paper_1005_3276_b200 import inputs, wz
+
+    table = {}
+    keys = [(1, None), (2, None), (3, None), (4, 1), ("5a", None)] + ([("5b", None)] if full else [])
+    for key, nsrc_override in keys:
+        cfg = inputs.CONFIGS[key]
+        dims, nsrc = cfg["dims"], nsrc_override or cfg["nsrc"]
+        npdt = np.complex64 if cfg["dtype"] == "c64" else np.complex128
+        phi = inputs.make_phi(cfg["seed"], dims, cfg["sigma"], npdt)
+        b = inputs.make_sources(cfg["seed"], nsrc, dims, npdt)
+        d_phi, d_b = torch.from_numpy(phi).to(dev), torch.from_numpy(b).to(dev)
+        plan = wz.Plan(dims, cfg["dtype"], nsrc, dev)
+        x = torch.empty(b.shape, dtype=torch.complex128, device=dev)
+        row = {"lattice": "x".join(map(str, dims)), "dtype": cfg["dtype"], "sources": nsrc, "tol": cfg["tol"]}
+        for graph in (True, False):
+            plan.set_graph(graph)
+            best = None
+            for rep in range(3 if key in (1, 2, 3) else 1):
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record()
+                _, infos = plan.cg_solve(d_phi, d_b, cfg["m"], cfg["g"], cfg["rho"], cfg["tol"], 500000, out=x,
+                                         raise_on_fail=False)
+                e1.record()
+                e1.synchronize()
+                t = e0.elapsed_time(e1) * 1e-3
+                best = t if best is None else min(best, t)
+            its = sum(i.iterations for i in infos)
+            row["graph" if graph else "stream_launches"] = {
+                "time_to_solution_s": best, "iterations": [i.iterations for i in infos], "iterations_per_s": its / best,
+                "us_per_iteration_per_source": 1e6 * best / max(its, 1),
+                "worst_true_residual": max(i.rel_residual_true for i in infos),
+                "all_converged": all(i.converged for i in infos)}
+        row["graph_speedup"] = row["stream_launches"]["time_to_solution_s"] / row["graph"]["time_to_solution_s"]
+        plan.close()
+        if key in (1, 2, 3):
+            phi128, b0 = phi.astype(np.complex128), b[0].astype(np.complex128)
+            fn = orc.cg_c64ru if cfg["dtype"] == "c64" else orc.cg
+            threads = orc.set_threads(0)
+            if key == 3:
+                t0 = time.perf_counter()
+                _, io = fn(phi128, b0, cfg["m"], cfg["g"], cfg["rho"], cfg["tol"], 40)
+                per_it = (time.perf_counter() - t0) / max(io.iterations, 1)
+                row["oracle"] = {"kind": "extrapolated: 40-iteration sample x the GPU's iteration count of source 0",
+                                 "threads": threads, "s_per_iteration": per_it,
+                                 "time_to_solution_s_source0": per_it * row["graph"]["iterations"][0]}
+            else:
+                t0 = time.perf_counter()
+                _, io = fn(phi128, b0, cfg["m"], cfg["g"], cfg["rho"], cfg["tol"], 100000)
+                dt = time.perf_counter() - t0
+                row["oracle"] = {"kind": "full solve", "threads": threads, "iterations": io.iterations,
+                                 "time_to_solution_s_source0": dt}
+        table["config_%s%s" % (key, "_single_source" if nsrc_override else "")] = row
+    return table
 
 
 def oracle_iters_for(cfg):
@@ -151,7 +260,8 @@ def run_reference(args):
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot_t / max(args.steps, 1),
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": "config %s: %s lattice, %s" % (key, "x".join(map(str, cfg["dims"])), cfg["dtype"])},
+        "config": {"workload": workload_string(key, cfg, args.sources or cfg["nsrc"]),
+                   "sample": "the oracle runs a bounded sample of this workload: " + text},
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": text},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -300,9 +410,14 @@ def run_wz(args):
         v["gbs"] = v["algo_bytes"] / (v["us"] * 1e-6) / 1e9
         v["frac"] = v["gbs"] / peak
     dom = max(kinds, key=lambda k: kinds[k]["share"])
-    traffic = load_traffic().get(dom)
+    tr = load_traffic()
+    traffic = tr.get(dom)
     roofline = {"bound": "hbm", "kernel": dom, "achieved": kinds[dom]["gbs"], "peak": peak, "unit": "GB/s",
-                "frac": kinds[dom]["frac"], "traffic": traffic, "peak_source": peak_src,
+                "frac": kinds[dom]["frac"], "traffic": traffic,
+                "traffic_source": tr.get("_source", "none") + " (static file, refreshed with every kernel change; "
+                                  "not measured in this run)",
+                "peak_source": peak_src, "nominal_peak": NOMINAL_HBM_GBS,
+                "frac_of_nominal": kinds[dom]["gbs"] / NOMINAL_HBM_GBS,
                 "algo_bytes_per_launch": kinds[dom]["algo_bytes"], "us_per_launch": kinds[dom]["us"],
                 "share_of_step": kinds[dom]["share"],
                 "all_kernels": {k: {"us": round(v["us"], 2), "GB/s": round(v["gbs"], 1), "frac": round(v["frac"], 3),
@@ -317,7 +432,9 @@ def run_wz(args):
                    "reliable_updates_per_source": [i.reliable_updates for i in infos],
                    "time_to_solution_s_per_source": secs / args.steps / nsrc,
                    "all_converged": conv, "worst_true_residual": worst_true,
-                   "cg_algorithmic_GBs": 18.5 * u / (per_iter_us * 1e-6) / 1e9})
+                   "cg_algorithmic_GBs": 18.5 * u / (per_iter_us * 1e-6) / 1e9,
+                   "cg_frac_of_measured_peak": 18.5 * u / (per_iter_us * 1e-6) / 1e9 / peak,
+                   "cg_frac_of_nominal_8TBs": 18.5 * u / (per_iter_us * 1e-6) / 1e9 / NOMINAL_HBM_GBS})
 
     if not args.no_extras:
         extras["preconditioned"] = time_preconditioned(plan, d_phi, d_b, d_x, cfg, secs / args.steps)
@@ -327,7 +444,11 @@ def run_wz(args):
     cpu = None
     if not args.no_cpu_baseline and world == 1:
         ips, threads, text, _ = oracle_sample(cfg, oracle_iters_for(cfg))
-        cpu = {"value": ips, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": text}
+        cpu = {"value": ips, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": text,
+               # two columns (1 thread, all cores); FFT, M^dag M and CG per iteration of the oracle
+               "all_cores": oracle_pieces(cfg, 0), "one_thread": oracle_pieces(cfg, 1)}
+        if not args.no_extras:
+            extras["other_configs"] = small_config_table(dev, args.full_table)
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
@@ -335,8 +456,7 @@ def run_wz(args):
         "scaling": "weak", "vs_baseline": None, "dtype": "f32 (complex64 vectors, f64 reductions, complex128 reliable updates)"
         if cfg["dtype"] == "c64" else "f64",
         "data": "synthetic",
-        "config": {"workload": "config %s: %s lattice, %s, %d Gaussian sources per GPU to tol %g, m=%g g=%g rho=%g, seed %d"
-                   % (key, "x".join(map(str, dims)), cfg["dtype"], nsrc, tol, m, g, rho, cfg["seed"]),
+        "config": {"workload": workload_string(key, cfg, nsrc),
                    "l2": "no flush: working set of one solve (8 vectors, %.0f MB) exceeds the 126 MB L2" % (8.25 * u / 1e6),
                    "sources": "independent, advanced in lock step through shared launches; sharded across ranks, phi replicated"},
         "max_iter": args.max_iter, "valid": bool(conv),

@@ -964,3 +964,66 @@ def test_rational_apply_multishift_vs_oracle(wz, orc, inp, dims, dtype, tol):
         assert rel(out.cpu().numpy(), ref) <= bound
         its = [max(i.iterations for i in row) for row in infos]
         print("rational multishift %s %s cutoff %g: iterations per shift %s" % (dims, dtype, cutoff, its))
+
+
+# ---- every solver path once on the two smallest lattices.  compute-sanitizer is closed on
+#      this GPU pool (profiles/r02_sanitizer.md), so the test carries its own checks: the caller's output
+#      buffers sit between canary regions (out-of-bounds writes), and every solve is repeated and must
+#      reproduce bit for bit (a race in the ticket-counter reductions, the deferred x update or the in-place
+#      p / r rewrites would show up as run-to-run differences) ----
+
+def _guarded(shape, dtype, pad=4096):
+    """A tensor of `shape` carved out of a larger allocation with canaries on both sides."""
+    n = int(np.prod(shape))
+    buf = torch.full((n + 2 * pad,), 7.25 - 1.5j, dtype=dtype, device="cuda")
+    return buf[pad:pad + n].view(shape), buf, pad
+
+
+def _canaries_intact(buf, pad):
+    v = torch.tensor(7.25 - 1.5j, dtype=buf.dtype, device=buf.device)
+    return bool((buf[:pad] == v).all() and (buf[-pad:] == v).all())
+
+
+@pytest.mark.parametrize("dims", [(4, 4, 4, 4), (8, 8, 8, 8)])
+def test_small_solves_all_paths(wz, orc, inp, dims):
+    m, g, rho = 0.1, 0.5, 1.0
+    for dtype, tol in (("c128", 1e-10), ("c64", 1e-6)):
+        phi = inp.make_phi(1, dims, 0.3, NPDT[dtype])
+        b = inp.make_sources(1, 2, dims, NPDT[dtype])
+        phi128 = phi.astype(np.complex128)
+        plan = wz.Plan(dims, dtype, 2)
+        d_phi, d_b = torch.from_numpy(phi).cuda(), torch.from_numpy(b).cuda()
+        cases = {"plain": {}, "pc": {"precondition": True}, "shift": {"sigma": 0.3},
+                 "shift_pc": {"precondition": True, "sigma": 0.3}}
+        for graph in (True, False):
+            plan.set_graph(graph)
+            for name, kw in cases.items():
+                xg, xbuf, pad = _guarded(b.shape, torch.complex128)
+                x, infos = plan.cg_solve(d_phi, d_b, m, g, rho, tol, 5000, out=xg, **kw)
+                assert _canaries_intact(xbuf, pad), (dtype, name)
+                x2, infos2 = plan.cg_solve(d_phi, d_b, m, g, rho, tol, 5000, **kw)
+                assert torch.equal(x, x2) and [i.iterations for i in infos] == [i.iterations for i in infos2]
+                sigma = kw.get("sigma", 0.0)
+                for j in range(2):
+                    xj = x[j].cpu().numpy()
+                    res = rel(orc.apply_MdagM(phi128, xj, m, g, rho) + sigma * xj, b[j].astype(np.complex128))
+                    assert infos[j].converged and res <= (20 * tol if "pc" in name else tol * (1 + 1e-3)), (dtype, name, res)
+                if dtype == "c64" and name == "plain":
+                    assert infos[0].reliable_updates >= 1
+        xg, xbuf, pad = _guarded((3,) + b.shape, torch.complex128)
+        x, infos = plan.cg_solve_multishift(d_phi, d_b, m, g, [0.0, 0.3, 30.0], rho, tol, 5000, out=xg)
+        assert _canaries_intact(xbuf, pad)
+        x2, _ = plan.cg_solve_multishift(d_phi, d_b, m, g, [0.0, 0.3, 30.0], rho, tol, 5000)
+        assert torch.equal(x, x2)
+        assert all(i.converged and i.rel_residual_true <= tol * (1 + 1e-3) for row in infos for i in row)
+        a0, al, be = inp.rational_ladder(4, 1e-1, 1e2)
+        out, _ = plan.rational_apply(d_phi, d_b, m, g, a0, al, be, rho, tol, 5000)
+        out2, _ = plan.rational_apply(d_phi, d_b, m, g, a0, al, be, rho, tol, 5000, multishift=True)
+        assert rel(out2.cpu().numpy(), out.cpu().numpy()) <= (1e-8 if dtype == "c128" else 1e-4)
+        fg, fbuf, pad = _guarded(b.shape, plan.tdtype)
+        f = plan.fft4d(d_b, +1, True, out=fg)
+        qg, qbuf, qpad = _guarded(b.shape, plan.tdtype)
+        plan.apply_MdagM(d_phi, d_b, m, g, rho, out=qg)
+        assert _canaries_intact(fbuf, pad) and _canaries_intact(qbuf, qpad)
+        assert rel(plan.fft4d(f, -1, True).cpu().numpy(), b.astype(np.complex128)) <= 2 * TOL[dtype]
+        assert len(plan.locality_profile(0)) == 1 + sum(d // 2 for d in dims)
