@@ -169,4 +169,26 @@ __device__ __forceinline__ void grid_reduce(double v, const RedArgs& ra, int blk
   }
 }
 
+// The pass kernels (wz_p01.cuh) only leave their per-CTA partial: with one 512-thread CTA per SM, waiting for the
+// ticket (fence + atomic round trip) kept the whole SM idle for ~1 us per CTA, 6-7 % of passes C and E' (ncu source
+// view, profiles/r02_*).  The total and the scalar update are taken by k_finalize, a one-CTA-per-source launch
+// right behind the pass (wz_lib.cu: launch_p01); same fixed order of summation, no atomics.
+__device__ __forceinline__ void block_partial(double v, const RedArgs& ra, int blk, double* sh) {
+  double t = block_sum(v, sh);
+  if (threadIdx.x == 0) ra.partials[blk] = t;
+}
+
+constexpr int FINALIZE_NT = 256;
+template <int FIN>
+__global__ void __launch_bounds__(FINALIZE_NT) k_finalize(RedArgs red, int nblk, const CGState* gate) {
+  const int src = blockIdx.x;
+  if (gate && !cg_active(gate + src)) return;  // an idle source: its CTAs returned before writing partials
+  const RedArgs ra = red.for_source(src);
+  __shared__ double sh[33];
+  double acc = 0.0;
+  for (int i = threadIdx.x; i < nblk; i += blockDim.x) acc += ra.partials[i];
+  const double tot = block_sum(acc, sh);
+  if (threadIdx.x == 0) cg_finalize<FIN>(tot, ra.st, ra.store);
+}
+
 }  // namespace wz

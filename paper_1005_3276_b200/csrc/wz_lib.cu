@@ -350,6 +350,19 @@ wz_status launch_p01(wz_plan* pl, int kind, const P01Kern<R>& k, const P01Args<R
     k.fn<<<dim3((unsigned)nseg_tiles, (unsigned)nf), k.nt, k.smem, pl->lstream>>>(args);
   }
   WZ_CUDA(cudaGetLastError());
+  if (args.red.partials) {
+    // the pass left one partial per CTA (4 spin components x tiles per source): total + scalar update
+    const int nblk = 4 * nseg_tiles;
+    ProfScope ps(pl, WZ_K_OTHER);
+    switch (k.fin) {
+      case FIN_PQ: k_finalize<FIN_PQ><<<nb, FINALIZE_NT, 0, pl->lstream>>>(args.red, nblk, args.gate); break;
+      case FIN_RR: k_finalize<FIN_RR><<<nb, FINALIZE_NT, 0, pl->lstream>>>(args.red, nblk, args.gate); break;
+      case FIN_RRS: k_finalize<FIN_RRS><<<nb, FINALIZE_NT, 0, pl->lstream>>>(args.red, nblk, args.gate); break;
+      case FIN_PP: k_finalize<FIN_PP><<<nb, FINALIZE_NT, 0, pl->lstream>>>(args.red, nblk, args.gate); break;
+      default: k_finalize<FIN_STORE><<<nb, FINALIZE_NT, 0, pl->lstream>>>(args.red, nblk, args.gate); break;
+    }
+    WZ_CUDA(cudaGetLastError());
+  }
   return WZ_OK;
 }
 

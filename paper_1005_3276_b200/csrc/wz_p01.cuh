@@ -285,7 +285,7 @@ k_p01(const P01Args<R> a) {
     if constexpr (MODE == P01_FWDCG && FIN == FIN_PP) {
       // shifted solves: <p,p> of this source for alpha = rho / (||M p||^2 + sigma <p,p>)
       const int blk = comp * gridDim.x + bx;
-      grid_reduce<FIN_PP>(accp, a.red.for_source(src), blk, 4 * gridDim.x, red_sh);
+      block_partial(accp, a.red.for_source(src), blk, red_sh);  // k_finalize<FIN_PP> follows (launch_p01)
     }
   } else {
     // ---- inverse half: axis 1 first (from HBM), then axis 0 ----
@@ -458,7 +458,7 @@ k_p01(const P01Args<R> a) {
       }
       if (a.red.partials) {  // one reduction per source: its 4 spin components x all segments
         const int blk = comp * gridDim.x + bx;
-        grid_reduce<FIN>(acc, a.red.for_source(src), blk, 4 * gridDim.x, red_sh);
+        block_partial(acc, a.red.for_source(src), blk, red_sh);  // k_finalize<FIN> follows (launch_p01)
       }
     }
   }

@@ -15,6 +15,7 @@ template <typename R>
 struct P01Kern {
   void (*fn)(const P01Args<R>) = nullptr;
   int nt = 0, nseg = 0;
+  int fin = FIN_STORE;  // what k_finalize does with the kernel's reduction (if it has one)
   size_t smem = 0;
 };
 template <typename R>
@@ -73,7 +74,7 @@ P01Kern<R> make_p01_kern() {
   using C = P01Cfg<R, L0, L1, NSEG, T0, T1>;
   P01Kern<R> k;
   k.fn = k_p01<R, L0, L1, NSEG, T0, T1, MODE, FIN, IC>;
-  k.nt = C::NT; k.nseg = NSEG; k.smem = C::SMEM;
+  k.nt = C::NT; k.nseg = NSEG; k.smem = C::SMEM; k.fin = FIN;
   return k;
 }
 template <typename R, int L0, int L1, int IC = 0>
