@@ -350,7 +350,7 @@ wz_status launch_p01(wz_plan* pl, int kind, const P01Kern<R>& k, const P01Args<R
     k.fn<<<dim3((unsigned)nseg_tiles, (unsigned)nf), k.nt, k.smem, pl->lstream>>>(args);
   }
   WZ_CUDA(cudaGetLastError());
-  if (args.red.partials) {
+  if (args.red.partials && k.split_finalize) {
     // the pass left one partial per CTA (4 spin components x tiles per source): total + scalar update
     const int nblk = 4 * nseg_tiles;
     ProfScope ps(pl, WZ_K_OTHER);

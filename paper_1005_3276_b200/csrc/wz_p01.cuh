@@ -147,6 +147,16 @@ struct p01_minb {  // TPL = 2: 16 values per thread, 64 registers; TPL = 1: 32 v
   static constexpr int v = (sizeof(R) == 4 && L0 == 32 && L1 == 32 && NT <= want) ? (want / NT) : 1;
 };
 
+// Where the total of a reduction is taken.  Large tiles (one or two big CTAs per SM, hundreds of microseconds per
+// launch): the pass leaves per-CTA partials and a one-CTA-per-source kernel right behind it takes the total (the
+// fence + ticket round trip of the in-kernel version kept the SM idle ~1 us per CTA: 6-7 % of passes C and E' at
+// 32^4).  Small tiles (launch-bound lattices, a few microseconds per launch): the last CTA to arrive takes the total
+// inside the pass (one kernel node fewer per reduction in the iteration graph).
+template <int L0, int L1>
+struct p01_split_finalize {
+  static constexpr bool v = (L0 * L1 >= 1024);
+};
+
 template <typename R, int L0, int L1, int NSEG, int T0, int T1, int MODE, int FIN, int IC = 0>
 __global__ void __launch_bounds__(P01Cfg<R, L0, L1, NSEG, T0, T1>::NT, p01_minb<R, L0, L1, P01Cfg<R, L0, L1, NSEG, T0, T1>::NT, T0>::v)
 k_p01(const P01Args<R> a) {
@@ -285,7 +295,8 @@ k_p01(const P01Args<R> a) {
     if constexpr (MODE == P01_FWDCG && FIN == FIN_PP) {
       // shifted solves: <p,p> of this source for alpha = rho / (||M p||^2 + sigma <p,p>)
       const int blk = comp * gridDim.x + bx;
-      block_partial(accp, a.red.for_source(src), blk, red_sh);  // k_finalize<FIN_PP> follows (launch_p01)
+      if constexpr (p01_split_finalize<L0, L1>::v) block_partial(accp, a.red.for_source(src), blk, red_sh);  // k_finalize<FIN_PP> follows (launch_p01)
+      else grid_reduce<FIN_PP>(accp, a.red.for_source(src), blk, 4 * gridDim.x, red_sh);
     }
   } else {
     // ---- inverse half: axis 1 first (from HBM), then axis 0 ----
@@ -458,7 +469,8 @@ k_p01(const P01Args<R> a) {
       }
       if (a.red.partials) {  // one reduction per source: its 4 spin components x all segments
         const int blk = comp * gridDim.x + bx;
-        block_partial(acc, a.red.for_source(src), blk, red_sh);  // k_finalize<FIN> follows (launch_p01)
+        if constexpr (p01_split_finalize<L0, L1>::v) block_partial(acc, a.red.for_source(src), blk, red_sh);  // k_finalize<FIN> follows (launch_p01)
+        else grid_reduce<FIN>(acc, a.red.for_source(src), blk, 4 * gridDim.x, red_sh);
       }
     }
   }

@@ -16,6 +16,7 @@ struct P01Kern {
   void (*fn)(const P01Args<R>) = nullptr;
   int nt = 0, nseg = 0;
   int fin = FIN_STORE;  // what k_finalize does with the kernel's reduction (if it has one)
+  bool split_finalize = false;  // the kernel leaves partials; k_finalize<fin> must follow (p01_split_finalize)
   size_t smem = 0;
 };
 template <typename R>
@@ -74,7 +75,7 @@ P01Kern<R> make_p01_kern() {
   using C = P01Cfg<R, L0, L1, NSEG, T0, T1>;
   P01Kern<R> k;
   k.fn = k_p01<R, L0, L1, NSEG, T0, T1, MODE, FIN, IC>;
-  k.nt = C::NT; k.nseg = NSEG; k.smem = C::SMEM; k.fin = FIN;
+  k.nt = C::NT; k.nseg = NSEG; k.smem = C::SMEM; k.fin = FIN; k.split_finalize = p01_split_finalize<L0, L1>::v;
   return k;
 }
 template <typename R, int L0, int L1, int IC = 0>
