@@ -184,6 +184,19 @@ wz_status wz_rational_apply_multishift(wz_plan *plan, const void *phi, const voi
                                        const double *alphas, const double *betas, int nshift, double pc_cutoff,
                                        double tol, int max_iter, int nbatch, wz_cg_info *info);
 
+/* ---- Defect correction ("mixed precision conjugate gradient") ----
+ * wz_cg_solve_dc (WZ_C64 plans; WZ_EINVAL otherwise): a complex128 outer loop around complex64 inner solves,
+ *   X = 0;  repeat:  d = b - M^dag M X  in complex128;  stop if ||d|| <= tol ||b||;
+ *                    plain complex64 CG (no reliable updates) on M^dag M e = d to ||r|| <= inner_tol ||d||;  X += e.
+ * The other route to double-precision tolerances with complex64 vectors, next to the reliable updates of
+ * wz_cg_solve (which keep the search direction across the corrections; this loop restarts the Krylov space).
+ * 0 < inner_tol < 1.  info.iterations = inner iterations in total, info.reliable_updates = outer corrections,
+ * both residual fields = ||b - M^dag M x|| / ||b|| recomputed in complex128.  x: complex128, must not alias b.
+ * Synchronises the stream; WZ_ENOTCONVERGED if the iteration budget max_iter ran out. */
+wz_status wz_cg_solve_dc(wz_plan *plan, const void *phi, const void *b, void *x,
+                         const double m[2], const double g[2], double rho,
+                         double tol, double inner_tol, int max_iter, int nbatch, wz_cg_info *info);
+
 /* ---- Locality probe (Eq. 3.9-3.11, Fig. 1) ----
  * wz_apply_Dslash: out = Dslash in = (1 - D2/2)^-1 D1 in (the fermion matrix at m = g = 0); in != out.
  * wz_locality_profile: psi = Dslash eta for a unit point source at the origin in spin component

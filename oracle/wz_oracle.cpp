@@ -947,4 +947,67 @@ int orc_cg_multishift(int method, const int* L, const double* phi, const double*
   return 0;
 }
 
+// ----------------------------------------------------------------------------
+// O9 (NEXT-3). Defect correction: complex128 outer loop around a complex64 inner CG
+// (single precision "could however be used for a mixed precision conjugate
+// gradient", ref. [37]; SURVEY 8(f) NEXT-3 "complex64 inner / complex128 outer").  Unlike the
+// reliable updates of O4' the inner solver is restarted from scratch at every outer step:
+//   X = 0;  r = b                                   (complex128)
+//   outer step:  stop if ||r|| <= tol ||b||;
+//                inner: plain CG (the loop of orc_cg, NO reliable updates) on A e = round64(r), e_0 = 0,
+//                       every vector rounded to float after every update, reductions in double,
+//                       until its recursive residual <= inner_tol * ||round64(r)|| (or the iteration budget ends);
+//                X += e;  r = b - A X              (complex128)
+// info->iterations = inner iterations in total, info->reliable_updates = outer corrections taken.
+// ----------------------------------------------------------------------------
+int orc_cg_dc(int method, const int* L, const double* phi, const double* b_, double* X_,
+              const double* m, const double* g, double rho, double tol, double inner_tol, int max_iter,
+              orc_cg_info* info) {
+  const long V = (long)L[0] * L[1] * L[2] * L[3];
+  const long n = 4 * V;
+  const cd* b = reinterpret_cast<const cd*>(b_);
+  cd* X = reinterpret_cast<cd*>(X_);
+  std::vector<cd> R(b, b + n), e(n), r(n), p(n), q(n);
+  for (long i = 0; i < n; ++i) X[i] = 0.0;
+  const double bnorm = std::sqrt(dot_re(b, b, n));
+  double Rnorm = bnorm;
+  int total = 0, outer = 0, converged = (bnorm == 0.0);
+  while (!converged && total < max_iter) {
+    // inner solve A e = round64(R)
+    for (long i = 0; i < n; ++i) { r[i] = round_c64(R[i]); p[i] = r[i]; e[i] = 0.0; }
+    double rr = dot_re(r.data(), r.data(), n);
+    const double stop = inner_tol * std::sqrt(rr);
+    while (total < max_iter) {
+      ++total;
+      int rc = orc_apply_MdagM(method, L, phi, m, g, rho, reinterpret_cast<double*>(p.data()),
+                               reinterpret_cast<double*>(q.data()));
+      if (rc) return rc;
+      for (long i = 0; i < n; ++i) q[i] = round_c64(q[i]);
+      const double alpha = rr / dot_re(p.data(), q.data(), n);
+      for (long i = 0; i < n; ++i) {
+        e[i] = round_c64(e[i] + alpha * p[i]);
+        r[i] = round_c64(r[i] - alpha * q[i]);
+      }
+      const double rr_new = dot_re(r.data(), r.data(), n);
+      if (std::sqrt(rr_new) <= stop) break;
+      const double beta = rr_new / rr;
+      rr = rr_new;
+      for (long i = 0; i < n; ++i) p[i] = round_c64(r[i] + beta * p[i]);
+    }
+    ++outer;
+    for (long i = 0; i < n; ++i) X[i] += e[i];
+    orc_apply_MdagM(method, L, phi, m, g, rho, X_, reinterpret_cast<double*>(q.data()));
+    double tr = 0.0;
+    for (long i = 0; i < n; ++i) { R[i] = b[i] - q[i]; tr += std::norm(R[i]); }
+    Rnorm = std::sqrt(tr);
+    if (Rnorm <= tol * bnorm) converged = 1;
+  }
+  info->iterations = total;
+  info->reliable_updates = outer;
+  info->converged = converged;
+  info->rel_residual_recursive = bnorm > 0 ? Rnorm / bnorm : 0.0;
+  info->rel_residual_true = bnorm > 0 ? Rnorm / bnorm : 0.0;
+  return 0;
+}
+
 }  // extern "C"

@@ -326,3 +326,21 @@ def cg_multishift(phi, b, m, g, sigmas, rho=1.0, tol=1e-10, max_iter=100000, met
     out = [CGInfo(i.iterations, i.reliable_updates, bool(i.converged), i.rel_residual_recursive,
                   i.rel_residual_true, np.zeros(0)) for i in infos[:d]]
     return X, out, int(mv.value)
+
+
+def cg_dc(phi, b, m, g, rho=1.0, tol=1e-10, inner_tol=1e-3, max_iter=100000, method="auto"):
+    """Defect correction (oracle O9): complex128 outer loop, complex64-rounded inner CG restarted at every
+    outer step.  Returns (X, CGInfo) with iterations = inner iterations in total and reliable_updates =
+    the number of outer corrections."""
+    phi = np.ascontiguousarray(phi, dtype=np.complex128)
+    b = np.ascontiguousarray(b, dtype=np.complex128)
+    dims = phi.shape
+    X = np.zeros_like(b)
+    info = _Info()
+    rc = lib().orc_cg_dc(_method(dims, method), _dims(dims), _dp(phi), _dp(b), _dp(X), _c2(m), _c2(g),
+                         ctypes.c_double(rho), ctypes.c_double(tol), ctypes.c_double(inner_tol), int(max_iter),
+                         ctypes.byref(info))
+    if rc:
+        raise ValueError("oracle cg_dc failed")
+    return X, CGInfo(info.iterations, info.reliable_updates, bool(info.converged), info.rel_residual_recursive,
+                     info.rel_residual_true, np.zeros(0))

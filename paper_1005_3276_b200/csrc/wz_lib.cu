@@ -832,8 +832,10 @@ int vec_grid(long n_real, int per_thread) {
 template <typename R>
 wz_status cg_batch(wz_plan* pl, const cpx<R>* phi, const cpx<R>* b, cpx<double>* X, const double m[2],
                    const double g[2], double rho, double tol, int max_iter, int nb, wz_cg_info* info,
-                   bool pc, double sigma = 0.0, const double* tol_per_source = nullptr) {
+                   bool pc, double sigma = 0.0, const double* tol_per_source = nullptr, bool reliable = true) {
   // tol_per_source (optional, nb entries): overrides tol source by source (defect-correction solves)
+  // reliable = false (complex64 only): plain CG on the recursive residual, no reliable updates (the inner solver of
+  // wz_cg_solve_dc); X still receives the float iterate folded into complex128 at exit
   // sigma: shift of the system (M^dag M + sigma) x = b (Eq. 7.13); with pc the system
   // iterated on is Eq. 7.14, (Mtilde^dag Mtilde + sigma (M0^-1)^dag M0^-1) xtilde = btilde
   constexpr bool kRU = (sizeof(R) == 4);
@@ -848,7 +850,7 @@ wz_status cg_batch(wz_plan* pl, const cpx<R>* phi, const cpx<R>* b, cpx<double>*
   std::vector<CGState> h(nb);
   memset(h.data(), 0, sizeof(CGState) * nb);
   for (int j = 0; j < nb; ++j) {
-    h[j].tol = tol_per_source ? tol_per_source[j] : tol; h[j].delta = kDelta; h[j].max_iter = max_iter; h[j].use_ru = kRU ? 1 : 0;
+    h[j].tol = tol_per_source ? tol_per_source[j] : tol; h[j].delta = kDelta; h[j].max_iter = max_iter; h[j].use_ru = (kRU && reliable) ? 1 : 0;
     h[j].true_rr = -1.0; h[j].shift = pc ? 0.0 : sigma;  // pc: the shift is inside pass C's reduction
     if (max_iter == 0) h[j].stop = 1;
   }
@@ -1030,7 +1032,7 @@ wz_status cg_batch(wz_plan* pl, const cpx<R>* phi, const cpx<R>* b, cpx<double>*
     if (!pc) {
       // true residual at exit: complex64 solves that converged carry it from their last
       // reliable update; everything else recomputes it now
-      if (kRU && fin[j].converged) continue;
+      if (kRU && reliable && fin[j].converged) continue;
       if ((s = residual128(j, kRU)) != WZ_OK) return s;  // C64, not converged: fold xs into X first
       continue;
     }
@@ -1329,6 +1331,98 @@ extern "C" wz_status wz_cg_solve_multishift(wz_plan* pl, const void* phi, const 
   for (int i = 0; i < nshift * nbatch; ++i)
     if (!info[i].converged) return WZ_ENOTCONVERGED;
   return WZ_OK;
+}
+
+// =============================== defect correction ==============================
+// complex128 outer loop around complex64 inner solves restarted at every step (oracle O9; PAPER.md:957;
+// SURVEY 8(f) NEXT-3 "complex64 inner / complex128 outer").  WZ_C64 plans.
+extern "C" wz_status wz_cg_solve_dc(wz_plan* pl, const void* phi_, const void* b_, void* x_, const double m[2],
+                                    const double g[2], double rho, double tol, double inner_tol, int max_iter,
+                                    int nbatch, wz_cg_info* info) {
+  g_err[0] = 0;
+  if (!pl || !phi_ || !b_ || !x_ || !m || !g || !info) return WZ_EINVAL;
+  if (pl->dtype != WZ_C64) return WZ_EINVAL;
+  if (!(rho > 0.0 && rho < 2.0) || !(tol > 0.0) || !(inner_tol > 0.0 && inner_tol < 1.0) || max_iter < 0) return WZ_EINVAL;
+  if (nbatch < 0 || nbatch > pl->max_batch || x_ == b_) return WZ_EINVAL;
+  if (nbatch == 0) return WZ_OK;
+  WZ_ON_DEVICE(pl);
+  const int nb = nbatch;
+  const long n = 8 * pl->V;
+  const size_t n1 = (size_t)4 * pl->V;
+  cudaStream_t st = pl->stream;
+  const cpx<float>* phi = (const cpx<float>*)phi_;
+  const cpx<float>* b = (const cpx<float>*)b_;
+  cpx<double>* X = (cpx<double>*)x_;
+  const int gv2 = vec_grid(n, 2);
+  if (!pl->ms_true && !dev_alloc(pl, &pl->ms_true, (size_t)WZ_MAX_SHIFTS * pl->max_batch)) return WZ_ENOMEM;
+  if (!pl->ms_rhs) {
+    float* a = nullptr;
+    if (!dev_alloc(pl, &a, (size_t)pl->max_batch * 2 * n1)) return WZ_ENOMEM;
+    pl->ms_rhs = a;
+  }
+  if (!pl->ms_e && !dev_alloc(pl, &pl->ms_e, (size_t)pl->max_batch * n1)) return WZ_ENOMEM;
+  {
+    ProfScope ps(pl, WZ_K_OTHER);
+    k_f2d<<<vec_grid(2 * pl->V, 1), CGK_NT, 0, st>>>((double*)pl->phi128, (const float*)phi, 2 * pl->V);
+  }
+  WZ_CUDA(cudaGetLastError());
+  WZ_CUDA(cudaMemsetAsync(X, 0, sizeof(cpx<double>) * n1 * nb, st));
+  std::vector<double> tr(nb, 0.0), bnorm(nb, 0.0), tolj(nb);
+  std::vector<int> done(nb, 0), iters(nb, 0), outer(nb, 0);
+  std::vector<wz_cg_info> inner(nb);
+  for (;;) {
+    {  // defects d_j = b_j - A X_j in complex128, rounded to complex64 as the inner right-hand sides
+      struct Override {
+        wz_plan* p;
+        explicit Override(wz_plan* q) : p(q) { p->prof_override = WZ_K_OTHER; }
+        ~Override() { p->prof_override = -1; }
+      } ov(pl);
+      for (int j = 0; j < nb; ++j) {
+        if (done[j]) continue;
+        wz_status s = apply_MdagM_impl<double>(pl, pl->phi128, m, g, rho, X + j * n1, pl->q128, 1, false);
+        if (s != WZ_OK) return s;
+        RedArgs ra = red_of(pl).for_source(j);
+        ra.store = pl->ms_true + j;
+        ProfScope ps(pl, WZ_K_OTHER);
+        k_resid<float, float, FIN_STORE><<<dim3(gv2, 1), CGK_NT, 0, st>>>((const float*)(b + j * n1), (const double*)pl->q128,
+                                                                          (float*)pl->ms_rhs + j * n, n, ra);
+        WZ_CUDA(cudaGetLastError());
+      }
+    }
+    WZ_CUDA(cudaMemcpyAsync(tr.data(), pl->ms_true, sizeof(double) * nb, cudaMemcpyDeviceToHost, st));
+    WZ_CUDA(cudaStreamSynchronize(st));
+    bool all_done = true;
+    int spent = 0;
+    for (int j = 0; j < nb; ++j) {
+      if (outer[j] == 0 && !done[j]) bnorm[j] = std::sqrt(tr[j]);  // X = 0: the defect is b itself
+      if (!done[j] && (bnorm[j] == 0.0 || std::sqrt(tr[j]) <= tol * bnorm[j])) done[j] = 1;
+      if (!done[j]) all_done = false;
+      spent = std::max(spent, iters[j]);
+    }
+    if (all_done || spent >= max_iter) break;
+    for (int j = 0; j < nb; ++j) tolj[j] = done[j] ? 1e30 : inner_tol;
+    wz_status s = cg_batch<float>(pl, phi, (const cpx<float>*)pl->ms_rhs, pl->ms_e, m, g, rho, inner_tol, max_iter - spent,
+                                  nb, inner.data(), false, 0.0, tolj.data(), false);
+    if (s != WZ_OK) return s;
+    for (int j = 0; j < nb; ++j) {
+      if (done[j]) continue;
+      ProfScope ps(pl, WZ_K_OTHER);
+      k_rat_term<double><<<dim3(gv2, 1), CGK_NT, 0, st>>>((double*)(X + j * n1), (const double*)(pl->ms_e + j * n1), 1.0, n, 0);
+      WZ_CUDA(cudaGetLastError());
+      iters[j] += inner[j].iterations;
+      outer[j] += 1;
+    }
+  }
+  bool ok = true;
+  for (int j = 0; j < nb; ++j) {
+    info[j].iterations = iters[j];
+    info[j].reliable_updates = outer[j];
+    info[j].converged = done[j];
+    info[j].rel_residual_true = bnorm[j] > 0 ? std::sqrt(tr[j]) / bnorm[j] : 0.0;
+    info[j].rel_residual_recursive = info[j].rel_residual_true;
+    if (!done[j]) ok = false;
+  }
+  return ok ? WZ_OK : WZ_ENOTCONVERGED;
 }
 
 static wz_status cg_solve_any(wz_plan* pl, const void* phi, const void* b, void* x, const double m[2],

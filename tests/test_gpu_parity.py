@@ -1027,3 +1027,41 @@ def test_small_solves_all_paths(wz, orc, inp, dims):
         assert _canaries_intact(fbuf, pad) and _canaries_intact(qbuf, qpad)
         assert rel(plan.fft4d(f, -1, True).cpu().numpy(), b.astype(np.complex128)) <= 2 * TOL[dtype]
         assert len(plan.locality_profile(0)) == 1 + sum(d // 2 for d in dims)
+
+
+# ---- NEXT-3: defect correction, complex64 inner / complex128 outer (oracle O9) ----
+
+@pytest.mark.parametrize("dims,inner_tol", [((8, 8, 8, 8), 1e-3), ((16, 16, 16, 16), 1e-3), ((8, 8, 8, 8), 1e-1)])
+def test_cg_dc_vs_oracle(wz, orc, inp, dims, inner_tol):
+    """complex64 inner solves restarted inside a complex128 outer loop, to the double-precision tolerance
+    1e-10: the same number of outer corrections as the oracle's loop, inner iterations within 5 % (G10),
+    true residual recomputed by the oracle, solution against the complex128 oracle; and side by side
+    with the reliable-update route of wz_cg_solve to the same tolerance."""
+    m, g, rho, tol = 0.05, 1.0, 1.0, 1e-10
+    phi = inp.make_phi(2, dims, 0.3, np.complex64)
+    b = inp.make_sources(2, 2, dims, np.complex64)
+    plan = wz.Plan(dims, "c64", 2)
+    d_phi, d_b = torch.from_numpy(phi).cuda(), torch.from_numpy(b).cuda()
+    x, infos = plan.cg_solve_dc(d_phi, d_b, m, g, rho, tol, inner_tol, 200000)
+    xr, iru = plan.cg_solve(d_phi, d_b, m, g, rho, tol, 200000)
+    x = x.cpu().numpy()
+    phi128 = phi.astype(np.complex128)
+    for j in range(2):
+        bj = b[j].astype(np.complex128)
+        Xo, io = orc.cg_dc(phi128, bj, m, g, rho, tol, inner_tol, 200000)
+        true_res = rel(orc.apply_MdagM(phi128, x[j], m, g, rho), bj)
+        print("dc %s inner_tol %g: inner iterations gpu=%d oracle=%d, outer gpu=%d oracle=%d, true residual %.2e; "
+              "reliable-update route: %d iterations" % (dims, inner_tol, infos[j].iterations, io.iterations,
+                                                          infos[j].reliable_updates, io.reliable_updates, true_res,
+                                                          iru[j].iterations))
+        assert infos[j].converged and io.converged
+        assert true_res <= tol * (1 + 1e-3) and abs(true_res - infos[j].rel_residual_true) <= 0.05 * tol
+        assert abs(infos[j].reliable_updates - io.reliable_updates) <= 1
+        assert abs(infos[j].iterations - io.iterations) <= max(2, int(0.05 * io.iterations))
+        assert rel(x[j], Xo) <= 1e-7
+    with pytest.raises(wz.WZError) as e:
+        wz.Plan(dims, "c128", 1).cg_solve_dc(d_phi.to(torch.complex128), d_b[:1].to(torch.complex128), m, g)
+    assert e.value.status == wz.WZ_EINVAL
+    with pytest.raises(wz.WZError) as e:
+        plan.cg_solve_dc(d_phi, d_b, m, g, rho, tol, 1.5)
+    assert e.value.status == wz.WZ_EINVAL

@@ -63,3 +63,32 @@ def test_cg_c64ru_reaches_true_tolerance(orc):
     # the complex64 variant needs at least as many iterations as exact-arithmetic-like complex128
     assert info.iterations >= infod.iterations - 2
     assert info.iterations <= 1.3 * infod.iterations + 20
+
+
+def test_cg_dc_reaches_double_tolerance_and_matches_dense_solve(orc):
+    """O9, defect correction (NEXT-3): complex64 inner solves inside a complex128 outer loop reach a
+    double-precision tolerance; the solution against the dense solve, the reported residual against an
+    independently recomputed one, and the structure of the loop (several outer corrections, each worth
+    about inner_tol)."""
+    dims = (4, 4, 4, 4)
+    cfg = inputs.CONFIGS[1]
+    phi = inputs.make_phi(1, dims, cfg["sigma"]).astype(np.complex64).astype(np.complex128)
+    b = inputs.make_source(1, 0, dims).astype(np.complex64).astype(np.complex128)
+    M = dense_route.fermion_matrix_dense(dims, phi, cfg["m"], cfg["g"], 1.0)
+    A = M.conj().T @ M
+    xd = np.linalg.solve(A, b.reshape(-1)).reshape(b.shape)
+    X, info = orc.cg_dc(phi, b, cfg["m"], cfg["g"], 1.0, 1e-10, 1e-3, 20000, "naive")
+    assert info.converged and info.rel_residual_true <= 1e-10
+    res = np.linalg.norm(b.reshape(-1) - A @ X.reshape(-1)) / np.linalg.norm(b)
+    assert abs(res - info.rel_residual_true) <= 1e-3 * res + 2e-12  # rounding floor of the dense matrix (eps * cond)
+    assert np.linalg.norm(X - xd) <= 1e-7 * np.linalg.norm(xd)
+    assert 3 <= info.reliable_updates <= 6          # 1e-10 in steps of about 1e-3
+    # against the two other routes to the same tolerance: restarts cost iterations (never fewer than plain CG)
+    _, i128 = orc.cg(phi, b, cfg["m"], cfg["g"], 1.0, 1e-10, 20000, "naive")
+    _, iru = orc.cg_c64ru(phi, b, cfg["m"], cfg["g"], 1.0, 1e-10, 20000, 0.1, "naive")
+    assert info.iterations >= i128.iterations and iru.iterations >= i128.iterations - 2
+    # a loose inner tolerance means more outer steps; one outer step with inner_tol <= tol is plain complex64 CG
+    _, i2 = orc.cg_dc(phi, b, cfg["m"], cfg["g"], 1.0, 1e-10, 1e-1, 20000, "naive")
+    assert i2.converged and i2.reliable_updates > info.reliable_updates
+    _, i3 = orc.cg_dc(phi, b, cfg["m"], cfg["g"], 1.0, 1e-5, 1e-7, 20000, "naive")
+    assert i3.converged and i3.reliable_updates == 1
