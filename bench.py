@@ -234,6 +234,66 @@ def small_config_table(dev, full=False):
     return table
 
 
+def paper_lattice_table(dev):
+    """The paper's own lattices (Tables V, VI): 4D FFT of a spinor field (Gflop/s by the
+    paper's 5 N log2 N with N = 4V, reading G13) and the CG solve at Table VI's parameters m = 1, g = 1/5 with and
+    without preconditioning, single and double precision.  Synthetic Gaussian phi (sigma = 0.5) stands in for the
+    paper's RHMC configurations; the paper's numbers (GTX 285) ride along as context."""
+    import math
+
+    import numpy as np
+    import torch
+
+    from paper_1005_3276_b200 import inputs, wz
+
+    paper = {  # (seconds, iterations) NPC / PC and FFT Gflop/s "cuFFT" / "ours", Tables VI and V
+        ("8^3x32", "c64"): {"npc": (1.3, 830), "pc": (0.038, 8), "fft_gflops": (6.9, 24)},
+        ("8^3x32", "c128"): {"npc": (4.9, 1600), "pc": (0.13, 15), "fft_gflops": (4.4, 11)},
+        ("16^3x32", "c64"): {"npc": (7.1, 870), "pc": (0.20, 8), "fft_gflops": (14, 71)},
+        ("16^3x32", "c128"): {"npc": (31, 1800), "pc": (0.74, 15), "fft_gflops": (10, 35)},
+        ("32^3x64", "c64"): {"npc": (420, 1600), "pc": (6.8, 8), "fft_gflops": (20, None)},
+        ("32^3x64", "c128"): {"npc": (2200, 3900), "pc": (25, 15), "fft_gflops": (10, None)},
+    }
+    out = {}
+    for name, dims in (("8^3x32", (32, 8, 8, 8)), ("16^3x32", (32, 16, 16, 16)), ("32^3x64", (64, 32, 32, 32))):
+        for dtype, tol in (("c64", 1e-6), ("c128", 1e-12)):
+            npdt = np.complex64 if dtype == "c64" else np.complex128
+            phi = torch.from_numpy(inputs.make_phi(5, dims, 0.5, npdt)).to(dev)
+            b = torch.from_numpy(inputs.make_sources(5, 1, dims, npdt)).to(dev)
+            plan = wz.Plan(dims, dtype, 1, dev)
+            row = {"paper_GTX285": paper[(name, dtype)]}
+            f = torch.empty_like(b)
+            ts = []
+            for i in range(8):
+                a, e = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record()
+                plan.fft4d(b, +1, True, out=f)
+                e.record()
+                e.synchronize()
+                if i >= 3:
+                    ts.append(a.elapsed_time(e) * 1e-3)
+            n4 = b.numel()
+            row["fft4d_us"] = 1e6 * statistics.median(ts)
+            row["fft4d_gflops_5NlogN"] = 5.0 * n4 * math.log2(n4 / 4) / statistics.median(ts) / 1e9
+            for pc in (False, True):
+                best, infos = None, None
+                for rep in range(2):
+                    a, e = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    a.record()
+                    _, infos = plan.cg_solve(phi, b, 1.0, 0.2, 1.0, tol, 100000, raise_on_fail=False, precondition=pc)
+                    e.record()
+                    e.synchronize()
+                    t = a.elapsed_time(e) * 1e-3
+                    best = t if best is None else min(best, t)
+                row["pc" if pc else "npc"] = {"secs": best, "iterations": infos[0].iterations,
+                                              "true_residual": infos[0].rel_residual_true,
+                                              "converged": infos[0].converged}
+            row["pc_speedup"] = row["npc"]["secs"] / row["pc"]["secs"]
+            plan.close()
+            out["%s_%s" % (name, dtype)] = row
+    return out
+
+
 def oracle_iters_for(cfg):
     V = 1
     for d in cfg["dims"]:
@@ -449,6 +509,7 @@ def run_wz(args):
                "all_cores": oracle_pieces(cfg, 0), "one_thread": oracle_pieces(cfg, 1)}
         if not args.no_extras:
             extras["other_configs"] = small_config_table(dev, args.full_table)
+            extras["paper_lattices_tables_V_VI"] = paper_lattice_table(dev)
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
@@ -571,28 +632,44 @@ def time_preconditioned(plan, d_phi, d_b, d_x, cfg, plain_secs):
 
 
 def time_rational(plan, d_phi, d_b, d_x, cfg):
-    """NEXT-2 (Eq. 7.6-7.7, 927-950, Table VII): the degree-20 rational sum at the paper's
-    heatbath parameters m = 1, g = 0.1 for the whole batch -- one solve per shift, preconditioned
-    (Eq. 7.14) up to beta = 100, plain above.  The shifts are a synthetic geometric ladder
-    (inputs.rational_ladder): the paper's coefficients are not printed."""
+    """NEXT-2 (Eq. 7.6-7.7, 927-950, Table VII): the degree-20 rational sum, three ways --
+    one plain solve per shift (Eq. 7.13), the paper's rule (preconditioned, Eq. 7.14, up to beta = 100, plain
+    above), and multi-shift CG (all shifts above the cutoff, or all shifts, from one Krylov space) -- at the
+    paper's heatbath parameters m = 1, g = 0.1 for the whole batch and at the workload's own coupling for two
+    sources.  The shifts are a synthetic geometric ladder (inputs.rational_ladder): the paper's coefficients
+    are not printed."""
     import torch
 
     from paper_1005_3276_b200 import inputs
 
     a0, al, be = inputs.rational_ladder(20, 1e-2, 1e3)
-    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    a.record()
-    _, infos = plan.rational_apply(d_phi, d_b, 1.0, 0.1, a0, al, be, cfg["rho"], cfg["tol"], 5000, out=d_x,
-                                   raise_on_fail=False)
-    b.record()
-    b.synchronize()
-    its = [[i.iterations for i in row] for row in infos]
-    return {"secs_batch": a.elapsed_time(b) * 1e-3, "sources": len(its[0]), "shifts": 20,
-            "iterations_total_per_source": sum(max(row) for row in its),
-            "iterations_per_shift_max": [max(row) for row in its],
-            "all_converged": all(i.converged for row in infos for i in row),
-            "worst_true_residual": max(i.rel_residual_true for row in infos for i in row),
-            "paper": "Table VII, GTX 285, single: 360-540 iterations in total over 20 shifts, 0.93-220 s"}
+
+    def run(phi, b, out, m, g, cutoff, ms, max_iter):
+        a, e = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        _, infos = plan.rational_apply(phi, b, m, g, a0, al, be, cfg["rho"], cfg["tol"], max_iter, out=out,
+                                       raise_on_fail=False, pc_cutoff=cutoff, multishift=ms)
+        e.record()
+        e.synchronize()
+        its = [[i.iterations for i in row] for row in infos]
+        return {"secs": a.elapsed_time(e) * 1e-3, "sources": len(its[0]),
+                "iterations_per_shift_max": [max(row) for row in its],
+                "iterations_sum_over_shifts": sum(max(row) for row in its),
+                "all_converged": all(i.converged for row in infos for i in row),
+                "worst_true_residual": max(i.rel_residual_true for row in infos for i in row)}
+
+    res = {"shifts": 20, "paper": "Table VII, GTX 285, single: 360-540 iterations in total over 20 shifts, 0.93-220 s"}
+    res["table_VII_parameters_m1_g0.1"] = {
+        "paper_rule_pc_up_to_100": run(d_phi, d_b, d_x, 1.0, 0.1, 100.0, False, 5000),
+        "multishift_above_100": run(d_phi, d_b, d_x, 1.0, 0.1, 100.0, True, 5000),
+        "multishift_all_shifts": run(d_phi, d_b, d_x, 1.0, 0.1, -1.0, True, 5000),
+        "plain_solve_per_shift": run(d_phi, d_b, d_x, 1.0, 0.1, -1.0, False, 5000)}
+    b2, x2 = d_b[:2].contiguous(), d_x[:2].contiguous()
+    res["workload_coupling_m%g_g%g_2_sources" % (cfg["m"], cfg["g"])] = {
+        "paper_rule_pc_up_to_100": run(d_phi, b2, x2, cfg["m"], cfg["g"], 100.0, False, 100000),
+        "multishift_all_shifts": run(d_phi, b2, x2, cfg["m"], cfg["g"], -1.0, True, 100000),
+        "plain_solve_per_shift": run(d_phi, b2, x2, cfg["m"], cfg["g"], -1.0, False, 100000)}
+    return res
 
 
 def time_mixed(plan, d_phi, d_b, cfg, dev, nsrc=2):
