@@ -30,6 +30,7 @@ void p01f([[maybe_unused]] std::vector<P01Entry<float>>& v) {
   v.push_back(make_p01<R, 64, 64, 4096>());
   v.push_back(make_p01<R, 64, 64>());
   v.push_back(make_p01<R, 64, 32>());
+  v.push_back(make_p01<R, 64, 1>());  // single-axis passes of the 64x64 lattices (wz_lib.cu: pass01)
 #elif WZ_MOD == 2
   v.push_back(make_p01<R, 4, 4>());
   v.push_back(make_p01<R, 8, 8>());
@@ -47,6 +48,7 @@ void p01d([[maybe_unused]] std::vector<P01Entry<double>>& v) {
   v.push_back(make_p01<R, 32, 32, 1024>());
   v.push_back(make_p01<R, 48, 24, 576>());
   v.push_back(make_p01<R, 64, 64, 4096>());
+  v.push_back(make_p01<R, 64, 1>());  // single-axis passes of the 64x64 lattices (wz_lib.cu: pass01)
 #elif WZ_MOD == 4
   v.push_back(make_p01<R, 4, 4>());
   v.push_back(make_p01<R, 8, 8>());
@@ -69,7 +71,7 @@ void p23f([[maybe_unused]] std::vector<P23Entry<float>>& v) {
   v.push_back(make_p23<R, 16, 16>());
   v.push_back(make_p23<R, 32, 32>());
   v.push_back(make_p23<R, 24, 24>());
-  v.push_back(make_p23<R, 64, 64>());
+  v.push_back(make_p23<R, 64, 64, 2>());  // one component pair per CTA (67 KB): three CTAs per SM instead of one
 #endif
 }
 void p23d([[maybe_unused]] std::vector<P23Entry<double>>& v) {

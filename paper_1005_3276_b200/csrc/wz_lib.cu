@@ -109,6 +109,10 @@ template <typename R>
 struct OpWS {
   const P01Entry<R>* p01 = nullptr;
   const P23Entry<R>* p23 = nullptr;
+  // single-axis decomposition of the (x0,x1) pass (64x64 lattices: a two-axis tile with runs longer than 32 bytes does
+  // not fit in shared memory): p0s transforms axis 0 (all modes; inner volume L1*I), p1s axis 1 (x0 slices as fields)
+  const P01Entry<R>* p0s = nullptr;
+  const P01Entry<R>* p1s = nullptr;
   R* tab = nullptr;        // momentum tables [2][4][64]
   cpx<R>* t = nullptr;     // FFT temporary, max_batch spinors
   cpx<R>* t2 = nullptr;    // second FFT temporary (only where the multiply pass is out of place)
@@ -257,12 +261,20 @@ wz_status setup_ws(wz_plan* pl, OpWS<R>& ws, int nbatch_t) {
   ws.p23 = find_p23<R>(pl->L[2], pl->L[3]);
   if (!ws.p01 || !ws.p23) return WZ_EUNSUPPORTED;
   if (pl->I % ws.p01->nseg()) return WZ_EUNSUPPORTED;
-  const auto* a = ws.p01;
-  if (!set_smem_kern(a->fwdcg_s) || !set_smem_kern(a->endcg_s)) return WZ_ECUDA;
-  if (!set_smem_kern(a->fwd) || !set_smem_kern(a->inv) || !set_smem_kern(a->mid) ||
-      !set_smem_kern(a->mid_pq) || !set_smem_kern(a->end) || !set_smem_kern(a->fwdcg) ||
-      !set_smem_kern(a->endcg))
-    return WZ_ECUDA;
+  if (pl->L[0] * pl->L[1] > 2048) {
+    const auto* e0 = find_p01<R>(pl->L[0], 1, 0);
+    const auto* e1 = find_p01<R>(pl->L[1], 1, 0);
+    if (e0 && e1 && ((long)pl->L[1] * pl->I) % e0->nseg() == 0 && pl->I % e1->nseg() == 0) { ws.p0s = e0; ws.p1s = e1; }
+  }
+  const P01Entry<R>* entries[3] = {ws.p01, ws.p0s, ws.p1s};
+  for (const P01Entry<R>* a : entries) {
+    if (!a) continue;
+    if (!set_smem_kern(a->fwdcg_s) || !set_smem_kern(a->endcg_s)) return WZ_ECUDA;
+    if (!set_smem_kern(a->fwd) || !set_smem_kern(a->inv) || !set_smem_kern(a->mid) ||
+        !set_smem_kern(a->mid_pq) || !set_smem_kern(a->end) || !set_smem_kern(a->fwdcg) ||
+        !set_smem_kern(a->endcg))
+      return WZ_ECUDA;
+  }
   const auto* b = ws.p23;
   if (!set_smem(b->fwd, b->smem) || !set_smem(b->inv, b->smem) || !set_smem(b->mult, b->smem) ||
       !set_smem(b->multpc, b->smem_pc) || (b->diagpc && !set_smem(b->diagpc, b->smem_pc)))
@@ -338,8 +350,10 @@ int next_sweep(wz_plan* pl) {
 
 // (x0,x1) pass over nf = 4*nbatch fields
 template <typename R>
-wz_status launch_p01(wz_plan* pl, int kind, const P01Kern<R>& k, const P01Args<R>& args_in, int nb) {
-  const int nseg_tiles = (int)(pl->I / k.nseg), nf = 4 * nb;
+wz_status launch_p01(wz_plan* pl, int kind, const P01Kern<R>& k, const P01Args<R>& args_in, int nb, int fmul = 1) {
+  // args_in.I: inner volume the tiles run over (L2*L3, or L1*L2*L3 in the axis-0 kernel of the single-axis
+  // decomposition); fmul: fields per (source, spin) (L0 in its axis-1 kernel)
+  const int nseg_tiles = (int)(args_in.I / k.nseg), nf = 4 * nb * fmul;
   P01Args<R> args = args_in;
   args.rev = next_sweep(pl);
   // pass C launches spin-fastest: the four CTAs that share one phi tile run together (380 -> 360 us per launch
@@ -362,6 +376,39 @@ wz_status launch_p01(wz_plan* pl, int kind, const P01Kern<R>& k, const P01Args<R
       default: k_finalize<FIN_STORE><<<nb, FINALIZE_NT, 0, pl->lstream>>>(args.red, nblk, args.gate); break;
     }
     WZ_CUDA(cudaGetLastError());
+  }
+  return WZ_OK;
+}
+
+// One (x0,x1) pass in the mode `mk` names.  Two-axis tiles: one launch.  Single-axis decomposition (ws.p0s): the
+// axis-0 kernel carries the mode (twist, site-local step, CG fusion) and plain axis-1 transforms run before it
+// (inverse-type modes), after it (forward-type modes) or both (MID), in place on the FFT temporary, with every x0
+// slice passed as a field of its own.  +2u of traffic per axis-1 launch, but every run is 512 bytes long.
+// per-source partials of the reductions of the (x0,x1) passes: 4 spin components x tiles
+template <typename R>
+int partials_needed(const wz_plan* pl, const OpWS<R>& ws) {
+  if (ws.p0s) return (int)((long)pl->L[1] * pl->I / ws.p0s->min_nseg()) * 4;
+  return (int)(pl->I / ws.p01->min_nseg()) * 4;
+}
+
+enum { PASS_FWD_TYPE = 1, PASS_INV_TYPE = 2, PASS_MID_TYPE = 3 };
+template <typename R>
+wz_status pass01(wz_plan* pl, OpWS<R>& ws, int kind, P01Kern<R> P01Entry<R>::*mk, int type, const P01Args<R>& a, int nb) {
+  if (!ws.p0s) return launch_p01<R>(pl, kind, ws.p01->*mk, a, nb);
+  const int L0 = pl->L[0];
+  wz_status s;
+  P01Args<R> ax{};  // the axis-1 sub-pass: fields = (source, spin, x0), no twist, no scale
+  ax.I = pl->I; ax.apbc = 0; ax.scale = R(1); ax.gate = a.gate; ax.fdiv = L0;
+  if (type == PASS_INV_TYPE || type == PASS_MID_TYPE) {
+    ax.in = a.in; ax.out = const_cast<cpx<R>*>(a.in);  // in place (a.in is the FFT temporary in these modes)
+    if ((s = launch_p01<R>(pl, WZ_K_P01_INV, ws.p1s->inv, ax, nb, L0)) != WZ_OK) return s;
+  }
+  P01Args<R> a0 = a;
+  a0.I = (long)pl->L[1] * pl->I;
+  if ((s = launch_p01<R>(pl, kind, ws.p0s->*mk, a0, nb)) != WZ_OK) return s;
+  if (type == PASS_FWD_TYPE || type == PASS_MID_TYPE) {
+    ax.in = a.out; ax.out = a.out;
+    if ((s = launch_p01<R>(pl, WZ_K_P01_FWD, ws.p1s->fwd, ax, nb, L0)) != WZ_OK) return s;
   }
   return WZ_OK;
 }
@@ -426,7 +473,7 @@ wz_status fft4d_impl(wz_plan* pl, int direction, int apbc, const cpx<R>* in, cpx
   b.rho = R(1); b.sign = R(1);
   if (direction > 0) {
     a.in = in; a.out = out;
-    wz_status s = launch_p01<R>(pl, WZ_K_P01_FWD, ws.p01->fwd, a, nb);
+    wz_status s = pass01<R>(pl, ws, WZ_K_P01_FWD, &P01Entry<R>::fwd, PASS_FWD_TYPE, a, nb);
     if (s != WZ_OK) return s;
     b.in = out; b.out = out;
     return launch_p23<R>(pl, WZ_K_P23_FFT, *ws.p23, ws.p23->fwd, b, nb);
@@ -435,7 +482,7 @@ wz_status fft4d_impl(wz_plan* pl, int direction, int apbc, const cpx<R>* in, cpx
   wz_status s = launch_p23<R>(pl, WZ_K_P23_FFT, *ws.p23, ws.p23->inv, b, nb);
   if (s != WZ_OK) return s;
   a.in = out; a.out = out; a.scale = (R)(1.0 / (double)pl->V);
-  return launch_p01<R>(pl, WZ_K_P01_INV, ws.p01->inv, a, nb);
+  return pass01<R>(pl, ws, WZ_K_P01_INV, &P01Entry<R>::inv, PASS_INV_TYPE, a, nb);
 }
 
 // ---- out = M in or M^dag in: passes A, B, E --------------------------
@@ -446,7 +493,7 @@ wz_status apply_M_impl(wz_plan* pl, int dagger, const cpx<R>* phi, const double 
   P01Args<R> a{};
   a.I = pl->I; a.apbc = 1; a.scale = R(1);
   a.in = in; a.out = ws.t;
-  wz_status s = launch_p01<R>(pl, WZ_K_P01_FWD, ws.p01->fwd, a, nb);
+  wz_status s = pass01<R>(pl, ws, WZ_K_P01_FWD, &P01Entry<R>::fwd, PASS_FWD_TYPE, a, nb);
   if (s != WZ_OK) return s;
   P23Args<R> b{};
   b.nplanes = pl->L[0] * pl->L[1]; b.L1 = pl->L[1]; b.scale = (R)(1.0 / (double)pl->V);
@@ -455,7 +502,7 @@ wz_status apply_M_impl(wz_plan* pl, int dagger, const cpx<R>* phi, const double 
   if ((s = mult_pass<R>(pl, ws, b, cur, nb)) != WZ_OK) return s;
   a.in = cur; a.out = cur;
   a.psi = in; a.phi = phi; a.site_out = out; a.op = make_op<R>(m, g, rho, dagger);
-  return launch_p01<R>(pl, WZ_K_P01_END, ws.p01->end, a, nb);
+  return pass01<R>(pl, ws, WZ_K_P01_END, &P01Entry<R>::end, PASS_INV_TYPE, a, nb);
 }
 
 // ---- out = M^dag M in: passes A-E.  With `cg` set (nb = 1) the kernels are gated on
@@ -474,7 +521,7 @@ wz_status apply_MdagM_impl(wz_plan* pl, const cpx<R>* phi, const double m[2], co
   P01Args<R> a{};
   a.I = pl->I; a.apbc = 1; a.scale = R(1); a.gate = gate;
   a.in = in; a.out = ws.t;
-  if ((s = launch_p01<R>(pl, WZ_K_P01_FWD, ws.p01->fwd, a, nb)) != WZ_OK) return s;  // A
+  if ((s = pass01<R>(pl, ws, WZ_K_P01_FWD, &P01Entry<R>::fwd, PASS_FWD_TYPE, a, nb)) != WZ_OK) return s;  // A
   P23Args<R> b{};
   b.nplanes = pl->L[0] * pl->L[1]; b.L1 = pl->L[1]; b.scale = invV;
   b.tab = ws.tab; b.rho = (R)rho; b.sign = pc ? R(-1) : R(1); b.gate = gate;
@@ -486,10 +533,10 @@ wz_status apply_MdagM_impl(wz_plan* pl, const cpx<R>* phi, const double m[2], co
   if (pc) a.op.shift = (R)sigma_pc;
   if (cg) {
     a.red = red_of(pl);
-    if ((int)(pl->I / ws.p01->min_nseg()) * 4 > pl->npartials) return WZ_EINVAL;
-    s = launch_p01<R>(pl, WZ_K_P01_MID, ws.p01->mid_pq, a, nb);  // C
+    if (partials_needed(pl, ws) > pl->npartials) return WZ_EINVAL;
+    s = pass01<R>(pl, ws, WZ_K_P01_MID, &P01Entry<R>::mid_pq, PASS_MID_TYPE, a, nb);  // C
   } else {
-    s = launch_p01<R>(pl, WZ_K_P01_MID, ws.p01->mid, a, nb);
+    s = pass01<R>(pl, ws, WZ_K_P01_MID, &P01Entry<R>::mid, PASS_MID_TYPE, a, nb);
   }
   if (s != WZ_OK) return s;
   b.sign = pc ? R(1) : R(-1);
@@ -498,7 +545,7 @@ wz_status apply_MdagM_impl(wz_plan* pl, const cpx<R>* phi, const double m[2], co
   a.in = cur; a.out = cur;
   a.red = RedArgs{};
   a.psi = ws.chi; a.site_out = out; a.op = make_op<R>(m, g, rho, 1, pc);
-  return launch_p01<R>(pl, WZ_K_P01_END, ws.p01->end, a, nb);  // E
+  return pass01<R>(pl, ws, WZ_K_P01_END, &P01Entry<R>::end, PASS_INV_TYPE, a, nb);  // E
 }
 
 // ---- out = M0^-1 in (dagger = 0) or (M0^-1)^dag in, Eq. (7.11): forward FFT, the 4x4 free
@@ -511,7 +558,7 @@ wz_status apply_M0inv_impl(wz_plan* pl, int dagger, const double m[2], double rh
   P01Args<R> a{};
   a.I = pl->I; a.apbc = 1; a.scale = R(1);
   a.in = in; a.out = ws.t;
-  if ((s = launch_p01<R>(pl, WZ_K_P01_FWD, ws.p01->fwd, a, nb)) != WZ_OK) return s;
+  if ((s = pass01<R>(pl, ws, WZ_K_P01_FWD, &P01Entry<R>::fwd, PASS_FWD_TYPE, a, nb)) != WZ_OK) return s;
   P23Args<R> b{};
   b.nplanes = pl->L[0] * pl->L[1]; b.L1 = pl->L[1]; b.scale = (R)(1.0 / (double)pl->V);
   b.tab = ws.tab; b.rho = (R)rho; b.sign = dagger ? R(1) : R(-1);
@@ -519,7 +566,7 @@ wz_status apply_M0inv_impl(wz_plan* pl, int dagger, const double m[2], double rh
   cpx<R>* cur = ws.t;
   if ((s = mult_pass<R>(pl, ws, b, cur, nb)) != WZ_OK) return s;
   a.in = cur; a.out = out;  // 1/V already applied by the multiply pass
-  return launch_p01<R>(pl, WZ_K_P01_INV, ws.p01->inv, a, nb);
+  return pass01<R>(pl, ws, WZ_K_P01_INV, &P01Entry<R>::inv, PASS_INV_TYPE, a, nb);
 }
 
 // ---- one CG iteration = five kernels: A' (x += alpha p pending from the
@@ -536,7 +583,7 @@ wz_status cg_iteration(wz_plan* pl, const cpx<R>* phi, const double m[2], const 
   // with pc the shift enters pass C instead (Eq. 7.14: + sigma (M0^-1)^dag M0^-1, see wz_p01.cuh)
   const bool sh = sigma != 0.0 && !pc;
   OpWS<R>& ws = ws_of<R>(pl);
-  if ((int)(pl->I / ws.p01->min_nseg()) * 4 > pl->npartials) return WZ_EINVAL;
+  if (partials_needed(pl, ws) > pl->npartials) return WZ_EINVAL;
   const R invV = (R)(1.0 / (double)pl->V);
   const size_t off = (size_t)s0 * 4 * pl->V;  // first spinor of the block
   r += off; p += off; x += off;
@@ -551,7 +598,7 @@ wz_status cg_iteration(wz_plan* pl, const cpx<R>* phi, const double m[2], const 
   a.I = pl->I; a.apbc = 1; a.scale = R(1); a.gate = gate;
   a.in = p; a.out = t; a.cg_r = r; a.cg_p = p; a.cg_x = x;
   if (sh) a.red = red;
-  if ((s = launch_p01<R>(pl, WZ_K_P01_FWDCG, sh ? ws.p01->fwdcg_s : ws.p01->fwdcg, a, nb)) != WZ_OK) return s;
+  if ((s = pass01<R>(pl, ws, WZ_K_P01_FWDCG, sh ? &P01Entry<R>::fwdcg_s : &P01Entry<R>::fwdcg, PASS_FWD_TYPE, a, nb)) != WZ_OK) return s;
   P23Args<R> b{};
   b.nplanes = pl->L[0] * pl->L[1]; b.L1 = pl->L[1]; b.scale = invV;
   b.tab = ws.tab; b.rho = (R)rho; b.sign = pc ? R(-1) : R(1); b.gate = gate;
@@ -562,14 +609,14 @@ wz_status cg_iteration(wz_plan* pl, const cpx<R>* phi, const double m[2], const 
   a.psi = p; a.phi = phi; a.site_out = chi; a.op = make_op<R>(m, g, rho, 0, pc);
   if (pc) a.op.shift = (R)sigma;
   a.red = red;
-  if ((s = launch_p01<R>(pl, WZ_K_P01_MID, ws.p01->mid_pq, a, nb)) != WZ_OK) return s;
+  if ((s = pass01<R>(pl, ws, WZ_K_P01_MID, &P01Entry<R>::mid_pq, PASS_MID_TYPE, a, nb)) != WZ_OK) return s;
   b.sign = pc ? R(1) : R(-1);
   b.pc = pc ? 2 : 0;
   if ((s = mult_pass<R>(pl, ws, b, cur, nb, t, t2)) != WZ_OK) return s;
   a.in = cur; a.out = cur;
   a.psi = chi; a.site_out = nullptr; a.op = make_op<R>(m, g, rho, 1, pc);
   a.cg_r = r; a.cg_p = p; a.cg_x = x; a.op.shift = sh ? (R)sigma : R(0);
-  return launch_p01<R>(pl, WZ_K_P01_ENDCG, sh ? ws.p01->endcg_s : ws.p01->endcg, a, nb);
+  return pass01<R>(pl, ws, WZ_K_P01_ENDCG, sh ? &P01Entry<R>::endcg_s : &P01Entry<R>::endcg, PASS_INV_TYPE, a, nb);
 }
 
 }  // namespace
@@ -686,6 +733,8 @@ wz_status wz_plan_create(wz_plan** plan, int T, int L1, int L2, int L3, wz_dtype
     // reduction workspace per source: a row of partials wide enough for every grid used
     long np = (pl->I / 2) * 4;
     if (np < 4096) np = 4096;
+    if (pl->wsd.p01) np = std::max<long>(np, partials_needed(pl, pl->wsd));
+    if (dtype == WZ_C64 && pl->wsf.p01) np = std::max<long>(np, partials_needed(pl, pl->wsf));
     pl->npartials = (int)np;
     if (!dev_alloc(pl, &pl->partials, (size_t)np * max_batch) || !dev_alloc(pl, &pl->counter, (size_t)max_batch) ||
         !dev_alloc(pl, &pl->d_state, (size_t)max_batch)) { s = WZ_ENOMEM; break; }

@@ -123,6 +123,8 @@ struct P01Args {
   cpx<R>* cg_x;       // FWDCG (read+write)
   const CGState* gate;  // [nbatch]; if set and this source's solve is idle, the CTA returns at once
   int rev;              // 1: CTAs take the tiles in reverse order (see launch_p01: L2 reuse across launches)
+  int fdiv;             // fields per (source, spin) pair: 1, or L0 when the x0 slices are passed as separate fields
+                        //    (the axis-1 sub-pass of the single-axis decomposition); 0 is read as 1
   int comp_fast;        // 1: launch order = (source, tile, spin) with spin fastest: the four CTAs that share one
                         //    phi tile run together, so phi comes from HBM once per source instead of four times
 };
@@ -133,10 +135,12 @@ struct P01Cfg {
   static constexpr int NR0 = L0 / TPL0, NR1 = L1 / TPL1;
   static constexpr int NT_A = L1 * NSEG * TPL0;  // threads when lines run along axis 0
   static constexpr int NT_B = L0 * NSEG * TPL1;  // threads when lines run along axis 1
-  static constexpr int NT_RAW = NT_A > NT_B ? NT_A : NT_B;
+  // L1 == 1: a single-axis pass (lines along axis 0 only, no tile exchange): the decomposition of the 64x64
+  // lattices, where a two-axis tile with runs longer than 32 bytes does not fit (wz_lib.cu: split01)
+  static constexpr int NT_RAW = (L1 == 1) ? NT_A : (NT_A > NT_B ? NT_A : NT_B);
   static constexpr int NT = (NT_RAW + 31) / 32 * 32;
   static constexpr int PITCH0 = L1 * NSEG + NSEG;  // padded x0 stride (elements)
-  static constexpr size_t SMEM = sizeof(cpx<R>) * (size_t)L0 * PITCH0;
+  static constexpr size_t SMEM = (L1 == 1) ? 0 : sizeof(cpx<R>) * (size_t)L0 * PITCH0;
 };
 
 // Resident CTAs per SM the register allocation must allow: 32x32 complex64 tiles aim at
@@ -154,7 +158,7 @@ struct p01_minb {  // TPL = 2: 16 values per thread, 64 registers; TPL = 1: 32 v
 // inside the pass (one kernel node fewer per reduction in the iteration graph).
 template <int L0, int L1>
 struct p01_split_finalize {
-  static constexpr bool v = (L0 * L1 >= 1024);
+  static constexpr bool v = (L0 * L1 >= 1024) || L1 == 1;
 };
 
 template <typename R, int L0, int L1, int NSEG, int T0, int T1, int MODE, int FIN, int IC = 0>
@@ -180,7 +184,8 @@ k_p01(const P01Args<R> a) {
     bx = (int)(q % gridDim.x);
     f = (int)(q / gridDim.x) * 4 + (int)(lin & 3);
   }
-  const int comp = f & 3, src = f >> 2;
+  const int fq = (a.fdiv > 1) ? f / a.fdiv : f;
+  const int comp = fq & 3, src = fq >> 2;
   // forward modes: the idle test of this source is issued now but consumed only after the
   // first loads are in flight (measured: pays there, not in the inverse modes)
   int idle = 0;
@@ -271,26 +276,33 @@ k_p01(const P01Args<R> a) {
       if (idle) return;
     }
     F0::run(x, jA);
-    if (actA) {
+    if constexpr (L1 == 1) {
+      if (actA) {
 #pragma unroll
-      for (int k = 0; k < NR0; ++k) {
-        const int n0 = F0::out_pos(k, jA);
-        sm[n0 * PITCH0 + x1A * NSEG + sA] = x[k];
+        for (int k = 0; k < NR0; ++k) gout[(long)F0::out_pos(k, jA) * I + sA] = x[k];
       }
-    }
-    __syncthreads();
-    cpx<R> y[NR1];
+    } else {
+      if (actA) {
 #pragma unroll
-    for (int k = 0; k < NR1; ++k) {
-      cpx<R> v = {R(0), R(0)};
-      if (actB) v = sm[x0B * PITCH0 + F1::in_pos(k, jB) * NSEG + sB];
-      y[k] = v;
-    }
-    F1::run(y, jB);
-    if (actB) {
+        for (int k = 0; k < NR0; ++k) {
+          const int n0 = F0::out_pos(k, jA);
+          sm[n0 * PITCH0 + x1A * NSEG + sA] = x[k];
+        }
+      }
+      __syncthreads();
+      cpx<R> y[NR1];
 #pragma unroll
-      for (int k = 0; k < NR1; ++k)
-        gout[((long)x0B * L1 + F1::out_pos(k, jB)) * I + sB] = y[k];
+      for (int k = 0; k < NR1; ++k) {
+        cpx<R> v = {R(0), R(0)};
+        if (actB) v = sm[x0B * PITCH0 + F1::in_pos(k, jB) * NSEG + sB];
+        y[k] = v;
+      }
+      F1::run(y, jB);
+      if (actB) {
+#pragma unroll
+        for (int k = 0; k < NR1; ++k)
+          gout[((long)x0B * L1 + F1::out_pos(k, jB)) * I + sB] = y[k];
+      }
     }
     if constexpr (MODE == P01_FWDCG && FIN == FIN_PP) {
       // shifted solves: <p,p> of this source for alpha = rho / (||M p||^2 + sigma <p,p>)
@@ -302,16 +314,9 @@ k_p01(const P01Args<R> a) {
     // ---- inverse half: axis 1 first (from HBM), then axis 0 ----
     using G1 = LineFFT<R, L1, -1, VAR_DIT, TPL1>;
     using G0 = LineFFT<R, L0, -1, VAR_DIT, TPL0>;
-    {
-      cpx<R> y[NR1];
-#pragma unroll
-      for (int k = 0; k < NR1; ++k) {
-        cpx<R> v = {R(0), R(0)};
-        if (actB) v = gin[((long)x0B * L1 + G1::in_pos(k, jB)) * I + sB];
-        y[k] = v;
-      }
+    // operands of the site-local step (this thread's axis-0 line), one L2 prefetch hint per 32-byte sector
+    auto prefetch_operands = [&]() {
       if constexpr (MODE != P01_INV) {
-        // operands of the site-local step (this thread's axis-0 line), one hint per 32-byte sector
         if (actA && (sA * (int)sizeof(cpx<R>)) % 32 == 0) {
           const long fo = (long)f * V + i0;
 #pragma unroll
@@ -323,19 +328,39 @@ k_p01(const P01Args<R> a) {
           }
         }
       }
-      G1::run(y, jB);
-      if (actB) {
-#pragma unroll
-        for (int k = 0; k < NR1; ++k) sm[x0B * PITCH0 + G1::out_pos(k, jB) * NSEG + sB] = y[k];
-      }
-    }
-    __syncthreads();
+    };
     cpx<R> x[NR0];
+    if constexpr (L1 == 1) {
 #pragma unroll
-    for (int k = 0; k < NR0; ++k) {
-      cpx<R> v = {R(0), R(0)};
-      if (actA) v = sm[G0::in_pos(k, jA) * PITCH0 + x1A * NSEG + sA];
-      x[k] = v;
+      for (int k = 0; k < NR0; ++k) {
+        cpx<R> v = {R(0), R(0)};
+        if (actA) v = gin[(long)G0::in_pos(k, jA) * I + sA];
+        x[k] = v;
+      }
+      prefetch_operands();
+    } else {
+      {
+        cpx<R> y[NR1];
+#pragma unroll
+        for (int k = 0; k < NR1; ++k) {
+          cpx<R> v = {R(0), R(0)};
+          if (actB) v = gin[((long)x0B * L1 + G1::in_pos(k, jB)) * I + sB];
+          y[k] = v;
+        }
+        prefetch_operands();
+        G1::run(y, jB);
+        if (actB) {
+#pragma unroll
+          for (int k = 0; k < NR1; ++k) sm[x0B * PITCH0 + G1::out_pos(k, jB) * NSEG + sB] = y[k];
+        }
+      }
+      __syncthreads();
+#pragma unroll
+      for (int k = 0; k < NR0; ++k) {
+        cpx<R> v = {R(0), R(0)};
+        if (actA) v = sm[G0::in_pos(k, jA) * PITCH0 + x1A * NSEG + sA];
+        x[k] = v;
+      }
     }
     G0::run(x, jA);
     // post-twist exp(+i pi x0/T) and 1/V
@@ -447,24 +472,31 @@ k_p01(const P01Args<R> a) {
           z[out_index<NR0>(k)] = v;
         }
         F0::run(z, jA);
-        __syncthreads();  // every axis-0 read of the tile is done
-        if (actA) {
+        if constexpr (L1 == 1) {
+          if (actA) {
 #pragma unroll
-          for (int k = 0; k < NR0; ++k) sm[F0::out_pos(k, jA) * PITCH0 + x1A * NSEG + sA] = z[k];
-        }
-        __syncthreads();
-        cpx<R> y[NR1];
+            for (int k = 0; k < NR0; ++k) gout[(long)F0::out_pos(k, jA) * I + sA] = z[k];
+          }
+        } else {
+          __syncthreads();  // every axis-0 read of the tile is done
+          if (actA) {
 #pragma unroll
-        for (int k = 0; k < NR1; ++k) {
-          cpx<R> v = {R(0), R(0)};
-          if (actB) v = sm[x0B * PITCH0 + F1::in_pos(k, jB) * NSEG + sB];
-          y[k] = v;
-        }
-        F1::run(y, jB);
-        if (actB) {
+            for (int k = 0; k < NR0; ++k) sm[F0::out_pos(k, jA) * PITCH0 + x1A * NSEG + sA] = z[k];
+          }
+          __syncthreads();
+          cpx<R> y[NR1];
 #pragma unroll
-          for (int k = 0; k < NR1; ++k)
-            gout[((long)x0B * L1 + F1::out_pos(k, jB)) * I + sB] = y[k];
+          for (int k = 0; k < NR1; ++k) {
+            cpx<R> v = {R(0), R(0)};
+            if (actB) v = sm[x0B * PITCH0 + F1::in_pos(k, jB) * NSEG + sB];
+            y[k] = v;
+          }
+          F1::run(y, jB);
+          if (actB) {
+#pragma unroll
+            for (int k = 0; k < NR1; ++k)
+              gout[((long)x0B * L1 + F1::out_pos(k, jB)) * I + sB] = y[k];
+          }
         }
       }
       if (a.red.partials) {  // one reduction per source: its 4 spin components x all segments

@@ -65,7 +65,8 @@ template <typename R, int L> struct tune_tpl23 {  // axes 2,3
 // 512-thread CTA per SM.
 template <typename R, int L0, int L1, int MODE> struct tune_nseg {
   static constexpr bool fwd = (MODE == P01_FWD || MODE == P01_FWDCG);
-  static constexpr int v = (sizeof(R) == 4) ? (L0 * L1 > 2048 ? 4 : (L0 * L1 == 1024 ? (fwd ? 8 : 16) : 8))
+  static constexpr int v = (L1 == 1) ? (int)(512 / (2 * sizeof(R)))  // single-axis pass: 512-byte runs, no tile in shared memory
+                         : (sizeof(R) == 4) ? (L0 * L1 > 2048 ? 4 : (L0 * L1 == 1024 ? (fwd ? 8 : 16) : 8))
                                             : (L0 * L1 > 2048 ? 2 : 4);
 };
 

@@ -1065,3 +1065,17 @@ def test_cg_dc_vs_oracle(wz, orc, inp, dims, inner_tol):
     with pytest.raises(wz.WZError) as e:
         plan.cg_solve_dc(d_phi, d_b, m, g, rho, tol, 1.5)
     assert e.value.status == wz.WZ_EINVAL
+
+
+def test_M0inv_at_64x4_complex128(wz, orc, inp):
+    """The free inverse where a CTA of the contiguous pass holds only one component pair (64x64 complex128
+    planes): off-diagonal launch + accumulating diagonal launch (P23_DIAGPC) against the oracle, both signs."""
+    dims = (64, 64, 64, 64)
+    b = inp.make_source(5, 0, dims)
+    plan = wz.Plan(dims, "c128", 1)
+    d_b = torch.from_numpy(b).cuda()
+    m = 0.3 + 0.1j
+    for dagger in (False, True):
+        out = plan.apply_M0inv(d_b, m, 1.0, dagger).cpu().numpy()
+        ref = orc.apply_M0inv(dims, b, m, 1.0, dagger)
+        assert rel(out, ref) <= TOL["c128"]
