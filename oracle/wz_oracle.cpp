@@ -25,6 +25,14 @@
 //                                adjoint / Hermiticity / positivity.
 //   cg / cg_c64ru              : dense Cholesky solve on 2^4, 4^4; constant-phi closed
 //                                form; true residual recomputed independently.
+//   apply_M0inv / cg_pc        : inverse of the g = 0 apply_M; dense solution; Table VI's 8 / 15 iterations
+//                                (tests/golden/table_VI_pc_iterations.txt = PAPER.md:937-942).
+//   cg_shift / cg_shift_pc     : dense solves of Eq. 7.13 per shift; sigma = 0 special cases; free field.
+//   cg_multishift (O8)         : dense solves per shift; the single-shift loop's iteration counts and solutions;
+//                                the sequential rational sum.
+//   cg_dc (O9)                 : dense solve; independently recomputed residual; outer-step structure.
+//   Parity unpinned by anything the paper fixes: the ITERATION COUNT the reliable-update trigger of cg_c64ru
+//   produces (delta = 0.1, "keep p": reading G9 is not in the paper) -- the solution it returns is pinned.
 //   The solve at 16^4 and above with non-constant phi has no printed value in the
 //   paper to compare with: there "parity unpinned by a printed value" -- it is
 //   covered by the same code path pinned at 2^4/4^4 plus the residual check.
