@@ -226,6 +226,30 @@ wz_status wz_plan_set_block(wz_plan *plan, int sources_per_block);
  * of pairs recorded, or -1 on a bad argument. */
 int wz_plan_cg_history(const wz_plan *plan, int source, int *iterations, double *rel_residual, int cap);
 
+/* ---- M^dag M without a plan and without any device allocation ----
+ * For callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses that
+ * forbid it).  out = M^dag M in, as wz_apply_MdagM, but the scratch of the matvec (the FFT temporary, chi = M in,
+ * the momentum tables) lives in a file-scope device array of WZ_NOALLOC_MAX_BYTES (+ 4 KB) inside the library,
+ * which every GPU that loads the library holds until the process exits.  The call makes no cudaMalloc, cudaFree or
+ * other allocating CUDA call; it only enqueues kernels on `stream` (the momentum tables are recomputed on the device
+ * by a small kernel each call).  Works on the CURRENT device: `stream` (a cudaStream_t, 0 = legacy default stream)
+ * and all pointers must belong to it.  The first call on a device also does the one-time set-up (address of the
+ * array, upload of the twiddle tables): make that first call outside a stream capture.
+ *  - T, L1, L2, L3, dtype: the lattice and element type (no plan); phi, in, out, m, g, rho: as wz_apply_MdagM;
+ *    in != out.
+ *  - LIMIT: the call needs 2 * nbatch * (4 * T*L1*L2*L3 * sizeof(complex)) bytes of scratch (3 * ... for 64 x 64
+ *    (x2,x3) planes); more than WZ_NOALLOC_MAX_BYTES = 8 MiB (e.g. one 16^4 complex128 or one 32x16^3 complex64
+ *    source, four 16^4 complex64 sources) returns WZ_EINVAL with the byte counts in wz_last_error().  Unsupported
+ *    extents: WZ_EUNSUPPORTED.
+ *  - ALL calls share the one array, on every stream: two calls that overlap on the GPU race (serialise them on
+ *    one stream or with events).  The array keeps the last call's contents; nothing in it has to start at zero
+ *    (every byte a call reads it has written before), so no clearing is needed between calls.
+ * Results agree with wz_apply_MdagM to rounding (the tables come from the device's sinpi instead of the host's sin). */
+#define WZ_NOALLOC_MAX_BYTES (8u << 20)
+wz_status wz_apply_MdagM_noalloc(int T, int L1, int L2, int L3, wz_dtype dtype, const void *phi,
+                                 const double m[2], const double g[2], double rho,
+                                 const void *in, void *out, int nbatch, void *stream);
+
 /* Number of kernel launches this plan has enqueued so far (for bench.py's
  * gpu_launches), and a reset. */
 unsigned long long wz_plan_launch_count(const wz_plan *plan);

@@ -1725,3 +1725,130 @@ wz_status wz_apply_MtdagMt(wz_plan* pl, const void* phi, const double m[2], cons
 }
 
 }  // extern "C"
+
+// =============================== no-allocation entry point =======================
+// wz_apply_MdagM_noalloc: M^dag M without a plan and without any device allocation, for callers that cannot call
+// cudaMalloc (code under CUDA graph capture, tight serving loops).  The matvec's scratch -- the FFT temporary t,
+// chi = M psi, and the momentum tables -- lives in ONE file-scope device array of WZ_NOALLOC_MAX_BYTES (+ 4 KB of
+// tables) that every GPU loading the library holds until exit.  All calls share it: calls that overlap on the GPU
+// race.  Nothing in it has to start at zero: every byte a call reads is written earlier in the same call.
+namespace {
+
+constexpr size_t kNoAllocTabBytes = 4096;  // momentum tables [2][4][64], double at most
+static __device__ __align__(256) unsigned char g_noalloc_scratch[kNoAllocTabBytes + WZ_NOALLOC_MAX_BYTES];
+
+// Per device: the DEVICE address of g_noalloc_scratch.  In host code the array's name is only a host-side stand-in
+// for the symbol, never a device address: cudaGetSymbolAddress (with that device current) gives the address.
+constexpr int kNoAllocMaxDevices = 64;
+std::mutex g_noalloc_mu;
+unsigned char* g_noalloc_ptr[kNoAllocMaxDevices] = {nullptr};
+
+wz_status noalloc_setup(int dev, unsigned char** ptr) {
+  if (dev < 0 || dev >= kNoAllocMaxDevices) return WZ_EINVAL;
+  std::lock_guard<std::mutex> lock(g_noalloc_mu);
+  if (!g_noalloc_ptr[dev]) {
+    if (!init_twiddles(dev)) return WZ_ECUDA;  // __constant__ twiddle tables of the kernel modules, once per device
+    unsigned char* p = nullptr;
+    WZ_CUDA(cudaGetSymbolAddress((void**)&p, g_noalloc_scratch));
+    if (!p) { snprintf(g_err, sizeof(g_err), "cudaGetSymbolAddress(g_noalloc_scratch) gave a null address"); return WZ_ECUDA; }
+    g_noalloc_ptr[dev] = p;
+  }
+  *ptr = g_noalloc_ptr[dev];
+  return WZ_OK;
+}
+
+// Momentum tables (as setup_ws computes them on the host), written by the device straight into the head of the
+// scratch array: device code may name the array directly.  tab[0][mu][n] = sin p_mu, tab[1][mu][n] = sin^2(p_mu/2),
+// p_0 = 2 pi (n + 1/2)/T, p_i = 2 pi n/L_i; sinpi() reduces the argument exactly.
+template <typename R>
+__global__ void k_noalloc_tables(int L0, int L1, int L2, int L3) {
+  R* tab = reinterpret_cast<R*>(g_noalloc_scratch);
+  const int L[4] = {L0, L1, L2, L3};
+  for (int i = threadIdx.x; i < 2 * 4 * 64; i += blockDim.x) {
+    const int which = i / 256, mu = (i / 64) % 4, n = i % 64;
+    double v = 0.0;
+    if (n < L[mu]) {
+      const double x = 2.0 * ((double)n + (mu == 0 ? 0.5 : 0.0)) / (double)L[mu];  // p / pi
+      if (which == 0) {
+        v = sinpi(x);
+      } else {
+        const double s = sinpi(0.5 * x);
+        v = s * s;
+      }
+    }
+    tab[i] = (R)v;
+  }
+}
+
+template <typename R>
+wz_status noalloc_MdagM(int T, int L1, int L2, int L3, const void* phi, const double m[2], const double g[2],
+                        double rho, const void* in, void* out, int nb, cudaStream_t stream, int dev,
+                        unsigned char* scratch) {
+  // A plan object on the host stack: lattice, stream, kernel choices; its "workspace" points into the static array.
+  wz_plan pl;
+  pl.L[0] = T; pl.L[1] = L1; pl.L[2] = L2; pl.L[3] = L3;
+  pl.I = (long)L2 * L3;
+  pl.V = (long)T * L1 * pl.I;
+  pl.dtype = (sizeof(R) == 4) ? WZ_C64 : WZ_C128;
+  pl.max_batch = nb;
+  pl.stream = stream; pl.lstream = stream;
+  pl.dev = dev;
+  memset(&pl.iter_key, 0, sizeof(pl.iter_key));
+  int sms = 0;
+  if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && sms > 0) pl.num_sms = sms;
+  OpWS<R>& ws = ws_of<R>(&pl);
+  ws.p01 = find_p01<R>(T, L1, pl.I);
+  ws.p23 = find_p23<R>(L2, L3);
+  if (!ws.p01 || !ws.p23 || pl.I % ws.p01->nseg()) return WZ_EUNSUPPORTED;
+  if (T * L1 > 2048) {  // single-axis decomposition, as setup_ws chooses it
+    const auto* e0 = find_p01<R>(T, 1, 0);
+    const auto* e1 = find_p01<R>(L1, 1, 0);
+    if (e0 && e1 && ((long)L1 * pl.I) % e0->nseg() == 0 && pl.I % e1->nseg() == 0) { ws.p0s = e0; ws.p1s = e1; }
+  }
+  // scratch: [tables 4 KB][t][t2 where the multiply pass is out of place][chi], nb spinors each
+  const size_t u = (size_t)4 * pl.V * sizeof(cpx<R>);
+  const int nvec = 2 + (ws.p23->nhalf == 2 ? 1 : 0);
+  const size_t need = (size_t)nvec * nb * u;
+  if (need > (size_t)WZ_NOALLOC_MAX_BYTES) {
+    snprintf(g_err, sizeof(g_err), "wz_apply_MdagM_noalloc: this call needs %zu bytes of scratch (%d temporaries x %d "
+             "sources x %zu bytes per spinor), the static array holds WZ_NOALLOC_MAX_BYTES = %zu",
+             need, nvec, nb, u, (size_t)WZ_NOALLOC_MAX_BYTES);
+    return WZ_EINVAL;
+  }
+  const P01Entry<R>* entries[3] = {ws.p01, ws.p0s, ws.p1s};
+  for (const P01Entry<R>* e : entries) {
+    if (!e) continue;
+    if (!set_smem_kern(e->fwd) || !set_smem_kern(e->inv) || !set_smem_kern(e->mid) || !set_smem_kern(e->end)) return WZ_ECUDA;
+  }
+  if (!set_smem(ws.p23->mult, ws.p23->smem)) return WZ_ECUDA;
+  ws.tab = reinterpret_cast<R*>(scratch);
+  unsigned char* vec = scratch + kNoAllocTabBytes;
+  ws.t = reinterpret_cast<cpx<R>*>(vec);
+  if (nvec == 3) ws.t2 = reinterpret_cast<cpx<R>*>(vec + (size_t)nb * u);
+  ws.chi = reinterpret_cast<cpx<R>*>(vec + (size_t)(nvec - 1) * nb * u);
+  k_noalloc_tables<R><<<1, 256, 0, stream>>>(T, L1, L2, L3);
+  WZ_CUDA(cudaGetLastError());
+  return apply_MdagM_impl<R>(&pl, (const cpx<R>*)phi, m, g, rho, (const cpx<R>*)in, (cpx<R>*)out, nb, false);
+}
+
+}  // namespace
+
+extern "C" wz_status wz_apply_MdagM_noalloc(int T, int L1, int L2, int L3, wz_dtype dtype, const void* phi,
+                                            const double m[2], const double g[2], double rho, const void* in,
+                                            void* out, int nbatch, void* stream) {
+  g_err[0] = 0;
+  if (!phi || !m || !g || !in || !out || in == out) return WZ_EINVAL;
+  if (T < 2 || L1 < 2 || L2 < 2 || L3 < 2 || (T & 1) || nbatch < 0) return WZ_EINVAL;
+  if (dtype != WZ_C64 && dtype != WZ_C128) return WZ_EINVAL;
+  if (!(rho > 0.0 && rho < 2.0)) return WZ_EINVAL;
+  if (!wz_supported(T, L1, L2, L3, dtype)) return WZ_EUNSUPPORTED;
+  if (nbatch == 0) return WZ_OK;
+  int dev = 0;
+  WZ_CUDA(cudaGetDevice(&dev));  // works on the CURRENT device: `stream` and every pointer must belong to it
+  unsigned char* scratch = nullptr;
+  wz_status s = noalloc_setup(dev, &scratch);
+  if (s != WZ_OK) return s;
+  if (dtype == WZ_C64)
+    return noalloc_MdagM<float>(T, L1, L2, L3, phi, m, g, rho, in, out, nbatch, (cudaStream_t)stream, dev, scratch);
+  return noalloc_MdagM<double>(T, L1, L2, L3, phi, m, g, rho, in, out, nbatch, (cudaStream_t)stream, dev, scratch);
+}

@@ -27,7 +27,7 @@ EXPORTS = [
     "wz_apply_M0inv", "wz_apply_MtdagMt", "wz_cg_solve_pc", "wz_apply_Dslash", "wz_locality_profile",
     "wz_cg_solve_shift", "wz_cg_solve_shift_pc", "wz_rational_apply",
     "wz_plan_set_graph", "wz_plan_cg_history", "wz_plan_set_block",
-    "wz_cg_solve_multishift", "wz_rational_apply_multishift", "wz_cg_solve_dc",
+    "wz_cg_solve_multishift", "wz_rational_apply_multishift", "wz_cg_solve_dc", "wz_apply_MdagM_noalloc",
 ]
 
 
@@ -87,6 +87,7 @@ def lib() -> ctypes.CDLL:
         L.wz_rational_apply_multishift.argtypes = L.wz_rational_apply.argtypes
         L.wz_cg_solve_multishift.argtypes = [vp, vp, vp, vp, d2, d2, cd, d2, ci, cd, ci, ci, ctypes.POINTER(_CGInfo)]
         L.wz_cg_solve_dc.argtypes = [vp, vp, vp, vp, d2, d2, cd, cd, cd, ci, ci, ctypes.POINTER(_CGInfo)]
+        L.wz_apply_MdagM_noalloc.argtypes = [ci, ci, ci, ci, ci, vp, d2, d2, cd, vp, vp, ci, vp]
         L.wz_apply_M0inv.argtypes = [vp, ci, d2, cd, vp, vp, ci]
         L.wz_apply_MtdagMt.argtypes = [vp, vp, d2, d2, cd, vp, vp, ci]
         L.wz_apply_Dslash.argtypes = [vp, cd, vp, vp, ci]
@@ -375,6 +376,38 @@ class Plan:
                        bool(infos[i * nb + j].converged), infos[i * nb + j].rel_residual_recursive,
                        infos[i * nb + j].rel_residual_true) for j in range(nb)] for i in range(d)]
         return out, res
+
+
+NOALLOC_MAX_BYTES = 8 << 20  # WZ_NOALLOC_MAX_BYTES of include/wz.h
+
+
+def apply_MdagM_noalloc(phi, psi, m, g, rho: float = 1.0, out=None, stream=None):
+    """out = M^dag M psi through wz_apply_MdagM_noalloc: no plan, no device allocation inside the call (its
+    scratch is a static device array of NOALLOC_MAX_BYTES inside libwz.so, shared by all calls: overlapping
+    calls race).  `out` must be given if the caller may not allocate.  Lattice and dtype are taken from phi."""
+    if not (phi.is_cuda and psi.is_cuda and phi.is_contiguous() and psi.is_contiguous()):
+        raise ValueError("expected contiguous CUDA tensors")
+    if phi.dtype not in (torch.complex64, torch.complex128) or psi.dtype != phi.dtype or phi.dim() != 4:
+        raise ValueError("phi: [T, L1, L2, L3] complex64 or complex128; psi of the same dtype")
+    dims = tuple(int(d) for d in phi.shape)
+    if tuple(psi.shape) == (4,) + dims:
+        nb = 1
+    elif psi.dim() == 6 and tuple(psi.shape[1:]) == (4,) + dims:
+        nb = int(psi.shape[0])
+    else:
+        raise ValueError("expected psi of shape [nbatch,]4,T,L1,L2,L3")
+    if out is None:
+        out = torch.empty_like(psi)
+    if out.shape != psi.shape or out.dtype != psi.dtype or out.device != psi.device or not out.is_contiguous() \
+            or phi.device != psi.device:
+        raise ValueError("out must match psi; phi, psi, out on one device")
+    with torch.cuda.device(psi.device):
+        st = stream if stream is not None else torch.cuda.current_stream(psi.device)
+        _check(lib().wz_apply_MdagM_noalloc(dims[0], dims[1], dims[2], dims[3],
+                                            WZ_C64 if phi.dtype == torch.complex64 else WZ_C128,
+                                            phi.data_ptr(), _c2(m), _c2(g), float(rho), psi.data_ptr(),
+                                            out.data_ptr(), nb, ctypes.c_void_p(st.cuda_stream)))
+    return out
 
 
 # module-level aliases with the C names
