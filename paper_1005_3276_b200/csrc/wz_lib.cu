@@ -114,6 +114,8 @@ struct OpWS {
   const P01Entry<R>* p0s = nullptr;
   const P01Entry<R>* p1s = nullptr;
   R* tab = nullptr;        // momentum tables [2][4][64]
+  R* ctab = nullptr;       // c(p) per momentum site for the rho below (ensure_ctab); V entries
+  R ctab_rho = R(-1);
   cpx<R>* t = nullptr;     // FFT temporary, max_batch spinors
   cpx<R>* t2 = nullptr;    // second FFT temporary (only where the multiply pass is out of place)
   cpx<R>* chi = nullptr;   // chi = M psi,   max_batch spinors
@@ -174,6 +176,7 @@ struct wz_plan {
   // CUDA graph of one chunk of CG iterations (north star iii): captured once per distinct set of
   // solve arguments on a private stream, replayed on `stream`
   int use_graph = 1;
+  int no_ctab = 0;  // 1: never build the c(p) table (wz_apply_MdagM_noalloc: no device allocation)
   int block = 0;  // sources per block of the CG iteration (0: the whole batch in lock step)
   cudaStream_t cap_stream = nullptr;
   cudaGraphExec_t iter_graph = nullptr;
@@ -277,10 +280,12 @@ wz_status setup_ws(wz_plan* pl, OpWS<R>& ws, int nbatch_t) {
   }
   const auto* b = ws.p23;
   if (!set_smem(b->fwd, b->smem) || !set_smem(b->inv, b->smem) || !set_smem(b->mult, b->smem) ||
-      !set_smem(b->multpc, b->smem_pc) || (b->diagpc && !set_smem(b->diagpc, b->smem_pc)))
+      !set_smem(b->multpc, b->smem_pc) || (b->diagpc && !set_smem(b->diagpc, b->smem_pc)) ||
+      (b->multt && !set_smem(b->multt, b->smem)))
     return WZ_ECUDA;
   wave_ctas(pl, (const void*)b->mult, b->nt, b->smem);  // occupancy queries now, not inside a stream capture
   wave_ctas(pl, (const void*)b->multpc, b->nt, b->smem_pc);
+  if (b->multt) wave_ctas(pl, (const void*)b->multt, b->nt, b->smem);
   if (b->diagpc) wave_ctas(pl, (const void*)b->diagpc, b->nt, b->smem_pc);
   wave_ctas(pl, (const void*)b->fwd, b->nt, b->smem);
   wave_ctas(pl, (const void*)b->inv, b->nt, b->smem);
@@ -432,7 +437,13 @@ wz_status mult_pass(wz_plan* pl, OpWS<R>& ws, P23Args<R>& b, cpx<R>*& cur, int n
   if (!t) { t = ws.t; t2 = ws.t2; }  // the two temporaries (whole batch, or the block a CG iteration works on)
   cpx<R>* dst = (ws.p23->nhalf == 2) ? ((cur == t) ? t2 : t) : cur;
   b.in = cur; b.out = dst;
-  wz_status s = launch_p23<R>(pl, WZ_K_P23_MULT, *ws.p23, b.pc ? ws.p23->multpc : ws.p23->mult, b, nb);
+  void (*kern)(const P23Args<R>) = b.pc ? ws.p23->multpc : ws.p23->mult;
+  b.ctab = nullptr;
+  if (!b.pc && ws.ctab && ws.ctab_rho == b.rho && ws.p23->multt) {  // c(p) from the table built for this rho
+    kern = ws.p23->multt;
+    b.ctab = ws.ctab;
+  }
+  wz_status s = launch_p23<R>(pl, WZ_K_P23_MULT, *ws.p23, kern, b, nb);
   // two components per CTA: the diagonal term of M0^-1 needs the pair the CTA does not hold -> second launch
   if (s == WZ_OK && b.pc && ws.p23->diagpc) s = launch_p23<R>(pl, WZ_K_P23_MULT, *ws.p23, ws.p23->diagpc, b, nb);
   cur = dst;
@@ -460,6 +471,24 @@ OpParams<R> make_op(const double m[2], const double g[2], double rho, int dagger
   op.g2_re = (R)(2.0 * g[0]); op.g2_im = (R)(2.0 * g[1]);
   op.rho = (R)rho; op.dagger = dagger; op.pc = pc; op.shift = R(0);
   return op;
+}
+
+// c(p) table of the multiply pass (wz_p23.cuh, P23_MULTT) for this rho: allocated on first use, rebuilt when rho
+// changes.  Called at entry-point level only (never inside a stream capture); a pass launched while the table is
+// missing or belongs to another rho computes c(p) on the fly as before.
+template <typename R>
+wz_status ensure_ctab(wz_plan* pl, OpWS<R>& ws, double rho) {
+  if (pl->no_ctab || !ws.p23 || !ws.p23->multt) return WZ_OK;
+  if (!ws.ctab && !dev_alloc(pl, &ws.ctab, (size_t)pl->V)) { ws.ctab = nullptr; cudaGetLastError(); return WZ_OK; }  // no memory: on the fly
+  if (ws.ctab_rho == (R)rho) return WZ_OK;
+  {
+    ProfScope ps(pl, WZ_K_OTHER);
+    const int grid = (int)std::min<long>((pl->V + CGK_NT - 1) / CGK_NT, 148L * 8);
+    k_ctab<R><<<grid, CGK_NT, 0, pl->lstream>>>(ws.ctab, ws.tab, pl->L[0], pl->L[1], pl->L[2], pl->L[3], (R)rho);
+  }
+  WZ_CUDA(cudaGetLastError());
+  ws.ctab_rho = (R)rho;
+  return WZ_OK;
 }
 
 // ---- 4D FFT (steps a1, a2 / a4, a5) ---------------------------------------------
@@ -490,10 +519,12 @@ template <typename R>
 wz_status apply_M_impl(wz_plan* pl, int dagger, const cpx<R>* phi, const double m[2], const double g[2],
                        double rho, const cpx<R>* in, cpx<R>* out, int nb) {
   OpWS<R>& ws = ws_of<R>(pl);
+  wz_status s = ensure_ctab<R>(pl, ws, rho);
+  if (s != WZ_OK) return s;
   P01Args<R> a{};
   a.I = pl->I; a.apbc = 1; a.scale = R(1);
   a.in = in; a.out = ws.t;
-  wz_status s = pass01<R>(pl, ws, WZ_K_P01_FWD, &P01Entry<R>::fwd, PASS_FWD_TYPE, a, nb);
+  s = pass01<R>(pl, ws, WZ_K_P01_FWD, &P01Entry<R>::fwd, PASS_FWD_TYPE, a, nb);
   if (s != WZ_OK) return s;
   P23Args<R> b{};
   b.nplanes = pl->L[0] * pl->L[1]; b.L1 = pl->L[1]; b.scale = (R)(1.0 / (double)pl->V);
@@ -518,6 +549,7 @@ wz_status apply_MdagM_impl(wz_plan* pl, const cpx<R>* phi, const double m[2], co
   const CGState* gate = cg ? pl->d_state : nullptr;
   const R invV = (R)(1.0 / (double)pl->V);
   wz_status s;
+  if (!pc && (s = ensure_ctab<R>(pl, ws, rho)) != WZ_OK) return s;
   P01Args<R> a{};
   a.I = pl->I; a.apbc = 1; a.scale = R(1); a.gate = gate;
   a.in = in; a.out = ws.t;
@@ -895,6 +927,7 @@ wz_status cg_batch(wz_plan* pl, const cpx<R>* phi, const cpx<R>* b, cpx<double>*
   R* r = (R*)pl->r; R* p = (R*)pl->p; R* xs = (R*)pl->xs;
   const int gv = vec_grid(n, N), gv2 = vec_grid(n, 2), gv4 = vec_grid(n, 4);
   wz_status s;
+  if (!pc && (s = ensure_ctab<R>(pl, ws_of<R>(pl), rho)) != WZ_OK) return s;
 
   std::vector<CGState> h(nb);
   memset(h.data(), 0, sizeof(CGState) * nb);
@@ -1154,6 +1187,7 @@ wz_status ms_batch(wz_plan* pl, const cpx<R>* phi, const cpx<R>* b, cpx<double>*
   for (int i = 1; i < ns; ++i)
     if (sigmas[i] < sigmas[base]) base = i;
   const double sigma0 = sigmas[base];
+  if ((s = ensure_ctab<R>(pl, ws_of<R>(pl), rho)) != WZ_OK) return s;
 
   // workspace
   const size_t need = (size_t)ns * pl->max_batch;
@@ -1793,6 +1827,7 @@ wz_status noalloc_MdagM(int T, int L1, int L2, int L3, const void* phi, const do
   pl.max_batch = nb;
   pl.stream = stream; pl.lstream = stream;
   pl.dev = dev;
+  pl.no_ctab = 1;  // no device allocation here: c(p) on the fly
   memset(&pl.iter_key, 0, sizeof(pl.iter_key));
   int sms = 0;
   if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && sms > 0) pl.num_sms = sms;

@@ -15,7 +15,10 @@
 
 namespace wz {
 
-enum { P23_FFT = 0, P23_MULT = 1, P23_MULTPC = 2, P23_DIAGPC = 3 };
+enum { P23_FFT = 0, P23_MULT = 1, P23_MULTPC = 2, P23_DIAGPC = 3, P23_MULTT = 4 };
+// MULTT: MULT with c(p) read from the plan's table (args.ctab, one value per momentum site, built by k_ctab for the
+// plan's rho) instead of one sqrt + one divide + one shuffle per site: the table (4 MB at 32^4 complex64) is shared by
+// every source, spin component and launch and stays in the 126 MB L2.
 // MULTPC: the multiply with args.pc = 1 or 2.  DIAGPC (two components per CTA only): the diagonal term of the same
 // operator, accumulated onto the output of a MULTPC launch (there the CTA does not hold the other pair).
 // Preconditioner (Eq. 7.11): with args.pc set, the multiply applies the free
@@ -52,6 +55,7 @@ struct P23Args {
   const CGState* gate;  // [nbatch], indexed by blockIdx.y
   int rev;              // 1: CTAs take (plane, source) in reverse order (L2 reuse across launches)
   int pf_dist;          // > 0: L2-prefetch the planes of the CTA pf_dist launches-in-order ahead (one wave)
+  const R* ctab;        // MULTT: c(p) = 2 rho / (s + Mw) per momentum site, [L0*L1][L3][L2] (n2 fastest)
 };
 
 // NC = spin components per CTA: 4 (whole plane quad, in place), or 2 when four planes
@@ -110,7 +114,8 @@ k_p23(const P23Args<R> a) {
   constexpr int G3 = Cfg::G3, RPW = Cfg::RPW, WPP = Cfg::WPP;
   constexpr bool kDiag = (MODE == P23_DIAGPC);   // out += F^-1 (m or m^*)/D F in, component by component
   constexpr bool kPC = (MODE == P23_MULTPC);
-  constexpr bool kMult = (MODE == P23_MULT || kPC);
+  constexpr bool kTab = (MODE == P23_MULTT);     // c(p) from the table
+  constexpr bool kMult = (MODE == P23_MULT || kPC || kTab);
   constexpr bool kMom = kMult || kDiag;          // works in momentum space between two transforms
   constexpr bool kStage = kPC && NC == 4;        // diagonal term of M0^-1 inside this launch (needs all four components)
   constexpr int D1 = kMom ? +1 : DIR;  // direction of the first half
@@ -235,6 +240,27 @@ k_p23(const P23Args<R> a) {
       const R dm_re = a.m_re;
       const R dm_im = ((cdiag < 2) == (a.pc == 1)) ? a.m_im : -a.m_im;
       [[maybe_unused]] const cpx<R>* smO = sm + (slotB ^ 2) * CPITCH + n2 * PITCH;  // kStage: same row, other pair
+      if constexpr (kTab) {
+        // c(p) from the table; sign and the 1/V of the inverse transform ride on the row coefficients
+        const R ks = a.sign * a.scale;
+        const R p0 = P0 * ks, p1 = P1 * ks, p3 = P3 * ks, q0 = Q0 * ks, q1 = Q1 * ks, q3 = Q3 * ks;
+        // table layout [plane][n3][n2]: the 16 rows of a warp half read 16 consecutive values (one wavefront per load)
+        const R* crow = a.ctab + (long)plane * L2 * L3 + n2;
+        R cv[NR3];
+#pragma unroll
+        for (int k = 0; k < NR3; ++k) cv[k] = __ldg(crow + F3::out_pos(k, jB) * L2);
+#pragma unroll
+        for (int k = 0; k < NR3; ++k) {
+          const int n3 = F3::out_pos(k, jB);
+          const R s3 = sn[3 * 64 + n3];
+          const cpx<R> own = y[k];
+          const cpx<R> oth = shfl_xor_c(own, RPW);
+          const R Pi = p1 + p3 * s3, Qi = q1 + q3 * s3;
+          const R tr = p0 * own.re - Pi * own.im + q0 * oth.re - Qi * oth.im;
+          const R ti = p0 * own.im + Pi * own.re + q0 * oth.im + Qi * oth.re;
+          w[out_index<NR3>(k)] = {-cv[k] * ti, cv[k] * tr};  // times i c(p)
+        }
+      } else
 #pragma unroll
       for (int k = 0; k < NR3 / 2; ++k) {
         // c(p) for registers k and k + NR3/2: this lane evaluates one, its pair partner (lane ^ RPW) the other
@@ -327,6 +353,25 @@ k_p23(const P23Args<R> a) {
         }
       }
     }
+  }
+}
+
+// c(p) = 2 rho / (s + Mw) (cancellation-free branch for Mw < 0) at every momentum site, for P23_MULTT.
+template <typename R>
+__global__ void k_ctab(R* __restrict__ ctab, const R* __restrict__ tab, int L0, int L1, int L2, int L3, R rho) {
+  const long V = (long)L0 * L1 * L2 * L3;
+  const R* sn = tab;
+  const R* sh = tab + 4 * 64;
+  for (long i = (long)blockIdx.x * blockDim.x + threadIdx.x; i < V; i += (long)gridDim.x * blockDim.x) {
+    long t = i;
+    const int n3 = (int)(t % L3); t /= L3;
+    const int n2 = (int)(t % L2); t /= L2;
+    const int n1 = (int)(t % L1); t /= L1;
+    const int n0 = (int)t;
+    const R s0 = sn[0 * 64 + n0], s1 = sn[1 * 64 + n1], s2 = sn[2 * 64 + n2], s3 = sn[3 * 64 + n3];
+    const R S2 = s0 * s0 + s1 * s1 + s2 * s2 + s3 * s3;
+    const R Mw = rho - R(2) * (sh[0 * 64 + n0] + sh[1 * 64 + n1] + sh[2 * 64 + n2] + sh[3 * 64 + n3]);
+    ctab[(((long)n0 * L1 + n1) * L3 + n3) * L2 + n2] = overlap_c(Mw, S2, R(2) * rho);  // [plane][n3][n2]
   }
 }
 

@@ -44,6 +44,7 @@ struct P23Entry {
   void (*inv)(const P23Args<R>);
   void (*mult)(const P23Args<R>);
   void (*multpc)(const P23Args<R>);  // multiply with the free inverse (preconditioner)
+  void (*multt)(const P23Args<R>) = nullptr;   // multiply with c(p) from the plan's table (P23_MULTT)
   void (*diagpc)(const P23Args<R>) = nullptr;  // nhalf = 2 only: diagonal term of the free inverse, accumulated (wz_p23.cuh)
 };
 
@@ -104,6 +105,7 @@ P23Entry<R> make_p23() {
   e.inv = k_p23<R, L2, L3, T2, T3, P23_FFT, -1, NC>;
   e.mult = k_p23<R, L2, L3, T2, T3, P23_MULT, +1, NC>;
   e.multpc = k_p23<R, L2, L3, T2, T3, P23_MULTPC, +1, NC>;
+  e.multt = k_p23<R, L2, L3, T2, T3, P23_MULTT, +1, NC>;
   if constexpr (NC == 2) e.diagpc = k_p23<R, L2, L3, T2, T3, P23_DIAGPC, +1, NC>;
   return e;
 }
