@@ -12,6 +12,8 @@
 #include <set>
 #include <vector>
 
+#include <cuda.h>  // CUtensorMap types only; cuTensorMapEncodeTiled is resolved at run time (no libcuda link)
+
 #include "../../include/wz.h"
 #include "wz_cgk.cuh"
 #include "wz_tables.cuh"
@@ -176,6 +178,7 @@ struct wz_plan {
   // CUDA graph of one chunk of CG iterations (north star iii): captured once per distinct set of
   // solve arguments on a private stream, replayed on `stream`
   int use_graph = 1;
+  int tile_prefetch = 1;  // wave-ahead TMA prefetch of the strided input tiles of pass C
   int no_ctab = 0;  // 1: never build the c(p) table (wz_apply_MdagM_noalloc: no device allocation)
   int block = 0;  // sources per block of the CG iteration (0: the whole batch in lock step)
   cudaStream_t cap_stream = nullptr;
@@ -353,6 +356,45 @@ int next_sweep(wz_plan* pl) {
   return pl->sweep;
 }
 
+// ---- TMA descriptor of a field array [nf][l0][l1][inner] of complex<R>, box = one strided tile l0 x l1 x nseg ----
+// Rank 4 in reals: (2*inner, l1, l0, nf), box (2*nseg, l1, l0, 1).  Host-side encoding only (no device work, no
+// allocation); used by k_p01 to prefetch whole tiles into L2 (wz_p01.cuh).  Returns false where the driver entry
+// point is missing or the shape is outside the TMA limits: the kernels then run without the prefetch.
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+EncodeTiledFn encode_tiled_fn() {
+  static EncodeTiledFn fn = [] {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) != cudaSuccess ||
+        q != cudaDriverEntryPointSuccess)
+      p = nullptr;
+    cudaGetLastError();
+    return (EncodeTiledFn)p;
+  }();
+  return fn;
+}
+template <typename R>
+bool make_tile_tmap(TMapBlob* out, const void* base, long inner, int l0, int l1, int nseg, long nf) {
+  static_assert(sizeof(CUtensorMap) == sizeof(TMapBlob), "CUtensorMap is 128 bytes");
+  EncodeTiledFn enc = encode_tiled_fn();
+  if (!enc || !base || ((uintptr_t)base & 15) || l0 > 256 || l1 > 256 || 2 * nseg > 256) return false;
+  if ((2 * nseg * sizeof(R)) % 16 || (inner * 2 * sizeof(R)) % 16) return false;
+  const cuuint64_t gdim[4] = {(cuuint64_t)(2 * inner), (cuuint64_t)l1, (cuuint64_t)l0, (cuuint64_t)nf};
+  const cuuint64_t gstr[3] = {(cuuint64_t)(2 * inner * sizeof(R)), (cuuint64_t)(2 * inner * sizeof(R)) * l1,
+                              (cuuint64_t)(2 * inner * sizeof(R)) * l1 * l0};
+  const cuuint32_t box[4] = {(cuuint32_t)(2 * nseg), (cuuint32_t)l1, (cuuint32_t)l0, 1u};
+  const cuuint32_t estr[4] = {1u, 1u, 1u, 1u};
+  CUtensorMap tm;
+  const CUresult r = enc(&tm, sizeof(R) == 4 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4u,
+                         const_cast<void*>(base), gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                         CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) return false;
+  memcpy(out, &tm, sizeof(tm));
+  return true;
+}
+
 // (x0,x1) pass over nf = 4*nbatch fields
 template <typename R>
 wz_status launch_p01(wz_plan* pl, int kind, const P01Kern<R>& k, const P01Args<R>& args_in, int nb, int fmul = 1) {
@@ -364,6 +406,13 @@ wz_status launch_p01(wz_plan* pl, int kind, const P01Kern<R>& k, const P01Args<R
   // pass C launches spin-fastest: the four CTAs that share one phi tile run together (380 -> 360 us per launch
   // at 32^4 x 12); the same order slows pass E' (296 -> 346 us) and is not used there
   args.comp_fast = (kind == WZ_K_P01_MID) ? 1 : 0;
+  args.tm_ahead = 0;
+  if (pl->tile_prefetch && kind == WZ_K_P01_MID) {  // pass C only: the other inverse-type passes do not gain (wz_p01.cuh)
+    const int wave = wave_ctas(pl, (const void*)k.fn, k.nt, k.smem);
+    if ((long)nseg_tiles * nf > 2L * wave &&  // at least two waves: something to run ahead of
+        make_tile_tmap<R>(&args.tm_in, args.in, args_in.I, k.l0, k.l1, k.nseg, nf))
+      args.tm_ahead = wave;
+  }
   {
     ProfScope ps(pl, kind);
     k.fn<<<dim3((unsigned)nseg_tiles, (unsigned)nf), k.nt, k.smem, pl->lstream>>>(args);

@@ -105,6 +105,18 @@ __device__ __forceinline__ void prefetch_l2(const void* p) {
   asm volatile("prefetch.global.L2 [%0];" ::"l"(p));
 }
 
+// A CUtensorMap (TMA descriptor) carried by value in the kernel parameters; encoded on the host
+// (wz_lib.cu: make_tile_tmap).  Used only to PREFETCH whole strided tiles into L2, one instruction per tile.
+struct alignas(64) TMapBlob {
+  unsigned long long v[16];
+};
+// L2 prefetch of the box at (c0, c1, c2, c3) of a rank-4 tiled tensor map (innermost coordinate first).
+__device__ __forceinline__ void tma_prefetch_l2_4d(const TMapBlob* tm, int c0, int c1, int c2, int c3) {
+  asm volatile("cp.async.bulk.prefetch.tensor.4d.L2.global.tile [%0, {%1, %2, %3, %4}];"
+               ::"l"(reinterpret_cast<unsigned long long>(tm)), "r"(c0), "r"(c1), "r"(c2), "r"(c3)
+               : "memory");
+}
+
 template <typename R>
 struct P01Args {
   const cpx<R>* in;   // [nf][L0][L1][I]
@@ -125,6 +137,11 @@ struct P01Args {
   int rev;              // 1: CTAs take the tiles in reverse order (see launch_p01: L2 reuse across launches)
   int fdiv;             // fields per (source, spin) pair: 1, or L0 when the x0 slices are passed as separate fields
                         //    (the axis-1 sub-pass of the single-axis decomposition); 0 is read as 1
+  // Wave-ahead tile prefetch (pass C): tm_in describes `in` as [nf][L0][L1][2*I reals] with a box of one
+  // tile; the CTA prefetches the input tile of the CTA tm_ahead launches further on (one wave of resident CTAs)
+  // into L2 with ONE TMA instruction, so that CTA later pays L2 instead of HBM latency for its first loads.
+  TMapBlob tm_in;
+  int tm_ahead;         // 0: off
   int comp_fast;        // 1: launch order = (source, tile, spin) with spin fastest: the four CTAs that share one
                         //    phi tile run together, so phi comes from HBM once per source instead of four times
 };
@@ -163,7 +180,7 @@ struct p01_split_finalize {
 
 template <typename R, int L0, int L1, int NSEG, int T0, int T1, int MODE, int FIN, int IC = 0>
 __global__ void __launch_bounds__(P01Cfg<R, L0, L1, NSEG, T0, T1>::NT, p01_minb<R, L0, L1, P01Cfg<R, L0, L1, NSEG, T0, T1>::NT, T0>::v)
-k_p01(const P01Args<R> a) {
+k_p01(const __grid_constant__ P01Args<R> a) {
   using Cfg = P01Cfg<R, L0, L1, NSEG, T0, T1>;
   constexpr int TPL0 = Cfg::TPL0, TPL1 = Cfg::TPL1, NR0 = Cfg::NR0, NR1 = Cfg::NR1;
   constexpr int PITCH0 = Cfg::PITCH0;
@@ -312,6 +329,30 @@ k_p01(const P01Args<R> a) {
     }
   } else {
     // ---- inverse half: axis 1 first (from HBM), then axis 0 ----
+    // Pass C only, issued LATE in the CTA's life (before its forward half, about a quarter of its time left): the CTA
+    // tm_ahead launches further on takes over an SM a few microseconds later.  Measured at 32^4 x 12: pass C 360 -> 339 us.
+    // (Issued at the start, a whole wave early, the tiles were evicted again by the ~80 MB that stream through L2 per
+    // wave and came from HBM twice: 360 -> 396 us.  Pass E' gains nothing at any issue point, 306 -> 306...329 us.)
+    auto prefetch_next_tile = [&]() {
+      if (a.tm_ahead > 0 && tid == 0) {
+        const unsigned tot = gridDim.x * gridDim.y;
+        const unsigned l2 = blockIdx.y * gridDim.x + blockIdx.x + (unsigned)a.tm_ahead;  // launch order, x fastest
+        if (l2 < tot) {
+          int bx2, f2;  // the same launch-order -> (tile, field) map as above
+          if (a.comp_fast) {
+            const unsigned lin = a.rev ? tot - 1 - l2 : l2;
+            const unsigned q = lin >> 2;
+            bx2 = (int)(q % gridDim.x);
+            f2 = (int)(q / gridDim.x) * 4 + (int)(lin & 3);
+          } else {
+            const unsigned xr = l2 % gridDim.x, yr = l2 / gridDim.x;
+            bx2 = a.rev ? (int)(gridDim.x - 1 - xr) : (int)xr;
+            f2 = a.rev ? (int)(gridDim.y - 1 - yr) : (int)yr;
+          }
+          tma_prefetch_l2_4d(&a.tm_in, 2 * bx2 * NSEG, 0, 0, f2);
+        }
+      }
+    };
     using G1 = LineFFT<R, L1, -1, VAR_DIT, TPL1>;
     using G0 = LineFFT<R, L0, -1, VAR_DIT, TPL0>;
     // operands of the site-local step (this thread's axis-0 line), one L2 prefetch hint per 32-byte sector
@@ -460,6 +501,7 @@ k_p01(const P01Args<R> a) {
         }
       }
       if constexpr (MODE == P01_MID) {
+        prefetch_next_tile();  // pass C: the forward half (about a quarter of the CTA's time) is left
         // forward again: pre-twist, DFT axis 0 (halves in -> DIF variant), DFT axis 1
         using F0 = LineFFT<R, L0, +1, VAR_DIF, TPL0>;
         using F1 = LineFFT<R, L1, +1, VAR_DIT, TPL1>;

@@ -15,6 +15,7 @@ template <typename R>
 struct P01Kern {
   void (*fn)(const P01Args<R>) = nullptr;
   int nt = 0, nseg = 0;
+  int l0 = 0, l1 = 0;   // tile extents along axes 0, 1 (for the TMA tile prefetch)
   int fin = FIN_STORE;  // what k_finalize does with the kernel's reduction (if it has one)
   bool split_finalize = false;  // the kernel leaves partials; k_finalize<fin> must follow (p01_split_finalize)
   size_t smem = 0;
@@ -77,7 +78,7 @@ P01Kern<R> make_p01_kern() {
   using C = P01Cfg<R, L0, L1, NSEG, T0, T1>;
   P01Kern<R> k;
   k.fn = k_p01<R, L0, L1, NSEG, T0, T1, MODE, FIN, IC>;
-  k.nt = C::NT; k.nseg = NSEG; k.smem = C::SMEM; k.fin = FIN; k.split_finalize = p01_split_finalize<L0, L1>::v;
+  k.nt = C::NT; k.nseg = NSEG; k.smem = C::SMEM; k.l0 = L0; k.l1 = L1; k.fin = FIN; k.split_finalize = p01_split_finalize<L0, L1>::v;
   return k;
 }
 template <typename R, int L0, int L1, int IC = 0>

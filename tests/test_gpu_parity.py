@@ -821,6 +821,7 @@ def test_graph_replay_equals_stream_launches(wz, inp, dims, dtype):
     plan = wz.Plan(dims, dtype, 2)
     tol = 1e-10 if dtype == "c128" else 1e-6
     res = {}
+    plan.cg_solve(phi, b, 0.05, 1.0, 1.0, tol, 8, raise_on_fail=False)  # the plan's first solve also builds its c(p) table (one launch)
     for on in (True, False, True):
         plan.set_graph(on)
         plan.reset_launch_count()
