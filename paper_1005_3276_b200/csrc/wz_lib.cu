@@ -178,7 +178,7 @@ struct wz_plan {
   // CUDA graph of one chunk of CG iterations (north star iii): captured once per distinct set of
   // solve arguments on a private stream, replayed on `stream`
   int use_graph = 1;
-  int tile_prefetch = 1;  // wave-ahead TMA prefetch of the strided input tiles of pass C
+  int tile_prefetch = 1;  // wave-ahead TMA prefetch of the strided input tiles of passes C and A'
   int no_ctab = 0;  // 1: never build the c(p) table (wz_apply_MdagM_noalloc: no device allocation)
   int block = 0;  // sources per block of the CG iteration (0: the whole batch in lock step)
   cudaStream_t cap_stream = nullptr;
@@ -336,10 +336,9 @@ wz_status launch(wz_plan* pl, int kind, void (*k)(const A), dim3 grid, int nt, s
   return WZ_OK;
 }
 
-// Wave-ahead L2 prefetch of the contiguous pass (wz_p23.cuh): distance = half of the CTAs resident on the
-// whole GPU at once (half a wave).  Measured at 32^4 complex64, 12 sources: k_p23 207.7 -> 190 us per launch
-// at a quarter to a half wave, 193 at one, 200 at 1.5.
-constexpr int kPrefetchPercent = 50;
+// Wave-ahead L2 prefetch of the contiguous pass (wz_p23.cuh): distance = the CTAs resident on the whole GPU at once
+// (one wave), issued late in the CTA (measurements there).
+constexpr int kPrefetchPercent = 100;
 int wave_ctas(wz_plan* pl, const void* fn, int nt, size_t smem) {
   auto it = pl->occ_cache.find(fn);
   if (it != pl->occ_cache.end()) return it->second;
@@ -407,7 +406,7 @@ wz_status launch_p01(wz_plan* pl, int kind, const P01Kern<R>& k, const P01Args<R
   // at 32^4 x 12); the same order slows pass E' (296 -> 346 us) and is not used there
   args.comp_fast = (kind == WZ_K_P01_MID) ? 1 : 0;
   args.tm_ahead = 0;
-  if (pl->tile_prefetch && kind == WZ_K_P01_MID) {  // pass C only: the other inverse-type passes do not gain (wz_p01.cuh)
+  if (pl->tile_prefetch && (kind == WZ_K_P01_MID || kind == WZ_K_P01_FWDCG)) {  // passes C and A' (wz_p01.cuh: E' does not gain)
     const int wave = wave_ctas(pl, (const void*)k.fn, k.nt, k.smem);
     if ((long)nseg_tiles * nf > 2L * wave &&  // at least two waves: something to run ahead of
         make_tile_tmap<R>(&args.tm_in, args.in, args_in.I, k.l0, k.l1, k.nseg, nf))

@@ -137,7 +137,7 @@ struct P01Args {
   int rev;              // 1: CTAs take the tiles in reverse order (see launch_p01: L2 reuse across launches)
   int fdiv;             // fields per (source, spin) pair: 1, or L0 when the x0 slices are passed as separate fields
                         //    (the axis-1 sub-pass of the single-axis decomposition); 0 is read as 1
-  // Wave-ahead tile prefetch (pass C): tm_in describes `in` as [nf][L0][L1][2*I reals] with a box of one
+  // Wave-ahead tile prefetch (passes C, A'): tm_in describes `in` as [nf][L0][L1][2*I reals] with a box of one
   // tile; the CTA prefetches the input tile of the CTA tm_ahead launches further on (one wave of resident CTAs)
   // into L2 with ONE TMA instruction, so that CTA later pays L2 instead of HBM latency for its first loads.
   TMapBlob tm_in;
@@ -227,6 +227,32 @@ k_p01(const __grid_constant__ P01Args<R> a) {
   const bool actB = lineB < L0 * NSEG;
   const int x0B = lineB / NSEG, sB = lineB % NSEG;
 
+  // Passes C and A', issued LATE in the CTA's life (C: before its forward half, about a quarter of its time left;
+  // A': the tile of p, before the transforms): the CTA
+  // tm_ahead launches further on takes over an SM a few microseconds later.  Measured at 32^4 x 12: pass C 360 -> 339 us.
+  // (Issued at the start, a whole wave early, the tiles were evicted again by the ~80 MB that stream through L2 per
+  // wave and came from HBM twice: 360 -> 396 us.  Pass E' gains nothing at any issue point, 306 -> 306...329 us; pass A'
+  // 445 -> 436 us.  Prefetching the operand tiles (r, x; p, phi) the same way lost: C 342 -> 366, A' 436 -> 467 us.)
+  auto prefetch_next_tile = [&]() {
+    if (a.tm_ahead > 0 && tid == 0) {
+      const unsigned tot = gridDim.x * gridDim.y;
+      const unsigned l2 = blockIdx.y * gridDim.x + blockIdx.x + (unsigned)a.tm_ahead;  // launch order, x fastest
+      if (l2 < tot) {
+        int bx2, f2;  // the same launch-order -> (tile, field) map as above
+        if (a.comp_fast) {
+          const unsigned lin = a.rev ? tot - 1 - l2 : l2;
+          const unsigned q = lin >> 2;
+          bx2 = (int)(q % gridDim.x);
+          f2 = (int)(q / gridDim.x) * 4 + (int)(lin & 3);
+        } else {
+          const unsigned xr = l2 % gridDim.x, yr = l2 / gridDim.x;
+          bx2 = a.rev ? (int)(gridDim.x - 1 - xr) : (int)xr;
+          f2 = a.rev ? (int)(gridDim.y - 1 - yr) : (int)yr;
+        }
+        tma_prefetch_l2_4d(&a.tm_in, 2 * bx2 * NSEG, 0, 0, f2);
+      }
+    }
+  };
   if constexpr (MODE == P01_FWD || MODE == P01_FWDCG) {
     using F0 = LineFFT<R, L0, +1, VAR_DIT, TPL0>;
     using F1 = LineFFT<R, L1, +1, VAR_DIT, TPL1>;
@@ -292,6 +318,7 @@ k_p01(const __grid_constant__ P01Args<R> a) {
       }
       if (idle) return;
     }
+    if constexpr (MODE == P01_FWDCG) prefetch_next_tile();
     F0::run(x, jA);
     if constexpr (L1 == 1) {
       if (actA) {
@@ -329,30 +356,6 @@ k_p01(const __grid_constant__ P01Args<R> a) {
     }
   } else {
     // ---- inverse half: axis 1 first (from HBM), then axis 0 ----
-    // Pass C only, issued LATE in the CTA's life (before its forward half, about a quarter of its time left): the CTA
-    // tm_ahead launches further on takes over an SM a few microseconds later.  Measured at 32^4 x 12: pass C 360 -> 339 us.
-    // (Issued at the start, a whole wave early, the tiles were evicted again by the ~80 MB that stream through L2 per
-    // wave and came from HBM twice: 360 -> 396 us.  Pass E' gains nothing at any issue point, 306 -> 306...329 us.)
-    auto prefetch_next_tile = [&]() {
-      if (a.tm_ahead > 0 && tid == 0) {
-        const unsigned tot = gridDim.x * gridDim.y;
-        const unsigned l2 = blockIdx.y * gridDim.x + blockIdx.x + (unsigned)a.tm_ahead;  // launch order, x fastest
-        if (l2 < tot) {
-          int bx2, f2;  // the same launch-order -> (tile, field) map as above
-          if (a.comp_fast) {
-            const unsigned lin = a.rev ? tot - 1 - l2 : l2;
-            const unsigned q = lin >> 2;
-            bx2 = (int)(q % gridDim.x);
-            f2 = (int)(q / gridDim.x) * 4 + (int)(lin & 3);
-          } else {
-            const unsigned xr = l2 % gridDim.x, yr = l2 / gridDim.x;
-            bx2 = a.rev ? (int)(gridDim.x - 1 - xr) : (int)xr;
-            f2 = a.rev ? (int)(gridDim.y - 1 - yr) : (int)yr;
-          }
-          tma_prefetch_l2_4d(&a.tm_in, 2 * bx2 * NSEG, 0, 0, f2);
-        }
-      }
-    };
     using G1 = LineFFT<R, L1, -1, VAR_DIT, TPL1>;
     using G0 = LineFFT<R, L0, -1, VAR_DIT, TPL0>;
     // operands of the site-local step (this thread's axis-0 line), one L2 prefetch hint per 32-byte sector

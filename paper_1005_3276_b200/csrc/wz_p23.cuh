@@ -157,6 +157,24 @@ k_p23(const P23Args<R> a) {
   const int slotB = warpB ? (wB / WPP) * 2 + hB : 0;
   cpx<R>* smB = sm + slotB * CPITCH + (actB ? n2B : 0) * PITCH;
 
+  // Planes of the CTA one wave of resident CTAs further on -> L2 (one bulk prefetch per spin plane): that CTA then pays
+  // L2 instead of HBM latency for its first loads.  Issued LATE (before the inverse axis-2 step, the last phase):
+  // measured at 32^4 x 12 per launch: no prefetch 208 us; at CTA start, half a wave ahead 182; at CTA start, one wave
+  // 183; after the axis-2 transform 183; before the inverse axis-2 step, half a wave 179, one wave 177, 1.5 waves 178.
+  auto prefetch_planes = [&]() {
+    if constexpr (NC == 4) {
+      const int dist = a.pf_dist;
+      if (dist > 0 && tid < 4) {
+        const long lin = (long)blockIdx.y * gridDim.x + blockIdx.x + dist;
+        if (lin < (long)gridDim.y * gridDim.x) {
+          long by = lin / gridDim.x, bx = lin % gridDim.x;  // launch order -> data order
+          if (a.rev) { by = gridDim.y - 1 - by; bx = gridDim.x - 1 - bx; }
+          const cpx<R>* pf = a.in + ((by * 4 + tid) * a.nplanes + bx) * PL;
+          asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(pf), "r"((unsigned)(PL * sizeof(cpx<R>))));
+        }
+      }
+    }
+  };
   // ---- half 1, axis 2 (lanes run along x3: coalesced HBM reads) ----
   if (tid < Cfg::NT_A) {
     using F2 = LineFFT<R, L2, D1, VAR_DIT, TPL2>;
@@ -167,19 +185,6 @@ k_p23(const P23Args<R> a) {
       cpx<R> v = {R(0), R(0)};
       if (actA) v = gin[(long)F2::in_pos(k, jA) * L3 + x3A];
       x[k] = v;
-    }
-    // next wave's planes -> L2 while this CTA computes (one bulk prefetch per spin plane): the CTA that
-    // takes them later pays L2 latency instead of HBM latency
-    if constexpr (NC == 4) {
-      if (a.pf_dist > 0 && tid < 4) {
-        const long lin = (long)blockIdx.y * gridDim.x + blockIdx.x + a.pf_dist;
-        if (lin < (long)gridDim.y * gridDim.x) {
-          long by = lin / gridDim.x, bx = lin % gridDim.x;  // launch order -> data order
-          if (a.rev) { by = gridDim.y - 1 - by; bx = gridDim.x - 1 - bx; }
-          const cpx<R>* pf = a.in + ((by * 4 + tid) * a.nplanes + bx) * PL;
-          asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(pf), "r"((unsigned)(PL * sizeof(cpx<R>))));
-        }
-      }
     }
     F2::run(x, jA);
     if (actA) {
@@ -329,6 +334,7 @@ k_p23(const P23Args<R> a) {
       a.out[(fbase + (long)cout_of(ci) * a.nplanes + plane) * PL + r] = cscale(v, a.scale);
     }
   } else {
+    prefetch_planes();
     // ---- inverse axis 2, coalesced HBM writes; slot s now holds output component cout_of(s) ----
     if (tid < Cfg::NT_A) {
       using G2 = LineFFT<R, L2, -1, VAR_DIT, TPL2>;
