@@ -35,7 +35,7 @@ __device__ __forceinline__ cpx<double> ldg_c(const cpx<double>* p) {
 // in L2 (createpolicy + .L2::cache_hint) leaves more of the 126 MB L2 to what the NEXT launch reads first
 // (the tail of r written here; see next_sweep() in wz_lib.cu).  Measured at 32^4 complex64, 12 sources:
 // pass E' 307.6 -> 291 us per launch.  The same hint on x / r in pass A' and on the chi store of pass C
-// made those passes slower (420 -> 599 us, 380 -> 406 us) and is not used (profiles/r01_notes.md).
+// made those passes slower (420 -> 599 us, 380 -> 406 us; round-1 A/B runs) and is not used.
 #ifndef WZ_EVICT
 #define WZ_EVICT 1
 #endif
