@@ -1018,4 +1018,91 @@ int orc_cg_dc(int method, const int* L, const double* phi, const double* b_, dou
   return 0;
 }
 
+// ----------------------------------------------------------------------------
+// O10 (NEXT-3, third form). Defect correction with 16-bit STORAGE of the iteration vectors
+// ("mixed precision conjugate gradient"; SURVEY 8(f) NEXT-3 "a half-precision-storage
+// inner solver with defect correction").  Arithmetic stays wider; what is rounded is what a solver
+// would keep in memory between passes.  Model (stated, not derived from any kernel):
+//   * orc_round_f16: IEEE binary16, round to nearest even, subnormals kept, magnitudes above the largest
+//     finite value saturate to +-65504;
+//   * outer loop as O9 (complex128): R = b - A X; stop if ||R|| <= tol ||b||;
+//   * inner solve on the NORMALISED defect: s = sqrt(n) / ||R|| (unit rms, so that every stored value sits in
+//     binary16's normal range without per-vector scales), r_0 = f16(s R), p_0 = r_0, e_0 = 0;
+//     plain CG on A e = r_0 where after every update r and p are rounded to binary16, chi = M p is rounded to
+//     binary16 before M^dag is applied (chi is the one intermediate of A = M^dag M that is stored), the
+//     accumulated e is rounded to float, reductions in double; alpha = rho / ||chi||^2 with the UNROUNDED chi;
+//     stop when ||r|| <= inner_tol ||r_0||;  X += e / s.
+// info->iterations = inner iterations in total, info->reliable_updates = outer corrections.
+// ----------------------------------------------------------------------------
+double orc_round_f16(double x) {
+  if (x != x) return x;
+  const double ax = std::fabs(x);
+  if (ax == 0.0) return x;
+  const double max_f16 = 65504.0;
+  double q;
+  if (ax < 6.103515625e-05) {            // below 2^-14: subnormal spacing 2^-24
+    q = std::nearbyint(ax * 16777216.0) / 16777216.0;
+  } else {
+    int e;
+    std::frexp(ax, &e);                  // ax = m 2^e, m in [0.5, 1): 11 significant bits -> spacing 2^(e-11)
+    const double ulp = std::ldexp(1.0, e - 11);
+    q = std::nearbyint(ax / ulp) * ulp;  // nearbyint: round to nearest even in the default rounding mode
+  }
+  if (q > max_f16) q = max_f16;
+  return x < 0 ? -q : q;
+}
+static inline cd round_c16(cd z) { return cd(orc_round_f16(z.real()), orc_round_f16(z.imag())); }
+
+int orc_cg_dc_f16(int method, const int* L, const double* phi, const double* b_, double* X_,
+                  const double* m, const double* g, double rho, double tol, double inner_tol, int max_iter,
+                  orc_cg_info* info) {
+  const long V = (long)L[0] * L[1] * L[2] * L[3];
+  const long n = 4 * V;
+  const cd* b = reinterpret_cast<const cd*>(b_);
+  cd* X = reinterpret_cast<cd*>(X_);
+  std::vector<cd> R(b, b + n), e(n), r(n), p(n), chi(n), chi16(n), q(n);
+  for (long i = 0; i < n; ++i) X[i] = 0.0;
+  const double bnorm = std::sqrt(dot_re(b, b, n));
+  double Rnorm = bnorm;
+  int total = 0, outer = 0, converged = (bnorm == 0.0);
+  while (!converged && total < max_iter) {
+    const double s = std::sqrt((double)n) / Rnorm;  // the inner right-hand side has unit rms
+    for (long i = 0; i < n; ++i) { r[i] = round_c16(s * R[i]); p[i] = r[i]; e[i] = 0.0; }
+    double rr = dot_re(r.data(), r.data(), n);
+    const double stop = inner_tol * std::sqrt(rr);
+    while (total < max_iter) {
+      ++total;
+      int rc = orc_apply_M(method, L, phi, m, g, rho, 0, reinterpret_cast<double*>(p.data()),
+                           reinterpret_cast<double*>(chi.data()));
+      if (rc) return rc;
+      for (long i = 0; i < n; ++i) chi16[i] = round_c16(chi[i]);  // chi as stored
+      orc_apply_M(method, L, phi, m, g, rho, 1, reinterpret_cast<double*>(chi16.data()),
+                  reinterpret_cast<double*>(q.data()));
+      const double alpha = rr / dot_re(chi.data(), chi.data(), n);  // <p, A p> = ||M p||^2
+      for (long i = 0; i < n; ++i) {
+        e[i] = round_c64(e[i] + alpha * p[i]);
+        r[i] = round_c16(r[i] - alpha * q[i]);
+      }
+      const double rr_new = dot_re(r.data(), r.data(), n);
+      if (std::sqrt(rr_new) <= stop) break;
+      const double beta = rr_new / rr;
+      rr = rr_new;
+      for (long i = 0; i < n; ++i) p[i] = round_c16(r[i] + beta * p[i]);
+    }
+    ++outer;
+    for (long i = 0; i < n; ++i) X[i] += e[i] / s;
+    orc_apply_MdagM(method, L, phi, m, g, rho, X_, reinterpret_cast<double*>(q.data()));
+    double tr = 0.0;
+    for (long i = 0; i < n; ++i) { R[i] = b[i] - q[i]; tr += std::norm(R[i]); }
+    Rnorm = std::sqrt(tr);
+    if (Rnorm <= tol * bnorm) converged = 1;
+  }
+  info->iterations = total;
+  info->reliable_updates = outer;
+  info->converged = converged;
+  info->rel_residual_recursive = bnorm > 0 ? Rnorm / bnorm : 0.0;
+  info->rel_residual_true = bnorm > 0 ? Rnorm / bnorm : 0.0;
+  return 0;
+}
+
 }  // extern "C"

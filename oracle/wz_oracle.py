@@ -344,3 +344,29 @@ def cg_dc(phi, b, m, g, rho=1.0, tol=1e-10, inner_tol=1e-3, max_iter=100000, met
         raise ValueError("oracle cg_dc failed")
     return X, CGInfo(info.iterations, info.reliable_updates, bool(info.converged), info.rel_residual_recursive,
                      info.rel_residual_true, np.zeros(0))
+
+
+def round_f16(x):
+    """The oracle's IEEE binary16 rounding model (round to nearest even, saturating), element-wise on float64."""
+    L = lib()
+    L.orc_round_f16.restype = ctypes.c_double
+    L.orc_round_f16.argtypes = [ctypes.c_double]
+    a = np.asarray(x, dtype=np.float64)
+    return np.array([L.orc_round_f16(float(v)) for v in a.ravel()]).reshape(a.shape)
+
+
+def cg_dc_f16(phi, b, m, g, rho=1.0, tol=1e-6, inner_tol=1e-1, max_iter=100000, method="auto"):
+    """Defect correction with binary16 STORAGE of the inner solver's r, p, chi (oracle O10).  Returns (X, CGInfo)
+    with iterations = inner iterations in total and reliable_updates = outer corrections."""
+    phi = np.ascontiguousarray(phi, dtype=np.complex128)
+    b = np.ascontiguousarray(b, dtype=np.complex128)
+    dims = phi.shape
+    X = np.zeros_like(b)
+    info = _Info()
+    rc = lib().orc_cg_dc_f16(_method(dims, method), _dims(dims), _dp(phi), _dp(b), _dp(X), _c2(m), _c2(g),
+                             ctypes.c_double(rho), ctypes.c_double(tol), ctypes.c_double(inner_tol), int(max_iter),
+                             ctypes.byref(info))
+    if rc:
+        raise ValueError("oracle cg_dc_f16 failed")
+    return X, CGInfo(info.iterations, info.reliable_updates, bool(info.converged), info.rel_residual_recursive,
+                     info.rel_residual_true, np.zeros(0))

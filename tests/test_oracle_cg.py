@@ -144,3 +144,44 @@ def test_cg_trajectory_is_fixed_early_and_rounding_decides_late(orc):
     vals = list(counts.values())
     assert max(vals) - min(vals) >= 3          # +-2 is not determined by the method at this stop
     assert max(vals) - min(vals) <= 0.02 * min(vals)   # ... but 1.5 % is
+
+
+def test_round_f16_model_equals_ieee_binary16(orc):
+    """The oracle's binary16 rounding model against numpy's float16 conversion (an independent IEEE
+    implementation): random values over the whole range, ties, subnormals, the largest finite value; the one
+    stated difference is saturation (numpy overflows to inf)."""
+    rng = np.random.default_rng(5)
+    x = np.concatenate([rng.standard_normal(4000) * 10.0 ** rng.integers(-9, 5, 4000),
+                        np.array([0.0, -0.0, 1.0, 1.0 + 2.0 ** -11, 1.0 + 3 * 2.0 ** -11, 2.0 ** -14, 2.0 ** -24, 2.0 ** -25,
+                                  3 * 2.0 ** -25, 6.0e-8, 65504.0, 65519.0, -65519.0, 1e-30])])
+    got = orc.round_f16(x)
+    with np.errstate(over="ignore"):
+        want = x.astype(np.float16).astype(np.float64)
+    assert np.array_equal(got, want)
+    assert orc.round_f16(np.array([65520.0, 1e9, -7e4])).tolist() == [65504.0, 65504.0, -65504.0]  # saturates
+
+
+def test_cg_dc_f16_converges_to_the_dense_solution(orc):
+    """O10: defect correction with binary16 storage of r, p, chi reaches the single-precision tolerance; solution
+    against the dense solve, residual recomputed independently, several outer corrections of about inner_tol each,
+    and a modest iteration overhead over the complex64 loop O9 (measured at 8^4 / 16^4: +9 ... +25 %)."""
+    dims = (4, 4, 4, 4)
+    cfg = inputs.CONFIGS[1]
+    phi = inputs.make_phi(1, dims, cfg["sigma"]).astype(np.complex64).astype(np.complex128)
+    b = inputs.make_source(1, 0, dims).astype(np.complex64).astype(np.complex128)
+    M = dense_route.fermion_matrix_dense(dims, phi, cfg["m"], cfg["g"], 1.0)
+    A = M.conj().T @ M
+    xd = np.linalg.solve(A, b.reshape(-1)).reshape(b.shape)
+    X, info = orc.cg_dc_f16(phi, b, cfg["m"], cfg["g"], 1.0, 1e-6, 1e-1, 20000, "naive")
+    assert info.converged and info.rel_residual_true <= 1e-6
+    res = np.linalg.norm(b.reshape(-1) - A @ X.reshape(-1)) / np.linalg.norm(b)
+    assert abs(res - info.rel_residual_true) <= 1e-3 * res + 2e-12
+    assert np.linalg.norm(X - xd) <= 1e-3 * np.linalg.norm(xd)   # kappa * tol
+    assert 5 <= info.reliable_updates <= 9                        # 1e-6 in steps of about 1e-1
+    _, i64 = orc.cg_dc(phi, b, cfg["m"], cfg["g"], 1.0, 1e-6, 1e-3, 20000, "naive")
+    print("4^4: binary16 storage %d iterations in %d corrections, complex64 loop %d in %d"
+          % (info.iterations, info.reliable_updates, i64.iterations, i64.reliable_updates))
+    assert 0.8 * i64.iterations <= info.iterations <= 1.6 * i64.iterations
+    # a tighter inner tolerance than binary16 can deliver per correction still converges (more iterations per step)
+    _, i2 = orc.cg_dc_f16(phi, b, cfg["m"], cfg["g"], 1.0, 1e-6, 1e-2, 20000, "naive")
+    assert i2.converged and i2.reliable_updates < info.reliable_updates
