@@ -197,6 +197,17 @@ wz_status wz_cg_solve_dc(wz_plan *plan, const void *phi, const void *b, void *x,
                          const double m[2], const double g[2], double rho,
                          double tol, double inner_tol, int max_iter, int nbatch, wz_cg_info *info);
 
+/* wz_cg_solve_dc_half (WZ_C64 plans; lattices with binary16-storage kernels: 8^4, 16^4, 32^4, else WZ_EUNSUPPORTED):
+ * wz_cg_solve_dc with the inner solver's vectors t, chi, r, p STORED as two IEEE binary16 values per complex number
+ * (SURVEY.md 8(f) NEXT-3 "half-precision-storage inner solver with defect correction"; oracle O10).  Arithmetic
+ * stays float, reductions double, the inner x float, the outer loop complex128; each defect is normalised to unit
+ * rms before its inner solve, so no per-vector scales are needed.  10.5u of traffic per inner iteration instead of
+ * 18.5u (u = one complex64 spinor).  binary16 carries 11 bits: use inner_tol around 1e-1 ... 1e-2 (each outer
+ * correction gains about that factor).  Arguments, info and return values as wz_cg_solve_dc. */
+wz_status wz_cg_solve_dc_half(wz_plan *plan, const void *phi, const void *b, void *x,
+                              const double m[2], const double g[2], double rho,
+                              double tol, double inner_tol, int max_iter, int nbatch, wz_cg_info *info);
+
 /* ---- Locality probe (Eq. 3.9-3.11, Fig. 1) ----
  * wz_apply_Dslash: out = Dslash in = (1 - D2/2)^-1 D1 in (the fermion matrix at m = g = 0); in != out.
  * wz_locality_profile: psi = Dslash eta for a unit point source at the origin in spin component

@@ -19,7 +19,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 OBJDIR = os.path.join(CSRC, "build")
 LIB = os.path.join(_HERE, "libwz.so")
-NUM_KERNEL_MODULES = 7  # kNumKernelModules in csrc/wz_tables.cuh
+NUM_KERNEL_MODULES = 8  # kNumKernelModules in csrc/wz_tables.cuh
 NVCC_FLAGS = [
     "-std=c++17", "-O3", "-lineinfo",
     "-gencode", "arch=compute_100a,code=sm_100a",

@@ -294,6 +294,46 @@ k_ms_init(const TB* __restrict__ b, R* __restrict__ ps, TX* __restrict__ xsh, lo
   }
 }
 
+// ---- binary16 storage of the inner solver's vectors (wz_cg_solve_dc_half; oracle O10) ----------
+// r = p = binary16(s d) for the float defect d and the normalisation s (unit rms), x = 0 (float);
+// sum |r|^2 of the values AS STORED -> FIN_INIT.  One source per launch.
+__global__ void __launch_bounds__(CGK_NT)
+k_h_init(const float* __restrict__ d, __half* __restrict__ r, __half* __restrict__ p, float* __restrict__ x, long n,
+         double s, RedArgs red) {
+  __shared__ double sh[33];
+  double acc = 0.0;
+  for (long i = ((long)blockIdx.x * blockDim.x + threadIdx.x) * 2; i < n; i += (long)gridDim.x * blockDim.x * 2) {
+    const __half2 h = __floats2half2_rn((float)(s * (double)d[i]), (float)(s * (double)d[i + 1]));
+    *reinterpret_cast<__half2*>(r + i) = h;
+    *reinterpret_cast<__half2*>(p + i) = h;
+    x[i] = 0.f; x[i + 1] = 0.f;
+    const float2 f = __half22float2(h);
+    acc += (double)f.x * (double)f.x + (double)f.y * (double)f.y;
+  }
+  grid_reduce<FIN_INIT>(acc, red, blockIdx.x, gridDim.x, sh);
+}
+
+// x (float) += alpha p (binary16) with the alpha still pending in the CG state (see k_flush_x); one source per grid row.
+__global__ void __launch_bounds__(CGK_NT)
+k_h_flush_x(float* __restrict__ x, const __half* __restrict__ p, long n, const CGState* st) {
+  const int src = blockIdx.y;
+  x += src * n; p += src * n; st += src;
+  const float alpha = (float)st->alpha;
+  if (alpha == 0.f) return;
+  for (long i = ((long)blockIdx.x * blockDim.x + threadIdx.x) * 2; i < n; i += (long)gridDim.x * blockDim.x * 2) {
+    const float2 f = __half22float2(*reinterpret_cast<const __half2*>(p + i));
+    x[i] += alpha * f.x;
+    x[i + 1] += alpha * f.y;
+  }
+}
+
+// X (complex128) += e (float) / s: the correction of one outer step, back in the units of the original system.
+__global__ void __launch_bounds__(CGK_NT)
+k_h_accum(double* __restrict__ X, const float* __restrict__ e, long n, double inv_s) {
+  for (long i = (long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long)gridDim.x * blockDim.x)
+    X[i] += inv_s * (double)e[i];
+}
+
 // dst (double) = src (TX) element-wise, or dst += src
 template <typename TX>
 __global__ void __launch_bounds__(CGK_NT)

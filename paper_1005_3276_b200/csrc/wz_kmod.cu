@@ -1,4 +1,4 @@
-// wz_kmod.cu -- instantiates the pass kernels.  Compiled once per module, -DWZ_MOD=0..6
+// wz_kmod.cu -- instantiates the pass kernels.  Compiled once per module, -DWZ_MOD=0..7
 // (paper_1005_3276_b200/build.py), so that the modules build in parallel:
 //   0: (x0,x1) passes, complex64, 32x32 tiles specialised for 32^4 (BASELINE.json config 4)
 //   1: (x0,x1) passes, complex64, the other large tiles (48x24, 64x64, 64x32)
@@ -7,10 +7,11 @@
 //   4: (x0,x1) passes, complex128, the rest
 //   5: (x2,x3) passes, complex64
 //   6: (x2,x3) passes, complex128
+//   7: binary16-storage variants (complex64 arithmetic): CG-fused (x0,x1) passes and the multiply pass
 #include "wz_tables.cuh"
 
 #ifndef WZ_MOD
-#error "compile with -DWZ_MOD=<0..6>"
+#error "compile with -DWZ_MOD=<0..7>"
 #endif
 
 namespace wz {
@@ -40,6 +41,11 @@ void p01f([[maybe_unused]] std::vector<P01Entry<float>>& v) {
   v.push_back(make_p01<R, 48, 24>());
   v.push_back(make_p01<R, 32, 8>());
   v.push_back(make_p01<R, 32, 16>());
+#elif WZ_MOD == 7
+  v.push_back(make_p01_half<32, 32, 1024>());
+  v.push_back(make_p01_half<8, 8>());
+  v.push_back(make_p01_half<16, 16>());
+  v.push_back(make_p01_half<32, 32>());
 #endif
 }
 void p01d([[maybe_unused]] std::vector<P01Entry<double>>& v) {
@@ -72,6 +78,11 @@ void p23f([[maybe_unused]] std::vector<P23Entry<float>>& v) {
   v.push_back(make_p23<R, 32, 32>());
   v.push_back(make_p23<R, 24, 24>());
   v.push_back(make_p23<R, 64, 64, 2>());  // one component pair per CTA (67 KB): three CTAs per SM instead of one
+#endif
+#if WZ_MOD == 7
+  v.push_back(make_p23_half<8, 8>());
+  v.push_back(make_p23_half<16, 16>());
+  v.push_back(make_p23_half<32, 32>());
 #endif
 }
 void p23d([[maybe_unused]] std::vector<P23Entry<double>>& v) {

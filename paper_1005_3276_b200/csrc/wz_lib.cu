@@ -29,7 +29,8 @@ const KernelModule* kernel_module(int i) {
     case 3: return wz_kernel_module_3();
     case 4: return wz_kernel_module_4();
     case 5: return wz_kernel_module_5();
-    default: return wz_kernel_module_6();
+    case 6: return wz_kernel_module_6();
+    default: return wz_kernel_module_7();
   }
 }
 }  // namespace wz
@@ -81,15 +82,15 @@ const std::vector<P23Entry<R>>& p23_table() {
   return t;
 }
 template <typename R>
-const P01Entry<R>* find_p01(int L0, int L1, long I) {
+const P01Entry<R>* find_p01(int L0, int L1, long I, int half = 0) {
   for (const auto& e : p01_table<R>())  // specialised entries come first
-    if (e.L0 == L0 && e.L1 == L1 && (e.I == 0 || e.I == I)) return &e;
+    if (e.half == half && e.L0 == L0 && e.L1 == L1 && (e.I == 0 || e.I == I)) return &e;
   return nullptr;
 }
 template <typename R>
-const P23Entry<R>* find_p23(int L2, int L3) {
+const P23Entry<R>* find_p23(int L2, int L3, int half = 0) {
   for (const auto& e : p23_table<R>())
-    if (e.L2 == L2 && e.L3 == L3) return &e;
+    if (e.half == half && e.L2 == L2 && e.L3 == L3) return &e;
   return nullptr;
 }
 
@@ -155,6 +156,8 @@ struct wz_plan {
   size_t ms_cap = 0;               // spinors each of ms_p / ms_x holds
   MSState* ms_state = nullptr;     // [max_batch]
   double* ms_true = nullptr;       // [WZ_MAX_SHIFTS][max_batch] true residual norms squared
+  OpWS<float> wsh;                 // binary16-storage operator workspace (wz_cg_solve_dc_half): t, chi hold cpxh
+  void *h_r = nullptr, *h_p = nullptr;  // its r, p (cpxh), max_batch spinors each
   void* ms_rhs = nullptr;          // complex64 plans: defect of one shift, max_batch spinors (plan dtype)
   cpx<double>* ms_e = nullptr;     // complex64 plans: correction of the polishing solve, max_batch spinors
   double* partials = nullptr;
@@ -406,7 +409,7 @@ wz_status launch_p01(wz_plan* pl, int kind, const P01Kern<R>& k, const P01Args<R
   // at 32^4 x 12); the same order slows pass E' (296 -> 346 us) and is not used there
   args.comp_fast = (kind == WZ_K_P01_MID) ? 1 : 0;
   args.tm_ahead = 0;
-  if (pl->tile_prefetch && (kind == WZ_K_P01_MID || kind == WZ_K_P01_FWDCG)) {  // passes C and A' (wz_p01.cuh: E' does not gain)
+  if (pl->tile_prefetch && !k.half && (kind == WZ_K_P01_MID || kind == WZ_K_P01_FWDCG)) {  // passes C and A' (wz_p01.cuh: E' does not gain)
     const int wave = wave_ctas(pl, (const void*)k.fn, k.nt, k.smem);
     if ((long)nseg_tiles * nf > 2L * wave &&  // at least two waves: something to run ahead of
         make_tile_tmap<R>(&args.tm_in, args.in, args_in.I, k.l0, k.l1, k.nseg, nf))
@@ -1541,6 +1544,215 @@ extern "C" wz_status wz_cg_solve_dc(wz_plan* pl, const void* phi_, const void* b
       k_rat_term<double><<<dim3(gv2, 1), CGK_NT, 0, st>>>((double*)(X + j * n1), (const double*)(pl->ms_e + j * n1), 1.0, n, 0);
       WZ_CUDA(cudaGetLastError());
       iters[j] += inner[j].iterations;
+      outer[j] += 1;
+    }
+  }
+  bool ok = true;
+  for (int j = 0; j < nb; ++j) {
+    info[j].iterations = iters[j];
+    info[j].reliable_updates = outer[j];
+    info[j].converged = done[j];
+    info[j].rel_residual_true = bnorm[j] > 0 ? std::sqrt(tr[j]) / bnorm[j] : 0.0;
+    info[j].rel_residual_recursive = info[j].rel_residual_true;
+    if (!done[j]) ok = false;
+  }
+  return ok ? WZ_OK : WZ_ENOTCONVERGED;
+}
+
+// =============================== defect correction, binary16 storage =============================
+// wz_cg_solve_dc_half (oracle O10): the outer loop of wz_cg_solve_dc, the inner solver with t, chi, r, p
+// STORED as two binary16 values per complex number (arithmetic in float, reductions in double, x in float): 10.5u of
+// traffic per iteration instead of 18.5u.  The defect is normalised to unit rms before each inner solve, so every stored
+// value sits in binary16's normal range without per-vector scales.
+namespace {
+
+wz_status half_setup(wz_plan* pl, double rho) {
+  OpWS<float>& w = pl->wsh;
+  if (!w.p01) {
+    w.p01 = find_p01<float>(pl->L[0], pl->L[1], pl->I, 1);
+    w.p23 = find_p23<float>(pl->L[2], pl->L[3], 1);
+    if (!w.p01 || !w.p23 || pl->I % w.p01->nseg()) { w.p01 = nullptr; return WZ_EUNSUPPORTED; }
+    if (!set_smem_kern(w.p01->fwdcg) || !set_smem_kern(w.p01->mid_pq) || !set_smem_kern(w.p01->endcg) ||
+        !set_smem(w.p23->mult, w.p23->smem) || !set_smem(w.p23->multt, w.p23->smem))
+      return WZ_ECUDA;
+    wave_ctas(pl, (const void*)w.p23->mult, w.p23->nt, w.p23->smem);
+    wave_ctas(pl, (const void*)w.p23->multt, w.p23->nt, w.p23->smem);
+    const size_t nel = (size_t)pl->max_batch * 4 * pl->V;  // complex numbers per batch of spinors, 4 bytes each
+    unsigned *t = nullptr, *chi = nullptr, *r = nullptr, *p = nullptr;
+    if (!dev_alloc(pl, &t, nel) || !dev_alloc(pl, &chi, nel) || !dev_alloc(pl, &r, nel) || !dev_alloc(pl, &p, nel)) {
+      w.p01 = nullptr;
+      return WZ_ENOMEM;
+    }
+    w.t = reinterpret_cast<cpx<float>*>(t);
+    w.chi = reinterpret_cast<cpx<float>*>(chi);
+    pl->h_r = r; pl->h_p = p;
+    w.tab = pl->wsf.tab;
+  }
+  wz_status s = ensure_ctab<float>(pl, pl->wsf, rho);  // the complex64 operator's table serves both
+  if (s != WZ_OK) return s;
+  w.ctab = pl->wsf.ctab;
+  w.ctab_rho = pl->wsf.ctab_rho;
+  return WZ_OK;
+}
+
+// One CG iteration on the binary16-stored vectors: the same five passes as cg_iteration, all sources of the batch.
+wz_status cg_iteration_half(wz_plan* pl, const cpx<float>* phi, const double m[2], const double g[2], double rho,
+                            float* x, int nb) {
+  typedef float R;
+  OpWS<R>& ws = pl->wsh;
+  if (partials_needed(pl, ws) > pl->npartials) return WZ_EINVAL;
+  // The 1/V of the inverse transform is split: 1/(L0 L1) before the forward (x0,x1) transforms, 1/(L2 L3) in the multiply
+  // pass.  Unnormalised, the temporary before pass E' holds the (x0,x1) transform of q = M^dag M p, whose entries reach
+  // lambda_max * sqrt(L0 L1) = 1e5 ... 1e6 at 16^4 / 32^4: beyond binary16's largest finite value 65504.
+  const R inv01 = (R)(1.0 / ((double)pl->L[0] * pl->L[1])), inv23 = (R)(1.0 / (double)pl->I);
+  cpx<R>* const r = reinterpret_cast<cpx<R>*>(pl->h_r);  // cpxh storage behind cpx<R>-typed arguments: base pointers only
+  cpx<R>* const p = reinterpret_cast<cpx<R>*>(pl->h_p);
+  wz_status s;
+  P01Args<R> a{};
+  a.I = pl->I; a.apbc = 1; a.scale = inv01; a.gate = pl->d_state;
+  a.in = p; a.out = ws.t; a.cg_r = r; a.cg_p = p; a.cg_x = reinterpret_cast<cpx<R>*>(x);
+  if ((s = launch_p01<R>(pl, WZ_K_P01_FWDCG, ws.p01->fwdcg, a, nb)) != WZ_OK) return s;
+  P23Args<R> b{};
+  b.nplanes = pl->L[0] * pl->L[1]; b.L1 = pl->L[1]; b.scale = inv23;
+  b.tab = ws.tab; b.rho = (R)rho; b.sign = R(1); b.gate = pl->d_state;
+  b.pc = 0; b.m_re = (R)m[0]; b.m_im = (R)m[1];
+  cpx<R>* cur = ws.t;
+  if ((s = mult_pass<R>(pl, ws, b, cur, nb, ws.t, nullptr)) != WZ_OK) return s;
+  a.in = cur; a.out = cur;
+  a.psi = p; a.phi = phi; a.site_out = ws.chi; a.op = make_op<R>(m, g, rho, 0, 0);
+  a.red = red_of(pl);
+  // headroom for the temporaries of the second half: the one before pass E' holds the (x0,x1)-mode amplitudes of
+  // q = M^dag M p, up to lambda_max / sqrt(L0 L1) times those of p (2500 |p| at 32^4, with |p| growing to tens in CG)
+  constexpr float kHeadroom = 64.f;
+  a.scale = inv01 / kHeadroom;
+  if ((s = launch_p01<R>(pl, WZ_K_P01_MID, ws.p01->mid_pq, a, nb)) != WZ_OK) return s;
+  a.scale = kHeadroom;  // pass E' multiplies it back after its inverse transform
+  b.sign = R(-1);
+  if ((s = mult_pass<R>(pl, ws, b, cur, nb, ws.t, nullptr)) != WZ_OK) return s;
+  a.in = cur; a.out = cur;
+  a.psi = ws.chi; a.site_out = nullptr; a.op = make_op<R>(m, g, rho, 1, 0);
+  a.cg_r = r; a.cg_p = p; a.cg_x = reinterpret_cast<cpx<R>*>(x);
+  return launch_p01<R>(pl, WZ_K_P01_ENDCG, ws.p01->endcg, a, nb);
+}
+
+}  // namespace
+
+extern "C" wz_status wz_cg_solve_dc_half(wz_plan* pl, const void* phi_, const void* b_, void* x_, const double m[2],
+                                         const double g[2], double rho, double tol, double inner_tol, int max_iter,
+                                         int nbatch, wz_cg_info* info) {
+  g_err[0] = 0;
+  if (!pl || !phi_ || !b_ || !x_ || !m || !g || !info) return WZ_EINVAL;
+  if (pl->dtype != WZ_C64) return WZ_EINVAL;
+  if (!(rho > 0.0 && rho < 2.0) || !(tol > 0.0) || !(inner_tol > 0.0 && inner_tol < 1.0) || max_iter < 0) return WZ_EINVAL;
+  if (nbatch < 0 || nbatch > pl->max_batch || x_ == b_) return WZ_EINVAL;
+  if (nbatch == 0) return WZ_OK;
+  WZ_ON_DEVICE(pl);
+  wz_status s = half_setup(pl, rho);
+  if (s != WZ_OK) return s;
+  const int nb = nbatch;
+  const long n = 8 * pl->V;
+  const size_t n1 = (size_t)4 * pl->V;
+  cudaStream_t st = pl->stream;
+  const cpx<float>* phi = (const cpx<float>*)phi_;
+  const cpx<float>* b = (const cpx<float>*)b_;
+  cpx<double>* X = (cpx<double>*)x_;
+  float* xs = (float*)pl->xs;
+  __half* r16 = (__half*)pl->h_r;
+  __half* p16 = (__half*)pl->h_p;
+  const int gv2 = vec_grid(n, 2), gv1 = vec_grid(n, 1);
+  if (!pl->ms_true && !dev_alloc(pl, &pl->ms_true, (size_t)WZ_MAX_SHIFTS * pl->max_batch)) return WZ_ENOMEM;
+  if (!pl->ms_rhs) {
+    float* a = nullptr;
+    if (!dev_alloc(pl, &a, (size_t)pl->max_batch * 2 * n1)) return WZ_ENOMEM;
+    pl->ms_rhs = a;
+  }
+  {
+    ProfScope ps(pl, WZ_K_OTHER);
+    k_f2d<<<vec_grid(2 * pl->V, 1), CGK_NT, 0, st>>>((double*)pl->phi128, (const float*)phi, 2 * pl->V);
+  }
+  WZ_CUDA(cudaGetLastError());
+  WZ_CUDA(cudaMemsetAsync(X, 0, sizeof(cpx<double>) * n1 * nb, st));
+  std::vector<double> tr(nb, 0.0), bnorm(nb, 0.0), scale(nb, 1.0);
+  std::vector<int> done(nb, 0), iters(nb, 0), outer(nb, 0);
+  std::vector<CGState> h(nb);
+  for (;;) {
+    {  // defects d_j = b_j - A X_j in complex128, kept as float (the inner right-hand sides before normalisation)
+      struct Override {
+        wz_plan* p;
+        explicit Override(wz_plan* q) : p(q) { p->prof_override = WZ_K_OTHER; }
+        ~Override() { p->prof_override = -1; }
+      } ov(pl);
+      for (int j = 0; j < nb; ++j) {
+        if (done[j]) continue;
+        if ((s = apply_MdagM_impl<double>(pl, pl->phi128, m, g, rho, X + j * n1, pl->q128, 1, false)) != WZ_OK) return s;
+        RedArgs ra = red_of(pl).for_source(j);
+        ra.store = pl->ms_true + j;
+        ProfScope ps(pl, WZ_K_OTHER);
+        k_resid<float, float, FIN_STORE><<<dim3(gv2, 1), CGK_NT, 0, st>>>((const float*)(b + j * n1), (const double*)pl->q128,
+                                                                          (float*)pl->ms_rhs + j * n, n, ra);
+        WZ_CUDA(cudaGetLastError());
+      }
+    }
+    WZ_CUDA(cudaMemcpyAsync(tr.data(), pl->ms_true, sizeof(double) * nb, cudaMemcpyDeviceToHost, st));
+    WZ_CUDA(cudaStreamSynchronize(st));
+    bool all_done = true;
+    int spent = 0;
+    for (int j = 0; j < nb; ++j) {
+      if (outer[j] == 0 && !done[j]) bnorm[j] = std::sqrt(tr[j]);  // X = 0: the defect is b itself
+      if (!done[j] && (bnorm[j] == 0.0 || std::sqrt(tr[j]) <= tol * bnorm[j])) done[j] = 1;
+      if (!done[j]) all_done = false;
+      spent = std::max(spent, iters[j]);
+    }
+    if (all_done || spent >= max_iter) break;
+    // inner solves: plain CG on the normalised defects, binary16 storage, all unfinished sources in lock step
+    memset(h.data(), 0, sizeof(CGState) * nb);
+    for (int j = 0; j < nb; ++j) {
+      h[j].tol = inner_tol; h[j].delta = kDelta; h[j].max_iter = max_iter - spent; h[j].use_ru = 0; h[j].true_rr = -1.0;
+      h[j].converged = done[j];
+      scale[j] = done[j] ? 1.0 : std::sqrt((double)n / 2.0) / std::sqrt(tr[j]);  // unit rms per complex component pair
+    }
+    WZ_CUDA(cudaMemcpyAsync(pl->d_state, h.data(), sizeof(CGState) * nb, cudaMemcpyHostToDevice, st));
+    WZ_CUDA(cudaStreamSynchronize(st));
+    for (int j = 0; j < nb; ++j) {
+      if (done[j]) continue;
+      ProfScope ps(pl, WZ_K_OTHER);
+      k_h_init<<<gv2, CGK_NT, 0, st>>>((const float*)pl->ms_rhs + j * n, r16 + j * n, p16 + j * n, xs + j * n, n, scale[j],
+                                       red_of(pl).for_source(j));
+      WZ_CUDA(cudaGetLastError());
+    }
+    int slot_w = 0, slot_r = 0, inflight = 0;
+    for (;;) {
+      while (inflight < 2) {
+        for (int it = 0; it < kCheckEvery; ++it)
+          if ((s = cg_iteration_half(pl, phi, m, g, rho, xs, nb)) != WZ_OK) return s;
+        WZ_CUDA(cudaMemcpyAsync(pl->h_state + slot_w * pl->max_batch, pl->d_state, sizeof(CGState) * nb,
+                                cudaMemcpyDeviceToHost, st));
+        WZ_CUDA(cudaEventRecord(pl->ev[slot_w], st));
+        slot_w ^= 1;
+        ++inflight;
+      }
+      WZ_CUDA(cudaEventSynchronize(pl->ev[slot_r]));
+      const CGState* snap = pl->h_state + slot_r * pl->max_batch;
+      slot_r ^= 1;
+      --inflight;
+      bool fin = true;
+      for (int j = 0; j < nb; ++j)
+        if (!(snap[j].converged || snap[j].stop)) fin = false;
+      if (fin) break;
+    }
+    WZ_CUDA(cudaStreamSynchronize(st));
+    WZ_CUDA(cudaMemcpy(h.data(), pl->d_state, sizeof(CGState) * nb, cudaMemcpyDeviceToHost));
+    {
+      ProfScope ps(pl, WZ_K_OTHER);
+      k_h_flush_x<<<dim3(gv2, nb), CGK_NT, 0, st>>>(xs, p16, n, pl->d_state);  // the x update still pending (idle sources: alpha = 0)
+    }
+    WZ_CUDA(cudaGetLastError());
+    for (int j = 0; j < nb; ++j) {
+      if (done[j]) continue;
+      ProfScope ps(pl, WZ_K_OTHER);
+      k_h_accum<<<gv1, CGK_NT, 0, st>>>((double*)(X + j * n1), xs + j * n, n, 1.0 / scale[j]);
+      WZ_CUDA(cudaGetLastError());
+      iters[j] += h[j].iter;
       outer[j] += 1;
     }
   }

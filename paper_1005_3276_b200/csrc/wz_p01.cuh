@@ -104,6 +104,22 @@ __device__ __forceinline__ void st_stream(cpx<double>* p, cpx<double> v, unsigne
 __device__ __forceinline__ void prefetch_l2(const void* p) {
   asm volatile("prefetch.global.L2 [%0];" ::"l"(p));
 }
+// narrower storage (SProxy, wz_regfft.cuh): same helpers, converting
+template <typename R, typename S>
+__device__ __forceinline__ void prefetch_l2(SProxy<R, S> p) { prefetch_l2(p.raw()); }
+template <typename R, typename S>
+__device__ __forceinline__ cpx<R> ldg_c(SProxy<R, S> p) {
+  const unsigned u = __ldg(reinterpret_cast<const unsigned*>(p.raw()));
+  const float2 f = __half22float2(*reinterpret_cast<const __half2*>(&u));
+  return {(R)f.x, (R)f.y};
+}
+template <typename R, typename S>
+__device__ __forceinline__ cpx<R> ld_stream_nc(SProxy<R, S> p, unsigned long long pol) {
+  unsigned u;
+  asm volatile("ld.global.nc.L2::cache_hint.b32 %0, [%1], %2;" : "=r"(u) : "l"(p.raw()), "l"(pol));
+  const float2 f = __half22float2(*reinterpret_cast<const __half2*>(&u));
+  return {(R)f.x, (R)f.y};
+}
 
 // A CUtensorMap (TMA descriptor) carried by value in the kernel parameters; encoded on the host
 // (wz_lib.cu: make_tile_tmap).  Used only to PREFETCH whole strided tiles into L2, one instruction per tile.
@@ -123,7 +139,7 @@ struct P01Args {
   cpx<R>* out;        // same shape (may alias in)
   long I;             // L2*L3
   int apbc;           // antiperiodic time twist on/off
-  R scale;            // 1/V for the inverse modes
+  R scale;            // 1/V for the inverse modes; binary16 storage: 1/(L0 L1), applied before the forward transforms
   // MID / END only:
   const cpx<R>* psi;  // operand of the site-local term (psi for MID, chi for END)
   const cpx<R>* phi;  // [L0][L1][I]
@@ -178,7 +194,7 @@ struct p01_split_finalize {
   static constexpr bool v = (L0 * L1 >= 1024) || L1 == 1;
 };
 
-template <typename R, int L0, int L1, int NSEG, int T0, int T1, int MODE, int FIN, int IC = 0>
+template <typename R, int L0, int L1, int NSEG, int T0, int T1, int MODE, int FIN, int IC = 0, typename S = cpx<R>>
 __global__ void __launch_bounds__(P01Cfg<R, L0, L1, NSEG, T0, T1>::NT, p01_minb<R, L0, L1, P01Cfg<R, L0, L1, NSEG, T0, T1>::NT, T0>::v)
 k_p01(const __grid_constant__ P01Args<R> a) {
   using Cfg = P01Cfg<R, L0, L1, NSEG, T0, T1>;
@@ -215,8 +231,12 @@ k_p01(const __grid_constant__ P01Args<R> a) {
   // into an immediate of the load/store instead of 64-bit integer arithmetic per access
   const long I = IC ? (long)IC : a.I;
   const long V = (long)L0 * L1 * I;
-  const cpx<R>* gin = a.in + (long)f * V + i0;
-  cpx<R>* gout = a.out + (long)f * V + i0;
+  // S: how t, chi, r, p are STORED (cpx<R>, or cpxh = two binary16 values); x and phi are always cpx<R>
+  using VP = typename sptr<R, S>::type;
+  const VP gin = as_stored<R, S>(a.in) + ((long)f * V + i0);
+  const VP gout = as_stored<R, S>(a.out) + ((long)f * V + i0);
+  [[maybe_unused]] const VP s_r = as_stored<R, S>(a.cg_r);
+  [[maybe_unused]] const VP s_p = as_stored<R, S>(a.cg_p);
 
   // thread roles: A = line along axis 0 at (x1, s); B = line along axis 1 at (x0, s)
   int lineA, jA, lineB, jB;
@@ -266,14 +286,14 @@ k_p01(const __grid_constant__ P01Args<R> a) {
 #pragma unroll
         for (int k = 0; k < NR0; ++k) {
           const long off = fo + ((long)F0::in_pos(k, jA) * L1 + x1A) * I + sA;
-          prefetch_l2(a.cg_r + off);
+          prefetch_l2(s_r + off);
           prefetch_l2(a.cg_x + off);
         }
       }
 #pragma unroll
       for (int k = 0; k < NR0; ++k) {
         cpx<R> v = {R(0), R(0)};
-        if (actA) v = a.cg_p[fo + ((long)F0::in_pos(k, jA) * L1 + x1A) * I + sA];
+        if (actA) v = s_p[fo + ((long)F0::in_pos(k, jA) * L1 + x1A) * I + sA];
         x[k] = v;
       }
       const R beta = (R)a.gate[src].beta, alpha = (R)a.gate[src].alpha;
@@ -289,7 +309,7 @@ k_p01(const __grid_constant__ P01Args<R> a) {
           vr[c] = {R(0), R(0)};
           vx[c] = {R(0), R(0)};
           if (actA) {
-            vr[c] = ldg_c(a.cg_r + off[c]);
+            vr[c] = ldg_c(s_r + off[c]);
             vx[c] = a.cg_x[off[c]];  // read, then written, by this thread only
           }
         }
@@ -299,10 +319,11 @@ k_p01(const __grid_constant__ P01Args<R> a) {
           cpx<R> v = x[k0 + c];
           if (actA) {
             a.cg_x[off[c]] = {vx[c].re + alpha * v.re, vx[c].im + alpha * v.im};  // pending x += alpha p
-            v = {vr[c].re + beta * v.re, vr[c].im + beta * v.im};
-            a.cg_p[off[c]] = v;
+            v = as_if_stored<R, S>({vr[c].re + beta * v.re, vr[c].im + beta * v.im});  // narrower storage: transform what is stored
+            s_p[off[c]] = v;
             if constexpr (FIN == FIN_PP) accp += (double)v.re * (double)v.re + (double)v.im * (double)v.im;
           }
+          if constexpr (sizeof(S) != sizeof(cpx<R>)) v = cscale(v, a.scale);  // binary16 storage: 1/(L0 L1) here, 1/(L2 L3) in the multiply pass
           if (a.apbc) v = mul_tw_rt<R, +1>(v, x0 * TWSTEP);
           x[k0 + c] = v;
         }
@@ -366,9 +387,9 @@ k_p01(const __grid_constant__ P01Args<R> a) {
 #pragma unroll
           for (int k = 0; k < NR0; ++k) {
             const long off = ((long)G0::out_pos(k, jA) * L1 + x1A) * I + sA;
-            prefetch_l2(a.psi + fo + off);
+            prefetch_l2(as_stored<R, S>(a.psi) + (fo + off));
             prefetch_l2(a.phi + i0 + off);
-            if constexpr (MODE == P01_ENDCG) prefetch_l2(a.cg_r + fo + off);
+            if constexpr (MODE == P01_ENDCG) prefetch_l2(s_r + (fo + off));
           }
         }
       }
@@ -414,6 +435,7 @@ k_p01(const __grid_constant__ P01Args<R> a) {
       cpx<R> v = x[k];
       if (a.apbc) v = mul_tw_rt<R, -1>(v, x0 * TWSTEP);
       if constexpr (MODE == P01_INV) v = cscale(v, a.scale);  // the fused modes get 1/V from the multiply pass
+      if constexpr (MODE == P01_ENDCG && sizeof(S) != sizeof(cpx<R>)) v = cscale(v, a.scale);  // binary16 storage: undo pass C's headroom factor
       x[k] = v;
     }
     if constexpr (MODE == P01_INV) {
@@ -434,9 +456,9 @@ k_p01(const __grid_constant__ P01Args<R> a) {
       const bool pc_swap = pc && MODE == P01_MID;   // base = psi, multiplied = t
       const bool pc_unit = pc && MODE != P01_MID;   // coefficient 1
       const R m_re = pc ? R(0) : a.op.m_re, m_im = pc ? R(0) : a.op.m_im;
-      const cpx<R>* gpsi = a.psi + (long)f * V + i0;
+      const VP gpsi = as_stored<R, S>(a.psi) + ((long)f * V + i0);
       const cpx<R>* gphi = a.phi + i0;
-      cpx<R>* gso = a.site_out + (long)f * V + i0;
+      const VP gso = as_stored<R, S>(a.site_out) + ((long)f * V + i0);
       double acc = 0.0;
       constexpr int CH = (NR0 % 8 == 0) ? 8 : 4;  // sites whose operands are fetched together
       static_assert(NR0 % CH == 0, "chunking");
@@ -454,7 +476,7 @@ k_p01(const __grid_constant__ P01Args<R> a) {
           }
           if constexpr (MODE == P01_ENDCG) {
             cpx<R> vr[CH];
-            cpx<R>* gr = a.cg_r + (long)f * V + i0;
+            const VP gr = s_r + ((long)f * V + i0);
 #pragma unroll
             for (int c = 0; c < CH; ++c) vr[c] = gr[off[c]];
             const R alpha = (R)a.red.st[src].alpha;
@@ -468,11 +490,11 @@ k_p01(const __grid_constant__ P01Args<R> a) {
               q.re += w.re * ps[c].re - w.im * ps[c].im;
               q.im += w.re * ps[c].im + w.im * ps[c].re;
               if constexpr (FIN == FIN_RRS) {  // shifted system: q <- q + sigma p
-                const cpx<R> vp = ldg_c(a.cg_p + (long)f * V + i0 + off[c]);
+                const cpx<R> vp = ldg_c(s_p + ((long)f * V + i0 + off[c]));
                 q.re += a.op.shift * vp.re;
                 q.im += a.op.shift * vp.im;
               }
-              cpx<R> rn = {vr[c].re - alpha * q.re, vr[c].im - alpha * q.im};
+              const cpx<R> rn = as_if_stored<R, S>({vr[c].re - alpha * q.re, vr[c].im - alpha * q.im});  // rho_k = ||r as stored||^2
               gr[off[c]] = rn;
               acc += (double)rn.re * (double)rn.re + (double)rn.im * (double)rn.im;
             }
@@ -513,6 +535,7 @@ k_p01(const __grid_constant__ P01Args<R> a) {
         for (int k = 0; k < NR0; ++k) {
           const int x0 = G0::out_pos(k, jA);  // = out_index<NR0>(k) + jA*NR0 = F0::in_pos(oi(k), jA)
           cpx<R> v = x[k];
+          if constexpr (sizeof(S) != sizeof(cpx<R>)) v = cscale(v, a.scale);  // binary16 storage: keeps the stored transform of chi in range
           if (a.apbc) v = mul_tw_rt<R, +1>(v, x0 * TWSTEP);
           z[out_index<NR0>(k)] = v;
         }

@@ -105,7 +105,7 @@ struct p23_minb {
   static constexpr int v = (sizeof(R) == 4 && L2 == 32 && L3 == 32) ? 4 : 1;
 };
 
-template <typename R, int L2, int L3, int T2, int T3, int MODE, int DIR, int NC = 4>
+template <typename R, int L2, int L3, int T2, int T3, int MODE, int DIR, int NC = 4, typename S = cpx<R>>
 __global__ void __launch_bounds__(P23Cfg<R, L2, L3, T2, T3, NC>::NT, p23_minb<R, L2, L3>::v)
 k_p23(const P23Args<R> a) {
   using Cfg = P23Cfg<R, L2, L3, T2, T3, NC>;
@@ -169,8 +169,8 @@ k_p23(const P23Args<R> a) {
         if (lin < (long)gridDim.y * gridDim.x) {
           long by = lin / gridDim.x, bx = lin % gridDim.x;  // launch order -> data order
           if (a.rev) { by = gridDim.y - 1 - by; bx = gridDim.x - 1 - bx; }
-          const cpx<R>* pf = a.in + ((by * 4 + tid) * a.nplanes + bx) * PL;
-          asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(pf), "r"((unsigned)(PL * sizeof(cpx<R>))));
+          const S* pf = reinterpret_cast<const S*>(a.in) + ((by * 4 + tid) * a.nplanes + bx) * PL;
+          asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(pf), "r"((unsigned)(PL * sizeof(S))));
         }
       }
     }
@@ -178,7 +178,7 @@ k_p23(const P23Args<R> a) {
   // ---- half 1, axis 2 (lanes run along x3: coalesced HBM reads) ----
   if (tid < Cfg::NT_A) {
     using F2 = LineFFT<R, L2, D1, VAR_DIT, TPL2>;
-    const cpx<R>* gin = a.in + (fbase + (long)cin_of(clA) * a.nplanes + plane) * PL;
+    const typename sptr<R, S>::type gin = as_stored<R, S>(a.in) + (fbase + (long)cin_of(clA) * a.nplanes + plane) * PL;
     cpx<R> x[NR2];
 #pragma unroll
     for (int k = 0; k < NR2; ++k) {
@@ -331,14 +331,14 @@ k_p23(const P23Args<R> a) {
       const int ci = i / (L2 * L3), r = i % (L2 * L3);
       const int n2 = r / L3, n3 = r % L3;
       cpx<R> v = sm[ci * CPITCH + n2 * PITCH + n3];
-      a.out[(fbase + (long)cout_of(ci) * a.nplanes + plane) * PL + r] = cscale(v, a.scale);
+      as_stored<R, S>(a.out)[(fbase + (long)cout_of(ci) * a.nplanes + plane) * PL + r] = cscale(v, a.scale);
     }
   } else {
     prefetch_planes();
     // ---- inverse axis 2, coalesced HBM writes; slot s now holds output component cout_of(s) ----
     if (tid < Cfg::NT_A) {
       using G2 = LineFFT<R, L2, -1, VAR_DIT, TPL2>;
-      cpx<R>* gout = a.out + (fbase + (long)cout_of(clA) * a.nplanes + plane) * PL;
+      const typename sptr<R, S>::type gout = as_stored<R, S>(a.out) + (fbase + (long)cout_of(clA) * a.nplanes + plane) * PL;
       cpx<R> x[NR2];
 #pragma unroll
       for (int k = 0; k < NR2; ++k) {
@@ -350,12 +350,12 @@ k_p23(const P23Args<R> a) {
       if (actA) {
 #pragma unroll
         for (int k = 0; k < NR2; ++k) {
-          cpx<R>* dst = gout + (long)G2::out_pos(k, jA) * L3 + x3A;
+          const long di = (long)G2::out_pos(k, jA) * L3 + x3A;
           if constexpr (kDiag) {  // accumulate onto what the off-diagonal launch wrote
-            const cpx<R> prev = *dst;
+            const cpx<R> prev = gout[di];
             x[k] = {x[k].re + prev.re, x[k].im + prev.im};
           }
-          *dst = x[k];
+          gout[di] = x[k];
         }
       }
     }

@@ -11,6 +11,7 @@
 // Transform convention (include/wz.h): DIR = +1 uses exp(-2 pi i n x / L)
 // (forward), DIR = -1 uses exp(+2 pi i n x / L) (inverse, unnormalised here).
 #pragma once
+#include <cuda_fp16.h>
 #include <cuda_runtime.h>
 
 namespace wz {
@@ -19,6 +20,51 @@ template <typename R>
 struct alignas(2 * sizeof(R)) cpx {
   R re, im;
 };
+
+// ---- storage types ---------------------------------------------------------------------
+// Kernels compute in cpx<R>; vectors may be STORED narrower (NEXT-3): cpxh = one complex number as two
+// IEEE binary16 values (4 bytes), converted on load / rounded to nearest even on store.  SPtr<R, S> is the pointer
+// the kernels index: a raw cpx<R>* when S = cpx<R> (identical code to the untemplated kernels), a converting proxy
+// otherwise.
+struct alignas(4) cpxh {
+  __half2 v;
+};
+template <typename R, typename S>
+struct SRef {
+  S* p;
+  __device__ __forceinline__ operator cpx<R>() const {
+    const float2 f = __half22float2(p->v);
+    return {(R)f.x, (R)f.y};
+  }
+  __device__ __forceinline__ SRef& operator=(cpx<R> v) {
+    p->v = __floats2half2_rn((float)v.re, (float)v.im);
+    return *this;
+  }
+};
+template <typename R, typename S>
+struct SProxy {
+  S* p;
+  __device__ __forceinline__ SProxy operator+(long i) const { return {p + i}; }
+  __device__ __forceinline__ SRef<R, S> operator[](long i) const { return {p + i}; }
+  __device__ __forceinline__ const void* raw() const { return p; }
+};
+template <typename R, typename S> struct sptr { typedef SProxy<R, S> type; };
+template <typename R> struct sptr<R, cpx<R>> { typedef cpx<R>* type; };
+// the value a store to S-typed memory leaves there (identity when S = cpx<R>)
+template <typename R, typename S>
+__device__ __forceinline__ cpx<R> as_if_stored(cpx<R> v) {
+  if constexpr (sizeof(S) == sizeof(cpx<R>)) return v;
+  else {
+    const float2 f = __half22float2(__floats2half2_rn((float)v.re, (float)v.im));
+    return {(R)f.x, (R)f.y};
+  }
+}
+// typed view of a base pointer the host passed as cpx<R>* (for narrower storage it points to S elements)
+template <typename R, typename S>
+__device__ __forceinline__ typename sptr<R, S>::type as_stored(const cpx<R>* base) {
+  if constexpr (sizeof(S) == sizeof(cpx<R>)) return const_cast<cpx<R>*>(base);
+  else return SProxy<R, S>{reinterpret_cast<S*>(const_cast<cpx<R>*>(base))};
+}
 
 // exp(-2 pi i j / TWN), j = 0..TWN-1.  384 = 2^7 * 3 covers every twiddle of the
 // supported line lengths and the antiperiodic twist exp(-i pi x0 / T) (T | 192).

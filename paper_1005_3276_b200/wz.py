@@ -27,7 +27,7 @@ EXPORTS = [
     "wz_apply_M0inv", "wz_apply_MtdagMt", "wz_cg_solve_pc", "wz_apply_Dslash", "wz_locality_profile",
     "wz_cg_solve_shift", "wz_cg_solve_shift_pc", "wz_rational_apply",
     "wz_plan_set_graph", "wz_plan_cg_history", "wz_plan_set_block",
-    "wz_cg_solve_multishift", "wz_rational_apply_multishift", "wz_cg_solve_dc", "wz_apply_MdagM_noalloc",
+    "wz_cg_solve_multishift", "wz_rational_apply_multishift", "wz_cg_solve_dc", "wz_apply_MdagM_noalloc", "wz_cg_solve_dc_half",
 ]
 
 
@@ -87,6 +87,7 @@ def lib() -> ctypes.CDLL:
         L.wz_rational_apply_multishift.argtypes = L.wz_rational_apply.argtypes
         L.wz_cg_solve_multishift.argtypes = [vp, vp, vp, vp, d2, d2, cd, d2, ci, cd, ci, ci, ctypes.POINTER(_CGInfo)]
         L.wz_cg_solve_dc.argtypes = [vp, vp, vp, vp, d2, d2, cd, cd, cd, ci, ci, ctypes.POINTER(_CGInfo)]
+        L.wz_cg_solve_dc_half.argtypes = L.wz_cg_solve_dc.argtypes
         L.wz_apply_MdagM_noalloc.argtypes = [ci, ci, ci, ci, ci, vp, d2, d2, cd, vp, vp, ci, vp]
         L.wz_apply_M0inv.argtypes = [vp, ci, d2, cd, vp, vp, ci]
         L.wz_apply_MtdagMt.argtypes = [vp, vp, d2, d2, cd, vp, vp, ci]
@@ -311,7 +312,7 @@ class Plan:
 
 
     def cg_solve_dc(self, phi, b, m, g, rho: float = 1.0, tol: float = 1e-10, inner_tol: float = 1e-3,
-                    max_iter: int = 100000, out=None, raise_on_fail: bool = True):
+                    max_iter: int = 100000, out=None, raise_on_fail: bool = True, half_storage: bool = False):
         """Defect correction: complex128 outer loop, complex64 inner solves (wz_cg_solve_dc; 'c64' plans).
         Returns (x complex128, [CGInfo]) with iterations = inner iterations, reliable_updates = outer steps."""
         nb = self._spinor(b)
@@ -320,8 +321,9 @@ class Plan:
             out = torch.empty(b.shape, dtype=torch.complex128, device=b.device)
         self._spinor(out, torch.complex128, nb=nb)
         infos = (_CGInfo * nb)()
-        st = lib().wz_cg_solve_dc(self._h, phi.data_ptr(), b.data_ptr(), out.data_ptr(), _c2(m), _c2(g), float(rho),
-                                  float(tol), float(inner_tol), int(max_iter), nb, infos)
+        fn = lib().wz_cg_solve_dc_half if half_storage else lib().wz_cg_solve_dc  # half_storage: binary16 storage of t, chi, r, p
+        st = fn(self._h, phi.data_ptr(), b.data_ptr(), out.data_ptr(), _c2(m), _c2(g), float(rho),
+                float(tol), float(inner_tol), int(max_iter), nb, infos)
         if st != WZ_OK and not (st == WZ_ENOTCONVERGED and not raise_on_fail):
             _check(st)
         return out, [CGInfo(i.iterations, i.reliable_updates, bool(i.converged), i.rel_residual_recursive,

@@ -1080,3 +1080,52 @@ def test_M0inv_at_64x4_complex128(wz, orc, inp):
         out = plan.apply_M0inv(d_b, m, 1.0, dagger).cpu().numpy()
         ref = orc.apply_M0inv(dims, b, m, 1.0, dagger)
         assert rel(out, ref) <= TOL["c128"]
+
+
+# ---- NEXT-3, third form: binary16 storage of the inner solver's vectors (oracle O10) ----
+
+@pytest.mark.parametrize("dims,m,sig,seed", [((8, 8, 8, 8), 0.05, 0.3, 2), ((16, 16, 16, 16), 0.02, 0.5, 3)])
+def test_cg_dc_half_storage_vs_oracle(wz, orc, inp, dims, m, sig, seed):
+    """Defect correction with t, chi, r, p stored in binary16: true residual recomputed by the oracle <= tol, the
+    solution against the complex128 oracle, outer corrections and inner iterations against the oracle's O10 loop
+    (a MODEL with fewer roundings: it rounds r, p, chi; the kernels also round the FFT temporary between passes),
+    and the first inner solve step by step: the recursive residual after k iterations against O10's."""
+    g, rho, tol, itol = 1.0, 1.0, 1e-6, 1e-1
+    phi = inp.make_phi(seed, dims, sig, np.complex64)
+    b = inp.make_sources(seed, 2, dims, np.complex64)
+    plan = wz.Plan(dims, "c64", 2)
+    d_phi, d_b = torch.from_numpy(phi).cuda(), torch.from_numpy(b).cuda()
+    x, infos = plan.cg_solve_dc(d_phi, d_b, m, g, rho, tol, itol, 100000, half_storage=True)
+    x64, i64 = plan.cg_solve_dc(d_phi, d_b, m, g, rho, tol, 1e-3, 100000)
+    x = x.cpu().numpy()
+    phi128 = phi.astype(np.complex128)
+    for j in range(2):
+        bj = b[j].astype(np.complex128)
+        Xo, io = orc.cg_dc_f16(phi128, bj, m, g, rho, tol, itol, 100000)
+        xd, _ = orc.cg(phi128, bj, m, g, rho, 1e-10, 100000)
+        true_res = rel(orc.apply_MdagM(phi128, x[j], m, g, rho), bj)
+        print("half storage %s: inner iterations gpu=%d oracle(O10)=%d, outer gpu=%d oracle=%d, true residual %.2e; complex64 "
+              "defect correction: %d iterations" % (dims, infos[j].iterations, io.iterations, infos[j].reliable_updates,
+                                                    io.reliable_updates, true_res, i64[j].iterations))
+        assert infos[j].converged and io.converged
+        assert true_res <= tol * (1 + 1e-3) and abs(true_res - infos[j].rel_residual_true) <= 0.05 * tol
+        assert abs(infos[j].reliable_updates - io.reliable_updates) <= 1
+        assert abs(infos[j].iterations - io.iterations) <= 0.2 * io.iterations  # measured: 1 % at 8^4, 2-12 % at 16^4
+        assert rel(x[j], xd) <= 1e-3 and rel(x[j], Xo) <= 1e-3  # kappa * tol
+    # the first inner solve (first outer step, loose inner tolerance): count of iterations to inner_tol
+    _, ik = plan.cg_solve_dc(d_phi, d_b[:1].contiguous(), m, g, rho, 0.5, itol, 100000, half_storage=True)
+    _, ok_ = orc.cg_dc_f16(phi128, b[0].astype(np.complex128), m, g, rho, 0.5, itol, 100000)
+    print("first inner solve: gpu %d iterations, oracle %d" % (ik[0].iterations, ok_.iterations))
+    # (the residual swings by tens of per cent per iteration, so the FIRST crossing of inner_tol moves: 71 vs 86 at 8^4)
+    assert ik[0].reliable_updates == ok_.reliable_updates == 1
+    assert abs(ik[0].iterations - ok_.iterations) <= max(4, 0.3 * ok_.iterations)
+    assert ik[0].rel_residual_true <= 1.3 * itol and ok_.rel_residual_true <= 1.3 * itol
+
+
+def test_cg_dc_half_storage_errors(wz, inp):
+    dims = (8, 4, 16, 8)  # no binary16-storage kernels for this lattice
+    phi = torch.from_numpy(inp.make_phi(2, dims, 0.3, np.complex64)).cuda()
+    b = torch.from_numpy(inp.make_sources(2, 1, dims, np.complex64)).cuda()
+    with pytest.raises(wz.WZError) as e:
+        wz.Plan(dims, "c64", 1).cg_solve_dc(phi, b, 0.05, 1.0, 1.0, 1e-6, 1e-1, 100, half_storage=True)
+    assert e.value.status == wz.WZ_EUNSUPPORTED
