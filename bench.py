@@ -501,6 +501,10 @@ def run_wz(args):
         extras["heatbath_rational_sum"] = time_rational(plan, d_phi, d_b, d_x, cfg)
         extras["mixed_precision_to_1e-10"] = time_mixed(plan, d_phi, d_b, cfg, dev)
 
+    if not args.no_extras and key == 4:
+        extras["binary16_storage_to_1e-6"] = time_half_storage(plan, d_phi, d_b, d_x, cfg, secs / args.steps,
+                                                               [i.iterations for i in infos])
+
     cpu = None
     if not args.no_cpu_baseline and world == 1:
         ips, threads, text, _ = oracle_sample(cfg, oracle_iters_for(cfg))
@@ -670,6 +674,29 @@ def time_rational(plan, d_phi, d_b, d_x, cfg):
         "multishift_all_shifts": run(d_phi, b2, x2, cfg["m"], cfg["g"], -1.0, True, 100000),
         "plain_solve_per_shift": run(d_phi, b2, x2, cfg["m"], cfg["g"], -1.0, False, 100000)}
     return res
+
+
+def time_half_storage(plan, d_phi, d_b, d_x, cfg, c64_secs, c64_iterations):
+    """NEXT-3, third form (oracle O10): the same batch to the same tolerance by wz_cg_solve_dc_half --
+    defect correction with the inner solver's t, chi, r, p stored in binary16 (10.5u of traffic per iteration instead
+    of 18.5u) -- next to the complex64 solver of the timed steps.  The true residual is recomputed in complex128."""
+    import torch
+
+    a, e = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record()
+    _, infos = plan.cg_solve_dc(d_phi, d_b, cfg["m"], cfg["g"], cfg["rho"], cfg["tol"], 1e-1, 400000, out=d_x,
+                                raise_on_fail=False, half_storage=True)
+    e.record()
+    e.synchronize()
+    t = a.elapsed_time(e) * 1e-3
+    its = [i.iterations for i in infos]
+    return {"secs": t, "inner_tol": 1e-1, "inner_iterations": its, "outer_corrections": [i.reliable_updates for i in infos],
+            "us_per_source_iteration": 1e6 * t / max(sum(its), 1), "worst_true_residual": max(i.rel_residual_true for i in infos),
+            "all_converged": all(i.converged for i in infos),
+            "complex64_solver": {"secs": c64_secs, "iterations": c64_iterations,
+                                 "us_per_source_iteration": 1e6 * c64_secs / max(sum(c64_iterations), 1)},
+            "speedup_per_iteration": (c64_secs / max(sum(c64_iterations), 1)) / (t / max(sum(its), 1)),
+            "speedup_time_to_solution": c64_secs / t}
 
 
 def time_mixed(plan, d_phi, d_b, cfg, dev, nsrc=2):

@@ -31,6 +31,7 @@
 //   cg_multishift (O8)         : dense solves per shift; the single-shift loop's iteration counts and solutions;
 //                                the sequential rational sum.
 //   cg_dc (O9)                 : dense solve; independently recomputed residual; outer-step structure.
+//   cg_dc_f16 (O10)            : rounding model against numpy float16; dense solve; overhead over O9.
 //   Parity unpinned by anything the paper fixes: the ITERATION COUNT the reliable-update trigger of cg_c64ru
 //   produces (delta = 0.1, "keep p": reading G9 is not in the paper) -- the solution it returns is pinned.
 //   The solve at 16^4 and above with non-constant phi has no printed value in the
