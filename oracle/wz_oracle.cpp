@@ -31,7 +31,7 @@
 //   cg_multishift (O8)         : dense solves per shift; the single-shift loop's iteration counts and solutions;
 //                                the sequential rational sum.
 //   cg_dc (O9)                 : dense solve; independently recomputed residual; outer-step structure.
-//   cg_dc_f16 (O10)            : rounding model against numpy float16; dense solve; overhead over O9.
+//   cg_dc_f16 (O10), cg_f16ru (O11): rounding model against numpy float16; dense solve; overhead over O9 / O4'.
 //   Parity unpinned by anything the paper fixes: the ITERATION COUNT the reliable-update trigger of cg_c64ru
 //   produces (delta = 0.1, "keep p": reading G9 is not in the paper) -- the solution it returns is pinned.
 //   The solve at 16^4 and above with non-constant phi has no printed value in the
@@ -1103,6 +1103,80 @@ int orc_cg_dc_f16(int method, const int* L, const double* phi, const double* b_,
   info->converged = converged;
   info->rel_residual_recursive = bnorm > 0 ? Rnorm / bnorm : 0.0;
   info->rel_residual_true = bnorm > 0 ? Rnorm / bnorm : 0.0;
+  return 0;
+}
+
+// ----------------------------------------------------------------------------
+// O11 (NEXT-3, third form, with reliable updates). binary16 storage as in O10, but the Krylov space survives the
+// corrections: the loop of O4' (reading G9) on the NORMALISED system.  s = sqrt(n)/||b||, r = p = f16(s b), x = 0 (float),
+// X = 0 (complex128); per iteration chi = M p, q = M^dag f16(chi), alpha = rho/||chi||^2, x = f32(x + alpha p),
+// r = f16(r - alpha q); rmax = max ||r|| since the last update.  When ||r|| < delta rmax or ||r|| <= tol s ||b||:
+//   X += x / s; x = 0; R = b - A X (complex128); converged if ||R|| <= tol ||b||; else RESCALE to unit rms again:
+//   s' = sqrt(n)/||R||, f = s'/s: r = f16(s' R), p = f16(f p), rho_{k-1} <- f^2 rho_{k-1}, rho_k = ||r||^2, rmax = ||r||, s = s';
+// then beta = rho_k/rho_{k-1}, p = f16(r + beta p) as always.
+// ----------------------------------------------------------------------------
+int orc_cg_f16ru(int method, const int* L, const double* phi, const double* b_, double* X_,
+                 const double* m, const double* g, double rho, double tol, int max_iter, double delta,
+                 orc_cg_info* info) {
+  const long V = (long)L[0] * L[1] * L[2] * L[3];
+  const long n = 4 * V;
+  const cd* b = reinterpret_cast<const cd*>(b_);
+  cd* X = reinterpret_cast<cd*>(X_);
+  std::vector<cd> x(n, 0.0), r(n), p(n), chi(n), chi16(n), q(n);
+  const double bnorm = std::sqrt(dot_re(b, b, n));
+  for (long i = 0; i < n; ++i) X[i] = 0.0;
+  int k = 0, nru = 0, converged = (bnorm == 0.0);
+  double true_rel = converged ? 0.0 : 1.0;
+  double s = converged ? 1.0 : std::sqrt((double)n) / bnorm;
+  for (long i = 0; i < n; ++i) { r[i] = round_c16(s * b[i]); p[i] = r[i]; }
+  double rr = dot_re(r.data(), r.data(), n);
+  double rmax = std::sqrt(rr);
+  while (!converged && k < max_iter) {
+    ++k;
+    int rc = orc_apply_M(method, L, phi, m, g, rho, 0, reinterpret_cast<double*>(p.data()), reinterpret_cast<double*>(chi.data()));
+    if (rc) return rc;
+    for (long i = 0; i < n; ++i) chi16[i] = round_c16(chi[i]);
+    orc_apply_M(method, L, phi, m, g, rho, 1, reinterpret_cast<double*>(chi16.data()), reinterpret_cast<double*>(q.data()));
+    const double alpha = rr / dot_re(chi.data(), chi.data(), n);
+    for (long i = 0; i < n; ++i) {
+      x[i] = round_c64(x[i] + alpha * p[i]);
+      r[i] = round_c16(r[i] - alpha * q[i]);
+    }
+    double rr_new = dot_re(r.data(), r.data(), n);
+    double rn = std::sqrt(rr_new);
+    if (rn > rmax) rmax = rn;
+    if (rn < delta * rmax || rn <= tol * s * bnorm) {
+      ++nru;
+      for (long i = 0; i < n; ++i) { X[i] += x[i] / s; x[i] = 0.0; }
+      orc_apply_MdagM(method, L, phi, m, g, rho, X_, reinterpret_cast<double*>(q.data()));
+      double tr = 0.0;
+      for (long i = 0; i < n; ++i) tr += std::norm(b[i] - q[i]);
+      const double Rn = std::sqrt(tr);
+      true_rel = Rn / bnorm;
+      if (Rn <= tol * bnorm) { converged = 1; break; }
+      const double s_new = std::sqrt((double)n) / Rn, f = s_new / s;
+      for (long i = 0; i < n; ++i) { r[i] = round_c16(s_new * (b[i] - q[i])); p[i] = round_c16(f * p[i]); }
+      rr *= f * f;
+      s = s_new;
+      rr_new = dot_re(r.data(), r.data(), n);
+      rmax = std::sqrt(rr_new);
+    }
+    const double beta = rr_new / rr;
+    rr = rr_new;
+    for (long i = 0; i < n; ++i) p[i] = round_c16(r[i] + beta * p[i]);
+  }
+  if (!converged) {
+    for (long i = 0; i < n; ++i) X[i] += x[i] / s;
+    orc_apply_MdagM(method, L, phi, m, g, rho, X_, reinterpret_cast<double*>(q.data()));
+    double tr = 0.0;
+    for (long i = 0; i < n; ++i) tr += std::norm(b[i] - q[i]);
+    true_rel = bnorm > 0 ? std::sqrt(tr) / bnorm : 0.0;
+  }
+  info->iterations = k;
+  info->reliable_updates = nru;
+  info->converged = converged;
+  info->rel_residual_recursive = std::sqrt(rr) / (s * (bnorm > 0 ? bnorm : 1.0));
+  info->rel_residual_true = true_rel;
   return 0;
 }
 

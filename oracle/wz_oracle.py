@@ -370,3 +370,20 @@ def cg_dc_f16(phi, b, m, g, rho=1.0, tol=1e-6, inner_tol=1e-1, max_iter=100000, 
         raise ValueError("oracle cg_dc_f16 failed")
     return X, CGInfo(info.iterations, info.reliable_updates, bool(info.converged), info.rel_residual_recursive,
                      info.rel_residual_true, np.zeros(0))
+
+
+def cg_f16ru(phi, b, m, g, rho=1.0, tol=1e-6, max_iter=100000, delta=0.1, method="auto"):
+    """binary16 storage of r, p, chi with complex128 reliable updates and rescaling (oracle O11).
+    Returns (X, CGInfo)."""
+    phi = np.ascontiguousarray(phi, dtype=np.complex128)
+    b = np.ascontiguousarray(b, dtype=np.complex128)
+    dims = phi.shape
+    X = np.zeros_like(b)
+    info = _Info()
+    rc = lib().orc_cg_f16ru(_method(dims, method), _dims(dims), _dp(phi), _dp(b), _dp(X), _c2(m), _c2(g),
+                            ctypes.c_double(rho), ctypes.c_double(tol), int(max_iter), ctypes.c_double(delta),
+                            ctypes.byref(info))
+    if rc:
+        raise ValueError("oracle cg_f16ru failed")
+    return X, CGInfo(info.iterations, info.reliable_updates, bool(info.converged), info.rel_residual_recursive,
+                     info.rel_residual_true, np.zeros(0))

@@ -185,3 +185,27 @@ def test_cg_dc_f16_converges_to_the_dense_solution(orc):
     # a tighter inner tolerance than binary16 can deliver per correction still converges (more iterations per step)
     _, i2 = orc.cg_dc_f16(phi, b, cfg["m"], cfg["g"], 1.0, 1e-6, 1e-2, 20000, "naive")
     assert i2.converged and i2.reliable_updates < info.reliable_updates
+
+
+def test_cg_f16ru_converges_to_the_dense_solution(orc):
+    """O11: binary16 storage with complex128 reliable updates and rescaling: dense solution, independently recomputed
+    residual, and an iteration count close to the complex64 reliable-update loop O4' (measured with the oracle's
+    operators: 8^4 680 against 645, config 3 at 16^4 2352 against 2197) -- well below O10's restarts."""
+    dims = (4, 4, 4, 4)
+    cfg = inputs.CONFIGS[1]
+    phi = inputs.make_phi(1, dims, cfg["sigma"]).astype(np.complex64).astype(np.complex128)
+    b = inputs.make_source(1, 0, dims).astype(np.complex64).astype(np.complex128)
+    M = dense_route.fermion_matrix_dense(dims, phi, cfg["m"], cfg["g"], 1.0)
+    A = M.conj().T @ M
+    xd = np.linalg.solve(A, b.reshape(-1)).reshape(b.shape)
+    X, info = orc.cg_f16ru(phi, b, cfg["m"], cfg["g"], 1.0, 1e-6, 20000, 0.1, "naive")
+    assert info.converged and info.rel_residual_true <= 1e-6 and info.reliable_updates >= 5
+    res = np.linalg.norm(b.reshape(-1) - A @ X.reshape(-1)) / np.linalg.norm(b)
+    assert abs(res - info.rel_residual_true) <= 1e-3 * res + 2e-12
+    assert np.linalg.norm(X - xd) <= 1e-3 * np.linalg.norm(xd)
+    _, iru = orc.cg_c64ru(phi, b, cfg["m"], cfg["g"], 1.0, 1e-6, 20000, 0.1, "naive")
+    _, idc = orc.cg_dc_f16(phi, b, cfg["m"], cfg["g"], 1.0, 1e-6, 1e-1, 20000, "naive")
+    print("4^4: binary16 + reliable updates %d iterations (%d updates); complex64 + reliable updates %d; binary16 restarts %d"
+          % (info.iterations, info.reliable_updates, iru.iterations, idc.iterations))
+    assert iru.iterations - 2 <= info.iterations <= 1.15 * iru.iterations
+    assert info.iterations <= idc.iterations
