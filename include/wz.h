@@ -208,6 +208,15 @@ wz_status wz_cg_solve_dc_half(wz_plan *plan, const void *phi, const void *b, voi
                               const double m[2], const double g[2], double rho,
                               double tol, double inner_tol, int max_iter, int nbatch, wz_cg_info *info);
 
+/* wz_cg_solve_half (WZ_C64 plans; lattices as wz_cg_solve_dc_half): wz_cg_solve with t, chi, r, p STORED in binary16
+ * (oracle O11).  The loop of wz_cg_solve for WZ_C64 plans -- float arithmetic, double reductions, complex128 reliable
+ * updates (reading G9), the search direction kept across them -- on the system normalised to unit rms; every
+ * reliable update rescales r and p to unit rms again, so the stored values never leave binary16's normal range.
+ * 10.5u of traffic per iteration instead of 18.5u.  Arguments, info and return values as wz_cg_solve. */
+wz_status wz_cg_solve_half(wz_plan *plan, const void *phi, const void *b, void *x,
+                           const double m[2], const double g[2], double rho,
+                           double tol, int max_iter, int nbatch, wz_cg_info *info);
+
 /* ---- Locality probe (Eq. 3.9-3.11, Fig. 1) ----
  * wz_apply_Dslash: out = Dslash in = (1 - D2/2)^-1 D1 in (the fermion matrix at m = g = 0); in != out.
  * wz_locality_profile: psi = Dslash eta for a unit point source at the origin in spin component

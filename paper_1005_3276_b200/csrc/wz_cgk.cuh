@@ -334,6 +334,38 @@ k_h_accum(double* __restrict__ X, const float* __restrict__ e, long n, double in
     X[i] += inv_s * (double)e[i];
 }
 
+// Reliable update of the binary16-storage solver: r = binary16(s' d) for the recomputed float defect d, p = binary16(f p)
+// (both back at unit rms); sum |r|^2 as stored -> FIN_HRU.  One source per launch.
+__global__ void __launch_bounds__(CGK_NT)
+k_h_rescale(const float* __restrict__ d, __half* __restrict__ r, __half* __restrict__ p, long n, double s_new, float f,
+            RedArgs red) {
+  __shared__ double sh[33];
+  double acc = 0.0;
+  for (long i = ((long)blockIdx.x * blockDim.x + threadIdx.x) * 2; i < n; i += (long)gridDim.x * blockDim.x * 2) {
+    const __half2 h = __floats2half2_rn((float)(s_new * (double)d[i]), (float)(s_new * (double)d[i + 1]));
+    *reinterpret_cast<__half2*>(r + i) = h;
+    const float2 pv = __half22float2(*reinterpret_cast<const __half2*>(p + i));
+    *reinterpret_cast<__half2*>(p + i) = __floats2half2_rn(f * pv.x, f * pv.y);
+    const float2 g = __half22float2(h);
+    acc += (double)g.x * (double)g.x + (double)g.y * (double)g.y;
+  }
+  grid_reduce<FIN_HRU>(acc, red, blockIdx.x, gridDim.x, sh);
+}
+// what FIN_HRU needs (f^2, the new scaled ||b||), or: the update found the true residual below tol
+__global__ void k_h_patch(CGState* st, double f2, double bnorm_scaled, int converged) {
+  st->aux = f2;
+  st->pp = bnorm_scaled;
+  if (converged) { st->converged = 1; st->need_ru = 0; st->n_ru += 1; }
+}
+// X (complex128) += x (float) / s;  x = 0
+__global__ void __launch_bounds__(CGK_NT)
+k_h_accum_clear(double* __restrict__ X, float* __restrict__ x, long n, double inv_s) {
+  for (long i = (long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long)gridDim.x * blockDim.x) {
+    X[i] += inv_s * (double)x[i];
+    x[i] = 0.f;
+  }
+}
+
 // dst (double) = src (TX) element-wise, or dst += src
 template <typename TX>
 __global__ void __launch_bounds__(CGK_NT)

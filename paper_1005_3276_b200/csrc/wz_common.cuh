@@ -47,7 +47,9 @@ __device__ __forceinline__ bool cg_active(const CGState* st) {
 }
 
 // What the last block of a reduction does with the total.
-enum { FIN_STORE = 0, FIN_PQ = 1, FIN_RR = 2, FIN_RU = 3, FIN_INIT = 4, FIN_TRUE = 5, FIN_AUX = 6, FIN_PP = 7, FIN_RRS = 8 };
+enum { FIN_STORE = 0, FIN_PQ = 1, FIN_RR = 2, FIN_RU = 3, FIN_INIT = 4, FIN_TRUE = 5, FIN_AUX = 6, FIN_PP = 7, FIN_RRS = 8, FIN_HRU = 9 };
+// FIN_HRU: reliable update of the binary16-storage solver (wz_cg_solve_half): the vectors were rescaled by f, st->aux = f^2
+// and st->pp = the new scaled ||b|| were left by k_h_patch.
 // FIN_PP / FIN_RRS select the shifted-system variants of passes A' / E' (wz_cg_solve_shift); FIN_RRS
 // finalises like FIN_RR.
 
@@ -95,6 +97,15 @@ __device__ __forceinline__ void cg_finalize(double total, CGState* st, double* s
     st->rr = total;
     st->need_ru = 0;
     if (!st->converged && st->iter >= st->max_iter) st->stop = 1;
+  } else if (FIN == FIN_HRU) {  // r = s' (b - A X) as stored in binary16, p rescaled by f = s'/s
+    st->n_ru += 1;
+    st->rmax = sqrt(total);
+    st->true_rr = total;
+    st->beta = total / (st->aux * st->rr);  // rho_{k-1} in the new units
+    st->rr = total;
+    st->bnorm = st->pp;
+    st->need_ru = 0;
+    if (st->iter >= st->max_iter) st->stop = 1;
   } else if (FIN == FIN_TRUE) {
     st->true_rr = total;
   } else if (FIN == FIN_AUX) {

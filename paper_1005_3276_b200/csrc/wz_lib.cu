@@ -1768,6 +1768,164 @@ extern "C" wz_status wz_cg_solve_dc_half(wz_plan* pl, const void* phi_, const vo
   return ok ? WZ_OK : WZ_ENOTCONVERGED;
 }
 
+// wz_cg_solve_half (oracle O11): binary16 storage of t, chi, r, p with complex128 RELIABLE UPDATES: the loop
+// of wz_cg_solve for WZ_C64 plans (reading G9) on the system normalised to unit rms; at every update the vectors are
+// rescaled to unit rms again, so they never leave binary16's normal range and the search direction survives.
+extern "C" wz_status wz_cg_solve_half(wz_plan* pl, const void* phi_, const void* b_, void* x_, const double m[2],
+                                      const double g[2], double rho, double tol, int max_iter, int nbatch,
+                                      wz_cg_info* info) {
+  g_err[0] = 0;
+  if (!pl || !phi_ || !b_ || !x_ || !m || !g || !info) return WZ_EINVAL;
+  if (pl->dtype != WZ_C64) return WZ_EINVAL;
+  if (!(rho > 0.0 && rho < 2.0) || !(tol > 0.0) || max_iter < 0) return WZ_EINVAL;
+  if (nbatch < 0 || nbatch > pl->max_batch || x_ == b_) return WZ_EINVAL;
+  if (nbatch == 0) return WZ_OK;
+  WZ_ON_DEVICE(pl);
+  wz_status s = half_setup(pl, rho);
+  if (s != WZ_OK) return s;
+  const int nb = nbatch;
+  const long n = 8 * pl->V;
+  const size_t n1 = (size_t)4 * pl->V;
+  cudaStream_t st = pl->stream;
+  const cpx<float>* phi = (const cpx<float>*)phi_;
+  const cpx<float>* b = (const cpx<float>*)b_;
+  cpx<double>* X = (cpx<double>*)x_;
+  float* xs = (float*)pl->xs;
+  __half* r16 = (__half*)pl->h_r;
+  __half* p16 = (__half*)pl->h_p;
+  const int gv2 = vec_grid(n, 2), gv1 = vec_grid(n, 1);
+  if (!pl->ms_true && !dev_alloc(pl, &pl->ms_true, (size_t)WZ_MAX_SHIFTS * pl->max_batch)) return WZ_ENOMEM;
+  if (!pl->ms_rhs) {
+    float* a = nullptr;
+    if (!dev_alloc(pl, &a, (size_t)pl->max_batch * 2 * n1)) return WZ_ENOMEM;
+    pl->ms_rhs = a;
+  }
+  {
+    ProfScope ps(pl, WZ_K_OTHER);
+    k_f2d<<<vec_grid(2 * pl->V, 1), CGK_NT, 0, st>>>((double*)pl->phi128, (const float*)phi, 2 * pl->V);
+  }
+  WZ_CUDA(cudaGetLastError());
+  WZ_CUDA(cudaMemsetAsync(X, 0, sizeof(cpx<double>) * n1 * nb, st));
+  std::vector<double> tr(nb, 0.0), bnorm(nb, 0.0), scale(nb, 1.0), true_rel(nb, -1.0);
+  {  // ||b_j||
+    RedArgs ra = red_of(pl);
+    ra.store = pl->ms_true;
+    ProfScope ps(pl, WZ_K_OTHER);
+    k_norm2<float, FIN_STORE><<<dim3(gv2, nb), CGK_NT, 0, st>>>((const float*)b, n, ra);
+  }
+  WZ_CUDA(cudaGetLastError());
+  WZ_CUDA(cudaMemcpyAsync(tr.data(), pl->ms_true, sizeof(double) * nb, cudaMemcpyDeviceToHost, st));
+  WZ_CUDA(cudaStreamSynchronize(st));
+  std::vector<CGState> h(nb);
+  memset(h.data(), 0, sizeof(CGState) * nb);
+  for (int j = 0; j < nb; ++j) {
+    bnorm[j] = std::sqrt(tr[j]);
+    h[j].tol = tol; h[j].delta = kDelta; h[j].max_iter = max_iter; h[j].use_ru = 1; h[j].true_rr = -1.0;
+    if (bnorm[j] == 0.0) { h[j].converged = 1; true_rel[j] = 0.0; }
+    else scale[j] = std::sqrt((double)n / 2.0) / bnorm[j];
+    if (max_iter == 0) h[j].stop = 1;
+  }
+  WZ_CUDA(cudaMemcpyAsync(pl->d_state, h.data(), sizeof(CGState) * nb, cudaMemcpyHostToDevice, st));
+  WZ_CUDA(cudaStreamSynchronize(st));
+  for (int j = 0; j < nb; ++j) {
+    if (bnorm[j] == 0.0) continue;
+    ProfScope ps(pl, WZ_K_OTHER);
+    k_h_init<<<gv2, CGK_NT, 0, st>>>((const float*)b + j * n, r16 + j * n, p16 + j * n, xs + j * n, n, scale[j],
+                                     red_of(pl).for_source(j));
+    WZ_CUDA(cudaGetLastError());
+  }
+  // X_j += x_j / s_j (x cleared), then the defect of source j in complex128: float copy in ms_rhs, ||d||^2 on the host
+  auto fold_and_defect = [&](int j) -> wz_status {
+    {
+      ProfScope ps(pl, WZ_K_OTHER);
+      k_h_flush_x<<<dim3(gv2, 1), CGK_NT, 0, st>>>(xs + j * n, p16 + j * n, n, pl->d_state + j);
+    }
+    {
+      ProfScope ps(pl, WZ_K_OTHER);
+      k_clear_alpha<<<1, 1, 0, st>>>(pl->d_state + j);
+    }
+    {
+      ProfScope ps(pl, WZ_K_OTHER);
+      k_h_accum_clear<<<gv1, CGK_NT, 0, st>>>((double*)(X + j * n1), xs + j * n, n, 1.0 / scale[j]);
+    }
+    WZ_CUDA(cudaGetLastError());
+    struct Override {
+      wz_plan* p;
+      explicit Override(wz_plan* q) : p(q) { p->prof_override = WZ_K_OTHER; }
+      ~Override() { p->prof_override = -1; }
+    } ov(pl);
+    wz_status s2 = apply_MdagM_impl<double>(pl, pl->phi128, m, g, rho, X + j * n1, pl->q128, 1, false);
+    if (s2 != WZ_OK) return s2;
+    RedArgs ra = red_of(pl).for_source(j);
+    ra.store = pl->ms_true + j;
+    {
+      ProfScope ps(pl, WZ_K_OTHER);
+      k_resid<float, float, FIN_STORE><<<dim3(gv2, 1), CGK_NT, 0, st>>>((const float*)(b + j * n1), (const double*)pl->q128,
+                                                                        (float*)pl->ms_rhs + j * n, n, ra);
+    }
+    WZ_CUDA(cudaGetLastError());
+    WZ_CUDA(cudaMemcpyAsync(&tr[j], pl->ms_true + j, sizeof(double), cudaMemcpyDeviceToHost, st));
+    WZ_CUDA(cudaStreamSynchronize(st));
+    return WZ_OK;
+  };
+  int slot_w = 0, slot_r = 0, inflight = 0;
+  std::vector<int> ru_served(nb, 0);
+  for (;;) {
+    while (inflight < 2) {
+      for (int it = 0; it < kCheckEvery; ++it)
+        if ((s = cg_iteration_half(pl, phi, m, g, rho, xs, nb)) != WZ_OK) return s;
+      WZ_CUDA(cudaMemcpyAsync(pl->h_state + slot_w * pl->max_batch, pl->d_state, sizeof(CGState) * nb,
+                              cudaMemcpyDeviceToHost, st));
+      WZ_CUDA(cudaEventRecord(pl->ev[slot_w], st));
+      slot_w ^= 1;
+      ++inflight;
+    }
+    WZ_CUDA(cudaEventSynchronize(pl->ev[slot_r]));
+    const CGState* snap = pl->h_state + slot_r * pl->max_batch;
+    slot_r ^= 1;
+    --inflight;
+    bool all_done = true;
+    for (int j = 0; j < nb; ++j) {
+      if (snap[j].converged || snap[j].stop) continue;
+      all_done = false;
+      if (!(snap[j].need_ru && snap[j].n_ru == ru_served[j])) continue;
+      if ((s = fold_and_defect(j)) != WZ_OK) return s;  // reliable update (G9), on the normalised system
+      const double Rn = std::sqrt(tr[j]);
+      ProfScope ps(pl, WZ_K_OTHER);
+      if (Rn <= tol * bnorm[j]) {
+        true_rel[j] = Rn / bnorm[j];
+        k_h_patch<<<1, 1, 0, st>>>(pl->d_state + j, 1.0, 0.0, 1);
+      } else {
+        const double s_new = std::sqrt((double)n / 2.0) / Rn, f = s_new / scale[j];
+        k_h_patch<<<1, 1, 0, st>>>(pl->d_state + j, f * f, s_new * bnorm[j], 0);
+        k_h_rescale<<<gv2, CGK_NT, 0, st>>>((const float*)pl->ms_rhs + j * n, r16 + j * n, p16 + j * n, n, s_new, (float)f,
+                                            red_of(pl).for_source(j));
+        pl->launches++;
+        scale[j] = s_new;
+      }
+      WZ_CUDA(cudaGetLastError());
+      ++ru_served[j];
+    }
+    if (all_done) break;
+  }
+  WZ_CUDA(cudaStreamSynchronize(st));
+  WZ_CUDA(cudaMemcpy(h.data(), pl->d_state, sizeof(CGState) * nb, cudaMemcpyDeviceToHost));
+  bool ok = true;
+  for (int j = 0; j < nb; ++j) {
+    if (true_rel[j] < 0.0) {  // stopped at max_iter: fold what there is, recompute the residual
+      if ((s = fold_and_defect(j)) != WZ_OK) return s;
+      true_rel[j] = std::sqrt(tr[j]) / bnorm[j];
+    }
+    info[j].iterations = h[j].iter;
+    info[j].reliable_updates = ru_served[j];
+    info[j].converged = h[j].converged;
+    info[j].rel_residual_recursive = h[j].bnorm > 0 ? std::sqrt(h[j].rr) / h[j].bnorm : 0.0;
+    info[j].rel_residual_true = true_rel[j];
+    if (!h[j].converged) ok = false;
+  }
+  return ok ? WZ_OK : WZ_ENOTCONVERGED;
+}
+
 static wz_status cg_solve_any(wz_plan* pl, const void* phi, const void* b, void* x, const double m[2],
                               const double g[2], double rho, double tol, int max_iter, int nbatch,
                               wz_cg_info* info, bool pc, double sigma = 0.0) {

@@ -27,7 +27,7 @@ EXPORTS = [
     "wz_apply_M0inv", "wz_apply_MtdagMt", "wz_cg_solve_pc", "wz_apply_Dslash", "wz_locality_profile",
     "wz_cg_solve_shift", "wz_cg_solve_shift_pc", "wz_rational_apply",
     "wz_plan_set_graph", "wz_plan_cg_history", "wz_plan_set_block",
-    "wz_cg_solve_multishift", "wz_rational_apply_multishift", "wz_cg_solve_dc", "wz_apply_MdagM_noalloc", "wz_cg_solve_dc_half",
+    "wz_cg_solve_multishift", "wz_rational_apply_multishift", "wz_cg_solve_dc", "wz_apply_MdagM_noalloc", "wz_cg_solve_dc_half", "wz_cg_solve_half",
 ]
 
 
@@ -80,6 +80,7 @@ def lib() -> ctypes.CDLL:
         L.wz_apply_MdagM.argtypes = [vp, vp, d2, d2, cd, vp, vp, ci]
         L.wz_cg_solve.argtypes = [vp, vp, vp, vp, d2, d2, cd, cd, ci, ci, ctypes.POINTER(_CGInfo)]
         L.wz_cg_solve_pc.argtypes = L.wz_cg_solve.argtypes
+        L.wz_cg_solve_half.argtypes = L.wz_cg_solve.argtypes
         L.wz_cg_solve_shift.argtypes = [vp, vp, vp, vp, d2, d2, cd, cd, cd, ci, ci, ctypes.POINTER(_CGInfo)]
         L.wz_cg_solve_shift_pc.argtypes = L.wz_cg_solve_shift.argtypes
         L.wz_rational_apply.argtypes = [vp, vp, vp, vp, d2, d2, cd, cd, d2, d2, ci, cd, cd, ci, ci,
@@ -285,7 +286,8 @@ class Plan:
         return out
 
     def cg_solve(self, phi, b, m, g, rho: float = 1.0, tol: float = 1e-6, max_iter: int = 100000,
-                 out=None, raise_on_fail: bool = True, precondition: bool = False, sigma=None):
+                 out=None, raise_on_fail: bool = True, precondition: bool = False, sigma=None,
+                 half_storage: bool = False):
         """Solve M^dag M x = b per source (precondition=True: through the free-inverse
         preconditioned system, wz_cg_solve_pc; sigma given: the shifted system
         (M^dag M + sigma) x = b, wz_cg_solve_shift; both: Eq. 7.14, wz_cg_solve_shift_pc).
@@ -297,11 +299,17 @@ class Plan:
         self._spinor(out, torch.complex128, nb=nb)
         infos = (_CGInfo * nb)()
         if sigma is not None:
+            if half_storage:
+                raise ValueError("half_storage: plain system only")
             fn = lib().wz_cg_solve_shift_pc if precondition else lib().wz_cg_solve_shift
             st = fn(self._h, phi.data_ptr(), b.data_ptr(), out.data_ptr(), _c2(m), _c2(g),
                     float(rho), float(sigma), float(tol), int(max_iter), nb, infos)
         else:
             fn = lib().wz_cg_solve_pc if precondition else lib().wz_cg_solve
+            if half_storage:  # binary16 storage of t, chi, r, p (wz_cg_solve_half); plain system only
+                if precondition:
+                    raise ValueError("half_storage: plain system only")
+                fn = lib().wz_cg_solve_half
             st = fn(self._h, phi.data_ptr(), b.data_ptr(), out.data_ptr(), _c2(m), _c2(g),
                     float(rho), float(tol), int(max_iter), nb, infos)
         if st != WZ_OK and not (st == WZ_ENOTCONVERGED and not raise_on_fail):
