@@ -378,18 +378,19 @@ EncodeTiledFn encode_tiled_fn() {
   return fn;
 }
 template <typename R>
-bool make_tile_tmap(TMapBlob* out, const void* base, long inner, int l0, int l1, int nseg, long nf) {
+bool make_tile_tmap(TMapBlob* out, const void* base, long inner, int l0, int l1, int nseg, long nf, bool half = false) {
+  const size_t esz = half ? 2 : sizeof(R);  // bytes of one real number as stored
   static_assert(sizeof(CUtensorMap) == sizeof(TMapBlob), "CUtensorMap is 128 bytes");
   EncodeTiledFn enc = encode_tiled_fn();
   if (!enc || !base || ((uintptr_t)base & 15) || l0 > 256 || l1 > 256 || 2 * nseg > 256) return false;
-  if ((2 * nseg * sizeof(R)) % 16 || (inner * 2 * sizeof(R)) % 16) return false;
+  if ((2 * nseg * esz) % 16 || (inner * 2 * esz) % 16) return false;
   const cuuint64_t gdim[4] = {(cuuint64_t)(2 * inner), (cuuint64_t)l1, (cuuint64_t)l0, (cuuint64_t)nf};
-  const cuuint64_t gstr[3] = {(cuuint64_t)(2 * inner * sizeof(R)), (cuuint64_t)(2 * inner * sizeof(R)) * l1,
-                              (cuuint64_t)(2 * inner * sizeof(R)) * l1 * l0};
+  const cuuint64_t gstr[3] = {(cuuint64_t)(2 * inner * esz), (cuuint64_t)(2 * inner * esz) * l1,
+                              (cuuint64_t)(2 * inner * esz) * l1 * l0};
   const cuuint32_t box[4] = {(cuuint32_t)(2 * nseg), (cuuint32_t)l1, (cuuint32_t)l0, 1u};
   const cuuint32_t estr[4] = {1u, 1u, 1u, 1u};
   CUtensorMap tm;
-  const CUresult r = enc(&tm, sizeof(R) == 4 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4u,
+  const CUresult r = enc(&tm, half ? CU_TENSOR_MAP_DATA_TYPE_FLOAT16 : (sizeof(R) == 4 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_FLOAT64), 4u,
                          const_cast<void*>(base), gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
                          CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   if (r != CUDA_SUCCESS) return false;
@@ -409,10 +410,10 @@ wz_status launch_p01(wz_plan* pl, int kind, const P01Kern<R>& k, const P01Args<R
   // at 32^4 x 12); the same order slows pass E' (296 -> 346 us) and is not used there
   args.comp_fast = (kind == WZ_K_P01_MID) ? 1 : 0;
   args.tm_ahead = 0;
-  if (pl->tile_prefetch && !k.half && (kind == WZ_K_P01_MID || kind == WZ_K_P01_FWDCG)) {  // passes C and A' (wz_p01.cuh: E' does not gain)
+  if (pl->tile_prefetch && (kind == WZ_K_P01_MID || kind == WZ_K_P01_FWDCG)) {  // passes C and A' (wz_p01.cuh: E' does not gain)
     const int wave = wave_ctas(pl, (const void*)k.fn, k.nt, k.smem);
     if ((long)nseg_tiles * nf > 2L * wave &&  // at least two waves: something to run ahead of
-        make_tile_tmap<R>(&args.tm_in, args.in, args_in.I, k.l0, k.l1, k.nseg, nf))
+        make_tile_tmap<R>(&args.tm_in, args.in, args_in.I, k.l0, k.l1, k.nseg, nf, k.half != 0))
       args.tm_ahead = wave;
   }
   {
