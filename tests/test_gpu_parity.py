@@ -557,10 +557,11 @@ def test_cg_shift_pc_vs_oracle(wz, orc, inp, dims, dtype, tol):
     plan = wz.Plan(dims, dtype, 2)
     d_phi, d_b = torch.from_numpy(phi).cuda(), torch.from_numpy(b).cuda()
     phi128 = phi.astype(np.complex128)
+    nchk = 1 if dims[0] == 48 else 2  # the oracle's naive DFT at 48x24^3 takes ~13 s per solve: one source there
     for sigma in (0.01, 1.0, 100.0):
         x, infos = plan.cg_solve(d_phi, d_b, m, g, rho, tol, 2000, precondition=True, sigma=sigma)
         x = x.cpu().numpy()
-        for j in range(2):
+        for j in range(nchk):
             bj = b[j].astype(np.complex128)
             xo, io = orc.cg_shift_pc(phi128, bj, m, g, sigma, rho, tol, 2000)
             true_res = rel(orc.apply_MdagM(phi128, x[j], m, g, rho) + sigma * x[j], bj)
@@ -1099,7 +1100,7 @@ def test_cg_dc_half_storage_vs_oracle(wz, orc, inp, dims, m, sig, seed):
     x64, i64 = plan.cg_solve_dc(d_phi, d_b, m, g, rho, tol, 1e-3, 100000)
     x = x.cpu().numpy()
     phi128 = phi.astype(np.complex128)
-    for j in range(2):
+    for j in range(2 if dims[0] == 8 else 1):  # one oracle solve at 16^4 (a minute each)
         bj = b[j].astype(np.complex128)
         Xo, io = orc.cg_dc_f16(phi128, bj, m, g, rho, tol, itol, 100000)
         xd, _ = orc.cg(phi128, bj, m, g, rho, 1e-10, 100000)
@@ -1149,7 +1150,7 @@ def test_cg_half_storage_reliable_updates_vs_oracle(wz, orc, inp, dims, m, sig, 
     _, i64 = plan.cg_solve(d_phi, d_b, m, g, rho, tol, 100000)
     x = x.cpu().numpy()
     phi128 = phi.astype(np.complex128)
-    for j in range(2):
+    for j in range(2 if dims[0] == 8 else 1):  # one oracle solve at 16^4 (a minute each)
         bj = b[j].astype(np.complex128)
         Xo, io = orc.cg_f16ru(phi128, bj, m, g, rho, tol, 100000)
         xd, _ = orc.cg(phi128, bj, m, g, rho, 1e-10, 100000)
