@@ -66,12 +66,13 @@ template <typename R, int L> struct tune_tpl23 {  // axes 2,3
 // NSEG: consecutive (x2,x3) sites per strided tile: tile L0 x L1 x NSEG <= 136 KB.  Each (x0,x1) row
 // contributes one run of NSEG*8 bytes, and every run costs one L1 tag lookup per access: at 32^4
 // complex64 going from 32-byte to 64-/128-byte runs took the iteration from 173 to 141 us per source.
-// Forward modes: 64-byte runs, two 256-thread CTAs per SM; inverse modes: 128-byte runs, one
-// 512-thread CTA per SM.
+// Inverse modes and pass A': 128-byte runs, one 512-thread CTA per SM; the stand-alone forward mode: 64-byte runs, two
+// 256-thread CTAs per SM.  (Pass A' with 128-byte runs lost before it had the TMA tile prefetch, 457 against 434 us; with
+// it A' is unchanged, 437 against 435 us, and the passes around it run 1-2 % faster: 8307 -> 8380 it/s on the same box.)
 template <typename R, int L0, int L1, int MODE> struct tune_nseg {
   static constexpr bool fwd = (MODE == P01_FWD || MODE == P01_FWDCG);
   static constexpr int v = (L1 == 1) ? (int)(512 / (2 * sizeof(R)))  // single-axis pass: 512-byte runs, no tile in shared memory
-                         : (sizeof(R) == 4) ? (L0 * L1 > 2048 ? 4 : (L0 * L1 == 1024 ? (fwd ? 8 : 16) : 8))
+                         : (sizeof(R) == 4) ? (L0 * L1 > 2048 ? 4 : (L0 * L1 == 1024 ? (MODE == P01_FWD ? 8 : 16) : 8))
                                             : (L0 * L1 > 2048 ? 2 : 4);
 };
 
