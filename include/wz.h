@@ -197,7 +197,7 @@ wz_status wz_cg_solve_dc(wz_plan *plan, const void *phi, const void *b, void *x,
                          const double m[2], const double g[2], double rho,
                          double tol, double inner_tol, int max_iter, int nbatch, wz_cg_info *info);
 
-/* wz_cg_solve_dc_half (WZ_C64 plans; lattices with binary16-storage kernels: 8^4, 16^4, 32^4, else WZ_EUNSUPPORTED):
+/* wz_cg_solve_dc_half (WZ_C64 plans; lattices with binary16-storage kernels: 8^4, 16^4, 32^4, 48x24^3, else WZ_EUNSUPPORTED):
  * wz_cg_solve_dc with the inner solver's vectors t, chi, r, p STORED as two IEEE binary16 values per complex number
  * (SURVEY.md 8(f) NEXT-3 "half-precision-storage inner solver with defect correction"; oracle O10).  Arithmetic
  * stays float, reductions double, the inner x float, the outer loop complex128; each defect is normalised to unit

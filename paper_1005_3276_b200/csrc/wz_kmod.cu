@@ -46,6 +46,7 @@ void p01f([[maybe_unused]] std::vector<P01Entry<float>>& v) {
   v.push_back(make_p01_half<8, 8>());
   v.push_back(make_p01_half<16, 16>());
   v.push_back(make_p01_half<32, 32>());
+  v.push_back(make_p01_half<48, 24, 576>());
 #endif
 }
 void p01d([[maybe_unused]] std::vector<P01Entry<double>>& v) {
@@ -83,6 +84,7 @@ void p23f([[maybe_unused]] std::vector<P23Entry<float>>& v) {
   v.push_back(make_p23_half<8, 8>());
   v.push_back(make_p23_half<16, 16>());
   v.push_back(make_p23_half<32, 32>());
+  v.push_back(make_p23_half<24, 24>());
 #endif
 }
 void p23d([[maybe_unused]] std::vector<P23Entry<double>>& v) {

@@ -118,7 +118,7 @@ P23Entry<R> make_p23() {
 // ---- binary16 storage (NEXT-3): the three CG-fused (x0,x1) passes and the multiply pass with S = cpxh.
 // Tiles of 16 sites in every mode at 32x32 (64-byte runs of 4-byte elements; the shared-memory tile stays complex64).
 template <int L0, int L1, int MODE> struct tune_nseg_half {
-  static constexpr int v = (L0 * L1 >= 1024) ? 16 : 8;
+  static constexpr int v = (L0 * L1 == 1024) ? 16 : 8;
 };
 template <int L0, int L1, int MODE, int FIN, int IC>
 P01Kern<float> make_p01_kern_half() {
